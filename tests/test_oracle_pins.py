@@ -1,0 +1,479 @@
+"""Pins for the oracle (CPU only): what the paper and the mathematics fix, independent of the
+oracle's own formulas. SURVEY.md section 8(c) table "What pins the oracle"; DESIGN.md section 5.
+
+A plausible mistake anywhere in oracle/icon_oracle.c (dropped term, wrong sign or index,
+transposed operand, wrong tangent orientation) fails at least one test here."""
+import numpy as np
+import pytest
+
+import seeded_inputs as si
+from conftest import read_golden
+
+A = 6.371e6
+OMEGA = 7.29212e-5
+
+
+# ----------------------------------------------------------------------------------------------
+# counts, structure
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("k", [0, 1, 2, 3, 4, 5])
+def test_counts_and_structure(oracle_grid, k):
+    g = oracle_grid(k)
+    nc = 20 * 4 ** (k + 1)                       # north_star: cells = 20*4^(k+1)
+    assert (g.nc, g.ne, g.nv) == (nc, 3 * nc // 2, nc // 2 + 2)
+    deg = g.v_deg
+    assert (deg == 5).sum() == 12 and (deg == 6).sum() == g.nv - 12     # exactly 12 pentagons
+    assert (g.e2c[:, 0] != g.e2c[:, 1]).all()
+    assert (g.e2c[:, 0] < g.e2c[:, 1]).all()     # canonical numbering: first touch is the lower cell
+    e = np.arange(g.ne)[:, None]
+    assert (g.e2e4 != e).all()
+    # every edge appears in exactly two c2e rows, once with each sign
+    cnt = np.bincount(g.c2e.ravel(), minlength=g.ne)
+    assert (cnt == 2).all()
+    sgn = np.zeros(g.ne, dtype=np.int64)
+    np.add.at(sgn, g.c2e.ravel(), g.c_os.ravel().astype(np.int64))
+    assert (sgn == 0).all()
+    # every edge appears in exactly two fans, with opposite signs
+    real = g.v_os != 0
+    cntv = np.bincount(g.v2e[real], minlength=g.ne)
+    assert (cntv == 2).all()
+    sgv = np.zeros(g.ne, dtype=np.int64)
+    np.add.at(sgv, g.v2e[real], g.v_os[real].astype(np.int64))
+    assert (sgv == 0).all()
+    # pentagon pads repeat slot 0
+    pent = deg == 5
+    assert (g.v2e[pent, 5] == g.v2e[pent, 0]).all() and (g.v_os[pent, 5] == 0).all()
+    assert (g.geofac_rot[pent, 5] == 0).all()
+
+
+def test_table_checksums(oracle_grid):
+    for row in read_golden("table_checksums.txt"):
+        k = int(row[0])
+        g = oracle_grid(k)
+        got = [int(g.table(n).astype(np.int64).sum()) for n in ("c2e", "e2c", "e2v", "e2e4", "v2e")]
+        assert got == [int(x) for x in row[1:]], "R2B%d" % k
+
+
+def test_r2b0_table_rows(oracle_grid):
+    g = oracle_grid(0)
+    for row in read_golden("r2b0_tables.txt"):
+        name, first = row[0], int(row[1])
+        vals = np.array([int(x) for x in row[3:]])
+        tab = g.table(name)
+        cols = tab.shape[1]
+        got = tab[first:first + vals.size // cols].ravel()
+        assert (got == vals).all(), name
+
+
+def test_r2b0_geometry_values(oracle_grid):
+    g = oracle_grid(0)
+    # closed forms for the icosahedron's first bisection
+    assert abs(0.5 * np.arccos(1 / np.sqrt(5)) - 0.553574358897) < 1e-12
+    assert abs(np.pi / 5 - 0.628318530718) < 1e-12
+    scale = {"l_e": A, "d_e": A, "a_c": A * A, "a_v": A * A}
+    want = {}
+    for name, val, mult in read_golden("r2b0_geometry.txt"):
+        want.setdefault(name, []).append((float(val), int(mult)))
+    for name, items in want.items():
+        x = g.table(name) / scale[name]
+        vals = np.array([v for v, _ in items])
+        nearest = np.abs(x[:, None] - vals[None, :]).argmin(1)
+        assert np.abs(x - vals[nearest]).max() < 1e-12, name
+        for j, (_, mult) in enumerate(items):
+            assert (nearest == j).sum() > 0
+            if mult > 0:
+                assert (nearest == j).sum() == mult, (name, j)
+
+
+# ----------------------------------------------------------------------------------------------
+# brute force: an independent dict-based construction of P-1..P-6 in pure Python
+# ----------------------------------------------------------------------------------------------
+def _brute_topology(k):
+    lat = np.arctan(0.5)
+    P = [(0.0, 0.0, 1.0)]
+    for i in range(5):
+        lon = np.deg2rad(72.0 * i)
+        P.append((np.cos(lat) * np.cos(lon), np.cos(lat) * np.sin(lon), np.sin(lat)))
+    for i in range(5):
+        lon = np.deg2rad(36.0 + 72.0 * i)
+        P.append((np.cos(lat) * np.cos(lon), np.cos(lat) * np.sin(lon), -np.sin(lat)))
+    P.append((0.0, 0.0, -1.0))
+    P = [np.array(p) for p in P]
+    cells = []
+    for i in range(5):
+        j = (i + 1) % 5
+        cells += [(0, 1 + i, 1 + j), (1 + i, 6 + i, 1 + j), (6 + i, 6 + j, 1 + j), (11, 6 + j, 6 + i)]
+    for _ in range(k + 1):
+        mid = {}
+
+        def m(a, b):
+            key = (min(a, b), max(a, b))
+            if key not in mid:
+                p = P[a] + P[b]
+                P.append(p / np.sqrt((p * p).sum()))
+                mid[key] = len(P) - 1
+            return mid[key]
+        new = []
+        for (a, b, c) in cells:
+            ab, bc, ca = m(a, b), m(b, c), m(c, a)
+            new += [(a, ab, ca), (ab, b, bc), (ca, bc, c), (ab, bc, ca)]
+        cells = new
+    vid, c2v = {}, []
+    for cell in cells:
+        row = []
+        for v in cell:
+            if v not in vid:
+                vid[v] = len(vid)
+            row.append(vid[v])
+        c2v.append(row)
+    xyz = np.zeros((len(vid), 3))
+    for old, new in vid.items():
+        xyz[new] = P[old]
+    eid, e2v, e2c, c2e = {}, [], [], []
+    for c, (a, b, d) in enumerate(c2v):
+        row = []
+        for (p, q) in ((a, b), (b, d), (d, a)):
+            key = (min(p, q), max(p, q))
+            if key not in eid:
+                eid[key] = len(eid)
+                e2v.append([p, q])
+                e2c.append([c, -1])
+            else:
+                e2c[eid[key]][1] = c
+            row.append(eid[key])
+        c2e.append(row)
+    e2e4 = []
+    for e, (c0, c1) in enumerate(e2c):
+        row = []
+        for c in (c0, c1):
+            j = c2e[c].index(e)
+            row += [c2e[c][(j + 1) % 3], c2e[c][(j + 2) % 3]]
+        e2e4.append(row)
+    return np.array(c2v), np.array(c2e), np.array(e2c), np.array(e2v), np.array(e2e4), xyz
+
+
+@pytest.mark.parametrize("k", [0, 1, 2])
+def test_brute_force_topology(oracle_grid, k):
+    g = oracle_grid(k)
+    c2v, c2e, e2c, e2v, e2e4, xyz = _brute_topology(k)
+    assert (g.c2v == c2v).all() and (g.c2e == c2e).all() and (g.e2c == e2c).all()
+    assert (g.e2v == e2v).all() and (g.e2e4 == e2e4).all()
+    assert np.abs(g.vert_xyz - xyz).max() < 1e-15
+    # fans: CCW order means consecutive fan edges bound the listed cell, and the geometric angle
+    # of the fan edges around the vertex increases counter-clockwise seen from outside
+    for v in range(g.nv):
+        d = g.v_deg[v]
+        p = g.vert_xyz[v]
+        for i in range(d):
+            ea, eb, c = g.v2e[v, i], g.v2e[v, (i + 1) % d], g.v2c[v, i]
+            assert ea in g.c2e[c] and eb in g.c2e[c] and v in g.c2v[c]
+            xa, xb = g.edge_xyz[ea] - p, g.edge_xyz[eb] - p
+            assert np.dot(np.cross(xa, xb), p) > 0            # CCW about the outward normal
+        assert len(set(g.v2e[v, :d])) == d
+
+
+def test_orientation_conventions(oracle_grid):
+    """P-4: n_e points from e2c[e][0] to e2c[e][1]; t_e = n_e x x_e = -tau_e."""
+    g = oracle_grid(3)
+    dc = g.cell_xyz[g.e2c[:, 1]] - g.cell_xyz[g.e2c[:, 0]]
+    assert ((dc * g.edge_normal).sum(1) > 0).all()
+    tau = g.vert_xyz[g.e2v[:, 1]] - g.vert_xyz[g.e2v[:, 0]]
+    tau /= np.linalg.norm(tau, axis=1)[:, None]
+    t = np.cross(g.edge_normal, g.edge_xyz)
+    assert np.abs(t + tau).max() < 1e-14
+    assert np.abs(np.linalg.norm(g.edge_normal, axis=1) - 1).max() < 1e-14
+    assert np.abs((g.edge_normal * g.edge_xyz).sum(1)).max() < 1e-14
+    # cell centres are circumcentres: equidistant from the three vertices
+    d = np.stack([np.linalg.norm(g.cell_xyz - g.vert_xyz[g.c2v[:, j]], axis=1) for j in range(3)], 1)
+    assert np.abs(d - d[:, :1]).max() < 1e-14
+    # C-grid orthogonality: the dual arc passes through the edge midpoint
+    lin = g.c_lin.sum(1)
+    assert np.abs(lin - 1).max() < 1e-12
+    assert (g.c_lin > 0).all()
+    assert np.abs(g.inv_d_e * g.d_e - 1).max() < 1e-15
+    assert np.abs(g.f_e - 2 * OMEGA * g.edge_xyz[:, 2]).max() == 0
+
+
+# ----------------------------------------------------------------------------------------------
+# invariants of the discretisation
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("k", [0, 1, 2, 3, 4])
+def test_area_closure(oracle_grid, k):
+    g = oracle_grid(k)
+    assert abs(g.a_c.sum() / (4 * np.pi * A * A) - 1) < 1e-15 * (1 + k) * 4
+    assert abs(g.a_v.sum() / (4 * np.pi * A * A) - 1) < 1e-15 * (1 + k) * 4
+
+
+@pytest.mark.parametrize("k,flags", [(0, 0), (2, 0), (4, 0), (3, 1)])
+def test_discrete_gauss(oracle_grid, k, flags):
+    """sum_c A_c div_c = 0 on the closed sphere, to round-off, for random vn"""
+    g = oracle_grid(k, 7, flags)
+    rng = np.random.default_rng(11)
+    vn = rng.standard_normal((g.ne, 3))
+    div, _ = g.div_vort(vn, 3)
+    num = np.abs((g.a_c[:, None] * div).sum(0))
+    den = (np.abs(vn) * g.l_e[:, None]).sum(0)
+    assert (num / den).max() < 1e-16
+
+
+@pytest.mark.parametrize("k,flags", [(0, 0), (2, 0), (4, 0), (3, 1)])
+def test_curl_of_gradient_vanishes(oracle_grid, k, flags):
+    """rot(grad_n psi) = 0 (mimetic identity); pins v_os against the e2c order"""
+    g = oracle_grid(k, 7, flags)
+    rng = np.random.default_rng(12)
+    psi = rng.standard_normal((g.nc, 2))
+    gradn = (psi[g.e2c[:, 1]] - psi[g.e2c[:, 0]]) * g.inv_d_e[:, None]
+    _, vort = g.div_vort(gradn, 2)
+    h = np.sqrt(g.a_c.mean())
+    assert np.abs(vort).max() / (np.abs(gradn).max() / h) < 1e-15
+    # and the same identity with a wrong-signed fan entry must be far from zero (the pin bites)
+    bad = gradn.copy()
+    bad[g.v2e[5, 0]] *= -1
+    _, vort_bad = g.div_vort(bad, 2)
+    assert np.abs(vort_bad).max() / (np.abs(gradn).max() / h) > 1e-3
+
+
+@pytest.mark.parametrize("k", [0, 2, 4])
+def test_weights(oracle_grid, k):
+    g = oracle_grid(k)
+    assert np.abs(g.bln.sum(1) - 1).max() < 1e-15 * 4
+    assert (g.bln > 0.2).all() and (g.bln < 0.55).all()
+    # bln reproduces linear functions in the gnomonic plane of the cell centre: the gnomonic image
+    # of the cell centre itself is the origin, so sum_j bln_j * P(x_j) = 0
+    cc = g.cell_xyz
+    acc = np.zeros_like(cc)
+    for j in range(3):
+        x = g.edge_xyz[g.c2e[:, j]]
+        Pj = x / (x * cc).sum(1)[:, None] - cc
+        acc += g.bln[:, j:j + 1] * Pj
+    assert np.abs(acc).max() < 1e-15
+    # RBF normalisation identity (P-11): a locally uniform flow along t_e is returned exactly
+    t = np.cross(g.edge_normal, g.edge_xyz)
+    s = np.zeros(g.ne)
+    for j in range(4):
+        s += g.rbf[:, j] * (g.edge_normal[g.e2e4[:, j]] * t).sum(1)
+    assert np.abs(s - 1).max() < 1e-14
+    assert np.abs(g.rbf).sum(1).max() < 1.3
+    # a uniform flow along n_e has (nearly) no tangential component
+    s = np.zeros(g.ne)
+    for j in range(4):
+        s += g.rbf[:, j] * (g.edge_normal[g.e2e4[:, j]] * g.edge_normal).sum(1)
+    assert np.abs(s).max() < 0.2
+    # folded factors
+    le = g.l_e[g.c2e]
+    assert np.abs(g.geofac_div - le * g.c_os / g.a_c[:, None]).max() / np.abs(g.geofac_div).max() < 1e-15
+    de = g.d_e[g.v2e]
+    assert np.abs(g.geofac_rot - de * g.v_os / g.a_v[:, None]).max() / np.abs(g.geofac_rot).max() < 1e-15
+
+
+# ----------------------------------------------------------------------------------------------
+# solid-body rotation closed forms (first-order convergence values of SURVEY 8(c))
+# ----------------------------------------------------------------------------------------------
+def _solid_body(g, u0=20.0):
+    x, n = g.edge_xyz, g.edge_normal
+    vel = np.stack([-x[:, 1], x[:, 0], np.zeros(g.ne)], 1) * u0
+    return vel, (vel * n).sum(1)
+
+
+def _solid_body_errors(g):
+    u0 = 20.0
+    omp = u0 / A
+    vel, vn_sb = _solid_body(g, u0)
+    K = 6
+    zh = si.z_half_levels(K)
+    zf = 0.5 * (zh[:-1] + zh[1:])
+    vn = np.repeat(vn_sb[:, None], K, 1)
+    div, vort = g.div_vort(vn, K)
+    err = {}
+    err["zeta"] = np.abs(vort - 2 * omp * g.vert_xyz[:, 2:3]).max() / (2 * omp)
+    err["div"] = np.abs(div).max() / omp
+    out = g.velocity_tendencies(vn, np.zeros((g.nc, K + 1)), zh, K)
+    t = np.cross(g.edge_normal, g.edge_xyz)
+    err["vt"] = np.abs(out["vt"] - (vel * t).sum(1)[:, None]).max() / u0
+    cos2 = 1 - g.cell_xyz[:, 2] ** 2
+    err["ke_c"] = np.abs(out["ke_c"] - 0.5 * u0 * u0 * cos2[:, None]).max() / (0.5 * u0 * u0)
+    gam, w0 = 1e-5, 0.1
+    prof = 1 + gam * zf
+    vn = vn_sb[:, None] * prof[None, :]
+    w = np.full((g.nc, K + 1), w0)
+    out = g.velocity_tendencies(vn, w, zh, K)
+    x = g.edge_xyz
+    sinp = x[:, 2]
+    cosp = np.sqrt(1 - sinp ** 2)
+    north = (np.array([0, 0, 1.0])[None, :] - sinp[:, None] * x) / cosp[:, None]
+    nn = (north * g.edge_normal).sum(1)
+    exact = -((prof[None, :] ** 2 * (u0 * u0 / A) + prof[None, :] * 2 * OMEGA * u0) * (sinp * cosp * nn)[:, None]) \
+        - w0 * gam * vn_sb[:, None]
+    err["tendency"] = np.abs(out["ddt_vn"] - exact).max() / np.abs(exact).max()
+    out0 = g.velocity_tendencies(vn, np.zeros_like(w), zh, K)
+    dv = (out["ddt_vn"] - out0["ddt_vn"]) + w0 * gam * vn_sb[:, None]
+    err["vertical"] = np.abs(dv).max() / np.abs(w0 * gam * vn_sb).max()
+    return err
+
+
+def test_solid_body_closed_forms(oracle_grid):
+    gold = {r[0]: ([float(x) for x in r[1:6]], float(r[6])) for r in read_golden("solid_body_errors.txt")}
+    for k in range(5):
+        err = _solid_body_errors(oracle_grid(k))
+        for name, (vals, tol) in gold.items():
+            assert abs(err[name] / vals[k] - 1) < tol, (name, k, err[name], vals[k])
+        # P-14: the vertical term is exact for profiles linear in z
+        assert err["vertical"] < 1e-12
+
+
+def test_vertical_term_exact_for_linear_profiles(oracle_grid):
+    """w d(vn)/dz with vn = a + b z at every edge, arbitrary (stretched) levels, incl. both ends"""
+    g = oracle_grid(1)
+    K = 9
+    zh = si.z_half_levels(K)
+    zf = 0.5 * (zh[:-1] + zh[1:])
+    rng = np.random.default_rng(3)
+    b = rng.standard_normal(g.ne) * 1e-3
+    vn = 1.0 + b[:, None] * zf[None, :]
+    w = rng.standard_normal((g.nc, K + 1))
+    o1 = g.velocity_tendencies(vn, w, zh, K)
+    o0 = g.velocity_tendencies(vn, np.zeros_like(w), zh, K)
+    wf = 0.5 * (w[:, :-1] + w[:, 1:])
+    w_e = g.c_lin[:, :1] * wf[g.e2c[:, 0]] + g.c_lin[:, 1:] * wf[g.e2c[:, 1]]
+    want = -w_e * b[:, None]
+    got = o1["ddt_vn"] - o0["ddt_vn"]
+    assert np.abs(got - want).max() / np.abs(want).max() < 1e-11
+
+
+# ----------------------------------------------------------------------------------------------
+# special cases that reduce to library routines; internal consistency of the two evaluation paths
+# ----------------------------------------------------------------------------------------------
+def test_operators_equal_sparse_matrix_products(oracle_grid):
+    """div, vort, vt, KE_c are (sparse matrix) x (field): re-evaluate with scipy.sparse"""
+    import scipy.sparse as sp
+    g = oracle_grid(2)
+    K = 5
+    rng = np.random.default_rng(5)
+    vn = rng.standard_normal((g.ne, K))
+    w = rng.standard_normal((g.nc, K + 1))
+    zh = si.z_half_levels(K)
+
+    def mat(idx, coef, ncols):
+        r = np.repeat(np.arange(idx.shape[0]), idx.shape[1])
+        return sp.csr_matrix((coef.ravel(), (r, idx.ravel())), shape=(idx.shape[0], ncols))
+    D = mat(g.c2e, g.geofac_div, g.ne)
+    R = mat(g.v2e, g.geofac_rot, g.ne)
+    T = mat(g.e2e4, g.rbf, g.ne)
+    B = mat(g.c2e, g.bln, g.ne)
+    div, vort = g.div_vort(vn, K)
+    out = g.velocity_tendencies(vn, w, zh, K)
+    assert np.abs(div - D @ vn).max() < 1e-15 * abs(D).max() * 10
+    assert np.abs(vort - R @ vn).max() < 1e-15 * abs(R).max() * 10
+    vt = T @ vn
+    assert np.abs(out["vt"] - vt).max() < 1e-14
+    ke_c = B @ (0.5 * (vn * vn + vt * vt))
+    assert np.abs(out["ke_c"] - ke_c).max() < 1e-13
+    assert np.abs(out["vort"] - vort).max() == 0
+    # the tendency, re-assembled with numpy from the definition (S5-S7), all levels incl. the ends
+    dz = zh[:-1] - zh[1:]
+    zf = 0.5 * (zh[:-1] + zh[1:])
+    vn_ie = np.zeros((g.ne, K + 1))
+    gk = dz[:-1] / (dz[:-1] + dz[1:])
+    vn_ie[:, 1:K] = gk * vn[:, 1:] + (1 - gk) * vn[:, :-1]
+    vn_ie[:, 0] = vn[:, 0] + (vn[:, 0] - vn[:, 1]) * (zh[0] - zf[0]) / (zf[0] - zf[1])
+    vn_ie[:, K] = vn[:, K - 1] + (vn[:, K - 1] - vn[:, K - 2]) * (zh[K] - zf[K - 1]) / (zf[K - 1] - zf[K - 2])
+    wf = 0.5 * (w[:, :-1] + w[:, 1:])
+    w_e = g.c_lin[:, :1] * wf[g.e2c[:, 0]] + g.c_lin[:, 1:] * wf[g.e2c[:, 1]]
+    H = (ke_c[g.e2c[:, 1]] - ke_c[g.e2c[:, 0]]) * g.inv_d_e[:, None] \
+        + vt * (g.f_e[:, None] + 0.5 * (vort[g.e2v[:, 0]] + vort[g.e2v[:, 1]]))
+    V = w_e * (vn_ie[:, :-1] - vn_ie[:, 1:]) / dz
+    ref = -(H + V)
+    m = g.velocity_tendencies(vn, w, zh, K, with_scale=True)["m_ddt"]
+    assert (np.abs(out["ddt_vn"] - ref) <= 1e-14 * m).all()
+
+
+@pytest.mark.parametrize("k,flags", [(2, 0), (3, 1)])
+def test_sampled_evaluation_matches_full_arrays(oracle_grid, k, flags):
+    g = oracle_grid(k, 7, flags)
+    K = 7
+    rng = np.random.default_rng(8)
+    vn = rng.standard_normal((g.ne, K + 2))      # ldk > nlev
+    w = rng.standard_normal((g.nc, K + 3))
+    zh = si.z_half_levels(K)
+    full = g.velocity_tendencies(vn, w, zh, K, with_scale=True)
+    div, vort, md, mv = g.div_vort(vn, K, with_scale=True)
+    for what, arr, m, n in (("ddt_vn", full["ddt_vn"], full["m_ddt"], g.ne), ("div", div, md, g.nc),
+                            ("vort", vort, mv, g.nv)):
+        idx, lev = si.sample_points(1, n, K, 500)
+        val, ms = g.sample(what, idx, lev, vn, K, w=w, z_half=zh)
+        assert (np.abs(val - arr[idx, lev]) <= 1e-14 * m[idx, lev]).all(), what
+        assert np.abs(ms - m[idx, lev]).max() <= 1e-14 * np.abs(m).max()
+
+
+# ----------------------------------------------------------------------------------------------
+# seeded permutation (P-7)
+# ----------------------------------------------------------------------------------------------
+def _perm_from_positions(a_perm, a_canon, decimals=12):
+    """new id of canonical entity i, recovered geometrically (unique positions)"""
+    key = lambda a: [tuple(r) for r in np.round(a, decimals) + 0.0]
+    pos = {t: i for i, t in enumerate(key(a_perm))}
+    return np.array([pos[t] for t in key(a_canon)])
+
+
+def test_permutation_equivariance(oracle_grid):
+    k, seed = 2, 4
+    g0, g1 = oracle_grid(k), oracle_grid(k, seed, 1)
+    pv = _perm_from_positions(g1.vert_xyz, g0.vert_xyz)
+    pe = _perm_from_positions(g1.edge_xyz, g0.edge_xyz)
+    pc = _perm_from_positions(g1.cell_xyz, g0.cell_xyz)
+    for p, n in ((pv, g0.nv), (pe, g0.ne), (pc, g0.nc)):
+        assert sorted(p) == list(range(n))
+        assert (p != np.arange(n)).mean() > 0.9          # it really is a shuffle
+    # rows move, entries are renumbered, slot order is kept
+    assert (g1.c2e[pc] == pe[g0.c2e]).all() and (g1.c2v[pc] == pv[g0.c2v]).all()
+    assert (g1.e2c[pe] == pc[g0.e2c]).all() and (g1.e2v[pe] == pv[g0.e2v]).all()
+    assert (g1.e2e4[pe] == pe[g0.e2e4]).all()
+    assert (g1.v2e[pv] == pe[g0.v2e]).all() and (g1.v2c[pv] == pc[g0.v2c]).all()
+    assert (g1.c_os[pc] == g0.c_os).all() and (g1.v_os[pv] == g0.v_os).all()
+    # permuted-grid outputs, un-permuted, reproduce canonical-grid outputs
+    K = 4
+    rng = np.random.default_rng(2)
+    vn0 = rng.standard_normal((g0.ne, K))
+    w0 = rng.standard_normal((g0.nc, K + 1))
+    zh = si.z_half_levels(K)
+    vn1 = np.empty_like(vn0)
+    vn1[pe] = vn0
+    w1 = np.empty_like(w0)
+    w1[pc] = w0
+    o0 = g0.velocity_tendencies(vn0, w0, zh, K, with_scale=True)
+    o1 = g1.velocity_tendencies(vn1, w1, zh, K)
+    assert (np.abs(o1["ddt_vn"][pe] - o0["ddt_vn"]) <= 1e-13 * o0["m_ddt"]).all()
+    # different seeds give different permutations; same seed the same
+    g2 = oracle_grid(k, seed + 1, 1)
+    assert not (g2.c2e == g1.c2e).all()
+
+
+def test_mix64_reference_values(oracle_mod):
+    """P-7 mixer restated in Python integers; ranks must reproduce the oracle's permutation"""
+    M = (1 << 64) - 1
+
+    def mix64(seed, stream, i):
+        z = (seed + 0x9E3779B97F4A7C15 * (i + 1) + 0xD1B54A32D192ED03 * (stream + 1)) & M
+        z ^= z >> 30
+        z = (z * 0xBF58476D1CE4E5B9) & M
+        z ^= z >> 27
+        z = (z * 0x94D049BB133111EB) & M
+        z ^= z >> 31
+        return z
+    seed, k = 4, 1
+    g0, g1 = oracle_mod.Grid(k), oracle_mod.Grid(k, seed, 1)
+    for stream, n, canon, perm in ((0, g0.nc, g0.cell_xyz, g1.cell_xyz), (1, g0.ne, g0.edge_xyz, g1.edge_xyz),
+                                   (2, g0.nv, g0.vert_xyz, g1.vert_xyz)):
+        keys = [(mix64(seed, stream, i), i) for i in range(n)]
+        order = sorted(range(n), key=lambda i: keys[i])
+        new_of_old = np.empty(n, dtype=np.int64)
+        new_of_old[order] = np.arange(n)
+        assert np.abs(perm[new_of_old] - canon).max() < 1e-12
+
+
+def test_fp32_rounded_grid(oracle_grid):
+    g = oracle_grid(2)
+    r = g.rounded_f32()
+    assert (r.c2e == g.c2e).all()
+    for name in ("rbf", "bln", "geofac_div", "geofac_rot", "inv_d_e", "f_e", "c_lin"):
+        assert (r.table(name) == g.table(name).astype(np.float32).astype(np.float64)).all()
