@@ -1,0 +1,340 @@
+#!/usr/bin/env python
+"""bench.py -- the headline measurement (BASELINE.json metric): ddt_vn edge-level points/s and
+achieved HBM GB/s of the dycore sweep on one B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path: one
+dycore_velocity_tendencies call + one dycore_div_vort call on seeded synthetic fields (DESIGN.md
+section 4) of BASELINE.json configs[2] (R2B8 x 90 levels fp64, the headline roofline config) unless
+--config says otherwise. Prints ONE JSON line (rank 0). The path does not shard ("replicas only",
+DESIGN.md section 9): with N > 1 every rank runs an independent replica on its own GPU.
+
+--impl reference times the oracle (oracle/, plain C loops) on the host cores on a bounded sample
+of the same workload; it is a deliberately slow program, not a target.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import seeded_inputs as si  # noqa: E402
+
+METRIC = "ddt_vn edge-level points/s"
+UNIT = "Gpts/s"
+FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
+
+
+def workload_name(config):
+    c = si.CONFIGS[config]
+    return "config%d: R2B%d x %d levels %s%s" % (config, c["k"], c["nlev"], c["dtype"], " permuted" if c["permute"] else "")
+
+
+def algorithmic_bytes(nc, ne, nv, nlev, g):
+    """compulsory traffic: every input read once, every output written once,
+    one pass over the static tables; g = bytes per floating-point element"""
+    tend = (ne * nlev + nc * (nlev + 1) + ne * nlev) * g \
+        + ne * (16 + 4 * g + 8 + 8 + g + g + 2 * g) + nc * (12 + 3 * g) + nv * (24 + 6 * g)
+    dv = (ne * nlev + nc * nlev + nv * nlev) * g + nc * (12 + 3 * g) + nv * (24 + 6 * g)
+    return tend, dv
+
+
+def peak_hbm_gbs():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region"""
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_step_seconds(og, vn, w, zh, nlev, reps):
+    ts = []
+    for _ in range(reps):
+        t0 = time.perf_counter()
+        og.velocity_tendencies(vn, w, zh, nlev)
+        og.div_vort(vn, nlev)
+        ts.append(time.perf_counter() - t0)
+    return ts
+
+
+def cpu_threads():
+    try:
+        n = len(os.sched_getaffinity(0))
+    except AttributeError:
+        n = os.cpu_count() or 1
+    env = os.environ.get("OMP_NUM_THREADS")
+    return min(n, int(env)) if env and env.isdigit() else n
+
+
+def oracle_sample(config, k_sample):
+    """the oracle on a bounded sample: the same field recipe and level count on a coarser R2Bk grid"""
+    import oracle
+    cfg = si.CONFIGS[config]
+    og = oracle.Grid(k_sample, si.PERMUTE_SEED if cfg["permute"] else 0, 1 if cfg["permute"] else 0)
+    vn, w, zh = si.make_fields(config, og.edge_xyz, og.edge_normal, og.nc)
+    vn, w = vn.astype(np.float64), w.astype(np.float64)
+    if cfg["dtype"] == "f32":
+        og = og.rounded_f32()
+    return og, vn, w, zh, cfg["nlev"]
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores"""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    k_sample = min(si.CONFIGS[args.config]["k"], 6)
+    og, vn, w, zh, nlev = oracle_sample(args.config, k_sample)
+    oracle_step_seconds(og, vn, w, zh, nlev, args.warmup)
+    ts = oracle_step_seconds(og, vn, w, zh, nlev, args.steps)
+    t = float(np.mean(ts))
+    val = og.ne * nlev / t / 1e9
+    sample = "R2B%d x %d levels (%d edge-level points per step), same field recipe as %s" % (
+        k_sample, nlev, og.ne * nlev, workload_name(args.config))
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(args.config), "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cpu_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2511_02021_b200 as lib
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product has no CPU path")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    lib.load_library()
+
+    cfg = si.CONFIGS[args.config]
+    nlev = cfg["nlev"]
+    f32 = cfg["dtype"] == "f32"
+    gsize = 4 if f32 else 8
+    ldk = (nlev + 3) // 4 * 4 if f32 else (nlev + 1) // 2 * 2
+    ldk_w = (nlev + 4) // 4 * 4 if f32 else (nlev + 2) // 2 * 2
+    flags = lib.ICON_PERMUTE if cfg["permute"] else 0
+    t0 = time.perf_counter()
+    g = lib.IconGrid(cfg["k"], si.PERMUTE_SEED if cfg["permute"] else 0, flags)
+    if args.variant is not None:
+        g.set_option(lib.ICON_OPT_TENDENCY_KERNEL, args.variant)
+    t_grid = time.perf_counter() - t0
+    vn_h, w_h, zh = si.make_fields(args.config, g.table_host("edge_xyz"), g.table_host("edge_normal"), g.nc,
+                                   ldk=ldk, ldk_w=ldk_w, pad_value=0.0)
+    tdt = torch.float32 if f32 else torch.float64
+    vn = torch.from_numpy(vn_h).to(dev)
+    w = torch.from_numpy(w_h).to(dev)
+    ddt = torch.zeros((g.ne, ldk), dtype=tdt, device=dev)
+    div = torch.zeros((g.nc, ldk), dtype=tdt, device=dev)
+    vort = torch.zeros((g.nv, ldk), dtype=tdt, device=dev)
+    bytes_tend, bytes_dv = algorithmic_bytes(g.nc, g.ne, g.nv, nlev, gsize)
+    l2_flush = None
+    if bytes_tend < 512 * 2 ** 20:      # small configs are L2 resident: flush between iterations
+        l2_flush = torch.empty(256 * 2 ** 20, dtype=torch.uint8, device=dev)
+
+    def step(ev=None):
+        if l2_flush is not None:
+            l2_flush.fill_(1)
+        if ev:
+            ev[0].record()
+        lib.dycore_velocity_tendencies(g, zh, vn, w, ddt, nlev)
+        if ev:
+            ev[1].record()
+        lib.dycore_div_vort(g, vn, div, vort, nlev)
+        if ev:
+            ev[2].record()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    launches0 = g.launch_count
+    barrier()
+    for i in range(args.steps):
+        step(evs[i])
+    barrier()
+    launches = g.launch_count - launches0
+    clocks = sampler.stop() if rank == 0 else None
+    t_tend = np.array([e[0].elapsed_time(e[1]) for e in evs]) * 1e-3
+    t_dv = np.array([e[1].elapsed_time(e[2]) for e in evs]) * 1e-3
+    t_step = float((t_tend + t_dv).mean())
+    if world > 1:
+        tt = torch.tensor([t_step], dtype=torch.float64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        t_step_max = float(tt.item())
+    else:
+        t_step_max = t_step
+    pts = g.ne * nlev
+    value = world * pts / t_step_max / 1e9
+
+    # end to end through the C-ABI with HOST buffers (pinned), copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        hv, hw = torch.from_numpy(vn_h).pin_memory(), torch.from_numpy(w_h).pin_memory()
+        h_ddt = torch.zeros((g.ne, ldk), dtype=tdt).pin_memory()
+        h_div = torch.zeros((g.nc, ldk), dtype=tdt).pin_memory()
+        h_vort = torch.zeros((g.nv, ldk), dtype=tdt).pin_memory()
+        lib.dycore_step_host(g, zh, hv, hw, h_ddt, h_div, h_vort, nlev)
+        barrier()
+        n_e2e = max(1, min(args.steps, 3))
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            lib.dycore_step_host(g, zh, hv, hw, h_ddt, h_div, h_vort, nlev)
+        torch.cuda.synchronize()
+        t_e2e = (time.perf_counter() - t0) / n_e2e
+        if world > 1:
+            tt = torch.tensor([t_e2e], dtype=torch.float64, device=dev)
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            t_e2e = float(tt.item())
+        e2e = {"value": world * pts / t_e2e / 1e9, "unit": UNIT,
+               "h2d_bytes_per_step": int(hv.numel() + hw.numel()) * gsize,
+               "d2h_bytes_per_step": int(h_ddt.numel() + h_div.numel() + h_vort.numel()) * gsize,
+               "ms_per_step": t_e2e * 1e3, "steps": n_e2e}
+        del hv, hw, h_ddt, h_div, h_vort
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    peak, peak_src = peak_hbm_gbs()
+    t_tend_avg = float(t_tend.mean())
+    achieved = bytes_tend / t_tend_avg / 1e9
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tp):
+        try:
+            traffic = json.load(open(tp)).get("config%d" % args.config, {}).get("tendency_dram_bytes_per_launch")
+        except Exception:
+            traffic = None
+    roofline = {"bound": "hbm", "kernel": "dycore_velocity_tendencies", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": bytes_tend, "kernel_ms": t_tend_avg * 1e3,
+                "frac_of_nominal_8TBs": achieved / 8000.0,
+                "div_vort": {"achieved": bytes_dv / float(t_dv.mean()) / 1e9, "frac": bytes_dv / float(t_dv.mean()) / 1e9 / peak,
+                             "kernel_ms": float(t_dv.mean()) * 1e3, "algorithmic_bytes_per_launch": bytes_dv}}
+
+    cpu_baseline = None
+    if not args.no_cpu_baseline and world == 1:
+        k_sample = min(cfg["k"], 6)
+        og, ovn, ow, ozh, onlev = oracle_sample(args.config, k_sample)
+        oracle_step_seconds(og, ovn, ow, ozh, onlev, 1)
+        ts, t_begin = [], time.perf_counter()
+        while len(ts) < 3 or (time.perf_counter() - t_begin < 10.0 and len(ts) < 50):
+            ts += oracle_step_seconds(og, ovn, ow, ozh, onlev, 1)
+        cpu_baseline = {"value": og.ne * onlev / float(np.mean(ts)) / 1e9, "unit": UNIT, "cores": cpu_threads(), "kind": "oracle",
+                        "sample": "R2B%d x %d levels fp64 oracle, %d timed steps (%.1f s), same field recipe" % (
+                            k_sample, onlev, len(ts), sum(ts))}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": t_step_max * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": cfg["dtype"], "data": "synthetic",
+            "config": {"workload": workload_name(args.config), "nc": g.nc, "ne": g.ne, "nv": g.nv, "nlev": nlev,
+                       "ldk": ldk, "ldk_w": ldk_w, "step": "dycore_velocity_tendencies + dycore_div_vort",
+                       "l2": "flushed between iterations" if l2_flush is not None else "inputs larger than L2",
+                       "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "tendency_kernel_variant": args.variant, "grid_create_s": t_grid},
+            "gpts_tendency_only": pts / t_tend_avg / 1e9,
+            "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": int(launches),
+            "clocks": clocks}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", type=int, default=3, choices=sorted(si.CONFIGS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--variant", type=int, default=None, help="ICON_OPT_TENDENCY_KERNEL override")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    return run_reference(args) if args.impl == "reference" else run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,169 @@
+/*
+ * icon_dycore.h -- C-ABI of the B200-native implementation of the velocity-tendency /
+ * divergence / vorticity stencil sweep of ICON's non-hydrostatic dynamical core
+ * (arxiv/paper_2511_02021; hot path named by BASELINE.json north_star; scope SURVEY.md 8).
+ *
+ * What the paper fixes: computations on an icosahedral-triangular C-grid (section 2)
+ * and its dual of hexagons and 12 pentagons, reached through integer index arrays
+ * (section 3.2); fields stay resident on the GPU for the whole run, no host copies
+ * in the time loop (section 3.1); static coefficient + index tables are read-only
+ * inputs of every stencil statement (the e_bln_c_s / ieidx excerpt); the
+ * dynamical core is memory-bandwidth bound. Everything the paper leaves
+ * open is fixed by the readings P-1..P-17 listed in DESIGN.md section 3.
+ *
+ * Conventions
+ *   - Plain C types only. "dev" pointers are CUDA device pointers, "host" pointers are host memory.
+ *   - Fields are level-contiguous: x[i*ldk + k], 0 <= k < nlev, k = 0 at the model top; i is the
+ *     USER id of the cell / edge / vertex (the ids of the public tables). ldk >= nlev
+ *     (ldk_w >= nlev+1 for w). Field pointers must be 16-byte aligned and ldk*sizeof(T) must be a
+ *     multiple of 16. Padding lanes k >= nlev are never read for arithmetic and never written.
+ *   - dtype ICON_F64: fields and coefficients are double. ICON_F32: fields are float and the
+ *     coefficients are the fp64 ones rounded to float once (reading P-17).
+ *   - Every call returns ICON_OK or a negative error code; no exceptions, no abort, no output to
+ *     stdout/stderr. icon_last_error() returns a thread-local message for the last failure.
+ *   - Compute calls enqueue kernels on the caller's CUDA stream and return without synchronising.
+ *     Field buffers are caller-owned, never retained; outputs must not alias inputs.
+ *   - There is NO CPU fallback: compute calls return ICON_ECUDA when no CUDA device is usable.
+ */
+#ifndef ICON_DYCORE_H
+#define ICON_DYCORE_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct icon_grid icon_grid_t;   /* opaque; owns host and device copies of all tables */
+
+enum { ICON_OK = 0, ICON_EINVAL = -1, ICON_ENOMEM = -2, ICON_ECUDA = -3, ICON_EUNSUPPORTED = -4 };
+enum { ICON_F64 = 0, ICON_F32 = 1 };
+/* element types reported by icon_grid_table_host */
+enum { ICON_T_I32 = 10, ICON_T_I8 = 11, ICON_T_F64 = 12, ICON_T_F32 = 13 };
+
+/* icon_grid_create flags */
+enum {
+    ICON_PERMUTE = 1u,            /* seeded random renumbering of cells/edges/vertices (P-7, config 4) */
+    ICON_LOCALITY_WORKLIST = 2u,  /* internal tables laid out in generation (spatially local) order and
+                                     kernels walk that order; results are identical. Implied by
+                                     ICON_PERMUTE unless ICON_NO_WORKLIST is given. */
+    ICON_HOST_ONLY = 4u,          /* build host tables only; no CUDA device is touched (table tests) */
+    ICON_NO_WORKLIST = 8u         /* with ICON_PERMUTE: walk the permuted ids directly (ablation) */
+};
+
+/* table selectors for icon_grid_table_host / icon_grid_table_device */
+enum {
+    ICON_TAB_C2V = 0,      /* int32 [nc][3] vertices of a cell, counter-clockwise (P-2, P-3) */
+    ICON_TAB_C2E,          /* int32 [nc][3] edge j joins vertex slots j and j+1 (P-3) */
+    ICON_TAB_E2C,          /* int32 [ne][2] first-touch cell, second-touch cell (P-3) */
+    ICON_TAB_E2V,          /* int32 [ne][2] direction of the edge (P-3, P-4) */
+    ICON_TAB_E2E4,         /* int32 [ne][4] the four other edges of the two adjacent cells (P-6) */
+    ICON_TAB_V2E,          /* int32 [nv][6] fan edges counter-clockwise; pentagon slot 5 = slot 0 (P-5) */
+    ICON_TAB_V2C,          /* int32 [nv][6] fan cells; cell i lies between fan edges i and i+1 (P-5) */
+    ICON_TAB_V_DEG,        /* int32 [nv]    5 or 6 (exactly 12 fives) */
+    ICON_TAB_C_OS,         /* int8  [nc][3] +1 if the cell is e2c[.][0] of that edge else -1 (P-4) */
+    ICON_TAB_V_OS,         /* int8  [nv][6] -1 if v == e2v[.][0] else +1; 0 in the pentagon pad (P-5) */
+    ICON_TAB_VERT_XYZ,     /* f64 [nv][3] unit sphere */
+    ICON_TAB_CELL_XYZ,     /* f64 [nc][3] spherical circumcentres (P-8) */
+    ICON_TAB_EDGE_XYZ,     /* f64 [ne][3] edge midpoints x_e (P-4) */
+    ICON_TAB_EDGE_NORMAL,  /* f64 [ne][3] n_e = tau_e x x_e, from e2c[.][0] to e2c[.][1] (P-4) */
+    ICON_TAB_L_E,          /* f64 [ne] primal edge length, m */
+    ICON_TAB_D_E,          /* f64 [ne] dual edge length, m */
+    ICON_TAB_INV_D_E,      /* f64 [ne] 1/d_e */
+    ICON_TAB_F_E,          /* f64 [ne] Coriolis parameter 2*Omega*z(x_e) */
+    ICON_TAB_C_LIN,        /* f64 [ne][2] cell-to-edge linear weights (P-9) */
+    ICON_TAB_RBF,          /* f64 [ne][4] tangential-wind reconstruction weights (P-11) */
+    ICON_TAB_A_C,          /* f64 [nc] cell area, m^2 */
+    ICON_TAB_BLN,          /* f64 [nc][3] edge-to-cell weights, the paper's e_bln_c_s (P-10) */
+    ICON_TAB_A_V,          /* f64 [nv] dual-cell area, m^2 */
+    ICON_TAB_GEOFAC_DIV,   /* f64 [nc][3] l_e*c_os/A_c */
+    ICON_TAB_GEOFAC_ROT,   /* f64 [nv][6] d_e*v_os/A_v, 0 in the pentagon pad */
+    ICON_TAB_COUNT
+};
+
+/* runtime options (icon_grid_set_option); defaults are the fastest validated variants */
+enum {
+    ICON_OPT_TENDENCY_KERNEL = 0, /* 0 = unfused 3-kernel pipeline through an HBM workspace;
+                                     1 = fused gather kernel (no workspace). */
+    ICON_OPT_COUNT
+};
+
+/*
+ * icon_grid_create -- SURVEY.md 8(a) rows G1-G3; readings P-1..P-11.
+ * Builds the R2Bk grid (k+1 bisections of the unit icosahedron, 0 <= k <= 9), its canonical
+ * first-touch numbering, all index tables, geometry and coefficients on the host, optionally
+ * renumbers cells/edges/vertices by the seeded permutation (ICON_PERMUTE; seed is ignored
+ * otherwise), and uploads the tables the kernels need to the current CUDA device (unless
+ * ICON_HOST_ONLY). Not part of any timed region (the paper excludes initialisation).
+ * *out is owned by the caller until icon_grid_destroy. Errors: ICON_EINVAL (k, flags, out),
+ * ICON_ENOMEM, ICON_ECUDA (no device / upload failed).
+ */
+int icon_grid_create(int bisections_k, uint64_t seed, unsigned flags, icon_grid_t** out);
+void icon_grid_destroy(icon_grid_t* g);
+
+/* nc = 20*4^(k+1), ne = 3nc/2, nv = nc/2+2. Any output pointer may be NULL. */
+int icon_grid_counts(const icon_grid_t* g, int64_t* nc, int64_t* ne, int64_t* nv);
+
+/* Host view of a public table (user ids). *ptr stays valid until icon_grid_destroy and must not
+ * be written. dtype receives ICON_T_*. */
+int icon_grid_table_host(const icon_grid_t* g, int which, const void** ptr, int* dtype, int64_t* rows, int* cols);
+
+/* Device copy of a public table in user order, uploaded on first request and then cached.
+ * dtype: ICON_F64 or ICON_F32 selects the element type of floating-point tables (ignored for
+ * integer tables). ICON_EUNSUPPORTED on a ICON_HOST_ONLY grid. */
+int icon_grid_table_device(icon_grid_t* g, int which, int dtype, const void** dptr);
+
+int icon_grid_set_option(icon_grid_t* g, int option, int value);
+
+/*
+ * dycore_div_vort -- SURVEY.md 8(a) steps S1, S2 (north_star: "cell divergence from normal winds
+ * (c2e gather with edge lengths, orientation signs and cell areas), relative vorticity at vertices
+ * (v2e gather with dual lengths and dual areas)").
+ *   div(c,k)  = sum_{j<3} geofac_div(c,j) * vn(c2e[c][j], k)
+ *   vort(v,k) = sum_{j<6} geofac_rot(v,j) * vn(v2e[v][j], k)      (pentagon pad coefficient is 0)
+ * vn [ne][ldk] dev in; div [nc][ldk], vort [nv][ldk] dev out. 1 <= nlev <= ldk.
+ */
+int dycore_div_vort(icon_grid_t* g, int dtype, int nlev, int ldk,
+                    const void* vn, void* div, void* vort, void* cuda_stream);
+
+/*
+ * dycore_velocity_tendencies -- SURVEY.md 8(a) steps S3-S7 (north_star: "tangential wind by RBF
+ * reconstruction from the 4 neighbouring edges (e2e4 table), kinetic energy at edges and cells, and
+ * the normal-wind tendency ddt_vn = -(dKE/dn + (zeta+f)*vt + w*dvn/dz), with w on nlev+1 half
+ * levels"; the edge->cell kinetic-energy interpolation is PAPER.md:164-167).
+ *   vt(e,k)   = sum_{j<4} rbf(e,j) * vn(e2e4[e][j], k)
+ *   KE_e      = 1/2 (vn^2 + vt^2);  KE_c(c,k) = sum_{j<3} bln(c,j) * KE_e(c2e[c][j], k)
+ *   ddt_vn    = -[ (KE_c(c1)-KE_c(c0)) / d_e + vt * (f_e + 1/2(zeta(v0)+zeta(v1)))
+ *                  + w_e * (vn_ie(k) - vn_ie(k+1)) / dz_k ]
+ *   w_e = c_lin(e,0) w_f(c0,k) + c_lin(e,1) w_f(c1,k), w_f(c,k) = 1/2 (w(c,k)+w(c,k+1)),
+ *   vn_ie = vn interpolated linearly in z to half levels, linear extrapolation at k=0 and k=nlev (P-14).
+ * z_half [nlev+1] HOST, strictly decreasing (read during the call, not retained).
+ * vn [ne][ldk], w [nc][ldk_w] dev in; ddt_vn [ne][ldk] dev out.
+ * vt_opt [ne][ldk], ke_c_opt [nc][ldk], vort_opt [nv][ldk]: dev out, NULL = do not store.
+ * 2 <= nlev <= ldk, nlev+1 <= ldk_w, nlev <= 4096.
+ */
+int dycore_velocity_tendencies(icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w,
+                               const double* z_half,
+                               const void* vn, const void* w, void* ddt_vn,
+                               void* vt_opt, void* ke_c_opt, void* vort_opt, void* cuda_stream);
+
+/*
+ * dycore_step_host -- one velocity-tendency + div/vort step with HOST field buffers (the
+ * end-to-end path of bench.py): copies vn and w to the device, runs dycore_velocity_tendencies and
+ * dycore_div_vort, copies ddt_vn, div and vort back, and synchronises. Host buffers should be
+ * pinned for full PCIe bandwidth. Device staging buffers are owned by the grid handle and
+ * allocated on first use. Same shapes and constraints as the two device calls.
+ */
+int dycore_step_host(icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
+                     const void* vn_host, const void* w_host,
+                     void* ddt_vn_host, void* div_host, void* vort_host);
+
+/* number of kernels the library has launched through this handle since creation */
+int64_t icon_grid_launch_count(const icon_grid_t* g);
+
+const char* icon_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ICON_DYCORE_H */

@@ -1,0 +1,187 @@
+"""Thin ctypes binding over libicon_dycore.so (include/icon_dycore.h). Argument marshalling only:
+every step of the hot path runs in the library's CUDA kernels. PyTorch is used by callers for
+device memory and streams; this module accepts torch tensors or raw device pointers (ints).
+
+There is no CPU fallback: if the shared library is missing or no CUDA device is usable, calls
+raise.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIBPATH = os.path.join(_HERE, "libicon_dycore.so")
+
+ICON_OK, ICON_EINVAL, ICON_ENOMEM, ICON_ECUDA, ICON_EUNSUPPORTED = 0, -1, -2, -3, -4
+ICON_F64, ICON_F32 = 0, 1
+ICON_T_I32, ICON_T_I8, ICON_T_F64, ICON_T_F32 = 10, 11, 12, 13
+ICON_PERMUTE, ICON_LOCALITY_WORKLIST, ICON_HOST_ONLY, ICON_NO_WORKLIST = 1, 2, 4, 8
+ICON_OPT_TENDENCY_KERNEL = 0
+
+TABLES = ("c2v", "c2e", "e2c", "e2v", "e2e4", "v2e", "v2c", "v_deg", "c_os", "v_os",
+          "vert_xyz", "cell_xyz", "edge_xyz", "edge_normal", "l_e", "d_e", "inv_d_e", "f_e", "c_lin", "rbf",
+          "a_c", "bln", "a_v", "geofac_div", "geofac_rot")
+TABLE_ID = {n: i for i, n in enumerate(TABLES)}
+
+# every symbol include/icon_dycore.h declares
+EXPORTS = ("icon_grid_create", "icon_grid_destroy", "icon_grid_counts", "icon_grid_table_host",
+           "icon_grid_table_device", "icon_grid_set_option", "dycore_div_vort", "dycore_velocity_tendencies",
+           "dycore_step_host", "icon_grid_launch_count", "icon_last_error")
+
+
+class IconError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("libicon_dycore error %d: %s" % (code, msg))
+        self.code = code
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen the in-tree CUDA library; fails loudly when it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIBPATH):
+        raise ImportError("%s is missing: run `python -m paper_2511_02021_b200.build` (needs nvcc). "
+                          "There is no CPU fallback." % _LIBPATH)
+    L = ctypes.CDLL(_LIBPATH)
+    P, i64, ci = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int
+    L.icon_grid_create.restype = ci
+    L.icon_grid_create.argtypes = [ci, ctypes.c_uint64, ctypes.c_uint, ctypes.POINTER(P)]
+    L.icon_grid_destroy.restype = None
+    L.icon_grid_destroy.argtypes = [P]
+    L.icon_grid_counts.restype = ci
+    L.icon_grid_counts.argtypes = [P, ctypes.POINTER(i64), ctypes.POINTER(i64), ctypes.POINTER(i64)]
+    L.icon_grid_table_host.restype = ci
+    L.icon_grid_table_host.argtypes = [P, ci, ctypes.POINTER(P), ctypes.POINTER(ci), ctypes.POINTER(i64), ctypes.POINTER(ci)]
+    L.icon_grid_table_device.restype = ci
+    L.icon_grid_table_device.argtypes = [P, ci, ci, ctypes.POINTER(P)]
+    L.icon_grid_set_option.restype = ci
+    L.icon_grid_set_option.argtypes = [P, ci, ci]
+    L.icon_grid_launch_count.restype = i64
+    L.icon_grid_launch_count.argtypes = [P]
+    L.dycore_div_vort.restype = ci
+    L.dycore_div_vort.argtypes = [P, ci, ci, ci, P, P, P, P]
+    L.dycore_velocity_tendencies.restype = ci
+    L.dycore_velocity_tendencies.argtypes = [P, ci, ci, ci, ci, P, P, P, P, P, P, P, P]
+    L.dycore_step_host.restype = ci
+    L.dycore_step_host.argtypes = [P, ci, ci, ci, ci, P, P, P, P, P, P]
+    L.icon_last_error.restype = ctypes.c_char_p
+    L.icon_last_error.argtypes = []
+    _lib = L
+    return L
+
+
+def _check(rc):
+    if rc != ICON_OK:
+        raise IconError(rc, load_library().icon_last_error().decode(errors="replace"))
+
+
+def _dptr(x):
+    """device (or host) pointer of a torch tensor / numpy array / int / None"""
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return ctypes.c_void_p(x)
+    if isinstance(x, np.ndarray):
+        return ctypes.c_void_p(x.ctypes.data)
+    return ctypes.c_void_p(x.data_ptr())
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+        return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+    if isinstance(stream, int):
+        return ctypes.c_void_p(stream)
+    return ctypes.c_void_p(stream.cuda_stream)
+
+
+_NP = {ICON_T_I32: np.int32, ICON_T_I8: np.int8, ICON_T_F64: np.float64, ICON_T_F32: np.float32}
+
+
+class IconGrid:
+    """icon_grid_t handle (R2Bk grid + tables on host and device)."""
+
+    def __init__(self, k, seed=0, flags=0):
+        self._L = load_library()
+        h = ctypes.c_void_p()
+        _check(self._L.icon_grid_create(int(k), int(seed), int(flags), ctypes.byref(h)))
+        self._h = h
+        self.k, self.seed, self.flags = int(k), int(seed), int(flags)
+        nc, ne, nv = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int64()
+        _check(self._L.icon_grid_counts(h, ctypes.byref(nc), ctypes.byref(ne), ctypes.byref(nv)))
+        self.nc, self.ne, self.nv = nc.value, ne.value, nv.value
+
+    def close(self):
+        h, self._h = getattr(self, "_h", None), None
+        if h:
+            self._L.icon_grid_destroy(h)
+
+    def __del__(self):
+        self.close()
+
+    def table_host(self, name):
+        """numpy view (read-only copy semantics: do not write) of a public table"""
+        ptr, dt, rows, cols = ctypes.c_void_p(), ctypes.c_int(), ctypes.c_int64(), ctypes.c_int()
+        _check(self._L.icon_grid_table_host(self._h, TABLE_ID[name], ctypes.byref(ptr), ctypes.byref(dt),
+                                            ctypes.byref(rows), ctypes.byref(cols)))
+        npdt = np.dtype(_NP[dt.value])
+        n = rows.value * cols.value
+        buf = (ctypes.c_char * (n * npdt.itemsize)).from_address(ptr.value)
+        a = np.frombuffer(buf, dtype=npdt, count=n)
+        a.flags.writeable = False
+        return a.reshape(rows.value, cols.value) if cols.value > 1 else a
+
+    def table_device(self, name, dtype=ICON_F64):
+        p = ctypes.c_void_p()
+        _check(self._L.icon_grid_table_device(self._h, TABLE_ID[name], dtype, ctypes.byref(p)))
+        return p.value
+
+    def set_option(self, option, value):
+        _check(self._L.icon_grid_set_option(self._h, option, value))
+
+    @property
+    def launch_count(self):
+        return int(self._L.icon_grid_launch_count(self._h))
+
+
+def icon_grid_create(k, seed=0, flags=0):
+    return IconGrid(k, seed, flags)
+
+
+def _dtype_of(t):
+    import torch
+    if t.dtype == torch.float64:
+        return ICON_F64
+    if t.dtype == torch.float32:
+        return ICON_F32
+    raise TypeError("fields must be float64 or float32 tensors")
+
+
+def dycore_div_vort(grid, vn, div, vort, nlev, stream=None):
+    """S1+S2. vn [ne][ldk], div [nc][ldk], vort [nv][ldk]: CUDA tensors of one dtype."""
+    _check(grid._L.dycore_div_vort(grid._h, _dtype_of(vn), int(nlev), int(vn.shape[1]), _dptr(vn), _dptr(div),
+                                   _dptr(vort), _stream_ptr(stream)))
+
+
+def dycore_velocity_tendencies(grid, z_half, vn, w, ddt_vn, nlev, vt=None, ke_c=None, vort=None, stream=None):
+    """S3-S7. z_half: host float64 [nlev+1]; vn/ddt_vn [ne][ldk], w [nc][ldk_w]: CUDA tensors."""
+    z = np.ascontiguousarray(z_half, dtype=np.float64)
+    if z.size != nlev + 1:
+        raise ValueError("z_half must have nlev+1 entries")
+    _check(grid._L.dycore_velocity_tendencies(grid._h, _dtype_of(vn), int(nlev), int(vn.shape[1]), int(w.shape[1]),
+                                              _dptr(z), _dptr(vn), _dptr(w), _dptr(ddt_vn), _dptr(vt), _dptr(ke_c),
+                                              _dptr(vort), _stream_ptr(stream)))
+
+
+def dycore_step_host(grid, z_half, vn_host, w_host, ddt_vn_host, div_host, vort_host, nlev):
+    """End-to-end step on HOST buffers (pinned torch CPU tensors or numpy arrays)."""
+    z = np.ascontiguousarray(z_half, dtype=np.float64)
+    f64 = (vn_host.dtype == np.float64) if isinstance(vn_host, np.ndarray) else (str(vn_host.dtype) == "torch.float64")
+    _check(grid._L.dycore_step_host(grid._h, ICON_F64 if f64 else ICON_F32, int(nlev), int(vn_host.shape[1]),
+                                    int(w_host.shape[1]), _dptr(z), _dptr(vn_host), _dptr(w_host), _dptr(ddt_vn_host),
+                                    _dptr(div_host), _dptr(vort_host)))

@@ -1,0 +1,496 @@
+// api.cu -- the C-ABI of libicon_dycore (include/icon_dycore.h): argument checks, table upload,
+// per-call coefficient preparation and kernel launches on the caller's stream. No torch types,
+// no CPU fallback: every compute entry point fails with ICON_ECUDA when no device is usable.
+#include <cuda_runtime.h>
+
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/icon_dycore.h"
+#include "device_grid.hpp"
+#include "kernels.cuh"
+
+namespace {
+
+thread_local std::string t_last_error;
+
+int fail(int code, const std::string& msg) {
+    t_last_error = msg;
+    return code;
+}
+int fail_cuda(cudaError_t e, const char* what) {
+    t_last_error = std::string(what) + ": " + cudaGetErrorString(e);
+    return ICON_ECUDA;
+}
+
+#define CU_TRY(expr)                                      \
+    do {                                                  \
+        cudaError_t _e = (expr);                          \
+        if (_e != cudaSuccess) return fail_cuda(_e, #expr); \
+    } while (0)
+
+template <class T>
+int dev_alloc(icon_grid* g, size_t count, T** out) {
+    void* p = nullptr;
+    cudaError_t e = cudaMalloc(&p, count * sizeof(T) + 16);
+    if (e != cudaSuccess) {
+        t_last_error = std::string("cudaMalloc: ") + cudaGetErrorString(e);
+        return e == cudaErrorMemoryAllocation ? ICON_ENOMEM : ICON_ECUDA;
+    }
+    g->owned.push_back(p);
+    *out = static_cast<T*>(p);
+    return ICON_OK;
+}
+void dev_release(icon_grid* g, void* p) {
+    if (!p) return;
+    for (auto& q : g->owned)
+        if (q == p) {
+            cudaFree(p);
+            q = nullptr;
+        }
+}
+
+// upload rows of `src` ([n][cols], user order) to the device; when user_of_pos is non-empty the
+// device copy is in work order: row p = src row user_of_pos[p].
+template <class S, class D>
+int upload_rows(icon_grid* g, const std::vector<S>& src, int cols, const std::vector<int32_t>& user_of_pos, D** out) {
+    const size_t n = src.size() / (size_t)cols;
+    std::vector<D> tmp(src.size());
+    if (user_of_pos.empty()) {
+        for (size_t i = 0; i < src.size(); ++i) tmp[i] = (D)src[i];
+    } else {
+#pragma omp parallel for schedule(static)
+        for (int64_t p = 0; p < (int64_t)n; ++p)
+            for (int s = 0; s < cols; ++s) tmp[(size_t)p * cols + s] = (D)src[(size_t)user_of_pos[p] * cols + s];
+    }
+    int rc = dev_alloc(g, tmp.size(), out);
+    if (rc != ICON_OK) return rc;
+    CU_TRY(cudaMemcpy(*out, tmp.data(), tmp.size() * sizeof(D), cudaMemcpyHostToDevice));
+    return ICON_OK;
+}
+
+int upload_inverse(icon_grid* g, const std::vector<int32_t>& user_of_pos, int32_t** out_user, int32_t** out_pos) {
+    if (user_of_pos.empty()) return ICON_OK;
+    std::vector<int32_t> pos(user_of_pos.size());
+    for (size_t p = 0; p < user_of_pos.size(); ++p) pos[(size_t)user_of_pos[p]] = (int32_t)p;
+    int rc = dev_alloc(g, pos.size(), out_user);
+    if (rc != ICON_OK) return rc;
+    CU_TRY(cudaMemcpy(*out_user, user_of_pos.data(), pos.size() * 4, cudaMemcpyHostToDevice));
+    rc = dev_alloc(g, pos.size(), out_pos);
+    if (rc != ICON_OK) return rc;
+    CU_TRY(cudaMemcpy(*out_pos, pos.data(), pos.size() * 4, cudaMemcpyHostToDevice));
+    return ICON_OK;
+}
+
+const std::vector<int32_t> kIdentity;
+
+int upload_index_tables(icon_grid* g) {
+    const icon::HostGrid& h = g->host;
+    const auto& uc = g->worklist ? h.user_of_pos_c : kIdentity;
+    const auto& ue = g->worklist ? h.user_of_pos_e : kIdentity;
+    const auto& uv = g->worklist ? h.user_of_pos_v : kIdentity;
+    int rc;
+    if ((rc = upload_rows(g, h.c2e, 3, uc, &g->tab.c2e))) return rc;
+    if ((rc = upload_rows(g, h.e2c, 2, ue, &g->tab.e2c))) return rc;
+    if ((rc = upload_rows(g, h.e2v, 2, ue, &g->tab.e2v))) return rc;
+    if ((rc = upload_rows(g, h.e2e4, 4, ue, &g->tab.e2e4))) return rc;
+    if ((rc = upload_rows(g, h.v2e, 6, uv, &g->tab.v2e))) return rc;
+    if ((rc = upload_inverse(g, uc, &g->tab.user_c, &g->tab.pos_c))) return rc;
+    if ((rc = upload_inverse(g, ue, &g->tab.user_e, &g->tab.pos_e))) return rc;
+    if ((rc = upload_inverse(g, uv, &g->tab.user_v, &g->tab.pos_v))) return rc;
+    return ICON_OK;
+}
+
+template <class T>
+int ensure_coeffs(icon_grid* g, icon::DevCoeffs<T>& c) {
+    if (c.ready) return ICON_OK;
+    const icon::HostGrid& h = g->host;
+    const auto& uc = g->worklist ? h.user_of_pos_c : kIdentity;
+    const auto& ue = g->worklist ? h.user_of_pos_e : kIdentity;
+    const auto& uv = g->worklist ? h.user_of_pos_v : kIdentity;
+    int rc;
+    if ((rc = upload_rows(g, h.rbf, 4, ue, &c.rbf))) return rc;
+    if ((rc = upload_rows(g, h.bln, 3, uc, &c.bln))) return rc;
+    if ((rc = upload_rows(g, h.geofac_div, 3, uc, &c.geofac_div))) return rc;
+    if ((rc = upload_rows(g, h.geofac_rot, 6, uv, &c.geofac_rot))) return rc;
+    if ((rc = upload_rows(g, h.inv_d_e, 1, ue, &c.inv_d_e))) return rc;
+    if ((rc = upload_rows(g, h.f_e, 1, ue, &c.f_e))) return rc;
+    if ((rc = upload_rows(g, h.c_lin, 2, ue, &c.c_lin))) return rc;
+    c.ready = true;
+    return ICON_OK;
+}
+
+// Reading P-14 folded into three per-level coefficients:
+//   (vn_ie(k) - vn_ie(k+1)) / dz_k = A_k vn(k-1) + B_k vn(k) + C_k vn(k+1)
+// half level kh is a two-point linear combination of full levels: interior kh uses (kh, kh-1)
+// with weights (g, 1-g), g = dz_{kh-1}/(dz_{kh-1}+dz_kh); kh = 0 and kh = K extrapolate linearly in
+// z from the two nearest full levels.
+void vertical_coefficients(const double* zh, int K, std::vector<double>& abc) {
+    abc.assign(3 * (size_t)K, 0.0);
+    auto zf = [&](int k) { return 0.5 * (zh[k] + zh[k + 1]); };
+    auto add_half = [&](int k, int kh, double sign) {
+        int ia, ib;
+        double ca, cb;
+        if (kh == 0) {
+            double r = (zh[0] - zf(0)) / (zf(0) - zf(1));
+            ia = 0; ca = 1.0 + r; ib = 1; cb = -r;
+        } else if (kh == K) {
+            double r = (zh[K] - zf(K - 1)) / (zf(K - 1) - zf(K - 2));
+            ia = K - 1; ca = 1.0 + r; ib = K - 2; cb = -r;
+        } else {
+            double up = zh[kh - 1] - zh[kh], dn = zh[kh] - zh[kh + 1];
+            double gk = up / (up + dn);
+            ia = kh; ca = gk; ib = kh - 1; cb = 1.0 - gk;
+        }
+        const double inv_dz = 1.0 / (zh[k] - zh[k + 1]);
+        abc[(size_t)(ia - k + 1) * K + k] += sign * ca * inv_dz;
+        abc[(size_t)(ib - k + 1) * K + k] += sign * cb * inv_dz;
+    };
+    for (int k = 0; k < K; ++k) {
+        add_half(k, k, +1.0);
+        add_half(k, k + 1, -1.0);
+    }
+}
+
+int get_level_coeffs(icon_grid* g, int dtype, int nlev, const double* z_half, cudaStream_t s, void** out) {
+    for (int k = 0; k < nlev; ++k)
+        if (!(z_half[k] > z_half[k + 1])) return fail(ICON_EINVAL, "z_half must be strictly decreasing");
+    for (auto& lc : g->level_coeffs)
+        if (lc.dtype == dtype && (int)lc.z_half.size() == nlev + 1 &&
+            std::memcmp(lc.z_half.data(), z_half, sizeof(double) * (nlev + 1)) == 0) {
+            *out = lc.abc;
+            return ICON_OK;
+        }
+    std::vector<double> abc;
+    vertical_coefficients(z_half, nlev, abc);
+    icon::LevelCoeffs lc;
+    lc.dtype = dtype;
+    lc.z_half.assign(z_half, z_half + nlev + 1);
+    int rc;
+    if (dtype == ICON_F64) {
+        double* d = nullptr;
+        if ((rc = dev_alloc(g, abc.size(), &d))) return rc;
+        // pageable source: the runtime stages it before returning, so `abc` may die afterwards
+        CU_TRY(cudaMemcpyAsync(d, abc.data(), abc.size() * 8, cudaMemcpyHostToDevice, s));
+        lc.abc = d;
+    } else {
+        std::vector<float> f(abc.begin(), abc.end());
+        float* d = nullptr;
+        if ((rc = dev_alloc(g, f.size(), &d))) return rc;
+        CU_TRY(cudaMemcpyAsync(d, f.data(), f.size() * 4, cudaMemcpyHostToDevice, s));
+        lc.abc = d;
+    }
+    if (g->level_coeffs.size() >= 16) {   // bounded cache
+        dev_release(g, g->level_coeffs.front().abc);
+        g->level_coeffs.erase(g->level_coeffs.begin());
+    }
+    g->level_coeffs.push_back(lc);
+    *out = lc.abc;
+    return ICON_OK;
+}
+
+int check_field(const void* p, const char* name) {
+    if (!p) return fail(ICON_EINVAL, std::string(name) + " is NULL");
+    if (reinterpret_cast<uintptr_t>(p) % 16) return fail(ICON_EINVAL, std::string(name) + " is not 16-byte aligned");
+    return ICON_OK;
+}
+
+int check_common(icon_grid* g, int dtype, int nlev, int ldk, int min_lev) {
+    if (!g) return fail(ICON_EINVAL, "grid handle is NULL");
+    if (g->host_only) return fail(ICON_ECUDA, "grid was created with ICON_HOST_ONLY: no device tables, and there is no CPU path");
+    if (dtype != ICON_F64 && dtype != ICON_F32) return fail(ICON_EINVAL, "dtype must be ICON_F64 or ICON_F32");
+    if (nlev < min_lev || nlev > 4096) return fail(ICON_EINVAL, "nlev out of range");
+    if (ldk < nlev) return fail(ICON_EINVAL, "ldk < nlev");
+    const int es = dtype == ICON_F64 ? 8 : 4;
+    if (((int64_t)ldk * es) % 16) return fail(ICON_EINVAL, "ldk*sizeof(T) must be a multiple of 16");
+    return ICON_OK;
+}
+
+template <class T>
+int ensure_workspace(icon_grid* g, int dtype, int64_t ldk) {
+    icon::Workspace& ws = g->ws;
+    if (ws.dtype == dtype && ws.ldk == ldk) return ICON_OK;
+    dev_release(g, ws.vt); dev_release(g, ws.ke_e); dev_release(g, ws.ke_c); dev_release(g, ws.vort);
+    ws = icon::Workspace();
+    int rc;
+    T *a, *b, *c, *d;
+    if ((rc = dev_alloc(g, (size_t)(g->host.ne * ldk), &a))) return rc;
+    if ((rc = dev_alloc(g, (size_t)(g->host.ne * ldk), &b))) return rc;
+    if ((rc = dev_alloc(g, (size_t)(g->host.nc * ldk), &c))) return rc;
+    if ((rc = dev_alloc(g, (size_t)(g->host.nv * ldk), &d))) return rc;
+    ws.vt = a; ws.ke_e = b; ws.ke_c = c; ws.vort = d;
+    ws.dtype = dtype; ws.ldk = ldk;
+    return ICON_OK;
+}
+
+template <class T>
+int tendencies_impl(icon_grid* g, icon::DevCoeffs<T>& c, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
+                    const void* vn, const void* w, void* ddt_vn, void* vt_opt, void* ke_c_opt, void* vort_opt,
+                    cudaStream_t s) {
+    int rc;
+    if ((rc = ensure_coeffs(g, c))) return rc;
+    void* abc = nullptr;
+    if ((rc = get_level_coeffs(g, dtype, nlev, z_half, s, &abc))) return rc;
+    const bool want_opt = vt_opt || ke_c_opt || vort_opt;
+    int n;
+    if (g->options[ICON_OPT_TENDENCY_KERNEL] == 0 || want_opt) {
+        // optional outputs are produced by the unfused pipeline, which materialises them anyway
+        if ((rc = ensure_workspace<T>(g, dtype, ldk))) return rc;
+        T* vt = vt_opt ? (T*)vt_opt : (T*)g->ws.vt;
+        T* kc = ke_c_opt ? (T*)ke_c_opt : (T*)g->ws.ke_c;
+        T* vo = vort_opt ? (T*)vort_opt : (T*)g->ws.vort;
+        n = icon::launch_tendencies_unfused<T>(*g, c, nlev, ldk, ldk_w, (const T*)abc, (const T*)vn, (const T*)w,
+                                               (T*)ddt_vn, vt, (T*)g->ws.ke_e, kc, vo, s);
+    } else {
+        n = icon::launch_tendencies_fused<T>(*g, c, nlev, ldk, ldk_w, (const T*)abc, (const T*)vn, (const T*)w,
+                                             (T*)ddt_vn, nullptr, nullptr, nullptr, s);
+    }
+    if (n < 0) return fail_cuda((cudaError_t)(-n), "kernel launch");
+    g->launches += n;
+    return ICON_OK;
+}
+
+struct TableInfo {
+    const void* ptr;
+    int dtype;
+    int64_t rows;
+    int cols;
+};
+int table_info(const icon_grid* g, int which, TableInfo* t) {
+    const icon::HostGrid& h = g->host;
+    auto I = [&](const std::vector<int32_t>& v, int64_t rows, int cols) { *t = {v.data(), ICON_T_I32, rows, cols}; };
+    auto B = [&](const std::vector<int8_t>& v, int64_t rows, int cols) { *t = {v.data(), ICON_T_I8, rows, cols}; };
+    auto D = [&](const std::vector<double>& v, int64_t rows, int cols) { *t = {v.data(), ICON_T_F64, rows, cols}; };
+    switch (which) {
+        case ICON_TAB_C2V: I(h.c2v, h.nc, 3); break;
+        case ICON_TAB_C2E: I(h.c2e, h.nc, 3); break;
+        case ICON_TAB_E2C: I(h.e2c, h.ne, 2); break;
+        case ICON_TAB_E2V: I(h.e2v, h.ne, 2); break;
+        case ICON_TAB_E2E4: I(h.e2e4, h.ne, 4); break;
+        case ICON_TAB_V2E: I(h.v2e, h.nv, 6); break;
+        case ICON_TAB_V2C: I(h.v2c, h.nv, 6); break;
+        case ICON_TAB_V_DEG: I(h.v_deg, h.nv, 1); break;
+        case ICON_TAB_C_OS: B(h.c_os, h.nc, 3); break;
+        case ICON_TAB_V_OS: B(h.v_os, h.nv, 6); break;
+        case ICON_TAB_VERT_XYZ: D(h.vert_xyz, h.nv, 3); break;
+        case ICON_TAB_CELL_XYZ: D(h.cell_xyz, h.nc, 3); break;
+        case ICON_TAB_EDGE_XYZ: D(h.edge_xyz, h.ne, 3); break;
+        case ICON_TAB_EDGE_NORMAL: D(h.edge_normal, h.ne, 3); break;
+        case ICON_TAB_L_E: D(h.l_e, h.ne, 1); break;
+        case ICON_TAB_D_E: D(h.d_e, h.ne, 1); break;
+        case ICON_TAB_INV_D_E: D(h.inv_d_e, h.ne, 1); break;
+        case ICON_TAB_F_E: D(h.f_e, h.ne, 1); break;
+        case ICON_TAB_C_LIN: D(h.c_lin, h.ne, 2); break;
+        case ICON_TAB_RBF: D(h.rbf, h.ne, 4); break;
+        case ICON_TAB_A_C: D(h.a_c, h.nc, 1); break;
+        case ICON_TAB_BLN: D(h.bln, h.nc, 3); break;
+        case ICON_TAB_A_V: D(h.a_v, h.nv, 1); break;
+        case ICON_TAB_GEOFAC_DIV: D(h.geofac_div, h.nc, 3); break;
+        case ICON_TAB_GEOFAC_ROT: D(h.geofac_rot, h.nv, 6); break;
+        default: return fail(ICON_EINVAL, "unknown table selector");
+    }
+    return ICON_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* icon_last_error(void) { return t_last_error.c_str(); }
+
+int icon_grid_create(int bisections_k, uint64_t seed, unsigned flags, icon_grid_t** out) {
+    if (!out) return fail(ICON_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (bisections_k < 0 || bisections_k > 9) return fail(ICON_EINVAL, "bisections_k must be in 0..9");
+    if (flags & ~(ICON_PERMUTE | ICON_LOCALITY_WORKLIST | ICON_HOST_ONLY | ICON_NO_WORKLIST))
+        return fail(ICON_EINVAL, "unknown flag bits");
+    icon_grid* g = new (std::nothrow) icon_grid();
+    if (!g) return fail(ICON_ENOMEM, "out of host memory");
+    g->flags = flags;
+    g->seed = seed;
+    g->host_only = (flags & ICON_HOST_ONLY) != 0;
+    g->options[ICON_OPT_TENDENCY_KERNEL] = 1;
+    try {
+        std::string err = icon::build_host_grid(bisections_k, seed, (flags & ICON_PERMUTE) != 0, g->host);
+        if (!err.empty()) {
+            delete g;
+            return fail(ICON_EINVAL, err);
+        }
+    } catch (const std::bad_alloc&) {
+        delete g;
+        return fail(ICON_ENOMEM, "out of host memory while building the grid");
+    }
+    // the work order (generation order) differs from the user order only on permuted grids
+    g->worklist = (flags & ICON_PERMUTE) && !(flags & ICON_NO_WORKLIST);
+    if (!g->host_only) {
+        int ndev = 0;
+        cudaError_t e = cudaGetDeviceCount(&ndev);
+        if (e != cudaSuccess || ndev == 0) {
+            delete g;
+            return fail(ICON_ECUDA, "no usable CUDA device (there is no CPU fallback)");
+        }
+        int rc = ICON_OK;
+        e = cudaGetDevice(&g->device);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&g->num_sms, cudaDevAttrMultiProcessorCount, g->device);
+        if (e != cudaSuccess) rc = fail_cuda(e, "cudaGetDevice");
+        if (rc == ICON_OK) rc = upload_index_tables(g);
+        if (rc == ICON_OK) rc = ensure_coeffs(g, g->c64);
+        if (rc != ICON_OK) {
+            std::string keep = t_last_error;
+            icon_grid_destroy(g);
+            t_last_error = keep;
+            return rc;
+        }
+    }
+    *out = g;
+    return ICON_OK;
+}
+
+void icon_grid_destroy(icon_grid_t* g) {
+    if (!g) return;
+    for (void* p : g->owned)
+        if (p) cudaFree(p);
+    if (g->stage.stream) cudaStreamDestroy(g->stage.stream);
+    delete g;
+}
+
+int icon_grid_counts(const icon_grid_t* g, int64_t* nc, int64_t* ne, int64_t* nv) {
+    if (!g) return fail(ICON_EINVAL, "grid handle is NULL");
+    if (nc) *nc = g->host.nc;
+    if (ne) *ne = g->host.ne;
+    if (nv) *nv = g->host.nv;
+    return ICON_OK;
+}
+
+int icon_grid_table_host(const icon_grid_t* g, int which, const void** ptr, int* dtype, int64_t* rows, int* cols) {
+    if (!g) return fail(ICON_EINVAL, "grid handle is NULL");
+    TableInfo t;
+    int rc = table_info(g, which, &t);
+    if (rc) return rc;
+    if (ptr) *ptr = t.ptr;
+    if (dtype) *dtype = t.dtype;
+    if (rows) *rows = t.rows;
+    if (cols) *cols = t.cols;
+    return ICON_OK;
+}
+
+int icon_grid_table_device(icon_grid_t* g, int which, int dtype, const void** dptr) {
+    if (!g || !dptr) return fail(ICON_EINVAL, "NULL argument");
+    if (g->host_only) return fail(ICON_EUNSUPPORTED, "grid was created with ICON_HOST_ONLY");
+    if (dtype != ICON_F64 && dtype != ICON_F32) return fail(ICON_EINVAL, "dtype must be ICON_F64 or ICON_F32");
+    TableInfo t;
+    int rc = table_info(g, which, &t);
+    if (rc) return rc;
+    const int key_dtype = t.dtype == ICON_T_F64 ? dtype : -1;
+    auto key = std::make_pair(which, key_dtype);
+    auto it = g->public_dev.find(key);
+    if (it != g->public_dev.end()) {
+        *dptr = it->second;
+        return ICON_OK;
+    }
+    const size_t n = (size_t)t.rows * t.cols;
+    void* d = nullptr;
+    if (t.dtype == ICON_T_F64 && dtype == ICON_F32) {
+        const double* src = (const double*)t.ptr;
+        std::vector<float> f(src, src + n);
+        float* p;
+        if ((rc = dev_alloc(g, n, &p))) return rc;
+        CU_TRY(cudaMemcpy(p, f.data(), n * 4, cudaMemcpyHostToDevice));
+        d = p;
+    } else {
+        const size_t es = t.dtype == ICON_T_F64 ? 8 : (t.dtype == ICON_T_I32 ? 4 : 1);
+        char* p;
+        if ((rc = dev_alloc(g, n * es, &p))) return rc;
+        CU_TRY(cudaMemcpy(p, t.ptr, n * es, cudaMemcpyHostToDevice));
+        d = p;
+    }
+    g->public_dev[key] = d;
+    *dptr = d;
+    return ICON_OK;
+}
+
+int icon_grid_set_option(icon_grid_t* g, int option, int value) {
+    if (!g) return fail(ICON_EINVAL, "grid handle is NULL");
+    if (option < 0 || option >= ICON_OPT_COUNT) return fail(ICON_EINVAL, "unknown option");
+    if (option == ICON_OPT_TENDENCY_KERNEL && (value < 0 || value > 1)) return fail(ICON_EINVAL, "bad option value");
+    g->options[option] = value;
+    return ICON_OK;
+}
+
+int64_t icon_grid_launch_count(const icon_grid_t* g) { return g ? g->launches : 0; }
+
+int dycore_div_vort(icon_grid_t* g, int dtype, int nlev, int ldk, const void* vn, void* div, void* vort,
+                    void* cuda_stream) {
+    int rc = check_common(g, dtype, nlev, ldk, 1);
+    if (rc) return rc;
+    if ((rc = check_field(vn, "vn")) || (rc = check_field(div, "div")) || (rc = check_field(vort, "vort"))) return rc;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    int n;
+    if (dtype == ICON_F64) {
+        if ((rc = ensure_coeffs(g, g->c64))) return rc;
+        n = icon::launch_div_vort<double>(*g, g->c64, nlev, ldk, (const double*)vn, (double*)div, (double*)vort, s);
+    } else {
+        if ((rc = ensure_coeffs(g, g->c32))) return rc;
+        n = icon::launch_div_vort<float>(*g, g->c32, nlev, ldk, (const float*)vn, (float*)div, (float*)vort, s);
+    }
+    if (n < 0) return fail_cuda((cudaError_t)(-n), "kernel launch");
+    g->launches += n;
+    return ICON_OK;
+}
+
+int dycore_velocity_tendencies(icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
+                               const void* vn, const void* w, void* ddt_vn, void* vt_opt, void* ke_c_opt,
+                               void* vort_opt, void* cuda_stream) {
+    int rc = check_common(g, dtype, nlev, ldk, 2);
+    if (rc) return rc;
+    if (ldk_w < nlev + 1) return fail(ICON_EINVAL, "ldk_w < nlev+1");
+    if (((int64_t)ldk_w * (dtype == ICON_F64 ? 8 : 4)) % 16) return fail(ICON_EINVAL, "ldk_w*sizeof(T) must be a multiple of 16");
+    if (!z_half) return fail(ICON_EINVAL, "z_half is NULL");
+    if ((rc = check_field(vn, "vn")) || (rc = check_field(w, "w")) || (rc = check_field(ddt_vn, "ddt_vn"))) return rc;
+    if (vt_opt && (rc = check_field(vt_opt, "vt_opt"))) return rc;
+    if (ke_c_opt && (rc = check_field(ke_c_opt, "ke_c_opt"))) return rc;
+    if (vort_opt && (rc = check_field(vort_opt, "vort_opt"))) return rc;
+    if (ddt_vn == vn || ddt_vn == w) return fail(ICON_EINVAL, "outputs must not alias inputs");
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    if (dtype == ICON_F64)
+        return tendencies_impl<double>(g, g->c64, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, vt_opt, ke_c_opt, vort_opt, s);
+    return tendencies_impl<float>(g, g->c32, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, vt_opt, ke_c_opt, vort_opt, s);
+}
+
+int dycore_step_host(icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
+                     const void* vn_host, const void* w_host, void* ddt_vn_host, void* div_host, void* vort_host) {
+    int rc = check_common(g, dtype, nlev, ldk, 2);
+    if (rc) return rc;
+    if (!vn_host || !w_host || !ddt_vn_host || !div_host || !vort_host) return fail(ICON_EINVAL, "NULL host buffer");
+    const size_t es = dtype == ICON_F64 ? 8 : 4;
+    icon::HostStage& st = g->stage;
+    if (!st.stream) CU_TRY(cudaStreamCreateWithFlags(&st.stream, cudaStreamNonBlocking));
+    if (st.dtype != dtype || st.ldk != ldk || st.ldk_w != ldk_w) {
+        dev_release(g, st.vn); dev_release(g, st.w); dev_release(g, st.ddt); dev_release(g, st.div); dev_release(g, st.vort);
+        st.vn = st.w = st.ddt = st.div = st.vort = nullptr;
+        char *a, *b, *c, *d, *e;
+        if ((rc = dev_alloc(g, (size_t)g->host.ne * ldk * es, &a))) return rc;
+        if ((rc = dev_alloc(g, (size_t)g->host.nc * ldk_w * es, &b))) return rc;
+        if ((rc = dev_alloc(g, (size_t)g->host.ne * ldk * es, &c))) return rc;
+        if ((rc = dev_alloc(g, (size_t)g->host.nc * ldk * es, &d))) return rc;
+        if ((rc = dev_alloc(g, (size_t)g->host.nv * ldk * es, &e))) return rc;
+        st.vn = a; st.w = b; st.ddt = c; st.div = d; st.vort = e;
+        st.dtype = dtype; st.ldk = ldk; st.ldk_w = ldk_w;
+    }
+    const size_t ne = (size_t)g->host.ne, nc = (size_t)g->host.nc, nv = (size_t)g->host.nv;
+    CU_TRY(cudaMemcpyAsync(st.vn, vn_host, ne * ldk * es, cudaMemcpyHostToDevice, st.stream));
+    CU_TRY(cudaMemcpyAsync(st.w, w_host, nc * ldk_w * es, cudaMemcpyHostToDevice, st.stream));
+    if ((rc = dycore_velocity_tendencies(g, dtype, nlev, ldk, ldk_w, z_half, st.vn, st.w, st.ddt, nullptr, nullptr,
+                                         nullptr, st.stream)))
+        return rc;
+    if ((rc = dycore_div_vort(g, dtype, nlev, ldk, st.vn, st.div, st.vort, st.stream))) return rc;
+    CU_TRY(cudaMemcpyAsync(ddt_vn_host, st.ddt, ne * ldk * es, cudaMemcpyDeviceToHost, st.stream));
+    CU_TRY(cudaMemcpyAsync(div_host, st.div, nc * ldk * es, cudaMemcpyDeviceToHost, st.stream));
+    CU_TRY(cudaMemcpyAsync(vort_host, st.vort, nv * ldk * es, cudaMemcpyDeviceToHost, st.stream));
+    CU_TRY(cudaStreamSynchronize(st.stream));
+    return ICON_OK;
+}
+
+}  // extern "C"

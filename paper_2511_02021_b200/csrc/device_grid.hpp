@@ -1,0 +1,85 @@
+// device_grid.hpp -- the opaque icon_grid handle: host tables + device tables + workspaces.
+// Internal header of libicon_dycore.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+#include <map>
+#include <vector>
+
+#include "host_grid.hpp"
+
+namespace icon {
+
+// Device tables the kernels read. Rows are in WORK ORDER (generation order = spatially local,
+// identical to user order unless the grid is permuted); entries are USER ids, so they address
+// the caller's fields directly.
+template <class T>
+struct DevCoeffs {
+    T* rbf = nullptr;         // [ne][4]
+    T* bln = nullptr;         // [nc][3]
+    T* geofac_div = nullptr;  // [nc][3]
+    T* geofac_rot = nullptr;  // [nv][6]
+    T* inv_d_e = nullptr;     // [ne]
+    T* f_e = nullptr;         // [ne]
+    T* c_lin = nullptr;       // [ne][2]
+    bool ready = false;
+};
+
+struct DevTables {
+    int32_t* c2e = nullptr;   // [nc][3]
+    int32_t* e2c = nullptr;   // [ne][2]
+    int32_t* e2v = nullptr;   // [ne][2]
+    int32_t* e2e4 = nullptr;  // [ne][4]
+    int32_t* v2e = nullptr;   // [nv][6]
+    // user id of work position p; nullptr = identity
+    int32_t* user_c = nullptr;
+    int32_t* user_e = nullptr;
+    int32_t* user_v = nullptr;
+    // work position of user id (inverse of the above); nullptr = identity
+    int32_t* pos_c = nullptr;
+    int32_t* pos_e = nullptr;
+    int32_t* pos_v = nullptr;
+};
+
+// per-level coefficients of the vertical term (reading P-14), device copy for one z_half
+struct LevelCoeffs {
+    std::vector<double> z_half;   // host key
+    int dtype = 0;
+    void* abc = nullptr;          // device [3][nlev] of T: A_k, B_k, C_k
+};
+
+struct Workspace {                // unfused pipeline intermediates, [n][ldk] of T
+    int dtype = -1;
+    int64_t ldk = 0;
+    void *vt = nullptr, *ke_e = nullptr, *ke_c = nullptr, *vort = nullptr;
+};
+
+struct HostStage {                // device staging for dycore_step_host
+    int dtype = -1;
+    int64_t ldk = 0, ldk_w = 0;
+    void *vn = nullptr, *w = nullptr, *ddt = nullptr, *div = nullptr, *vort = nullptr;
+    cudaStream_t stream = nullptr;
+};
+
+}  // namespace icon
+
+struct icon_grid {
+    icon::HostGrid host;
+    unsigned flags = 0;
+    uint64_t seed = 0;
+    bool host_only = false;
+    bool worklist = false;        // work order differs from user order
+    int device = -1;
+    int num_sms = 0;
+    icon::DevTables tab;
+    icon::DevCoeffs<double> c64;
+    icon::DevCoeffs<float> c32;
+    std::vector<icon::LevelCoeffs> level_coeffs;
+    icon::Workspace ws;
+    icon::HostStage stage;
+    std::map<std::pair<int, int>, void*> public_dev;   // (which, dtype) -> device copy in user order
+    std::vector<void*> owned;                          // every device allocation, freed on destroy
+    int options[8] = {0};
+    int64_t launches = 0;
+};

@@ -1,0 +1,288 @@
+// kernels.cu -- sm_100a kernels for the dycore sweep.
+//
+// Layout facts every kernel here relies on (include/icon_dycore.h):
+//   fields are level-contiguous x[i*ldk + k]; a warp owns ONE entity column and its 32 lanes walk
+//   consecutive levels, so every gather of a neighbour column is a fully coalesced 256-byte
+//   (fp64) / 128-byte (fp32) read, whatever the horizontal numbering is; neighbour indices and
+//   coefficients are warp-uniform and are read once per column, not once per point (the
+//   index-lookup amortisation of PAPER.md:186).
+#include "kernels.cuh"
+
+namespace icon {
+namespace {
+
+constexpr int kWarp = 32;
+
+__device__ __forceinline__ int lane_id() { return threadIdx.x & 31; }
+__device__ __forceinline__ int warp_in_block() { return threadIdx.x >> 5; }
+
+template <class T>
+__device__ __forceinline__ T ldg(const T* p) {
+    return __ldg(p);
+}
+
+// ------------------------------------------------------------------------------------------
+// S1 + S2: div(c,k) = sum_j geofac_div(c,j) vn(c2e[c][j],k); vort(v,k) = sum_j geofac_rot(v,j) vn(v2e[v][j],k)
+// block = 12 warps: warps 0..7 take 8 consecutive cells, warps 8..11 take the 4 vertices of the
+// same stretch of the generation order, so both read the same vn columns while they are in L1/L2.
+// ------------------------------------------------------------------------------------------
+template <class T>
+__global__ void __launch_bounds__(384) k_div_vort(int64_t nc, int64_t nv, int nlev, int64_t ldk,
+                                                  const int32_t* __restrict__ c2e, const T* __restrict__ geofac_div,
+                                                  const int32_t* __restrict__ v2e, const T* __restrict__ geofac_rot,
+                                                  const int32_t* __restrict__ user_c, const int32_t* __restrict__ user_v,
+                                                  const T* __restrict__ vn, T* __restrict__ div, T* __restrict__ vort) {
+    const int w = warp_in_block(), lane = lane_id();
+    if (w < 8) {
+        const int64_t p = (int64_t)blockIdx.x * 8 + w;
+        if (p >= nc) return;
+        const int64_t c = user_c ? user_c[p] : p;
+        const T* col0 = vn + (int64_t)ldg(c2e + 3 * p) * ldk;
+        const T* col1 = vn + (int64_t)ldg(c2e + 3 * p + 1) * ldk;
+        const T* col2 = vn + (int64_t)ldg(c2e + 3 * p + 2) * ldk;
+        const T g0 = ldg(geofac_div + 3 * p), g1 = ldg(geofac_div + 3 * p + 1), g2 = ldg(geofac_div + 3 * p + 2);
+        T* out = div + c * ldk;
+        for (int k = lane; k < nlev; k += kWarp) out[k] = g0 * col0[k] + g1 * col1[k] + g2 * col2[k];
+    } else {
+        const int64_t p = (int64_t)blockIdx.x * 4 + (w - 8);
+        if (p >= nv) return;
+        const int64_t v = user_v ? user_v[p] : p;
+        const T* col[6];
+        T g[6];
+#pragma unroll
+        for (int j = 0; j < 6; ++j) {
+            col[j] = vn + (int64_t)ldg(v2e + 6 * p + j) * ldk;
+            g[j] = ldg(geofac_rot + 6 * p + j);
+        }
+        T* out = vort + v * ldk;
+        for (int k = lane; k < nlev; k += kWarp) {
+            T s = g[0] * col[0][k];
+#pragma unroll
+            for (int j = 1; j < 6; ++j) s += g[j] * col[j][k];
+            out[k] = s;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// unfused pipeline (validation baseline; intermediates through HBM)
+// ------------------------------------------------------------------------------------------
+// S3 + S4a: vt = sum_j rbf(e,j) vn(e2e4[e][j]); KE_e = 1/2 (vn^2 + vt^2)
+template <class T>
+__global__ void __launch_bounds__(256) k_vt_kee(int64_t ne, int nlev, int64_t ldk, const int32_t* __restrict__ e2e4,
+                                                const T* __restrict__ rbf, const int32_t* __restrict__ user_e,
+                                                const T* __restrict__ vn, T* __restrict__ vt, T* __restrict__ ke_e) {
+    const int64_t p = (int64_t)blockIdx.x * 8 + warp_in_block();
+    if (p >= ne) return;
+    const int lane = lane_id();
+    const int64_t e = user_e ? user_e[p] : p;
+    const T* col[4];
+    T r[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        col[j] = vn + (int64_t)ldg(e2e4 + 4 * p + j) * ldk;
+        r[j] = ldg(rbf + 4 * p + j);
+    }
+    const T* own = vn + e * ldk;
+    for (int k = lane; k < nlev; k += kWarp) {
+        T t = r[0] * col[0][k] + r[1] * col[1][k] + r[2] * col[2][k] + r[3] * col[3][k];
+        T n = own[k];
+        vt[e * ldk + k] = t;
+        ke_e[e * ldk + k] = (T)0.5 * (n * n + t * t);
+    }
+}
+
+// S4b + S2: KE_c = sum_j bln(c,j) KE_e(c2e[c][j]); zeta
+template <class T>
+__global__ void __launch_bounds__(384) k_kec_vort(int64_t nc, int64_t nv, int nlev, int64_t ldk,
+                                                  const int32_t* __restrict__ c2e, const T* __restrict__ bln,
+                                                  const int32_t* __restrict__ v2e, const T* __restrict__ geofac_rot,
+                                                  const int32_t* __restrict__ user_c, const int32_t* __restrict__ user_v,
+                                                  const T* __restrict__ ke_e, const T* __restrict__ vn,
+                                                  T* __restrict__ ke_c, T* __restrict__ vort) {
+    const int w = warp_in_block(), lane = lane_id();
+    if (w < 8) {
+        const int64_t p = (int64_t)blockIdx.x * 8 + w;
+        if (p >= nc) return;
+        const int64_t c = user_c ? user_c[p] : p;
+        const T* col0 = ke_e + (int64_t)ldg(c2e + 3 * p) * ldk;
+        const T* col1 = ke_e + (int64_t)ldg(c2e + 3 * p + 1) * ldk;
+        const T* col2 = ke_e + (int64_t)ldg(c2e + 3 * p + 2) * ldk;
+        const T b0 = ldg(bln + 3 * p), b1 = ldg(bln + 3 * p + 1), b2 = ldg(bln + 3 * p + 2);
+        T* out = ke_c + c * ldk;
+        for (int k = lane; k < nlev; k += kWarp) out[k] = b0 * col0[k] + b1 * col1[k] + b2 * col2[k];
+    } else {
+        const int64_t p = (int64_t)blockIdx.x * 4 + (w - 8);
+        if (p >= nv) return;
+        const int64_t v = user_v ? user_v[p] : p;
+        const T* col[6];
+        T g[6];
+#pragma unroll
+        for (int j = 0; j < 6; ++j) {
+            col[j] = vn + (int64_t)ldg(v2e + 6 * p + j) * ldk;
+            g[j] = ldg(geofac_rot + 6 * p + j);
+        }
+        T* out = vort + v * ldk;
+        for (int k = lane; k < nlev; k += kWarp) {
+            T s = g[0] * col[0][k];
+#pragma unroll
+            for (int j = 1; j < 6; ++j) s += g[j] * col[j][k];
+            out[k] = s;
+        }
+    }
+}
+
+// vertical difference (vn_ie(k) - vn_ie(k+1))/dz_k = A_k vn(k-1) + B_k vn(k) + C_k vn(k+1)
+// with A_0 = C_{K-1} = 0 (reading P-14 folded into per-level coefficients on the host)
+template <class T>
+__device__ __forceinline__ T vertical_diff(const T* __restrict__ col, const T* __restrict__ abc, int nlev, int k) {
+    const int km = k > 0 ? k - 1 : 0, kp = k < nlev - 1 ? k + 1 : nlev - 1;
+    return ldg(abc + k) * col[km] + ldg(abc + nlev + k) * col[k] + ldg(abc + 2 * nlev + k) * col[kp];
+}
+
+// S5 + S6 + S7
+template <class T>
+__global__ void __launch_bounds__(256) k_ddt_vn(int64_t ne, int nlev, int64_t ldk, int64_t ldk_w,
+                                                const int32_t* __restrict__ e2c, const int32_t* __restrict__ e2v,
+                                                const T* __restrict__ inv_d_e, const T* __restrict__ f_e,
+                                                const T* __restrict__ c_lin, const int32_t* __restrict__ user_e,
+                                                const T* __restrict__ abc, const T* __restrict__ vn,
+                                                const T* __restrict__ w, const T* __restrict__ vt,
+                                                const T* __restrict__ ke_c, const T* __restrict__ vort,
+                                                T* __restrict__ ddt_vn) {
+    const int64_t p = (int64_t)blockIdx.x * 8 + warp_in_block();
+    if (p >= ne) return;
+    const int lane = lane_id();
+    const int64_t e = user_e ? user_e[p] : p;
+    const int64_t c0 = ldg(e2c + 2 * p), c1 = ldg(e2c + 2 * p + 1), v0 = ldg(e2v + 2 * p), v1 = ldg(e2v + 2 * p + 1);
+    const T inv_d = ldg(inv_d_e + p), f = ldg(f_e + p), cl0 = ldg(c_lin + 2 * p), cl1 = ldg(c_lin + 2 * p + 1);
+    const T* col = vn + e * ldk;
+    for (int k = lane; k < nlev; k += kWarp) {
+        T gradk = (ke_c[c1 * ldk + k] - ke_c[c0 * ldk + k]) * inv_d;
+        T zeta_e = (T)0.5 * (vort[v0 * ldk + k] + vort[v1 * ldk + k]);
+        T H = gradk + vt[e * ldk + k] * (f + zeta_e);
+        T wf0 = (T)0.5 * (w[c0 * ldk_w + k] + w[c0 * ldk_w + k + 1]);
+        T wf1 = (T)0.5 * (w[c1 * ldk_w + k] + w[c1 * ldk_w + k + 1]);
+        T w_e = cl0 * wf0 + cl1 * wf1;
+        ddt_vn[e * ldk + k] = -(H + w_e * vertical_diff(col, abc, nlev, k));
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// fused gather kernel (variant 1): one warp per edge column, every intermediate recomputed in
+// registers from the 15-edge vn stencil; nothing but vn, w and the tables is read, nothing but
+// ddt_vn is written.
+// ------------------------------------------------------------------------------------------
+template <class T>
+__global__ void __launch_bounds__(256) k_tend_gather(int64_t ne, int nlev, int64_t ldk, int64_t ldk_w,
+                                                     const int32_t* __restrict__ c2e, const int32_t* __restrict__ e2c,
+                                                     const int32_t* __restrict__ e2v, const int32_t* __restrict__ e2e4,
+                                                     const int32_t* __restrict__ v2e, const T* __restrict__ rbf,
+                                                     const T* __restrict__ bln, const T* __restrict__ geofac_rot,
+                                                     const T* __restrict__ inv_d_e, const T* __restrict__ f_e,
+                                                     const T* __restrict__ c_lin, const int32_t* __restrict__ user_e,
+                                                     const int32_t* __restrict__ pos_e, const int32_t* __restrict__ pos_c,
+                                                     const int32_t* __restrict__ pos_v, const T* __restrict__ abc,
+                                                     const T* __restrict__ vn, const T* __restrict__ w,
+                                                     T* __restrict__ ddt_vn) {
+    const int64_t p = (int64_t)blockIdx.x * 8 + warp_in_block();
+    if (p >= ne) return;
+    const int lane = lane_id();
+    const int64_t e = user_e ? user_e[p] : p;
+    const int64_t c[2] = {ldg(e2c + 2 * p), ldg(e2c + 2 * p + 1)};
+    const int64_t v[2] = {ldg(e2v + 2 * p), ldg(e2v + 2 * p + 1)};
+    const T inv_d = ldg(inv_d_e + p), f = ldg(f_e + p), cl0 = ldg(c_lin + 2 * p), cl1 = ldg(c_lin + 2 * p + 1);
+    const T* col = vn + e * ldk;
+    for (int k = lane; k < nlev; k += kWarp) {
+        // KE at the two cells: each from its three edges, each edge's vt from its four neighbours
+        T kec[2];
+#pragma unroll
+        for (int s = 0; s < 2; ++s) {
+            const int64_t pc = pos_c ? pos_c[c[s]] : c[s];
+            T acc = (T)0;
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+                const int64_t ej = ldg(c2e + 3 * pc + j);
+                const int64_t pj = pos_e ? pos_e[ej] : ej;
+                T t = (T)0;
+#pragma unroll
+                for (int q = 0; q < 4; ++q) t += ldg(rbf + 4 * pj + q) * vn[(int64_t)ldg(e2e4 + 4 * pj + q) * ldk + k];
+                const T n = vn[ej * ldk + k];
+                acc += ldg(bln + 3 * pc + j) * ((T)0.5 * (n * n + t * t));
+            }
+            kec[s] = acc;
+        }
+        T zeta[2];
+#pragma unroll
+        for (int s = 0; s < 2; ++s) {
+            const int64_t pv = pos_v ? pos_v[v[s]] : v[s];
+            T acc = (T)0;
+#pragma unroll
+            for (int j = 0; j < 6; ++j) acc += ldg(geofac_rot + 6 * pv + j) * vn[(int64_t)ldg(v2e + 6 * pv + j) * ldk + k];
+            zeta[s] = acc;
+        }
+        T vt = (T)0;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) vt += ldg(rbf + 4 * p + q) * vn[(int64_t)ldg(e2e4 + 4 * p + q) * ldk + k];
+        T H = (kec[1] - kec[0]) * inv_d + vt * (f + (T)0.5 * (zeta[0] + zeta[1]));
+        T wf0 = (T)0.5 * (w[c[0] * ldk_w + k] + w[c[0] * ldk_w + k + 1]);
+        T wf1 = (T)0.5 * (w[c[1] * ldk_w + k] + w[c[1] * ldk_w + k + 1]);
+        ddt_vn[e * ldk + k] = -(H + (cl0 * wf0 + cl1 * wf1) * vertical_diff(col, abc, nlev, k));
+    }
+}
+
+inline unsigned blocks_for(int64_t n, int per_block) { return (unsigned)((n + per_block - 1) / per_block); }
+
+}  // namespace
+
+template <class T>
+int launch_div_vort(const icon_grid& g, const DevCoeffs<T>& c, int nlev, int64_t ldk, const T* vn, T* div, T* vort,
+                    cudaStream_t s) {
+    const int64_t nc = g.host.nc, nv = g.host.nv;
+    unsigned nb = blocks_for(nc, 8);
+    unsigned nbv = blocks_for(nv, 4);
+    if (nbv > nb) nb = nbv;
+    k_div_vort<T><<<nb, 384, 0, s>>>(nc, nv, nlev, ldk, g.tab.c2e, c.geofac_div, g.tab.v2e, c.geofac_rot, g.tab.user_c,
+                                     g.tab.user_v, vn, div, vort);
+    cudaError_t err = cudaGetLastError();
+    return err == cudaSuccess ? 1 : -(int)err;
+}
+
+template <class T>
+int launch_tendencies_unfused(const icon_grid& g, const DevCoeffs<T>& c, int nlev, int64_t ldk, int64_t ldk_w,
+                              const T* abc, const T* vn, const T* w, T* ddt_vn, T* vt, T* ke_e, T* ke_c, T* vort,
+                              cudaStream_t s) {
+    const int64_t nc = g.host.nc, ne = g.host.ne, nv = g.host.nv;
+    k_vt_kee<T><<<blocks_for(ne, 8), 256, 0, s>>>(ne, nlev, ldk, g.tab.e2e4, c.rbf, g.tab.user_e, vn, vt, ke_e);
+    unsigned nb = blocks_for(nc, 8), nbv = blocks_for(nv, 4);
+    if (nbv > nb) nb = nbv;
+    k_kec_vort<T><<<nb, 384, 0, s>>>(nc, nv, nlev, ldk, g.tab.c2e, c.bln, g.tab.v2e, c.geofac_rot, g.tab.user_c,
+                                     g.tab.user_v, ke_e, vn, ke_c, vort);
+    k_ddt_vn<T><<<blocks_for(ne, 8), 256, 0, s>>>(ne, nlev, ldk, ldk_w, g.tab.e2c, g.tab.e2v, c.inv_d_e, c.f_e, c.c_lin,
+                                                  g.tab.user_e, abc, vn, w, vt, ke_c, vort, ddt_vn);
+    cudaError_t err = cudaGetLastError();
+    return err == cudaSuccess ? 3 : -(int)err;
+}
+
+template <class T>
+int launch_tendencies_fused(const icon_grid& g, const DevCoeffs<T>& c, int nlev, int64_t ldk, int64_t ldk_w,
+                            const T* abc, const T* vn, const T* w, T* ddt_vn, T*, T*, T*, cudaStream_t s) {
+    const int64_t ne = g.host.ne;
+    k_tend_gather<T><<<blocks_for(ne, 8), 256, 0, s>>>(ne, nlev, ldk, ldk_w, g.tab.c2e, g.tab.e2c, g.tab.e2v, g.tab.e2e4,
+                                                       g.tab.v2e, c.rbf, c.bln, c.geofac_rot, c.inv_d_e, c.f_e, c.c_lin,
+                                                       g.tab.user_e, g.tab.pos_e, g.tab.pos_c, g.tab.pos_v, abc, vn, w,
+                                                       ddt_vn);
+    cudaError_t err = cudaGetLastError();
+    return err == cudaSuccess ? 1 : -(int)err;
+}
+
+#define ICON_INSTANTIATE(T)                                                                                             \
+    template int launch_div_vort<T>(const icon_grid&, const DevCoeffs<T>&, int, int64_t, const T*, T*, T*, cudaStream_t); \
+    template int launch_tendencies_unfused<T>(const icon_grid&, const DevCoeffs<T>&, int, int64_t, int64_t, const T*,     \
+                                              const T*, const T*, T*, T*, T*, T*, T*, cudaStream_t);                      \
+    template int launch_tendencies_fused<T>(const icon_grid&, const DevCoeffs<T>&, int, int64_t, int64_t, const T*,       \
+                                            const T*, const T*, T*, T*, T*, T*, cudaStream_t);
+ICON_INSTANTIATE(double)
+ICON_INSTANTIATE(float)
+
+}  // namespace icon

@@ -1,0 +1,29 @@
+// kernels.cuh -- launcher declarations of the sm_100a kernels (internal).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+#include "device_grid.hpp"
+
+namespace icon {
+
+// S1 + S2 in one launch. Returns the number of kernels launched (>0) or a negative cudaError.
+template <class T>
+int launch_div_vort(const icon_grid& g, const DevCoeffs<T>& c, int nlev, int64_t ldk, const T* vn, T* div, T* vort,
+                    cudaStream_t s);
+
+// S3-S7, unfused: vt/KE_e -> KE_c, zeta -> ddt_vn, intermediates in HBM (workspace or the
+// caller's optional outputs).
+template <class T>
+int launch_tendencies_unfused(const icon_grid& g, const DevCoeffs<T>& c, int nlev, int64_t ldk, int64_t ldk_w,
+                              const T* abc, const T* vn, const T* w, T* ddt_vn, T* vt, T* ke_e, T* ke_c, T* vort,
+                              cudaStream_t s);
+
+// S3-S7, fused gather kernel: every intermediate stays on chip.
+template <class T>
+int launch_tendencies_fused(const icon_grid& g, const DevCoeffs<T>& c, int nlev, int64_t ldk, int64_t ldk_w,
+                            const T* abc, const T* vn, const T* w, T* ddt_vn, T* vt_opt, T* ke_c_opt, T* vort_opt,
+                            cudaStream_t s);
+
+}  // namespace icon

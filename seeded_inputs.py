@@ -85,13 +85,13 @@ def make_fields(config, edge_xyz, edge_normal, nc, nlev=None, ldk=None, ldk_w=No
     ldk_w = nlev + 1 if ldk_w is None else ldk_w
     ne = edge_xyz.shape[0]
     vn = np.empty((ne, ldk), dtype=np.float64)
-    _fill_normal(np.random.Generator(np.random.PCG64(1000 + config)), vn[:, :nlev] if ldk == nlev else vn, 1.0)
+    _fill_normal(np.random.Generator(np.random.PCG64(1000 + config)), vn[:, :nlev], 1.0)
     base = solid_body_vn(edge_xyz, edge_normal)
     if jet:
         base = base + galewsky_jet_vn(edge_xyz, edge_normal)
-    vn += base[:, None]
+    vn[:, :nlev] += base[:, None]
     w = np.empty((nc, ldk_w), dtype=np.float64)
-    _fill_normal(np.random.Generator(np.random.PCG64(2000 + config)), w, 0.1)
+    _fill_normal(np.random.Generator(np.random.PCG64(2000 + config)), w[:, :nlev + 1], 0.1)
     if ldk > nlev:
         vn[:, nlev:] = pad_value
     if ldk_w > nlev + 1:

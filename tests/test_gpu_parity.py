@@ -1,0 +1,269 @@
+"""GPU parity tests (run on the B200 box with -m gpu): the CUDA path, called through the C-ABI,
+against the oracle element by element on the same seeded inputs.
+
+Tolerance (BASELINE.json north_star "relative 1e-12 per point in fp64, 1e-5 in the fp32 variant",
+reading P-16 of DESIGN.md section 3): |gpu - oracle| <= tol * M(p), M(p) = sum of the absolute
+values of the terms entering point p, computed by the oracle next to each output.
+"""
+import numpy as np
+import pytest
+
+import seeded_inputs as si
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"f64": 1e-12, "f32": 1e-5}
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("-m gpu tests need a CUDA device")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def lib():
+    import paper_2511_02021_b200 as lib
+    lib.load_library()          # raises if the CUDA extension has not been built: no fallback
+    return lib
+
+
+_libgrids = {}
+
+
+def lib_grid(lib, k, seed=0, flags=0):
+    key = (k, seed, flags)
+    if key not in _libgrids:
+        _libgrids[key] = lib.IconGrid(k, seed, flags)
+    return _libgrids[key]
+
+
+def run_gpu(torch, lib, g, vn, w, zh, nlev, variant, want_opt=False, sentinel=None):
+    """returns dict of numpy outputs from dycore_velocity_tendencies + dycore_div_vort"""
+    dev = torch.device("cuda:0")
+    tdt = torch.float64 if vn.dtype == np.float64 else torch.float32
+    d_vn = torch.from_numpy(vn).to(dev)
+    d_w = torch.from_numpy(w).to(dev)
+    ldk = vn.shape[1]
+
+    def out(n):
+        t = torch.empty((n, ldk), dtype=tdt, device=dev)
+        t.fill_(float("nan") if sentinel is None else sentinel)
+        return t
+    ddt, div, vort = out(g.ne), out(g.nc), out(g.nv)
+    opt = dict(vt=out(g.ne), ke_c=out(g.nc), vort=out(g.nv)) if want_opt else {}
+    g.set_option(lib.ICON_OPT_TENDENCY_KERNEL, variant)
+    n0 = g.launch_count
+    lib.dycore_velocity_tendencies(g, zh, d_vn, d_w, ddt, nlev, **opt)
+    lib.dycore_div_vort(g, d_vn, div, vort, nlev)
+    torch.cuda.synchronize()
+    assert g.launch_count > n0
+    res = dict(ddt_vn=ddt.cpu().numpy(), div=div.cpu().numpy(), vort=vort.cpu().numpy())
+    for k_, t in opt.items():
+        res[k_ + "_opt"] = t.cpu().numpy()
+    return res
+
+
+def oracle_reference(og, vn, w, zh, nlev, f32):
+    """oracle outputs + tolerance scales; fp32 variant: fp64 arithmetic on fp32-rounded inputs (P-17)"""
+    o = og.rounded_f32() if f32 else og
+    vn64, w64 = vn.astype(np.float64), w.astype(np.float64)
+    vn64 = np.where(np.isnan(vn64), 0.0, vn64)       # padding lanes: never enter the compared levels
+    w64 = np.where(np.isnan(w64), 0.0, w64)
+    t = o.velocity_tendencies(vn64, w64, zh, nlev, with_scale=True)
+    div, vort, md, mv = o.div_vort(vn64, nlev, with_scale=True)
+    t.update(div=div, m_div=md, vort_dv=vort, m_vort=mv)
+    return t
+
+
+def assert_close(name, got, want, scale, tol, nlev):
+    got = got[:, :nlev].astype(np.float64)
+    err = np.abs(got - want[:, :nlev])
+    bound = tol * scale[:, :nlev]
+    bad = ~(err <= bound)
+    assert not bad.any(), "%s: %d points outside tol*M, worst err/M = %.3e" % (
+        name, bad.sum(), (err / np.maximum(scale[:, :nlev], 1e-300)).max())
+
+
+def check_all(res, ref, nlev, tol, opt=False):
+    assert_close("ddt_vn", res["ddt_vn"], ref["ddt_vn"], ref["m_ddt"], tol, nlev)
+    assert_close("div", res["div"], ref["div"], ref["m_div"], tol, nlev)
+    assert_close("vort", res["vort"], ref["vort_dv"], ref["m_vort"], tol, nlev)
+    if opt:
+        assert_close("vort_opt", res["vort_opt"], ref["vort"], ref["m_vort"], tol, nlev)
+        # vt: sum of 4 products, scale = |vn| level of the stencil (<= max |vn| * sum|rbf| ~ 1.3 max|vn|)
+        s_vt = np.full_like(ref["vt"], 1.3 * np.abs(ref["vt"]).max() + 1.0)
+        assert_close("vt_opt", res["vt_opt"], ref["vt"], s_vt, tol, nlev)
+        assert_close("ke_c_opt", res["ke_c_opt"], ref["ke_c"], np.abs(ref["ke_c"]) + np.abs(ref["ke_c"]).mean(), tol, nlev)
+
+
+# ----------------------------------------------------------------------------------------------
+# configs[0]: R2B4 x 90 fp64, element by element, every kernel variant, optional outputs
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", [0, 1])
+def test_config1_r2b4_fp64_elementwise(torch_cuda, lib, oracle_grid, variant):
+    og = oracle_grid(4)
+    g = lib_grid(lib, 4)
+    vn, w, zh = si.make_fields(1, og.edge_xyz, og.edge_normal, og.nc)
+    ref = oracle_reference(og, vn, w, zh, 90, False)
+    res = run_gpu(torch_cuda, lib, g, vn, w, zh, 90, variant, want_opt=(variant == 0))
+    check_all(res, ref, 90, TOL["f64"], opt=(variant == 0))
+    res = run_gpu(torch_cuda, lib, g, vn, w, zh, 90, variant, want_opt=True)
+    check_all(res, ref, 90, TOL["f64"], opt=True)
+
+
+def test_library_geometry_fed_to_oracle(torch_cuda, lib, oracle_mod, oracle_grid):
+    """P-18: operator parity with the oracle evaluating on the LIBRARY's exported tables"""
+    g = lib_grid(lib, 3)
+    t = {n: g.table_host(n) for n in ("c2e", "e2c", "e2v", "e2e4", "v2e", "rbf", "bln", "geofac_rot", "geofac_div",
+                                      "inv_d_e", "f_e", "c_lin")}
+    nlev = 17
+    vn, w, zh = si.make_fields(1, g.table_host("edge_xyz"), g.table_host("edge_normal"), g.nc, nlev=nlev, ldk=18, ldk_w=18)
+    vn64, w64 = np.nan_to_num(vn), np.nan_to_num(w)
+    ref = oracle_mod.velocity_tendencies_from_arrays(t, vn64, w64, zh, nlev)
+    div, md = oracle_mod.divergence(t["c2e"], t["geofac_div"], vn64, nlev)
+    vort, mv = oracle_mod.vorticity(t["v2e"], t["geofac_rot"], vn64, nlev)
+    ref.update(div=div, m_div=md, vort_dv=vort, m_vort=mv)
+    for variant in (0, 1):
+        res = run_gpu(torch_cuda, lib, g, vn, w, zh, nlev, variant)
+        check_all(res, ref, nlev, TOL["f64"])
+
+
+# ----------------------------------------------------------------------------------------------
+# edge cases: tiny grids, ragged level counts, minimum nlev, padded leading dimension
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("k,nlev,ldk,ldk_w", [(0, 2, 2, 4), (0, 3, 4, 4), (1, 31, 32, 32), (1, 33, 34, 34),
+                                               (2, 64, 64, 66), (2, 65, 66, 66), (3, 90, 96, 92), (2, 130, 130, 132)])
+@pytest.mark.parametrize("variant", [0, 1])
+def test_ragged_levels_and_padding(torch_cuda, lib, oracle_grid, k, nlev, ldk, ldk_w, variant):
+    og = oracle_grid(k)
+    g = lib_grid(lib, k)
+    vn, w, zh = si.make_fields(1, og.edge_xyz, og.edge_normal, og.nc, nlev=nlev, ldk=ldk, ldk_w=ldk_w)
+    ref = oracle_reference(og, vn, w, zh, nlev, False)
+    sentinel = -12345.5
+    res = run_gpu(torch_cuda, lib, g, vn, w, zh, nlev, variant, sentinel=sentinel)
+    check_all(res, ref, nlev, TOL["f64"])
+    for name in ("ddt_vn", "div", "vort"):            # padding lanes of outputs are left untouched
+        assert (res[name][:, nlev:] == sentinel).all(), name
+
+
+@pytest.mark.parametrize("flags_extra", [0, 8])
+@pytest.mark.parametrize("variant", [0, 1])
+def test_permuted_grid_fp64(torch_cuda, lib, oracle_grid, flags_extra, variant):
+    """seeded renumbering, with the locality work-list (default) and without (ICON_NO_WORKLIST)"""
+    og = oracle_grid(3, si.PERMUTE_SEED, 1)
+    g = lib_grid(lib, 3, si.PERMUTE_SEED, 1 | flags_extra)
+    nlev = 40
+    vn, w, zh = si.make_fields(4, og.edge_xyz, og.edge_normal, og.nc, nlev=nlev, ldk=40, ldk_w=42, dtype="f64")
+    ref = oracle_reference(og, vn, w, zh, nlev, False)
+    res = run_gpu(torch_cuda, lib, g, vn, w, zh, nlev, variant, want_opt=True)
+    check_all(res, ref, nlev, TOL["f64"], opt=True)
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_fp32_variant_permuted_r2b4(torch_cuda, lib, oracle_grid, variant):
+    """config 4 at a size the oracle finishes in seconds: fp32 fields, permuted ids, tol 1e-5"""
+    og = oracle_grid(4, si.PERMUTE_SEED, 1)
+    g = lib_grid(lib, 4, si.PERMUTE_SEED, 1)
+    vn, w, zh = si.make_fields(4, og.edge_xyz, og.edge_normal, og.nc, ldk=92, ldk_w=92)
+    assert vn.dtype == np.float32
+    ref = oracle_reference(og, vn, w, zh, 90, True)
+    res = run_gpu(torch_cuda, lib, g, vn, w, zh, 90, variant, want_opt=True)
+    check_all(res, ref, 90, TOL["f32"], opt=True)
+
+
+def test_argument_errors_on_device(torch_cuda, lib):
+    torch = torch_cuda
+    g = lib_grid(lib, 1)
+    dev = torch.device("cuda:0")
+    vn = torch.zeros((g.ne, 6), dtype=torch.float64, device=dev)
+    w = torch.zeros((g.nc, 8), dtype=torch.float64, device=dev)
+    out = torch.zeros_like(vn)
+    zh = si.z_half_levels(6)
+    with pytest.raises(lib.IconError):                 # z_half not strictly decreasing
+        lib.dycore_velocity_tendencies(g, zh[::-1].copy(), vn, w, out, 6)
+    with pytest.raises(lib.IconError):                 # output aliases input
+        lib.dycore_velocity_tendencies(g, zh, vn, w, vn, 6)
+    with pytest.raises(lib.IconError):                 # nlev > ldk
+        lib.dycore_div_vort(g, vn, torch.zeros((g.nc, 6), dtype=torch.float64, device=dev),
+                            torch.zeros((g.nv, 6), dtype=torch.float64, device=dev), 7)
+    vn3 = torch.zeros((g.ne, 3), dtype=torch.float64, device=dev)   # ldk*8 not a multiple of 16
+    with pytest.raises(lib.IconError):
+        lib.dycore_div_vort(g, vn3, torch.zeros((g.nc, 3), dtype=torch.float64, device=dev),
+                            torch.zeros((g.nv, 3), dtype=torch.float64, device=dev), 3)
+
+
+def test_step_host_end_to_end(torch_cuda, lib, oracle_grid):
+    """dycore_step_host: host buffers in, host buffers out, same numbers as the device calls"""
+    torch = torch_cuda
+    og = oracle_grid(3)
+    g = lib_grid(lib, 3)
+    vn, w, zh = si.make_fields(1, og.edge_xyz, og.edge_normal, og.nc, nlev=30, ldk=30, ldk_w=32)
+    ref = oracle_reference(og, vn, w, zh, 30, False)
+    h_vn, h_w = torch.from_numpy(vn).pin_memory(), torch.from_numpy(w).pin_memory()
+    ddt = torch.zeros((g.ne, 30), dtype=torch.float64).pin_memory()
+    div = torch.zeros((g.nc, 30), dtype=torch.float64).pin_memory()
+    vort = torch.zeros((g.nv, 30), dtype=torch.float64).pin_memory()
+    g.set_option(lib.ICON_OPT_TENDENCY_KERNEL, 1)
+    lib.dycore_step_host(g, zh, h_vn, h_w, ddt, div, vort, 30)
+    check_all(dict(ddt_vn=ddt.numpy(), div=div.numpy(), vort=vort.numpy()), ref, 30, TOL["f64"])
+
+
+# ----------------------------------------------------------------------------------------------
+# full-size configs (BASELINE.json configs[1..4]) in the launch configuration bench.py times:
+# sampled outputs the oracle computes one by one
+# ----------------------------------------------------------------------------------------------
+def _need_host_gb(gb):
+    import psutil
+    avail = psutil.virtual_memory().available / 2 ** 30
+    if avail < gb:
+        pytest.skip("needs %.0f GB of host memory, %.0f GB available" % (gb, avail))
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("config,host_gb", [(2, 6), (3, 60), (4, 40), (5, 90)])
+def test_full_size_sampled(torch_cuda, lib, oracle_mod, config, host_gb):
+    torch = torch_cuda
+    _need_host_gb(host_gb)
+    cfg = si.CONFIGS[config]
+    flags = 1 if cfg["permute"] else 0
+    seed = si.PERMUTE_SEED if cfg["permute"] else 0
+    nlev = cfg["nlev"]
+    f32 = cfg["dtype"] == "f32"
+    ldk = 92 if f32 else nlev            # fp32: ldk*4 must be a multiple of 16
+    ldk_w = 92 if f32 else nlev + 1 + (nlev + 1) % 2
+    g = lib.IconGrid(cfg["k"], seed, flags)
+    og = oracle_mod.Grid(cfg["k"], seed, flags)
+    for name in ("c2e", "e2c", "e2v", "e2e4", "v2e"):          # bit-exact tables at full size
+        assert np.array_equal(g.table_host(name), og.table(name)), name
+    vn, w, zh = si.make_fields(config, og.edge_xyz, og.edge_normal, og.nc, ldk=ldk, ldk_w=ldk_w)
+    dev = torch.device("cuda:0")
+    d_vn, d_w = torch.from_numpy(vn).to(dev), torch.from_numpy(w).to(dev)
+    ddt = torch.full((g.ne, ldk), float("nan"), dtype=d_vn.dtype, device=dev)
+    div = torch.full((g.nc, ldk), float("nan"), dtype=d_vn.dtype, device=dev)
+    vort = torch.full((g.nv, ldk), float("nan"), dtype=d_vn.dtype, device=dev)
+    lib.dycore_velocity_tendencies(g, zh, d_vn, d_w, ddt, nlev)   # default = the variant bench.py times
+    lib.dycore_div_vort(g, d_vn, div, vort, nlev)
+    torch.cuda.synchronize()
+    o = og.rounded_f32() if f32 else og
+    vn64 = np.nan_to_num(vn.astype(np.float64)) if f32 else np.nan_to_num(vn)
+    w64 = np.nan_to_num(w.astype(np.float64)) if f32 else np.nan_to_num(w)
+    tol = TOL[cfg["dtype"]]
+    nsamp = 20000
+    for what, arr, n in (("ddt_vn", ddt, g.ne), ("div", div, g.nc), ("vort", vort, g.nv)):
+        idx, lev = si.sample_points(300 + config, n, nlev, nsamp)
+        got = arr[torch.from_numpy(idx).to(dev), torch.from_numpy(lev.astype(np.int64)).to(dev)].cpu().numpy().astype(np.float64)
+        want, m = o.sample(what, idx, lev, vn64, nlev, w=w64, z_half=zh)
+        err = np.abs(got - want)
+        assert (err <= tol * m).all(), "%s config %d: worst err/M %.3e" % (what, config, (err / m).max())
+        # properties that hold at any size: every level of every column was written
+        assert not torch.isnan(arr[:, :nlev]).any(), what
+    # discrete Gauss on the GPU result: area-weighted divergence sums to ~0 per level
+    a_c = torch.from_numpy(og.a_c).to(dev).to(torch.float64)
+    l_e = torch.from_numpy(og.l_e).to(dev).to(torch.float64)
+    num = (a_c[:, None] * div[:, :nlev].to(torch.float64)).sum(0).abs()
+    den = (l_e[:, None] * d_vn[:, :nlev].to(torch.float64).abs()).sum(0)
+    assert (num / den).max().item() < (1e-6 if f32 else 1e-13)
+    g.close()

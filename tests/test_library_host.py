@@ -1,0 +1,85 @@
+"""CPU-only tests of the C-ABI library: it loads, exports every symbol include/icon_dycore.h declares,
+its host-side grid generator reproduces the oracle's tables bit-for-bit (two different algorithms,
+SURVEY.md section 8(c) P-18 / test tier T2), and compute calls fail loudly without a GPU."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_2511_02021_b200 as lib
+from paper_2511_02021_b200 import binding
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def L():
+    from paper_2511_02021_b200 import build
+    build.build()
+    return lib.load_library()
+
+
+def test_exports_every_declared_symbol(L):
+    header = open(os.path.join(ROOT, "include", "icon_dycore.h")).read()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\b((?:icon|dycore)_[a-z_0-9]+)\s*\(", header))
+    assert declared == set(binding.EXPORTS)
+    for name in declared:
+        assert getattr(L, name) is not None
+    # table selectors in the header and in the binding agree
+    tabs = re.findall(r"ICON_TAB_([A-Z0-9_]+)", header)
+    tabs = [t.lower() for t in tabs if t != "COUNT"]
+    assert tuple(tabs) == binding.TABLES
+
+
+@pytest.mark.parametrize("k,seed,flags", [(0, 0, 0), (1, 0, 0), (2, 0, 0), (3, 0, 0), (4, 0, 0), (5, 0, 0),
+                                          (2, 4, 1), (4, 4, 1), (3, 99, 1)])
+def test_tables_bit_exact_and_geometry_close(L, oracle_mod, k, seed, flags):
+    g = lib.IconGrid(k, seed, flags | lib.ICON_HOST_ONLY)
+    o = oracle_mod.Grid(k, seed, flags)
+    assert (g.nc, g.ne, g.nv) == (o.nc, o.ne, o.nv)
+    for name in lib.TABLES:
+        a, b = g.table_host(name), o.table(name)
+        assert a.shape == b.shape and a.dtype == b.dtype, name
+        if a.dtype.kind == "i":
+            assert (a == b).all(), name                       # bit-exact index / sign tables
+        else:
+            scale = np.abs(b).max()
+            assert np.abs(a - b).max() <= 1e-12 * scale, name  # P-18: geometry at 1e-12 relative
+    g.close()
+
+
+def test_no_cpu_fallback_and_argument_errors(L):
+    g = lib.IconGrid(1, 0, lib.ICON_HOST_ONLY)
+    dummy = np.zeros(64)
+    p = ctypes.c_void_p(dummy.ctypes.data)
+    rc = L.dycore_div_vort(g._h, 0, 4, 4, p, p, p, None)
+    assert rc == binding.ICON_ECUDA                           # host-only grid: no device tables, no CPU path
+    assert b"no CPU path" in L.icon_last_error()
+    z = np.linspace(1.0, 0.0, 5)
+    rc = L.dycore_velocity_tendencies(g._h, 0, 4, 4, 5, ctypes.c_void_p(z.ctypes.data), p, p, p, None, None, None, None)
+    assert rc == binding.ICON_ECUDA
+    rc = L.icon_grid_table_device(g._h, 0, 0, ctypes.byref(ctypes.c_void_p()))
+    assert rc == binding.ICON_EUNSUPPORTED
+    h = ctypes.c_void_p()
+    assert L.icon_grid_create(10, 0, 4, ctypes.byref(h)) == binding.ICON_EINVAL
+    assert L.icon_grid_create(-1, 0, 4, ctypes.byref(h)) == binding.ICON_EINVAL
+    assert L.icon_grid_create(1, 0, 1 << 10, ctypes.byref(h)) == binding.ICON_EINVAL
+    assert L.icon_grid_create(1, 0, 4, None) == binding.ICON_EINVAL
+    assert L.dycore_div_vort(None, 0, 4, 4, p, p, p, None) == binding.ICON_EINVAL
+    assert L.icon_grid_set_option(g._h, 99, 0) == binding.ICON_EINVAL
+    with pytest.raises(lib.IconError):
+        g.table_device("c2e")
+    g.close()
+
+
+def test_create_without_device_fails_loudly(L):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    h = ctypes.c_void_p()
+    rc = L.icon_grid_create(0, 0, 0, ctypes.byref(h))
+    assert rc == binding.ICON_ECUDA and not h.value
+    assert b"no CPU fallback" in L.icon_last_error()
