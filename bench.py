@@ -180,8 +180,11 @@ def run_ours(args):
     nlev = cfg["nlev"]
     f32 = cfg["dtype"] == "f32"
     gsize = 4 if f32 else 8
-    ldk = (nlev + 3) // 4 * 4 if f32 else (nlev + 1) // 2 * 2
-    ldk_w = (nlev + 4) // 4 * 4 if f32 else (nlev + 2) // 2 * 2
+    # columns padded to whole 128-byte lines so that every 32-level chunk of a column is line aligned
+    # (DESIGN.md section 5); the roofline counts the nlev levels only, never the padding
+    line = 32 if f32 else 16
+    ldk = args.ldk or (nlev + line - 1) // line * line
+    ldk_w = args.ldk_w or (nlev + 1 + line - 1) // line * line
     flags = lib.ICON_PERMUTE if cfg["permute"] else 0
     t0 = time.perf_counter()
     g = lib.IconGrid(cfg["k"], si.PERMUTE_SEED if cfg["permute"] else 0, flags)
@@ -328,6 +331,8 @@ def main():
     ap.add_argument("--config", type=int, default=3, choices=sorted(si.CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--variant", type=int, default=None, help="ICON_OPT_TENDENCY_KERNEL override")
+    ap.add_argument("--ldk", type=int, default=0, help="leading dimension of vn/ddt_vn/div/vort (default: padded to 128 B)")
+    ap.add_argument("--ldk-w", type=int, default=0, dest="ldk_w")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -84,7 +84,8 @@ enum {
 /* runtime options (icon_grid_set_option); defaults are the fastest validated variants */
 enum {
     ICON_OPT_TENDENCY_KERNEL = 0, /* 0 = unfused 3-kernel pipeline through an HBM workspace;
-                                     1 = fused gather kernel (no workspace). */
+                                     1 = fused per-edge gather kernel (no workspace);
+                                     2 = fused register-resident patch kernel (default). */
     ICON_OPT_COUNT
 };
 
@@ -114,6 +115,19 @@ int icon_grid_table_host(const icon_grid_t* g, int which, const void** ptr, int*
 int icon_grid_table_device(icon_grid_t* g, int which, int dtype, const void** dptr);
 
 int icon_grid_set_option(icon_grid_t* g, int option, int value);
+
+/*
+ * icon_grid_worklist_stats -- builds (once, on the host; works on ICON_HOST_ONLY grids) the tile /
+ * patch work-list the fused kernels walk (SURVEY.md 8(a) G3 "optional internal work-list ordering";
+ * the index-lookup amortisation of PAPER.md:186) and reports its shape:
+ *   out[0] patches (= nc/4)   out[1] tiles (16 patches = 64 cells each)
+ *   out[2] halo-cell tasks    out[3] corner-vertex tasks (summed over tiles)
+ *   out[4] largest halo count of a tile   out[5] largest vertex count of a tile
+ *   out[6] midpoint vertices stored by patches   out[7] corner vertices stored by tiles
+ * (out[6] + out[7] == nv: every vertex is written exactly once by the div/vort kernel).
+ * ICON_EUNSUPPORTED if the tables do not describe a 4-child bisection hierarchy.
+ */
+int icon_grid_worklist_stats(icon_grid_t* g, int64_t out[8]);
 
 /*
  * dycore_div_vort -- SURVEY.md 8(a) steps S1, S2 (north_star: "cell divergence from normal winds

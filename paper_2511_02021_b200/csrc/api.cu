@@ -6,6 +6,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <type_traits>
 #include <vector>
 
 #include "../../include/icon_dycore.h"
@@ -122,6 +123,58 @@ int ensure_coeffs(icon_grid* g, icon::DevCoeffs<T>& c) {
     return ICON_OK;
 }
 
+template <class D, class S>
+int upload_vec(icon_grid* g, const std::vector<S>& src, D** out) {
+    std::vector<D> conv;
+    const D* data;
+    if constexpr (std::is_same<D, S>::value) {
+        data = src.data();
+    } else {
+        conv.assign(src.begin(), src.end());
+        data = conv.data();
+    }
+    int rc = dev_alloc(g, src.size() ? src.size() : 1, out);
+    if (rc != ICON_OK) return rc;
+    if (!src.empty()) CU_TRY(cudaMemcpy(*out, data, src.size() * sizeof(D), cudaMemcpyHostToDevice));
+    return ICON_OK;
+}
+
+int ensure_patch_host(icon_grid* g) {
+    if (g->patch_host_ready) return ICON_OK;
+    std::string err;
+    try {
+        err = icon::build_patch_tables(g->host, g->patch_host);
+    } catch (const std::bad_alloc&) {
+        return fail(ICON_ENOMEM, "out of host memory while building the patch tables");
+    }
+    if (!err.empty()) return fail(ICON_EUNSUPPORTED, err);
+    g->patch_host_ready = true;
+    return ICON_OK;
+}
+
+// tile / patch work-list of the fused kernels: built on the host once, uploaded once per dtype
+template <class T>
+int ensure_patch_tables(icon_grid* g, icon::DevPatchTables<T>& p) {
+    if (p.ready) return ICON_OK;
+    int rc0 = ensure_patch_host(g);
+    if (rc0) return rc0;
+    const icon::PatchTables& h = g->patch_host;
+    int rc;
+    if ((rc = upload_vec(g, h.patch_ids, &p.patch_ids))) return rc;
+    if ((rc = upload_vec(g, h.patch_coef, &p.patch_coef))) return rc;
+    if ((rc = upload_vec(g, h.tile_hdr, &p.tile_hdr))) return rc;
+    if ((rc = upload_vec(g, h.halo_ids, &p.halo_ids))) return rc;
+    if ((rc = upload_vec(g, h.halo_coef, &p.halo_coef))) return rc;
+    if ((rc = upload_vec(g, h.vert_ids, &p.vert_ids))) return rc;
+    if ((rc = upload_vec(g, h.vert_coef, &p.vert_coef))) return rc;
+    if ((rc = upload_vec(g, h.vert_store, &p.vert_store))) return rc;
+    if ((rc = upload_vec(g, h.mid_store, &p.mid_store))) return rc;
+    if ((rc = upload_vec(g, h.mid_vertex, &p.mid_vertex))) return rc;
+    p.n_patches = h.n_patches; p.n_tiles = h.n_tiles; p.max_halo = h.max_halo; p.max_vert = h.max_vert;
+    p.ready = true;
+    return ICON_OK;
+}
+
 // Reading P-14 folded into three per-level coefficients:
 //   (vn_ie(k) - vn_ie(k+1)) / dz_k = A_k vn(k-1) + B_k vn(k) + C_k vn(k+1)
 // half level kh is a two-point linear combination of full levels: interior kh uses (kh, kh-1)
@@ -226,7 +279,7 @@ int ensure_workspace(icon_grid* g, int dtype, int64_t ldk) {
 }
 
 template <class T>
-int tendencies_impl(icon_grid* g, icon::DevCoeffs<T>& c, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
+int tendencies_impl(icon_grid* g, icon::DevCoeffs<T>& c, icon::DevPatchTables<T>& pt, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
                     const void* vn, const void* w, void* ddt_vn, void* vt_opt, void* ke_c_opt, void* vort_opt,
                     cudaStream_t s) {
     int rc;
@@ -243,9 +296,13 @@ int tendencies_impl(icon_grid* g, icon::DevCoeffs<T>& c, int dtype, int nlev, in
         T* vo = vort_opt ? (T*)vort_opt : (T*)g->ws.vort;
         n = icon::launch_tendencies_unfused<T>(*g, c, nlev, ldk, ldk_w, (const T*)abc, (const T*)vn, (const T*)w,
                                                (T*)ddt_vn, vt, (T*)g->ws.ke_e, kc, vo, s);
-    } else {
+    } else if (g->options[ICON_OPT_TENDENCY_KERNEL] == 1) {
         n = icon::launch_tendencies_fused<T>(*g, c, nlev, ldk, ldk_w, (const T*)abc, (const T*)vn, (const T*)w,
                                              (T*)ddt_vn, nullptr, nullptr, nullptr, s);
+    } else {
+        if ((rc = ensure_patch_tables(g, pt))) return rc;
+        n = icon::launch_tendencies_patch<T>(*g, pt, nlev, ldk, ldk_w, (const T*)abc, (const T*)vn, (const T*)w,
+                                             (T*)ddt_vn, s);
     }
     if (n < 0) return fail_cuda((cudaError_t)(-n), "kernel launch");
     g->launches += n;
@@ -311,7 +368,7 @@ int icon_grid_create(int bisections_k, uint64_t seed, unsigned flags, icon_grid_
     g->flags = flags;
     g->seed = seed;
     g->host_only = (flags & ICON_HOST_ONLY) != 0;
-    g->options[ICON_OPT_TENDENCY_KERNEL] = 1;
+    g->options[ICON_OPT_TENDENCY_KERNEL] = 2;
     try {
         std::string err = icon::build_host_grid(bisections_k, seed, (flags & ICON_PERMUTE) != 0, g->host);
         if (!err.empty()) {
@@ -414,12 +471,31 @@ int icon_grid_table_device(icon_grid_t* g, int which, int dtype, const void** dp
 int icon_grid_set_option(icon_grid_t* g, int option, int value) {
     if (!g) return fail(ICON_EINVAL, "grid handle is NULL");
     if (option < 0 || option >= ICON_OPT_COUNT) return fail(ICON_EINVAL, "unknown option");
-    if (option == ICON_OPT_TENDENCY_KERNEL && (value < 0 || value > 1)) return fail(ICON_EINVAL, "bad option value");
+    if (option == ICON_OPT_TENDENCY_KERNEL && (value < 0 || value > 2)) return fail(ICON_EINVAL, "bad option value");
     g->options[option] = value;
     return ICON_OK;
 }
 
 int64_t icon_grid_launch_count(const icon_grid_t* g) { return g ? g->launches : 0; }
+
+int icon_grid_worklist_stats(icon_grid_t* g, int64_t out[8]) {
+    if (!g || !out) return fail(ICON_EINVAL, "NULL argument");
+    int rc = ensure_patch_host(g);
+    if (rc) return rc;
+    const icon::PatchTables& h = g->patch_host;
+    out[0] = h.n_patches;
+    out[1] = h.n_tiles;
+    out[2] = (int64_t)(h.halo_ids.size() / icon::kHaloIdWords);
+    out[3] = (int64_t)(h.vert_ids.size() / icon::kVertIdWords);
+    out[4] = h.max_halo;
+    out[5] = h.max_vert;
+    int64_t mids = 0, cors = 0;
+    for (int32_t m : h.mid_store) mids += (m & 1) + ((m >> 1) & 1) + ((m >> 2) & 1);
+    for (int32_t v : h.vert_store) cors += v;
+    out[6] = mids;
+    out[7] = cors;
+    return ICON_OK;
+}
 
 int dycore_div_vort(icon_grid_t* g, int dtype, int nlev, int ldk, const void* vn, void* div, void* vort,
                     void* cuda_stream) {
@@ -455,8 +531,8 @@ int dycore_velocity_tendencies(icon_grid_t* g, int dtype, int nlev, int ldk, int
     if (ddt_vn == vn || ddt_vn == w) return fail(ICON_EINVAL, "outputs must not alias inputs");
     cudaStream_t s = (cudaStream_t)cuda_stream;
     if (dtype == ICON_F64)
-        return tendencies_impl<double>(g, g->c64, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, vt_opt, ke_c_opt, vort_opt, s);
-    return tendencies_impl<float>(g, g->c32, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, vt_opt, ke_c_opt, vort_opt, s);
+        return tendencies_impl<double>(g, g->c64, g->p64, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, vt_opt, ke_c_opt, vort_opt, s);
+    return tendencies_impl<float>(g, g->c32, g->p32, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, vt_opt, ke_c_opt, vort_opt, s);
 }
 
 int dycore_step_host(icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
