@@ -280,11 +280,14 @@ def run_ours(args):
     peak, peak_src = peak_hbm_gbs()
     t_tend_avg = float(t_tend.mean())
     achieved = bytes_tend / t_tend_avg / 1e9
-    traffic = None
-    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    traffic = None          # ncu dram__bytes_read.sum + dram__bytes_write.sum of the committed capture, per launch
+    tp = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(tp):
         try:
-            traffic = json.load(open(tp)).get("config%d" % args.config, {}).get("tendency_dram_bytes_per_launch")
+            for ln in open(tp).read().splitlines()[1:]:
+                f = ln.split(",")
+                if len(f) >= 3 and f[0] == str(args.config) and f[1] == "dycore_velocity_tendencies":
+                    traffic = int(f[2])
         except Exception:
             traffic = None
     roofline = {"bound": "hbm", "kernel": "dycore_velocity_tendencies", "achieved": achieved, "peak": peak, "unit": "GB/s",
