@@ -175,6 +175,27 @@ int ensure_patch_tables(icon_grid* g, icon::DevPatchTables<T>& p) {
     return ICON_OK;
 }
 
+template <class T>
+int ensure_sc_tables(icon_grid* g, icon::DevScTables<T>& p) {
+    if (p.ready) return ICON_OK;
+    if (!g->sc_host_ready) {
+        std::string err;
+        try {
+            err = icon::build_sc_tables(g->host, g->sc_host);
+        } catch (const std::bad_alloc&) {
+            return fail(ICON_ENOMEM, "out of host memory while building the patch records");
+        }
+        if (!err.empty()) return fail(ICON_EUNSUPPORTED, err);
+        g->sc_host_ready = true;
+    }
+    int rc;
+    if ((rc = upload_vec(g, g->sc_host.ids, &p.ids))) return rc;
+    if ((rc = upload_vec(g, g->sc_host.coef, &p.coef))) return rc;
+    p.n_patches = g->sc_host.n_patches;
+    p.ready = true;
+    return ICON_OK;
+}
+
 // Reading P-14 folded into three per-level coefficients:
 //   (vn_ie(k) - vn_ie(k+1)) / dz_k = A_k vn(k-1) + B_k vn(k) + C_k vn(k+1)
 // half level kh is a two-point linear combination of full levels: interior kh uses (kh, kh-1)
@@ -279,7 +300,7 @@ int ensure_workspace(icon_grid* g, int dtype, int64_t ldk) {
 }
 
 template <class T>
-int tendencies_impl(icon_grid* g, icon::DevCoeffs<T>& c, icon::DevPatchTables<T>& pt, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
+int tendencies_impl(icon_grid* g, icon::DevCoeffs<T>& c, icon::DevPatchTables<T>& pt, icon::DevScTables<T>& st, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
                     const void* vn, const void* w, void* ddt_vn, void* vt_opt, void* ke_c_opt, void* vort_opt,
                     cudaStream_t s) {
     int rc;
@@ -299,6 +320,10 @@ int tendencies_impl(icon_grid* g, icon::DevCoeffs<T>& c, icon::DevPatchTables<T>
     } else if (g->options[ICON_OPT_TENDENCY_KERNEL] == 1) {
         n = icon::launch_tendencies_fused<T>(*g, c, nlev, ldk, ldk_w, (const T*)abc, (const T*)vn, (const T*)w,
                                              (T*)ddt_vn, nullptr, nullptr, nullptr, s);
+    } else if (g->options[ICON_OPT_TENDENCY_KERNEL] == 3) {
+        if ((rc = ensure_sc_tables(g, st))) return rc;
+        n = icon::launch_tendencies_sc<T>(*g, st, nlev, ldk, ldk_w, (const T*)abc, (const T*)vn, (const T*)w,
+                                          (T*)ddt_vn, s);
     } else {
         if ((rc = ensure_patch_tables(g, pt))) return rc;
         n = icon::launch_tendencies_patch<T>(*g, pt, nlev, ldk, ldk_w, (const T*)abc, (const T*)vn, (const T*)w,
@@ -368,7 +393,7 @@ int icon_grid_create(int bisections_k, uint64_t seed, unsigned flags, icon_grid_
     g->flags = flags;
     g->seed = seed;
     g->host_only = (flags & ICON_HOST_ONLY) != 0;
-    g->options[ICON_OPT_TENDENCY_KERNEL] = 2;
+    g->options[ICON_OPT_TENDENCY_KERNEL] = 3;
     try {
         std::string err = icon::build_host_grid(bisections_k, seed, (flags & ICON_PERMUTE) != 0, g->host);
         if (!err.empty()) {
@@ -471,7 +496,7 @@ int icon_grid_table_device(icon_grid_t* g, int which, int dtype, const void** dp
 int icon_grid_set_option(icon_grid_t* g, int option, int value) {
     if (!g) return fail(ICON_EINVAL, "grid handle is NULL");
     if (option < 0 || option >= ICON_OPT_COUNT) return fail(ICON_EINVAL, "unknown option");
-    if (option == ICON_OPT_TENDENCY_KERNEL && (value < 0 || value > 2)) return fail(ICON_EINVAL, "bad option value");
+    if (option == ICON_OPT_TENDENCY_KERNEL && (value < 0 || value > 3)) return fail(ICON_EINVAL, "bad option value");
     g->options[option] = value;
     return ICON_OK;
 }
@@ -531,8 +556,8 @@ int dycore_velocity_tendencies(icon_grid_t* g, int dtype, int nlev, int ldk, int
     if (ddt_vn == vn || ddt_vn == w) return fail(ICON_EINVAL, "outputs must not alias inputs");
     cudaStream_t s = (cudaStream_t)cuda_stream;
     if (dtype == ICON_F64)
-        return tendencies_impl<double>(g, g->c64, g->p64, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, vt_opt, ke_c_opt, vort_opt, s);
-    return tendencies_impl<float>(g, g->c32, g->p32, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, vt_opt, ke_c_opt, vort_opt, s);
+        return tendencies_impl<double>(g, g->c64, g->p64, g->s64, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, vt_opt, ke_c_opt, vort_opt, s);
+    return tendencies_impl<float>(g, g->c32, g->p32, g->s32, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, vt_opt, ke_c_opt, vort_opt, s);
 }
 
 int dycore_step_host(icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,

@@ -9,6 +9,7 @@
 
 #include "host_grid.hpp"
 #include "patch_tables.hpp"
+#include "sc_tables.hpp"
 
 namespace icon {
 
@@ -62,6 +63,15 @@ struct DevPatchTables {
     bool ready = false;
 };
 
+// Device copy of the self-contained patch records (sc_tables.hpp), coefficient words in T.
+template <class T>
+struct DevScTables {
+    int32_t* ids = nullptr;
+    T* coef = nullptr;
+    int64_t n_patches = 0;
+    bool ready = false;
+};
+
 // per-level coefficients of the vertical term (reading P-14), device copy for one z_half
 struct LevelCoeffs {
     std::vector<double> z_half;   // host key
@@ -99,6 +109,10 @@ struct icon_grid {
     bool patch_host_ready = false;
     icon::DevPatchTables<double> p64;
     icon::DevPatchTables<float> p32;
+    icon::ScTables sc_host;                            // built on first use of the self-contained kernel
+    bool sc_host_ready = false;
+    icon::DevScTables<double> s64;
+    icon::DevScTables<float> s32;
     std::vector<icon::LevelCoeffs> level_coeffs;
     icon::Workspace ws;
     icon::HostStage stage;

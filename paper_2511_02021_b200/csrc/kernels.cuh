@@ -32,4 +32,10 @@ template <class T>
 int launch_tendencies_patch(const icon_grid& g, const DevPatchTables<T>& p, int nlev, int64_t ldk, int64_t ldk_w,
                             const T* abc, const T* vn, const T* w, T* ddt_vn, cudaStream_t s);
 
+// S2-S7, self-contained patch kernel (kernels_sc.cu): one warp per patch, all level chunks of a
+// column in flight at once, no exchange between warps; reads vn, w and the records, writes ddt_vn.
+template <class T>
+int launch_tendencies_sc(const icon_grid& g, const DevScTables<T>& p, int nlev, int64_t ldk, int64_t ldk_w,
+                         const T* abc, const T* vn, const T* w, T* ddt_vn, cudaStream_t s);
+
 }  // namespace icon

@@ -102,7 +102,7 @@ def check_all(res, ref, nlev, tol, opt=False):
 # ----------------------------------------------------------------------------------------------
 # configs[0]: R2B4 x 90 fp64, element by element, every kernel variant, optional outputs
 # ----------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("variant", [0, 1, 2])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3])
 def test_config1_r2b4_fp64_elementwise(torch_cuda, lib, oracle_grid, variant):
     og = oracle_grid(4)
     g = lib_grid(lib, 4)
@@ -126,7 +126,7 @@ def test_library_geometry_fed_to_oracle(torch_cuda, lib, oracle_mod, oracle_grid
     div, md = oracle_mod.divergence(t["c2e"], t["geofac_div"], vn64, nlev)
     vort, mv = oracle_mod.vorticity(t["v2e"], t["geofac_rot"], vn64, nlev)
     ref.update(div=div, m_div=md, vort_dv=vort, m_vort=mv)
-    for variant in (0, 1, 2):
+    for variant in (0, 1, 2, 3):
         res = run_gpu(torch_cuda, lib, g, vn, w, zh, nlev, variant)
         check_all(res, ref, nlev, TOL["f64"])
 
@@ -136,7 +136,7 @@ def test_library_geometry_fed_to_oracle(torch_cuda, lib, oracle_mod, oracle_grid
 # ----------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("k,nlev,ldk,ldk_w", [(0, 2, 2, 4), (0, 3, 4, 4), (1, 31, 32, 32), (1, 33, 34, 34),
                                                (2, 64, 64, 66), (2, 65, 66, 66), (3, 90, 96, 92), (2, 130, 130, 132)])
-@pytest.mark.parametrize("variant", [0, 1, 2])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3])
 def test_ragged_levels_and_padding(torch_cuda, lib, oracle_grid, k, nlev, ldk, ldk_w, variant):
     og = oracle_grid(k)
     g = lib_grid(lib, k)
@@ -150,7 +150,7 @@ def test_ragged_levels_and_padding(torch_cuda, lib, oracle_grid, k, nlev, ldk, l
 
 
 @pytest.mark.parametrize("flags_extra", [0, 8])
-@pytest.mark.parametrize("variant", [0, 1, 2])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3])
 def test_permuted_grid_fp64(torch_cuda, lib, oracle_grid, flags_extra, variant):
     """seeded renumbering, with the locality work-list (default) and without (ICON_NO_WORKLIST)"""
     og = oracle_grid(3, si.PERMUTE_SEED, 1)
@@ -162,7 +162,7 @@ def test_permuted_grid_fp64(torch_cuda, lib, oracle_grid, flags_extra, variant):
     check_all(res, ref, nlev, TOL["f64"], opt=True)
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3])
 def test_fp32_variant_permuted_r2b4(torch_cuda, lib, oracle_grid, variant):
     """config 4 at a size the oracle finishes in seconds: fp32 fields, permuted ids, tol 1e-5"""
     og = oracle_grid(4, si.PERMUTE_SEED, 1)
