@@ -85,7 +85,13 @@ enum {
 enum {
     ICON_OPT_TENDENCY_KERNEL = 0, /* 0 = unfused 3-kernel pipeline through an HBM workspace;
                                      1 = fused per-edge gather kernel (no workspace);
-                                     2 = fused register-resident patch kernel (default). */
+                                     2 = fused register-resident patch kernel with shared-memory exchange;
+                                     3 = self-contained patch kernel (one warp per patch, columns through L1);
+                                     4 = column-cache kernel (default): whole columns staged in shared memory
+                                         by bulk asynchronous copies on a host-built schedule; level counts
+                                         it cannot hold (nlev > 95) fall back to 3. */
+    ICON_OPT_CC_SHAPE = 1,        /* pipeline shape of kernel 4 (consumer warps / patches per step / ring
+                                     depth): 0 = 7/1/9 (default), 1 = 8/2/5, 2 = 6/2/5, 3 = 7/1/10. */
     ICON_OPT_COUNT
 };
 

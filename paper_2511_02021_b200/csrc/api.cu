@@ -3,6 +3,7 @@
 // no CPU fallback: every compute entry point fails with ICON_ECUDA when no device is usable.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cstring>
 #include <new>
 #include <string>
@@ -175,23 +176,90 @@ int ensure_patch_tables(icon_grid* g, icon::DevPatchTables<T>& p) {
     return ICON_OK;
 }
 
+int ensure_sc_host(icon_grid* g);
+
 template <class T>
 int ensure_sc_tables(icon_grid* g, icon::DevScTables<T>& p) {
     if (p.ready) return ICON_OK;
-    if (!g->sc_host_ready) {
-        std::string err;
-        try {
-            err = icon::build_sc_tables(g->host, g->sc_host);
-        } catch (const std::bad_alloc&) {
-            return fail(ICON_ENOMEM, "out of host memory while building the patch records");
-        }
-        if (!err.empty()) return fail(ICON_EUNSUPPORTED, err);
-        g->sc_host_ready = true;
-    }
-    int rc;
+    int rc = ensure_sc_host(g);
+    if (rc) return rc;
     if ((rc = upload_vec(g, g->sc_host.ids, &p.ids))) return rc;
     if ((rc = upload_vec(g, g->sc_host.coef, &p.coef))) return rc;
     p.n_patches = g->sc_host.n_patches;
+    p.ready = true;
+    return ICON_OK;
+}
+
+int ensure_sc_host(icon_grid* g) {
+    if (g->sc_host_ready) return ICON_OK;
+    std::string err;
+    try {
+        err = icon::build_sc_tables(g->host, g->sc_host);
+    } catch (const std::bad_alloc&) {
+        return fail(ICON_ENOMEM, "out of host memory while building the patch records");
+    }
+    if (!err.empty()) return fail(ICON_EUNSUPPORTED, err);
+    g->sc_host_ready = true;
+    return ICON_OK;
+}
+
+// Column-cache schedule + patch records for (T, nlev): built on the host once, uploaded once.
+// Returns ICON_OK with p.unsupported set when this (T, nlev) cannot use the kernel (the caller
+// then uses the self-contained patch kernel).
+template <class T>
+int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev) {
+    const int shape = g->options[ICON_OPT_CC_SHAPE];
+    if (p.nlev == nlev && p.shape == shape && (p.ready || p.unsupported)) return ICON_OK;
+    dev_release(g, p.steps); dev_release(g, p.loads); dev_release(g, p.records);
+    dev_release(g, p.cta_patch_begin); dev_release(g, p.cta_step_begin);
+    p = icon::DevCcTables<T>();
+    p.nlev = nlev;
+    p.shape = shape;
+    const icon::CcShape& sh = icon::cc_shape(shape);
+    const int n_slots_max = icon::cc_max_slots<T>(shape, nlev, g->smem_optin);
+    const int slot_bytes = icon::cc_slot_bytes<T>(nlev);
+    if (icon::cc_levels_per_lane(nlev) == 0 || nlev * (int)sizeof(T) < 16 || n_slots_max < icon::kScIdWords) {
+        p.unsupported = true;
+        return ICON_OK;
+    }
+    int rc = ensure_sc_host(g);
+    if (rc) return rc;
+    const icon::ScTables& sc = g->sc_host;
+    const int n_slots = std::min(n_slots_max, 65535 / (slot_bytes / 16));
+    icon::CcSchedule cs;
+    std::vector<unsigned char> rec;
+    const size_t rb = (size_t)icon::kScCoefWords * sizeof(T) + icon::kCcRecordTail;
+    try {
+        std::string err = icon::build_cc_schedule(sc, g->num_sms, n_slots, slot_bytes / 16, sh.group, sh.depth, cs);
+        if (!err.empty()) {
+            p.unsupported = true;
+            return ICON_OK;
+        }
+        rec.assign((size_t)sc.n_patches * rb, 0);
+#pragma omp parallel for schedule(static)
+        for (int64_t q = 0; q < sc.n_patches; ++q) {
+            unsigned char* r = rec.data() + (size_t)q * rb;
+            T* cf = reinterpret_cast<T*>(r);
+            for (int i = 0; i < icon::kScCoefWords; ++i) cf[i] = (T)sc.coef[(size_t)q * icon::kScCoefWords + i];
+            int32_t* oid = reinterpret_cast<int32_t*>(r + (size_t)icon::kScCoefWords * sizeof(T));
+            const int32_t* id = &sc.ids[(size_t)q * icon::kScIdWords];
+            for (int x = 0; x < 3; ++x) {
+                oid[x] = id[icon::SID_I0 + x];
+                oid[3 + x] = id[icon::SID_B0 + 2 * x];
+            }
+            std::memcpy(r + (size_t)icon::kScCoefWords * sizeof(T) + 32, &cs.patch_slots[(size_t)q * icon::kCcSlotWords],
+                        icon::kCcSlotWords * 2);
+        }
+    } catch (const std::bad_alloc&) {
+        return fail(ICON_ENOMEM, "out of host memory while building the column-cache schedule");
+    }
+    if ((rc = upload_vec(g, cs.steps, &p.steps))) return rc;
+    if ((rc = upload_vec(g, cs.loads, &p.loads))) return rc;
+    if ((rc = upload_vec(g, rec, &p.records))) return rc;
+    if ((rc = upload_vec(g, cs.cta_patch_begin, &p.cta_patch_begin))) return rc;
+    if ((rc = upload_vec(g, cs.cta_step_begin, &p.cta_step_begin))) return rc;
+    p.n_ctas = cs.n_ctas; p.n_slots = cs.n_slots; p.slot_bytes = slot_bytes;
+    p.stats[0] = (int64_t)cs.steps.size(); p.stats[1] = cs.n_sync_steps; p.stats[2] = cs.n_vn_loads; p.stats[3] = cs.n_w_loads;
     p.ready = true;
     return ICON_OK;
 }
@@ -300,7 +368,8 @@ int ensure_workspace(icon_grid* g, int dtype, int64_t ldk) {
 }
 
 template <class T>
-int tendencies_impl(icon_grid* g, icon::DevCoeffs<T>& c, icon::DevPatchTables<T>& pt, icon::DevScTables<T>& st, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
+int tendencies_impl(icon_grid* g, icon::DevCoeffs<T>& c, icon::DevPatchTables<T>& pt, icon::DevScTables<T>& st,
+                    icon::DevCcTables<T>& ct, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
                     const void* vn, const void* w, void* ddt_vn, void* vt_opt, void* ke_c_opt, void* vort_opt,
                     cudaStream_t s) {
     int rc;
@@ -309,7 +378,14 @@ int tendencies_impl(icon_grid* g, icon::DevCoeffs<T>& c, icon::DevPatchTables<T>
     if ((rc = get_level_coeffs(g, dtype, nlev, z_half, s, &abc))) return rc;
     const bool want_opt = vt_opt || ke_c_opt || vort_opt;
     int n;
-    if (g->options[ICON_OPT_TENDENCY_KERNEL] == 0 || want_opt) {
+    int variant = g->options[ICON_OPT_TENDENCY_KERNEL];
+    if (variant == 4 && !want_opt) {
+        if ((rc = ensure_cc_tables(g, ct, nlev))) return rc;
+        if (ct.unsupported) variant = 3;      // level count / dtype the column cache cannot hold
+    }
+    if (variant == 4 && !want_opt) {
+        n = icon::launch_tendencies_cc<T>(*g, ct, nlev, ldk, ldk_w, (const T*)abc, (const T*)vn, (const T*)w, (T*)ddt_vn, s);
+    } else if (variant == 0 || want_opt) {
         // optional outputs are produced by the unfused pipeline, which materialises them anyway
         if ((rc = ensure_workspace<T>(g, dtype, ldk))) return rc;
         T* vt = vt_opt ? (T*)vt_opt : (T*)g->ws.vt;
@@ -317,10 +393,10 @@ int tendencies_impl(icon_grid* g, icon::DevCoeffs<T>& c, icon::DevPatchTables<T>
         T* vo = vort_opt ? (T*)vort_opt : (T*)g->ws.vort;
         n = icon::launch_tendencies_unfused<T>(*g, c, nlev, ldk, ldk_w, (const T*)abc, (const T*)vn, (const T*)w,
                                                (T*)ddt_vn, vt, (T*)g->ws.ke_e, kc, vo, s);
-    } else if (g->options[ICON_OPT_TENDENCY_KERNEL] == 1) {
+    } else if (variant == 1) {
         n = icon::launch_tendencies_fused<T>(*g, c, nlev, ldk, ldk_w, (const T*)abc, (const T*)vn, (const T*)w,
                                              (T*)ddt_vn, nullptr, nullptr, nullptr, s);
-    } else if (g->options[ICON_OPT_TENDENCY_KERNEL] == 3) {
+    } else if (variant == 3) {
         if ((rc = ensure_sc_tables(g, st))) return rc;
         n = icon::launch_tendencies_sc<T>(*g, st, nlev, ldk, ldk_w, (const T*)abc, (const T*)vn, (const T*)w,
                                           (T*)ddt_vn, s);
@@ -393,7 +469,7 @@ int icon_grid_create(int bisections_k, uint64_t seed, unsigned flags, icon_grid_
     g->flags = flags;
     g->seed = seed;
     g->host_only = (flags & ICON_HOST_ONLY) != 0;
-    g->options[ICON_OPT_TENDENCY_KERNEL] = 3;
+    g->options[ICON_OPT_TENDENCY_KERNEL] = 4;
     try {
         std::string err = icon::build_host_grid(bisections_k, seed, (flags & ICON_PERMUTE) != 0, g->host);
         if (!err.empty()) {
@@ -416,6 +492,7 @@ int icon_grid_create(int bisections_k, uint64_t seed, unsigned flags, icon_grid_
         int rc = ICON_OK;
         e = cudaGetDevice(&g->device);
         if (e == cudaSuccess) e = cudaDeviceGetAttribute(&g->num_sms, cudaDevAttrMultiProcessorCount, g->device);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&g->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, g->device);
         if (e != cudaSuccess) rc = fail_cuda(e, "cudaGetDevice");
         if (rc == ICON_OK) rc = upload_index_tables(g);
         if (rc == ICON_OK) rc = ensure_coeffs(g, g->c64);
@@ -496,7 +573,8 @@ int icon_grid_table_device(icon_grid_t* g, int which, int dtype, const void** dp
 int icon_grid_set_option(icon_grid_t* g, int option, int value) {
     if (!g) return fail(ICON_EINVAL, "grid handle is NULL");
     if (option < 0 || option >= ICON_OPT_COUNT) return fail(ICON_EINVAL, "unknown option");
-    if (option == ICON_OPT_TENDENCY_KERNEL && (value < 0 || value > 3)) return fail(ICON_EINVAL, "bad option value");
+    if (option == ICON_OPT_CC_SHAPE && (value < 0 || value >= icon::kCcNumShapes)) return fail(ICON_EINVAL, "bad option value");
+    if (option == ICON_OPT_TENDENCY_KERNEL && (value < 0 || value > 4)) return fail(ICON_EINVAL, "bad option value");
     g->options[option] = value;
     return ICON_OK;
 }
@@ -556,8 +634,8 @@ int dycore_velocity_tendencies(icon_grid_t* g, int dtype, int nlev, int ldk, int
     if (ddt_vn == vn || ddt_vn == w) return fail(ICON_EINVAL, "outputs must not alias inputs");
     cudaStream_t s = (cudaStream_t)cuda_stream;
     if (dtype == ICON_F64)
-        return tendencies_impl<double>(g, g->c64, g->p64, g->s64, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, vt_opt, ke_c_opt, vort_opt, s);
-    return tendencies_impl<float>(g, g->c32, g->p32, g->s32, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, vt_opt, ke_c_opt, vort_opt, s);
+        return tendencies_impl<double>(g, g->c64, g->p64, g->s64, g->cc64, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, vt_opt, ke_c_opt, vort_opt, s);
+    return tendencies_impl<float>(g, g->c32, g->p32, g->s32, g->cc32, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, vt_opt, ke_c_opt, vort_opt, s);
 }
 
 int dycore_step_host(icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,

@@ -1,0 +1,192 @@
+// cc_schedule.cpp -- builds the column-cache schedule (cc_schedule.hpp) by simulating, per CTA,
+// the reference stream of its patches against a pool of n_slots shared-memory slots.
+#include "cc_schedule.hpp"
+
+#include <algorithm>
+#include <atomic>
+#include <unordered_map>
+
+namespace icon {
+namespace {
+
+constexpr int kRefs = SID_PAD;            // 43 columns per patch: 36 vn, then 7 w
+constexpr int kFirstCell = SID_T0;        // id slots >= this are cell (w) columns
+constexpr int32_t kNever = 0x7fffffff;
+
+struct CtaResult {
+    std::vector<CcStep> steps;
+    std::vector<CcLoad> loads;
+    int64_t n_sync = 0, n_vn = 0, n_w = 0;
+    bool ok = true;
+};
+
+inline uint64_t key_of(int slot_in_patch, int32_t id) {
+    return ((uint64_t)(uint32_t)id << 1) | (slot_in_patch >= kFirstCell ? 1u : 0u);
+}
+
+void simulate_cta(const ScTables& sc, int64_t pb, int64_t pe, int n_slots, int slot_units, int kCcGroup, int max_depth,
+                  uint16_t* patch_slots, CtaResult& r) {
+    const int64_t n_steps = (pe - pb + kCcGroup - 1) / kCcGroup;
+    // pass 1: the distinct columns of every step
+    std::vector<std::vector<uint64_t>> keys((size_t)n_steps);
+    for (int64_t s = 0; s < n_steps; ++s) {
+        auto& ks = keys[(size_t)s];
+        const int64_t p0 = pb + s * kCcGroup, p1 = std::min(pe, p0 + kCcGroup);
+        for (int64_t p = p0; p < p1; ++p)
+            for (int i = 0; i < kRefs; ++i) ks.push_back(key_of(i, sc.ids[(size_t)p * kScIdWords + i]));
+        std::sort(ks.begin(), ks.end());
+        ks.erase(std::unique(ks.begin(), ks.end()), ks.end());
+    }
+    // pass 2 (backward): the next step that uses each of them
+    std::vector<std::vector<int32_t>> next_use((size_t)n_steps);
+    {
+        std::unordered_map<uint64_t, int32_t> seen;
+        seen.reserve(4096);
+        for (int64_t s = n_steps - 1; s >= 0; --s) {
+            const auto& ks = keys[(size_t)s];
+            auto& nu = next_use[(size_t)s];
+            nu.resize(ks.size());
+            for (size_t i = 0; i < ks.size(); ++i) {
+                auto it = seen.find(ks[i]);
+                nu[i] = it == seen.end() ? kNever : it->second;
+                seen[ks[i]] = (int32_t)s;
+            }
+        }
+    }
+    // pass 3 (forward): residency
+    std::unordered_map<uint64_t, int32_t> resident;      // key -> slot
+    resident.reserve((size_t)n_slots * 2);
+    std::vector<uint64_t> slot_key((size_t)n_slots, ~0ull);
+    std::vector<int32_t> slot_last((size_t)n_slots, -1000), slot_next((size_t)n_slots, kNever);
+    std::vector<int32_t> cand;
+    std::vector<size_t> miss;
+    std::unordered_map<uint64_t, int32_t> step_slot;     // key -> slot, for this step's patches
+    r.steps.reserve((size_t)n_steps);
+    for (int64_t s = 0; s < n_steps; ++s) {
+        const auto& ks = keys[(size_t)s];
+        const auto& nu = next_use[(size_t)s];
+        step_slot.clear();
+        miss.clear();
+        for (size_t i = 0; i < ks.size(); ++i) {
+            auto it = resident.find(ks[i]);
+            if (it == resident.end()) {
+                miss.push_back(i);
+            } else {
+                slot_last[(size_t)it->second] = (int32_t)s;
+                slot_next[(size_t)it->second] = nu[i];
+                step_slot[ks[i]] = it->second;
+            }
+        }
+        int depth = max_depth;
+        for (; depth >= 1; --depth) {
+            cand.clear();
+            for (int32_t q = 0; q < n_slots; ++q)
+                if (slot_last[(size_t)q] <= (int32_t)s - depth) cand.push_back(q);
+            if (cand.size() >= miss.size()) break;
+        }
+        const int sync = depth < max_depth;
+        if (cand.size() < miss.size()) {
+            r.ok = false;
+            return;
+        }
+        // Belady: give up the columns whose next use is farthest (empty slots first)
+        std::partial_sort(cand.begin(), cand.begin() + (ptrdiff_t)miss.size(), cand.end(), [&](int32_t a, int32_t b) {
+            const int32_t na = slot_key[(size_t)a] == ~0ull ? kNever : slot_next[(size_t)a];
+            const int32_t nb = slot_key[(size_t)b] == ~0ull ? kNever : slot_next[(size_t)b];
+            if (na != nb) return na > nb;
+            const bool ea = slot_key[(size_t)a] == ~0ull, eb = slot_key[(size_t)b] == ~0ull;
+            if (ea != eb) return ea;
+            return a < b;
+        });
+        CcStep st;
+        st.load_begin = (uint32_t)r.loads.size();
+        st.n_vn = st.n_w = 0;
+        st.n_patches = (uint16_t)(std::min(pe, pb + (s + 1) * kCcGroup) - (pb + s * kCcGroup));
+        st.depth = (uint16_t)depth;
+        st.pad = 0;
+        for (int kind = 0; kind < 2; ++kind)
+            for (size_t m = 0; m < miss.size(); ++m) {
+                const uint64_t k = ks[miss[m]];
+                if ((int)(k & 1) != kind) continue;
+                const int32_t q = cand[m];
+                if (slot_key[(size_t)q] != ~0ull) resident.erase(slot_key[(size_t)q]);
+                slot_key[(size_t)q] = k;
+                slot_last[(size_t)q] = (int32_t)s;
+                slot_next[(size_t)q] = nu[miss[m]];
+                resident[k] = q;
+                step_slot[k] = q;
+                CcLoad ld;
+                ld.id = (uint32_t)(k >> 1);
+                ld.slot = (uint16_t)q;
+                ld.kind = (uint16_t)kind;
+                r.loads.push_back(ld);
+                if (kind) ++st.n_w; else ++st.n_vn;
+            }
+        r.n_sync += sync;
+        r.n_vn += st.n_vn;
+        r.n_w += st.n_w;
+        r.steps.push_back(st);
+        const int64_t p0 = pb + s * kCcGroup, p1 = std::min(pe, p0 + kCcGroup);
+        for (int64_t p = p0; p < p1; ++p) {
+            uint16_t* o = patch_slots + (size_t)p * kCcSlotWords;
+            for (int i = 0; i < kRefs; ++i)
+                o[i] = (uint16_t)(step_slot[key_of(i, sc.ids[(size_t)p * kScIdWords + i])] * slot_units);
+            for (int i = kRefs; i < kCcSlotWords; ++i) o[i] = 0;
+        }
+    }
+}
+
+}  // namespace
+
+std::string build_cc_schedule(const ScTables& sc, int n_ctas, int n_slots, int slot_units, int group, int depth,
+                              CcSchedule& out) {
+    const int kCcGroup = group;
+    const int64_t np = sc.n_patches;
+    if (np <= 0 || n_ctas <= 0) return "cc schedule: empty grid";
+    if (n_slots < kRefs) return "cc schedule: fewer shared-memory slots than one patch needs";
+    if ((int64_t)n_slots * slot_units > 65535) return "cc schedule: slot offsets do not fit 16 bits";
+    const int64_t max_ctas = (np + kCcGroup - 1) / kCcGroup;
+    if (n_ctas > max_ctas) n_ctas = (int)max_ctas;
+    out = CcSchedule();
+    out.n_ctas = n_ctas;
+    out.n_slots = n_slots;
+    out.slot_units = slot_units;
+    out.group = group;
+    out.depth = depth;
+    out.cta_patch_begin.resize((size_t)n_ctas + 1);
+    // whole steps per CTA, spread evenly
+    const int64_t total_steps = max_ctas;
+    for (int b = 0; b <= n_ctas; ++b)
+        out.cta_patch_begin[(size_t)b] = std::min(np, (total_steps * b / n_ctas) * kCcGroup);
+    out.patch_slots.assign((size_t)np * kCcSlotWords, 0);
+    std::vector<CtaResult> res((size_t)n_ctas);
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int b = 0; b < n_ctas; ++b)
+        simulate_cta(sc, out.cta_patch_begin[(size_t)b], out.cta_patch_begin[(size_t)b + 1], n_slots, slot_units,
+                     group, depth, out.patch_slots.data(), res[(size_t)b]);
+    out.cta_step_begin.assign((size_t)n_ctas + 1, 0);
+    size_t n_loads = 0;
+    for (int b = 0; b < n_ctas; ++b) {
+        if (!res[(size_t)b].ok) return "cc schedule: one step needs more columns than there are shared-memory slots";
+        out.cta_step_begin[(size_t)b + 1] = out.cta_step_begin[(size_t)b] + (int64_t)res[(size_t)b].steps.size();
+        n_loads += res[(size_t)b].loads.size();
+    }
+    if (n_loads > 0xffffffffull) return "cc schedule: load list too long";
+    out.steps.reserve((size_t)out.cta_step_begin[(size_t)n_ctas]);
+    out.loads.reserve(n_loads);
+    for (int b = 0; b < n_ctas; ++b) {
+        const uint32_t base = (uint32_t)out.loads.size();
+        for (CcStep st : res[(size_t)b].steps) {
+            st.load_begin += base;
+            out.steps.push_back(st);
+        }
+        out.loads.insert(out.loads.end(), res[(size_t)b].loads.begin(), res[(size_t)b].loads.end());
+        out.n_sync_steps += res[(size_t)b].n_sync;
+        out.n_vn_loads += res[(size_t)b].n_vn;
+        out.n_w_loads += res[(size_t)b].n_w;
+        res[(size_t)b] = CtaResult();
+    }
+    return std::string();
+}
+
+}  // namespace icon

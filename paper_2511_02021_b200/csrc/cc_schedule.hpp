@@ -1,0 +1,74 @@
+// cc_schedule.hpp -- host-built schedule of the COLUMN-CACHE tendency kernel (kernels_cc.cu;
+// internal header).
+//
+// The kernel keeps whole vn / w columns in shared memory ("slots") and fills them with bulk
+// asynchronous copies (cp.async.bulk, the 1-D TMA path) issued by a producer warp; eight consumer
+// warps each finish one self-contained patch (sc_tables.hpp) per STEP from those slots. Which
+// column sits in which slot at which step is decided HERE, on the host, once per grid: the work
+// order of every CTA is fixed (a contiguous range of the generation order), so the whole future
+// of the reference stream is known and the replacement is Belady's (evict the column whose next
+// use is farthest). The device never searches or hashes anything: a step is a list of
+// (column id, slot) loads plus, per patch, the slot of each of its 43 columns.
+//
+// Pipeline rule the schedule guarantees (kernels_cc.cu relies on it): the loads of step s only
+// overwrite slots whose last reader ran in a step <= s-2, so they can be in flight while step
+// s-1 computes; a step flagged `sync` may also overwrite slots last read in step s-1 and the
+// producer waits for that step to drain first (rare: only when two consecutive steps together
+// need more columns than there are slots).
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "sc_tables.hpp"
+
+namespace icon {
+
+// pipeline shapes of the kernel (kernels_cc.cu): consumer warps, patches per step, ring depth.
+// One producer warp is added to `warps`; with 8 warps per CTA a thread may use 255 registers,
+// with 9 only 168 (the register file is split over the four SM sub-partitions).
+struct CcShape {
+    int warps, group, depth;
+};
+constexpr int kCcNumShapes = 4;
+constexpr CcShape kCcShapes[kCcNumShapes] = {{7, 1, 9}, {8, 2, 5}, {6, 2, 5}, {7, 1, 10}};
+inline const CcShape& cc_shape(int i) { return kCcShapes[i >= 0 && i < kCcNumShapes ? i : 0]; }
+constexpr int kCcBarrierBytes = 256;
+// a patch record on the device = kScCoefWords coefficients (T), then 8 int32 (user ids of the six
+// owned edges i0 i1 i2 b0 b2 b4, 2 pad), then kCcSlotWords uint16 slot offsets
+constexpr int kCcRecordTail = 32 + 96;
+constexpr int kCcSlotWords = 48;     // uint16 per patch: 43 slot offsets (order of sc_tables.hpp id slots) + pad
+
+struct CcStep {                      // 16 bytes
+    uint32_t load_begin;             // first entry of this step in `loads`
+    uint16_t n_vn, n_w;              // vn columns first, then w columns
+    uint16_t n_patches;              // 1..group
+    uint16_t depth;                  // the loads may be issued once step s-depth has drained (1..schedule depth)
+    uint32_t pad;
+};
+
+struct CcLoad {                      // 8 bytes
+    uint32_t id;                     // user id of the edge (vn) or cell (w) column
+    uint16_t slot;                   // slot index
+    uint16_t kind;                   // 0 = vn, 1 = w
+};
+
+struct CcSchedule {
+    int n_ctas = 0, n_slots = 0;
+    int group = 0;                           // patches per step
+    int depth = 0;                           // steps a load may run ahead of its readers (pipeline depth)
+    int slot_units = 0;                      // slot size in 16-byte units (slot offsets are stored in these units)
+    std::vector<int64_t> cta_patch_begin;    // [n_ctas + 1]
+    std::vector<int64_t> cta_step_begin;     // [n_ctas + 1]
+    std::vector<CcStep> steps;
+    std::vector<CcLoad> loads;
+    std::vector<uint16_t> patch_slots;       // [n_patches][kCcSlotWords], slot * slot_units
+    // statistics (icon_grid_worklist_stats, tests)
+    int64_t n_sync_steps = 0, n_vn_loads = 0, n_w_loads = 0;
+};
+
+// Returns an empty string on success, else an error message (e.g. too few slots for one step).
+std::string build_cc_schedule(const ScTables& sc, int n_ctas, int n_slots, int slot_units, int group, int depth,
+                              CcSchedule& out);
+
+}  // namespace icon

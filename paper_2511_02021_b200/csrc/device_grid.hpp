@@ -10,6 +10,7 @@
 #include "host_grid.hpp"
 #include "patch_tables.hpp"
 #include "sc_tables.hpp"
+#include "cc_schedule.hpp"
 
 namespace icon {
 
@@ -72,6 +73,23 @@ struct DevScTables {
     bool ready = false;
 };
 
+// Device copy of the column-cache schedule (cc_schedule.hpp) for one (T, nlev): records are the
+// patch records of kernels_cc.cu (coefficients in T + owned edge ids + slot offsets).
+template <class T>
+struct DevCcTables {
+    CcStep* steps = nullptr;
+    CcLoad* loads = nullptr;
+    unsigned char* records = nullptr;
+    int64_t* cta_patch_begin = nullptr;
+    int64_t* cta_step_begin = nullptr;
+    int n_ctas = 0, n_slots = 0, slot_bytes = 0;
+    int nlev = -1;                 // the level count the slot size was derived from
+    int shape = -1;                // index into kCcShapes the schedule was built for
+    bool ready = false;
+    bool unsupported = false;      // this (T, nlev) cannot use the kernel: callers fall back
+    int64_t stats[4] = {0, 0, 0, 0};   // steps, steps that wait for their predecessor, vn loads, w loads
+};
+
 // per-level coefficients of the vertical term (reading P-14), device copy for one z_half
 struct LevelCoeffs {
     std::vector<double> z_half;   // host key
@@ -113,6 +131,9 @@ struct icon_grid {
     bool sc_host_ready = false;
     icon::DevScTables<double> s64;
     icon::DevScTables<float> s32;
+    icon::DevCcTables<double> cc64;                    // built on first use of the column-cache kernel
+    icon::DevCcTables<float> cc32;
+    int smem_optin = 0;                                // cudaDevAttrMaxSharedMemoryPerBlockOptin
     std::vector<icon::LevelCoeffs> level_coeffs;
     icon::Workspace ws;
     icon::HostStage stage;

@@ -1,0 +1,531 @@
+// kernels_cc.cu -- column-cache kernel for the velocity tendency, sm_100a.
+//
+// Same arithmetic per patch as kernels_sc.cu (one warp finishes one self-contained patch, lanes =
+// levels, no exchange between warps), but the vn / w columns no longer come through the L1: a
+// PRODUCER warp moves whole columns from HBM into shared-memory slots with bulk asynchronous copies
+// (cp.async.bulk = the 1-D TMA path, completion on an mbarrier), following a schedule the host
+// computed once per grid (cc_schedule.hpp: which column into which slot at which step, Belady
+// replacement). CONSUMER warps read the slots:
+//
+//   * every column crosses L2 -> SM once per residency instead of once per patch that touches it
+//     (~14 instead of 43 column fetches per patch), and the fetches are in flight for one or more
+//     whole steps ahead of their readers without holding a single register;
+//   * a lane owns L CONSECUTIVE levels (k = L*lane .. L*lane+L-1; L odd, so the 8-byte stride-L
+//     shared-memory reads are bank-conflict free), so the vertical stencil (S6) needs one shuffle
+//     up and one down per column instead of one pair per 32-level chunk, and a coefficient / slot
+//     lookup, which is warp-uniform, is paid once per L*32 levels;
+//   * ddt_vn columns are assembled in shared memory and leave with a bulk store, so the strided
+//     register layout never turns into uncoalesced global stores.
+//
+// Synchronisation: ring of D stages, full[s % D] (producer arms it with the byte count of step s,
+// the copies complete it) and done[s % D] (one arrival per consumer warp of the step's group). The
+// schedule guarantees that the loads of step s only overwrite slots last read in a step <= s-depth
+// (depth stored per step), and the producer issues them once those steps have drained.
+#include <cuda_pipeline.h>
+
+#include "kernels.cuh"
+#include "cc_schedule.hpp"
+
+namespace icon {
+namespace {
+
+constexpr unsigned kFull = 0xffffffffu;
+
+// ---- PTX wrappers (mbarrier + bulk copies) ------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+// global -> shared, completion counted in bytes on `bar`
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+// shared -> global, tracked by the issuing thread's bulk async-group
+__device__ __forceinline__ void bulk_s2g(void* dst, uint32_t src, uint32_t bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void bulk_wait_read() {
+    asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory");
+}
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+// generic-proxy writes to shared memory -> visible to the async proxy (bulk store source)
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// ---- device view of the schedule ------------------------------------------------------------------
+template <class T>
+struct CcDev {
+    const CcStep* steps;
+    const CcLoad* loads;
+    const unsigned char* records;     // [n_patches][record_bytes<T>()]
+    const int64_t* cta_patch_begin;   // [n_ctas + 1]
+    const int64_t* cta_step_begin;    // [n_ctas + 1]
+    int n_slots;
+    int slot_bytes;
+};
+
+// ---- L consecutive levels of one column, per lane ---------------------------------------------------
+template <class T, int L>
+struct Col {
+    T v[L];
+};
+#define FORL _Pragma("unroll") for (int l = 0; l < L; ++l)
+
+// value one level up (k-1) / down (k+1): inside the lane except at its ends
+template <class T, int L>
+__device__ __forceinline__ Col<T, L> level_up(const Col<T, L>& a) {
+    Col<T, L> r;
+    r.v[0] = __shfl_up_sync(kFull, a.v[L - 1], 1);
+#pragma unroll
+    for (int l = 1; l < L; ++l) r.v[l] = a.v[l - 1];
+    return r;
+}
+template <class T, int L>
+__device__ __forceinline__ Col<T, L> level_down(const Col<T, L>& a) {
+    Col<T, L> r;
+#pragma unroll
+    for (int l = 0; l < L - 1; ++l) r.v[l] = a.v[l + 1];
+    r.v[L - 1] = __shfl_down_sync(kFull, a.v[0], 1);
+    return r;
+}
+template <class T, int L>
+__device__ __forceinline__ Col<T, L> dot4(const T* r, const Col<T, L>& a, const Col<T, L>& b, const Col<T, L>& c,
+                                          const Col<T, L>& d) {
+    Col<T, L> o;
+    FORL o.v[l] = r[0] * a.v[l] + r[1] * b.v[l] + r[2] * c.v[l] + r[3] * d.v[l];
+    return o;
+}
+template <class T, int L>
+__device__ __forceinline__ Col<T, L> ke2(const Col<T, L>& n, const Col<T, L>& t) {   // n^2 + t^2 = 2 KE_e (S4)
+    Col<T, L> o;
+    FORL o.v[l] = n.v[l] * n.v[l] + t.v[l] * t.v[l];
+    return o;
+}
+template <class T, int L>
+__device__ __forceinline__ void axpy(Col<T, L>& acc, T a, const Col<T, L>& x) {
+    FORL acc.v[l] += a * x.v[l];
+}
+template <class T, int L>
+__device__ __forceinline__ Col<T, L> scale(T a, const Col<T, L>& x) {
+    Col<T, L> o;
+    FORL o.v[l] = a * x.v[l];
+    return o;
+}
+
+// N warp-uniform coefficients from shared memory (16-byte broadcasts)
+template <int N, class T>
+__device__ __forceinline__ void ld_coef(const T* __restrict__ p, T (&out)[N]) {
+    constexpr int per = 16 / sizeof(T);
+    static_assert(N % per == 0, "coefficient group must be a multiple of 16 bytes");
+    const int4* q = reinterpret_cast<const int4*>(p);
+#pragma unroll
+    for (int i = 0; i < N / per; ++i) {
+        int4 v = q[i];
+        T tmp[per];
+        *reinterpret_cast<int4*>(tmp) = v;
+#pragma unroll
+        for (int j = 0; j < per; ++j) out[i * per + j] = tmp[j];
+    }
+}
+// N slot offsets (uint16, units of 16 bytes) -> byte offsets
+template <int N>
+__device__ __forceinline__ void ld_slots(const uint16_t* __restrict__ p, uint32_t (&out)[N]) {
+    static_assert(N % 8 == 0, "slot group must be a multiple of 16 bytes");
+    const int4* q = reinterpret_cast<const int4*>(p);
+#pragma unroll
+    for (int i = 0; i < N / 8; ++i) {
+        int4 v = q[i];
+        const uint32_t w[4] = {(uint32_t)v.x, (uint32_t)v.y, (uint32_t)v.z, (uint32_t)v.w};
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            out[8 * i + 2 * j] = (w[j] & 0xffffu) << 4;
+            out[8 * i + 2 * j + 1] = (w[j] >> 16) << 4;
+        }
+    }
+}
+
+template <class T>
+__host__ __device__ constexpr int cc_record_bytes() { return kScCoefWords * (int)sizeof(T) + kCcRecordTail; }
+
+// W consumer warps in W/G groups of G; group g runs the steps s = g (mod W/G). D = ring depth.
+template <class T, int L, int W, int G, int D>
+__global__ void __launch_bounds__((W + 1) * 32, 1)
+k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, const T* __restrict__ vn,
+          const T* __restrict__ w, T* __restrict__ ddt_vn) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    using C = Col<T, L>;
+    constexpr int REC = cc_record_bytes<T>();
+    constexpr int NGRP = W / G;
+    static_assert(W % G == 0 && D > NGRP && D <= 16, "bad pipeline shape");
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int out_bytes = (nlev * (int)sizeof(T) + 15) & ~15;                 // staging column, 16-byte multiple
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem);                       // full[D], done[D]
+    unsigned char* rec_base = smem + kCcBarrierBytes;
+    unsigned char* out_base = rec_base + D * G * REC;
+    unsigned char* slot_base = out_base + W * 2 * out_bytes;
+    const uint32_t bar0 = smem_u32(bars);
+    auto full_bar = [&](int i) { return bar0 + 8u * (uint32_t)i; };
+    auto done_bar = [&](int i) { return bar0 + 8u * (uint32_t)(D + i); };
+
+    const int64_t pb = d.cta_patch_begin[blockIdx.x], pe = d.cta_patch_begin[blockIdx.x + 1];
+    const int64_t sb = d.cta_step_begin[blockIdx.x];
+    const int n_steps = (int)(d.cta_step_begin[blockIdx.x + 1] - sb);
+
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < D; ++i) {
+            mbar_init(full_bar(i), 1);
+            mbar_init(done_bar(i), G);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    if (warp == W) {
+        // ================= producer =================
+        const uint32_t bv = (uint32_t)out_bytes;                                          // vn column bytes
+        const uint32_t bw = (uint32_t)(((nlev + 1) * (int)sizeof(T) + 15) & ~15);         // w column bytes
+        const uint64_t cs = (uint64_t)ldk * sizeof(T), cs_w = (uint64_t)ldk_w * sizeof(T);
+        const uint32_t slot0 = smem_u32(slot_base), rec0 = smem_u32(rec_base);
+        int drained = 0;
+        // headers two steps ahead and the first 32 list entries one step ahead, so that the only
+        // latency on the issue path is the wait for the stage itself
+        auto hdr = [&](int s) {
+            CcStep z;
+            z.load_begin = 0; z.n_vn = 0; z.n_w = 0; z.n_patches = 0; z.depth = 1; z.pad = 0;
+            return s < n_steps ? d.steps[sb + s] : z;
+        };
+        auto entry = [&](const CcStep& st, int i) {
+            CcLoad z;
+            z.id = 0; z.slot = 0; z.kind = 0;
+            return i < st.n_vn + st.n_w ? d.loads[st.load_begin + i] : z;
+        };
+        CcStep st = hdr(0), st1 = hdr(1);
+        CcLoad e0 = entry(st, lane);
+        for (int s = 0; s < n_steps; ++s) {
+            const CcStep st2 = hdr(s + 2);
+            const CcLoad e1 = entry(st1, lane);
+            const int n_loads = st.n_vn + st.n_w;
+            while (drained < s - (int)st.depth + 1) {
+                mbar_wait(done_bar(drained % D), (uint32_t)((drained / D) & 1));
+                ++drained;
+            }
+            const uint32_t fb = full_bar(s % D);
+            if (lane == 0)
+                mbar_arrive_expect_tx(fb, st.n_vn * bv + st.n_w * bw + st.n_patches * (uint32_t)REC);
+            __syncwarp();
+            if (lane < st.n_patches) {
+                const int64_t p = pb + (int64_t)s * G + lane;
+                bulk_g2s(rec0 + (uint32_t)(((s % D) * G + lane) * REC), d.records + p * REC, (uint32_t)REC, fb);
+            }
+            for (int i = lane; i < n_loads; i += 32) {
+                const CcLoad e = i == lane ? e0 : d.loads[st.load_begin + i];
+                const unsigned char* src = e.kind ? reinterpret_cast<const unsigned char*>(w) + (uint64_t)e.id * cs_w
+                                                  : reinterpret_cast<const unsigned char*>(vn) + (uint64_t)e.id * cs;
+                bulk_g2s(slot0 + (uint32_t)e.slot * (uint32_t)d.slot_bytes, src, e.kind ? bw : bv, fb);
+            }
+            st = st1; st1 = st2; e0 = e1;
+        }
+        return;
+    }
+
+    // ================= consumers =================
+    const int grp = warp / G, wi = warp % G;
+    // per-lane level coefficients of the vertical term (reading P-14): levels L*lane + l
+    T cA[L], cB[L], cC[L];
+    int kv[L], kw[L];        // clamped level indices for vn / w reads (idle lanes re-read a valid level)
+    bool po[L];
+    FORL {
+        const int k = L * lane + l;
+        po[l] = k < nlev;
+        kv[l] = k < nlev ? k : nlev - 1;
+        kw[l] = k <= nlev ? k : nlev;
+        cA[l] = po[l] ? __ldg(abc + k) : (T)0;
+        cB[l] = po[l] ? __ldg(abc + nlev + k) : (T)0;
+        cC[l] = po[l] ? __ldg(abc + 2 * nlev + k) : (T)0;
+    }
+    unsigned char* my_out = out_base + warp * 2 * out_bytes;
+    const int bulk_out = (nlev * (int)sizeof(T)) & ~15;       // bytes of a ddt_vn column that leave by bulk store
+    const uint64_t cs = (uint64_t)ldk * sizeof(T);
+    int n_out = 0;
+
+    for (int s = grp; s < n_steps; s += NGRP) {
+        const int64_t p = pb + (int64_t)s * G + wi;
+        mbar_wait(full_bar(s % D), (uint32_t)((s / D) & 1));
+        if (p < pe) {
+            const unsigned char* rec = rec_base + ((s % D) * G + wi) * REC;
+            const T* cf = reinterpret_cast<const T*>(rec);
+            const int32_t* oid = reinterpret_cast<const int32_t*>(rec + kScCoefWords * sizeof(T));
+            const uint16_t* sl = reinterpret_cast<const uint16_t*>(rec + kScCoefWords * sizeof(T) + 32);
+
+            auto LD = [&](uint32_t off) {
+                const T* q = reinterpret_cast<const T*>(slot_base + off);
+                C c;
+                FORL c.v[l] = q[kv[l]];
+                return c;
+            };
+            auto WF = [&](uint32_t off) {       // w_f(k) = (w(k) + w(k+1)) / 2 (S6)
+                const T* q = reinterpret_cast<const T*>(slot_base + off);
+                C c;
+                FORL c.v[l] = q[kw[l]];
+                C dn = level_down(c);
+                FORL c.v[l] = (T)0.5 * (c.v[l] + dn.v[l]);
+                return c;
+            };
+            auto VD = [&](const C& x) {         // (vn_ie(k) - vn_ie(k+1)) / dz_k, reading P-14 folded into A, B, C
+                C up = level_up(x), dn = level_down(x), o;
+                FORL o.v[l] = cA[l] * up.v[l] + cB[l] * x.v[l] + cC[l] * dn.v[l];
+                return o;
+            };
+            auto ST = [&](int32_t id, const C& x) {
+                unsigned char* buf = my_out + (n_out & 1) * out_bytes;
+                if (lane == 0) bulk_wait_read<1>();        // the store that used this buffer two columns ago has read it
+                __syncwarp();
+                T* q = reinterpret_cast<T*>(buf);
+                FORL if (po[l]) q[L * lane + l] = x.v[l];
+                fence_proxy_async();
+                __syncwarp();
+                T* dst = reinterpret_cast<T*>(reinterpret_cast<unsigned char*>(ddt_vn) + (uint64_t)(uint32_t)id * cs);
+                if (lane == 0 && bulk_out > 0) {
+                    bulk_s2g(dst, smem_u32(buf), (uint32_t)bulk_out);
+                    bulk_commit();
+                }
+                FORL if (po[l] && (L * lane + l) * (int)sizeof(T) >= bulk_out) dst[L * lane + l] = x.v[l];
+                ++n_out;
+            };
+
+            uint32_t sE[24];                    // i0 i1 i2 b0..b5 om0..om5 oc0..oc5 x0[0..2]
+            ld_slots(sl + SID_I0, sE);
+            C vI[3], vB[6];
+#pragma unroll
+            for (int j = 0; j < 3; ++j) vI[j] = LD(sE[j]);
+#pragma unroll
+            for (int j = 0; j < 6; ++j) vB[j] = LD(sE[3 + j]);
+
+            // ---- interior edges: vt, KE_e; start the cell sums -------------------------------
+            T r12[12];
+            ld_coef(cf + SCF_RBF, r12);
+            C tI[3];
+            tI[0] = dot4(r12 + 0, vB[0], vB[5], vI[1], vI[2]);
+            tI[1] = dot4(r12 + 4, vB[1], vB[2], vI[2], vI[0]);
+            tI[2] = dot4(r12 + 8, vB[3], vB[4], vI[0], vI[1]);
+            T bl[12];
+            ld_coef(cf + SCF_BLN, bl);
+            C ke[4];
+            {
+                C kI0 = ke2(vI[0], tI[0]), kI1 = ke2(vI[1], tI[1]), kI2 = ke2(vI[2], tI[2]);
+                ke[0] = scale(bl[1], kI0);
+                ke[1] = scale(bl[5], kI1);
+                ke[2] = scale(bl[6], kI2);
+                FORL ke[3].v[l] = bl[9] * kI1.v[l] + bl[10] * kI2.v[l] + bl[11] * kI0.v[l];
+            }
+            // ---- midpoint vorticities (x 1/2): interior + boundary part ----------------------
+            T g18[20];
+            ld_coef(cf + SCF_ROT, g18);
+            C zm[3];
+            FORL {
+                zm[0].v[l] = g18[0] * vB[0].v[l] + g18[1] * vB[1].v[l] + g18[2] * vI[0].v[l] + g18[3] * vI[1].v[l];
+                zm[1].v[l] = g18[6] * vB[2].v[l] + g18[7] * vB[3].v[l] + g18[8] * vI[1].v[l] + g18[9] * vI[2].v[l];
+                zm[2].v[l] = g18[12] * vB[4].v[l] + g18[13] * vB[5].v[l] + g18[14] * vI[2].v[l] + g18[15] * vI[0].v[l];
+            }
+            // ---- corner vorticities (x 1/2): the part from the patch's own boundary edges ------
+            T gx[20];
+            ld_coef(cf + SCF_XROT, gx);
+            C zc[3];
+            FORL {
+                zc[0].v[l] = gx[0] * vB[0].v[l] + gx[5] * vB[5].v[l];
+                zc[1].v[l] = gx[6] * vB[2].v[l] + gx[11] * vB[1].v[l];
+                zc[2].v[l] = gx[12] * vB[4].v[l] + gx[17] * vB[3].v[l];
+            }
+            // ---- boundary edges b0..b5 with their outer columns ------------------------------
+            uint32_t sX[24];                    // x0[3..4] x1[0..4] x2[0..4] T0..T3 X0 X2 X4 + pad
+            ld_slots(sl + SID_X0 + 3, sX);
+            T rB[24];
+            ld_coef(cf + SCF_RBF + 12, rB);
+            T xrm[12], xro[12], xbl[12];
+            ld_coef(cf + SCF_XRM, xrm);
+            ld_coef(cf + SCF_XRO, xro);
+            ld_coef(cf + SCF_XBL, xbl);
+            C tBo[3], keX[3];
+#pragma unroll
+            for (int j = 0; j < 6; ++j) {
+                const C vM = LD(sE[9 + j]), vO = LD(sE[15 + j]);
+                // neighbour pairs (a, b) of the stencil of b_j inside the patch
+                const C& na = j == 0 ? vI[0] : j == 1 ? vB[2] : j == 2 ? vB[1] : j == 3 ? vI[2] : j == 4 ? vI[2] : vB[0];
+                const C& nb = j == 0 ? vB[5] : j == 1 ? vI[1] : j == 2 ? vI[1] : j == 3 ? vB[4] : j == 4 ? vB[3] : vI[0];
+                const C tB = dot4(rB + 4 * j, na, nb, vM, vO);
+                const C kB = ke2(vB[j], tB);
+                // KE_c of the patch cell that holds b_j (bln slot order of sc_tables.cpp)
+                constexpr int cell_of[6] = {0, 1, 1, 2, 2, 0};
+                constexpr int bslot[6] = {0, 3, 4, 7, 8, 2};
+                axpy(ke[cell_of[j]], bl[bslot[j]], kB);
+                // midpoint vorticity: om_j is fan slot 4 + (j & 1) of midpoint j / 2
+                axpy(zm[j / 2], g18[6 * (j / 2) + 4 + (j & 1)], vM);
+                if (j & 1) {
+                    // oc_j is slot 4 (oc_jp) of the corner of the next owned boundary edge
+                    const int xn = ((j + 1) % 6) / 2;
+                    axpy(zc[xn], gx[6 * xn + 4], vO);
+                } else {
+                    const int x = j / 2;
+                    // ring columns pm0 pm1 pcf n1 n2 of x: id slots SID_X0 + 5x ..; sE holds x0[0..2], sX the rest
+                    const uint32_t s_pm0 = x == 0 ? sE[21] : sX[5 * x - 3], s_pm1 = x == 0 ? sE[22] : sX[5 * x - 2];
+                    const uint32_t s_pcf = x == 0 ? sE[23] : sX[5 * x - 1];
+                    const uint32_t s_n1 = sX[5 * x], s_n2 = sX[5 * x + 1];
+                    const C pm0 = LD(s_pm0), pm1 = LD(s_pm1), pcf = LD(s_pcf), n1 = LD(s_n1), n2 = LD(s_n2);
+                    const C tM = dot4(xrm + 4 * x, vB[j], vO, pm0, pm1);
+                    const C tO = dot4(xro + 4 * x, vB[j], vM, n1, pcf);
+                    const C kM = ke2(vM, tM), kO = ke2(vO, tO);
+                    FORL keX[x].v[l] = xbl[3 * x] * kB.v[l] + xbl[3 * x + 1] * kM.v[l] + xbl[3 * x + 2] * kO.v[l];
+                    FORL zc[x].v[l] += gx[6 * x + 1] * vO.v[l] + gx[6 * x + 2] * n1.v[l] + gx[6 * x + 3] * n2.v[l];
+                    tBo[x] = tB;
+                }
+            }
+            // ---- horizontal part H of the six owned edges (S5); frees the KE / vorticity columns ----
+            T ec[24];
+            ld_coef(cf + SCF_EDGE, ec);
+            C H[6];
+#pragma unroll
+            for (int x = 0; x < 3; ++x) {       // interior: i0 (ab, ca), i1 (ab, bc), i2 (bc, ca); cells (T_x, T3)
+                const C& za = x == 2 ? zm[1] : zm[0];
+                const C& zb = x == 0 ? zm[2] : x == 1 ? zm[1] : zm[2];
+                const T* e4 = ec + 4 * x;
+                FORL H[x].v[l] = (ke[3].v[l] - ke[x].v[l]) * e4[0] + tI[x].v[l] * (e4[1] + (za.v[l] + zb.v[l]));
+            }
+#pragma unroll
+            for (int x = 0; x < 3; ++x) {       // boundary: b0 (a, ab), b2 (b, bc), b4 (c, ca); cells (T_x, X_2x)
+                const T* e4 = ec + 4 * (3 + x);
+                FORL H[3 + x].v[l] = (keX[x].v[l] - ke[x].v[l]) * e4[0] + tBo[x].v[l] * (e4[1] + (zm[x].v[l] + zc[x].v[l]));
+            }
+            // ---- cell-centre w (S6); these are the last reads of the slots -----------------------
+            C wf[4], wx[3];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) wf[j] = WF(sX[12 + j]);
+#pragma unroll
+            for (int x = 0; x < 3; ++x) wx[x] = WF(sX[16 + x]);
+            int32_t ido[8];
+            {
+                const int4 a = reinterpret_cast<const int4*>(oid)[0], b = reinterpret_cast<const int4*>(oid)[1];
+                ido[0] = a.x; ido[1] = a.y; ido[2] = a.z; ido[3] = a.w; ido[4] = b.x; ido[5] = b.y; ido[6] = b.z; ido[7] = b.w;
+            }
+            // everything this patch needs from the slots and its record is in registers: release the stage
+            __syncwarp();
+            if (lane == 0) mbar_arrive(done_bar(s % D));
+
+            // ---- vertical part and the tendency (S6, S7) -----------------------------------------
+#pragma unroll
+            for (int x = 0; x < 6; ++x) {
+                const C Dv = VD(x < 3 ? vI[x] : vB[2 * (x - 3)]);
+                const C& wl = wf[x < 3 ? x : x - 3];
+                const C& wh = x < 3 ? wf[3] : wx[x - 3];
+                const T* e4 = ec + 4 * x;
+                C o;
+                FORL o.v[l] = -(H[x].v[l] + (e4[2] * wl.v[l] + e4[3] * wh.v[l]) * Dv.v[l]);
+                ST(ido[x], o);
+            }
+        } else {
+            __syncwarp();
+            if (lane == 0) mbar_arrive(done_bar(s % D));
+        }
+    }
+    if (lane == 0) bulk_wait_all();
+}
+
+}  // namespace
+
+template <class T>
+int cc_slot_bytes(int nlev) { return (((nlev + 1) * (int)sizeof(T) + 15) & ~15); }
+
+template <class T>
+static size_t cc_fixed_smem(const CcShape& sh, int nlev) {
+    const int out_bytes = (nlev * (int)sizeof(T) + 15) & ~15;
+    return kCcBarrierBytes + (size_t)sh.depth * sh.group * cc_record_bytes<T>() + (size_t)sh.warps * 2 * out_bytes;
+}
+
+template <class T>
+int cc_max_slots(int shape, int nlev, int smem_optin) {
+    const long avail = (long)smem_optin - (long)cc_fixed_smem<T>(cc_shape(shape), nlev);
+    if (avail <= 0) return 0;
+    return (int)(avail / cc_slot_bytes<T>(nlev));
+}
+template int cc_max_slots<double>(int, int, int);
+template int cc_max_slots<float>(int, int, int);
+template int cc_slot_bytes<double>(int);
+template int cc_slot_bytes<float>(int);
+
+int cc_levels_per_lane(int nlev) { return nlev + 1 <= 32 ? 1 : nlev + 1 <= 96 ? 3 : 0; }
+
+namespace {
+template <class T, int L, int W, int G, int D>
+cudaError_t cc_launch_one(const CcDev<T>& d, int n_ctas, size_t smem, int nlev, int ldk, int ldk_w, const T* abc,
+                          const T* vn, const T* w, T* ddt_vn, cudaStream_t s) {
+    auto k = k_tend_cc<T, L, W, G, D>;
+    static size_t configured = 0;       // largest dynamic shared-memory size this instantiation was opted in for
+    if (smem > configured) {
+        cudaError_t err = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (err != cudaSuccess) return err;
+        configured = smem;
+    }
+    k<<<(unsigned)n_ctas, (W + 1) * 32, smem, s>>>(d, nlev, ldk, ldk_w, abc, vn, w, ddt_vn);
+    return cudaGetLastError();
+}
+template <class T, int W, int G, int D>
+cudaError_t cc_launch_shape(int L, const CcDev<T>& d, int n_ctas, size_t smem, int nlev, int ldk, int ldk_w,
+                            const T* abc, const T* vn, const T* w, T* ddt_vn, cudaStream_t s) {
+    if (L == 1) return cc_launch_one<T, 1, W, G, D>(d, n_ctas, smem, nlev, ldk, ldk_w, abc, vn, w, ddt_vn, s);
+    if (L == 3) return cc_launch_one<T, 3, W, G, D>(d, n_ctas, smem, nlev, ldk, ldk_w, abc, vn, w, ddt_vn, s);
+    return cudaErrorInvalidValue;
+}
+}  // namespace
+
+template <class T>
+int launch_tendencies_cc(const icon_grid& g, const DevCcTables<T>& p, int nlev, int64_t ldk, int64_t ldk_w,
+                         const T* abc, const T* vn, const T* w, T* ddt_vn, cudaStream_t s) {
+    CcDev<T> d;
+    d.steps = p.steps; d.loads = p.loads; d.records = p.records;
+    d.cta_patch_begin = p.cta_patch_begin; d.cta_step_begin = p.cta_step_begin;
+    d.n_slots = p.n_slots; d.slot_bytes = p.slot_bytes;
+    const size_t smem = cc_fixed_smem<T>(cc_shape(p.shape), nlev) + (size_t)p.n_slots * p.slot_bytes;
+    const int L = cc_levels_per_lane(nlev);
+    cudaError_t err;
+#define CC_CASE(i, W, G, D)                                                                                        \
+    case i:                                                                                                        \
+        static_assert(kCcShapes[i].warps == W && kCcShapes[i].group == G && kCcShapes[i].depth == D, "shape table"); \
+        err = cc_launch_shape<T, W, G, D>(L, d, p.n_ctas, smem, nlev, (int)ldk, (int)ldk_w, abc, vn, w, ddt_vn, s); \
+        break;
+    switch (p.shape) {
+        CC_CASE(0, 7, 1, 9)
+        CC_CASE(1, 8, 2, 5)
+        CC_CASE(2, 6, 2, 5)
+        CC_CASE(3, 7, 1, 10)
+        default: err = cudaErrorInvalidValue;
+    }
+#undef CC_CASE
+    (void)g;
+    return err == cudaSuccess ? 1 : -(int)err;
+}
+
+template int launch_tendencies_cc<double>(const icon_grid&, const DevCcTables<double>&, int, int64_t, int64_t,
+                                          const double*, const double*, const double*, double*, cudaStream_t);
+template int launch_tendencies_cc<float>(const icon_grid&, const DevCcTables<float>&, int, int64_t, int64_t,
+                                         const float*, const float*, const float*, float*, cudaStream_t);
+
+}  // namespace icon

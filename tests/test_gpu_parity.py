@@ -33,6 +33,10 @@ def lib():
 _libgrids = {}
 
 
+# ICON_OPT_TENDENCY_KERNEL values; 40..43 = kernel 4 (column cache) with ICON_OPT_CC_SHAPE 0..3
+VARIANTS = [0, 1, 2, 3, 40, 41, 42, 43]
+
+
 def lib_grid(lib, k, seed=0, flags=0):
     key = (k, seed, flags)
     if key not in _libgrids:
@@ -54,6 +58,9 @@ def run_gpu(torch, lib, g, vn, w, zh, nlev, variant, want_opt=False, sentinel=No
         return t
     ddt, div, vort = out(g.ne), out(g.nc), out(g.nv)
     opt = dict(vt=out(g.ne), ke_c=out(g.nc), vort=out(g.nv)) if want_opt else {}
+    if variant >= 40:         # 4x = column-cache kernel with pipeline shape x
+        g.set_option(lib.ICON_OPT_CC_SHAPE, variant - 40)
+        variant = 4
     g.set_option(lib.ICON_OPT_TENDENCY_KERNEL, variant)
     n0 = g.launch_count
     lib.dycore_velocity_tendencies(g, zh, d_vn, d_w, ddt, nlev, **opt)
@@ -102,7 +109,7 @@ def check_all(res, ref, nlev, tol, opt=False):
 # ----------------------------------------------------------------------------------------------
 # configs[0]: R2B4 x 90 fp64, element by element, every kernel variant, optional outputs
 # ----------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("variant", [0, 1, 2, 3])
+@pytest.mark.parametrize("variant", VARIANTS)
 def test_config1_r2b4_fp64_elementwise(torch_cuda, lib, oracle_grid, variant):
     og = oracle_grid(4)
     g = lib_grid(lib, 4)
@@ -126,7 +133,7 @@ def test_library_geometry_fed_to_oracle(torch_cuda, lib, oracle_mod, oracle_grid
     div, md = oracle_mod.divergence(t["c2e"], t["geofac_div"], vn64, nlev)
     vort, mv = oracle_mod.vorticity(t["v2e"], t["geofac_rot"], vn64, nlev)
     ref.update(div=div, m_div=md, vort_dv=vort, m_vort=mv)
-    for variant in (0, 1, 2, 3):
+    for variant in VARIANTS:
         res = run_gpu(torch_cuda, lib, g, vn, w, zh, nlev, variant)
         check_all(res, ref, nlev, TOL["f64"])
 
@@ -136,7 +143,7 @@ def test_library_geometry_fed_to_oracle(torch_cuda, lib, oracle_mod, oracle_grid
 # ----------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("k,nlev,ldk,ldk_w", [(0, 2, 2, 4), (0, 3, 4, 4), (1, 31, 32, 32), (1, 33, 34, 34),
                                                (2, 64, 64, 66), (2, 65, 66, 66), (3, 90, 96, 92), (2, 130, 130, 132)])
-@pytest.mark.parametrize("variant", [0, 1, 2, 3])
+@pytest.mark.parametrize("variant", VARIANTS)
 def test_ragged_levels_and_padding(torch_cuda, lib, oracle_grid, k, nlev, ldk, ldk_w, variant):
     og = oracle_grid(k)
     g = lib_grid(lib, k)
@@ -150,7 +157,7 @@ def test_ragged_levels_and_padding(torch_cuda, lib, oracle_grid, k, nlev, ldk, l
 
 
 @pytest.mark.parametrize("flags_extra", [0, 8])
-@pytest.mark.parametrize("variant", [0, 1, 2, 3])
+@pytest.mark.parametrize("variant", VARIANTS)
 def test_permuted_grid_fp64(torch_cuda, lib, oracle_grid, flags_extra, variant):
     """seeded renumbering, with the locality work-list (default) and without (ICON_NO_WORKLIST)"""
     og = oracle_grid(3, si.PERMUTE_SEED, 1)
@@ -160,9 +167,11 @@ def test_permuted_grid_fp64(torch_cuda, lib, oracle_grid, flags_extra, variant):
     ref = oracle_reference(og, vn, w, zh, nlev, False)
     res = run_gpu(torch_cuda, lib, g, vn, w, zh, nlev, variant, want_opt=True)
     check_all(res, ref, nlev, TOL["f64"], opt=True)
+    res = run_gpu(torch_cuda, lib, g, vn, w, zh, nlev, variant)
+    check_all(res, ref, nlev, TOL["f64"])
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2, 3])
+@pytest.mark.parametrize("variant", VARIANTS)
 def test_fp32_variant_permuted_r2b4(torch_cuda, lib, oracle_grid, variant):
     """config 4 at a size the oracle finishes in seconds: fp32 fields, permuted ids, tol 1e-5"""
     og = oracle_grid(4, si.PERMUTE_SEED, 1)
@@ -172,6 +181,8 @@ def test_fp32_variant_permuted_r2b4(torch_cuda, lib, oracle_grid, variant):
     ref = oracle_reference(og, vn, w, zh, 90, True)
     res = run_gpu(torch_cuda, lib, g, vn, w, zh, 90, variant, want_opt=True)
     check_all(res, ref, 90, TOL["f32"], opt=True)
+    res = run_gpu(torch_cuda, lib, g, vn, w, zh, 90, variant)
+    check_all(res, ref, 90, TOL["f32"])
 
 
 def test_argument_errors_on_device(torch_cuda, lib):
