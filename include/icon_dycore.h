@@ -91,7 +91,9 @@ enum {
                                          by bulk asynchronous copies on a host-built schedule; level counts
                                          it cannot hold (nlev > 95) fall back to 3. */
     ICON_OPT_CC_SHAPE = 1,        /* pipeline shape of kernel 4 (consumer warps / patches per step / ring
-                                     depth): 0 = 7/1/9 (default), 1 = 8/2/5, 2 = 6/2/5, 3 = 7/1/10. */
+                                     depth): 0 = 8/1/10 (default), 1 = 8/2/5, 2 = 8/1/9, 3 = 8/1/11. */
+    ICON_OPT_CC_L2_HINTS = 2,     /* L2 eviction hints of kernel 4, bit mask: 1 = ddt_vn stores evict-first,
+                                     2 = patch records evict-first, 4 = vn / w columns evict-last. Default 3. */
     ICON_OPT_COUNT
 };
 

@@ -470,6 +470,7 @@ int icon_grid_create(int bisections_k, uint64_t seed, unsigned flags, icon_grid_
     g->seed = seed;
     g->host_only = (flags & ICON_HOST_ONLY) != 0;
     g->options[ICON_OPT_TENDENCY_KERNEL] = 4;
+    g->options[ICON_OPT_CC_L2_HINTS] = 3;
     try {
         std::string err = icon::build_host_grid(bisections_k, seed, (flags & ICON_PERMUTE) != 0, g->host);
         if (!err.empty()) {
@@ -573,6 +574,7 @@ int icon_grid_table_device(icon_grid_t* g, int which, int dtype, const void** dp
 int icon_grid_set_option(icon_grid_t* g, int option, int value) {
     if (!g) return fail(ICON_EINVAL, "grid handle is NULL");
     if (option < 0 || option >= ICON_OPT_COUNT) return fail(ICON_EINVAL, "unknown option");
+    if (option == ICON_OPT_CC_L2_HINTS && (value < 0 || value > 7)) return fail(ICON_EINVAL, "bad option value");
     if (option == ICON_OPT_CC_SHAPE && (value < 0 || value >= icon::kCcNumShapes)) return fail(ICON_EINVAL, "bad option value");
     if (option == ICON_OPT_TENDENCY_KERNEL && (value < 0 || value > 4)) return fail(ICON_EINVAL, "bad option value");
     g->options[option] = value;

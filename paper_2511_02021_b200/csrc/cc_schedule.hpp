@@ -25,15 +25,21 @@
 namespace icon {
 
 // pipeline shapes of the kernel (kernels_cc.cu): consumer warps, patches per step, ring depth.
-// One producer warp is added to `warps`; with 8 warps per CTA a thread may use 255 registers,
-// with 9 only 168 (the register file is split over the four SM sub-partitions).
+// kCcProducers producer warps (one warpgroup) are added to `warps`; the CTA is launched with
+// 168 registers per thread and re-balances them with setmaxnreg: producers keep
+// kCcProducerRegs, consumers grow to kCcConsumerRegs
+// ((4 * 40 + 8 * 232) * 32 = 64512 <= 65536 registers of the SM).
+constexpr int kCcProducers = 4;
+constexpr int kCcProducerRegs = 40;
+constexpr int kCcConsumerRegs = 232;
 struct CcShape {
     int warps, group, depth;
 };
 constexpr int kCcNumShapes = 4;
-constexpr CcShape kCcShapes[kCcNumShapes] = {{7, 1, 9}, {8, 2, 5}, {6, 2, 5}, {7, 1, 10}};
+constexpr CcShape kCcShapes[kCcNumShapes] = {{8, 1, 10}, {8, 2, 5}, {8, 1, 9}, {8, 1, 11}};
 inline const CcShape& cc_shape(int i) { return kCcShapes[i >= 0 && i < kCcNumShapes ? i : 0]; }
-constexpr int kCcBarrierBytes = 256;
+constexpr int kCcBarrierBytes = 256;    // the mbarriers
+constexpr int kCcOutCols = 3;            // ddt_vn staging columns per consumer warp (one store batch)
 // a patch record on the device = kScCoefWords coefficients (T), then 8 int32 (user ids of the six
 // owned edges i0 i1 i2 b0 b2 b4, 2 pad), then kCcSlotWords uint16 slot offsets
 constexpr int kCcRecordTail = 32 + 96;

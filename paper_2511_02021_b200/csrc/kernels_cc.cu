@@ -23,6 +23,7 @@
 // (depth stored per step), and the producer issues them once those steps have drained.
 #include <cuda_pipeline.h>
 
+#include "../../include/icon_dycore.h"
 #include "kernels.cuh"
 #include "cc_schedule.hpp"
 
@@ -59,9 +60,28 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
                  "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
+// the same with an L2 eviction-priority hint (policy from l2_policy_*)
+__device__ __forceinline__ void bulk_g2s_hint(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar, uint64_t pol) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar), "l"(pol) : "memory");
+}
 // shared -> global, tracked by the issuing thread's bulk async-group
 __device__ __forceinline__ void bulk_s2g(void* dst, uint32_t src, uint32_t bytes) {
     asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_s2g_hint(void* dst, uint32_t src, uint32_t bytes, uint64_t pol) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;" ::"l"(dst), "r"(src),
+                 "r"(bytes), "l"(pol) : "memory");
+}
+__device__ __forceinline__ uint64_t l2_policy_evict_first() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ uint64_t l2_policy_evict_last() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
 }
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 template <int N>
@@ -169,20 +189,20 @@ __host__ __device__ constexpr int cc_record_bytes() { return kScCoefWords * (int
 
 // W consumer warps in W/G groups of G; group g runs the steps s = g (mod W/G). D = ring depth.
 template <class T, int L, int W, int G, int D>
-__global__ void __launch_bounds__((W + 1) * 32, 1)
-k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, const T* __restrict__ vn,
+__global__ void __launch_bounds__((W + kCcProducers) * 32, 1)
+k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restrict__ abc, const T* __restrict__ vn,
           const T* __restrict__ w, T* __restrict__ ddt_vn) {
     extern __shared__ __align__(128) unsigned char smem[];
     using C = Col<T, L>;
     constexpr int REC = cc_record_bytes<T>();
     constexpr int NGRP = W / G;
-    static_assert(W % G == 0 && D > NGRP && D <= 16, "bad pipeline shape");
+    static_assert(W % G == 0 && W % 4 == 0 && D > NGRP && D <= 16, "bad pipeline shape");
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int out_bytes = (nlev * (int)sizeof(T) + 15) & ~15;                 // staging column, 16-byte multiple
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem);                       // full[D], done[D]
     unsigned char* rec_base = smem + kCcBarrierBytes;
     unsigned char* out_base = rec_base + D * G * REC;
-    unsigned char* slot_base = out_base + W * 2 * out_bytes;
+    unsigned char* slot_base = out_base + W * kCcOutCols * out_bytes;
     const uint32_t bar0 = smem_u32(bars);
     auto full_bar = [&](int i) { return bar0 + 8u * (uint32_t)i; };
     auto done_bar = [&](int i) { return bar0 + 8u * (uint32_t)(D + i); };
@@ -200,14 +220,23 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
     }
     __syncthreads();
 
-    if (warp == W) {
-        // ================= producer =================
+    if (warp >= W) {
+        // ================= producers (one warpgroup) =================
+        // Issuing a bulk copy costs a ~100-cycle chain on the uniform datapath, so the list of a
+        // step is dealt round-robin to kCcProducers warps. Registers go to the consumers.
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kCcProducerRegs));
+        // hints: bit 0 = ddt_vn stores evict-first, bit 1 = patch records evict-first, bit 2 = columns evict-last
+        const int pw = warp - W;
         const uint32_t bv = (uint32_t)out_bytes;                                          // vn column bytes
         const uint32_t bw = (uint32_t)(((nlev + 1) * (int)sizeof(T) + 15) & ~15);         // w column bytes
         const uint64_t cs = (uint64_t)ldk * sizeof(T), cs_w = (uint64_t)ldk_w * sizeof(T);
         const uint32_t slot0 = smem_u32(slot_base), rec0 = smem_u32(rec_base);
+        const uint64_t pol_first = l2_policy_evict_first(), pol_last = l2_policy_evict_last();
+        const bool hint_rec = hints & 2, hint_col = hints & 4;
+        const uint2* lraw = reinterpret_cast<const uint2*>(d.loads);
+        const int mine = kCcProducers * lane + pw;          // this lane's entry of each round of 32 * kCcProducers
         int drained = 0;
-        // headers two steps ahead and the first 32 list entries one step ahead, so that the only
+        // headers two steps ahead and this lane's first list entry one step ahead, so that the only
         // latency on the issue path is the wait for the stage itself
         auto hdr = [&](int s) {
             CcStep z;
@@ -215,58 +244,62 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
             return s < n_steps ? d.steps[sb + s] : z;
         };
         auto entry = [&](const CcStep& st, int i) {
-            CcLoad z;
-            z.id = 0; z.slot = 0; z.kind = 0;
-            return i < st.n_vn + st.n_w ? d.loads[st.load_begin + i] : z;
+            return i < st.n_vn + st.n_w ? __ldg(lraw + st.load_begin + i) : make_uint2(0u, 0u);
         };
         CcStep st = hdr(0), st1 = hdr(1);
-        CcLoad e0 = entry(st, lane);
+        uint2 e0 = entry(st, mine);
         for (int s = 0; s < n_steps; ++s) {
             const CcStep st2 = hdr(s + 2);
-            const CcLoad e1 = entry(st1, lane);
+            const uint2 e1 = entry(st1, mine);
             const int n_loads = st.n_vn + st.n_w;
             while (drained < s - (int)st.depth + 1) {
                 mbar_wait(done_bar(drained % D), (uint32_t)((drained / D) & 1));
                 ++drained;
             }
             const uint32_t fb = full_bar(s % D);
-            if (lane == 0)
+            if (pw == 0 && lane == 0)
                 mbar_arrive_expect_tx(fb, st.n_vn * bv + st.n_w * bw + st.n_patches * (uint32_t)REC);
-            __syncwarp();
-            if (lane < st.n_patches) {
+            if (pw == kCcProducers - 1 && lane < (int)st.n_patches) {
                 const int64_t p = pb + (int64_t)s * G + lane;
-                bulk_g2s(rec0 + (uint32_t)(((s % D) * G + lane) * REC), d.records + p * REC, (uint32_t)REC, fb);
+                const uint32_t dst = rec0 + (uint32_t)(((s % D) * G + lane) * REC);
+                if (hint_rec) bulk_g2s_hint(dst, d.records + p * REC, (uint32_t)REC, fb, pol_first);
+                else bulk_g2s(dst, d.records + p * REC, (uint32_t)REC, fb);
             }
-            for (int i = lane; i < n_loads; i += 32) {
-                const CcLoad e = i == lane ? e0 : d.loads[st.load_begin + i];
-                const unsigned char* src = e.kind ? reinterpret_cast<const unsigned char*>(w) + (uint64_t)e.id * cs_w
-                                                  : reinterpret_cast<const unsigned char*>(vn) + (uint64_t)e.id * cs;
-                bulk_g2s(slot0 + (uint32_t)e.slot * (uint32_t)d.slot_bytes, src, e.kind ? bw : bv, fb);
+            for (int base = 0; base + mine < n_loads; base += 32 * kCcProducers) {
+                const uint2 e = base == 0 ? e0 : entry(st, base + mine);
+                // CcLoad: id | slot (low 16 bits) kind (high 16 bits)
+                const uint32_t slot = e.y & 0xffffu, kind = e.y >> 16;
+                const unsigned char* src = kind ? reinterpret_cast<const unsigned char*>(w) + (uint64_t)e.x * cs_w
+                                                : reinterpret_cast<const unsigned char*>(vn) + (uint64_t)e.x * cs;
+                const uint32_t dst = slot0 + slot * (uint32_t)d.slot_bytes;
+                if (hint_col) bulk_g2s_hint(dst, src, kind ? bw : bv, fb, pol_last);
+                else bulk_g2s(dst, src, kind ? bw : bv, fb);
             }
             st = st1; st1 = st2; e0 = e1;
         }
         return;
     }
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kCcConsumerRegs));
 
     // ================= consumers =================
     const int grp = warp / G, wi = warp % G;
     // per-lane level coefficients of the vertical term (reading P-14): levels L*lane + l
     T cA[L], cB[L], cC[L];
-    int kv[L], kw[L];        // clamped level indices for vn / w reads (idle lanes re-read a valid level)
-    bool po[L];
+    bool po[L], pw[L];       // this lane's levels that exist in a vn / ddt_vn column and in a w column
     FORL {
         const int k = L * lane + l;
         po[l] = k < nlev;
-        kv[l] = k < nlev ? k : nlev - 1;
-        kw[l] = k <= nlev ? k : nlev;
+        pw[l] = k <= nlev;
         cA[l] = po[l] ? __ldg(abc + k) : (T)0;
         cB[l] = po[l] ? __ldg(abc + nlev + k) : (T)0;
         cC[l] = po[l] ? __ldg(abc + 2 * nlev + k) : (T)0;
     }
-    unsigned char* my_out = out_base + warp * 2 * out_bytes;
+    unsigned char* my_out = out_base + warp * kCcOutCols * out_bytes;
     const int bulk_out = (nlev * (int)sizeof(T)) & ~15;       // bytes of a ddt_vn column that leave by bulk store
     const uint64_t cs = (uint64_t)ldk * sizeof(T);
-    int n_out = 0;
+    const uint32_t lane_off = (uint32_t)(L * lane * (int)sizeof(T));
+    const uint64_t pol_first = l2_policy_evict_first();
+    const bool hint_out = hints & 1;
 
     for (int s = grp; s < n_steps; s += NGRP) {
         const int64_t p = pb + (int64_t)s * G + wi;
@@ -278,15 +311,15 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
             const uint16_t* sl = reinterpret_cast<const uint16_t*>(rec + kScCoefWords * sizeof(T) + 32);
 
             auto LD = [&](uint32_t off) {
-                const T* q = reinterpret_cast<const T*>(slot_base + off);
+                const T* q = reinterpret_cast<const T*>(slot_base + off + lane_off);
                 C c;
-                FORL c.v[l] = q[kv[l]];
+                FORL c.v[l] = po[l] ? q[l] : (T)0;
                 return c;
             };
             auto WF = [&](uint32_t off) {       // w_f(k) = (w(k) + w(k+1)) / 2 (S6)
-                const T* q = reinterpret_cast<const T*>(slot_base + off);
+                const T* q = reinterpret_cast<const T*>(slot_base + off + lane_off);
                 C c;
-                FORL c.v[l] = q[kw[l]];
+                FORL c.v[l] = pw[l] ? q[l] : (T)0;
                 C dn = level_down(c);
                 FORL c.v[l] = (T)0.5 * (c.v[l] + dn.v[l]);
                 return c;
@@ -296,21 +329,34 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
                 FORL o.v[l] = cA[l] * up.v[l] + cB[l] * x.v[l] + cC[l] * dn.v[l];
                 return o;
             };
-            auto ST = [&](int32_t id, const C& x) {
-                unsigned char* buf = my_out + (n_out & 1) * out_bytes;
-                if (lane == 0) bulk_wait_read<1>();        // the store that used this buffer two columns ago has read it
+            // kCcOutCols finished ddt_vn columns leave together: staged in shared memory (stride-L
+            // writes, conflict free), one proxy fence, then one bulk store each
+            auto ST3 = [&](const int32_t* ids, const C* x) {
+                if (lane == 0) bulk_wait_read<0>();        // the previous batch has been read out of the staging columns
                 __syncwarp();
-                T* q = reinterpret_cast<T*>(buf);
-                FORL if (po[l]) q[L * lane + l] = x.v[l];
+#pragma unroll
+                for (int j = 0; j < kCcOutCols; ++j) {
+                    T* q = reinterpret_cast<T*>(my_out + j * out_bytes + lane_off);
+                    FORL if (po[l]) q[l] = x[j].v[l];
+                }
                 fence_proxy_async();
                 __syncwarp();
-                T* dst = reinterpret_cast<T*>(reinterpret_cast<unsigned char*>(ddt_vn) + (uint64_t)(uint32_t)id * cs);
                 if (lane == 0 && bulk_out > 0) {
-                    bulk_s2g(dst, smem_u32(buf), (uint32_t)bulk_out);
+#pragma unroll
+                    for (int j = 0; j < kCcOutCols; ++j) {
+                        void* dst = reinterpret_cast<unsigned char*>(ddt_vn) + (uint64_t)(uint32_t)ids[j] * cs;
+                        if (hint_out) bulk_s2g_hint(dst, smem_u32(my_out + j * out_bytes), (uint32_t)bulk_out, pol_first);
+                        else bulk_s2g(dst, smem_u32(my_out + j * out_bytes), (uint32_t)bulk_out);
+                    }
                     bulk_commit();
                 }
-                FORL if (po[l] && (L * lane + l) * (int)sizeof(T) >= bulk_out) dst[L * lane + l] = x.v[l];
-                ++n_out;
+                if (bulk_out < nlev * (int)sizeof(T)) {    // the last < 16 bytes of a column go out directly
+#pragma unroll
+                    for (int j = 0; j < kCcOutCols; ++j) {
+                        T* dst = reinterpret_cast<T*>(reinterpret_cast<unsigned char*>(ddt_vn) + (uint64_t)(uint32_t)ids[j] * cs);
+                        FORL if (po[l] && (L * lane + l) * (int)sizeof(T) >= bulk_out) dst[L * lane + l] = x[j].v[l];
+                    }
+                }
             };
 
             uint32_t sE[24];                    // i0 i1 i2 b0..b5 om0..om5 oc0..oc5 x0[0..2]
@@ -431,15 +477,20 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
             if (lane == 0) mbar_arrive(done_bar(s % D));
 
             // ---- vertical part and the tendency (S6, S7) -----------------------------------------
+            static_assert(kCcOutCols == 3, "six owned edges leave in two batches of three");
 #pragma unroll
-            for (int x = 0; x < 6; ++x) {
-                const C Dv = VD(x < 3 ? vI[x] : vB[2 * (x - 3)]);
-                const C& wl = wf[x < 3 ? x : x - 3];
-                const C& wh = x < 3 ? wf[3] : wx[x - 3];
-                const T* e4 = ec + 4 * x;
-                C o;
-                FORL o.v[l] = -(H[x].v[l] + (e4[2] * wl.v[l] + e4[3] * wh.v[l]) * Dv.v[l]);
-                ST(ido[x], o);
+            for (int h = 0; h < 2; ++h) {
+                C o[3];
+#pragma unroll
+                for (int j = 0; j < 3; ++j) {
+                    const int x = 3 * h + j;
+                    const C Dv = VD(h == 0 ? vI[j] : vB[2 * j]);
+                    const C& wl = wf[j];
+                    const C& wh = h == 0 ? wf[3] : wx[j];
+                    const T* e4 = ec + 4 * x;
+                    FORL o[j].v[l] = -(H[x].v[l] + (e4[2] * wl.v[l] + e4[3] * wh.v[l]) * Dv.v[l]);
+                }
+                ST3(ido + 3 * h, o);
             }
         } else {
             __syncwarp();
@@ -457,7 +508,7 @@ int cc_slot_bytes(int nlev) { return (((nlev + 1) * (int)sizeof(T) + 15) & ~15);
 template <class T>
 static size_t cc_fixed_smem(const CcShape& sh, int nlev) {
     const int out_bytes = (nlev * (int)sizeof(T) + 15) & ~15;
-    return kCcBarrierBytes + (size_t)sh.depth * sh.group * cc_record_bytes<T>() + (size_t)sh.warps * 2 * out_bytes;
+    return kCcBarrierBytes + (size_t)sh.depth * sh.group * cc_record_bytes<T>() + (size_t)sh.warps * kCcOutCols * out_bytes;
 }
 
 template <class T>
@@ -475,7 +526,7 @@ int cc_levels_per_lane(int nlev) { return nlev + 1 <= 32 ? 1 : nlev + 1 <= 96 ? 
 
 namespace {
 template <class T, int L, int W, int G, int D>
-cudaError_t cc_launch_one(const CcDev<T>& d, int n_ctas, size_t smem, int nlev, int ldk, int ldk_w, const T* abc,
+cudaError_t cc_launch_one(const CcDev<T>& d, int n_ctas, size_t smem, int nlev, int ldk, int ldk_w, int hints, const T* abc,
                           const T* vn, const T* w, T* ddt_vn, cudaStream_t s) {
     auto k = k_tend_cc<T, L, W, G, D>;
     static size_t configured = 0;       // largest dynamic shared-memory size this instantiation was opted in for
@@ -484,14 +535,14 @@ cudaError_t cc_launch_one(const CcDev<T>& d, int n_ctas, size_t smem, int nlev, 
         if (err != cudaSuccess) return err;
         configured = smem;
     }
-    k<<<(unsigned)n_ctas, (W + 1) * 32, smem, s>>>(d, nlev, ldk, ldk_w, abc, vn, w, ddt_vn);
+    k<<<(unsigned)n_ctas, (W + kCcProducers) * 32, smem, s>>>(d, nlev, ldk, ldk_w, hints, abc, vn, w, ddt_vn);
     return cudaGetLastError();
 }
 template <class T, int W, int G, int D>
-cudaError_t cc_launch_shape(int L, const CcDev<T>& d, int n_ctas, size_t smem, int nlev, int ldk, int ldk_w,
+cudaError_t cc_launch_shape(int L, const CcDev<T>& d, int n_ctas, size_t smem, int nlev, int ldk, int ldk_w, int hints,
                             const T* abc, const T* vn, const T* w, T* ddt_vn, cudaStream_t s) {
-    if (L == 1) return cc_launch_one<T, 1, W, G, D>(d, n_ctas, smem, nlev, ldk, ldk_w, abc, vn, w, ddt_vn, s);
-    if (L == 3) return cc_launch_one<T, 3, W, G, D>(d, n_ctas, smem, nlev, ldk, ldk_w, abc, vn, w, ddt_vn, s);
+    if (L == 1) return cc_launch_one<T, 1, W, G, D>(d, n_ctas, smem, nlev, ldk, ldk_w, hints, abc, vn, w, ddt_vn, s);
+    if (L == 3) return cc_launch_one<T, 3, W, G, D>(d, n_ctas, smem, nlev, ldk, ldk_w, hints, abc, vn, w, ddt_vn, s);
     return cudaErrorInvalidValue;
 }
 }  // namespace
@@ -509,17 +560,16 @@ int launch_tendencies_cc(const icon_grid& g, const DevCcTables<T>& p, int nlev, 
 #define CC_CASE(i, W, G, D)                                                                                        \
     case i:                                                                                                        \
         static_assert(kCcShapes[i].warps == W && kCcShapes[i].group == G && kCcShapes[i].depth == D, "shape table"); \
-        err = cc_launch_shape<T, W, G, D>(L, d, p.n_ctas, smem, nlev, (int)ldk, (int)ldk_w, abc, vn, w, ddt_vn, s); \
+        err = cc_launch_shape<T, W, G, D>(L, d, p.n_ctas, smem, nlev, (int)ldk, (int)ldk_w, g.options[ICON_OPT_CC_L2_HINTS], abc, vn, w, ddt_vn, s); \
         break;
     switch (p.shape) {
-        CC_CASE(0, 7, 1, 9)
+        CC_CASE(0, 8, 1, 10)
         CC_CASE(1, 8, 2, 5)
-        CC_CASE(2, 6, 2, 5)
-        CC_CASE(3, 7, 1, 10)
+        CC_CASE(2, 8, 1, 9)
+        CC_CASE(3, 8, 1, 11)
         default: err = cudaErrorInvalidValue;
     }
 #undef CC_CASE
-    (void)g;
     return err == cudaSuccess ? 1 : -(int)err;
 }
 
