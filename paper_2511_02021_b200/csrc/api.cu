@@ -225,7 +225,7 @@ int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev) {
     int rc = ensure_sc_host(g);
     if (rc) return rc;
     const icon::ScTables& sc = g->sc_host;
-    const int n_slots = std::min(n_slots_max, 65535 / (slot_bytes / 16));
+    const int n_slots = std::min(n_slots_max, 65535);
     icon::CcSchedule cs;
     std::vector<unsigned char> rec;
     const size_t rb = (size_t)icon::kScCoefWords * sizeof(T) + icon::kCcRecordTail;
@@ -247,8 +247,13 @@ int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev) {
                 oid[x] = id[icon::SID_I0 + x];
                 oid[3 + x] = id[icon::SID_B0 + 2 * x];
             }
-            std::memcpy(r + (size_t)icon::kScCoefWords * sizeof(T) + 32, &cs.patch_slots[(size_t)q * icon::kCcSlotWords],
-                        icon::kCcSlotWords * 2);
+            for (int x = 0; x < 6; ++x) {          // c_lin halved: the kernel forms w(k) + w(k+1) (exact scaling)
+                cf[icon::SCF_EDGE + 4 * x + 2] *= (T)0.5;
+                cf[icon::SCF_EDGE + 4 * x + 3] *= (T)0.5;
+            }
+            uint32_t* so = reinterpret_cast<uint32_t*>(r + (size_t)icon::kScCoefWords * sizeof(T) + 32);
+            for (int i = 0; i < icon::kCcSlotWords; ++i)
+                so[i] = (uint32_t)cs.patch_slots[(size_t)q * icon::kCcSlotWords + i] * (uint32_t)slot_bytes;
         }
     } catch (const std::bad_alloc&) {
         return fail(ICON_ENOMEM, "out of host memory while building the column-cache schedule");

@@ -130,7 +130,7 @@ void simulate_cta(const ScTables& sc, int64_t pb, int64_t pe, int n_slots, int s
         for (int64_t p = p0; p < p1; ++p) {
             uint16_t* o = patch_slots + (size_t)p * kCcSlotWords;
             for (int i = 0; i < kRefs; ++i)
-                o[i] = (uint16_t)(step_slot[key_of(i, sc.ids[(size_t)p * kScIdWords + i])] * slot_units);
+                o[i] = (uint16_t)step_slot[key_of(i, sc.ids[(size_t)p * kScIdWords + i])];
             for (int i = kRefs; i < kCcSlotWords; ++i) o[i] = 0;
         }
     }
@@ -144,7 +144,7 @@ std::string build_cc_schedule(const ScTables& sc, int n_ctas, int n_slots, int s
     const int64_t np = sc.n_patches;
     if (np <= 0 || n_ctas <= 0) return "cc schedule: empty grid";
     if (n_slots < kRefs) return "cc schedule: fewer shared-memory slots than one patch needs";
-    if ((int64_t)n_slots * slot_units > 65535) return "cc schedule: slot offsets do not fit 16 bits";
+    if (n_slots > 65535) return "cc schedule: slot indices do not fit 16 bits";
     const int64_t max_ctas = (np + kCcGroup - 1) / kCcGroup;
     if (n_ctas > max_ctas) n_ctas = (int)max_ctas;
     out = CcSchedule();

@@ -41,9 +41,12 @@ inline const CcShape& cc_shape(int i) { return kCcShapes[i >= 0 && i < kCcNumSha
 constexpr int kCcBarrierBytes = 256;    // the mbarriers
 constexpr int kCcOutCols = 3;            // ddt_vn staging columns per consumer warp (one store batch)
 // a patch record on the device = kScCoefWords coefficients (T), then 8 int32 (user ids of the six
-// owned edges i0 i1 i2 b0 b2 b4, 2 pad), then kCcSlotWords uint16 slot offsets
-constexpr int kCcRecordTail = 32 + 96;
-constexpr int kCcSlotWords = 48;     // uint16 per patch: 43 slot offsets (order of sc_tables.hpp id slots) + pad
+// owned edges i0 i1 i2 b0 b2 b4, 2 pad), then kCcSlotWords uint32 byte offsets of the slots; c_lin is
+// stored halved there (the kernel forms w(k) + w(k+1) = 2 w_f(k))
+constexpr int kCcSlotWords = 48;     // per patch: 43 slots (order of sc_tables.hpp id slots) + pad
+constexpr int kCcRecordTail = 32 + 4 * kCcSlotWords;
+// lanes past the end of a column read up to 3 * 32 levels * 8 bytes beyond their slot: readable pad after the last slot
+constexpr int kCcSlotTailPad = 768;
 
 struct CcStep {                      // 16 bytes
     uint32_t load_begin;             // first entry of this step in `loads`
@@ -63,12 +66,12 @@ struct CcSchedule {
     int n_ctas = 0, n_slots = 0;
     int group = 0;                           // patches per step
     int depth = 0;                           // steps a load may run ahead of its readers (pipeline depth)
-    int slot_units = 0;                      // slot size in 16-byte units (slot offsets are stored in these units)
+    int slot_units = 0;                      // slot size in 16-byte units
     std::vector<int64_t> cta_patch_begin;    // [n_ctas + 1]
     std::vector<int64_t> cta_step_begin;     // [n_ctas + 1]
     std::vector<CcStep> steps;
     std::vector<CcLoad> loads;
-    std::vector<uint16_t> patch_slots;       // [n_patches][kCcSlotWords], slot * slot_units
+    std::vector<uint16_t> patch_slots;       // [n_patches][kCcSlotWords], slot index
     // statistics (icon_grid_worklist_stats, tests)
     int64_t n_sync_steps = 0, n_vn_loads = 0, n_w_loads = 0;
 };

@@ -167,20 +167,15 @@ __device__ __forceinline__ void ld_coef(const T* __restrict__ p, T (&out)[N]) {
         for (int j = 0; j < per; ++j) out[i * per + j] = tmp[j];
     }
 }
-// N slot offsets (uint16, units of 16 bytes) -> byte offsets
+// N slot byte offsets (uint32) from the record
 template <int N>
-__device__ __forceinline__ void ld_slots(const uint16_t* __restrict__ p, uint32_t (&out)[N]) {
-    static_assert(N % 8 == 0, "slot group must be a multiple of 16 bytes");
+__device__ __forceinline__ void ld_slots(const uint32_t* __restrict__ p, uint32_t (&out)[N]) {
+    static_assert(N % 4 == 0, "slot group must be a multiple of 16 bytes");
     const int4* q = reinterpret_cast<const int4*>(p);
 #pragma unroll
-    for (int i = 0; i < N / 8; ++i) {
+    for (int i = 0; i < N / 4; ++i) {
         int4 v = q[i];
-        const uint32_t w[4] = {(uint32_t)v.x, (uint32_t)v.y, (uint32_t)v.z, (uint32_t)v.w};
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            out[8 * i + 2 * j] = (w[j] & 0xffffu) << 4;
-            out[8 * i + 2 * j + 1] = (w[j] >> 16) << 4;
-        }
+        out[4 * i] = (uint32_t)v.x; out[4 * i + 1] = (uint32_t)v.y; out[4 * i + 2] = (uint32_t)v.z; out[4 * i + 3] = (uint32_t)v.w;
     }
 }
 
@@ -285,11 +280,10 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
     const int grp = warp / G, wi = warp % G;
     // per-lane level coefficients of the vertical term (reading P-14): levels L*lane + l
     T cA[L], cB[L], cC[L];
-    bool po[L], pw[L];       // this lane's levels that exist in a vn / ddt_vn column and in a w column
+    bool po[L];              // this lane's levels that exist in a vn / ddt_vn column
     FORL {
         const int k = L * lane + l;
         po[l] = k < nlev;
-        pw[l] = k <= nlev;
         cA[l] = po[l] ? __ldg(abc + k) : (T)0;
         cB[l] = po[l] ? __ldg(abc + nlev + k) : (T)0;
         cC[l] = po[l] ? __ldg(abc + 2 * nlev + k) : (T)0;
@@ -298,6 +292,9 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
     const int bulk_out = (nlev * (int)sizeof(T)) & ~15;       // bytes of a ddt_vn column that leave by bulk store
     const uint64_t cs = (uint64_t)ldk * sizeof(T);
     const uint32_t lane_off = (uint32_t)(L * lane * (int)sizeof(T));
+    const unsigned char* my_slots = slot_base + lane_off;
+    bool below_missing[L];   // level k+1 does not exist (k = nlev-1) or belongs to a lane past the column end
+    FORL below_missing[l] = L * lane + l + 1 >= nlev;
     const uint64_t pol_first = l2_policy_evict_first();
     const bool hint_out = hints & 1;
 
@@ -308,24 +305,28 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
             const unsigned char* rec = rec_base + ((s % D) * G + wi) * REC;
             const T* cf = reinterpret_cast<const T*>(rec);
             const int32_t* oid = reinterpret_cast<const int32_t*>(rec + kScCoefWords * sizeof(T));
-            const uint16_t* sl = reinterpret_cast<const uint16_t*>(rec + kScCoefWords * sizeof(T) + 32);
+            const uint32_t* sl = reinterpret_cast<const uint32_t*>(rec + kScCoefWords * sizeof(T) + 32);
 
+            // Every lane reads its natural levels L*lane .. L*lane+L-1, whether they exist or not: the
+            // stride-L pattern is conflict free as a whole, lanes past the column end pick up stale
+            // bytes of the slot (or of the next one) that only ever reach outputs through the
+            // level-below neighbour of the last level, which VD masks.
             auto LD = [&](uint32_t off) {
-                const T* q = reinterpret_cast<const T*>(slot_base + off + lane_off);
+                const T* q = reinterpret_cast<const T*>(my_slots + off);
                 C c;
-                FORL c.v[l] = po[l] ? q[l] : (T)0;
+                FORL c.v[l] = q[l];
                 return c;
             };
-            auto WF = [&](uint32_t off) {       // w_f(k) = (w(k) + w(k+1)) / 2 (S6)
-                const T* q = reinterpret_cast<const T*>(slot_base + off + lane_off);
-                C c;
-                FORL c.v[l] = pw[l] ? q[l] : (T)0;
-                C dn = level_down(c);
-                FORL c.v[l] = (T)0.5 * (c.v[l] + dn.v[l]);
-                return c;
+            auto WS = [&](uint32_t off) {       // w(k) + w(k+1) = 2 w_f(k) (S6); the 1/2 is folded into c_lin
+                const C c = LD(off);
+                const C dn = level_down(c);
+                C o;
+                FORL o.v[l] = c.v[l] + dn.v[l];
+                return o;
             };
             auto VD = [&](const C& x) {         // (vn_ie(k) - vn_ie(k+1)) / dz_k, reading P-14 folded into A, B, C
                 C up = level_up(x), dn = level_down(x), o;
+                FORL if (below_missing[l]) dn.v[l] = (T)0;      // C_k = 0 there, but the stale value may be NaN
                 FORL o.v[l] = cA[l] * up.v[l] + cB[l] * x.v[l] + cC[l] * dn.v[l];
                 return o;
             };
@@ -464,9 +465,9 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
             // ---- cell-centre w (S6); these are the last reads of the slots -----------------------
             C wf[4], wx[3];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) wf[j] = WF(sX[12 + j]);
+            for (int j = 0; j < 4; ++j) wf[j] = WS(sX[12 + j]);
 #pragma unroll
-            for (int x = 0; x < 3; ++x) wx[x] = WF(sX[16 + x]);
+            for (int x = 0; x < 3; ++x) wx[x] = WS(sX[16 + x]);
             int32_t ido[8];
             {
                 const int4 a = reinterpret_cast<const int4*>(oid)[0], b = reinterpret_cast<const int4*>(oid)[1];
@@ -488,7 +489,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
                     const C& wl = wf[j];
                     const C& wh = h == 0 ? wf[3] : wx[j];
                     const T* e4 = ec + 4 * x;
-                    FORL o[j].v[l] = -(H[x].v[l] + (e4[2] * wl.v[l] + e4[3] * wh.v[l]) * Dv.v[l]);
+                    FORL o[j].v[l] = -H[x].v[l] - (e4[2] * wl.v[l] + e4[3] * wh.v[l]) * Dv.v[l];
                 }
                 ST3(ido + 3 * h, o);
             }
@@ -513,7 +514,7 @@ static size_t cc_fixed_smem(const CcShape& sh, int nlev) {
 
 template <class T>
 int cc_max_slots(int shape, int nlev, int smem_optin) {
-    const long avail = (long)smem_optin - (long)cc_fixed_smem<T>(cc_shape(shape), nlev);
+    const long avail = (long)smem_optin - (long)cc_fixed_smem<T>(cc_shape(shape), nlev) - kCcSlotTailPad;
     if (avail <= 0) return 0;
     return (int)(avail / cc_slot_bytes<T>(nlev));
 }
@@ -554,7 +555,7 @@ int launch_tendencies_cc(const icon_grid& g, const DevCcTables<T>& p, int nlev, 
     d.steps = p.steps; d.loads = p.loads; d.records = p.records;
     d.cta_patch_begin = p.cta_patch_begin; d.cta_step_begin = p.cta_step_begin;
     d.n_slots = p.n_slots; d.slot_bytes = p.slot_bytes;
-    const size_t smem = cc_fixed_smem<T>(cc_shape(p.shape), nlev) + (size_t)p.n_slots * p.slot_bytes;
+    const size_t smem = cc_fixed_smem<T>(cc_shape(p.shape), nlev) + (size_t)p.n_slots * p.slot_bytes + kCcSlotTailPad;
     const int L = cc_levels_per_lane(nlev);
     cudaError_t err;
 #define CC_CASE(i, W, G, D)                                                                                        \
