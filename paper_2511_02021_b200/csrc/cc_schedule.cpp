@@ -103,7 +103,7 @@ void simulate_cta(const ScTables& sc, int64_t pb, int64_t pe, int n_slots, int s
         st.n_vn = st.n_w = 0;
         st.n_patches = (uint16_t)(std::min(pe, pb + (s + 1) * kCcGroup) - (pb + s * kCcGroup));
         st.depth = (uint16_t)depth;
-        st.pad = 0;
+        st.ahead_begin = 0;
         for (int kind = 0; kind < 2; ++kind)
             for (size_t m = 0; m < miss.size(); ++m) {
                 const uint64_t k = ks[miss[m]];
@@ -186,6 +186,15 @@ std::string build_cc_schedule(const ScTables& sc, int n_ctas, int n_slots, int s
         out.n_w_loads += res[(size_t)b].n_w;
         res[(size_t)b] = CtaResult();
     }
+    for (int b = 0; b < n_ctas; ++b) {
+        const int64_t s0 = out.cta_step_begin[(size_t)b], s1 = out.cta_step_begin[(size_t)b + 1];
+        for (int64_t i = s0; i < s1; ++i)
+            out.steps[(size_t)i].ahead_begin = out.steps[(size_t)std::min(i + kCcAhead, s1 - 1)].load_begin;
+    }
+    // every producer lane may read one entry of a step's first round without a bounds check
+    CcLoad zero;
+    zero.id = 0; zero.slot = 0; zero.kind = 0;
+    out.loads.insert(out.loads.end(), (size_t)32 * kCcProducers, zero);
     return std::string();
 }
 

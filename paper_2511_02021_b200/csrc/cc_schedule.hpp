@@ -28,10 +28,11 @@ namespace icon {
 // kCcProducers producer warps (one warpgroup) are added to `warps`; the CTA is launched with
 // 168 registers per thread and re-balances them with setmaxnreg: producers keep
 // kCcProducerRegs, consumers grow to kCcConsumerRegs
-// ((4 * 40 + 8 * 232) * 32 = 64512 <= 65536 registers of the SM).
+// (the pool is what the launch allocated: 384 * 168 = (4 * 40 + 8 * 232) * 32 = 64512 registers).
 constexpr int kCcProducers = 4;
 constexpr int kCcProducerRegs = 40;
 constexpr int kCcConsumerRegs = 232;
+constexpr int kCcAhead = 3;              // steps the producers read the schedule ahead; `loads` is padded for it
 struct CcShape {
     int warps, group, depth;
 };
@@ -53,7 +54,7 @@ struct CcStep {                      // 16 bytes
     uint16_t n_vn, n_w;              // vn columns first, then w columns
     uint16_t n_patches;              // 1..group
     uint16_t depth;                  // the loads may be issued once step s-depth has drained (1..schedule depth)
-    uint32_t pad;
+    uint32_t ahead_begin;            // load_begin of step s + kCcAhead of the same CTA (the producers' prefetch)
 };
 
 struct CcLoad {                      // 8 bytes

@@ -17,11 +17,17 @@
 //   * ddt_vn columns are assembled in shared memory and leave with a bulk store, so the strided
 //     register layout never turns into uncoalesced global stores.
 //
-// Synchronisation: ring of D stages, full[s % D] (producer arms it with the byte count of step s,
-// the copies complete it) and done[s % D] (one arrival per consumer warp of the step's group). The
-// schedule guarantees that the loads of step s only overwrite slots last read in a step <= s-depth
-// (depth stored per step), and the producer issues them once those steps have drained.
+// Synchronisation: ring of NB barrier pairs, full[s % NB] (one arrival per producer warp, the first
+// one arms it with the byte count of step s, the copies complete it) and done[s % NB] (one arrival per
+// consumer warp of the step's group). The schedule guarantees that the loads of step s only overwrite
+// slots last read in a step <= s-depth (depth <= D stored per step), and the producers issue them once
+// those steps have drained. NB >= D is a multiple of the number of consumer groups, so the steps s and
+// s-NB that share a barrier belong to the same group: a warp never waits on a barrier whose previous
+// phase is still open (a parity wait would fall through), and since every producer warp arrives on
+// every step none of them can fall a whole ring behind either.
 #include <cuda_pipeline.h>
+
+#include <cstdio>
 
 #include "../../include/icon_dycore.h"
 #include "kernels.cuh"
@@ -44,7 +50,24 @@ __device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t byt
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+#ifdef CC_DEBUG
+// debug build: a wait that does not end reports where it hangs and traps
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity, int what = 0, int step = 0) {
+    for (long it = 0;; ++it) {
+        uint32_t ok;
+        asm volatile(
+            "{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}\n"
+            : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+        if (ok) return;
+        if (it > (1l << 22)) {
+            if ((threadIdx.x & 31) == 0)
+                printf("cc hang: block %d warp %d what %d step %d bar %u parity %u\n", blockIdx.x, threadIdx.x >> 5, what, step, bar, parity);
+            __trap();
+        }
+    }
+}
+#else
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity, int = 0, int = 0) {
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
@@ -55,6 +78,7 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
         "DONE_%=:\n"
         "}\n" ::"r"(bar), "r"(parity) : "memory");
 }
+#endif
 // global -> shared, completion counted in bytes on `bar`
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
@@ -200,15 +224,17 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
     unsigned char* slot_base = out_base + W * kCcOutCols * out_bytes;
     const uint32_t bar0 = smem_u32(bars);
     auto full_bar = [&](int i) { return bar0 + 8u * (uint32_t)i; };
-    auto done_bar = [&](int i) { return bar0 + 8u * (uint32_t)(D + i); };
+    constexpr int NB = NGRP * ((D + NGRP - 1) / NGRP);
+    static_assert(2 * NB * 8 <= kCcBarrierBytes, "barrier area too small");
+    auto done_bar = [&](int i) { return bar0 + 8u * (uint32_t)(NB + i); };
 
     const int64_t pb = d.cta_patch_begin[blockIdx.x], pe = d.cta_patch_begin[blockIdx.x + 1];
     const int64_t sb = d.cta_step_begin[blockIdx.x];
     const int n_steps = (int)(d.cta_step_begin[blockIdx.x + 1] - sb);
 
     if (threadIdx.x == 0) {
-        for (int i = 0; i < D; ++i) {
-            mbar_init(full_bar(i), 1);
+        for (int i = 0; i < NB; ++i) {
+            mbar_init(full_bar(i), kCcProducers);
             mbar_init(done_bar(i), G);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -231,46 +257,59 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
         const uint2* lraw = reinterpret_cast<const uint2*>(d.loads);
         const int mine = kCcProducers * lane + pw;          // this lane's entry of each round of 32 * kCcProducers
         int drained = 0;
-        // headers two steps ahead and this lane's first list entry one step ahead, so that the only
-        // latency on the issue path is the wait for the stage itself
-        auto hdr = [&](int s) {
-            CcStep z;
-            z.load_begin = 0; z.n_vn = 0; z.n_w = 0; z.n_patches = 0; z.depth = 1; z.pad = 0;
-            return s < n_steps ? d.steps[sb + s] : z;
-        };
-        auto entry = [&](const CcStep& st, int i) {
-            return i < st.n_vn + st.n_w ? __ldg(lraw + st.load_begin + i) : make_uint2(0u, 0u);
-        };
-        CcStep st = hdr(0), st1 = hdr(1);
-        uint2 e0 = entry(st, mine);
-        for (int s = 0; s < n_steps; ++s) {
-            const CcStep st2 = hdr(s + 2);
-            const uint2 e1 = entry(st1, mine);
-            const int n_loads = st.n_vn + st.n_w;
-            while (drained < s - (int)st.depth + 1) {
-                mbar_wait(done_bar(drained % D), (uint32_t)((drained / D) & 1));
-                ++drained;
+        // The schedule is read kCcAhead steps ahead through a register ring (the step loop is unrolled
+        // by kCcAhead so that the ring is statically indexed): header s+kCcAhead, and this lane's first
+        // list entry of step s+kCcAhead, whose position header s already names (CcStep::ahead_begin).
+        // Raw 16-/8-byte loads: no field is touched before its step, so nothing waits on them early.
+        const uint4* hraw = reinterpret_cast<const uint4*>(d.steps + sb);
+        uint4 h[kCcAhead];
+        uint2 e[kCcAhead];
+#pragma unroll
+        for (int u = 0; u < kCcAhead; ++u) {
+            h[u] = u < n_steps ? __ldg(hraw + u) : make_uint4(0u, 0u, 0u, 0u);
+            e[u] = make_uint2(0u, 0u);
+        }
+#pragma unroll
+        for (int u = 0; u < kCcAhead; ++u) e[u] = __ldg(lraw + h[u].x + mine);      // the list is padded: always readable
+        for (int s0 = 0; s0 < n_steps; s0 += kCcAhead) {
+#pragma unroll
+            for (int u = 0; u < kCcAhead; ++u) {
+                const int s = s0 + u;
+                if (s < n_steps) {
+                    // CcStep: load_begin | n_vn n_w | n_patches depth | ahead_begin
+                    const uint32_t load_begin = h[u].x, n_vn = h[u].y & 0xffffu, n_w = h[u].y >> 16;
+                    const uint32_t n_pat = h[u].z & 0xffffu, depth = h[u].z >> 16, ahead_begin = h[u].w;
+                    const uint2 e0 = e[u];
+                    if (s + kCcAhead < n_steps) {
+                        h[u] = __ldg(hraw + s + kCcAhead);
+                        e[u] = __ldg(lraw + ahead_begin + mine);
+                    }
+                    const int n_loads = (int)(n_vn + n_w);
+                    while (drained < s - (int)depth + 1) {
+                        mbar_wait(done_bar(drained % NB), (uint32_t)((drained / NB) & 1), 1, s);
+                        ++drained;
+                    }
+                    const uint32_t fb = full_bar(s % NB);
+                    if (pw == 0 && lane == 0) mbar_arrive_expect_tx(fb, n_vn * bv + n_w * bw + n_pat * (uint32_t)REC);
+                    if (pw != 0 && lane == 0) mbar_arrive(fb);
+                    if (pw == kCcProducers - 1 && lane < (int)n_pat) {
+                        const int64_t p = pb + (int64_t)s * G + lane;
+                        const uint32_t dst = rec0 + (uint32_t)(((s % D) * G + lane) * REC);
+                        if (hint_rec) bulk_g2s_hint(dst, d.records + p * REC, (uint32_t)REC, fb, pol_first);
+                        else bulk_g2s(dst, d.records + p * REC, (uint32_t)REC, fb);
+                    }
+                    for (int base = 0; base + mine < n_loads; base += 32 * kCcProducers) {
+                        const uint2 q = base == 0 ? e0 : __ldg(lraw + load_begin + base + mine);
+                        // CcLoad: id | slot (low 16 bits) kind (high 16 bits)
+                        const uint32_t slot = q.y & 0xffffu, kind = q.y >> 16;
+                        const unsigned char* src = kind ? reinterpret_cast<const unsigned char*>(w) + (uint64_t)q.x * cs_w
+                                                        : reinterpret_cast<const unsigned char*>(vn) + (uint64_t)q.x * cs;
+                        const uint32_t dst = slot0 + slot * (uint32_t)d.slot_bytes;
+                        if (hint_col) bulk_g2s_hint(dst, src, kind ? bw : bv, fb, pol_last);
+                        else bulk_g2s(dst, src, kind ? bw : bv, fb);
+                    }
+                }
             }
-            const uint32_t fb = full_bar(s % D);
-            if (pw == 0 && lane == 0)
-                mbar_arrive_expect_tx(fb, st.n_vn * bv + st.n_w * bw + st.n_patches * (uint32_t)REC);
-            if (pw == kCcProducers - 1 && lane < (int)st.n_patches) {
-                const int64_t p = pb + (int64_t)s * G + lane;
-                const uint32_t dst = rec0 + (uint32_t)(((s % D) * G + lane) * REC);
-                if (hint_rec) bulk_g2s_hint(dst, d.records + p * REC, (uint32_t)REC, fb, pol_first);
-                else bulk_g2s(dst, d.records + p * REC, (uint32_t)REC, fb);
-            }
-            for (int base = 0; base + mine < n_loads; base += 32 * kCcProducers) {
-                const uint2 e = base == 0 ? e0 : entry(st, base + mine);
-                // CcLoad: id | slot (low 16 bits) kind (high 16 bits)
-                const uint32_t slot = e.y & 0xffffu, kind = e.y >> 16;
-                const unsigned char* src = kind ? reinterpret_cast<const unsigned char*>(w) + (uint64_t)e.x * cs_w
-                                                : reinterpret_cast<const unsigned char*>(vn) + (uint64_t)e.x * cs;
-                const uint32_t dst = slot0 + slot * (uint32_t)d.slot_bytes;
-                if (hint_col) bulk_g2s_hint(dst, src, kind ? bw : bv, fb, pol_last);
-                else bulk_g2s(dst, src, kind ? bw : bv, fb);
-            }
-            st = st1; st1 = st2; e0 = e1;
         }
         return;
     }
@@ -300,7 +339,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
 
     for (int s = grp; s < n_steps; s += NGRP) {
         const int64_t p = pb + (int64_t)s * G + wi;
-        mbar_wait(full_bar(s % D), (uint32_t)((s / D) & 1));
+        mbar_wait(full_bar(s % NB), (uint32_t)((s / NB) & 1), 2, s);
         if (p < pe) {
             const unsigned char* rec = rec_base + ((s % D) * G + wi) * REC;
             const T* cf = reinterpret_cast<const T*>(rec);
@@ -475,7 +514,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
             }
             // everything this patch needs from the slots and its record is in registers: release the stage
             __syncwarp();
-            if (lane == 0) mbar_arrive(done_bar(s % D));
+            if (lane == 0) mbar_arrive(done_bar(s % NB));
 
             // ---- vertical part and the tendency (S6, S7) -----------------------------------------
             static_assert(kCcOutCols == 3, "six owned edges leave in two batches of three");
@@ -495,7 +534,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
             }
         } else {
             __syncwarp();
-            if (lane == 0) mbar_arrive(done_bar(s % D));
+            if (lane == 0) mbar_arrive(done_bar(s % NB));
         }
     }
     if (lane == 0) bulk_wait_all();
