@@ -94,6 +94,8 @@ enum {
                                      depth): 0 = 8/1/10 (default), 1 = 8/2/5, 2 = 8/1/9, 3 = 8/1/11. */
     ICON_OPT_CC_L2_HINTS = 2,     /* L2 eviction hints of kernel 4, bit mask: 1 = ddt_vn stores evict-first,
                                      2 = patch records evict-first, 4 = vn / w columns evict-last. Default 3. */
+    ICON_OPT_CC_MERGE = 3,        /* kernel 4: 1 (default) = columns with consecutive ids arrive as one bulk copy
+                                     when the field's column stride allows it; 0 = one copy per column. */
     ICON_OPT_COUNT
 };
 
@@ -136,6 +138,20 @@ int icon_grid_set_option(icon_grid_t* g, int option, int value);
  * ICON_EUNSUPPORTED if the tables do not describe a 4-child bisection hierarchy.
  */
 int icon_grid_worklist_stats(icon_grid_t* g, int64_t out[8]);
+
+/*
+ * icon_grid_cc_schedule_check -- builds on the host (works on ICON_HOST_ONLY grids) the column-cache
+ * schedule tendency kernel 4 would run for (dtype, nlev, ldk, ldk_w) with the current ICON_OPT_CC_*
+ * options on a device with `n_ctas` SMs and `smem_bytes` of opt-in shared memory per block, replays it
+ * with an independent checker (every patch finds each of its 43 columns in the slot its record names;
+ * no bulk copy overwrites a slot a running step still reads; byte counts match) and reports
+ *   out[0] steps   out[1] steps with reduced run-ahead   out[2] vn columns loaded   out[3] w columns loaded
+ *   out[4] bulk copies   out[5] slots   out[6] slot bytes   out[7] CTAs.
+ * ICON_EUNSUPPORTED: nlev or the memory size cannot hold the kernel; ICON_EINVAL: the check failed
+ * (icon_last_error names the rule).
+ */
+int icon_grid_cc_schedule_check(icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, int n_ctas, int smem_bytes,
+                                int64_t out[8]);
 
 /*
  * dycore_div_vort -- SURVEY.md 8(a) steps S1, S2 (north_star: "cell divergence from normal winds

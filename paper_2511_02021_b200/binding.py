@@ -20,6 +20,7 @@ ICON_PERMUTE, ICON_LOCALITY_WORKLIST, ICON_HOST_ONLY, ICON_NO_WORKLIST = 1, 2, 4
 ICON_OPT_TENDENCY_KERNEL = 0
 ICON_OPT_CC_SHAPE = 1
 ICON_OPT_CC_L2_HINTS = 2
+ICON_OPT_CC_MERGE = 3
 
 TABLES = ("c2v", "c2e", "e2c", "e2v", "e2e4", "v2e", "v2c", "v_deg", "c_os", "v_os",
           "vert_xyz", "cell_xyz", "edge_xyz", "edge_normal", "l_e", "d_e", "inv_d_e", "f_e", "c_lin", "rbf",
@@ -28,7 +29,7 @@ TABLE_ID = {n: i for i, n in enumerate(TABLES)}
 
 # every symbol include/icon_dycore.h declares
 EXPORTS = ("icon_grid_create", "icon_grid_destroy", "icon_grid_counts", "icon_grid_table_host",
-           "icon_grid_table_device", "icon_grid_set_option", "icon_grid_worklist_stats", "dycore_div_vort", "dycore_velocity_tendencies",
+           "icon_grid_table_device", "icon_grid_set_option", "icon_grid_worklist_stats", "icon_grid_cc_schedule_check", "dycore_div_vort", "dycore_velocity_tendencies",
            "dycore_step_host", "icon_grid_launch_count", "icon_last_error")
 
 
@@ -65,6 +66,8 @@ def load_library():
     L.icon_grid_set_option.argtypes = [P, ci, ci]
     L.icon_grid_worklist_stats.restype = ci
     L.icon_grid_worklist_stats.argtypes = [P, ctypes.POINTER(i64)]
+    L.icon_grid_cc_schedule_check.restype = ci
+    L.icon_grid_cc_schedule_check.argtypes = [P, ci, ci, ci, ci, ci, ci, ctypes.POINTER(i64)]
     L.icon_grid_launch_count.restype = i64
     L.icon_grid_launch_count.argtypes = [P]
     L.dycore_div_vort.restype = ci
@@ -153,6 +156,13 @@ class IconGrid:
         out = (ctypes.c_int64 * 8)()
         _check(self._L.icon_grid_worklist_stats(self._h, out))
         keys = ("patches", "tiles", "halo_tasks", "vertex_tasks", "max_halo", "max_vert", "mid_stored", "corner_stored")
+        return dict(zip(keys, [int(x) for x in out]))
+
+    def cc_schedule_check(self, dtype, nlev, ldk, ldk_w, n_ctas=148, smem_bytes=232448):
+        """build + independently validate the column-cache schedule of tendency kernel 4 (icon_grid_cc_schedule_check)"""
+        out = (ctypes.c_int64 * 8)()
+        _check(self._L.icon_grid_cc_schedule_check(self._h, dtype, nlev, ldk, ldk_w, n_ctas, smem_bytes, out))
+        keys = ("steps", "reduced_steps", "vn_columns", "w_columns", "copies", "slots", "slot_bytes", "ctas")
         return dict(zip(keys, [int(x) for x in out]))
 
     @property

@@ -203,21 +203,41 @@ int ensure_sc_host(icon_grid* g) {
     return ICON_OK;
 }
 
+// A slot as large as the caller's column stride lets runs of consecutive columns arrive as one bulk
+// copy (the copy engine, not HBM, limits small copies); taken when it costs < 128 bytes per slot.
+template <class T>
+icon::CcGeometry cc_geometry(int nlev, int64_t ldk, int64_t ldk_w, bool merge) {
+    icon::CcGeometry geom;
+    geom.col_bytes[0] = (nlev * (int)sizeof(T) + 15) & ~15;
+    geom.col_bytes[1] = icon::cc_slot_bytes<T>(nlev);
+    geom.stride_bytes[0] = (int)(ldk * (int64_t)sizeof(T));
+    geom.stride_bytes[1] = (int)(ldk_w * (int64_t)sizeof(T));
+    geom.slot_bytes = geom.col_bytes[1];
+    if (merge && geom.stride_bytes[0] >= geom.col_bytes[1] && geom.stride_bytes[0] < geom.col_bytes[1] + 128)
+        geom.slot_bytes = geom.stride_bytes[0];
+    if (!merge) geom.stride_bytes[0] = geom.stride_bytes[1] = 0;      // no stride equals the slot size: runs of 1
+    return geom;
+}
+
 // Column-cache schedule + patch records for (T, nlev): built on the host once, uploaded once.
 // Returns ICON_OK with p.unsupported set when this (T, nlev) cannot use the kernel (the caller
 // then uses the self-contained patch kernel).
 template <class T>
-int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev) {
+int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev, int64_t ldk, int64_t ldk_w) {
     const int shape = g->options[ICON_OPT_CC_SHAPE];
-    if (p.nlev == nlev && p.shape == shape && (p.ready || p.unsupported)) return ICON_OK;
+    const bool merge = g->options[ICON_OPT_CC_MERGE] != 0;
+    if (p.nlev == nlev && p.shape == shape && p.ldk == ldk && p.ldk_w == ldk_w && p.merge == merge && (p.ready || p.unsupported))
+        return ICON_OK;
     dev_release(g, p.steps); dev_release(g, p.loads); dev_release(g, p.records);
     dev_release(g, p.cta_patch_begin); dev_release(g, p.cta_step_begin);
     p = icon::DevCcTables<T>();
     p.nlev = nlev;
     p.shape = shape;
+    p.ldk = ldk; p.ldk_w = ldk_w; p.merge = merge;
     const icon::CcShape& sh = icon::cc_shape(shape);
-    const int n_slots_max = icon::cc_max_slots<T>(shape, nlev, g->smem_optin);
-    const int slot_bytes = icon::cc_slot_bytes<T>(nlev);
+    const icon::CcGeometry geom = cc_geometry<T>(nlev, ldk, ldk_w, merge);
+    const int slot_bytes = geom.slot_bytes;
+    const int n_slots_max = icon::cc_max_slots<T>(shape, nlev, slot_bytes, g->smem_optin);
     if (icon::cc_levels_per_lane(nlev) == 0 || nlev * (int)sizeof(T) < 16 || n_slots_max < icon::kScIdWords) {
         p.unsupported = true;
         return ICON_OK;
@@ -230,7 +250,7 @@ int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev) {
     std::vector<unsigned char> rec;
     const size_t rb = (size_t)icon::kScCoefWords * sizeof(T) + icon::kCcRecordTail;
     try {
-        std::string err = icon::build_cc_schedule(sc, g->num_sms, n_slots, slot_bytes / 16, sh.group, sh.depth, cs);
+        std::string err = icon::build_cc_schedule(sc, g->num_sms, n_slots, geom, sh.group, sh.depth, cs);
         if (!err.empty()) {
             p.unsupported = true;
             return ICON_OK;
@@ -254,6 +274,7 @@ int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev) {
             uint32_t* so = reinterpret_cast<uint32_t*>(r + (size_t)icon::kScCoefWords * sizeof(T) + 32);
             for (int i = 0; i < icon::kCcSlotWords; ++i)
                 so[i] = (uint32_t)cs.patch_slots[(size_t)q * icon::kCcSlotWords + i] * (uint32_t)slot_bytes;
+            so[icon::kCcMaskWord] = cs.patch_slots[(size_t)q * icon::kCcSlotWords + icon::kCcMaskWord];
         }
     } catch (const std::bad_alloc&) {
         return fail(ICON_ENOMEM, "out of host memory while building the column-cache schedule");
@@ -264,7 +285,7 @@ int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev) {
     if ((rc = upload_vec(g, cs.cta_patch_begin, &p.cta_patch_begin))) return rc;
     if ((rc = upload_vec(g, cs.cta_step_begin, &p.cta_step_begin))) return rc;
     p.n_ctas = cs.n_ctas; p.n_slots = cs.n_slots; p.slot_bytes = slot_bytes;
-    p.stats[0] = (int64_t)cs.steps.size(); p.stats[1] = cs.n_sync_steps; p.stats[2] = cs.n_vn_loads; p.stats[3] = cs.n_w_loads;
+    p.stats[0] = (int64_t)cs.steps.size(); p.stats[1] = cs.n_sync_steps; p.stats[2] = cs.n_vn_loads; p.stats[3] = cs.n_w_loads; p.stats[4] = cs.n_copies;
     p.ready = true;
     return ICON_OK;
 }
@@ -385,7 +406,7 @@ int tendencies_impl(icon_grid* g, icon::DevCoeffs<T>& c, icon::DevPatchTables<T>
     int n;
     int variant = g->options[ICON_OPT_TENDENCY_KERNEL];
     if (variant == 4 && !want_opt) {
-        if ((rc = ensure_cc_tables(g, ct, nlev))) return rc;
+        if ((rc = ensure_cc_tables(g, ct, nlev, ldk, ldk_w))) return rc;
         if (ct.unsupported) variant = 3;      // level count / dtype the column cache cannot hold
     }
     if (variant == 4 && !want_opt) {
@@ -476,6 +497,7 @@ int icon_grid_create(int bisections_k, uint64_t seed, unsigned flags, icon_grid_
     g->host_only = (flags & ICON_HOST_ONLY) != 0;
     g->options[ICON_OPT_TENDENCY_KERNEL] = 4;
     g->options[ICON_OPT_CC_L2_HINTS] = 3;
+    g->options[ICON_OPT_CC_MERGE] = 1;
     try {
         std::string err = icon::build_host_grid(bisections_k, seed, (flags & ICON_PERMUTE) != 0, g->host);
         if (!err.empty()) {
@@ -604,6 +626,35 @@ int icon_grid_worklist_stats(icon_grid_t* g, int64_t out[8]) {
     for (int32_t v : h.vert_store) cors += v;
     out[6] = mids;
     out[7] = cors;
+    return ICON_OK;
+}
+
+int icon_grid_cc_schedule_check(icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, int n_ctas, int smem_bytes,
+                                int64_t out[8]) {
+    if (!g || !out) return fail(ICON_EINVAL, "NULL argument");
+    if (dtype != ICON_F64 && dtype != ICON_F32) return fail(ICON_EINVAL, "dtype must be ICON_F64 or ICON_F32");
+    if (nlev < 2 || ldk < nlev || ldk_w < nlev + 1 || n_ctas < 1 || smem_bytes < 1) return fail(ICON_EINVAL, "bad argument");
+    if (icon::cc_levels_per_lane(nlev) == 0) return fail(ICON_EUNSUPPORTED, "nlev not supported by the column-cache kernel");
+    int rc = ensure_sc_host(g);
+    if (rc) return rc;
+    const int shape = g->options[ICON_OPT_CC_SHAPE];
+    const bool merge = g->options[ICON_OPT_CC_MERGE] != 0;
+    const bool f64 = dtype == ICON_F64;
+    const icon::CcGeometry geom = f64 ? cc_geometry<double>(nlev, ldk, ldk_w, merge) : cc_geometry<float>(nlev, ldk, ldk_w, merge);
+    const int n_slots = std::min(65535, f64 ? icon::cc_max_slots<double>(shape, nlev, geom.slot_bytes, smem_bytes)
+                                            : icon::cc_max_slots<float>(shape, nlev, geom.slot_bytes, smem_bytes));
+    icon::CcSchedule cs;
+    try {
+        std::string err = icon::build_cc_schedule(g->sc_host, n_ctas, n_slots, geom, icon::cc_shape(shape).group,
+                                                  icon::cc_shape(shape).depth, cs);
+        if (!err.empty()) return fail(ICON_EUNSUPPORTED, err);
+        err = icon::check_cc_schedule(g->sc_host, cs, g->host.ne, g->host.nc);
+        if (!err.empty()) return fail(ICON_EINVAL, err);
+    } catch (const std::bad_alloc&) {
+        return fail(ICON_ENOMEM, "out of host memory while building the column-cache schedule");
+    }
+    out[0] = (int64_t)cs.steps.size(); out[1] = cs.n_sync_steps; out[2] = cs.n_vn_loads; out[3] = cs.n_w_loads;
+    out[4] = cs.n_copies; out[5] = cs.n_slots; out[6] = geom.slot_bytes; out[7] = cs.n_ctas;
     return ICON_OK;
 }
 

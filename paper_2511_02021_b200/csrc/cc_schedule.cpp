@@ -16,7 +16,7 @@ constexpr int32_t kNever = 0x7fffffff;
 struct CtaResult {
     std::vector<CcStep> steps;
     std::vector<CcLoad> loads;
-    int64_t n_sync = 0, n_vn = 0, n_w = 0;
+    int64_t n_sync = 0, n_vn = 0, n_w = 0, n_copies = 0;
     bool ok = true;
 };
 
@@ -24,8 +24,8 @@ inline uint64_t key_of(int slot_in_patch, int32_t id) {
     return ((uint64_t)(uint32_t)id << 1) | (slot_in_patch >= kFirstCell ? 1u : 0u);
 }
 
-void simulate_cta(const ScTables& sc, int64_t pb, int64_t pe, int n_slots, int slot_units, int kCcGroup, int max_depth,
-                  uint16_t* patch_slots, CtaResult& r) {
+void simulate_cta(const ScTables& sc, int64_t pb, int64_t pe, int n_slots, const CcGeometry& geom, int kCcGroup,
+                  int max_depth, uint16_t* patch_slots, CtaResult& r) {
     const int64_t n_steps = (pe - pb + kCcGroup - 1) / kCcGroup;
     // pass 1: the distinct columns of every step
     std::vector<std::vector<uint64_t>> keys((size_t)n_steps);
@@ -58,6 +58,7 @@ void simulate_cta(const ScTables& sc, int64_t pb, int64_t pe, int n_slots, int s
     resident.reserve((size_t)n_slots * 2);
     std::vector<uint64_t> slot_key((size_t)n_slots, ~0ull);
     std::vector<int32_t> slot_last((size_t)n_slots, -1000), slot_next((size_t)n_slots, kNever);
+    std::vector<int32_t> slot_loaded((size_t)n_slots, -1000);      // the step whose copies filled the slot
     std::vector<int32_t> cand;
     std::vector<size_t> miss;
     std::unordered_map<uint64_t, int32_t> step_slot;     // key -> slot, for this step's patches
@@ -89,68 +90,128 @@ void simulate_cta(const ScTables& sc, int64_t pb, int64_t pe, int n_slots, int s
             r.ok = false;
             return;
         }
-        // Belady: give up the columns whose next use is farthest (empty slots first)
-        std::partial_sort(cand.begin(), cand.begin() + (ptrdiff_t)miss.size(), cand.end(), [&](int32_t a, int32_t b) {
-            const int32_t na = slot_key[(size_t)a] == ~0ull ? kNever : slot_next[(size_t)a];
-            const int32_t nb = slot_key[(size_t)b] == ~0ull ? kNever : slot_next[(size_t)b];
-            if (na != nb) return na > nb;
-            const bool ea = slot_key[(size_t)a] == ~0ull, eb = slot_key[(size_t)b] == ~0ull;
-            if (ea != eb) return ea;
-            return a < b;
+        // The misses, grouped into runs of consecutive column ids of one kind.
+        struct Run { int kind; uint32_t id; int len; size_t first; };   // first = index into `order`
+        std::vector<size_t> order(miss);                                 // indices into ks, by (kind, id)
+        std::sort(order.begin(), order.end(), [&](size_t a, size_t b2) {
+            const uint64_t ka = ks[a], kb = ks[b2];
+            if ((ka & 1) != (kb & 1)) return (ka & 1) < (kb & 1);
+            return (ka >> 1) < (kb >> 1);
         });
+        std::vector<Run> runs;
+        for (size_t m = 0; m < order.size(); ++m) {
+            const int kind = (int)(ks[order[m]] & 1);
+            const uint32_t id = (uint32_t)(ks[order[m]] >> 1);
+            const bool mergeable = geom.stride_bytes[kind] == geom.slot_bytes;
+            if (!runs.empty() && mergeable && runs.back().kind == kind && runs.back().len < kCcMaxRun &&
+                runs.back().id + (uint32_t)runs.back().len == id) {
+                ++runs.back().len;
+            } else {
+                runs.push_back(Run{kind, id, 1, m});
+            }
+        }
+        // Place the runs, longest first: a window of `len` consecutive evictable slots whose
+        // earliest next use is farthest (Belady on the window; empty slots count as never used
+        // again). A run that finds no window is split in two.
+        std::vector<char> evictable((size_t)n_slots, 0);
+        for (int32_t q : cand) evictable[(size_t)q] = 1;
+        auto worth = [&](int32_t q) { return slot_key[(size_t)q] == ~0ull ? kNever : slot_next[(size_t)q]; };
         CcStep st;
         st.load_begin = (uint32_t)r.loads.size();
-        st.n_vn = st.n_w = 0;
-        st.n_patches = (uint16_t)(std::min(pe, pb + (s + 1) * kCcGroup) - (pb + s * kCcGroup));
-        st.depth = (uint16_t)depth;
+        st.n_loads = 0;
+        st.n_patches = (uint8_t)(std::min(pe, pb + (s + 1) * kCcGroup) - (pb + s * kCcGroup));
+        st.depth = (uint8_t)depth;
+        st.tx16 = 0;
         st.ahead_begin = 0;
-        for (int kind = 0; kind < 2; ++kind)
-            for (size_t m = 0; m < miss.size(); ++m) {
-                const uint64_t k = ks[miss[m]];
-                if ((int)(k & 1) != kind) continue;
-                const int32_t q = cand[m];
+        std::vector<Run> work(runs);
+        std::stable_sort(work.begin(), work.end(), [](const Run& a, const Run& b2) { return a.len > b2.len; });
+        for (size_t w = 0; w < work.size(); ++w) {
+            const Run run = work[w];
+            int32_t best = -1, best_worth = -1;
+            int32_t streak = 0;
+            for (int32_t q = 0; q < n_slots; ++q) {
+                streak = evictable[(size_t)q] ? streak + 1 : 0;
+                if (streak >= run.len) {
+                    int32_t wmin = kNever;
+                    for (int32_t t = q - run.len + 1; t <= q; ++t) wmin = std::min(wmin, worth(t));
+                    if (wmin > best_worth) {
+                        best_worth = wmin;
+                        best = q - run.len + 1;
+                    }
+                }
+            }
+            if (best < 0) {
+                if (run.len == 1) {          // cannot happen: |cand| >= |miss|
+                    r.ok = false;
+                    return;
+                }
+                const int h = run.len / 2;
+                work.push_back(Run{run.kind, run.id, h, run.first});
+                work.push_back(Run{run.kind, run.id + (uint32_t)h, run.len - h, run.first + (size_t)h});
+                continue;
+            }
+            for (int t = 0; t < run.len; ++t) {
+                const int32_t q = best + t;
+                const size_t mi = order[run.first + (size_t)t];
+                const uint64_t k = ks[mi];
                 if (slot_key[(size_t)q] != ~0ull) resident.erase(slot_key[(size_t)q]);
                 slot_key[(size_t)q] = k;
                 slot_last[(size_t)q] = (int32_t)s;
-                slot_next[(size_t)q] = nu[miss[m]];
+                slot_next[(size_t)q] = nu[mi];
+                slot_loaded[(size_t)q] = (int32_t)s;
+                evictable[(size_t)q] = 0;
                 resident[k] = q;
                 step_slot[k] = q;
-                CcLoad ld;
-                ld.id = (uint32_t)(k >> 1);
-                ld.slot = (uint16_t)q;
-                ld.kind = (uint16_t)kind;
-                r.loads.push_back(ld);
-                if (kind) ++st.n_w; else ++st.n_vn;
             }
+            const int bytes = (run.len - 1) * geom.stride_bytes[run.kind] + geom.col_bytes[run.kind];
+            CcLoad ld;
+            ld.id = run.id;
+            ld.slot = (uint16_t)best;
+            ld.bytes16_kind = (uint16_t)((bytes / 16) | (run.kind << 15));
+            r.loads.push_back(ld);
+            ++st.n_loads;
+            st.tx16 += (uint32_t)(bytes / 16);
+            if (run.kind) r.n_w += run.len; else r.n_vn += run.len;
+            ++r.n_copies;
+        }
         r.n_sync += sync;
-        r.n_vn += st.n_vn;
-        r.n_w += st.n_w;
         r.steps.push_back(st);
         const int64_t p0 = pb + s * kCcGroup, p1 = std::min(pe, p0 + kCcGroup);
         for (int64_t p = p0; p < p1; ++p) {
             uint16_t* o = patch_slots + (size_t)p * kCcSlotWords;
-            for (int i = 0; i < kRefs; ++i)
-                o[i] = (uint16_t)step_slot[key_of(i, sc.ids[(size_t)p * kScIdWords + i])];
+            // bit r of the mask: a column of this patch was loaded by step s-r, whose copies may still
+            // be in flight when step s starts (copies of different steps complete in any order)
+            uint16_t mask = 0;
+            for (int i = 0; i < kRefs; ++i) {
+                const int32_t q = step_slot[key_of(i, sc.ids[(size_t)p * kScIdWords + i])];
+                o[i] = (uint16_t)q;
+                const int64_t age = s - slot_loaded[(size_t)q];
+                if (age > 0 && age < max_depth) mask |= (uint16_t)(1u << age);
+            }
             for (int i = kRefs; i < kCcSlotWords; ++i) o[i] = 0;
+            o[kCcMaskWord] = mask;
         }
     }
 }
 
 }  // namespace
 
-std::string build_cc_schedule(const ScTables& sc, int n_ctas, int n_slots, int slot_units, int group, int depth,
+std::string build_cc_schedule(const ScTables& sc, int n_ctas, int n_slots, const CcGeometry& geom, int group, int depth,
                               CcSchedule& out) {
     const int kCcGroup = group;
     const int64_t np = sc.n_patches;
     if (np <= 0 || n_ctas <= 0) return "cc schedule: empty grid";
     if (n_slots < kRefs) return "cc schedule: fewer shared-memory slots than one patch needs";
     if (n_slots > 65535) return "cc schedule: slot indices do not fit 16 bits";
+    if (geom.slot_bytes % 16 || geom.col_bytes[0] % 16 || geom.col_bytes[1] % 16 || geom.col_bytes[0] > geom.slot_bytes ||
+        geom.col_bytes[1] > geom.slot_bytes || (kCcMaxRun - 1) * (int64_t)geom.slot_bytes + geom.slot_bytes > 16 * 32767)
+        return "cc schedule: bad column geometry";
     const int64_t max_ctas = (np + kCcGroup - 1) / kCcGroup;
     if (n_ctas > max_ctas) n_ctas = (int)max_ctas;
     out = CcSchedule();
     out.n_ctas = n_ctas;
     out.n_slots = n_slots;
-    out.slot_units = slot_units;
+    out.geom = geom;
     out.group = group;
     out.depth = depth;
     out.cta_patch_begin.resize((size_t)n_ctas + 1);
@@ -162,8 +223,8 @@ std::string build_cc_schedule(const ScTables& sc, int n_ctas, int n_slots, int s
     std::vector<CtaResult> res((size_t)n_ctas);
 #pragma omp parallel for schedule(dynamic, 1)
     for (int b = 0; b < n_ctas; ++b)
-        simulate_cta(sc, out.cta_patch_begin[(size_t)b], out.cta_patch_begin[(size_t)b + 1], n_slots, slot_units,
-                     group, depth, out.patch_slots.data(), res[(size_t)b]);
+        simulate_cta(sc, out.cta_patch_begin[(size_t)b], out.cta_patch_begin[(size_t)b + 1], n_slots, geom, group,
+                     depth, out.patch_slots.data(), res[(size_t)b]);
     out.cta_step_begin.assign((size_t)n_ctas + 1, 0);
     size_t n_loads = 0;
     for (int b = 0; b < n_ctas; ++b) {
@@ -184,6 +245,7 @@ std::string build_cc_schedule(const ScTables& sc, int n_ctas, int n_slots, int s
         out.n_sync_steps += res[(size_t)b].n_sync;
         out.n_vn_loads += res[(size_t)b].n_vn;
         out.n_w_loads += res[(size_t)b].n_w;
+        out.n_copies += res[(size_t)b].n_copies;
         res[(size_t)b] = CtaResult();
     }
     for (int b = 0; b < n_ctas; ++b) {
@@ -193,7 +255,7 @@ std::string build_cc_schedule(const ScTables& sc, int n_ctas, int n_slots, int s
     }
     // every producer lane may read one entry of a step's first round without a bounds check
     CcLoad zero;
-    zero.id = 0; zero.slot = 0; zero.kind = 0;
+    zero.id = 0; zero.slot = 0; zero.bytes16_kind = 0;
     out.loads.insert(out.loads.end(), (size_t)32 * kCcProducers, zero);
     return std::string();
 }

@@ -39,46 +39,63 @@ struct CcShape {
 constexpr int kCcNumShapes = 4;
 constexpr CcShape kCcShapes[kCcNumShapes] = {{8, 1, 10}, {8, 2, 5}, {8, 1, 9}, {8, 1, 11}};
 inline const CcShape& cc_shape(int i) { return kCcShapes[i >= 0 && i < kCcNumShapes ? i : 0]; }
-constexpr int kCcBarrierBytes = 256;    // the mbarriers
+constexpr int kCcBarrierBytes = 512;    // the mbarriers
 constexpr int kCcOutCols = 3;            // ddt_vn staging columns per consumer warp (one store batch)
 // a patch record on the device = kScCoefWords coefficients (T), then 8 int32 (user ids of the six
 // owned edges i0 i1 i2 b0 b2 b4, 2 pad), then kCcSlotWords uint32 byte offsets of the slots; c_lin is
 // stored halved there (the kernel forms w(k) + w(k+1) = 2 w_f(k))
-constexpr int kCcSlotWords = 48;     // per patch: 43 slots (order of sc_tables.hpp id slots) + pad
+constexpr int kCcSlotWords = 48;     // per patch: 43 slots (order of sc_tables.hpp id slots), mask, pad
+constexpr int kCcMaskWord = 43;      // bit r set: one of the 43 columns was loaded by step s-r (0 < r < depth)
 constexpr int kCcRecordTail = 32 + 4 * kCcSlotWords;
 // lanes past the end of a column read up to 3 * 32 levels * 8 bytes beyond their slot: readable pad after the last slot
 constexpr int kCcSlotTailPad = 768;
 
 struct CcStep {                      // 16 bytes
     uint32_t load_begin;             // first entry of this step in `loads`
-    uint16_t n_vn, n_w;              // vn columns first, then w columns
-    uint16_t n_patches;              // 1..group
-    uint16_t depth;                  // the loads may be issued once step s-depth has drained (1..schedule depth)
+    uint16_t n_loads;                // bulk copies of this step (a copy moves a run of 1..kCcMaxRun columns)
+    uint8_t n_patches;               // 1..group
+    uint8_t depth;                   // the loads may be issued once step s-depth has drained (1..schedule depth)
+    uint32_t tx16;                   // bytes / 16 those copies deliver (patch records not included)
     uint32_t ahead_begin;            // load_begin of step s + kCcAhead of the same CTA (the producers' prefetch)
 };
 
-struct CcLoad {                      // 8 bytes
-    uint32_t id;                     // user id of the edge (vn) or cell (w) column
-    uint16_t slot;                   // slot index
-    uint16_t kind;                   // 0 = vn, 1 = w
+struct CcLoad {                      // 8 bytes: one bulk copy
+    uint32_t id;                     // user id of the first edge (vn) or cell (w) column of the run
+    uint16_t slot;                   // first slot; the run fills consecutive slots
+    uint16_t bytes16_kind;           // bit 15: 0 = vn, 1 = w; bits 0..14: bytes / 16 of the copy
 };
+
+// Byte geometry of the columns the schedule is built for. A run of n columns with consecutive ids
+// is one copy of (n-1)*stride + col bytes into n consecutive slots; that needs slot_bytes == stride,
+// so runs longer than 1 are only formed for a kind whose stride equals slot_bytes.
+struct CcGeometry {
+    int slot_bytes;                  // multiple of 16
+    int col_bytes[2];                // bytes copied for one vn / w column (multiple of 16)
+    int stride_bytes[2];             // distance of consecutive vn / w columns in the caller's field
+};
+constexpr int kCcMaxRun = 8;
 
 struct CcSchedule {
     int n_ctas = 0, n_slots = 0;
     int group = 0;                           // patches per step
     int depth = 0;                           // steps a load may run ahead of its readers (pipeline depth)
-    int slot_units = 0;                      // slot size in 16-byte units
+    CcGeometry geom = {0, {0, 0}, {0, 0}};
     std::vector<int64_t> cta_patch_begin;    // [n_ctas + 1]
     std::vector<int64_t> cta_step_begin;     // [n_ctas + 1]
     std::vector<CcStep> steps;
     std::vector<CcLoad> loads;
     std::vector<uint16_t> patch_slots;       // [n_patches][kCcSlotWords], slot index
     // statistics (icon_grid_worklist_stats, tests)
-    int64_t n_sync_steps = 0, n_vn_loads = 0, n_w_loads = 0;
+    int64_t n_sync_steps = 0, n_vn_loads = 0, n_w_loads = 0;   // columns loaded
+    int64_t n_copies = 0;                                      // bulk copies (runs)
 };
 
 // Returns an empty string on success, else an error message (e.g. too few slots for one step).
-std::string build_cc_schedule(const ScTables& sc, int n_ctas, int n_slots, int slot_units, int group, int depth,
+std::string build_cc_schedule(const ScTables& sc, int n_ctas, int n_slots, const CcGeometry& geom, int group, int depth,
                               CcSchedule& out);
+
+// cc_schedule_check.cpp: replays `cs` as the kernel would and checks the guarantees it relies on
+// (independent of the builder). Empty string = valid.
+std::string check_cc_schedule(const ScTables& sc, const CcSchedule& cs, int64_t n_edges, int64_t n_cells);
 
 }  // namespace icon

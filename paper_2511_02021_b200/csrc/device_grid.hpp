@@ -85,9 +85,11 @@ struct DevCcTables {
     int n_ctas = 0, n_slots = 0, slot_bytes = 0;
     int nlev = -1;                 // the level count the slot size was derived from
     int shape = -1;                // index into kCcShapes the schedule was built for
+    int64_t ldk = -1, ldk_w = -1;  // column strides the runs were merged for
+    bool merge = true;             // ICON_OPT_CC_MERGE it was built with
     bool ready = false;
     bool unsupported = false;      // this (T, nlev) cannot use the kernel: callers fall back
-    int64_t stats[4] = {0, 0, 0, 0};   // steps, steps that wait for their predecessor, vn loads, w loads
+    int64_t stats[5] = {0, 0, 0, 0, 0};   // steps, steps with reduced depth, vn columns, w columns, bulk copies
 };
 
 // per-level coefficients of the vertical term (reading P-14), device copy for one z_half

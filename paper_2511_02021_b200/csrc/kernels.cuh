@@ -44,12 +44,12 @@ int launch_tendencies_sc(const icon_grid& g, const DevScTables<T>& p, int nlev, 
 template <class T>
 int launch_tendencies_cc(const icon_grid& g, const DevCcTables<T>& p, int nlev, int64_t ldk, int64_t ldk_w,
                          const T* abc, const T* vn, const T* w, T* ddt_vn, cudaStream_t s);
-// shape helpers of that kernel: levels per lane (0 = nlev not supported), bytes of one slot, and
-// how many slots fit beside the fixed buffers in `smem_optin` bytes of shared memory
+// shape helpers of that kernel: levels per lane (0 = nlev not supported), bytes of one w column
+// (the smallest possible slot), and how many slots of `slot_bytes` fit beside the fixed buffers in `smem_optin` bytes of shared memory
 int cc_levels_per_lane(int nlev);
 template <class T>
 int cc_slot_bytes(int nlev);
 template <class T>
-int cc_max_slots(int shape, int nlev, int smem_optin);
+int cc_max_slots(int shape, int nlev, int slot_bytes, int smem_optin);
 
 }  // namespace icon

@@ -17,14 +17,19 @@
 //   * ddt_vn columns are assembled in shared memory and leave with a bulk store, so the strided
 //     register layout never turns into uncoalesced global stores.
 //
-// Synchronisation: ring of NB barrier pairs, full[s % NB] (one arrival per producer warp, the first
-// one arms it with the byte count of step s, the copies complete it) and done[s % NB] (one arrival per
+// Synchronisation: ring of NB barrier pairs, full[s % NB] (one arrival per producer warp, each
+// announcing the bytes of its share of step s before issuing them; the copies complete it) and done[s % NB] (one arrival per
 // consumer warp of the step's group). The schedule guarantees that the loads of step s only overwrite
 // slots last read in a step <= s-depth (depth <= D stored per step), and the producers issue them once
-// those steps have drained. NB >= D is a multiple of the number of consumer groups, so the steps s and
-// s-NB that share a barrier belong to the same group: a warp never waits on a barrier whose previous
-// phase is still open (a parity wait would fall through), and since every producer warp arrives on
-// every step none of them can fall a whole ring behind either.
+// those steps have drained. Copies of different steps complete in any order, so a patch that reads a
+// column filled by one of the steps s-1 .. s-D+1 (a "hit" on a column still in flight) also waits on
+// that step's full barrier; the record carries the mask.
+// A parity wait is only right while the barrier is in the awaited phase or the one after it. NB is a
+// multiple of the number of consumer groups NGRP (steps s and s-NB belong to the same group, which
+// has consumed s-NB), NB >= NGRP + D (when a group is at step s every step <= s-NGRP-D has drained,
+// so the previous phase of any barrier it waits on is closed) and NB >= 2D-1 (the next phase of a
+// barrier awaited for step s-r cannot open before step s itself has drained). Every producer warp
+// arrives on every step, so none of them can fall a whole ring behind either.
 #include <cuda_pipeline.h>
 
 #include <cstdio>
@@ -224,7 +229,9 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
     unsigned char* slot_base = out_base + W * kCcOutCols * out_bytes;
     const uint32_t bar0 = smem_u32(bars);
     auto full_bar = [&](int i) { return bar0 + 8u * (uint32_t)i; };
-    constexpr int NB = NGRP * ((D + NGRP - 1) / NGRP);
+    // NB >= 2D-1 and >= NGRP+D: see the parity argument in the header comment
+    constexpr int NBmin = (2 * D - 1 > NGRP + D) ? 2 * D - 1 : NGRP + D;
+    constexpr int NB = NGRP * ((NBmin + NGRP - 1) / NGRP);
     static_assert(2 * NB * 8 <= kCcBarrierBytes, "barrier area too small");
     auto done_bar = [&](int i) { return bar0 + 8u * (uint32_t)(NB + i); };
 
@@ -248,8 +255,6 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
         asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kCcProducerRegs));
         // hints: bit 0 = ddt_vn stores evict-first, bit 1 = patch records evict-first, bit 2 = columns evict-last
         const int pw = warp - W;
-        const uint32_t bv = (uint32_t)out_bytes;                                          // vn column bytes
-        const uint32_t bw = (uint32_t)(((nlev + 1) * (int)sizeof(T) + 15) & ~15);         // w column bytes
         const uint64_t cs = (uint64_t)ldk * sizeof(T), cs_w = (uint64_t)ldk_w * sizeof(T);
         const uint32_t slot0 = smem_u32(slot_base), rec0 = smem_u32(rec_base);
         const uint64_t pol_first = l2_policy_evict_first(), pol_last = l2_policy_evict_last();
@@ -276,37 +281,47 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
             for (int u = 0; u < kCcAhead; ++u) {
                 const int s = s0 + u;
                 if (s < n_steps) {
-                    // CcStep: load_begin | n_vn n_w | n_patches depth | ahead_begin
-                    const uint32_t load_begin = h[u].x, n_vn = h[u].y & 0xffffu, n_w = h[u].y >> 16;
-                    const uint32_t n_pat = h[u].z & 0xffffu, depth = h[u].z >> 16, ahead_begin = h[u].w;
+                    // CcStep: load_begin | n_loads n_patches depth | tx16 | ahead_begin
+                    const uint32_t load_begin = h[u].x, n_loads_u = h[u].y & 0xffffu, n_pat = (h[u].y >> 16) & 0xffu;
+                    const uint32_t depth = h[u].y >> 24, ahead_begin = h[u].w;       // h[u].z = tx16, for the checker
                     const uint2 e0 = e[u];
                     if (s + kCcAhead < n_steps) {
                         h[u] = __ldg(hraw + s + kCcAhead);
                         e[u] = __ldg(lraw + ahead_begin + mine);
                     }
-                    const int n_loads = (int)(n_vn + n_w);
+                    const int n_loads = (int)n_loads_u;
                     while (drained < s - (int)depth + 1) {
                         mbar_wait(done_bar(drained % NB), (uint32_t)((drained / NB) & 1), 1, s);
                         ++drained;
                     }
                     const uint32_t fb = full_bar(s % NB);
-                    if (pw == 0 && lane == 0) mbar_arrive_expect_tx(fb, n_vn * bv + n_w * bw + n_pat * (uint32_t)REC);
-                    if (pw != 0 && lane == 0) mbar_arrive(fb);
-                    if (pw == kCcProducers - 1 && lane < (int)n_pat) {
-                        const int64_t p = pb + (int64_t)s * G + lane;
-                        const uint32_t dst = rec0 + (uint32_t)(((s % D) * G + lane) * REC);
-                        if (hint_rec) bulk_g2s_hint(dst, d.records + p * REC, (uint32_t)REC, fb, pol_first);
-                        else bulk_g2s(dst, d.records + p * REC, (uint32_t)REC, fb);
+                    // Every producer warp announces the bytes of its own share before it issues them
+                    // (the transaction count of the barrier never runs negative), then copies.
+                    uint32_t my16 = 0;
+                    for (int base = 0; base + mine < n_loads; base += 32 * kCcProducers) {
+                        const uint2 q = base == 0 ? e0 : __ldg(lraw + load_begin + base + mine);
+                        my16 += (q.y >> 16) & 0x7fffu;
+                    }
+                    my16 = __reduce_add_sync(kFull, my16);
+                    const bool rec_warp = pw == kCcProducers - 1;
+                    if (lane == 0) mbar_arrive_expect_tx(fb, my16 * 16u + (rec_warp ? n_pat * (uint32_t)REC : 0u));
+                    __syncwarp();
+                    if (rec_warp && lane == 0) {
+                        // the records of a step's patches are consecutive in memory and in the ring: one copy
+                        const int64_t p = pb + (int64_t)s * G;
+                        const uint32_t dst = rec0 + (uint32_t)(((s % D) * G) * REC);
+                        if (hint_rec) bulk_g2s_hint(dst, d.records + p * REC, n_pat * (uint32_t)REC, fb, pol_first);
+                        else bulk_g2s(dst, d.records + p * REC, n_pat * (uint32_t)REC, fb);
                     }
                     for (int base = 0; base + mine < n_loads; base += 32 * kCcProducers) {
                         const uint2 q = base == 0 ? e0 : __ldg(lraw + load_begin + base + mine);
-                        // CcLoad: id | slot (low 16 bits) kind (high 16 bits)
-                        const uint32_t slot = q.y & 0xffffu, kind = q.y >> 16;
+                        // CcLoad: id | slot (bits 0..15) bytes/16 (bits 16..30) kind (bit 31)
+                        const uint32_t slot = q.y & 0xffffu, kind = q.y >> 31, bytes = ((q.y >> 16) & 0x7fffu) << 4;
                         const unsigned char* src = kind ? reinterpret_cast<const unsigned char*>(w) + (uint64_t)q.x * cs_w
                                                         : reinterpret_cast<const unsigned char*>(vn) + (uint64_t)q.x * cs;
                         const uint32_t dst = slot0 + slot * (uint32_t)d.slot_bytes;
-                        if (hint_col) bulk_g2s_hint(dst, src, kind ? bw : bv, fb, pol_last);
-                        else bulk_g2s(dst, src, kind ? bw : bv, fb);
+                        if (hint_col) bulk_g2s_hint(dst, src, bytes, fb, pol_last);
+                        else bulk_g2s(dst, src, bytes, fb);
                     }
                 }
             }
@@ -399,6 +414,14 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
                 }
             };
 
+            // columns this patch shares with the steps s-1 .. s-D+1 were copied on THEIR barriers, and
+            // copies of different steps land in any order: wait for the steps the record names
+            {
+                const uint32_t mask = sl[kCcMaskWord];
+#pragma unroll
+                for (int r = 1; r < D; ++r)
+                    if ((mask >> r) & 1u) mbar_wait(full_bar((s - r) % NB), (uint32_t)(((s - r) / NB) & 1), 3, s);
+            }
             uint32_t sE[24];                    // i0 i1 i2 b0..b5 om0..om5 oc0..oc5 x0[0..2]
             ld_slots(sl + SID_I0, sE);
             C vI[3], vB[6];
@@ -552,13 +575,13 @@ static size_t cc_fixed_smem(const CcShape& sh, int nlev) {
 }
 
 template <class T>
-int cc_max_slots(int shape, int nlev, int smem_optin) {
+int cc_max_slots(int shape, int nlev, int slot_bytes, int smem_optin) {
     const long avail = (long)smem_optin - (long)cc_fixed_smem<T>(cc_shape(shape), nlev) - kCcSlotTailPad;
     if (avail <= 0) return 0;
-    return (int)(avail / cc_slot_bytes<T>(nlev));
+    return (int)(avail / slot_bytes);
 }
-template int cc_max_slots<double>(int, int, int);
-template int cc_max_slots<float>(int, int, int);
+template int cc_max_slots<double>(int, int, int, int);
+template int cc_max_slots<float>(int, int, int, int);
 template int cc_slot_bytes<double>(int);
 template int cc_slot_bytes<float>(int);
 

@@ -185,6 +185,34 @@ def test_fp32_variant_permuted_r2b4(torch_cuda, lib, oracle_grid, variant):
     check_all(res, ref, 90, TOL["f32"])
 
 
+@pytest.mark.parametrize("shape", [0, 1, 2, 3])
+def test_column_cache_never_reads_a_stale_slot(torch_cuda, lib, oracle_grid, shape):
+    """Kernel 4 keeps columns in shared memory across steps. Repeating ONE input hides a read that comes too
+    early (the slot still holds the same column from the previous launch), so two different inputs alternate
+    and every launch is compared with the oracle. This is the test that caught bulk copies of an earlier step
+    still in flight when a later step read their slot."""
+    torch = torch_cuda
+    og = oracle_grid(4)
+    g = lib_grid(lib, 4)
+    dev = torch.device("cuda:0")
+    nlev = 90
+    sets = []
+    for cfg, fv, fw in ((1, 1.0, 1.0), (2, -3.0, 5.0)):
+        vn, w, zh = si.make_fields(cfg, og.edge_xyz, og.edge_normal, og.nc, nlev=nlev, ldk=90, ldk_w=92)
+        vn, w = np.nan_to_num(vn) * fv, np.nan_to_num(w) * fw
+        ref = og.velocity_tendencies(vn, w, zh, nlev, with_scale=True)
+        sets.append((torch.from_numpy(vn).to(dev), torch.from_numpy(w).to(dev), zh, ref))
+    g.set_option(lib.ICON_OPT_CC_SHAPE, shape)
+    g.set_option(lib.ICON_OPT_TENDENCY_KERNEL, 4)
+    for it in range(300):
+        d_vn, d_w, zh, ref = sets[it % 2]
+        ddt = torch.full((g.ne, 90), float("nan"), dtype=torch.float64, device=dev)
+        lib.dycore_velocity_tendencies(g, zh, d_vn, d_w, ddt, nlev)
+        torch.cuda.synchronize()
+        err = np.abs(ddt.cpu().numpy() - ref["ddt_vn"])
+        assert (err <= TOL["f64"] * ref["m_ddt"]).all(), "launch %d" % it
+
+
 def test_argument_errors_on_device(torch_cuda, lib):
     torch = torch_cuda
     g = lib_grid(lib, 1)
