@@ -96,6 +96,10 @@ enum {
                                      2 = patch records evict-first, 4 = vn / w columns evict-last. Default 3. */
     ICON_OPT_CC_MERGE = 3,        /* kernel 4: 1 (default) = columns with consecutive ids arrive as one bulk copy
                                      when the field's column stride allows it; 0 = one copy per column. */
+    ICON_OPT_CC_TILE = 4,         /* kernel 4: patches per tile of the round-robin work order (CTA b walks the tiles
+                                     b, b + #CTAs, ... so that neighbouring tiles are in flight together and share
+                                     their halo columns through the L2); even; 0 = one contiguous range per CTA.
+                                     Default 16. */
     ICON_OPT_COUNT
 };
 

@@ -21,6 +21,7 @@ ICON_OPT_TENDENCY_KERNEL = 0
 ICON_OPT_CC_SHAPE = 1
 ICON_OPT_CC_L2_HINTS = 2
 ICON_OPT_CC_MERGE = 3
+ICON_OPT_CC_TILE = 4
 
 TABLES = ("c2v", "c2e", "e2c", "e2v", "e2e4", "v2e", "v2c", "v_deg", "c_os", "v_os",
           "vert_xyz", "cell_xyz", "edge_xyz", "edge_normal", "l_e", "d_e", "inv_d_e", "f_e", "c_lin", "rbf",

@@ -226,14 +226,16 @@ template <class T>
 int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev, int64_t ldk, int64_t ldk_w) {
     const int shape = g->options[ICON_OPT_CC_SHAPE];
     const bool merge = g->options[ICON_OPT_CC_MERGE] != 0;
-    if (p.nlev == nlev && p.shape == shape && p.ldk == ldk && p.ldk_w == ldk_w && p.merge == merge && (p.ready || p.unsupported))
+    const int tile = g->options[ICON_OPT_CC_TILE];
+    if (p.nlev == nlev && p.shape == shape && p.ldk == ldk && p.ldk_w == ldk_w && p.merge == merge && p.tile == tile &&
+        (p.ready || p.unsupported))
         return ICON_OK;
     dev_release(g, p.steps); dev_release(g, p.loads); dev_release(g, p.records);
     dev_release(g, p.cta_patch_begin); dev_release(g, p.cta_step_begin);
     p = icon::DevCcTables<T>();
     p.nlev = nlev;
     p.shape = shape;
-    p.ldk = ldk; p.ldk_w = ldk_w; p.merge = merge;
+    p.ldk = ldk; p.ldk_w = ldk_w; p.merge = merge; p.tile = tile;
     const icon::CcShape& sh = icon::cc_shape(shape);
     const icon::CcGeometry geom = cc_geometry<T>(nlev, ldk, ldk_w, merge);
     const int slot_bytes = geom.slot_bytes;
@@ -250,7 +252,7 @@ int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev, int64_t ld
     std::vector<unsigned char> rec;
     const size_t rb = (size_t)icon::kScCoefWords * sizeof(T) + icon::kCcRecordTail;
     try {
-        std::string err = icon::build_cc_schedule(sc, g->num_sms, n_slots, geom, sh.group, sh.depth, cs);
+        std::string err = icon::build_cc_schedule(sc, g->num_sms, n_slots, geom, sh.group, sh.depth, g->options[ICON_OPT_CC_TILE], cs);
         if (!err.empty()) {
             p.unsupported = true;
             return ICON_OK;
@@ -260,9 +262,10 @@ int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev, int64_t ld
         for (int64_t q = 0; q < sc.n_patches; ++q) {
             unsigned char* r = rec.data() + (size_t)q * rb;
             T* cf = reinterpret_cast<T*>(r);
-            for (int i = 0; i < icon::kScCoefWords; ++i) cf[i] = (T)sc.coef[(size_t)q * icon::kScCoefWords + i];
+            const int64_t src = cs.patch_order[(size_t)q];       // record q belongs to work position q
+            for (int i = 0; i < icon::kScCoefWords; ++i) cf[i] = (T)sc.coef[(size_t)src * icon::kScCoefWords + i];
             int32_t* oid = reinterpret_cast<int32_t*>(r + (size_t)icon::kScCoefWords * sizeof(T));
-            const int32_t* id = &sc.ids[(size_t)q * icon::kScIdWords];
+            const int32_t* id = &sc.ids[(size_t)src * icon::kScIdWords];
             for (int x = 0; x < 3; ++x) {
                 oid[x] = id[icon::SID_I0 + x];
                 oid[3 + x] = id[icon::SID_B0 + 2 * x];
@@ -498,6 +501,7 @@ int icon_grid_create(int bisections_k, uint64_t seed, unsigned flags, icon_grid_
     g->options[ICON_OPT_TENDENCY_KERNEL] = 4;
     g->options[ICON_OPT_CC_L2_HINTS] = 3;
     g->options[ICON_OPT_CC_MERGE] = 1;
+    g->options[ICON_OPT_CC_TILE] = 16;
     try {
         std::string err = icon::build_host_grid(bisections_k, seed, (flags & ICON_PERMUTE) != 0, g->host);
         if (!err.empty()) {
@@ -601,6 +605,7 @@ int icon_grid_table_device(icon_grid_t* g, int which, int dtype, const void** dp
 int icon_grid_set_option(icon_grid_t* g, int option, int value) {
     if (!g) return fail(ICON_EINVAL, "grid handle is NULL");
     if (option < 0 || option >= ICON_OPT_COUNT) return fail(ICON_EINVAL, "unknown option");
+    if (option == ICON_OPT_CC_TILE && (value < 0 || value > 4096 || value % 2)) return fail(ICON_EINVAL, "bad option value");
     if (option == ICON_OPT_CC_L2_HINTS && (value < 0 || value > 7)) return fail(ICON_EINVAL, "bad option value");
     if (option == ICON_OPT_CC_SHAPE && (value < 0 || value >= icon::kCcNumShapes)) return fail(ICON_EINVAL, "bad option value");
     if (option == ICON_OPT_TENDENCY_KERNEL && (value < 0 || value > 4)) return fail(ICON_EINVAL, "bad option value");
@@ -646,7 +651,7 @@ int icon_grid_cc_schedule_check(icon_grid_t* g, int dtype, int nlev, int ldk, in
     icon::CcSchedule cs;
     try {
         std::string err = icon::build_cc_schedule(g->sc_host, n_ctas, n_slots, geom, icon::cc_shape(shape).group,
-                                                  icon::cc_shape(shape).depth, cs);
+                                                  icon::cc_shape(shape).depth, g->options[ICON_OPT_CC_TILE], cs);
         if (!err.empty()) return fail(ICON_EUNSUPPORTED, err);
         err = icon::check_cc_schedule(g->sc_host, cs, g->host.ne, g->host.nc);
         if (!err.empty()) return fail(ICON_EINVAL, err);

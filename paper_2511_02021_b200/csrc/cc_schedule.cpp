@@ -24,7 +24,7 @@ inline uint64_t key_of(int slot_in_patch, int32_t id) {
     return ((uint64_t)(uint32_t)id << 1) | (slot_in_patch >= kFirstCell ? 1u : 0u);
 }
 
-void simulate_cta(const ScTables& sc, int64_t pb, int64_t pe, int n_slots, const CcGeometry& geom, int kCcGroup,
+void simulate_cta(const ScTables& sc, const int64_t* order, int64_t pb, int64_t pe, int n_slots, const CcGeometry& geom, int kCcGroup,
                   int max_depth, uint16_t* patch_slots, CtaResult& r) {
     const int64_t n_steps = (pe - pb + kCcGroup - 1) / kCcGroup;
     // pass 1: the distinct columns of every step
@@ -33,7 +33,7 @@ void simulate_cta(const ScTables& sc, int64_t pb, int64_t pe, int n_slots, const
         auto& ks = keys[(size_t)s];
         const int64_t p0 = pb + s * kCcGroup, p1 = std::min(pe, p0 + kCcGroup);
         for (int64_t p = p0; p < p1; ++p)
-            for (int i = 0; i < kRefs; ++i) ks.push_back(key_of(i, sc.ids[(size_t)p * kScIdWords + i]));
+            for (int i = 0; i < kRefs; ++i) ks.push_back(key_of(i, sc.ids[(size_t)order[p] * kScIdWords + i]));
         std::sort(ks.begin(), ks.end());
         ks.erase(std::unique(ks.begin(), ks.end()), ks.end());
     }
@@ -91,17 +91,17 @@ void simulate_cta(const ScTables& sc, int64_t pb, int64_t pe, int n_slots, const
             return;
         }
         // The misses, grouped into runs of consecutive column ids of one kind.
-        struct Run { int kind; uint32_t id; int len; size_t first; };   // first = index into `order`
-        std::vector<size_t> order(miss);                                 // indices into ks, by (kind, id)
-        std::sort(order.begin(), order.end(), [&](size_t a, size_t b2) {
+        struct Run { int kind; uint32_t id; int len; size_t first; };   // first = index into `morder`
+        std::vector<size_t> morder(miss);                                 // indices into ks, by (kind, id)
+        std::sort(morder.begin(), morder.end(), [&](size_t a, size_t b2) {
             const uint64_t ka = ks[a], kb = ks[b2];
             if ((ka & 1) != (kb & 1)) return (ka & 1) < (kb & 1);
             return (ka >> 1) < (kb >> 1);
         });
         std::vector<Run> runs;
-        for (size_t m = 0; m < order.size(); ++m) {
-            const int kind = (int)(ks[order[m]] & 1);
-            const uint32_t id = (uint32_t)(ks[order[m]] >> 1);
+        for (size_t m = 0; m < morder.size(); ++m) {
+            const int kind = (int)(ks[morder[m]] & 1);
+            const uint32_t id = (uint32_t)(ks[morder[m]] >> 1);
             const bool mergeable = geom.stride_bytes[kind] == geom.slot_bytes;
             if (!runs.empty() && mergeable && runs.back().kind == kind && runs.back().len < kCcMaxRun &&
                 runs.back().id + (uint32_t)runs.back().len == id) {
@@ -152,7 +152,7 @@ void simulate_cta(const ScTables& sc, int64_t pb, int64_t pe, int n_slots, const
             }
             for (int t = 0; t < run.len; ++t) {
                 const int32_t q = best + t;
-                const size_t mi = order[run.first + (size_t)t];
+                const size_t mi = morder[run.first + (size_t)t];
                 const uint64_t k = ks[mi];
                 if (slot_key[(size_t)q] != ~0ull) resident.erase(slot_key[(size_t)q]);
                 slot_key[(size_t)q] = k;
@@ -183,7 +183,7 @@ void simulate_cta(const ScTables& sc, int64_t pb, int64_t pe, int n_slots, const
             // be in flight when step s starts (copies of different steps complete in any order)
             uint16_t mask = 0;
             for (int i = 0; i < kRefs; ++i) {
-                const int32_t q = step_slot[key_of(i, sc.ids[(size_t)p * kScIdWords + i])];
+                const int32_t q = step_slot[key_of(i, sc.ids[(size_t)order[p] * kScIdWords + i])];
                 o[i] = (uint16_t)q;
                 const int64_t age = s - slot_loaded[(size_t)q];
                 if (age > 0 && age < max_depth) mask |= (uint16_t)(1u << age);
@@ -197,7 +197,7 @@ void simulate_cta(const ScTables& sc, int64_t pb, int64_t pe, int n_slots, const
 }  // namespace
 
 std::string build_cc_schedule(const ScTables& sc, int n_ctas, int n_slots, const CcGeometry& geom, int group, int depth,
-                              CcSchedule& out) {
+                              int tile, CcSchedule& out) {
     const int kCcGroup = group;
     const int64_t np = sc.n_patches;
     if (np <= 0 || n_ctas <= 0) return "cc schedule: empty grid";
@@ -214,16 +214,37 @@ std::string build_cc_schedule(const ScTables& sc, int n_ctas, int n_slots, const
     out.geom = geom;
     out.group = group;
     out.depth = depth;
+    out.tile = tile;
     out.cta_patch_begin.resize((size_t)n_ctas + 1);
     // whole steps per CTA, spread evenly
     const int64_t total_steps = max_ctas;
     for (int b = 0; b <= n_ctas; ++b)
         out.cta_patch_begin[(size_t)b] = std::min(np, (total_steps * b / n_ctas) * kCcGroup);
+    // Work order: position -> patch of sc. tile == 0: generation order, each CTA a contiguous range.
+    // tile > 0: tiles of `tile` consecutive patches dealt round-robin, CTA b walks the tiles b, b+n_ctas,
+    // ...: at any time the CTAs work on neighbouring tiles, so a halo column that two tiles share is
+    // fetched twice within microseconds and the second fetch hits the L2 instead of HBM.
+    out.patch_order.resize((size_t)np);
+    if (tile > 0) {
+        if (tile % group) return "cc schedule: tile must be a multiple of the group";
+        const int64_t nt = (np + tile - 1) / tile;
+        if (n_ctas > nt) n_ctas = (int)nt;
+        out.n_ctas = n_ctas;
+        out.cta_patch_begin.assign((size_t)n_ctas + 1, 0);
+        int64_t pos = 0;
+        for (int b = 0; b < n_ctas; ++b) {
+            for (int64_t t = b; t < nt; t += n_ctas)
+                for (int64_t p = t * tile; p < std::min(np, (t + 1) * tile); ++p) out.patch_order[(size_t)pos++] = p;
+            out.cta_patch_begin[(size_t)b + 1] = pos;
+        }
+    } else {
+        for (int64_t p = 0; p < np; ++p) out.patch_order[(size_t)p] = p;
+    }
     out.patch_slots.assign((size_t)np * kCcSlotWords, 0);
     std::vector<CtaResult> res((size_t)n_ctas);
 #pragma omp parallel for schedule(dynamic, 1)
     for (int b = 0; b < n_ctas; ++b)
-        simulate_cta(sc, out.cta_patch_begin[(size_t)b], out.cta_patch_begin[(size_t)b + 1], n_slots, geom, group,
+        simulate_cta(sc, out.patch_order.data(), out.cta_patch_begin[(size_t)b], out.cta_patch_begin[(size_t)b + 1], n_slots, geom, group,
                      depth, out.patch_slots.data(), res[(size_t)b]);
     out.cta_step_begin.assign((size_t)n_ctas + 1, 0);
     size_t n_loads = 0;

@@ -80,19 +80,23 @@ struct CcSchedule {
     int group = 0;                           // patches per step
     int depth = 0;                           // steps a load may run ahead of its readers (pipeline depth)
     CcGeometry geom = {0, {0, 0}, {0, 0}};
-    std::vector<int64_t> cta_patch_begin;    // [n_ctas + 1]
+    int tile = 0;                            // patches per round-robin tile (0 = contiguous ranges)
+    std::vector<int64_t> patch_order;        // [n_patches] work position -> patch of the ScTables
+    std::vector<int64_t> cta_patch_begin;    // [n_ctas + 1], work positions
     std::vector<int64_t> cta_step_begin;     // [n_ctas + 1]
     std::vector<CcStep> steps;
     std::vector<CcLoad> loads;
-    std::vector<uint16_t> patch_slots;       // [n_patches][kCcSlotWords], slot index
+    std::vector<uint16_t> patch_slots;       // [work position][kCcSlotWords], slot index
     // statistics (icon_grid_worklist_stats, tests)
     int64_t n_sync_steps = 0, n_vn_loads = 0, n_w_loads = 0;   // columns loaded
     int64_t n_copies = 0;                                      // bulk copies (runs)
 };
 
 // Returns an empty string on success, else an error message (e.g. too few slots for one step).
+// `tile`: 0 = every CTA walks a contiguous range of the generation order; > 0 = tiles of that many
+// patches are dealt round-robin to the CTAs (CcSchedule::patch_order).
 std::string build_cc_schedule(const ScTables& sc, int n_ctas, int n_slots, const CcGeometry& geom, int group, int depth,
-                              CcSchedule& out);
+                              int tile, CcSchedule& out);
 
 // cc_schedule_check.cpp: replays `cs` as the kernel would and checks the guarantees it relies on
 // (independent of the builder). Empty string = valid.

@@ -25,6 +25,14 @@ std::string check_cc_schedule(const ScTables& sc, const CcSchedule& cs, int64_t 
     if (cs.n_ctas <= 0 || cs.group <= 0 || cs.depth <= 0) return "check: empty schedule";
     if (cs.cta_patch_begin.front() != 0 || cs.cta_patch_begin.back() != sc.n_patches) return "check: patches not covered";
     if (cs.cta_step_begin.front() != 0 || cs.cta_step_begin.back() != (int64_t)cs.steps.size()) return "check: steps not covered";
+    {   // the work order visits every patch exactly once
+        if ((int64_t)cs.patch_order.size() != sc.n_patches) return "check: work order has the wrong length";
+        std::vector<char> seen((size_t)sc.n_patches, 0);
+        for (int64_t p : cs.patch_order) {
+            if (p < 0 || p >= sc.n_patches || seen[(size_t)p]) return "check: work order is not a permutation";
+            seen[(size_t)p] = 1;
+        }
+    }
     std::atomic<int> err(0);
 #pragma omp parallel for schedule(dynamic, 1)
     for (int b = 0; b < cs.n_ctas; ++b) {
@@ -81,7 +89,7 @@ std::string check_cc_schedule(const ScTables& sc, const CcSchedule& cs, int64_t 
                 const unsigned mask = cs.patch_slots[(size_t)p * kCcSlotWords + kCcMaskWord];
                 for (int i = 0; i < SID_PAD; ++i) {
                     const size_t q = cs.patch_slots[(size_t)p * kCcSlotWords + i];
-                    const int64_t want = (int64_t)sc.ids[(size_t)p * kScIdWords + i] * 2 + (i >= SID_T0 ? 1 : 0);
+                    const int64_t want = (int64_t)sc.ids[(size_t)cs.patch_order[(size_t)p] * kScIdWords + i] * 2 + (i >= SID_T0 ? 1 : 0);
                     if (content[q] != want) { fail(12); break; }
                     last_read[q] = s;
                     // rule 6: a column filled by a step that has not necessarily drained (s-depth < s' < s)

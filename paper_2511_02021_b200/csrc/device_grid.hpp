@@ -87,6 +87,7 @@ struct DevCcTables {
     int shape = -1;                // index into kCcShapes the schedule was built for
     int64_t ldk = -1, ldk_w = -1;  // column strides the runs were merged for
     bool merge = true;             // ICON_OPT_CC_MERGE it was built with
+    int tile = -1;                 // ICON_OPT_CC_TILE it was built with
     bool ready = false;
     bool unsupported = false;      // this (T, nlev) cannot use the kernel: callers fall back
     int64_t stats[5] = {0, 0, 0, 0, 0};   // steps, steps with reduced depth, vn columns, w columns, bulk copies

@@ -113,12 +113,13 @@ def test_cc_schedule_replays_correctly(k, seed, flags, shape):
     g.set_option(lib.ICON_OPT_CC_SHAPE, shape)
     for dtype, nlev, ldk, ldk_w in ((0, 90, 96, 96), (0, 90, 90, 92), (1, 90, 92, 92), (0, 30, 30, 32), (0, 2, 2, 4),
                                     (0, 65, 66, 66)):
-        for merge in (1, 0):
+        for merge, tile in ((1, 16), (0, 16), (1, 0), (1, 64)):
             g.set_option(lib.ICON_OPT_CC_MERGE, merge)
+            g.set_option(lib.ICON_OPT_CC_TILE, tile)
             st = g.cc_schedule_check(dtype, nlev, ldk, ldk_w, n_ctas=148, smem_bytes=232448)
             np_ = g.nc // 4
             group = (1, 2, 1, 1)[shape]
-            assert st["ctas"] == min(148, -(-np_ // group))
+            assert st["ctas"] == min(148, -(-np_ // (tile or group)))
             assert st["steps"] >= -(-np_ // group)
             # every patch needs its 36 + 7 columns at least once per CTA range, never more than 43 per patch
             assert 6 * np_ <= st["vn_columns"] <= 36 * np_ and 4 * np_ <= st["w_columns"] <= 7 * np_
