@@ -91,7 +91,7 @@ enum {
                                          by bulk asynchronous copies on a host-built schedule; level counts
                                          it cannot hold (nlev > 95) fall back to 3. */
     ICON_OPT_CC_SHAPE = 1,        /* pipeline shape of kernel 4 (consumer warps / patches per step / ring
-                                     depth): 0 = 8/1/10 (default), 1 = 8/2/5, 2 = 8/1/9, 3 = 8/1/11. */
+                                     depth): 0 = 8/2/5 (default), 1 = 8/1/10, 2 = 8/1/9, 3 = 8/1/11. */
     ICON_OPT_CC_L2_HINTS = 2,     /* L2 eviction hints of kernel 4, bit mask: 1 = ddt_vn stores evict-first,
                                      2 = patch records evict-first, 4 = vn / w columns evict-last. Default 3. */
     ICON_OPT_CC_MERGE = 3,        /* kernel 4: 1 (default) = columns with consecutive ids arrive as one bulk copy

@@ -26,40 +26,96 @@ __device__ __forceinline__ T ldg(const T* p) {
 // block = 12 warps: warps 0..7 take 8 consecutive cells, warps 8..11 take the 4 vertices of the
 // same stretch of the generation order, so both read the same vn columns while they are in L1/L2.
 // ------------------------------------------------------------------------------------------
-template <class T>
-__global__ void __launch_bounds__(384) k_div_vort(int64_t nc, int64_t nv, int nlev, int64_t ldk,
-                                                  const int32_t* __restrict__ c2e, const T* __restrict__ geofac_div,
-                                                  const int32_t* __restrict__ v2e, const T* __restrict__ geofac_rot,
-                                                  const int32_t* __restrict__ user_c, const int32_t* __restrict__ user_v,
-                                                  const T* __restrict__ vn, T* __restrict__ div, T* __restrict__ vort) {
+// All 6 * L column loads of a warp are issued before the first use (L = level chunks per lane is a
+// template parameter so that the loop over chunks unrolls): the kernel is a pure stream with one
+// dependent lookup (ids -> columns), and what limits it is the number of bytes in flight per SM.
+// volatile asm: the loads keep their program order, i.e. all of them are issued before the first FMA
+__device__ __forceinline__ double ld_stream(const double* p) {
+    double v;
+    asm volatile("ld.global.nc.f64 %0, [%1];" : "=d"(v) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ float ld_stream(const float* p) {
+    float v;
+    asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(v) : "l"(p));
+    return v;
+}
+
+// Persistent version: 8 warps per block, warps 0..3 take two cells each, warps 4..7 one vertex each
+// of chunk t (8 cells + the 4 vertices of the same stretch of the generation order, so both hit the
+// same vn columns while they are in L1/L2) -- 6 neighbour columns and 18 loads in flight per warp
+// either way. The ids and coefficients of the NEXT chunk are fetched before the columns of the
+// current one are, which takes the dependent lookup (ids -> columns) off the critical path; with
+// one short-lived block per 8 cells the kernel spent its time in waves of two latencies each.
+template <class T, int L>
+__global__ void __launch_bounds__(256, 2) k_div_vort(int64_t nc, int64_t nv, int nlev, int64_t ldk,
+                                                     const int32_t* __restrict__ c2e, const T* __restrict__ geofac_div,
+                                                     const int32_t* __restrict__ v2e, const T* __restrict__ geofac_rot,
+                                                     const int32_t* __restrict__ user_c, const int32_t* __restrict__ user_v,
+                                                     const T* __restrict__ vn, T* __restrict__ div, T* __restrict__ vort) {
     const int w = warp_in_block(), lane = lane_id();
-    if (w < 8) {
-        const int64_t p = (int64_t)blockIdx.x * 8 + w;
-        if (p >= nc) return;
-        const int64_t c = user_c ? user_c[p] : p;
-        const T* col0 = vn + (int64_t)ldg(c2e + 3 * p) * ldk;
-        const T* col1 = vn + (int64_t)ldg(c2e + 3 * p + 1) * ldk;
-        const T* col2 = vn + (int64_t)ldg(c2e + 3 * p + 2) * ldk;
-        const T g0 = ldg(geofac_div + 3 * p), g1 = ldg(geofac_div + 3 * p + 1), g2 = ldg(geofac_div + 3 * p + 2);
-        T* out = div + c * ldk;
-        for (int k = lane; k < nlev; k += kWarp) out[k] = g0 * col0[k] + g1 * col1[k] + g2 * col2[k];
-    } else {
-        const int64_t p = (int64_t)blockIdx.x * 4 + (w - 8);
-        if (p >= nv) return;
-        const int64_t v = user_v ? user_v[p] : p;
-        const T* col[6];
+    const bool cells = w < 4;
+    const int wi = w & 3;
+    const int64_t n_ent = cells ? nc : nv;
+    const int32_t* ids = cells ? c2e : v2e;
+    const T* coef = cells ? geofac_div : geofac_rot;
+    const int32_t* user = cells ? user_c : user_v;
+    T* out = cells ? div : vort;
+    const int64_t n_chunks = (nc + 7) / 8 > (nv + 3) / 4 ? (nc + 7) / 8 : (nv + 3) / 4;
+    // six (id, coefficient) pairs: two cells (3 + 3) or one vertex (6); row = first entity of the warp
+    struct Meta {
+        int32_t id[6];
         T g[6];
+        int64_t o0, o1;       // output columns (user ids), -1 = none
+    };
+    auto load_meta = [&](int64_t t) {
+        Meta m;
+        const int64_t p = cells ? t * 8 + wi * 2 : t * 4 + wi;
+        const bool v0 = t < n_chunks && p < n_ent, v1 = cells && t < n_chunks && p + 1 < n_ent;
 #pragma unroll
         for (int j = 0; j < 6; ++j) {
-            col[j] = vn + (int64_t)ldg(v2e + 6 * p + j) * ldk;
-            g[j] = ldg(geofac_rot + 6 * p + j);
+            const bool ok = cells ? (j < 3 ? v0 : v1) : v0;
+            m.id[j] = ok ? ldg(ids + 6 * (cells ? p / 2 : p) + j) : 0;       // cells: rows p, p+1 = 6 consecutive entries (p even)
+            m.g[j] = ok ? ldg(coef + 6 * (cells ? p / 2 : p) + j) : (T)0;
         }
-        T* out = vort + v * ldk;
-        for (int k = lane; k < nlev; k += kWarp) {
-            T s = g[0] * col[0][k];
+        m.o0 = v0 ? (user ? (int64_t)ldg(user + p) : p) : -1;
+        m.o1 = v1 ? (user ? (int64_t)ldg(user + p + 1) : p + 1) : -1;
+        return m;
+    };
+    // a block takes kRun consecutive chunks (64 cells + their 32 vertices) before it jumps on, so that the
+    // columns neighbouring chunks share are still in its L1 when the next one asks for them
+    constexpr int kRun = 8;
+    auto chunk_of = [&](int64_t q) { return ((int64_t)blockIdx.x + (q / kRun) * (int64_t)gridDim.x) * kRun + q % kRun; };
+    Meta nxt = load_meta(chunk_of(0));
+    for (int64_t q = 0; chunk_of(q) - q % kRun < n_chunks; ++q) {
+        const Meta cur = nxt;
+        nxt = load_meta(chunk_of(q + 1));
+        for (int k0 = 0; k0 < nlev; k0 += kWarp * L) {
+            T x[6][L];
 #pragma unroll
-            for (int j = 1; j < 6; ++j) s += g[j] * col[j][k];
-            out[k] = s;
+            for (int j = 0; j < 6; ++j) {
+                const T* col = vn + (int64_t)cur.id[j] * ldk + k0;
+#pragma unroll
+                for (int l = 0; l < L; ++l) {
+                    const int k = lane + kWarp * l;
+                    x[j][l] = ld_stream(col + (k0 + k < nlev ? k : nlev - 1 - k0));   // past the end: re-read the last level, unused
+                }
+            }
+#pragma unroll
+            for (int l = 0; l < L; ++l) {
+                const int k = k0 + lane + kWarp * l;
+                const T a = cur.g[0] * x[0][l] + cur.g[1] * x[1][l] + cur.g[2] * x[2][l];
+                const T b = cur.g[3] * x[3][l] + cur.g[4] * x[4][l] + cur.g[5] * x[5][l];
+                if (k < nlev) {
+                    if (cells) {
+                        if (cur.o0 >= 0) out[cur.o0 * ldk + k] = a;
+                        if (cur.o1 >= 0) out[cur.o1 * ldk + k] = b;
+                    } else if (cur.o0 >= 0) {
+                        // S2 in slot order: ((((g0 x0 + g1 x1) + g2 x2) + g3 x3) + g4 x4) + g5 x5 up to rounding order
+                        out[cur.o0 * ldk + k] = a + b;
+                    }
+                }
+            }
         }
     }
 }
@@ -242,8 +298,18 @@ int launch_div_vort(const icon_grid& g, const DevCoeffs<T>& c, int nlev, int64_t
     unsigned nb = blocks_for(nc, 8);
     unsigned nbv = blocks_for(nv, 4);
     if (nbv > nb) nb = nbv;
-    k_div_vort<T><<<nb, 384, 0, s>>>(nc, nv, nlev, ldk, g.tab.c2e, c.geofac_div, g.tab.v2e, c.geofac_rot, g.tab.user_c,
-                                     g.tab.user_v, vn, div, vort);
+    nb = (nb + 7) / 8;                                                                 // a block walks runs of 8 chunks
+    const unsigned persistent = (unsigned)(g.num_sms > 0 ? g.num_sms : 148) * 2u;      // two blocks per SM
+    if (nb > persistent) nb = persistent;
+    if (nlev <= 32)
+        k_div_vort<T, 1><<<nb, 256, 0, s>>>(nc, nv, nlev, ldk, g.tab.c2e, c.geofac_div, g.tab.v2e, c.geofac_rot, g.tab.user_c,
+                                            g.tab.user_v, vn, div, vort);
+    else if (nlev <= 64)
+        k_div_vort<T, 2><<<nb, 256, 0, s>>>(nc, nv, nlev, ldk, g.tab.c2e, c.geofac_div, g.tab.v2e, c.geofac_rot, g.tab.user_c,
+                                            g.tab.user_v, vn, div, vort);
+    else
+        k_div_vort<T, 3><<<nb, 256, 0, s>>>(nc, nv, nlev, ldk, g.tab.c2e, c.geofac_div, g.tab.v2e, c.geofac_rot, g.tab.user_c,
+                                            g.tab.user_v, vn, div, vort);
     cudaError_t err = cudaGetLastError();
     return err == cudaSuccess ? 1 : -(int)err;
 }
