@@ -87,9 +87,11 @@ enum {
                                      1 = fused per-edge gather kernel (no workspace);
                                      2 = fused register-resident patch kernel with shared-memory exchange;
                                      3 = self-contained patch kernel (one warp per patch, columns through L1);
-                                     4 = column-cache kernel (default): whole columns staged in shared memory
-                                         by bulk asynchronous copies on a host-built schedule; level counts
-                                         it cannot hold (nlev > 95) fall back to 3. */
+                                     4 = column-cache kernel: whole columns staged in shared memory by bulk
+                                         asynchronous copies on a host-built schedule; level counts it cannot
+                                         hold (nlev > 95) fall back to 3;
+                                     5 = auto (default): 4 for fp64 with 32 <= nlev <= 95, 2 for nlev <= 31,
+                                         else 3 (the fastest measured variant of each regime). */
     ICON_OPT_CC_SHAPE = 1,        /* pipeline shape of kernel 4 (consumer warps / patches per step / ring
                                      depth): 0 = 8/2/5 (default), 1 = 8/1/10, 2 = 8/1/9, 3 = 8/1/11. */
     ICON_OPT_CC_L2_HINTS = 2,     /* L2 eviction hints of kernel 4, bit mask: 1 = ddt_vn stores evict-first,

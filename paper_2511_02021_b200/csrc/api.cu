@@ -408,6 +408,12 @@ int tendencies_impl(icon_grid* g, icon::DevCoeffs<T>& c, icon::DevPatchTables<T>
     const bool want_opt = vt_opt || ke_c_opt || vort_opt;
     int n;
     int variant = g->options[ICON_OPT_TENDENCY_KERNEL];
+    if (variant == 5) {
+        // auto, from the measurements on B200: the column cache wins where a lane owns
+        // three levels of 8-byte columns (33 <= nlev+1 <= 96, fp64); shallow columns are copy-request bound
+        // there and go to the exchange patch kernel, 4-byte columns to the self-contained patch kernel
+        variant = nlev + 1 <= 32 ? 2 : (sizeof(T) == 8 && icon::cc_levels_per_lane(nlev) == 3) ? 4 : 3;
+    }
     if (variant == 4 && !want_opt) {
         if ((rc = ensure_cc_tables(g, ct, nlev, ldk, ldk_w))) return rc;
         if (ct.unsupported) variant = 3;      // level count / dtype the column cache cannot hold
@@ -498,7 +504,7 @@ int icon_grid_create(int bisections_k, uint64_t seed, unsigned flags, icon_grid_
     g->flags = flags;
     g->seed = seed;
     g->host_only = (flags & ICON_HOST_ONLY) != 0;
-    g->options[ICON_OPT_TENDENCY_KERNEL] = 4;
+    g->options[ICON_OPT_TENDENCY_KERNEL] = 5;
     g->options[ICON_OPT_CC_L2_HINTS] = 3;
     g->options[ICON_OPT_CC_MERGE] = 1;
     g->options[ICON_OPT_CC_TILE] = 16;
@@ -608,7 +614,7 @@ int icon_grid_set_option(icon_grid_t* g, int option, int value) {
     if (option == ICON_OPT_CC_TILE && (value < 0 || value > 4096 || value % 2)) return fail(ICON_EINVAL, "bad option value");
     if (option == ICON_OPT_CC_L2_HINTS && (value < 0 || value > 7)) return fail(ICON_EINVAL, "bad option value");
     if (option == ICON_OPT_CC_SHAPE && (value < 0 || value >= icon::kCcNumShapes)) return fail(ICON_EINVAL, "bad option value");
-    if (option == ICON_OPT_TENDENCY_KERNEL && (value < 0 || value > 4)) return fail(ICON_EINVAL, "bad option value");
+    if (option == ICON_OPT_TENDENCY_KERNEL && (value < 0 || value > 5)) return fail(ICON_EINVAL, "bad option value");
     g->options[option] = value;
     return ICON_OK;
 }
