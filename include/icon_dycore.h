@@ -95,7 +95,9 @@ enum {
     ICON_OPT_CC_SHAPE = 1,        /* pipeline shape of kernel 4 (consumer warps / patches per step / ring
                                      depth): 0 = 8/2/5 (default), 1 = 8/1/10, 2 = 8/1/9, 3 = 8/1/11. */
     ICON_OPT_CC_L2_HINTS = 2,     /* L2 eviction hints of kernel 4, bit mask: 1 = ddt_vn stores evict-first,
-                                     2 = patch records evict-first, 4 = vn / w columns evict-last. Default 3. */
+                                     2 = patch records evict-first, 4 = vn / w columns evict-last, 16 = outputs leave by
+                                     plain coalesced stores (transposed in shared memory) instead of bulk stores.
+                                     Default 19. */
     ICON_OPT_CC_MERGE = 3,        /* kernel 4: 1 (default) = columns with consecutive ids arrive as one bulk copy
                                      when the field's column stride allows it; 0 = one copy per column. */
     ICON_OPT_CC_TILE = 4,         /* kernel 4: patches per tile of the round-robin work order (CTA b walks the tiles
@@ -190,6 +192,18 @@ int dycore_velocity_tendencies(icon_grid_t* g, int dtype, int nlev, int ldk, int
                                const double* z_half,
                                const void* vn, const void* w, void* ddt_vn,
                                void* vt_opt, void* ke_c_opt, void* vort_opt, void* cuda_stream);
+
+/*
+ * dycore_step -- one pass of the whole hot path: the outputs of
+ * dycore_velocity_tendencies (ddt_vn) and of dycore_div_vort (div, vort) for the same vn, w. Where the
+ * column-cache tendency kernel runs (ICON_OPT_TENDENCY_KERNEL 4, or 5 = auto in its regime) all three come
+ * out of ONE kernel that reads vn once: div of a patch's four cells and the vorticity at its three midpoint
+ * and three corner vertices are by-products of columns and sums the tendency needs anyway (every vertex of
+ * the grid is a midpoint or corner of some patch; the lowest patch index stores it). Elsewhere it is the two
+ * calls back to back. Same argument rules as the two calls; outputs must not alias inputs or each other.
+ */
+int dycore_step(icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
+                const void* vn, const void* w, void* ddt_vn, void* div, void* vort, void* cuda_stream);
 
 /*
  * dycore_step_host -- one velocity-tendency + div/vort step with HOST field buffers (the

@@ -31,7 +31,7 @@ TABLE_ID = {n: i for i, n in enumerate(TABLES)}
 # every symbol include/icon_dycore.h declares
 EXPORTS = ("icon_grid_create", "icon_grid_destroy", "icon_grid_counts", "icon_grid_table_host",
            "icon_grid_table_device", "icon_grid_set_option", "icon_grid_worklist_stats", "icon_grid_cc_schedule_check", "dycore_div_vort", "dycore_velocity_tendencies",
-           "dycore_step_host", "icon_grid_launch_count", "icon_last_error")
+           "dycore_step", "dycore_step_host", "icon_grid_launch_count", "icon_last_error")
 
 
 class IconError(RuntimeError):
@@ -75,6 +75,8 @@ def load_library():
     L.dycore_div_vort.argtypes = [P, ci, ci, ci, P, P, P, P]
     L.dycore_velocity_tendencies.restype = ci
     L.dycore_velocity_tendencies.argtypes = [P, ci, ci, ci, ci, P, P, P, P, P, P, P, P]
+    L.dycore_step.restype = ci
+    L.dycore_step.argtypes = [P, ci, ci, ci, ci, P, P, P, P, P, P, P]
     L.dycore_step_host.restype = ci
     L.dycore_step_host.argtypes = [P, ci, ci, ci, ci, P, P, P, P, P, P]
     L.icon_last_error.restype = ctypes.c_char_p
@@ -198,6 +200,15 @@ def dycore_velocity_tendencies(grid, z_half, vn, w, ddt_vn, nlev, vt=None, ke_c=
     _check(grid._L.dycore_velocity_tendencies(grid._h, _dtype_of(vn), int(nlev), int(vn.shape[1]), int(w.shape[1]),
                                               _dptr(z), _dptr(vn), _dptr(w), _dptr(ddt_vn), _dptr(vt), _dptr(ke_c),
                                               _dptr(vort), _stream_ptr(stream)))
+
+
+def dycore_step(grid, z_half, vn, w, ddt_vn, div, vort, nlev, stream=None):
+    """S1-S7 in one pass (one fused kernel where the column-cache kernel runs, else the two calls back to back)."""
+    z = np.ascontiguousarray(z_half, dtype=np.float64)
+    if z.size != nlev + 1:
+        raise ValueError("z_half must have nlev+1 entries")
+    _check(grid._L.dycore_step(grid._h, _dtype_of(vn), int(nlev), int(vn.shape[1]), int(w.shape[1]), _dptr(z), _dptr(vn),
+                               _dptr(w), _dptr(ddt_vn), _dptr(div), _dptr(vort), _stream_ptr(stream)))
 
 
 def dycore_step_host(grid, z_half, vn_host, w_host, ddt_vn_host, div_host, vort_host, nlev):

@@ -270,11 +270,13 @@ int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev, int64_t ld
                 oid[x] = id[icon::SID_I0 + x];
                 oid[3 + x] = id[icon::SID_B0 + 2 * x];
             }
+            for (int x = 0; x < 4; ++x) oid[6 + x] = id[icon::SID_T0 + x];
+            for (int x = 0; x < 6; ++x) oid[10 + x] = id[icon::SID_V0 + x];
             for (int x = 0; x < 6; ++x) {          // c_lin halved: the kernel forms w(k) + w(k+1) (exact scaling)
                 cf[icon::SCF_EDGE + 4 * x + 2] *= (T)0.5;
                 cf[icon::SCF_EDGE + 4 * x + 3] *= (T)0.5;
             }
-            uint32_t* so = reinterpret_cast<uint32_t*>(r + (size_t)icon::kScCoefWords * sizeof(T) + 32);
+            uint32_t* so = reinterpret_cast<uint32_t*>(r + (size_t)icon::kScCoefWords * sizeof(T) + 4 * icon::kCcRecordIds);
             for (int i = 0; i < icon::kCcSlotWords; ++i)
                 so[i] = (uint32_t)cs.patch_slots[(size_t)q * icon::kCcSlotWords + i] * (uint32_t)slot_bytes;
             so[icon::kCcMaskWord] = cs.patch_slots[(size_t)q * icon::kCcSlotWords + icon::kCcMaskWord];
@@ -400,7 +402,9 @@ template <class T>
 int tendencies_impl(icon_grid* g, icon::DevCoeffs<T>& c, icon::DevPatchTables<T>& pt, icon::DevScTables<T>& st,
                     icon::DevCcTables<T>& ct, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
                     const void* vn, const void* w, void* ddt_vn, void* vt_opt, void* ke_c_opt, void* vort_opt,
-                    cudaStream_t s) {
+                    cudaStream_t s, void* div_fused = nullptr, void* vort_fused = nullptr, bool* fused_done = nullptr) {
+    // div_fused / vort_fused: dycore_step asks for S1 + S2 from the same pass; only the column-cache kernel can
+    // (it sets *fused_done), with any other kernel the caller launches dycore_div_vort afterwards
     int rc;
     if ((rc = ensure_coeffs(g, c))) return rc;
     void* abc = nullptr;
@@ -418,8 +422,11 @@ int tendencies_impl(icon_grid* g, icon::DevCoeffs<T>& c, icon::DevPatchTables<T>
         if ((rc = ensure_cc_tables(g, ct, nlev, ldk, ldk_w))) return rc;
         if (ct.unsupported) variant = 3;      // level count / dtype the column cache cannot hold
     }
+    if (variant != 4 || want_opt) div_fused = vort_fused = nullptr;
+    if (fused_done) *fused_done = div_fused != nullptr;
     if (variant == 4 && !want_opt) {
-        n = icon::launch_tendencies_cc<T>(*g, ct, nlev, ldk, ldk_w, (const T*)abc, (const T*)vn, (const T*)w, (T*)ddt_vn, s);
+        n = icon::launch_tendencies_cc<T>(*g, ct, nlev, ldk, ldk_w, (const T*)abc, (const T*)vn, (const T*)w, (T*)ddt_vn,
+                                          (T*)div_fused, (T*)vort_fused, s);
     } else if (variant == 0 || want_opt) {
         // optional outputs are produced by the unfused pipeline, which materialises them anyway
         if ((rc = ensure_workspace<T>(g, dtype, ldk))) return rc;
@@ -505,7 +512,7 @@ int icon_grid_create(int bisections_k, uint64_t seed, unsigned flags, icon_grid_
     g->seed = seed;
     g->host_only = (flags & ICON_HOST_ONLY) != 0;
     g->options[ICON_OPT_TENDENCY_KERNEL] = 5;
-    g->options[ICON_OPT_CC_L2_HINTS] = 3;
+    g->options[ICON_OPT_CC_L2_HINTS] = 19;
     g->options[ICON_OPT_CC_MERGE] = 1;
     g->options[ICON_OPT_CC_TILE] = 16;
     try {
@@ -612,7 +619,7 @@ int icon_grid_set_option(icon_grid_t* g, int option, int value) {
     if (!g) return fail(ICON_EINVAL, "grid handle is NULL");
     if (option < 0 || option >= ICON_OPT_COUNT) return fail(ICON_EINVAL, "unknown option");
     if (option == ICON_OPT_CC_TILE && (value < 0 || value > 4096 || value % 2)) return fail(ICON_EINVAL, "bad option value");
-    if (option == ICON_OPT_CC_L2_HINTS && (value < 0 || value > 7)) return fail(ICON_EINVAL, "bad option value");
+    if (option == ICON_OPT_CC_L2_HINTS && (value < 0 || value > 31)) return fail(ICON_EINVAL, "bad option value");
     if (option == ICON_OPT_CC_SHAPE && (value < 0 || value >= icon::kCcNumShapes)) return fail(ICON_EINVAL, "bad option value");
     if (option == ICON_OPT_TENDENCY_KERNEL && (value < 0 || value > 5)) return fail(ICON_EINVAL, "bad option value");
     g->options[option] = value;
@@ -707,6 +714,31 @@ int dycore_velocity_tendencies(icon_grid_t* g, int dtype, int nlev, int ldk, int
     return tendencies_impl<float>(g, g->c32, g->p32, g->s32, g->cc32, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, vt_opt, ke_c_opt, vort_opt, s);
 }
 
+int dycore_step(icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, const double* z_half, const void* vn, const void* w,
+                void* ddt_vn, void* div, void* vort, void* cuda_stream) {
+    int rc = check_common(g, dtype, nlev, ldk, 2);
+    if (rc) return rc;
+    if (ldk_w < nlev + 1) return fail(ICON_EINVAL, "ldk_w < nlev + 1");
+    const int es = dtype == ICON_F64 ? 8 : 4;
+    if (((int64_t)ldk_w * es) % 16) return fail(ICON_EINVAL, "ldk_w*sizeof(T) must be a multiple of 16");
+    if (!z_half) return fail(ICON_EINVAL, "z_half is NULL");
+    if ((rc = check_field(vn, "vn")) || (rc = check_field(w, "w")) || (rc = check_field(ddt_vn, "ddt_vn")) ||
+        (rc = check_field(div, "div")) || (rc = check_field(vort, "vort")))
+        return rc;
+    if (ddt_vn == vn || ddt_vn == w || div == vn || div == w || vort == vn || vort == w || div == ddt_vn || vort == ddt_vn || div == vort)
+        return fail(ICON_EINVAL, "outputs must not alias inputs or each other");
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    bool fused = false;
+    if (dtype == ICON_F64)
+        rc = tendencies_impl<double>(g, g->c64, g->p64, g->s64, g->cc64, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, nullptr,
+                                     nullptr, nullptr, s, div, vort, &fused);
+    else
+        rc = tendencies_impl<float>(g, g->c32, g->p32, g->s32, g->cc32, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, nullptr,
+                                    nullptr, nullptr, s, div, vort, &fused);
+    if (rc || fused) return rc;
+    return dycore_div_vort(g, dtype, nlev, ldk, vn, div, vort, cuda_stream);
+}
+
 int dycore_step_host(icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
                      const void* vn_host, const void* w_host, void* ddt_vn_host, void* div_host, void* vort_host) {
     int rc = check_common(g, dtype, nlev, ldk, 2);
@@ -730,10 +762,7 @@ int dycore_step_host(icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, co
     const size_t ne = (size_t)g->host.ne, nc = (size_t)g->host.nc, nv = (size_t)g->host.nv;
     CU_TRY(cudaMemcpyAsync(st.vn, vn_host, ne * ldk * es, cudaMemcpyHostToDevice, st.stream));
     CU_TRY(cudaMemcpyAsync(st.w, w_host, nc * ldk_w * es, cudaMemcpyHostToDevice, st.stream));
-    if ((rc = dycore_velocity_tendencies(g, dtype, nlev, ldk, ldk_w, z_half, st.vn, st.w, st.ddt, nullptr, nullptr,
-                                         nullptr, st.stream)))
-        return rc;
-    if ((rc = dycore_div_vort(g, dtype, nlev, ldk, st.vn, st.div, st.vort, st.stream))) return rc;
+    if ((rc = dycore_step(g, dtype, nlev, ldk, ldk_w, z_half, st.vn, st.w, st.ddt, st.div, st.vort, st.stream))) return rc;
     CU_TRY(cudaMemcpyAsync(ddt_vn_host, st.ddt, ne * ldk * es, cudaMemcpyDeviceToHost, st.stream));
     CU_TRY(cudaMemcpyAsync(div_host, st.div, nc * ldk * es, cudaMemcpyDeviceToHost, st.stream));
     CU_TRY(cudaMemcpyAsync(vort_host, st.vort, nv * ldk * es, cudaMemcpyDeviceToHost, st.stream));

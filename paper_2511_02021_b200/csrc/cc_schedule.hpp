@@ -41,12 +41,13 @@ constexpr CcShape kCcShapes[kCcNumShapes] = {{8, 2, 5}, {8, 1, 10}, {8, 1, 9}, {
 inline const CcShape& cc_shape(int i) { return kCcShapes[i >= 0 && i < kCcNumShapes ? i : 0]; }
 constexpr int kCcBarrierBytes = 512;    // the mbarriers
 constexpr int kCcOutCols = 3;            // ddt_vn staging columns per consumer warp (one store batch)
-// a patch record on the device = kScCoefWords coefficients (T), then 8 int32 (user ids of the six
-// owned edges i0 i1 i2 b0 b2 b4, 2 pad), then kCcSlotWords uint32 byte offsets of the slots; c_lin is
+// a patch record on the device = kScCoefWords coefficients (T), then kCcRecordIds int32 (user ids of
+// the outputs), then kCcSlotWords uint32 byte offsets of the slots; c_lin is
 // stored halved there (the kernel forms w(k) + w(k+1) = 2 w_f(k))
 constexpr int kCcSlotWords = 48;     // per patch: 43 slots (order of sc_tables.hpp id slots), mask, pad
 constexpr int kCcMaskWord = 43;      // bit r set: one of the 43 columns was loaded by step s-r (0 < r < depth)
-constexpr int kCcRecordTail = 32 + 4 * kCcSlotWords;
+constexpr int kCcRecordIds = 16;     // int32: owned edges i0 i1 i2 b0 b2 b4, cells T0..T3, owned vertices ab bc ca a b c (-1 = not ours)
+constexpr int kCcRecordTail = 4 * kCcRecordIds + 4 * kCcSlotWords;
 // lanes past the end of a column read up to 3 * 32 levels * 8 bytes beyond their slot: readable pad after the last slot
 constexpr int kCcSlotTailPad = 768;
 

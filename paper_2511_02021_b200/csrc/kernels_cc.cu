@@ -212,10 +212,12 @@ template <class T>
 __host__ __device__ constexpr int cc_record_bytes() { return kScCoefWords * (int)sizeof(T) + kCcRecordTail; }
 
 // W consumer warps in W/G groups of G; group g runs the steps s = g (mod W/G). D = ring depth.
-template <class T, int L, int W, int G, int D>
+// FUSED: the same pass also stores div of the patch's four cells and the vorticity of the vertices the
+// patch owns (dycore_step): both are by-products of columns and sums the tendency needs anyway.
+template <class T, int L, int W, int G, int D, bool FUSED>
 __global__ void __launch_bounds__((W + kCcProducers) * 32, 1)
 k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restrict__ abc, const T* __restrict__ vn,
-          const T* __restrict__ w, T* __restrict__ ddt_vn) {
+          const T* __restrict__ w, T* __restrict__ ddt_vn, T* __restrict__ div, T* __restrict__ vort) {
     extern __shared__ __align__(128) unsigned char smem[];
     using C = Col<T, L>;
     constexpr int REC = cc_record_bytes<T>();
@@ -350,7 +352,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
     bool below_missing[L];   // level k+1 does not exist (k = nlev-1) or belongs to a lane past the column end
     FORL below_missing[l] = L * lane + l + 1 >= nlev;
     const uint64_t pol_first = l2_policy_evict_first();
-    const bool hint_out = hints & 1;
+    const bool hint_out = hints & 1, direct_out = hints & 16;
 
     for (int s = grp; s < n_steps; s += NGRP) {
         const int64_t p = pb + (int64_t)s * G + wi;
@@ -359,7 +361,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
             const unsigned char* rec = rec_base + ((s % D) * G + wi) * REC;
             const T* cf = reinterpret_cast<const T*>(rec);
             const int32_t* oid = reinterpret_cast<const int32_t*>(rec + kScCoefWords * sizeof(T));
-            const uint32_t* sl = reinterpret_cast<const uint32_t*>(rec + kScCoefWords * sizeof(T) + 32);
+            const uint32_t* sl = reinterpret_cast<const uint32_t*>(rec + kScCoefWords * sizeof(T) + kCcRecordIds * 4);
 
             // Every lane reads its natural levels L*lane .. L*lane+L-1, whether they exist or not: the
             // stride-L pattern is conflict free as a whole, lanes past the column end pick up stale
@@ -384,13 +386,39 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
                 FORL o.v[l] = cA[l] * up.v[l] + cB[l] * x.v[l] + cC[l] * dn.v[l];
                 return o;
             };
-            // kCcOutCols finished ddt_vn columns leave together: staged in shared memory (stride-L
-            // writes, conflict free), one proxy fence, then one bulk store each
-            auto ST3 = [&](const int32_t* ids, const C* x) {
+            // Up to kCcOutCols finished output columns leave together: staged in shared memory (stride-L
+            // writes, conflict free), one proxy fence, then one bulk store each; ids[j] < 0 = no column j
+            auto ST3 = [&](T* base, const int32_t* ids, const C* x) {
+                if (direct_out) {
+                    // transposed through the warp's staging columns and written with plain coalesced stores:
+                    // costs L1-pipe wavefronts (read back + store) but no copy-engine request, no proxy fence
+                    // and no wait for the previous batch to be read out
+                    __syncwarp();
+#pragma unroll
+                    for (int j = 0; j < kCcOutCols; ++j) {
+                        if (ids[j] < 0) continue;
+                        T* q = reinterpret_cast<T*>(my_out + j * out_bytes + lane_off);
+                        FORL if (po[l]) q[l] = x[j].v[l];
+                    }
+                    __syncwarp();
+#pragma unroll
+                    for (int j = 0; j < kCcOutCols; ++j) {
+                        if (ids[j] < 0) continue;
+                        const T* q = reinterpret_cast<const T*>(my_out + j * out_bytes);
+                        T* dst = reinterpret_cast<T*>(reinterpret_cast<unsigned char*>(base) + (uint64_t)(uint32_t)ids[j] * cs);
+#pragma unroll
+                        for (int c = 0; c < L; ++c) {
+                            const int k = c * 32 + lane;
+                            if (k < nlev) dst[k] = q[k];
+                        }
+                    }
+                    return;
+                }
                 if (lane == 0) bulk_wait_read<0>();        // the previous batch has been read out of the staging columns
                 __syncwarp();
 #pragma unroll
                 for (int j = 0; j < kCcOutCols; ++j) {
+                    if (ids[j] < 0) continue;
                     T* q = reinterpret_cast<T*>(my_out + j * out_bytes + lane_off);
                     FORL if (po[l]) q[l] = x[j].v[l];
                 }
@@ -399,7 +427,8 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
                 if (lane == 0 && bulk_out > 0) {
 #pragma unroll
                     for (int j = 0; j < kCcOutCols; ++j) {
-                        void* dst = reinterpret_cast<unsigned char*>(ddt_vn) + (uint64_t)(uint32_t)ids[j] * cs;
+                        if (ids[j] < 0) continue;
+                        void* dst = reinterpret_cast<unsigned char*>(base) + (uint64_t)(uint32_t)ids[j] * cs;
                         if (hint_out) bulk_s2g_hint(dst, smem_u32(my_out + j * out_bytes), (uint32_t)bulk_out, pol_first);
                         else bulk_s2g(dst, smem_u32(my_out + j * out_bytes), (uint32_t)bulk_out);
                     }
@@ -408,7 +437,8 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
                 if (bulk_out < nlev * (int)sizeof(T)) {    // the last < 16 bytes of a column go out directly
 #pragma unroll
                     for (int j = 0; j < kCcOutCols; ++j) {
-                        T* dst = reinterpret_cast<T*>(reinterpret_cast<unsigned char*>(ddt_vn) + (uint64_t)(uint32_t)ids[j] * cs);
+                        if (ids[j] < 0) continue;
+                        T* dst = reinterpret_cast<T*>(reinterpret_cast<unsigned char*>(base) + (uint64_t)(uint32_t)ids[j] * cs);
                         FORL if (po[l] && (L * lane + l) * (int)sizeof(T) >= bulk_out) dst[L * lane + l] = x[j].v[l];
                     }
                 }
@@ -430,6 +460,27 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
 #pragma unroll
             for (int j = 0; j < 6; ++j) vB[j] = LD(sE[3 + j]);
 
+            int32_t ido[16];                    // owned edges i0 i1 i2 b0 b2 b4 | cells T0..T3 | vertices ab bc ca a b c (-1 = not ours)
+#pragma unroll
+            for (int i = 0; i < (FUSED ? 4 : 2); ++i) {
+                const int4 a = reinterpret_cast<const int4*>(oid)[i];
+                ido[4 * i] = a.x; ido[4 * i + 1] = a.y; ido[4 * i + 2] = a.z; ido[4 * i + 3] = a.w;
+            }
+            if constexpr (FUSED) {
+                // ---- S1: div of the four cells from their edges (slot order of SCF_BLN) ------------
+                T gd[12];
+                ld_coef(cf + SCF_DIV, gd);
+                C dv[4];
+                FORL {
+                    dv[0].v[l] = gd[0] * vB[0].v[l] + gd[1] * vI[0].v[l] + gd[2] * vB[5].v[l];
+                    dv[1].v[l] = gd[3] * vB[1].v[l] + gd[4] * vB[2].v[l] + gd[5] * vI[1].v[l];
+                    dv[2].v[l] = gd[6] * vI[2].v[l] + gd[7] * vB[3].v[l] + gd[8] * vB[4].v[l];
+                    dv[3].v[l] = gd[9] * vI[1].v[l] + gd[10] * vI[2].v[l] + gd[11] * vI[0].v[l];
+                }
+                const int32_t c3[3] = {ido[6], ido[7], ido[8]}, c1[3] = {ido[9], -1, -1};
+                ST3(div, c3, dv);
+                ST3(div, c1, dv + 3);
+            }
             // ---- interior edges: vt, KE_e; start the cell sums -------------------------------
             T r12[12];
             ld_coef(cf + SCF_RBF, r12);
@@ -508,6 +559,16 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
                     tBo[x] = tB;
                 }
             }
+            if constexpr (FUSED) {
+                // ---- S2: zm, zc hold zeta / 2 at the three midpoints and the three corners ------------
+                C z2[3];
+#pragma unroll
+                for (int m = 0; m < 3; ++m) FORL z2[m].v[l] = (T)2 * zm[m].v[l];
+                ST3(vort, ido + 10, z2);
+#pragma unroll
+                for (int m = 0; m < 3; ++m) FORL z2[m].v[l] = (T)2 * zc[m].v[l];
+                ST3(vort, ido + 13, z2);
+            }
             // ---- horizontal part H of the six owned edges (S5); frees the KE / vorticity columns ----
             T ec[24];
             ld_coef(cf + SCF_EDGE, ec);
@@ -530,11 +591,6 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
             for (int j = 0; j < 4; ++j) wf[j] = WS(sX[12 + j]);
 #pragma unroll
             for (int x = 0; x < 3; ++x) wx[x] = WS(sX[16 + x]);
-            int32_t ido[8];
-            {
-                const int4 a = reinterpret_cast<const int4*>(oid)[0], b = reinterpret_cast<const int4*>(oid)[1];
-                ido[0] = a.x; ido[1] = a.y; ido[2] = a.z; ido[3] = a.w; ido[4] = b.x; ido[5] = b.y; ido[6] = b.z; ido[7] = b.w;
-            }
             // everything this patch needs from the slots and its record is in registers: release the stage
             __syncwarp();
             if (lane == 0) mbar_arrive(done_bar(s % NB));
@@ -553,7 +609,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
                     const T* e4 = ec + 4 * x;
                     FORL o[j].v[l] = -H[x].v[l] - (e4[2] * wl.v[l] + e4[3] * wh.v[l]) * Dv.v[l];
                 }
-                ST3(ido + 3 * h, o);
+                ST3(ddt_vn, ido + 3 * h, o);
             }
         } else {
             __syncwarp();
@@ -588,31 +644,34 @@ template int cc_slot_bytes<float>(int);
 int cc_levels_per_lane(int nlev) { return nlev + 1 <= 32 ? 1 : nlev + 1 <= 96 ? 3 : 0; }
 
 namespace {
-template <class T, int L, int W, int G, int D>
+template <class T, int L, int W, int G, int D, bool FUSED>
 cudaError_t cc_launch_one(const CcDev<T>& d, int n_ctas, size_t smem, int nlev, int ldk, int ldk_w, int hints, const T* abc,
-                          const T* vn, const T* w, T* ddt_vn, cudaStream_t s) {
-    auto k = k_tend_cc<T, L, W, G, D>;
+                          const T* vn, const T* w, T* ddt_vn, T* div, T* vort, cudaStream_t s) {
+    auto k = k_tend_cc<T, L, W, G, D, FUSED>;
     static size_t configured = 0;       // largest dynamic shared-memory size this instantiation was opted in for
     if (smem > configured) {
         cudaError_t err = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (err != cudaSuccess) return err;
         configured = smem;
     }
-    k<<<(unsigned)n_ctas, (W + kCcProducers) * 32, smem, s>>>(d, nlev, ldk, ldk_w, hints, abc, vn, w, ddt_vn);
+    k<<<(unsigned)n_ctas, (W + kCcProducers) * 32, smem, s>>>(d, nlev, ldk, ldk_w, hints, abc, vn, w, ddt_vn, div, vort);
     return cudaGetLastError();
 }
 template <class T, int W, int G, int D>
 cudaError_t cc_launch_shape(int L, const CcDev<T>& d, int n_ctas, size_t smem, int nlev, int ldk, int ldk_w, int hints,
-                            const T* abc, const T* vn, const T* w, T* ddt_vn, cudaStream_t s) {
-    if (L == 1) return cc_launch_one<T, 1, W, G, D>(d, n_ctas, smem, nlev, ldk, ldk_w, hints, abc, vn, w, ddt_vn, s);
-    if (L == 3) return cc_launch_one<T, 3, W, G, D>(d, n_ctas, smem, nlev, ldk, ldk_w, hints, abc, vn, w, ddt_vn, s);
+                            const T* abc, const T* vn, const T* w, T* ddt_vn, T* div, T* vort, cudaStream_t s) {
+    const bool fused = div != nullptr;
+    if (L == 1 && !fused) return cc_launch_one<T, 1, W, G, D, false>(d, n_ctas, smem, nlev, ldk, ldk_w, hints, abc, vn, w, ddt_vn, div, vort, s);
+    if (L == 3 && !fused) return cc_launch_one<T, 3, W, G, D, false>(d, n_ctas, smem, nlev, ldk, ldk_w, hints, abc, vn, w, ddt_vn, div, vort, s);
+    if (L == 1 && fused) return cc_launch_one<T, 1, W, G, D, true>(d, n_ctas, smem, nlev, ldk, ldk_w, hints, abc, vn, w, ddt_vn, div, vort, s);
+    if (L == 3 && fused) return cc_launch_one<T, 3, W, G, D, true>(d, n_ctas, smem, nlev, ldk, ldk_w, hints, abc, vn, w, ddt_vn, div, vort, s);
     return cudaErrorInvalidValue;
 }
 }  // namespace
 
 template <class T>
 int launch_tendencies_cc(const icon_grid& g, const DevCcTables<T>& p, int nlev, int64_t ldk, int64_t ldk_w,
-                         const T* abc, const T* vn, const T* w, T* ddt_vn, cudaStream_t s) {
+                         const T* abc, const T* vn, const T* w, T* ddt_vn, T* div, T* vort, cudaStream_t s) {
     CcDev<T> d;
     d.steps = p.steps; d.loads = p.loads; d.records = p.records;
     d.cta_patch_begin = p.cta_patch_begin; d.cta_step_begin = p.cta_step_begin;
@@ -623,7 +682,7 @@ int launch_tendencies_cc(const icon_grid& g, const DevCcTables<T>& p, int nlev, 
 #define CC_CASE(i, W, G, D)                                                                                        \
     case i:                                                                                                        \
         static_assert(kCcShapes[i].warps == W && kCcShapes[i].group == G && kCcShapes[i].depth == D, "shape table"); \
-        err = cc_launch_shape<T, W, G, D>(L, d, p.n_ctas, smem, nlev, (int)ldk, (int)ldk_w, g.options[ICON_OPT_CC_L2_HINTS], abc, vn, w, ddt_vn, s); \
+        err = cc_launch_shape<T, W, G, D>(L, d, p.n_ctas, smem, nlev, (int)ldk, (int)ldk_w, g.options[ICON_OPT_CC_L2_HINTS], abc, vn, w, ddt_vn, div, vort, s); \
         break;
     switch (p.shape) {
         CC_CASE(0, 8, 2, 5)
@@ -637,8 +696,8 @@ int launch_tendencies_cc(const icon_grid& g, const DevCcTables<T>& p, int nlev, 
 }
 
 template int launch_tendencies_cc<double>(const icon_grid&, const DevCcTables<double>&, int, int64_t, int64_t,
-                                          const double*, const double*, const double*, double*, cudaStream_t);
+                                          const double*, const double*, const double*, double*, double*, double*, cudaStream_t);
 template int launch_tendencies_cc<float>(const icon_grid&, const DevCcTables<float>&, int, int64_t, int64_t,
-                                         const float*, const float*, const float*, float*, cudaStream_t);
+                                         const float*, const float*, const float*, float*, float*, float*, cudaStream_t);
 
 }  // namespace icon

@@ -57,6 +57,19 @@ struct View {
         }
         return true;
     }
+    // geofac_div of cell c re-ordered to the edge slots e[0..2]
+    bool div_row(int32_t c, const int32_t e[3], double out[3]) const {
+        bool used[3] = {false, false, false};
+        for (int s = 0; s < 3; ++s) {
+            int hit = -1;
+            for (int q = 0; q < 3; ++q)
+                if (!used[q] && g.c2e[3 * (int64_t)c + q] == e[s]) { hit = q; break; }
+            if (hit < 0) return false;
+            used[hit] = true;
+            out[s] = g.geofac_div[3 * (int64_t)c + hit];
+        }
+        return true;
+    }
     bool bln_row(int32_t c, const int32_t e[3], double scale, double out[3]) const {
         bool used[3] = {false, false, false};
         for (int s = 0; s < 3; ++s) {
@@ -140,6 +153,11 @@ std::string build_sc_tables(const HostGrid& g, ScTables& t) {
         for (int x = 0; x < 9; ++x) ok &= c.rbf_row(self[x], nb[x], cf + SCF_RBF + 4 * x);
         const int32_t cell_e[4][3] = {{B[0], I[0], B[5]}, {B[1], B[2], I[1]}, {I[2], B[3], B[4]}, {I[1], I[2], I[0]}};
         for (int j = 0; j < 4; ++j) ok &= c.bln_row(L.T[j], cell_e[j], 0.5, cf + SCF_BLN + 3 * j);
+        for (int j = 0; j < 4; ++j) ok &= c.div_row(L.T[j], cell_e[j], cf + SCF_DIV + 3 * j);
+        {
+            const int32_t vs[6] = {L.vab, L.vbc, L.vca, L.va, L.vb, L.vc};
+            for (int j = 0; j < 6; ++j) id[SID_V0 + j] = vs[j];
+        }
         const int32_t midv[3] = {L.vab, L.vbc, L.vca};
         const int32_t fan[3][6] = {{B[0], B[1], I[0], I[1], M[0], M[1]},
                                    {B[2], B[3], I[1], I[2], M[2], M[3]},
@@ -214,6 +232,26 @@ std::string build_sc_tables(const HostGrid& g, ScTables& t) {
         if (!ok) bad = 1;
     }
     if (bad) return "sc tables: the grid is not a 4-child bisection hierarchy with a regular outer ring";
+    // vertex ownership: the lowest patch that has the vertex as a midpoint or a corner stores its vorticity
+    {
+        std::vector<int64_t> owner((size_t)g.nv, np);
+        for (int64_t p = 0; p < np; ++p)
+            for (int j = 0; j < 6; ++j) {
+                const int32_t v = t.ids[(size_t)p * kScIdWords + SID_V0 + j];
+                if (v < 0 || v >= g.nv) return "sc tables: bad vertex id";
+                if (owner[(size_t)v] > p) owner[(size_t)v] = p;
+            }
+        for (int64_t v = 0; v < g.nv; ++v)
+            if (owner[(size_t)v] == np) return "sc tables: a vertex is neither a midpoint nor a corner of any patch";
+#pragma omp parallel for schedule(static)
+        for (int64_t p = 0; p < np; ++p)
+            for (int j = 0; j < 6; ++j) {
+                int32_t& v = t.ids[(size_t)p * kScIdWords + SID_V0 + j];
+                if (owner[(size_t)v] != p) { v = -1; continue; }
+                for (int i = 0; i < j; ++i)          // a pentagon corner may appear twice in one patch? keep the first
+                    if (t.ids[(size_t)p * kScIdWords + SID_V0 + i] == v) { v = -1; break; }
+            }
+    }
     return std::string();
 }
 

@@ -13,6 +13,9 @@
 //   so KE_c(X_j) = bln . (KE_e(b_j), KE_e(om_j), KE_e(oc_j)) and
 //   zeta(C_x)   = rot . (b_j, oc_j, n1, n2, oc_jp, b_jp), jp = (j+5) mod 6, are local.
 //
+// The same columns also give div of the four cells and zeta at the three midpoints and three corners,
+// so a record also carries geofac_div and the vertices the patch owns (every vertex of the grid is
+// a midpoint or a corner of some patch; the lowest patch index owns it) -- dycore_step.
 // 36 edge columns and 7 cell columns per patch; coefficients re-ordered to these fixed slots
 // with the factors 1/2 of KE_e = (vn^2+vt^2)/2 and zeta_e = (zeta(v0)+zeta(v1))/2 folded in
 // (exact: scaling by a power of two commutes with every rounding).
@@ -25,8 +28,8 @@
 
 namespace icon {
 
-constexpr int kScIdWords = 44;      // int32 per patch: 36 edges, 7 cells, 1 pad (176 B)
-constexpr int kScCoefWords = 148;   // floating-point words per patch; every group starts on a multiple of 4 words
+constexpr int kScIdWords = 52;      // int32 per patch: 36 edges, 7 cells, 1 pad, 6 vertices, 2 pad (208 B)
+constexpr int kScCoefWords = 160;   // floating-point words per patch; every group starts on a multiple of 4 words
 
 enum {                // id slots
     SID_I0 = 0,       // i0 i1 i2
@@ -36,7 +39,8 @@ enum {                // id slots
     SID_X0 = 21,      // [3][5]: pm0 pm1 pcf n1 n2 of owned boundary edges b0, b2, b4
     SID_T0 = 36,      // T0..T3
     SID_XC0 = 40,     // X0 X2 X4
-    SID_PAD = 43
+    SID_PAD = 43,
+    SID_V0 = 44       // vertices ab bc ca a b c whose vorticity THIS patch stores (fused step), -1 = another patch does
 };
 enum {                // coefficient slots
     SCF_RBF = 0,      // [9][4] i0 i1 i2 b0..b5, neighbour order of patch_tables.cpp
@@ -47,7 +51,8 @@ enum {                // coefficient slots
     SCF_XRO = 104,   // [3][4] rbf of oc_j over (b_j, om_j, n1, pcf)
     SCF_XBL = 116,    // [3][3] bln of X_j over (b_j, om_j, oc_j) (x 1/2)
     SCF_XROT = 128,   // [3][6] rot of C_x over (b_j, oc_j, n1, n2, oc_jp, b_jp) (x 1/2)
-    SCF_USED = 146
+    SCF_USED = 146,
+    SCF_DIV = 148     // [4][3] geofac_div of T0..T3 over the cell edges in the order of SCF_BLN
 };
 
 struct ScTables {

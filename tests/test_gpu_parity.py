@@ -213,6 +213,71 @@ def test_column_cache_never_reads_a_stale_slot(torch_cuda, lib, oracle_grid, sha
         assert (err <= TOL["f64"] * ref["m_ddt"]).all(), "launch %d" % it
 
 
+@pytest.mark.parametrize("variant", [5, 40, 41, 3])
+@pytest.mark.parametrize("k,seed,flags,nlev,ldk,ldk_w,cfg", [(4, 0, 0, 90, 96, 96, 1), (4, 0, 0, 90, 90, 92, 1), (2, 0, 0, 33, 34, 34, 1),
+                                                         (1, 0, 0, 30, 30, 32, 1), (0, 0, 0, 3, 4, 4, 1),
+                                                         (3, si.PERMUTE_SEED, 1, 40, 40, 42, 4)])
+def test_dycore_step_matches_the_two_calls_and_the_oracle(torch_cuda, lib, oracle_grid, variant, k, seed, flags, nlev, ldk,
+                                                          ldk_w, cfg):
+    """dycore_step: ddt_vn, div and vort from one pass (one fused kernel where kernel 4 runs). Every level of every
+    column of all three outputs is written exactly once (NaN sentinel), pads stay untouched, values match the oracle."""
+    torch = torch_cuda
+    og = oracle_grid(k, seed, flags)
+    g = lib_grid(lib, k, seed, flags)
+    vn, w, zh = si.make_fields(cfg, og.edge_xyz, og.edge_normal, og.nc, nlev=nlev, ldk=ldk, ldk_w=ldk_w, dtype="f64")
+    ref = oracle_reference(og, vn, w, zh, nlev, False)
+    dev = torch.device("cuda:0")
+    d_vn, d_w = torch.from_numpy(vn).to(dev), torch.from_numpy(w).to(dev)
+    sentinel = -4321.25
+    outs = [torch.full((n, ldk), sentinel, dtype=torch.float64, device=dev) for n in (g.ne, g.nc, g.nv)]
+    if variant >= 40:
+        g.set_option(lib.ICON_OPT_CC_SHAPE, variant - 40)
+        variant = 4
+    g.set_option(lib.ICON_OPT_TENDENCY_KERNEL, variant)
+    n0 = g.launch_count
+    lib.dycore_step(g, zh, d_vn, d_w, outs[0], outs[1], outs[2], nlev)
+    torch.cuda.synchronize()
+    launches = g.launch_count - n0
+    fused_regime = variant == 4 or (variant == 5 and 32 <= nlev <= 95)
+    assert launches == (1 if fused_regime else 2)
+    res = dict(ddt_vn=outs[0].cpu().numpy(), div=outs[1].cpu().numpy(), vort=outs[2].cpu().numpy())
+    check_all(res, ref, nlev, TOL["f64"])
+    for name in ("ddt_vn", "div", "vort"):
+        assert (res[name][:, nlev:] == sentinel).all(), name
+        assert not (res[name][:, :nlev] == sentinel).any(), name
+    g.set_option(lib.ICON_OPT_TENDENCY_KERNEL, 5)
+    g.set_option(lib.ICON_OPT_CC_SHAPE, 0)
+
+
+@pytest.mark.parametrize("hints", [0, 3, 16, 19, 31])
+@pytest.mark.parametrize("dtype,nlev,ldk,ldk_w", [("f64", 90, 90, 92), ("f64", 33, 34, 34), ("f32", 90, 92, 92), ("f64", 3, 4, 4)])
+def test_column_cache_store_paths_and_hints(torch_cuda, lib, oracle_grid, hints, dtype, nlev, ldk, ldk_w):
+    """kernel 4: bulk stores (proxy fence, last < 16 bytes of a column stored directly) vs transposed coalesced stores,
+    with and without L2 eviction hints; tendency-only and fused step"""
+    torch = torch_cuda
+    og = oracle_grid(3)
+    g = lib_grid(lib, 3)
+    vn, w, zh = si.make_fields(1 if dtype == "f64" else 4, og.edge_xyz, og.edge_normal, og.nc, nlev=nlev, ldk=ldk, ldk_w=ldk_w,
+                               dtype=dtype)
+    ref = oracle_reference(og, vn, w, zh, nlev, dtype == "f32")
+    g.set_option(lib.ICON_OPT_CC_L2_HINTS, hints)
+    try:
+        res = run_gpu(torch, lib, g, vn, w, zh, nlev, 40, sentinel=-77.5)
+        check_all(res, ref, nlev, TOL[dtype])
+        assert (res["ddt_vn"][:, nlev:] == -77.5).all()
+        dev = torch.device("cuda:0")
+        outs = [torch.full((n, ldk), -77.5, dtype=torch.from_numpy(vn).dtype, device=dev) for n in (g.ne, g.nc, g.nv)]
+        lib.dycore_step(g, zh, torch.from_numpy(vn).to(dev), torch.from_numpy(w).to(dev), outs[0], outs[1], outs[2], nlev)
+        torch.cuda.synchronize()
+        res = dict(ddt_vn=outs[0].cpu().numpy(), div=outs[1].cpu().numpy(), vort=outs[2].cpu().numpy())
+        check_all(res, ref, nlev, TOL[dtype])
+        for name in res:
+            assert (res[name][:, nlev:] == -77.5).all(), name
+    finally:
+        g.set_option(lib.ICON_OPT_CC_L2_HINTS, 19)
+        g.set_option(lib.ICON_OPT_TENDENCY_KERNEL, 5)
+
+
 def test_argument_errors_on_device(torch_cuda, lib):
     torch = torch_cuda
     g = lib_grid(lib, 1)
