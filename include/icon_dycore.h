@@ -93,7 +93,7 @@ enum {
                                      5 = auto (default): 4 for fp64 with 32 <= nlev <= 95, 2 for nlev <= 31,
                                          else 3 (the fastest measured variant of each regime). */
     ICON_OPT_CC_SHAPE = 1,        /* pipeline shape of kernel 4 (consumer warps / patches per step / ring
-                                     depth): 0 = 8/2/5 (default), 1 = 8/1/10, 2 = 8/1/9, 3 = 8/1/11. */
+                                     depth): 0 = 8/2/5 (default), 1 = 8/1/10. */
     ICON_OPT_CC_L2_HINTS = 2,     /* L2 eviction hints of kernel 4, bit mask: 1 = ddt_vn stores evict-first,
                                      2 = patch records evict-first, 4 = vn / w columns evict-last, 16 = outputs leave by
                                      plain coalesced stores (transposed in shared memory) instead of bulk stores.

@@ -36,8 +36,8 @@ constexpr int kCcAhead = 3;              // steps the producers read the schedul
 struct CcShape {
     int warps, group, depth;
 };
-constexpr int kCcNumShapes = 4;
-constexpr CcShape kCcShapes[kCcNumShapes] = {{8, 2, 5}, {8, 1, 10}, {8, 1, 9}, {8, 1, 11}};
+constexpr int kCcNumShapes = 2;
+constexpr CcShape kCcShapes[kCcNumShapes] = {{8, 2, 5}, {8, 1, 10}};
 inline const CcShape& cc_shape(int i) { return kCcShapes[i >= 0 && i < kCcNumShapes ? i : 0]; }
 constexpr int kCcBarrierBytes = 512;    // the mbarriers
 constexpr int kCcOutCols = 3;            // ddt_vn staging columns per consumer warp (one store batch)

@@ -214,7 +214,9 @@ __host__ __device__ constexpr int cc_record_bytes() { return kScCoefWords * (int
 // W consumer warps in W/G groups of G; group g runs the steps s = g (mod W/G). D = ring depth.
 // FUSED: the same pass also stores div of the patch's four cells and the vorticity of the vertices the
 // patch owns (dycore_step): both are by-products of columns and sums the tendency needs anyway.
-template <class T, int L, int W, int G, int D, bool FUSED>
+// DIRECT: outputs leave by coalesced stores (transposed in shared memory) instead of bulk stores; a template
+// parameter because compiling both paths into one kernel overflowed the instruction cache.
+template <class T, int L, int W, int G, int D, bool FUSED, bool DIRECT>
 __global__ void __launch_bounds__((W + kCcProducers) * 32, 1)
 k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restrict__ abc, const T* __restrict__ vn,
           const T* __restrict__ w, T* __restrict__ ddt_vn, T* __restrict__ div, T* __restrict__ vort) {
@@ -352,7 +354,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
     bool below_missing[L];   // level k+1 does not exist (k = nlev-1) or belongs to a lane past the column end
     FORL below_missing[l] = L * lane + l + 1 >= nlev;
     const uint64_t pol_first = l2_policy_evict_first();
-    const bool hint_out = hints & 1, direct_out = hints & 16;
+    const bool hint_out = hints & 1;
 
     for (int s = grp; s < n_steps; s += NGRP) {
         const int64_t p = pb + (int64_t)s * G + wi;
@@ -389,7 +391,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
             // Up to kCcOutCols finished output columns leave together: staged in shared memory (stride-L
             // writes, conflict free), one proxy fence, then one bulk store each; ids[j] < 0 = no column j
             auto ST3 = [&](T* base, const int32_t* ids, const C* x) {
-                if (direct_out) {
+                if constexpr (DIRECT) {
                     // transposed through the warp's staging columns and written with plain coalesced stores:
                     // costs L1-pipe wavefronts (read back + store) but no copy-engine request, no proxy fence
                     // and no wait for the previous batch to be read out
@@ -412,8 +414,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
                             if (k < nlev) dst[k] = q[k];
                         }
                     }
-                    return;
-                }
+                } else {
                 if (lane == 0) bulk_wait_read<0>();        // the previous batch has been read out of the staging columns
                 __syncwarp();
 #pragma unroll
@@ -441,6 +442,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
                         T* dst = reinterpret_cast<T*>(reinterpret_cast<unsigned char*>(base) + (uint64_t)(uint32_t)ids[j] * cs);
                         FORL if (po[l] && (L * lane + l) * (int)sizeof(T) >= bulk_out) dst[L * lane + l] = x[j].v[l];
                     }
+                }
                 }
             };
 
@@ -644,10 +646,10 @@ template int cc_slot_bytes<float>(int);
 int cc_levels_per_lane(int nlev) { return nlev + 1 <= 32 ? 1 : nlev + 1 <= 96 ? 3 : 0; }
 
 namespace {
-template <class T, int L, int W, int G, int D, bool FUSED>
+template <class T, int L, int W, int G, int D, bool FUSED, bool DIRECT>
 cudaError_t cc_launch_one(const CcDev<T>& d, int n_ctas, size_t smem, int nlev, int ldk, int ldk_w, int hints, const T* abc,
                           const T* vn, const T* w, T* ddt_vn, T* div, T* vort, cudaStream_t s) {
-    auto k = k_tend_cc<T, L, W, G, D, FUSED>;
+    auto k = k_tend_cc<T, L, W, G, D, FUSED, DIRECT>;
     static size_t configured = 0;       // largest dynamic shared-memory size this instantiation was opted in for
     if (smem > configured) {
         cudaError_t err = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -660,11 +662,13 @@ cudaError_t cc_launch_one(const CcDev<T>& d, int n_ctas, size_t smem, int nlev, 
 template <class T, int W, int G, int D>
 cudaError_t cc_launch_shape(int L, const CcDev<T>& d, int n_ctas, size_t smem, int nlev, int ldk, int ldk_w, int hints,
                             const T* abc, const T* vn, const T* w, T* ddt_vn, T* div, T* vort, cudaStream_t s) {
-    const bool fused = div != nullptr;
-    if (L == 1 && !fused) return cc_launch_one<T, 1, W, G, D, false>(d, n_ctas, smem, nlev, ldk, ldk_w, hints, abc, vn, w, ddt_vn, div, vort, s);
-    if (L == 3 && !fused) return cc_launch_one<T, 3, W, G, D, false>(d, n_ctas, smem, nlev, ldk, ldk_w, hints, abc, vn, w, ddt_vn, div, vort, s);
-    if (L == 1 && fused) return cc_launch_one<T, 1, W, G, D, true>(d, n_ctas, smem, nlev, ldk, ldk_w, hints, abc, vn, w, ddt_vn, div, vort, s);
-    if (L == 3 && fused) return cc_launch_one<T, 3, W, G, D, true>(d, n_ctas, smem, nlev, ldk, ldk_w, hints, abc, vn, w, ddt_vn, div, vort, s);
+    const bool fused = div != nullptr, direct = (hints & 16) != 0;
+#define CC_ONE(LL, FF, DD) \
+    if (L == LL && fused == FF && direct == DD) \
+        return cc_launch_one<T, LL, W, G, D, FF, DD>(d, n_ctas, smem, nlev, ldk, ldk_w, hints, abc, vn, w, ddt_vn, div, vort, s);
+    CC_ONE(1, false, false) CC_ONE(1, false, true) CC_ONE(1, true, false) CC_ONE(1, true, true)
+    CC_ONE(3, false, false) CC_ONE(3, false, true) CC_ONE(3, true, false) CC_ONE(3, true, true)
+#undef CC_ONE
     return cudaErrorInvalidValue;
 }
 }  // namespace
@@ -687,8 +691,6 @@ int launch_tendencies_cc(const icon_grid& g, const DevCcTables<T>& p, int nlev, 
     switch (p.shape) {
         CC_CASE(0, 8, 2, 5)
         CC_CASE(1, 8, 1, 10)
-        CC_CASE(2, 8, 1, 9)
-        CC_CASE(3, 8, 1, 11)
         default: err = cudaErrorInvalidValue;
     }
 #undef CC_CASE

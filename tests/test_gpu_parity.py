@@ -33,8 +33,8 @@ def lib():
 _libgrids = {}
 
 
-# ICON_OPT_TENDENCY_KERNEL values; 40..43 = kernel 4 (column cache) with ICON_OPT_CC_SHAPE 0..3
-VARIANTS = [0, 1, 2, 3, 40, 41, 42, 43]
+# ICON_OPT_TENDENCY_KERNEL values; 40, 41 = kernel 4 (column cache) with ICON_OPT_CC_SHAPE 0, 1
+VARIANTS = [0, 1, 2, 3, 40, 41]
 
 
 def lib_grid(lib, k, seed=0, flags=0):
@@ -185,7 +185,7 @@ def test_fp32_variant_permuted_r2b4(torch_cuda, lib, oracle_grid, variant):
     check_all(res, ref, 90, TOL["f32"])
 
 
-@pytest.mark.parametrize("shape", [0, 1, 2, 3])
+@pytest.mark.parametrize("shape", [0, 1])
 def test_column_cache_never_reads_a_stale_slot(torch_cuda, lib, oracle_grid, shape):
     """Kernel 4 keeps columns in shared memory across steps. Repeating ONE input hides a read that comes too
     early (the slot still holds the same column from the previous launch), so two different inputs alternate

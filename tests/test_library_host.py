@@ -107,7 +107,7 @@ def test_worklist_covers_the_grid(L, k, seed, flags):
 # replayed by the independent checker of cc_schedule_check.cpp
 # ----------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("k,seed,flags", [(0, 0, 0), (2, 0, 0), (4, 0, 0), (3, 4, 1)])
-@pytest.mark.parametrize("shape", [0, 1, 2, 3])
+@pytest.mark.parametrize("shape", [0, 1])
 def test_cc_schedule_replays_correctly(k, seed, flags, shape):
     g = lib.IconGrid(k, seed, flags | binding.ICON_HOST_ONLY)
     g.set_option(lib.ICON_OPT_CC_SHAPE, shape)
@@ -118,7 +118,7 @@ def test_cc_schedule_replays_correctly(k, seed, flags, shape):
             g.set_option(lib.ICON_OPT_CC_TILE, tile)
             st = g.cc_schedule_check(dtype, nlev, ldk, ldk_w, n_ctas=148, smem_bytes=232448)
             np_ = g.nc // 4
-            group = (2, 1, 1, 1)[shape]
+            group = (2, 1)[shape]
             assert st["ctas"] == min(148, -(-np_ // (tile or group)))
             assert st["steps"] >= -(-np_ // group)
             # every patch needs its 36 + 7 columns at least once per CTA range, never more than 43 per patch
