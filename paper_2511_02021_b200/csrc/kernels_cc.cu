@@ -225,7 +225,9 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
     constexpr int REC = cc_record_bytes<T>();
     constexpr int NGRP = W / G;
     static_assert(W % G == 0 && W % 4 == 0 && D > NGRP && D <= 16, "bad pipeline shape");
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    // the shuffle tells the compiler that the warp index is warp-uniform: branches on it (role, patch in range)
+    // become uniform branches and the shuffles below need no divergence handling
+    const int warp = __shfl_sync(kFull, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
     const int out_bytes = (nlev * (int)sizeof(T) + 15) & ~15;                 // staging column, 16-byte multiple
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem);                       // full[D], done[D]
     unsigned char* rec_base = smem + kCcBarrierBytes;
