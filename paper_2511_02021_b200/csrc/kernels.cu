@@ -14,7 +14,8 @@ namespace {
 constexpr int kWarp = 32;
 
 __device__ __forceinline__ int lane_id() { return threadIdx.x & 31; }
-__device__ __forceinline__ int warp_in_block() { return threadIdx.x >> 5; }
+// through a shuffle so that the compiler knows the value is warp-uniform (uniform branches, no divergence handling)
+__device__ __forceinline__ int warp_in_block() { return __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0); }
 
 template <class T>
 __device__ __forceinline__ T ldg(const T* p) {

@@ -136,7 +136,7 @@ k_tend_patch(PatchDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ 
     const int cell_stride = L.cell_slots() * 64;      // elements per exchange buffer
     const int vert_stride = d.max_vert * 32;
 
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;      // warp-uniform for the compiler
     const int n_chunks = (nlev + 31) >> 5;
     const uint32_t cs = (uint32_t)ldk * (uint32_t)sizeof(T), cs_w = (uint32_t)ldk_w * (uint32_t)sizeof(T);   // column strides in bytes
 

@@ -132,7 +132,7 @@ k_tend_sc(ScDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
     extern __shared__ __align__(16) unsigned char smem[];
     using C = Col<T, L>;
     constexpr int rec = sc_record_bytes<T>();
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;      // warp-uniform for the compiler
     unsigned char* mybuf = smem + warp * 2 * rec;
     const int n_chunks = (nlev + kChunk - 1) / kChunk;
     const uint64_t cs = (uint64_t)ldk * sizeof(T), cs_w = (uint64_t)ldk_w * sizeof(T);
