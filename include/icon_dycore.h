@@ -91,7 +91,8 @@ enum {
                                          asynchronous copies on a host-built schedule; level counts it cannot
                                          hold (nlev > 95) fall back to 3;
                                      5 = auto (default): 4 for fp64 with 32 <= nlev <= 95, 2 for nlev <= 31,
-                                         else 3 (the fastest measured variant of each regime). */
+                                         else 3 (the fastest measured variant of each regime);
+                                         dycore_step takes 4 wherever it can hold the columns (nlev <= 95). */
     ICON_OPT_CC_SHAPE = 1,        /* pipeline shape of kernel 4 (consumer warps / patches per step / ring
                                      depth): 0 = 8/2/5 (default), 1 = 8/1/10. */
     ICON_OPT_CC_L2_HINTS = 2,     /* L2 eviction hints of kernel 4, bit mask: 1 = ddt_vn stores evict-first,

@@ -417,6 +417,8 @@ int tendencies_impl(icon_grid* g, icon::DevCoeffs<T>& c, icon::DevPatchTables<T>
         // three levels of 8-byte columns (33 <= nlev+1 <= 96, fp64); shallow columns are copy-request bound
         // there and go to the exchange patch kernel, 4-byte columns to the self-contained patch kernel
         variant = nlev + 1 <= 32 ? 2 : (sizeof(T) == 8 && icon::cc_levels_per_lane(nlev) == 3) ? 4 : 3;
+        // dycore_step: the fused column-cache pass beats tendency kernel + div_vort kernel in every measured regime
+        if (div_fused && icon::cc_levels_per_lane(nlev) != 0) variant = 4;
     }
     if (variant == 4 && !want_opt) {
         if ((rc = ensure_cc_tables(g, ct, nlev, ldk, ldk_w))) return rc;

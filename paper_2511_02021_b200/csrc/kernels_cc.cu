@@ -1,21 +1,34 @@
-// kernels_cc.cu -- column-cache kernel for the velocity tendency, sm_100a.
+// kernels_cc.cu -- column-cache kernel for the velocity tendency and, fused
+// into the same pass on request, divergence and vorticity (S1, S2: dycore_step), sm_100a.
 //
 // Same arithmetic per patch as kernels_sc.cu (one warp finishes one self-contained patch, lanes =
-// levels, no exchange between warps), but the vn / w columns no longer come through the L1: a
-// PRODUCER warp moves whole columns from HBM into shared-memory slots with bulk asynchronous copies
-// (cp.async.bulk = the 1-D TMA path, completion on an mbarrier), following a schedule the host
-// computed once per grid (cc_schedule.hpp: which column into which slot at which step, Belady
-// replacement). CONSUMER warps read the slots:
+// levels, no exchange between warps), but the vn / w columns no longer come through the L1: four
+// PRODUCER warps (one warpgroup, setmaxnreg down to 40 registers) move whole columns from HBM into
+// shared-memory slots with bulk asynchronous copies (cp.async.bulk = the 1-D TMA path, completion on
+// an mbarrier), following a schedule the host computed once per grid (cc_schedule.hpp: which columns
+// into which slots at which step, Belady replacement, consecutive ids merged into one copy). Eight
+// CONSUMER warps (setmaxnreg up to 232 registers) read the slots:
 //
 //   * every column crosses L2 -> SM once per residency instead of once per patch that touches it
-//     (~14 instead of 43 column fetches per patch), and the fetches are in flight for one or more
-//     whole steps ahead of their readers without holding a single register;
+//     (~15 instead of 43 column fetches per patch), and the fetches are in flight one or more steps
+//     ahead of their readers without holding a single register;
 //   * a lane owns L CONSECUTIVE levels (k = L*lane .. L*lane+L-1; L odd, so the 8-byte stride-L
 //     shared-memory reads are bank-conflict free), so the vertical stencil (S6) needs one shuffle
 //     up and one down per column instead of one pair per 32-level chunk, and a coefficient / slot
 //     lookup, which is warp-uniform, is paid once per L*32 levels;
-//   * ddt_vn columns are assembled in shared memory and leave with a bulk store, so the strided
-//     register layout never turns into uncoalesced global stores.
+//   * output columns are transposed through a per-warp staging column and leave with plain
+//     coalesced streaming stores (DIRECT; the alternative, bulk stores from the staging columns,
+//     costs a proxy fence and a wait for the copy engine to read the previous batch out);
+//   * FUSED: div of the patch's four cells comes from the nine in-patch columns, and the sums zm, zc
+//     the tendency needs ARE half the vorticity at the patch's three midpoint and three corner
+//     vertices; every vertex of the grid is one of those for some patch, the lowest patch stores it.
+//
+// Why four producer warps: issuing one bulk copy is a ~100-cycle serial chain on the uniform datapath
+// (R2UR / ELECT / UBLKCP), and an SM accepts one copy per ~31 cycles at best
+// (profiles/r01_bulk_copy_microbench.md), so the issue is spread over a warpgroup and runs of
+// columns are merged. Why the warp index goes through a shuffle: it makes the role / range branches
+// uniform for the compiler, which removed a third of the instructions (divergence handling around
+// every shuffle) -- the kernel had outgrown the instruction cache.
 //
 // Synchronisation: ring of NB barrier pairs, full[s % NB] (one arrival per producer warp, each
 // announcing the bytes of its share of step s before issuing them; the copies complete it) and done[s % NB] (one arrival per
@@ -413,7 +426,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
 #pragma unroll
                         for (int c = 0; c < L; ++c) {
                             const int k = c * 32 + lane;
-                            if (k < nlev) dst[k] = q[k];
+                            if (k < nlev) __stcs(dst + k, q[k]);       // streaming: outputs should not push halo columns out of L2
                         }
                     }
                 } else {
