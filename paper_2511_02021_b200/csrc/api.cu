@@ -227,7 +227,8 @@ int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev, int64_t ld
     const int shape = g->options[ICON_OPT_CC_SHAPE];
     const bool merge = g->options[ICON_OPT_CC_MERGE] != 0;
     const int tile = g->options[ICON_OPT_CC_TILE];
-    if (p.nlev == nlev && p.shape == shape && p.ldk == ldk && p.ldk_w == ldk_w && p.merge == merge && p.tile == tile &&
+    const bool direct = (g->options[ICON_OPT_CC_L2_HINTS] & 16) != 0;
+    if (p.nlev == nlev && p.shape == shape && p.ldk == ldk && p.ldk_w == ldk_w && p.merge == merge && p.tile == tile && p.direct == direct &&
         (p.ready || p.unsupported))
         return ICON_OK;
     dev_release(g, p.steps); dev_release(g, p.loads); dev_release(g, p.records);
@@ -235,11 +236,11 @@ int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev, int64_t ld
     p = icon::DevCcTables<T>();
     p.nlev = nlev;
     p.shape = shape;
-    p.ldk = ldk; p.ldk_w = ldk_w; p.merge = merge; p.tile = tile;
+    p.ldk = ldk; p.ldk_w = ldk_w; p.merge = merge; p.tile = tile; p.direct = direct;
     const icon::CcShape& sh = icon::cc_shape(shape);
     const icon::CcGeometry geom = cc_geometry<T>(nlev, ldk, ldk_w, merge);
     const int slot_bytes = geom.slot_bytes;
-    const int n_slots_max = icon::cc_max_slots<T>(shape, nlev, slot_bytes, g->smem_optin);
+    const int n_slots_max = icon::cc_max_slots<T>(shape, nlev, slot_bytes, g->smem_optin, direct);
     if (icon::cc_levels_per_lane(nlev) == 0 || nlev * (int)sizeof(T) < 16 || n_slots_max < icon::kScIdWords) {
         p.unsupported = true;
         return ICON_OK;
@@ -661,8 +662,8 @@ int icon_grid_cc_schedule_check(icon_grid_t* g, int dtype, int nlev, int ldk, in
     const bool merge = g->options[ICON_OPT_CC_MERGE] != 0;
     const bool f64 = dtype == ICON_F64;
     const icon::CcGeometry geom = f64 ? cc_geometry<double>(nlev, ldk, ldk_w, merge) : cc_geometry<float>(nlev, ldk, ldk_w, merge);
-    const int n_slots = std::min(65535, f64 ? icon::cc_max_slots<double>(shape, nlev, geom.slot_bytes, smem_bytes)
-                                            : icon::cc_max_slots<float>(shape, nlev, geom.slot_bytes, smem_bytes));
+    const int n_slots = std::min(65535, f64 ? icon::cc_max_slots<double>(shape, nlev, geom.slot_bytes, smem_bytes, (g->options[ICON_OPT_CC_L2_HINTS] & 16) != 0)
+                                            : icon::cc_max_slots<float>(shape, nlev, geom.slot_bytes, smem_bytes, (g->options[ICON_OPT_CC_L2_HINTS] & 16) != 0));
     icon::CcSchedule cs;
     try {
         std::string err = icon::build_cc_schedule(g->sc_host, n_ctas, n_slots, geom, icon::cc_shape(shape).group,

@@ -30,8 +30,8 @@ namespace icon {
 // kCcProducerRegs, consumers grow to kCcConsumerRegs
 // (the pool is what the launch allocated: 384 * 168 = (4 * 40 + 8 * 232) * 32 = 64512 registers).
 constexpr int kCcProducers = 4;
-constexpr int kCcProducerRegs = 40;
-constexpr int kCcConsumerRegs = 232;
+constexpr int kCcProducerRegs = 56;
+constexpr int kCcConsumerRegs = 224;
 constexpr int kCcAhead = 3;              // steps the producers read the schedule ahead; `loads` is padded for it
 struct CcShape {
     int warps, group, depth;

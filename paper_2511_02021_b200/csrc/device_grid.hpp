@@ -88,6 +88,7 @@ struct DevCcTables {
     int64_t ldk = -1, ldk_w = -1;  // column strides the runs were merged for
     bool merge = true;             // ICON_OPT_CC_MERGE it was built with
     int tile = -1;                 // ICON_OPT_CC_TILE it was built with
+    bool direct = true;            // store path (ICON_OPT_CC_L2_HINTS bit 16) the slot count was derived for
     bool ready = false;
     bool unsupported = false;      // this (T, nlev) cannot use the kernel: callers fall back
     int64_t stats[5] = {0, 0, 0, 0, 0};   // steps, steps with reduced depth, vn columns, w columns, bulk copies

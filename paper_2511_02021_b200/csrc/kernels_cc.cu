@@ -245,7 +245,8 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem);                       // full[D], done[D]
     unsigned char* rec_base = smem + kCcBarrierBytes;
     unsigned char* out_base = rec_base + D * G * REC;
-    unsigned char* slot_base = out_base + W * kCcOutCols * out_bytes;
+    constexpr int OUTC = DIRECT ? 1 : kCcOutCols;      // staging columns per consumer warp
+    unsigned char* slot_base = out_base + W * OUTC * out_bytes;
     const uint32_t bar0 = smem_u32(bars);
     auto full_bar = [&](int i) { return bar0 + 8u * (uint32_t)i; };
     // NB >= 2D-1 and >= NGRP+D: see the parity argument in the header comment
@@ -361,7 +362,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
         cB[l] = po[l] ? __ldg(abc + nlev + k) : (T)0;
         cC[l] = po[l] ? __ldg(abc + 2 * nlev + k) : (T)0;
     }
-    unsigned char* my_out = out_base + warp * kCcOutCols * out_bytes;
+    unsigned char* my_out = out_base + warp * OUTC * out_bytes;
     const int bulk_out = (nlev * (int)sizeof(T)) & ~15;       // bytes of a ddt_vn column that leave by bulk store
     const uint64_t cs = (uint64_t)ldk * sizeof(T);
     const uint32_t lane_off = (uint32_t)(L * lane * (int)sizeof(T));
@@ -407,26 +408,22 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
             // writes, conflict free), one proxy fence, then one bulk store each; ids[j] < 0 = no column j
             auto ST3 = [&](T* base, const int32_t* ids, const C* x) {
                 if constexpr (DIRECT) {
-                    // transposed through the warp's staging columns and written with plain coalesced stores:
+                    // transposed through the warp's staging column and written with plain coalesced stores:
                     // costs L1-pipe wavefronts (read back + store) but no copy-engine request, no proxy fence
                     // and no wait for the previous batch to be read out
-                    __syncwarp();
 #pragma unroll
                     for (int j = 0; j < kCcOutCols; ++j) {
                         if (ids[j] < 0) continue;
-                        T* q = reinterpret_cast<T*>(my_out + j * out_bytes + lane_off);
+                        __syncwarp();                       // the previous column has been read back
+                        T* q = reinterpret_cast<T*>(my_out + lane_off);
                         FORL if (po[l]) q[l] = x[j].v[l];
-                    }
-                    __syncwarp();
-#pragma unroll
-                    for (int j = 0; j < kCcOutCols; ++j) {
-                        if (ids[j] < 0) continue;
-                        const T* q = reinterpret_cast<const T*>(my_out + j * out_bytes);
+                        __syncwarp();
+                        const T* r = reinterpret_cast<const T*>(my_out);
                         T* dst = reinterpret_cast<T*>(reinterpret_cast<unsigned char*>(base) + (uint64_t)(uint32_t)ids[j] * cs);
 #pragma unroll
                         for (int c = 0; c < L; ++c) {
                             const int k = c * 32 + lane;
-                            if (k < nlev) __stcs(dst + k, q[k]);       // streaming: outputs should not push halo columns out of L2
+                            if (k < nlev) __stcs(dst + k, r[k]);       // streaming: outputs should not push halo columns out of L2
                         }
                     }
                 } else {
@@ -642,19 +639,20 @@ template <class T>
 int cc_slot_bytes(int nlev) { return (((nlev + 1) * (int)sizeof(T) + 15) & ~15); }
 
 template <class T>
-static size_t cc_fixed_smem(const CcShape& sh, int nlev) {
+static size_t cc_fixed_smem(const CcShape& sh, int nlev, bool direct) {
     const int out_bytes = (nlev * (int)sizeof(T) + 15) & ~15;
-    return kCcBarrierBytes + (size_t)sh.depth * sh.group * cc_record_bytes<T>() + (size_t)sh.warps * kCcOutCols * out_bytes;
+    return kCcBarrierBytes + (size_t)sh.depth * sh.group * cc_record_bytes<T>() +
+           (size_t)sh.warps * (direct ? 1 : kCcOutCols) * out_bytes;
 }
 
 template <class T>
-int cc_max_slots(int shape, int nlev, int slot_bytes, int smem_optin) {
-    const long avail = (long)smem_optin - (long)cc_fixed_smem<T>(cc_shape(shape), nlev) - kCcSlotTailPad;
+int cc_max_slots(int shape, int nlev, int slot_bytes, int smem_optin, bool direct) {
+    const long avail = (long)smem_optin - (long)cc_fixed_smem<T>(cc_shape(shape), nlev, direct) - kCcSlotTailPad;
     if (avail <= 0) return 0;
     return (int)(avail / slot_bytes);
 }
-template int cc_max_slots<double>(int, int, int, int);
-template int cc_max_slots<float>(int, int, int, int);
+template int cc_max_slots<double>(int, int, int, int, bool);
+template int cc_max_slots<float>(int, int, int, int, bool);
 template int cc_slot_bytes<double>(int);
 template int cc_slot_bytes<float>(int);
 
@@ -695,13 +693,14 @@ int launch_tendencies_cc(const icon_grid& g, const DevCcTables<T>& p, int nlev, 
     d.steps = p.steps; d.loads = p.loads; d.records = p.records;
     d.cta_patch_begin = p.cta_patch_begin; d.cta_step_begin = p.cta_step_begin;
     d.n_slots = p.n_slots; d.slot_bytes = p.slot_bytes;
-    const size_t smem = cc_fixed_smem<T>(cc_shape(p.shape), nlev) + (size_t)p.n_slots * p.slot_bytes + kCcSlotTailPad;
+    const bool direct = p.direct;        // the slot count was derived for this store path
+    const size_t smem = cc_fixed_smem<T>(cc_shape(p.shape), nlev, direct) + (size_t)p.n_slots * p.slot_bytes + kCcSlotTailPad;
     const int L = cc_levels_per_lane(nlev);
     cudaError_t err;
 #define CC_CASE(i, W, G, D)                                                                                        \
     case i:                                                                                                        \
         static_assert(kCcShapes[i].warps == W && kCcShapes[i].group == G && kCcShapes[i].depth == D, "shape table"); \
-        err = cc_launch_shape<T, W, G, D>(L, d, p.n_ctas, smem, nlev, (int)ldk, (int)ldk_w, g.options[ICON_OPT_CC_L2_HINTS], abc, vn, w, ddt_vn, div, vort, s); \
+        err = cc_launch_shape<T, W, G, D>(L, d, p.n_ctas, smem, nlev, (int)ldk, (int)ldk_w, (g.options[ICON_OPT_CC_L2_HINTS] & ~16) | (direct ? 16 : 0), abc, vn, w, ddt_vn, div, vort, s); \
         break;
     switch (p.shape) {
         CC_CASE(0, 8, 2, 5)
