@@ -37,7 +37,7 @@ struct CcShape {
     int warps, group, depth;
 };
 constexpr int kCcNumShapes = 2;
-constexpr CcShape kCcShapes[kCcNumShapes] = {{8, 2, 5}, {8, 1, 10}};
+constexpr CcShape kCcShapes[kCcNumShapes] = {{8, 2, 6}, {8, 2, 5}};
 inline const CcShape& cc_shape(int i) { return kCcShapes[i >= 0 && i < kCcNumShapes ? i : 0]; }
 constexpr int kCcBarrierBytes = 512;    // the mbarriers
 constexpr int kCcOutCols = 3;            // ddt_vn staging columns per consumer warp (one store batch)

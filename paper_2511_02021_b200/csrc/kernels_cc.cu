@@ -703,8 +703,8 @@ int launch_tendencies_cc(const icon_grid& g, const DevCcTables<T>& p, int nlev, 
         err = cc_launch_shape<T, W, G, D>(L, d, p.n_ctas, smem, nlev, (int)ldk, (int)ldk_w, (g.options[ICON_OPT_CC_L2_HINTS] & ~16) | (direct ? 16 : 0), abc, vn, w, ddt_vn, div, vort, s); \
         break;
     switch (p.shape) {
-        CC_CASE(0, 8, 2, 5)
-        CC_CASE(1, 8, 1, 10)
+        CC_CASE(0, 8, 2, 6)
+        CC_CASE(1, 8, 2, 5)
         default: err = cudaErrorInvalidValue;
     }
 #undef CC_CASE
