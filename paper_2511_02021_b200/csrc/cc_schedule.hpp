@@ -28,7 +28,7 @@ namespace icon {
 // kCcProducers producer warps (one warpgroup) are added to `warps`; the CTA is launched with
 // 168 registers per thread and re-balances them with setmaxnreg: producers keep
 // kCcProducerRegs, consumers grow to kCcConsumerRegs
-// (the pool is what the launch allocated: 384 * 168 = (4 * 40 + 8 * 232) * 32 = 64512 registers).
+// (the pool is what the launch allocated: 384 * 168 = (4 * 56 + 8 * 224) * 32 = 64512 registers).
 constexpr int kCcProducers = 4;
 constexpr int kCcProducerRegs = 56;
 constexpr int kCcConsumerRegs = 224;

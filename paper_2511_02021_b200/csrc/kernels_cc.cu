@@ -3,11 +3,11 @@
 //
 // Same arithmetic per patch as kernels_sc.cu (one warp finishes one self-contained patch, lanes =
 // levels, no exchange between warps), but the vn / w columns no longer come through the L1: four
-// PRODUCER warps (one warpgroup, setmaxnreg down to 40 registers) move whole columns from HBM into
+// PRODUCER warps (one warpgroup, setmaxnreg down to 56 registers) move whole columns from HBM into
 // shared-memory slots with bulk asynchronous copies (cp.async.bulk = the 1-D TMA path, completion on
 // an mbarrier), following a schedule the host computed once per grid (cc_schedule.hpp: which columns
 // into which slots at which step, Belady replacement, consecutive ids merged into one copy). Eight
-// CONSUMER warps (setmaxnreg up to 232 registers) read the slots:
+// CONSUMER warps (setmaxnreg up to 224 registers) read the slots:
 //
 //   * every column crosses L2 -> SM once per residency instead of once per patch that touches it
 //     (~15 instead of 43 column fetches per patch), and the fetches are in flight one or more steps
