@@ -106,6 +106,24 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def max_over_ranks(seconds, device=None):
+    """the slowest rank's time: every multi-GPU number is the max over ranks (replicas only: no data-path collective,
+    just this one scalar all-reduce after the timed region). Works on any initialised backend (nccl on the GPUs, gloo in
+    the CPU test)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(seconds)
+    tt = torch.tensor([seconds], dtype=torch.float64, device=device)
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    return float(tt.item())
+
+
+def aggregate_value(points_per_rank, seconds_max, world):
+    """whole-job throughput in Gpts/s: `world` independent replicas each finish points_per_rank in seconds_max"""
+    return world * points_per_rank / seconds_max / 1e9
+
+
 def oracle_step_seconds(og, vn, w, zh, nlev, reps):
     ts = []
     for _ in range(reps):
@@ -264,14 +282,9 @@ def run_ours(args):
     barrier()
     t_tend = np.array([e[0].elapsed_time(e[1]) for e in evs2]) * 1e-3
     t_dv = np.array([e[1].elapsed_time(e[2]) for e in evs2]) * 1e-3
-    if world > 1:
-        tt = torch.tensor([t_step], dtype=torch.float64, device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        t_step_max = float(tt.item())
-    else:
-        t_step_max = t_step
+    t_step_max = max_over_ranks(t_step, dev)
     pts = g.ne * nlev
-    value = world * pts / t_step_max / 1e9
+    value = aggregate_value(pts, t_step_max, world)
 
     # end to end through the C-ABI with HOST buffers (pinned), copies inside the timed region
     e2e = None
@@ -288,11 +301,8 @@ def run_ours(args):
             lib.dycore_step_host(g, zh, hv, hw, h_ddt, h_div, h_vort, nlev)
         torch.cuda.synchronize()
         t_e2e = (time.perf_counter() - t0) / n_e2e
-        if world > 1:
-            tt = torch.tensor([t_e2e], dtype=torch.float64, device=dev)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            t_e2e = float(tt.item())
-        e2e = {"value": world * pts / t_e2e / 1e9, "unit": UNIT,
+        t_e2e = max_over_ranks(t_e2e, dev)
+        e2e = {"value": aggregate_value(pts, t_e2e, world), "unit": UNIT,
                "h2d_bytes_per_step": int(hv.numel() + hw.numel()) * gsize,
                "d2h_bytes_per_step": int(h_ddt.numel() + h_div.numel() + h_vort.numel()) * gsize,
                "ms_per_step": t_e2e * 1e3, "steps": n_e2e}
