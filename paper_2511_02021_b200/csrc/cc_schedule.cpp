@@ -277,7 +277,7 @@ std::string build_cc_schedule(const ScTables& sc, int n_ctas, int n_slots, const
     // every producer lane may read one entry of a step's first round without a bounds check
     CcLoad zero;
     zero.id = 0; zero.slot = 0; zero.bytes16_kind = 0;
-    out.loads.insert(out.loads.end(), (size_t)32 * kCcProducers, zero);
+    out.loads.insert(out.loads.end(), (size_t)32 * kCcMaxProducers, zero);
     return std::string();
 }
 

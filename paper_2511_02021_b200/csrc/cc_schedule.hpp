@@ -27,11 +27,18 @@ namespace icon {
 // pipeline shapes of the kernel (kernels_cc.cu): consumer warps, patches per step, ring depth.
 // kCcProducers producer warps (one warpgroup) are added to `warps`; the CTA is launched with
 // 168 registers per thread and re-balances them with setmaxnreg: producers keep
-// kCcProducerRegs, consumers grow to kCcConsumerRegs
+// CcWarps<T>::producer_regs, consumers grow to CcWarps<T>::consumer_regs
 // (the pool is what the launch allocated: 384 * 168 = (4 * 56 + 8 * 224) * 32 = 64512 registers).
-constexpr int kCcProducers = 4;
-constexpr int kCcProducerRegs = 56;
-constexpr int kCcConsumerRegs = 224;
+// 8-byte columns: 4 producer warps with 56 registers, 8 consumer warps with 224 (launch: 384 threads x 168).
+// 4-byte columns: the consumers need fewer registers and the columns are half as long, i.e. twice the copies per byte,
+// so a second producer warpgroup issues them: 8 producer warps with 40 registers, consumers 216 (launch: 512 x 128).
+template <class T>
+struct CcWarps {
+    static constexpr int producers = sizeof(T) == 4 ? 8 : 4;
+    static constexpr int producer_regs = sizeof(T) == 4 ? 40 : 56;
+    static constexpr int consumer_regs = sizeof(T) == 4 ? 216 : 224;
+};
+constexpr int kCcMaxProducers = 8;
 constexpr int kCcAhead = 3;              // steps the producers read the schedule ahead; `loads` is padded for it
 struct CcShape {
     int warps, group, depth;
