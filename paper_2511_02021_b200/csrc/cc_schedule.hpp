@@ -32,11 +32,13 @@ namespace icon {
 // 8-byte columns: 4 producer warps with 56 registers, 8 consumer warps with 224 (launch: 384 threads x 168).
 // 4-byte columns: the consumers need fewer registers and the columns are half as long, i.e. twice the copies per byte,
 // so a second producer warpgroup issues them: 8 producer warps with 40 registers, consumers 216 (launch: 512 x 128).
-template <class T>
+// One level per lane (L = 1, nlev <= 31) is the same case: short columns, light consumers.
+template <class T, int L>
 struct CcWarps {
-    static constexpr int producers = sizeof(T) == 4 ? 8 : 4;
-    static constexpr int producer_regs = sizeof(T) == 4 ? 40 : 56;
-    static constexpr int consumer_regs = sizeof(T) == 4 ? 216 : 224;
+    static constexpr bool light = sizeof(T) == 4 || L == 1;
+    static constexpr int producers = light ? 8 : 4;
+    static constexpr int producer_regs = light ? 40 : 56;
+    static constexpr int consumer_regs = light ? 216 : 224;
 };
 constexpr int kCcMaxProducers = 8;
 constexpr int kCcAhead = 3;              // steps the producers read the schedule ahead; `loads` is padded for it

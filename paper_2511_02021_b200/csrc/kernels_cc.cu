@@ -230,12 +230,12 @@ __host__ __device__ constexpr int cc_record_bytes() { return kScCoefWords * (int
 // DIRECT: outputs leave by coalesced stores (transposed in shared memory) instead of bulk stores; a template
 // parameter because compiling both paths into one kernel overflowed the instruction cache.
 template <class T, int L, int W, int G, int D, bool FUSED, bool DIRECT>
-__global__ void __launch_bounds__((W + CcWarps<T>::producers) * 32, 1)
+__global__ void __launch_bounds__((W + CcWarps<T, L>::producers) * 32, 1)
 k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restrict__ abc, const T* __restrict__ vn,
           const T* __restrict__ w, T* __restrict__ ddt_vn, T* __restrict__ div, T* __restrict__ vort) {
     extern __shared__ __align__(128) unsigned char smem[];
     using C = Col<T, L>;
-    constexpr int kCcProducers = CcWarps<T>::producers;
+    constexpr int kCcProducers = CcWarps<T, L>::producers;
     constexpr int REC = cc_record_bytes<T>();
     constexpr int NGRP = W / G;
     static_assert(W % G == 0 && W % 4 == 0 && D > NGRP && D <= 16, "bad pipeline shape");
@@ -273,7 +273,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
         // ================= producers (one warpgroup) =================
         // Issuing a bulk copy costs a ~100-cycle chain on the uniform datapath, so the list of a
         // step is dealt round-robin to kCcProducers warps. Registers go to the consumers.
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(CcWarps<T>::producer_regs));
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(CcWarps<T, L>::producer_regs));
         // hints: bit 0 = ddt_vn stores evict-first, bit 1 = patch records evict-first, bit 2 = columns evict-last
         const int pw = warp - W;
         const uint64_t cs = (uint64_t)ldk * sizeof(T), cs_w = (uint64_t)ldk_w * sizeof(T);
@@ -349,7 +349,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
         }
         return;
     }
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(CcWarps<T>::consumer_regs));
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(CcWarps<T, L>::consumer_regs));
 
     // ================= consumers =================
     const int grp = warp / G, wi = warp % G;
@@ -670,7 +670,7 @@ cudaError_t cc_launch_one(const CcDev<T>& d, int n_ctas, size_t smem, int nlev, 
         if (err != cudaSuccess) return err;
         configured = smem;
     }
-    k<<<(unsigned)n_ctas, (W + CcWarps<T>::producers) * 32, smem, s>>>(d, nlev, ldk, ldk_w, hints, abc, vn, w, ddt_vn, div, vort);
+    k<<<(unsigned)n_ctas, (W + CcWarps<T, L>::producers) * 32, smem, s>>>(d, nlev, ldk, ldk_w, hints, abc, vn, w, ddt_vn, div, vort);
     return cudaGetLastError();
 }
 template <class T, int W, int G, int D>
