@@ -215,6 +215,8 @@ def run_ours(args):
         g.set_option(lib.ICON_OPT_CC_TILE, args.cc_tile)
     if args.cc_merge is not None:
         g.set_option(lib.ICON_OPT_CC_MERGE, args.cc_merge)
+    if args.cc_pace is not None:
+        g.set_option(lib.ICON_OPT_CC_PACE, args.cc_pace)
     if args.cc_shape is not None:
         g.set_option(lib.ICON_OPT_CC_SHAPE, args.cc_shape)
     t_grid = time.perf_counter() - t0
@@ -362,7 +364,7 @@ def run_ours(args):
                        "ldk": ldk, "ldk_w": ldk_w, "step": "dycore_step (ddt_vn + div + vort; one fused kernel)" if fused else "dycore_step = dycore_velocity_tendencies + dycore_div_vort",
                        "l2": "flushed between iterations" if l2_flush is not None else "inputs larger than L2",
                        "parallelism": "replicas only" if world > 1 else "single GPU",
-                       "tendency_kernel_variant": args.variant, "cc_shape": args.cc_shape, "cc_hints": args.cc_hints, "cc_tile": args.cc_tile, "cc_merge": args.cc_merge, "grid_create_s": t_grid},
+                       "tendency_kernel_variant": args.variant, "cc_shape": args.cc_shape, "cc_hints": args.cc_hints, "cc_tile": args.cc_tile, "cc_pace": args.cc_pace, "cc_merge": args.cc_merge, "grid_create_s": t_grid},
             "gpts_tendency_call_only": pts / t_tend_avg / 1e9,
             "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": int(launches),
             "clocks": clocks}
@@ -384,6 +386,7 @@ def main():
     ap.add_argument("--cc-hints", type=int, default=None, dest="cc_hints", help="ICON_OPT_CC_L2_HINTS override")
     ap.add_argument("--cc-tile", type=int, default=None, dest="cc_tile", help="ICON_OPT_CC_TILE override")
     ap.add_argument("--cc-merge", type=int, default=None, dest="cc_merge", help="ICON_OPT_CC_MERGE override")
+    ap.add_argument("--cc-pace", type=int, default=None, dest="cc_pace", help="ICON_OPT_CC_PACE override")
     ap.add_argument("--ldk", type=int, default=0, help="leading dimension of vn/ddt_vn/div/vort (default: padded to 128 B)")
     ap.add_argument("--ldk-w", type=int, default=0, dest="ldk_w")
     ap.add_argument("--no-e2e", action="store_true")

@@ -105,6 +105,9 @@ enum {
                                      b, b + #CTAs, ... so that neighbouring tiles are in flight together and share
                                      their halo columns through the L2); even; 0 = one contiguous range per CTA.
                                      Default 16. */
+    ICON_OPT_CC_PACE = 5,         /* kernel 4: the producers of all CTAs meet every this many steps (power of two; bounded
+                                     wait) so that the CTAs do not drift rounds apart and neighbouring tiles keep sharing
+                                     halo columns through the L2; 0 = never. Default 512; fused step (dycore_step) only. */
     ICON_OPT_COUNT
 };
 

@@ -22,6 +22,7 @@ ICON_OPT_CC_SHAPE = 1
 ICON_OPT_CC_L2_HINTS = 2
 ICON_OPT_CC_MERGE = 3
 ICON_OPT_CC_TILE = 4
+ICON_OPT_CC_PACE = 5
 
 TABLES = ("c2v", "c2e", "e2c", "e2v", "e2e4", "v2e", "v2c", "v_deg", "c_os", "v_os",
           "vert_xyz", "cell_xyz", "edge_xyz", "edge_normal", "l_e", "d_e", "inv_d_e", "f_e", "c_lin", "rbf",

@@ -232,7 +232,7 @@ int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev, int64_t ld
         (p.ready || p.unsupported))
         return ICON_OK;
     dev_release(g, p.steps); dev_release(g, p.loads); dev_release(g, p.records);
-    dev_release(g, p.cta_patch_begin); dev_release(g, p.cta_step_begin);
+    dev_release(g, p.cta_patch_begin); dev_release(g, p.cta_step_begin); dev_release(g, p.progress);
     p = icon::DevCcTables<T>();
     p.nlev = nlev;
     p.shape = shape;
@@ -291,6 +291,9 @@ int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev, int64_t ld
     if ((rc = upload_vec(g, cs.cta_patch_begin, &p.cta_patch_begin))) return rc;
     if ((rc = upload_vec(g, cs.cta_step_begin, &p.cta_step_begin))) return rc;
     p.n_ctas = cs.n_ctas; p.n_slots = cs.n_slots; p.slot_bytes = slot_bytes;
+    for (int b = 0; b < cs.n_ctas; ++b) p.cta_steps.push_back(cs.cta_step_begin[(size_t)b + 1] - cs.cta_step_begin[(size_t)b]);
+    if ((rc = dev_alloc(g, 1, &p.progress))) return rc;
+    CU_TRY(cudaMemset(p.progress, 0, sizeof(unsigned long long)));
     p.stats[0] = (int64_t)cs.steps.size(); p.stats[1] = cs.n_sync_steps; p.stats[2] = cs.n_vn_loads; p.stats[3] = cs.n_w_loads; p.stats[4] = cs.n_copies;
     p.ready = true;
     return ICON_OK;
@@ -518,6 +521,7 @@ int icon_grid_create(int bisections_k, uint64_t seed, unsigned flags, icon_grid_
     g->options[ICON_OPT_CC_L2_HINTS] = 19;
     g->options[ICON_OPT_CC_MERGE] = 1;
     g->options[ICON_OPT_CC_TILE] = 16;
+    g->options[ICON_OPT_CC_PACE] = 512;
     try {
         std::string err = icon::build_host_grid(bisections_k, seed, (flags & ICON_PERMUTE) != 0, g->host);
         if (!err.empty()) {
@@ -621,6 +625,7 @@ int icon_grid_table_device(icon_grid_t* g, int which, int dtype, const void** dp
 int icon_grid_set_option(icon_grid_t* g, int option, int value) {
     if (!g) return fail(ICON_EINVAL, "grid handle is NULL");
     if (option < 0 || option >= ICON_OPT_COUNT) return fail(ICON_EINVAL, "unknown option");
+    if (option == ICON_OPT_CC_PACE && (value < 0 || value > 65536 || (value & (value - 1)))) return fail(ICON_EINVAL, "bad option value");
     if (option == ICON_OPT_CC_TILE && (value < 0 || value > 4096 || value % 2)) return fail(ICON_EINVAL, "bad option value");
     if (option == ICON_OPT_CC_L2_HINTS && (value < 0 || value > 31)) return fail(ICON_EINVAL, "bad option value");
     if (option == ICON_OPT_CC_SHAPE && (value < 0 || value >= icon::kCcNumShapes)) return fail(ICON_EINVAL, "bad option value");

@@ -88,6 +88,10 @@ struct DevCcTables {
     int64_t ldk = -1, ldk_w = -1;  // column strides the runs were merged for
     bool merge = true;             // ICON_OPT_CC_MERGE it was built with
     int tile = -1;                 // ICON_OPT_CC_TILE it was built with
+    unsigned long long* progress = nullptr;   // device counter of the producers' pacing barriers, never reset
+    int64_t pace_events = 0;       // value of *progress once every launch so far has finished
+    int64_t max_steps = 0;
+    std::vector<int64_t> cta_steps;           // steps of every CTA
     bool direct = true;            // store path (ICON_OPT_CC_L2_HINTS bit 16) the slot count was derived for
     bool ready = false;
     bool unsupported = false;      // this (T, nlev) cannot use the kernel: callers fall back

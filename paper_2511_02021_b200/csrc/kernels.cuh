@@ -43,7 +43,7 @@ int launch_tendencies_sc(const icon_grid& g, const DevScTables<T>& p, int nlev, 
 // (cc_schedule.hpp); consumer warps finish one self-contained patch each from the slots. With div and
 // vort non-NULL the same pass also stores S1 and S2 (dycore_step); NULL = tendency only.
 template <class T>
-int launch_tendencies_cc(const icon_grid& g, const DevCcTables<T>& p, int nlev, int64_t ldk, int64_t ldk_w,
+int launch_tendencies_cc(const icon_grid& g, DevCcTables<T>& p, int nlev, int64_t ldk, int64_t ldk_w,
                          const T* abc, const T* vn, const T* w, T* ddt_vn, T* div, T* vort, cudaStream_t s);
 // shape helpers of that kernel: levels per lane (0 = nlev not supported), bytes of one w column
 // (the smallest possible slot), and how many slots of `slot_bytes` fit beside the fixed buffers in `smem_optin` bytes of shared memory

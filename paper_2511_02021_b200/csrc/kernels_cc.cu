@@ -232,7 +232,8 @@ __host__ __device__ constexpr int cc_record_bytes() { return kScCoefWords * (int
 template <class T, int L, int W, int G, int D, bool FUSED, bool DIRECT>
 __global__ void __launch_bounds__((W + CcWarps<T, L>::producers) * 32, 1)
 k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restrict__ abc, const T* __restrict__ vn,
-          const T* __restrict__ w, T* __restrict__ ddt_vn, T* __restrict__ div, T* __restrict__ vort) {
+          const T* __restrict__ w, T* __restrict__ ddt_vn, T* __restrict__ div, T* __restrict__ vort,
+          unsigned long long* pace_counter, unsigned long long pace_base, int pace_mask, int pace_last) {
     extern __shared__ __align__(128) unsigned char smem[];
     using C = Col<T, L>;
     constexpr int kCcProducers = CcWarps<T, L>::producers;
@@ -311,6 +312,25 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
                         e[u] = __ldg(lraw + ahead_begin + mine);
                     }
                     const int n_loads = (int)n_loads_u;
+                    // compiled into the fused fp64 three-levels-per-lane kernel only: the tendency-only kernel lost 3 %
+                    // to the mere presence of this block, and the light instantiations (fp32, one level per lane)
+                    // slowed down by 40-50 % with the barrier active
+                    if (FUSED && !CcWarps<T, L>::light && pace_mask && s && (s & pace_mask) == 0 && s <= pace_last) {
+                        // every pace_mask + 1 steps the producers of all CTAs meet (bounded wait: pacing is an
+                        // optimisation, never a condition for progress): SMs run at slightly different rates, and once
+                        // the CTAs are rounds apart neighbouring tiles no longer share their halo columns through the L2
+                        if (lane == 0) {
+                            if (pw == 0) asm volatile("red.relaxed.gpu.global.add.u64 [%0], 1;" ::"l"(pace_counter) : "memory");
+                            const unsigned long long need = pace_base + (unsigned long long)(s / (pace_mask + 1)) * gridDim.x;
+                            for (int spin = 0; spin < (1 << 15); ++spin) {
+                                unsigned long long have;
+                                asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(have) : "l"(pace_counter) : "memory");
+                                if (have >= need) break;
+                                __nanosleep(200);
+                            }
+                        }
+                        __syncwarp();
+                    }
                     while (drained < s - (int)depth + 1) {
                         mbar_wait(done_bar(drained % NB), (uint32_t)((drained / NB) & 1), 1, s);
                         ++drained;
@@ -662,7 +682,8 @@ int cc_levels_per_lane(int nlev) { return nlev + 1 <= 32 ? 1 : nlev + 1 <= 96 ? 
 namespace {
 template <class T, int L, int W, int G, int D, bool FUSED, bool DIRECT>
 cudaError_t cc_launch_one(const CcDev<T>& d, int n_ctas, size_t smem, int nlev, int ldk, int ldk_w, int hints, const T* abc,
-                          const T* vn, const T* w, T* ddt_vn, T* div, T* vort, cudaStream_t s) {
+                          const T* vn, const T* w, T* ddt_vn, T* div, T* vort, unsigned long long* pc, unsigned long long pb, int pm, int pl,
+                          cudaStream_t s) {
     auto k = k_tend_cc<T, L, W, G, D, FUSED, DIRECT>;
     static size_t configured = 0;       // largest dynamic shared-memory size this instantiation was opted in for
     if (smem > configured) {
@@ -670,16 +691,17 @@ cudaError_t cc_launch_one(const CcDev<T>& d, int n_ctas, size_t smem, int nlev, 
         if (err != cudaSuccess) return err;
         configured = smem;
     }
-    k<<<(unsigned)n_ctas, (W + CcWarps<T, L>::producers) * 32, smem, s>>>(d, nlev, ldk, ldk_w, hints, abc, vn, w, ddt_vn, div, vort);
+    k<<<(unsigned)n_ctas, (W + CcWarps<T, L>::producers) * 32, smem, s>>>(d, nlev, ldk, ldk_w, hints, abc, vn, w, ddt_vn, div, vort, pc, pb, pm, pl);
     return cudaGetLastError();
 }
 template <class T, int W, int G, int D>
 cudaError_t cc_launch_shape(int L, const CcDev<T>& d, int n_ctas, size_t smem, int nlev, int ldk, int ldk_w, int hints,
-                            const T* abc, const T* vn, const T* w, T* ddt_vn, T* div, T* vort, cudaStream_t s) {
+                            const T* abc, const T* vn, const T* w, T* ddt_vn, T* div, T* vort, unsigned long long* pc,
+                            unsigned long long pb, int pm, int pl, cudaStream_t s) {
     const bool fused = div != nullptr, direct = (hints & 16) != 0;
 #define CC_ONE(LL, FF, DD) \
     if (L == LL && fused == FF && direct == DD) \
-        return cc_launch_one<T, LL, W, G, D, FF, DD>(d, n_ctas, smem, nlev, ldk, ldk_w, hints, abc, vn, w, ddt_vn, div, vort, s);
+        return cc_launch_one<T, LL, W, G, D, FF, DD>(d, n_ctas, smem, nlev, ldk, ldk_w, hints, abc, vn, w, ddt_vn, div, vort, pc, pb, pm, pl, s);
     CC_ONE(1, false, false) CC_ONE(1, false, true) CC_ONE(1, true, false) CC_ONE(1, true, true)
     CC_ONE(3, false, false) CC_ONE(3, false, true) CC_ONE(3, true, false) CC_ONE(3, true, true)
 #undef CC_ONE
@@ -688,12 +710,21 @@ cudaError_t cc_launch_shape(int L, const CcDev<T>& d, int n_ctas, size_t smem, i
 }  // namespace
 
 template <class T>
-int launch_tendencies_cc(const icon_grid& g, const DevCcTables<T>& p, int nlev, int64_t ldk, int64_t ldk_w,
+int launch_tendencies_cc(const icon_grid& g, DevCcTables<T>& p, int nlev, int64_t ldk, int64_t ldk_w,
                          const T* abc, const T* vn, const T* w, T* ddt_vn, T* div, T* vort, cudaStream_t s) {
     CcDev<T> d;
     d.steps = p.steps; d.loads = p.loads; d.records = p.records;
     d.cta_patch_begin = p.cta_patch_begin; d.cta_step_begin = p.cta_step_begin;
     d.n_slots = p.n_slots; d.slot_bytes = p.slot_bytes;
+    // pacing: a barrier of the producers every `period` steps (power of two), counted in p.progress (never reset)
+    const int period = g.options[ICON_OPT_CC_PACE];
+    const bool heavy = sizeof(T) == 8 && cc_levels_per_lane(nlev) == 3;
+    const int pace_mask = period > 0 && p.progress && div != nullptr && heavy ? period - 1 : 0;      // fused fp64 step only
+    int64_t min_steps = 1 << 30;
+    for (int64_t n : p.cta_steps) min_steps = n < min_steps ? n : min_steps;
+    const int n_barriers = pace_mask ? (int)((min_steps - 1) / period) : 0;      // barriers every CTA reaches
+    const int pace_last = n_barriers * period;
+    const unsigned long long pace_base = (unsigned long long)p.pace_events;
     const bool direct = p.direct;        // the slot count was derived for this store path
     const size_t smem = cc_fixed_smem<T>(cc_shape(p.shape), nlev, direct) + (size_t)p.n_slots * p.slot_bytes + kCcSlotTailPad;
     const int L = cc_levels_per_lane(nlev);
@@ -701,7 +732,7 @@ int launch_tendencies_cc(const icon_grid& g, const DevCcTables<T>& p, int nlev, 
 #define CC_CASE(i, W, G, D)                                                                                        \
     case i:                                                                                                        \
         static_assert(kCcShapes[i].warps == W && kCcShapes[i].group == G && kCcShapes[i].depth == D, "shape table"); \
-        err = cc_launch_shape<T, W, G, D>(L, d, p.n_ctas, smem, nlev, (int)ldk, (int)ldk_w, (g.options[ICON_OPT_CC_L2_HINTS] & ~16) | (direct ? 16 : 0), abc, vn, w, ddt_vn, div, vort, s); \
+        err = cc_launch_shape<T, W, G, D>(L, d, p.n_ctas, smem, nlev, (int)ldk, (int)ldk_w, (g.options[ICON_OPT_CC_L2_HINTS] & ~16) | (direct ? 16 : 0), abc, vn, w, ddt_vn, div, vort, p.progress, pace_base, pace_mask, pace_last, s); \
         break;
     switch (p.shape) {
         CC_CASE(0, 8, 2, 6)
@@ -709,12 +740,16 @@ int launch_tendencies_cc(const icon_grid& g, const DevCcTables<T>& p, int nlev, 
         default: err = cudaErrorInvalidValue;
     }
 #undef CC_CASE
+    if (err == cudaSuccess && pace_mask) {
+        // every CTA adds one event per barrier it reaches: barriers k = 1 .. (its steps - 1) / period
+        p.pace_events += (int64_t)n_barriers * p.n_ctas;
+    }
     return err == cudaSuccess ? 1 : -(int)err;
 }
 
-template int launch_tendencies_cc<double>(const icon_grid&, const DevCcTables<double>&, int, int64_t, int64_t,
+template int launch_tendencies_cc<double>(const icon_grid&, DevCcTables<double>&, int, int64_t, int64_t,
                                           const double*, const double*, const double*, double*, double*, double*, cudaStream_t);
-template int launch_tendencies_cc<float>(const icon_grid&, const DevCcTables<float>&, int, int64_t, int64_t,
+template int launch_tendencies_cc<float>(const icon_grid&, DevCcTables<float>&, int, int64_t, int64_t,
                                          const float*, const float*, const float*, float*, float*, float*, cudaStream_t);
 
 }  // namespace icon
