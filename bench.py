@@ -351,7 +351,7 @@ def run_ours(args):
         og, ovn, ow, ozh, onlev = oracle_sample(args.config, k_sample)
         oracle_step_seconds(og, ovn, ow, ozh, onlev, 1)
         ts, t_begin = [], time.perf_counter()
-        while len(ts) < 3 or (time.perf_counter() - t_begin < 10.0 and len(ts) < 50):
+        while len(ts) < 3 or (time.perf_counter() - t_begin < 12.0 and len(ts) < 400):
             ts += oracle_step_seconds(og, ovn, ow, ozh, onlev, 1)
         cpu_baseline = {"value": og.ne * onlev / float(np.mean(ts)) / 1e9, "unit": UNIT, "cores": cpu_threads(), "kind": "oracle",
                         "sample": "R2B%d x %d levels fp64 oracle, %d timed steps (%.1f s), same field recipe" % (

@@ -249,6 +249,40 @@ def test_dycore_step_matches_the_two_calls_and_the_oracle(torch_cuda, lib, oracl
     g.set_option(lib.ICON_OPT_CC_SHAPE, 0)
 
 
+@pytest.mark.parametrize("period", [0, 4, 16, 512])
+def test_fused_step_pacing_barrier_periods(torch_cuda, lib, oracle_grid, period):
+    """The fused fp64 kernel's producers meet at a chip-wide counter every `period` steps (ICON_OPT_CC_PACE; DESIGN.md
+    section 6.1). The counter's base advances from launch to launch, so several launches run back to back on alternating
+    inputs; every one is compared with the oracle. R2B5 gives each CTA ~70 steps: periods 4 and 16 arm many barriers,
+    512 arms none, 0 switches pacing off."""
+    torch = torch_cuda
+    og = oracle_grid(5)
+    g = lib_grid(lib, 5)
+    dev = torch.device("cuda:0")
+    nlev = 90
+    sets = []
+    for cfg, fv in ((1, 1.0), (2, -2.0)):
+        vn, w, zh = si.make_fields(cfg, og.edge_xyz, og.edge_normal, og.nc, nlev=nlev, ldk=96, ldk_w=96)
+        vn, w = np.nan_to_num(vn) * fv, np.nan_to_num(w)
+        ref = oracle_reference(og, vn, w, zh, nlev, False)
+        sets.append((torch.from_numpy(vn).to(dev), torch.from_numpy(w).to(dev), zh, ref))
+    g.set_option(lib.ICON_OPT_TENDENCY_KERNEL, 5)
+    g.set_option(lib.ICON_OPT_CC_SHAPE, 0)
+    g.set_option(lib.ICON_OPT_CC_PACE, period)
+    try:
+        for it in range(6):
+            d_vn, d_w, zh, ref = sets[it % 2]
+            outs = [torch.full((n, 96), float("nan"), dtype=torch.float64, device=dev) for n in (g.ne, g.nc, g.nv)]
+            n0 = g.launch_count
+            lib.dycore_step(g, zh, d_vn, d_w, outs[0], outs[1], outs[2], nlev)
+            torch.cuda.synchronize()
+            assert g.launch_count - n0 == 1
+            res = dict(ddt_vn=outs[0].cpu().numpy(), div=outs[1].cpu().numpy(), vort=outs[2].cpu().numpy())
+            check_all(res, ref, nlev, TOL["f64"])
+    finally:
+        g.set_option(lib.ICON_OPT_CC_PACE, 512)
+
+
 @pytest.mark.parametrize("hints", [0, 3, 16, 19, 31])
 @pytest.mark.parametrize("dtype,nlev,ldk,ldk_w", [("f64", 90, 90, 92), ("f64", 33, 34, 34), ("f32", 90, 92, 92), ("f64", 3, 4, 4)])
 def test_column_cache_store_paths_and_hints(torch_cuda, lib, oracle_grid, hints, dtype, nlev, ldk, ldk_w):
