@@ -435,15 +435,6 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
 #pragma unroll
                     for (int j = 0; j < kCcOutCols; ++j) {
                         if (ids[j] < 0) continue;
-#ifdef CC_STORE_REG
-                        // experiment: no transposition, every lane stores its own L consecutive levels (stride-L
-                        // 8-byte stores: L1 sees L * sizeof(T) * 32 / 128 lines per instruction instead of 1-2)
-                        {
-                            T* dst = reinterpret_cast<T*>(reinterpret_cast<unsigned char*>(base) + (uint64_t)(uint32_t)ids[j] * cs);
-                            FORL if (po[l]) __stcs(dst + L * lane + l, x[j].v[l]);
-                            continue;
-                        }
-#endif
                         __syncwarp();                       // the previous column has been read back
                         T* q = reinterpret_cast<T*>(my_out + lane_off);
                         FORL if (po[l]) q[l] = x[j].v[l];
