@@ -736,7 +736,7 @@ int launch_tendencies_cc(const icon_grid& g, DevCcTables<T>& p, int nlev, int64_
         break;
     switch (p.shape) {
         CC_CASE(0, 8, 2, 6)
-        CC_CASE(1, 8, 2, 5)
+        CC_CASE(1, 8, CC_S1_G, CC_S1_D)
         default: err = cudaErrorInvalidValue;
     }
 #undef CC_CASE
