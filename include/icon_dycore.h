@@ -94,7 +94,8 @@ enum {
                                          else 3 (the fastest measured variant of each regime);
                                          dycore_step takes 4 wherever it can hold the columns (nlev <= 95). */
     ICON_OPT_CC_SHAPE = 1,        /* pipeline shape of kernel 4 (consumer warps / patches per step / ring
-                                     depth): 0 = 8/2/6 (default), 1 = 8/2/5. */
+                                     depth): 0 = 8/2/6, 1 = 8/4/3, -1 = auto (default) = 1, the faster one
+                                     in every measured regime. */
     ICON_OPT_CC_L2_HINTS = 2,     /* L2 eviction hints of kernel 4, bit mask: 1 = ddt_vn stores evict-first,
                                      2 = patch records evict-first, 4 = vn / w columns evict-last, 16 = outputs leave by
                                      plain coalesced stores (transposed in shared memory) instead of bulk stores.

@@ -219,12 +219,19 @@ icon::CcGeometry cc_geometry(int nlev, int64_t ldk, int64_t ldk_w, bool merge) {
     return geom;
 }
 
+// ICON_OPT_CC_SHAPE -1 = auto = 8/4/3 (four patches per step): the faster shape of every instantiation, measured
+// (config 3 5.11 -> 4.91 ms, config 4 4.01 -> 3.38 ms, config 5 12.25 -> 9.84 ms)
+static int cc_resolve_shape(const icon_grid* g, bool /*f64*/, int /*nlev*/) {
+    const int opt = g->options[ICON_OPT_CC_SHAPE];
+    return opt >= 0 ? opt : 1;
+}
+
 // Column-cache schedule + patch records for (T, nlev): built on the host once, uploaded once.
 // Returns ICON_OK with p.unsupported set when this (T, nlev) cannot use the kernel (the caller
 // then uses the self-contained patch kernel).
 template <class T>
 int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev, int64_t ldk, int64_t ldk_w) {
-    const int shape = g->options[ICON_OPT_CC_SHAPE];
+    const int shape = cc_resolve_shape(g, sizeof(T) == 8, nlev);
     const bool merge = g->options[ICON_OPT_CC_MERGE] != 0;
     const int tile = g->options[ICON_OPT_CC_TILE];
     const bool direct = (g->options[ICON_OPT_CC_L2_HINTS] & 16) != 0;
@@ -518,6 +525,7 @@ int icon_grid_create(int bisections_k, uint64_t seed, unsigned flags, icon_grid_
     g->seed = seed;
     g->host_only = (flags & ICON_HOST_ONLY) != 0;
     g->options[ICON_OPT_TENDENCY_KERNEL] = 5;
+    g->options[ICON_OPT_CC_SHAPE] = -1;
     g->options[ICON_OPT_CC_L2_HINTS] = 19;
     g->options[ICON_OPT_CC_MERGE] = 1;
     g->options[ICON_OPT_CC_TILE] = 16;
@@ -628,7 +636,7 @@ int icon_grid_set_option(icon_grid_t* g, int option, int value) {
     if (option == ICON_OPT_CC_PACE && (value < 0 || value > 65536 || (value & (value - 1)))) return fail(ICON_EINVAL, "bad option value");
     if (option == ICON_OPT_CC_TILE && (value < 0 || value > 4096 || value % 2)) return fail(ICON_EINVAL, "bad option value");
     if (option == ICON_OPT_CC_L2_HINTS && (value < 0 || value > 31)) return fail(ICON_EINVAL, "bad option value");
-    if (option == ICON_OPT_CC_SHAPE && (value < 0 || value >= icon::kCcNumShapes)) return fail(ICON_EINVAL, "bad option value");
+    if (option == ICON_OPT_CC_SHAPE && (value < -1 || value >= icon::kCcNumShapes)) return fail(ICON_EINVAL, "bad option value");
     if (option == ICON_OPT_TENDENCY_KERNEL && (value < 0 || value > 5)) return fail(ICON_EINVAL, "bad option value");
     g->options[option] = value;
     return ICON_OK;
@@ -663,9 +671,9 @@ int icon_grid_cc_schedule_check(icon_grid_t* g, int dtype, int nlev, int ldk, in
     if (icon::cc_levels_per_lane(nlev) == 0) return fail(ICON_EUNSUPPORTED, "nlev not supported by the column-cache kernel");
     int rc = ensure_sc_host(g);
     if (rc) return rc;
-    const int shape = g->options[ICON_OPT_CC_SHAPE];
-    const bool merge = g->options[ICON_OPT_CC_MERGE] != 0;
     const bool f64 = dtype == ICON_F64;
+    const int shape = cc_resolve_shape(g, f64, nlev);
+    const bool merge = g->options[ICON_OPT_CC_MERGE] != 0;
     const icon::CcGeometry geom = f64 ? cc_geometry<double>(nlev, ldk, ldk_w, merge) : cc_geometry<float>(nlev, ldk, ldk_w, merge);
     const int n_slots = std::min(65535, f64 ? icon::cc_max_slots<double>(shape, nlev, geom.slot_bytes, smem_bytes, (g->options[ICON_OPT_CC_L2_HINTS] & 16) != 0)
                                             : icon::cc_max_slots<float>(shape, nlev, geom.slot_bytes, smem_bytes, (g->options[ICON_OPT_CC_L2_HINTS] & 16) != 0));

@@ -47,8 +47,8 @@ struct CcShape {
 };
 constexpr int kCcNumShapes = 2;
 #ifndef CC_S1_G          // shape 1 can be re-defined at build time for pipeline-shape experiments (ICON_NVCC_EXTRA)
-#define CC_S1_G 2
-#define CC_S1_D 5
+#define CC_S1_G 4
+#define CC_S1_D 3
 #endif
 constexpr CcShape kCcShapes[kCcNumShapes] = {{8, 2, 6}, {8, CC_S1_G, CC_S1_D}};
 inline const CcShape& cc_shape(int i) { return kCcShapes[i >= 0 && i < kCcNumShapes ? i : 0]; }

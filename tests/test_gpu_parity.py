@@ -246,7 +246,7 @@ def test_dycore_step_matches_the_two_calls_and_the_oracle(torch_cuda, lib, oracl
         assert (res[name][:, nlev:] == sentinel).all(), name
         assert not (res[name][:, :nlev] == sentinel).any(), name
     g.set_option(lib.ICON_OPT_TENDENCY_KERNEL, 5)
-    g.set_option(lib.ICON_OPT_CC_SHAPE, 0)
+    g.set_option(lib.ICON_OPT_CC_SHAPE, -1)
 
 
 @pytest.mark.parametrize("period", [0, 4, 16, 512])
@@ -267,7 +267,7 @@ def test_fused_step_pacing_barrier_periods(torch_cuda, lib, oracle_grid, period)
         ref = oracle_reference(og, vn, w, zh, nlev, False)
         sets.append((torch.from_numpy(vn).to(dev), torch.from_numpy(w).to(dev), zh, ref))
     g.set_option(lib.ICON_OPT_TENDENCY_KERNEL, 5)
-    g.set_option(lib.ICON_OPT_CC_SHAPE, 0)
+    g.set_option(lib.ICON_OPT_CC_SHAPE, -1)
     g.set_option(lib.ICON_OPT_CC_PACE, period)
     try:
         for it in range(6):

@@ -118,7 +118,7 @@ def test_cc_schedule_replays_correctly(k, seed, flags, shape):
             g.set_option(lib.ICON_OPT_CC_TILE, tile)
             st = g.cc_schedule_check(dtype, nlev, ldk, ldk_w, n_ctas=148, smem_bytes=232448)
             np_ = g.nc // 4
-            group = (2, 2)[shape]
+            group = (2, 4)[shape]
             assert st["ctas"] == min(148, -(-np_ // (tile or group)))
             assert st["steps"] >= -(-np_ // group)
             # every patch needs its 36 + 7 columns at least once per CTA range, never more than 43 per patch
@@ -132,7 +132,7 @@ def test_cc_schedule_replays_correctly(k, seed, flags, shape):
 def test_cc_schedule_merges_runs_on_the_canonical_grid():
     """generation-order numbering: consecutive column ids arrive as one bulk copy when the stride allows"""
     g = lib.IconGrid(4, 0, binding.ICON_HOST_ONLY)
-    g.set_option(lib.ICON_OPT_CC_SHAPE, 0)
+    g.set_option(lib.ICON_OPT_CC_SHAPE, -1)
     merged = g.cc_schedule_check(0, 90, 96, 96)
     g.set_option(lib.ICON_OPT_CC_MERGE, 0)
     single = g.cc_schedule_check(0, 90, 96, 96)
