@@ -69,7 +69,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
@@ -80,10 +80,23 @@ class ClockSampler:
         for line in self.proc.stdout:
             self.lines.append(line.strip())
 
+    def wait_first_sample(self, timeout=8.0):
+        """nvidia-smi needs up to a second to start on a fresh box: wait for its first line BEFORE the warm-up, so that
+        the short timed region is not over before the first sample"""
+        t0 = time.perf_counter()
+        while self.proc and not self.lines and time.perf_counter() - t0 < timeout:
+            time.sleep(0.01)
+
+    def mark_begin(self):
+        self.n0 = len(self.lines)
+
+    def mark_end(self):
+        time.sleep(0.03)              # a line printed just after the region was sampled inside it
+        self.n1 = len(self.lines)
+
     def stop(self):
         if not self.proc:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.15)
         self.proc.terminate()
         try:
             self.proc.wait(timeout=5)
@@ -91,7 +104,11 @@ class ClockSampler:
             self.proc.kill()
         sm, mx, pw, reasons = [], [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for ln in self.lines:
+        n0, n1 = getattr(self, "n0", 0), getattr(self, "n1", len(self.lines))
+        window, note = self.lines[n0:n1], []
+        if not window:                # region shorter than one sampling period: the last samples of the warm-up (same load)
+            window, note = self.lines[max(0, n0 - 3):n1], ["no sample inside the timed region: last warm-up samples"]
+        for ln in window:
             f = [x.strip() for x in ln.split(",")]
             if len(f) < 7:
                 continue
@@ -103,7 +120,7 @@ class ClockSampler:
                 if v.lower().startswith("active"):
                     reasons.add(n)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons) + note}
 
 
 def max_over_ranks(seconds, device=None):
@@ -258,18 +275,21 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        sampler.wait_first_sample()
     for _ in range(args.warmup):
         step()
     barrier()
     evs = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(args.steps)]
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
     launches0 = g.launch_count
     barrier()
+    sampler.mark_begin()
     for i in range(args.steps):
         step(evs[i])
     barrier()
+    sampler.mark_end()
     launches = g.launch_count - launches0
     clocks = sampler.stop() if rank == 0 else None
     fused = launches == args.steps            # one kernel per step
