@@ -340,6 +340,94 @@ def test_vertical_term_exact_for_linear_profiles(oracle_grid):
     assert np.abs(got - want).max() / np.abs(want).max() < 1e-11
 
 
+def _arc(p, q):
+    """great-circle distance of unit vectors, atan2(|p x q|, p . q) (reading P-8), numpy"""
+    return np.arctan2(np.linalg.norm(np.cross(p, q), axis=1), (p * q).sum(1))
+
+
+@pytest.mark.parametrize("k,seed,flags", [(0, 0, 0), (2, 0, 0), (4, 0, 0), (3, 4, 1)])
+def test_c_lin_slot_order_from_geometry(oracle_grid, k, seed, flags):
+    """P-9 pins the SLOT ORDER of c_lin from geometry alone: slot 0 multiplies the value at e2c[e][0] and is
+    arc(x_e, c1)/d_e, so that linear interpolation along the dual arc holds: with signed abscissae s0 = -arc(x_e, c0),
+    s1 = +arc(x_e, c1) the weights satisfy c_lin0 * s0 + c_lin1 * s1 = 0 and the NEARER cell weighs more. Swapping the
+    two assignments in oracle/icon_oracle.c (c_lin[2e] <-> c_lin[2e+1]) fails both assertions on every unoptimised
+    grid, where the two distances differ by per cent (checked on a scratch copy of the oracle)."""
+    g = oracle_grid(k, seed, flags)
+    x, c0, c1 = g.edge_xyz, g.cell_xyz[g.e2c[:, 0]], g.cell_xyz[g.e2c[:, 1]]
+    a0, a1 = _arc(x, c0), _arc(x, c1)
+    d = g.d_e / A
+    assert np.abs(a0 + a1 - d).max() < 1e-14                 # the dual arc passes through x_e (P-8)
+    assert np.abs(a0 - a1).max() / d.max() > 1e-3            # the pin has teeth: the distances do differ
+    resid = g.c_lin[:, 0] * (-a0) + g.c_lin[:, 1] * a1
+    assert np.abs(resid).max() < 1e-15
+    differ = np.abs(a0 - a1) > 1e-9 * d
+    assert ((g.c_lin[:, 0] > g.c_lin[:, 1]) == (a0 < a1))[differ].all()
+    assert np.abs(g.c_lin[:, 0] - a1 / d).max() < 1e-14 and np.abs(g.c_lin[:, 1] - a0 / d).max() < 1e-14
+
+
+def test_vertical_term_uses_c_lin_slot0_for_cell0(oracle_grid):
+    """Operator-level pin of P-9 / S6: vn = a + b z per edge and a NON-uniform w. Expected -w_e b with w_e assembled
+    from numpy arc distances (never from g.c_lin): w_e = [arc(x_e,c1) w_f(c0) + arc(x_e,c0) w_f(c1)] / d_e, i.e. the
+    value linearly interpolated along the dual arc to the edge midpoint. Swapping the two factors in og_ddt_vn (or the
+    two table assignments) gives a relative error of order 1e-2 here (checked on a scratch copy of the oracle)."""
+    g = oracle_grid(2)
+    K = 7
+    zh = si.z_half_levels(K)
+    zf = 0.5 * (zh[:-1] + zh[1:])
+    rng = np.random.default_rng(11)
+    b = (1.0 + rng.random(g.ne)) * 1e-3
+    vn = 2.0 + b[:, None] * zf[None, :]
+    # w linear in a Cartesian coordinate: the exact interpolant along the (short) dual arc is nearly linear in arc
+    # length, and the two cells of an edge get clearly different values
+    w = np.repeat((1.0 + 50.0 * g.cell_xyz[:, 0] + 30.0 * g.cell_xyz[:, 2])[:, None], K + 1, axis=1)
+    w *= (1.0 + 0.1 * np.arange(K + 1))[None, :]
+    x, c0, c1 = g.edge_xyz, g.cell_xyz[g.e2c[:, 0]], g.cell_xyz[g.e2c[:, 1]]
+    a0, a1 = _arc(x, c0), _arc(x, c1)
+    wf = 0.5 * (w[:, :-1] + w[:, 1:])
+    w_e = (a1[:, None] * wf[g.e2c[:, 0]] + a0[:, None] * wf[g.e2c[:, 1]]) / (a0 + a1)[:, None]
+    want = -w_e * b[:, None]
+    got = g.velocity_tendencies(vn, w, zh, K)["ddt_vn"] - g.velocity_tendencies(vn, np.zeros_like(w), zh, K)["ddt_vn"]
+    assert np.abs(got - want).max() / np.abs(want).max() < 1e-11
+    # teeth: the swapped association differs from `want` by far more than the tolerance
+    w_swapped = (a0[:, None] * wf[g.e2c[:, 0]] + a1[:, None] * wf[g.e2c[:, 1]]) / (a0 + a1)[:, None]
+    assert np.abs(w_swapped - w_e).max() / np.abs(w_e).max() > 1e-3
+
+
+def test_tolerance_scale_is_the_sum_of_absolute_terms(oracle_grid):
+    """P-16: M(p) is EXACTLY the sum of the absolute values of the terms entering p -- two-sided, so an inflated
+    scale (which would loosen every parity test) fails as surely as a deflated one. Re-assembled with numpy from the
+    oracle's intermediate outputs and numpy arc distances."""
+    g = oracle_grid(2)
+    K = 6
+    rng = np.random.default_rng(17)
+    vn = rng.standard_normal((g.ne, K)) * 5
+    w = rng.standard_normal((g.nc, K + 1))
+    zh = si.z_half_levels(K)
+    o = g.velocity_tendencies(vn, w, zh, K, with_scale=True)
+    dz = zh[:-1] - zh[1:]
+    zf = 0.5 * (zh[:-1] + zh[1:])
+    vn_ie = np.zeros((g.ne, K + 1))
+    gk = dz[:-1] / (dz[:-1] + dz[1:])
+    vn_ie[:, 1:K] = gk * vn[:, 1:] + (1 - gk) * vn[:, :-1]
+    vn_ie[:, 0] = vn[:, 0] + (vn[:, 0] - vn[:, 1]) * (zh[0] - zf[0]) / (zf[0] - zf[1])
+    vn_ie[:, K] = vn[:, K - 1] + (vn[:, K - 1] - vn[:, K - 2]) * (zh[K] - zf[K - 1]) / (zf[K - 1] - zf[K - 2])
+    x, c0, c1 = g.edge_xyz, g.cell_xyz[g.e2c[:, 0]], g.cell_xyz[g.e2c[:, 1]]
+    a0, a1 = _arc(x, c0), _arc(x, c1)
+    wf = 0.5 * (w[:, :-1] + w[:, 1:])
+    w_e = (a1[:, None] * wf[g.e2c[:, 0]] + a0[:, None] * wf[g.e2c[:, 1]]) / (a0 + a1)[:, None]
+    kc, vt, zeta = o["ke_c"], o["vt"], o["vort"]
+    m = (np.abs(kc[g.e2c[:, 1]]) + np.abs(kc[g.e2c[:, 0]])) / g.d_e[:, None] \
+        + np.abs(vt) * (np.abs(g.f_e)[:, None] + 0.5 * (np.abs(zeta[g.e2v[:, 0]]) + np.abs(zeta[g.e2v[:, 1]]))) \
+        + np.abs(w_e) * (np.abs(vn_ie[:, :-1]) + np.abs(vn_ie[:, 1:])) / dz
+    assert (o["m_ddt"] <= 1.0000001 * m).all() and (o["m_ddt"] >= 0.9999999 * m).all()
+    assert (np.abs(o["ddt_vn"]) <= 1.0000001 * m).all()
+    div, vort, md, mv = g.div_vort(vn, K, with_scale=True)
+    m_div = sum(np.abs(g.geofac_div[:, j:j + 1] * vn[g.c2e[:, j]]) for j in range(3))
+    m_vort = sum(np.abs(g.geofac_rot[:, j:j + 1] * vn[g.v2e[:, j]]) for j in range(6))
+    assert (md <= 1.0000001 * m_div).all() and (md >= 0.9999999 * m_div).all()
+    assert (mv <= 1.0000001 * m_vort).all() and (mv >= 0.9999999 * m_vort).all()
+
+
 # ----------------------------------------------------------------------------------------------
 # special cases that reduce to library routines; internal consistency of the two evaluation paths
 # ----------------------------------------------------------------------------------------------
