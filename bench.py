@@ -48,6 +48,39 @@ def algorithmic_bytes(nc, ne, nv, nlev, g):
     return tend, dv
 
 
+KERNEL_SOURCES = ("kernels_cc.cu", "cc_schedule.cpp", "cc_schedule.hpp", "sc_tables.cpp", "sc_tables.hpp", "kernels.cu", "api.cu")
+
+
+def kernel_source_hash():
+    """sha256 (16 hex digits) of the sources that decide the kernels' DRAM traffic: profiles/traffic.csv is stamped with
+    it, and a capture made from other sources is not reported as this run's traffic"""
+    import hashlib
+    h = hashlib.sha256()
+    for name in KERNEL_SOURCES:
+        with open(os.path.join(ROOT, "paper_2511_02021_b200", "csrc", name), "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()[:16]
+
+
+def committed_traffic(config, call):
+    """ncu dram__bytes_read.sum + dram__bytes_write.sum per launch from profiles/traffic.csv (columns: config, call,
+    bytes, capture file, kernel source hash), or (None, why) when the capture was made from other kernel sources"""
+    tp = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(tp):
+        return None, "profiles/traffic.csv missing"
+    try:
+        have = kernel_source_hash()
+        for ln in open(tp).read().splitlines()[1:]:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) >= 5 and f[0] == str(config) and f[1] == call:
+                if f[4] != have:
+                    return None, "stale: captured from kernel sources %s, this tree is %s" % (f[4], have)
+                return int(f[2]), "profiles/%s (ncu --set full, kernel sources %s)" % (f[3], f[4])
+    except Exception as e:          # noqa: BLE001
+        return None, "unreadable: %s" % e
+    return None, "no capture for this config / call"
+
+
 def peak_hbm_gbs():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -61,7 +94,7 @@ def peak_hbm_gbs():
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled DURING the timed region"""
     Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
-        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap,clocks.mem"
 
     def __init__(self, index):
         self.index, self.proc, self.lines = index, None, []
@@ -102,7 +135,7 @@ class ClockSampler:
             self.proc.wait(timeout=5)
         except Exception:
             self.proc.kill()
-        sm, mx, pw, reasons = [], [], [], set()
+        sm, mx, pw, mem, reasons, capped = [], [], [], [], set(), 0
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         n0, n1 = getattr(self, "n0", 0), getattr(self, "n1", len(self.lines))
         window, note = self.lines[n0:n1], []
@@ -116,11 +149,18 @@ class ClockSampler:
                 sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
             except ValueError:
                 continue
+            try:
+                mem.append(float(f[7]))
+            except (IndexError, ValueError):
+                pass
             for n, v in zip(names, f[3:7]):
                 if v.lower().startswith("active"):
                     reasons.add(n)
+                    capped += n == "sw_power_cap"
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons) + note}
+                "sm_mhz_min": min(sm) if sm else None, "mem_mhz": float(np.median(mem)) if mem else None,
+                "power_w_max": max(pw) if pw else None, "power_w_median": float(np.median(pw)) if pw else None,
+                "samples": len(sm), "samples_sw_power_cap": capped, "reasons": sorted(reasons) + note}
 
 
 def max_over_ranks(seconds, device=None):
@@ -149,6 +189,16 @@ def oracle_step_seconds(og, vn, w, zh, nlev, reps):
         og.div_vort(vn, nlev)
         ts.append(time.perf_counter() - t0)
     return ts
+
+
+def set_oracle_threads(n):
+    """the oracle's loops are OpenMP loops inside oracle/libicon_oracle.so: set the team size of the libgomp it links"""
+    import ctypes
+    try:
+        ctypes.CDLL("libgomp.so.1").omp_set_num_threads(int(n))
+        return True
+    except OSError:
+        return False
 
 
 def cpu_threads():
@@ -226,16 +276,10 @@ def run_ours(args):
     g = lib.IconGrid(cfg["k"], si.PERMUTE_SEED if cfg["permute"] else 0, flags)
     if args.variant is not None:
         g.set_option(lib.ICON_OPT_TENDENCY_KERNEL, args.variant)
-    if args.cc_hints is not None:
-        g.set_option(lib.ICON_OPT_CC_L2_HINTS, args.cc_hints)
     if args.cc_tile is not None:
         g.set_option(lib.ICON_OPT_CC_TILE, args.cc_tile)
-    if args.cc_merge is not None:
-        g.set_option(lib.ICON_OPT_CC_MERGE, args.cc_merge)
     if args.cc_pace is not None:
         g.set_option(lib.ICON_OPT_CC_PACE, args.cc_pace)
-    if args.cc_shape is not None:
-        g.set_option(lib.ICON_OPT_CC_SHAPE, args.cc_shape)
     t_grid = time.perf_counter() - t0
     vn_h, w_h, zh = si.make_fields(args.config, g.table_host("edge_xyz"), g.table_host("edge_normal"), g.nc,
                                    ldk=ldk, ldk_w=ldk_w, pad_value=0.0)
@@ -295,6 +339,13 @@ def run_ours(args):
     fused = launches == args.steps            # one kernel per step
     t_steps = np.array([e[0].elapsed_time(e[1]) for e in evs]) * 1e-3
     t_step = float(t_steps.mean())
+    # sampled values of the TIMED output buffers (the last timed launch wrote them), checked against the oracle below
+    picks = {}
+    if rank == 0 and not args.no_parity_spot:
+        for what, arr, n in (("ddt_vn", ddt, g.ne), ("div", div, g.nc), ("vort", vort, g.nv)):
+            idx, lev = si.sample_points(700 + args.config, n, nlev, args.spot_points)
+            got = arr[torch.from_numpy(idx).to(dev), torch.from_numpy(lev.astype(np.int64)).to(dev)]
+            picks[what] = (idx, lev, got.cpu().numpy().astype(np.float64))
     # the two entry points on their own (not part of the headline)
     n2 = max(3, args.steps // 2)
     evs2 = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(n2)]
@@ -345,25 +396,44 @@ def run_ours(args):
     kname = "dycore_step (fused k_tend_cc)" if fused else "dycore_velocity_tendencies"
     kbytes, ktime = (bytes_fused, t_step) if fused else (bytes_tend, t_tend_avg)
     achieved = kbytes / ktime / 1e9
-    traffic = None          # ncu dram__bytes_read.sum + dram__bytes_write.sum of the committed capture, per launch
-    tp = os.path.join(ROOT, "profiles", "traffic.csv")
-    if os.path.exists(tp):
-        try:
-            for ln in open(tp).read().splitlines()[1:]:
-                f = ln.split(",")
-                if len(f) >= 3 and f[0] == str(args.config) and f[1] == ("dycore_step" if fused else "dycore_velocity_tendencies"):
-                    traffic = int(f[2])
-        except Exception:
-            traffic = None
+    traffic, traffic_src = committed_traffic(args.config, "dycore_step" if fused else "dycore_velocity_tendencies")
+    kt = (t_steps if fused else t_tend) * 1e3            # per-launch times of the dominant kernel, ms
+    # fields-only accounting beside the with-tables one (the fused kernel reads patch records, not the plain tables)
+    fields_fused = (2 * g.ne * nlev + g.nc * (nlev + 1) + (g.nc + g.nv) * nlev) * gsize
+    fields_tend = (2 * g.ne * nlev + g.nc * (nlev + 1)) * gsize
+    kfields = fields_fused if fused else fields_tend
     roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": kbytes, "kernel_ms": ktime * 1e3,
+                "kernel_ms_median": float(np.median(kt)), "kernel_ms_min": float(kt.min()), "kernel_ms_max": float(kt.max()),
+                "frac_at_median": kbytes / (float(np.median(kt)) * 1e-3) / 1e9 / peak,
+                "frac_at_min": kbytes / (float(kt.min()) * 1e-3) / 1e9 / peak,
                 "frac_of_nominal_8TBs": achieved / 8000.0,
+                "fields_only": {"bytes_per_launch": kfields, "frac": kfields / ktime / 1e9 / peak,
+                                "frac_of_nominal_8TBs": kfields / ktime / 1e9 / 8000.0},
                 "two_calls": {"tendencies": {"achieved": bytes_tend / t_tend_avg / 1e9, "frac": bytes_tend / t_tend_avg / 1e9 / peak,
                                              "kernel_ms": t_tend_avg * 1e3, "algorithmic_bytes_per_launch": bytes_tend},
                               "div_vort": {"achieved": bytes_dv / float(t_dv.mean()) / 1e9, "frac": bytes_dv / float(t_dv.mean()) / 1e9 / peak,
                                            "kernel_ms": float(t_dv.mean()) * 1e3, "algorithmic_bytes_per_launch": bytes_dv},
                               "ms_per_step": (t_tend_avg + float(t_dv.mean())) * 1e3}}
+
+    parity_spot = None
+    if picks:
+        # the oracle (oracle/, test infrastructure) evaluates the same sampled points one by one from the same inputs
+        import oracle
+        og = oracle.Grid(cfg["k"], si.PERMUTE_SEED if cfg["permute"] else 0, 1 if cfg["permute"] else 0)
+        o = og.rounded_f32() if f32 else og
+        vn64, w64 = (vn_h.astype(np.float64), w_h.astype(np.float64)) if f32 else (vn_h, w_h)
+        tol = 1e-5 if f32 else 1e-12
+        parity_spot = {"tolerance": tol, "points_per_output": args.spot_points, "what": "sampled points of the output buffers of "
+                       "the last timed launch vs oracle.sample, |gpu - oracle| / M(p) (reading P-16)", "ok": True}
+        for what, (idx, lev, got) in picks.items():
+            want, m = o.sample(what, idx, lev, vn64, nlev, w=w64, z_half=zh)
+            worst = float((np.abs(got - want) / np.maximum(m, 1e-300)).max())
+            parity_spot["worst_err_over_M_" + what] = worst
+            parity_spot["ok"] = bool(parity_spot["ok"] and worst <= tol and np.isfinite(got).all())
+        parity_spot["worst_err_over_M"] = max(v for k_, v in parity_spot.items() if k_.startswith("worst_err_over_M_"))
+        del og, o, vn64, w64
 
     cpu_baseline = None
     if not args.no_cpu_baseline and world == 1:
@@ -371,11 +441,23 @@ def run_ours(args):
         og, ovn, ow, ozh, onlev = oracle_sample(args.config, k_sample)
         oracle_step_seconds(og, ovn, ow, ozh, onlev, 1)
         ts, t_begin = [], time.perf_counter()
-        while len(ts) < 3 or (time.perf_counter() - t_begin < 12.0 and len(ts) < 400):
+        while len(ts) < 3 or (time.perf_counter() - t_begin < 10.0 and len(ts) < 400):
             ts += oracle_step_seconds(og, ovn, ow, ozh, onlev, 1)
-        cpu_baseline = {"value": og.ne * onlev / float(np.mean(ts)) / 1e9, "unit": UNIT, "cores": cpu_threads(), "kind": "oracle",
-                        "sample": "R2B%d x %d levels fp64 oracle, %d timed steps (%.1f s), same field recipe" % (
-                            k_sample, onlev, len(ts), sum(ts))}
+        cores = cpu_threads()
+        single = None
+        if set_oracle_threads(1):                 # the same sample on ONE thread
+            t1 = oracle_step_seconds(og, ovn, ow, ozh, onlev, 2)[-1:]
+            while sum(t1) < 6.0 and len(t1) < 50:
+                t1 += oracle_step_seconds(og, ovn, ow, ozh, onlev, 1)
+            set_oracle_threads(cores)
+            single = {"value": og.ne * onlev / float(np.mean(t1)) / 1e9, "unit": UNIT, "cores": 1, "steps": len(t1)}
+        cpu_baseline = {"value": og.ne * onlev / float(np.mean(ts)) / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
+                        "sample": "R2B%d x %d levels fp64 oracle, %d timed steps (%.1f s), same field recipe; the full R2B%d "
+                                  "grid is not timed because the oracle materialises every intermediate (about 30 GB of host "
+                                  "memory and minutes per step at R2B8): a bounded sample of the same recipe instead" % (
+                                      k_sample, onlev, len(ts), sum(ts), cfg["k"]),
+                        "single_thread": single}
+        del og, ovn, ow
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": t_step_max * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -384,10 +466,13 @@ def run_ours(args):
                        "ldk": ldk, "ldk_w": ldk_w, "step": "dycore_step (ddt_vn + div + vort; one fused kernel)" if fused else "dycore_step = dycore_velocity_tendencies + dycore_div_vort",
                        "l2": "flushed between iterations" if l2_flush is not None else "inputs larger than L2",
                        "parallelism": "replicas only" if world > 1 else "single GPU",
-                       "tendency_kernel_variant": args.variant, "cc_shape": args.cc_shape, "cc_hints": args.cc_hints, "cc_tile": args.cc_tile, "cc_pace": args.cc_pace, "cc_merge": args.cc_merge, "grid_create_s": t_grid},
+                       "tendency_kernel_variant": args.variant, "cc_tile": args.cc_tile, "cc_pace": args.cc_pace, "grid_create_s": t_grid},
             "gpts_tendency_call_only": pts / t_tend_avg / 1e9,
             "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": int(launches),
-            "clocks": clocks}
+            "step_ms": {"mean": float(t_steps.mean() * 1e3), "median": float(np.median(t_steps) * 1e3),
+                        "min": float(t_steps.min() * 1e3), "max": float(t_steps.max() * 1e3),
+                        "all": [round(float(x) * 1e3, 4) for x in t_steps]},
+            "parity_spot": parity_spot, "clocks": clocks}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -402,15 +487,14 @@ def main():
     ap.add_argument("--config", type=int, default=3, choices=sorted(si.CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--variant", type=int, default=None, help="ICON_OPT_TENDENCY_KERNEL override")
-    ap.add_argument("--cc-shape", type=int, default=None, dest="cc_shape", help="ICON_OPT_CC_SHAPE override")
-    ap.add_argument("--cc-hints", type=int, default=None, dest="cc_hints", help="ICON_OPT_CC_L2_HINTS override")
     ap.add_argument("--cc-tile", type=int, default=None, dest="cc_tile", help="ICON_OPT_CC_TILE override")
-    ap.add_argument("--cc-merge", type=int, default=None, dest="cc_merge", help="ICON_OPT_CC_MERGE override")
     ap.add_argument("--cc-pace", type=int, default=None, dest="cc_pace", help="ICON_OPT_CC_PACE override")
     ap.add_argument("--ldk", type=int, default=0, help="leading dimension of vn/ddt_vn/div/vort (default: padded to 128 B)")
     ap.add_argument("--ldk-w", type=int, default=0, dest="ldk_w")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-parity-spot", action="store_true", dest="no_parity_spot")
+    ap.add_argument("--spot-points", type=int, default=3000, dest="spot_points")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3

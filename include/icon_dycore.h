@@ -81,34 +81,22 @@ enum {
     ICON_TAB_COUNT
 };
 
-/* runtime options (icon_grid_set_option); defaults are the fastest validated variants */
+/* runtime options (icon_grid_set_option); the defaults are the measured optimum on B200 */
 enum {
-    ICON_OPT_TENDENCY_KERNEL = 0, /* 0 = unfused 3-kernel pipeline through an HBM workspace;
-                                     1 = fused per-edge gather kernel (no workspace);
-                                     2 = fused register-resident patch kernel with shared-memory exchange;
-                                     3 = self-contained patch kernel (one warp per patch, columns through L1);
+    ICON_OPT_TENDENCY_KERNEL = 0, /* 0 = unfused 3-kernel pipeline through an HBM workspace (also serves the optional
+                                         outputs vt_opt / ke_c_opt / vort_opt, whatever this option says);
+                                     3 = self-contained patch kernel (one warp per patch, columns through L1; any nlev);
                                      4 = column-cache kernel: whole columns staged in shared memory by bulk
                                          asynchronous copies on a host-built schedule; level counts it cannot
                                          hold (nlev > 95) fall back to 3;
-                                     5 = auto (default): 4 for fp64 with 32 <= nlev <= 95, 2 for nlev <= 31,
-                                         else 3 (the fastest measured variant of each regime);
-                                         dycore_step takes 4 wherever it can hold the columns (nlev <= 95). */
-    ICON_OPT_CC_SHAPE = 1,        /* pipeline shape of kernel 4 (consumer warps / patches per step / ring
-                                     depth): 0 = 8/2/6, 1 = 8/4/3, -1 = auto (default) = 1, the faster one
-                                     in every measured regime. */
-    ICON_OPT_CC_L2_HINTS = 2,     /* L2 eviction hints of kernel 4, bit mask: 1 = ddt_vn stores evict-first,
-                                     2 = patch records evict-first, 4 = vn / w columns evict-last, 16 = outputs leave by
-                                     plain coalesced stores (transposed in shared memory) instead of bulk stores.
-                                     Default 19. */
-    ICON_OPT_CC_MERGE = 3,        /* kernel 4: 1 (default) = columns with consecutive ids arrive as one bulk copy
-                                     when the field's column stride allows it; 0 = one copy per column. */
-    ICON_OPT_CC_TILE = 4,         /* kernel 4: patches per tile of the round-robin work order (CTA b walks the tiles
+                                     5 = auto (default) = 4 wherever it can hold the columns. */
+    ICON_OPT_CC_TILE = 1,         /* kernel 4: patches per tile of the round-robin work order (CTA b walks the tiles
                                      b, b + #CTAs, ... so that neighbouring tiles are in flight together and share
-                                     their halo columns through the L2); even; 0 = one contiguous range per CTA.
-                                     Default 16. */
-    ICON_OPT_CC_PACE = 5,         /* kernel 4: the producers of all CTAs meet every this many steps (power of two; bounded
+                                     their halo columns through the L2); a multiple of 4; 0 = one contiguous range per
+                                     CTA. Default 16. */
+    ICON_OPT_CC_PACE = 2,         /* kernel 4: the producers of all CTAs meet every this many steps (power of two; bounded
                                      wait) so that the CTAs do not drift rounds apart and neighbouring tiles keep sharing
-                                     halo columns through the L2; 0 = never. Default 512; fused step (dycore_step) only. */
+                                     halo columns through the L2; 0 = never. Default 512; fused fp64 step (dycore_step) only. */
     ICON_OPT_COUNT
 };
 
@@ -157,7 +145,7 @@ int icon_grid_worklist_stats(icon_grid_t* g, int64_t out[8]);
  * schedule tendency kernel 4 would run for (dtype, nlev, ldk, ldk_w) with the current ICON_OPT_CC_*
  * options on a device with `n_ctas` SMs and `smem_bytes` of opt-in shared memory per block, replays it
  * with an independent checker (every patch finds each of its 43 columns in the slot its record names;
- * no bulk copy overwrites a slot a running step still reads; byte counts match) and reports
+ * no bulk copy overwrites a slot a running step still reads or a copy still in flight fills; byte counts match) and reports
  *   out[0] steps   out[1] steps with reduced run-ahead   out[2] vn columns loaded   out[3] w columns loaded
  *   out[4] bulk copies   out[5] slots   out[6] slot bytes   out[7] CTAs.
  * ICON_EUNSUPPORTED: nlev or the memory size cannot hold the kernel; ICON_EINVAL: the check failed

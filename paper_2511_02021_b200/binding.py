@@ -18,11 +18,8 @@ ICON_F64, ICON_F32 = 0, 1
 ICON_T_I32, ICON_T_I8, ICON_T_F64, ICON_T_F32 = 10, 11, 12, 13
 ICON_PERMUTE, ICON_LOCALITY_WORKLIST, ICON_HOST_ONLY, ICON_NO_WORKLIST = 1, 2, 4, 8
 ICON_OPT_TENDENCY_KERNEL = 0
-ICON_OPT_CC_SHAPE = 1
-ICON_OPT_CC_L2_HINTS = 2
-ICON_OPT_CC_MERGE = 3
-ICON_OPT_CC_TILE = 4
-ICON_OPT_CC_PACE = 5
+ICON_OPT_CC_TILE = 1
+ICON_OPT_CC_PACE = 2
 
 TABLES = ("c2v", "c2e", "e2c", "e2v", "e2e4", "v2e", "v2c", "v_deg", "c_os", "v_os",
           "vert_xyz", "cell_xyz", "edge_xyz", "edge_normal", "l_e", "d_e", "inv_d_e", "f_e", "c_lin", "rbf",

@@ -206,48 +206,37 @@ int ensure_sc_host(icon_grid* g) {
 // A slot as large as the caller's column stride lets runs of consecutive columns arrive as one bulk
 // copy (the copy engine, not HBM, limits small copies); taken when it costs < 128 bytes per slot.
 template <class T>
-icon::CcGeometry cc_geometry(int nlev, int64_t ldk, int64_t ldk_w, bool merge) {
+icon::CcGeometry cc_geometry(int nlev, int64_t ldk, int64_t ldk_w) {
     icon::CcGeometry geom;
     geom.col_bytes[0] = (nlev * (int)sizeof(T) + 15) & ~15;
     geom.col_bytes[1] = icon::cc_slot_bytes<T>(nlev);
     geom.stride_bytes[0] = (int)(ldk * (int64_t)sizeof(T));
     geom.stride_bytes[1] = (int)(ldk_w * (int64_t)sizeof(T));
     geom.slot_bytes = geom.col_bytes[1];
-    if (merge && geom.stride_bytes[0] >= geom.col_bytes[1] && geom.stride_bytes[0] < geom.col_bytes[1] + 128)
+    if (geom.stride_bytes[0] >= geom.col_bytes[1] && geom.stride_bytes[0] < geom.col_bytes[1] + 128)
         geom.slot_bytes = geom.stride_bytes[0];
-    if (!merge) geom.stride_bytes[0] = geom.stride_bytes[1] = 0;      // no stride equals the slot size: runs of 1
     return geom;
 }
 
-// ICON_OPT_CC_SHAPE -1 = auto = 8/4/3 (four patches per step): the faster shape of every instantiation, measured
-// (config 3 5.11 -> 4.91 ms, config 4 4.01 -> 3.38 ms, config 5 12.25 -> 9.84 ms)
-static int cc_resolve_shape(const icon_grid* g, bool /*f64*/, int /*nlev*/) {
-    const int opt = g->options[ICON_OPT_CC_SHAPE];
-    return opt >= 0 ? opt : 1;
-}
+template <class T>
+constexpr int cc_record_size() { return icon::kScCoefWords * (int)sizeof(T) + icon::kCcRecordTail; }
 
 // Column-cache schedule + patch records for (T, nlev): built on the host once, uploaded once.
 // Returns ICON_OK with p.unsupported set when this (T, nlev) cannot use the kernel (the caller
 // then uses the self-contained patch kernel).
 template <class T>
 int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev, int64_t ldk, int64_t ldk_w) {
-    const int shape = cc_resolve_shape(g, sizeof(T) == 8, nlev);
-    const bool merge = g->options[ICON_OPT_CC_MERGE] != 0;
     const int tile = g->options[ICON_OPT_CC_TILE];
-    const bool direct = (g->options[ICON_OPT_CC_L2_HINTS] & 16) != 0;
-    if (p.nlev == nlev && p.shape == shape && p.ldk == ldk && p.ldk_w == ldk_w && p.merge == merge && p.tile == tile && p.direct == direct &&
-        (p.ready || p.unsupported))
+    if (p.nlev == nlev && p.ldk == ldk && p.ldk_w == ldk_w && p.tile == tile && (p.ready || p.unsupported))
         return ICON_OK;
     dev_release(g, p.steps); dev_release(g, p.loads); dev_release(g, p.records);
     dev_release(g, p.cta_patch_begin); dev_release(g, p.cta_step_begin); dev_release(g, p.progress);
     p = icon::DevCcTables<T>();
     p.nlev = nlev;
-    p.shape = shape;
-    p.ldk = ldk; p.ldk_w = ldk_w; p.merge = merge; p.tile = tile; p.direct = direct;
-    const icon::CcShape& sh = icon::cc_shape(shape);
-    const icon::CcGeometry geom = cc_geometry<T>(nlev, ldk, ldk_w, merge);
+    p.ldk = ldk; p.ldk_w = ldk_w; p.tile = tile;
+    const icon::CcGeometry geom = cc_geometry<T>(nlev, ldk, ldk_w);
     const int slot_bytes = geom.slot_bytes;
-    const int n_slots_max = icon::cc_max_slots<T>(shape, nlev, slot_bytes, g->smem_optin, direct);
+    const int n_slots_max = icon::cc_max_slots<T>(slot_bytes, g->smem_optin);
     if (icon::cc_levels_per_lane(nlev) == 0 || nlev * (int)sizeof(T) < 16 || n_slots_max < icon::kScIdWords) {
         p.unsupported = true;
         return ICON_OK;
@@ -258,9 +247,9 @@ int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev, int64_t ld
     const int n_slots = std::min(n_slots_max, 65535);
     icon::CcSchedule cs;
     std::vector<unsigned char> rec;
-    const size_t rb = (size_t)icon::kScCoefWords * sizeof(T) + icon::kCcRecordTail;
+    const size_t rb = (size_t)cc_record_size<T>();
     try {
-        std::string err = icon::build_cc_schedule(sc, g->num_sms, n_slots, geom, sh.group, sh.depth, g->options[ICON_OPT_CC_TILE], cs);
+        std::string err = icon::build_cc_schedule(sc, g->num_sms, n_slots, geom, icon::kCcGroup, icon::kCcDepth, tile, cs);
         if (!err.empty()) {
             p.unsupported = true;
             return ICON_OK;
@@ -298,10 +287,12 @@ int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev, int64_t ld
     if ((rc = upload_vec(g, cs.cta_patch_begin, &p.cta_patch_begin))) return rc;
     if ((rc = upload_vec(g, cs.cta_step_begin, &p.cta_step_begin))) return rc;
     p.n_ctas = cs.n_ctas; p.n_slots = cs.n_slots; p.slot_bytes = slot_bytes;
-    for (int b = 0; b < cs.n_ctas; ++b) p.cta_steps.push_back(cs.cta_step_begin[(size_t)b + 1] - cs.cta_step_begin[(size_t)b]);
+    p.min_steps = 1 << 30;
+    for (int b = 0; b < cs.n_ctas; ++b) p.min_steps = std::min(p.min_steps, cs.cta_step_begin[(size_t)b + 1] - cs.cta_step_begin[(size_t)b]);
     if ((rc = dev_alloc(g, 1, &p.progress))) return rc;
-    CU_TRY(cudaMemset(p.progress, 0, sizeof(unsigned long long)));
-    p.stats[0] = (int64_t)cs.steps.size(); p.stats[1] = cs.n_sync_steps; p.stats[2] = cs.n_vn_loads; p.stats[3] = cs.n_w_loads; p.stats[4] = cs.n_copies;
+    CU_TRY(cudaMemset(p.progress, 0, sizeof(unsigned long long)));      // synchronous: ordered before any later launch
+    p.stats[0] = (int64_t)cs.steps.size(); p.stats[1] = cs.n_sync_steps; p.stats[2] = cs.n_vn_loads; p.stats[3] = cs.n_w_loads;
+    p.stats[4] = cs.n_copies;
     p.ready = true;
     return ICON_OK;
 }
@@ -525,9 +516,6 @@ int icon_grid_create(int bisections_k, uint64_t seed, unsigned flags, icon_grid_
     g->seed = seed;
     g->host_only = (flags & ICON_HOST_ONLY) != 0;
     g->options[ICON_OPT_TENDENCY_KERNEL] = 5;
-    g->options[ICON_OPT_CC_SHAPE] = -1;
-    g->options[ICON_OPT_CC_L2_HINTS] = 19;
-    g->options[ICON_OPT_CC_MERGE] = 1;
     g->options[ICON_OPT_CC_TILE] = 16;
     g->options[ICON_OPT_CC_PACE] = 512;
     try {
@@ -634,9 +622,7 @@ int icon_grid_set_option(icon_grid_t* g, int option, int value) {
     if (!g) return fail(ICON_EINVAL, "grid handle is NULL");
     if (option < 0 || option >= ICON_OPT_COUNT) return fail(ICON_EINVAL, "unknown option");
     if (option == ICON_OPT_CC_PACE && (value < 0 || value > 65536 || (value & (value - 1)))) return fail(ICON_EINVAL, "bad option value");
-    if (option == ICON_OPT_CC_TILE && (value < 0 || value > 4096 || value % 2)) return fail(ICON_EINVAL, "bad option value");
-    if (option == ICON_OPT_CC_L2_HINTS && (value < 0 || value > 31)) return fail(ICON_EINVAL, "bad option value");
-    if (option == ICON_OPT_CC_SHAPE && (value < -1 || value >= icon::kCcNumShapes)) return fail(ICON_EINVAL, "bad option value");
+    if (option == ICON_OPT_CC_TILE && (value < 0 || value > 4096 || value % icon::kCcGroup)) return fail(ICON_EINVAL, "bad option value");
     if (option == ICON_OPT_TENDENCY_KERNEL && (value < 0 || value > 5)) return fail(ICON_EINVAL, "bad option value");
     g->options[option] = value;
     return ICON_OK;
@@ -672,15 +658,11 @@ int icon_grid_cc_schedule_check(icon_grid_t* g, int dtype, int nlev, int ldk, in
     int rc = ensure_sc_host(g);
     if (rc) return rc;
     const bool f64 = dtype == ICON_F64;
-    const int shape = cc_resolve_shape(g, f64, nlev);
-    const bool merge = g->options[ICON_OPT_CC_MERGE] != 0;
-    const icon::CcGeometry geom = f64 ? cc_geometry<double>(nlev, ldk, ldk_w, merge) : cc_geometry<float>(nlev, ldk, ldk_w, merge);
-    const int n_slots = std::min(65535, f64 ? icon::cc_max_slots<double>(shape, nlev, geom.slot_bytes, smem_bytes, (g->options[ICON_OPT_CC_L2_HINTS] & 16) != 0)
-                                            : icon::cc_max_slots<float>(shape, nlev, geom.slot_bytes, smem_bytes, (g->options[ICON_OPT_CC_L2_HINTS] & 16) != 0));
+    const icon::CcGeometry geom = f64 ? cc_geometry<double>(nlev, ldk, ldk_w) : cc_geometry<float>(nlev, ldk, ldk_w);
+    const int n_slots = std::min(65535, f64 ? icon::cc_max_slots<double>(geom.slot_bytes, smem_bytes) : icon::cc_max_slots<float>(geom.slot_bytes, smem_bytes));
     icon::CcSchedule cs;
     try {
-        std::string err = icon::build_cc_schedule(g->sc_host, n_ctas, n_slots, geom, icon::cc_shape(shape).group,
-                                                  icon::cc_shape(shape).depth, g->options[ICON_OPT_CC_TILE], cs);
+        std::string err = icon::build_cc_schedule(g->sc_host, n_ctas, n_slots, geom, icon::kCcGroup, icon::kCcDepth, g->options[ICON_OPT_CC_TILE], cs);
         if (!err.empty()) return fail(ICON_EUNSUPPORTED, err);
         err = icon::check_cc_schedule(g->sc_host, cs, g->host.ne, g->host.nc);
         if (!err.empty()) return fail(ICON_EINVAL, err);

@@ -90,18 +90,21 @@ void simulate_cta(const ScTables& sc, const int64_t* order, int64_t pb, int64_t 
             r.ok = false;
             return;
         }
-        // The misses, grouped into runs of consecutive column ids of one kind.
-        struct Run { int kind; uint32_t id; int len; size_t first; };   // first = index into `morder`
-        std::vector<size_t> morder(miss);                                 // indices into ks, by (kind, id)
-        std::sort(morder.begin(), morder.end(), [&](size_t a, size_t b2) {
-            const uint64_t ka = ks[a], kb = ks[b2];
-            if ((ka & 1) != (kb & 1)) return (ka & 1) < (kb & 1);
-            return (ka >> 1) < (kb >> 1);
+        // What this step loads: its misses (key, next use after this step)
+        struct Item { uint64_t key; int32_t next; };
+        std::vector<Item> items;
+        items.reserve(miss.size());
+        for (size_t mi : miss) items.push_back(Item{ks[mi], nu[mi]});
+        std::sort(items.begin(), items.end(), [](const Item& a, const Item& b2) {
+            if ((a.key & 1) != (b2.key & 1)) return (a.key & 1) < (b2.key & 1);
+            return (a.key >> 1) < (b2.key >> 1);
         });
+        // grouped into runs of consecutive column ids of one kind
+        struct Run { int kind; uint32_t id; int len; size_t first; };   // first = index into `items`
         std::vector<Run> runs;
-        for (size_t m = 0; m < morder.size(); ++m) {
-            const int kind = (int)(ks[morder[m]] & 1);
-            const uint32_t id = (uint32_t)(ks[morder[m]] >> 1);
+        for (size_t m = 0; m < items.size(); ++m) {
+            const int kind = (int)(items[m].key & 1);
+            const uint32_t id = (uint32_t)(items[m].key >> 1);
             const bool mergeable = geom.stride_bytes[kind] == geom.slot_bytes;
             if (!runs.empty() && mergeable && runs.back().kind == kind && runs.back().len < kCcMaxRun &&
                 runs.back().id + (uint32_t)runs.back().len == id) {
@@ -152,12 +155,12 @@ void simulate_cta(const ScTables& sc, const int64_t* order, int64_t pb, int64_t 
             }
             for (int t = 0; t < run.len; ++t) {
                 const int32_t q = best + t;
-                const size_t mi = morder[run.first + (size_t)t];
-                const uint64_t k = ks[mi];
+                const Item& it = items[run.first + (size_t)t];
+                const uint64_t k = it.key;
                 if (slot_key[(size_t)q] != ~0ull) resident.erase(slot_key[(size_t)q]);
                 slot_key[(size_t)q] = k;
                 slot_last[(size_t)q] = (int32_t)s;
-                slot_next[(size_t)q] = nu[mi];
+                slot_next[(size_t)q] = it.next;
                 slot_loaded[(size_t)q] = (int32_t)s;
                 evictable[(size_t)q] = 0;
                 resident[k] = q;

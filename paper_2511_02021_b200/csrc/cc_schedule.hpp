@@ -2,19 +2,22 @@
 // internal header).
 //
 // The kernel keeps whole vn / w columns in shared memory ("slots") and fills them with bulk
-// asynchronous copies (cp.async.bulk, the 1-D TMA path) issued by a producer warp; eight consumer
-// warps each finish one self-contained patch (sc_tables.hpp) per STEP from those slots. Which
-// column sits in which slot at which step is decided HERE, on the host, once per grid: the work
-// order of every CTA is fixed (a contiguous range of the generation order), so the whole future
-// of the reference stream is known and the replacement is Belady's (evict the column whose next
-// use is farthest). The device never searches or hashes anything: a step is a list of
-// (column id, slot) loads plus, per patch, the slot of each of its 43 columns.
+// asynchronous copies (cp.async.bulk, the 1-D TMA path) issued by a warpgroup of producer warps; eight
+// consumer warps in two groups each finish one self-contained patch (sc_tables.hpp) per STEP (= four
+// patches) from those slots. Which column sits in which slot at which step is decided HERE, on the host,
+// once per grid: the work order of every CTA is fixed (tiles of consecutive patches of the generation
+// order dealt round-robin to the CTAs), so the whole future of the reference stream is known and the
+// replacement is Belady's (evict the column whose next use is farthest). The device never searches or
+// hashes anything: a step is a list of (first column id, first slot, bytes) copies plus, per patch, the
+// slot of each of its 43 columns.
 //
-// Pipeline rule the schedule guarantees (kernels_cc.cu relies on it): the loads of step s only
-// overwrite slots whose last reader ran in a step <= s-2, so they can be in flight while step
-// s-1 computes; a step flagged `sync` may also overwrite slots last read in step s-1 and the
-// producer waits for that step to drain first (rare: only when two consecutive steps together
-// need more columns than there are slots).
+// Pipeline rule the schedule guarantees (kernels_cc.cu relies on it, cc_schedule_check.cpp replays it):
+// the loads of step s only overwrite slots whose last reader ran in a step <= s - depth(s), with
+// depth(s) = kCcDepth normally (the copies of step s are in flight while the steps s-1 .. s-depth+1
+// compute) and smaller (stored per step) only when the steps in flight together need more columns
+// than there are slots; the producers issue the copies of step s once step s - depth(s) has drained.
+// A patch that reads a column loaded by one of the steps s-1 .. s-kCcDepth+1 names that step in its
+// wait mask (copies of different steps complete in any order).
 #pragma once
 #include <cstdint>
 #include <string>
@@ -24,11 +27,13 @@
 
 namespace icon {
 
-// pipeline shapes of the kernel (kernels_cc.cu): consumer warps, patches per step, ring depth.
-// kCcProducers producer warps (one warpgroup) are added to `warps`; the CTA is launched with
-// 168 registers per thread and re-balances them with setmaxnreg: producers keep
-// CcWarps<T>::producer_regs, consumers grow to CcWarps<T>::consumer_regs
-// (the pool is what the launch allocated: 384 * 168 = (4 * 56 + 8 * 224) * 32 = 64512 registers).
+// Pipeline shape of the kernel (kernels_cc.cu): kCcWarps consumer warps in groups of kCcGroup (= patches per
+// step), ring of kCcDepth steps. Measured against 8/2/6 (two patches per step, ring of six) on B200: config 3
+// 5.11 -> 4.91 ms, config 4 4.01 -> 3.38 ms, config 5 12.25 -> 9.84 ms.
+constexpr int kCcWarps = 8, kCcGroup = 4, kCcDepth = 3;
+// Producer warps are added to the consumers; the CTA is launched with the registers of the average warp and
+// re-balances them with setmaxnreg: producers keep CcWarps::producer_regs, consumers grow to CcWarps::consumer_regs
+// (the pool is what the LAUNCH allocated: 384 * 168 = (4 * 56 + 8 * 224) * 32 = 64512 registers).
 // 8-byte columns: 4 producer warps with 56 registers, 8 consumer warps with 224 (launch: 384 threads x 168).
 // 4-byte columns: the consumers need fewer registers and the columns are half as long, i.e. twice the copies per byte,
 // so a second producer warpgroup issues them: 8 producer warps with 40 registers, consumers 216 (launch: 512 x 128).
@@ -42,18 +47,7 @@ struct CcWarps {
 };
 constexpr int kCcMaxProducers = 8;
 constexpr int kCcAhead = 3;              // steps the producers read the schedule ahead; `loads` is padded for it
-struct CcShape {
-    int warps, group, depth;
-};
-constexpr int kCcNumShapes = 2;
-#ifndef CC_S1_G          // shape 1 can be re-defined at build time for pipeline-shape experiments (ICON_NVCC_EXTRA)
-#define CC_S1_G 4
-#define CC_S1_D 3
-#endif
-constexpr CcShape kCcShapes[kCcNumShapes] = {{8, 2, 6}, {8, CC_S1_G, CC_S1_D}};
-inline const CcShape& cc_shape(int i) { return kCcShapes[i >= 0 && i < kCcNumShapes ? i : 0]; }
 constexpr int kCcBarrierBytes = 512;    // the mbarriers
-constexpr int kCcOutCols = 3;            // ddt_vn staging columns per consumer warp (one store batch)
 // a patch record on the device = kScCoefWords coefficients (T), then kCcRecordIds int32 (user ids of
 // the outputs), then kCcSlotWords uint32 byte offsets of the slots; c_lin is
 // stored halved there (the kernel forms w(k) + w(k+1) = 2 w_f(k))
@@ -69,7 +63,7 @@ struct CcStep {                      // 16 bytes
     uint16_t n_loads;                // bulk copies of this step (a copy moves a run of 1..kCcMaxRun columns)
     uint8_t n_patches;               // 1..group
     uint8_t depth;                   // the loads may be issued once step s-depth has drained (1..schedule depth)
-    uint32_t tx16;                   // bytes / 16 those copies deliver (patch records not included)
+    uint32_t tx16;                   // bytes / 16 those copies deliver (patch records not included); for the checker
     uint32_t ahead_begin;            // load_begin of step s + kCcAhead of the same CTA (the producers' prefetch)
 };
 

@@ -4,7 +4,8 @@
 //
 //   1. every bulk copy of a step lands in slots [slot, slot + n) inside the pool, n = columns of the run;
 //   2. it never overwrites a slot that a patch of the steps s-depth+1 .. s reads (those may still be
-//      running, or are this step's own hits);
+//      running, or are this step's own hits), nor a slot that one of those steps filled (its copy may still be in
+//      flight);
 //   3. after the copies of step s, each of the 43 slots a patch of step s names holds exactly the
 //      column (kind, id) its record names;
 //   4. the byte count the step header announces (tx16) is the sum of its copies, every copy is a
@@ -77,6 +78,7 @@ std::string check_cc_schedule(const ScTables& sc, const CcSchedule& cs, int64_t 
                 for (int64_t t = 0; t < n; ++t) {
                     const size_t q = (size_t)ld.slot + (size_t)t;
                     if (last_read[q] > s - st.depth) { fail(10); break; }          // a reader may still be running
+                    if (loaded_at[q] > s - st.depth) { fail(15); break; }          // an earlier copy into it may still be in flight
                     content[q] = ((int64_t)ld.id + t) * 2 + kind;
                     loaded_at[q] = s;
                     last_read[q] = -1000000;

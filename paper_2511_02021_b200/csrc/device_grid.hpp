@@ -84,15 +84,10 @@ struct DevCcTables {
     int64_t* cta_step_begin = nullptr;
     int n_ctas = 0, n_slots = 0, slot_bytes = 0;
     int nlev = -1;                 // the level count the slot size was derived from
-    int shape = -1;                // index into kCcShapes the schedule was built for
     int64_t ldk = -1, ldk_w = -1;  // column strides the runs were merged for
-    bool merge = true;             // ICON_OPT_CC_MERGE it was built with
     int tile = -1;                 // ICON_OPT_CC_TILE it was built with
     unsigned long long* progress = nullptr;   // device counter of the producers' pacing barriers, never reset
-    int64_t pace_events = 0;       // value of *progress once every launch so far has finished
-    int64_t max_steps = 0;
-    std::vector<int64_t> cta_steps;           // steps of every CTA
-    bool direct = true;            // store path (ICON_OPT_CC_L2_HINTS bit 16) the slot count was derived for
+    int64_t min_steps = 0;         // steps of the CTA with the fewest (pacing barriers every CTA reaches)
     bool ready = false;
     bool unsupported = false;      // this (T, nlev) cannot use the kernel: callers fall back
     int64_t stats[5] = {0, 0, 0, 0, 0};   // steps, steps with reduced depth, vn columns, w columns, bulk copies

@@ -51,6 +51,6 @@ int cc_levels_per_lane(int nlev);
 template <class T>
 int cc_slot_bytes(int nlev);
 template <class T>
-int cc_max_slots(int shape, int nlev, int slot_bytes, int smem_optin, bool direct);
+int cc_max_slots(int slot_bytes, int smem_optin);
 
 }  // namespace icon

@@ -1,31 +1,32 @@
 // kernels_cc.cu -- column-cache kernel for the velocity tendency and, fused
 // into the same pass on request, divergence and vorticity (S1, S2: dycore_step), sm_100a.
 //
-// Same arithmetic per patch as kernels_sc.cu (one warp finishes one self-contained patch, lanes =
-// levels, no exchange between warps), but the vn / w columns no longer come through the L1: four
-// PRODUCER warps (one warpgroup, setmaxnreg down to 56 registers) move whole columns from HBM into
+// One warp finishes one self-contained patch (sc_tables.hpp: four sibling cells, six owned edges,
+// 36 vn + 7 w columns, no exchange between warps), lanes = levels. The vn / w columns do not come
+// through the L1: PRODUCER warps (one warpgroup, setmaxnreg down) move whole columns from HBM into
 // shared-memory slots with bulk asynchronous copies (cp.async.bulk = the 1-D TMA path, completion on
 // an mbarrier), following a schedule the host computed once per grid (cc_schedule.hpp: which columns
 // into which slots at which step, Belady replacement, consecutive ids merged into one copy). Eight
-// CONSUMER warps (setmaxnreg up to 224 registers) read the slots:
+// CONSUMER warps (setmaxnreg up) read the slots:
 //
 //   * every column crosses L2 -> SM once per residency instead of once per patch that touches it
 //     (~15 instead of 43 column fetches per patch), and the fetches are in flight one or more steps
 //     ahead of their readers without holding a single register;
-//   * a lane owns L CONSECUTIVE levels (k = L*lane .. L*lane+L-1; L odd, so the 8-byte stride-L
-//     shared-memory reads are bank-conflict free), so the vertical stencil (S6) needs one shuffle
-//     up and one down per column instead of one pair per 32-level chunk, and a coefficient / slot
-//     lookup, which is warp-uniform, is paid once per L*32 levels;
-//   * output columns are transposed through a per-warp staging column and leave with plain
-//     coalesced streaming stores (DIRECT; the alternative, bulk stores from the staging columns,
-//     costs a proxy fence and a wait for the copy engine to read the previous batch out);
+//   * a lane owns L = 3 levels of a column, the PAIR 2*lane, 2*lane+1 and the single level 64+lane
+//     (L = 1, nlev <= 31: level = lane): a coefficient / slot lookup, which is warp-uniform, is paid once
+//     per 96 levels; a column is read with one 16-byte and one 8-byte conflict-free shared-memory load
+//     per lane, and an output column leaves STRAIGHT FROM REGISTERS with one 16-byte and one 8-byte
+//     coalesced streaming store -- no transposition through shared memory (the previous mapping, three
+//     consecutive levels per lane, paid 12 L1 wavefronts per output column for it, 144 of ~740 per
+//     patch); the vertical stencil (S6) costs two shuffles up and two down per column (inside the pair
+//     the neighbour level is in the lane's own registers);
 //   * FUSED: div of the patch's four cells comes from the nine in-patch columns, and the sums zm, zc
 //     the tendency needs ARE half the vorticity at the patch's three midpoint and three corner
 //     vertices; every vertex of the grid is one of those for some patch, the lowest patch stores it.
 //
-// Why four producer warps: issuing one bulk copy is a ~100-cycle serial chain on the uniform datapath
+// Why a warpgroup of producers: issuing one bulk copy is a ~100-cycle serial chain on the uniform datapath
 // (R2UR / ELECT / UBLKCP), and an SM accepts one copy per ~31 cycles at best
-// (profiles/r01_bulk_copy_microbench.md), so the issue is spread over a warpgroup and runs of
+// (profiles/r01_bulk_copy_microbench.md), so the issue is spread over four (eight) warps and runs of
 // columns are merged. Why the warp index goes through a shuffle: it makes the role / range branches
 // uniform for the compiler, which removed a third of the instructions (divergence handling around
 // every shuffle) -- the kernel had outgrown the instruction cache.
@@ -43,9 +44,8 @@
 // so the previous phase of any barrier it waits on is closed) and NB >= 2D-1 (the next phase of a
 // barrier awaited for step s-r cannot open before step s itself has drained). Every producer warp
 // arrives on every step, so none of them can fall a whole ring behind either.
-#include <cuda_pipeline.h>
-
 #include <cstdio>
+#include <mutex>
 
 #include "../../include/icon_dycore.h"
 #include "kernels.cuh"
@@ -69,7 +69,8 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
 #ifdef CC_DEBUG
-// debug build: a wait that does not end reports where it hangs and traps
+// debug build (python -m paper_2511_02021_b200.build --force with ICON_NVCC_EXTRA=-DCC_DEBUG): a wait that does
+// not end reports where it hangs and traps
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity, int what = 0, int step = 0) {
     for (long it = 0;; ++it) {
         uint32_t ok;
@@ -85,6 +86,9 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity, int wha
     }
 }
 #else
+// Plain polling loop on purpose: a try_wait with a suspend-time hint (500 ns, 2 us and 10 ms measured) made the fused
+// step 6 % slower whatever the value (4.69 ms against 4.41 ms), although the polling instructions are a quarter of all
+// instructions the kernel issues.
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity, int = 0, int = 0) {
     asm volatile(
         "{\n"
@@ -102,37 +106,16 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
                  "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
-// the same with an L2 eviction-priority hint (policy from l2_policy_*)
+// the same with an L2 eviction-priority hint
 __device__ __forceinline__ void bulk_g2s_hint(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar, uint64_t pol) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(dst),
                  "l"(src), "r"(bytes), "r"(bar), "l"(pol) : "memory");
-}
-// shared -> global, tracked by the issuing thread's bulk async-group
-__device__ __forceinline__ void bulk_s2g(void* dst, uint32_t src, uint32_t bytes) {
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void bulk_s2g_hint(void* dst, uint32_t src, uint32_t bytes, uint64_t pol) {
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;" ::"l"(dst), "r"(src),
-                 "r"(bytes), "l"(pol) : "memory");
 }
 __device__ __forceinline__ uint64_t l2_policy_evict_first() {
     uint64_t p;
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
     return p;
 }
-__device__ __forceinline__ uint64_t l2_policy_evict_last() {
-    uint64_t p;
-    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
-    return p;
-}
-__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void bulk_wait_read() {
-    asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory");
-}
-__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
-// generic-proxy writes to shared memory -> visible to the async proxy (bulk store source)
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 // ---- device view of the schedule ------------------------------------------------------------------
 template <class T>
@@ -146,28 +129,47 @@ struct CcDev {
     int slot_bytes;
 };
 
-// ---- L consecutive levels of one column, per lane ---------------------------------------------------
+// ---- the L levels of one column a lane owns ---------------------------------------------------------
+// L == 3: v[0], v[1] = levels 2*lane, 2*lane+1 (one 16-byte access), v[2] = level 64+lane. L == 1: level = lane.
 template <class T, int L>
 struct Col {
     T v[L];
 };
 #define FORL _Pragma("unroll") for (int l = 0; l < L; ++l)
 
-// value one level up (k-1) / down (k+1): inside the lane except at its ends
+template <int L>
+__device__ __forceinline__ int level_of(int lane, int l) { return L == 1 ? lane : (l < 2 ? 2 * lane + l : 64 + lane); }
+
+template <class T> struct Pair;
+template <> struct Pair<double> { using type = double2; };
+template <> struct Pair<float> { using type = float2; };
+
+// value one level up (k-1) / down (k+1). Inside the pair the neighbour is the lane's own register; across lanes one
+// shuffle per segment. The seam between the segments (levels 63 | 64) rides on the same shuffles: lane 31 feeds its
+// level 63 to lane 0's level 64 (up), lane 0 feeds its level 64 to lane 31's level 63 (down). Lanes whose neighbour
+// level does not exist get a value the caller masks.
 template <class T, int L>
-__device__ __forceinline__ Col<T, L> level_up(const Col<T, L>& a) {
+__device__ __forceinline__ Col<T, L> level_up(const Col<T, L>& a, int lane) {
     Col<T, L> r;
-    r.v[0] = __shfl_up_sync(kFull, a.v[L - 1], 1);
-#pragma unroll
-    for (int l = 1; l < L; ++l) r.v[l] = a.v[l - 1];
+    if constexpr (L == 1) {
+        r.v[0] = __shfl_up_sync(kFull, a.v[0], 1);
+    } else {
+        r.v[0] = __shfl_up_sync(kFull, a.v[1], 1);
+        r.v[1] = a.v[0];
+        r.v[2] = __shfl_sync(kFull, lane == 31 ? a.v[1] : a.v[2], (lane + 31) & 31);
+    }
     return r;
 }
 template <class T, int L>
-__device__ __forceinline__ Col<T, L> level_down(const Col<T, L>& a) {
+__device__ __forceinline__ Col<T, L> level_down(const Col<T, L>& a, int lane) {
     Col<T, L> r;
-#pragma unroll
-    for (int l = 0; l < L - 1; ++l) r.v[l] = a.v[l + 1];
-    r.v[L - 1] = __shfl_down_sync(kFull, a.v[0], 1);
+    if constexpr (L == 1) {
+        r.v[0] = __shfl_down_sync(kFull, a.v[0], 1);
+    } else {
+        r.v[0] = a.v[1];
+        r.v[1] = __shfl_sync(kFull, lane == 0 ? a.v[2] : a.v[0], (lane + 1) & 31);
+        r.v[2] = __shfl_down_sync(kFull, a.v[2], 1);
+    }
     return r;
 }
 template <class T, int L>
@@ -224,18 +226,17 @@ __device__ __forceinline__ void ld_slots(const uint32_t* __restrict__ p, uint32_
 template <class T>
 __host__ __device__ constexpr int cc_record_bytes() { return kScCoefWords * (int)sizeof(T) + kCcRecordTail; }
 
-// W consumer warps in W/G groups of G; group g runs the steps s = g (mod W/G). D = ring depth.
+// kCcWarps consumer warps in two groups of kCcGroup; group g runs the steps s = g (mod 2); ring depth kCcDepth.
 // FUSED: the same pass also stores div of the patch's four cells and the vorticity of the vertices the
 // patch owns (dycore_step): both are by-products of columns and sums the tendency needs anyway.
-// DIRECT: outputs leave by coalesced stores (transposed in shared memory) instead of bulk stores; a template
-// parameter because compiling both paths into one kernel overflowed the instruction cache.
-template <class T, int L, int W, int G, int D, bool FUSED, bool DIRECT>
-__global__ void __launch_bounds__((W + CcWarps<T, L>::producers) * 32, 1)
-k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restrict__ abc, const T* __restrict__ vn,
+template <class T, int L, bool FUSED>
+__global__ void __launch_bounds__((kCcWarps + CcWarps<T, L>::producers) * 32, 1)
+k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, const T* __restrict__ vn,
           const T* __restrict__ w, T* __restrict__ ddt_vn, T* __restrict__ div, T* __restrict__ vort,
-          unsigned long long* pace_counter, unsigned long long pace_base, int pace_mask, int pace_last) {
+          unsigned long long* pace_counter, unsigned long long pace_per_launch, int pace_mask, int pace_last) {
     extern __shared__ __align__(128) unsigned char smem[];
     using C = Col<T, L>;
+    constexpr int W = kCcWarps, G = kCcGroup, D = kCcDepth;
     constexpr int kCcProducers = CcWarps<T, L>::producers;
     constexpr int REC = cc_record_bytes<T>();
     constexpr int NGRP = W / G;
@@ -243,12 +244,9 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
     // the shuffle tells the compiler that the warp index is warp-uniform: branches on it (role, patch in range)
     // become uniform branches and the shuffles below need no divergence handling
     const int warp = __shfl_sync(kFull, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
-    const int out_bytes = (nlev * (int)sizeof(T) + 15) & ~15;                 // staging column, 16-byte multiple
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem);                       // full[D], done[D]
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem);                       // full[NB], done[NB]
     unsigned char* rec_base = smem + kCcBarrierBytes;
-    unsigned char* out_base = rec_base + D * G * REC;
-    constexpr int OUTC = DIRECT ? 1 : kCcOutCols;      // staging columns per consumer warp
-    unsigned char* slot_base = out_base + W * OUTC * out_bytes;
+    unsigned char* slot_base = rec_base + D * G * REC;
     const uint32_t bar0 = smem_u32(bars);
     auto full_bar = [&](int i) { return bar0 + 8u * (uint32_t)i; };
     // NB >= 2D-1 and >= NGRP+D: see the parity argument in the header comment
@@ -271,19 +269,28 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
     __syncthreads();
 
     if (warp >= W) {
-        // ================= producers (one warpgroup) =================
+        // ================= producers (one or two warpgroups) =================
         // Issuing a bulk copy costs a ~100-cycle chain on the uniform datapath, so the list of a
         // step is dealt round-robin to kCcProducers warps. Registers go to the consumers.
         asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(CcWarps<T, L>::producer_regs));
-        // hints: bit 0 = ddt_vn stores evict-first, bit 1 = patch records evict-first, bit 2 = columns evict-last
         const int pw = warp - W;
         const uint64_t cs = (uint64_t)ldk * sizeof(T), cs_w = (uint64_t)ldk_w * sizeof(T);
         const uint32_t slot0 = smem_u32(slot_base), rec0 = smem_u32(rec_base);
-        const uint64_t pol_first = l2_policy_evict_first(), pol_last = l2_policy_evict_last();
-        const bool hint_rec = hints & 2, hint_col = hints & 4;
+        const uint64_t pol_first = l2_policy_evict_first();
         const uint2* lraw = reinterpret_cast<const uint2*>(d.loads);
         const int mine = kCcProducers * lane + pw;          // this lane's entry of each round of 32 * kCcProducers
         int drained = 0;
+        // Pacing epoch: the counter is never reset and every launch adds exactly pace_per_launch events, so the
+        // events of all earlier launches are the multiple of pace_per_launch at or below the value this CTA reads
+        // before it adds its own first event (launches of one handle are stream-ordered; the counter cannot reach
+        // the next multiple before every CTA, this one included, has added all of its events). Kept on the device so
+        // that a captured CUDA graph replays correctly.
+        unsigned long long pace_base = 0;
+        if (FUSED && !CcWarps<T, L>::light && pace_mask && lane == 0) {
+            unsigned long long have;
+            asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(have) : "l"(pace_counter) : "memory");
+            pace_base = have - have % pace_per_launch;
+        }
         // The schedule is read kCcAhead steps ahead through a register ring (the step loop is unrolled
         // by kCcAhead so that the ring is statically indexed): header s+kCcAhead, and this lane's first
         // list entry of step s+kCcAhead, whose position header s already names (CcStep::ahead_begin).
@@ -349,10 +356,10 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
                     __syncwarp();
                     if (rec_warp && lane == 0) {
                         // the records of a step's patches are consecutive in memory and in the ring: one copy
+                        // (evict-first: a record is read once)
                         const int64_t p = pb + (int64_t)s * G;
                         const uint32_t dst = rec0 + (uint32_t)(((s % D) * G) * REC);
-                        if (hint_rec) bulk_g2s_hint(dst, d.records + p * REC, n_pat * (uint32_t)REC, fb, pol_first);
-                        else bulk_g2s(dst, d.records + p * REC, n_pat * (uint32_t)REC, fb);
+                        bulk_g2s_hint(dst, d.records + p * REC, n_pat * (uint32_t)REC, fb, pol_first);
                     }
                     for (int base = 0; base + mine < n_loads; base += 32 * kCcProducers) {
                         const uint2 q = base == 0 ? e0 : __ldg(lraw + load_begin + base + mine);
@@ -360,9 +367,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
                         const uint32_t slot = q.y & 0xffffu, kind = q.y >> 31, bytes = ((q.y >> 16) & 0x7fffu) << 4;
                         const unsigned char* src = kind ? reinterpret_cast<const unsigned char*>(w) + (uint64_t)q.x * cs_w
                                                         : reinterpret_cast<const unsigned char*>(vn) + (uint64_t)q.x * cs;
-                        const uint32_t dst = slot0 + slot * (uint32_t)d.slot_bytes;
-                        if (hint_col) bulk_g2s_hint(dst, src, bytes, fb, pol_last);
-                        else bulk_g2s(dst, src, bytes, fb);
+                        bulk_g2s(slot0 + slot * (uint32_t)d.slot_bytes, src, bytes, fb);
                     }
                 }
             }
@@ -373,25 +378,22 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
 
     // ================= consumers =================
     const int grp = warp / G, wi = warp % G;
-    // per-lane level coefficients of the vertical term (reading P-14): levels L*lane + l
+    // per-lane level coefficients of the vertical term (reading P-14)
     T cA[L], cB[L], cC[L];
     bool po[L];              // this lane's levels that exist in a vn / ddt_vn column
+    bool below_missing[L];   // level k+1 does not exist (k = nlev-1) or lies past the column end
     FORL {
-        const int k = L * lane + l;
+        const int k = level_of<L>(lane, l);
         po[l] = k < nlev;
+        below_missing[l] = k + 1 >= nlev;
         cA[l] = po[l] ? __ldg(abc + k) : (T)0;
         cB[l] = po[l] ? __ldg(abc + nlev + k) : (T)0;
         cC[l] = po[l] ? __ldg(abc + 2 * nlev + k) : (T)0;
     }
-    unsigned char* my_out = out_base + warp * OUTC * out_bytes;
-    const int bulk_out = (nlev * (int)sizeof(T)) & ~15;       // bytes of a ddt_vn column that leave by bulk store
     const uint64_t cs = (uint64_t)ldk * sizeof(T);
-    const uint32_t lane_off = (uint32_t)(L * lane * (int)sizeof(T));
-    const unsigned char* my_slots = slot_base + lane_off;
-    bool below_missing[L];   // level k+1 does not exist (k = nlev-1) or belongs to a lane past the column end
-    FORL below_missing[l] = L * lane + l + 1 >= nlev;
-    const uint64_t pol_first = l2_policy_evict_first();
-    const bool hint_out = hints & 1;
+    // this lane's two read positions inside every slot
+    const unsigned char* my_pair = slot_base + (L == 1 ? lane : 2 * lane) * (int)sizeof(T);
+    const unsigned char* my_single = slot_base + (64 + lane) * (int)sizeof(T);
 
     for (int s = grp; s < n_steps; s += NGRP) {
         const int64_t p = pb + (int64_t)s * G + wi;
@@ -402,80 +404,47 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
             const int32_t* oid = reinterpret_cast<const int32_t*>(rec + kScCoefWords * sizeof(T));
             const uint32_t* sl = reinterpret_cast<const uint32_t*>(rec + kScCoefWords * sizeof(T) + kCcRecordIds * 4);
 
-            // Every lane reads its natural levels L*lane .. L*lane+L-1, whether they exist or not: the
-            // stride-L pattern is conflict free as a whole, lanes past the column end pick up stale
-            // bytes of the slot (or of the next one) that only ever reach outputs through the
-            // level-below neighbour of the last level, which VD masks.
+            // Every lane reads its levels whether they exist or not: lanes past the column end pick up stale bytes of
+            // the slot (or of the next one; the pool ends with a readable pad) that only ever reach outputs through
+            // the level-below neighbour of the last level, which VD masks.
             auto LD = [&](uint32_t off) {
-                const T* q = reinterpret_cast<const T*>(my_slots + off);
                 C c;
-                FORL c.v[l] = q[l];
+                if constexpr (L == 1) {
+                    c.v[0] = *reinterpret_cast<const T*>(my_pair + off);
+                } else {
+                    const typename Pair<T>::type pr = *reinterpret_cast<const typename Pair<T>::type*>(my_pair + off);
+                    c.v[0] = pr.x; c.v[1] = pr.y;
+                    c.v[2] = *reinterpret_cast<const T*>(my_single + off);
+                }
                 return c;
             };
             auto WS = [&](uint32_t off) {       // w(k) + w(k+1) = 2 w_f(k) (S6); the 1/2 is folded into c_lin
                 const C c = LD(off);
-                const C dn = level_down(c);
+                const C dn = level_down(c, lane);
                 C o;
                 FORL o.v[l] = c.v[l] + dn.v[l];
                 return o;
             };
             auto VD = [&](const C& x) {         // (vn_ie(k) - vn_ie(k+1)) / dz_k, reading P-14 folded into A, B, C
-                C up = level_up(x), dn = level_down(x), o;
+                C up = level_up(x, lane), dn = level_down(x, lane), o;
                 FORL if (below_missing[l]) dn.v[l] = (T)0;      // C_k = 0 there, but the stale value may be NaN
                 FORL o.v[l] = cA[l] * up.v[l] + cB[l] * x.v[l] + cC[l] * dn.v[l];
                 return o;
             };
-            // Up to kCcOutCols finished output columns leave together: staged in shared memory (stride-L
-            // writes, conflict free), one proxy fence, then one bulk store each; ids[j] < 0 = no column j
-            auto ST3 = [&](T* base, const int32_t* ids, const C* x) {
-                if constexpr (DIRECT) {
-                    // transposed through the warp's staging column and written with plain coalesced stores:
-                    // costs L1-pipe wavefronts (read back + store) but no copy-engine request, no proxy fence
-                    // and no wait for the previous batch to be read out
-#pragma unroll
-                    for (int j = 0; j < kCcOutCols; ++j) {
-                        if (ids[j] < 0) continue;
-                        __syncwarp();                       // the previous column has been read back
-                        T* q = reinterpret_cast<T*>(my_out + lane_off);
-                        FORL if (po[l]) q[l] = x[j].v[l];
-                        __syncwarp();
-                        const T* r = reinterpret_cast<const T*>(my_out);
-                        T* dst = reinterpret_cast<T*>(reinterpret_cast<unsigned char*>(base) + (uint64_t)(uint32_t)ids[j] * cs);
-#pragma unroll
-                        for (int c = 0; c < L; ++c) {
-                            const int k = c * 32 + lane;
-                            if (k < nlev) __stcs(dst + k, r[k]);       // streaming: outputs should not push halo columns out of L2
-                        }
-                    }
+            // one finished output column, straight from the registers: coalesced streaming stores (outputs should
+            // not push halo columns out of the L2); id < 0 = not ours
+            auto ST = [&](T* base, int32_t id, const C& x) {
+                if (id < 0) return;
+                T* dst = reinterpret_cast<T*>(reinterpret_cast<unsigned char*>(base) + (uint64_t)(uint32_t)id * cs);
+                if constexpr (L == 1) {
+                    if (po[0]) __stcs(dst + lane, x.v[0]);
                 } else {
-                if (lane == 0) bulk_wait_read<0>();        // the previous batch has been read out of the staging columns
-                __syncwarp();
-#pragma unroll
-                for (int j = 0; j < kCcOutCols; ++j) {
-                    if (ids[j] < 0) continue;
-                    T* q = reinterpret_cast<T*>(my_out + j * out_bytes + lane_off);
-                    FORL if (po[l]) q[l] = x[j].v[l];
-                }
-                fence_proxy_async();
-                __syncwarp();
-                if (lane == 0 && bulk_out > 0) {
-#pragma unroll
-                    for (int j = 0; j < kCcOutCols; ++j) {
-                        if (ids[j] < 0) continue;
-                        void* dst = reinterpret_cast<unsigned char*>(base) + (uint64_t)(uint32_t)ids[j] * cs;
-                        if (hint_out) bulk_s2g_hint(dst, smem_u32(my_out + j * out_bytes), (uint32_t)bulk_out, pol_first);
-                        else bulk_s2g(dst, smem_u32(my_out + j * out_bytes), (uint32_t)bulk_out);
-                    }
-                    bulk_commit();
-                }
-                if (bulk_out < nlev * (int)sizeof(T)) {    // the last < 16 bytes of a column go out directly
-#pragma unroll
-                    for (int j = 0; j < kCcOutCols; ++j) {
-                        if (ids[j] < 0) continue;
-                        T* dst = reinterpret_cast<T*>(reinterpret_cast<unsigned char*>(base) + (uint64_t)(uint32_t)ids[j] * cs);
-                        FORL if (po[l] && (L * lane + l) * (int)sizeof(T) >= bulk_out) dst[L * lane + l] = x[j].v[l];
-                    }
-                }
+                    using P2 = typename Pair<T>::type;
+                    P2 pr;
+                    pr.x = x.v[0]; pr.y = x.v[1];
+                    if (po[1]) __stcs(reinterpret_cast<P2*>(dst) + lane, pr);
+                    else if (po[0]) __stcs(dst + 2 * lane, x.v[0]);
+                    if (po[2]) __stcs(dst + 64 + lane, x.v[2]);
                 }
             };
 
@@ -505,16 +474,15 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
                 // ---- S1: div of the four cells from their edges (slot order of SCF_BLN) ------------
                 T gd[12];
                 ld_coef(cf + SCF_DIV, gd);
-                C dv[4];
-                FORL {
-                    dv[0].v[l] = gd[0] * vB[0].v[l] + gd[1] * vI[0].v[l] + gd[2] * vB[5].v[l];
-                    dv[1].v[l] = gd[3] * vB[1].v[l] + gd[4] * vB[2].v[l] + gd[5] * vI[1].v[l];
-                    dv[2].v[l] = gd[6] * vI[2].v[l] + gd[7] * vB[3].v[l] + gd[8] * vB[4].v[l];
-                    dv[3].v[l] = gd[9] * vI[1].v[l] + gd[10] * vI[2].v[l] + gd[11] * vI[0].v[l];
-                }
-                const int32_t c3[3] = {ido[6], ido[7], ido[8]}, c1[3] = {ido[9], -1, -1};
-                ST3(div, c3, dv);
-                ST3(div, c1, dv + 3);
+                C dv;
+                FORL dv.v[l] = gd[0] * vB[0].v[l] + gd[1] * vI[0].v[l] + gd[2] * vB[5].v[l];
+                ST(div, ido[6], dv);
+                FORL dv.v[l] = gd[3] * vB[1].v[l] + gd[4] * vB[2].v[l] + gd[5] * vI[1].v[l];
+                ST(div, ido[7], dv);
+                FORL dv.v[l] = gd[6] * vI[2].v[l] + gd[7] * vB[3].v[l] + gd[8] * vB[4].v[l];
+                ST(div, ido[8], dv);
+                FORL dv.v[l] = gd[9] * vI[1].v[l] + gd[10] * vI[2].v[l] + gd[11] * vI[0].v[l];
+                ST(div, ido[9], dv);
             }
             // ---- interior edges: vt, KE_e; start the cell sums -------------------------------
             T r12[12];
@@ -596,13 +564,18 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
             }
             if constexpr (FUSED) {
                 // ---- S2: zm, zc hold zeta / 2 at the three midpoints and the three corners ------------
-                C z2[3];
 #pragma unroll
-                for (int m = 0; m < 3; ++m) FORL z2[m].v[l] = (T)2 * zm[m].v[l];
-                ST3(vort, ido + 10, z2);
+                for (int m = 0; m < 3; ++m) {
+                    C z2;
+                    FORL z2.v[l] = (T)2 * zm[m].v[l];
+                    ST(vort, ido[10 + m], z2);
+                }
 #pragma unroll
-                for (int m = 0; m < 3; ++m) FORL z2[m].v[l] = (T)2 * zc[m].v[l];
-                ST3(vort, ido + 13, z2);
+                for (int m = 0; m < 3; ++m) {
+                    C z2;
+                    FORL z2.v[l] = (T)2 * zc[m].v[l];
+                    ST(vort, ido[13 + m], z2);
+                }
             }
             // ---- horizontal part H of the six owned edges (S5); frees the KE / vorticity columns ----
             T ec[24];
@@ -631,27 +604,22 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, int hints, const T* __restri
             if (lane == 0) mbar_arrive(done_bar(s % NB));
 
             // ---- vertical part and the tendency (S6, S7) -----------------------------------------
-            static_assert(kCcOutCols == 3, "six owned edges leave in two batches of three");
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                C o[3];
-#pragma unroll
-                for (int j = 0; j < 3; ++j) {
-                    const int x = 3 * h + j;
-                    const C Dv = VD(h == 0 ? vI[j] : vB[2 * j]);
-                    const C& wl = wf[j];
-                    const C& wh = h == 0 ? wf[3] : wx[j];
-                    const T* e4 = ec + 4 * x;
-                    FORL o[j].v[l] = -H[x].v[l] - (e4[2] * wl.v[l] + e4[3] * wh.v[l]) * Dv.v[l];
-                }
-                ST3(ddt_vn, ido + 3 * h, o);
+            for (int x = 0; x < 6; ++x) {
+                const int j = x % 3;
+                const C Dv = VD(x < 3 ? vI[j] : vB[2 * j]);
+                const C& wl = wf[j];
+                const C& wh = x < 3 ? wf[3] : wx[j];
+                const T* e4 = ec + 4 * x;
+                C o;
+                FORL o.v[l] = -H[x].v[l] - (e4[2] * wl.v[l] + e4[3] * wh.v[l]) * Dv.v[l];
+                ST(ddt_vn, ido[x], o);
             }
         } else {
             __syncwarp();
             if (lane == 0) mbar_arrive(done_bar(s % NB));
         }
     }
-    if (lane == 0) bulk_wait_all();
 }
 
 }  // namespace
@@ -660,52 +628,43 @@ template <class T>
 int cc_slot_bytes(int nlev) { return (((nlev + 1) * (int)sizeof(T) + 15) & ~15); }
 
 template <class T>
-static size_t cc_fixed_smem(const CcShape& sh, int nlev, bool direct) {
-    const int out_bytes = (nlev * (int)sizeof(T) + 15) & ~15;
-    return kCcBarrierBytes + (size_t)sh.depth * sh.group * cc_record_bytes<T>() +
-           (size_t)sh.warps * (direct ? 1 : kCcOutCols) * out_bytes;
+static size_t cc_fixed_smem() {
+    return kCcBarrierBytes + (size_t)kCcDepth * kCcGroup * cc_record_bytes<T>();
 }
 
 template <class T>
-int cc_max_slots(int shape, int nlev, int slot_bytes, int smem_optin, bool direct) {
-    const long avail = (long)smem_optin - (long)cc_fixed_smem<T>(cc_shape(shape), nlev, direct) - kCcSlotTailPad;
+int cc_max_slots(int slot_bytes, int smem_optin) {
+    const long avail = (long)smem_optin - (long)cc_fixed_smem<T>() - kCcSlotTailPad;
     if (avail <= 0) return 0;
     return (int)(avail / slot_bytes);
 }
-template int cc_max_slots<double>(int, int, int, int, bool);
-template int cc_max_slots<float>(int, int, int, int, bool);
+template int cc_max_slots<double>(int, int);
+template int cc_max_slots<float>(int, int);
 template int cc_slot_bytes<double>(int);
 template int cc_slot_bytes<float>(int);
 
 int cc_levels_per_lane(int nlev) { return nlev + 1 <= 32 ? 1 : nlev + 1 <= 96 ? 3 : 0; }
 
 namespace {
-template <class T, int L, int W, int G, int D, bool FUSED, bool DIRECT>
-cudaError_t cc_launch_one(const CcDev<T>& d, int n_ctas, size_t smem, int nlev, int ldk, int ldk_w, int hints, const T* abc,
-                          const T* vn, const T* w, T* ddt_vn, T* div, T* vort, unsigned long long* pc, unsigned long long pb, int pm, int pl,
-                          cudaStream_t s) {
-    auto k = k_tend_cc<T, L, W, G, D, FUSED, DIRECT>;
-    static size_t configured = 0;       // largest dynamic shared-memory size this instantiation was opted in for
-    if (smem > configured) {
-        cudaError_t err = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (err != cudaSuccess) return err;
-        configured = smem;
+template <class T, int L, bool FUSED>
+cudaError_t cc_launch_one(const CcDev<T>& d, int device, int n_ctas, size_t smem, int nlev, int ldk, int ldk_w, const T* abc,
+                          const T* vn, const T* w, T* ddt_vn, T* div, T* vort, unsigned long long* pc, unsigned long long ppl,
+                          int pm, int pl, cudaStream_t s) {
+    auto k = k_tend_cc<T, L, FUSED>;
+    // the opt-in for > 48 KB of dynamic shared memory is a per-DEVICE attribute of the function: remembered per device
+    static std::mutex mu;
+    static size_t configured[64] = {0};       // largest size this instantiation was opted in for, per device ordinal
+    {
+        std::lock_guard<std::mutex> lock(mu);
+        const bool known = device >= 0 && device < 64;
+        if (!known || smem > configured[device]) {
+            cudaError_t err = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (err != cudaSuccess) return err;
+            if (known) configured[device] = smem;
+        }
     }
-    k<<<(unsigned)n_ctas, (W + CcWarps<T, L>::producers) * 32, smem, s>>>(d, nlev, ldk, ldk_w, hints, abc, vn, w, ddt_vn, div, vort, pc, pb, pm, pl);
+    k<<<(unsigned)n_ctas, (kCcWarps + CcWarps<T, L>::producers) * 32, smem, s>>>(d, nlev, ldk, ldk_w, abc, vn, w, ddt_vn, div, vort, pc, ppl, pm, pl);
     return cudaGetLastError();
-}
-template <class T, int W, int G, int D>
-cudaError_t cc_launch_shape(int L, const CcDev<T>& d, int n_ctas, size_t smem, int nlev, int ldk, int ldk_w, int hints,
-                            const T* abc, const T* vn, const T* w, T* ddt_vn, T* div, T* vort, unsigned long long* pc,
-                            unsigned long long pb, int pm, int pl, cudaStream_t s) {
-    const bool fused = div != nullptr, direct = (hints & 16) != 0;
-#define CC_ONE(LL, FF, DD) \
-    if (L == LL && fused == FF && direct == DD) \
-        return cc_launch_one<T, LL, W, G, D, FF, DD>(d, n_ctas, smem, nlev, ldk, ldk_w, hints, abc, vn, w, ddt_vn, div, vort, pc, pb, pm, pl, s);
-    CC_ONE(1, false, false) CC_ONE(1, false, true) CC_ONE(1, true, false) CC_ONE(1, true, true)
-    CC_ONE(3, false, false) CC_ONE(3, false, true) CC_ONE(3, true, false) CC_ONE(3, true, true)
-#undef CC_ONE
-    return cudaErrorInvalidValue;
 }
 }  // namespace
 
@@ -718,32 +677,21 @@ int launch_tendencies_cc(const icon_grid& g, DevCcTables<T>& p, int nlev, int64_
     d.n_slots = p.n_slots; d.slot_bytes = p.slot_bytes;
     // pacing: a barrier of the producers every `period` steps (power of two), counted in p.progress (never reset)
     const int period = g.options[ICON_OPT_CC_PACE];
-    const bool heavy = sizeof(T) == 8 && cc_levels_per_lane(nlev) == 3;
-    const int pace_mask = period > 0 && p.progress && div != nullptr && heavy ? period - 1 : 0;      // fused fp64 step only
-    int64_t min_steps = 1 << 30;
-    for (int64_t n : p.cta_steps) min_steps = n < min_steps ? n : min_steps;
-    const int n_barriers = pace_mask ? (int)((min_steps - 1) / period) : 0;      // barriers every CTA reaches
-    const int pace_last = n_barriers * period;
-    const unsigned long long pace_base = (unsigned long long)p.pace_events;
-    const bool direct = p.direct;        // the slot count was derived for this store path
-    const size_t smem = cc_fixed_smem<T>(cc_shape(p.shape), nlev, direct) + (size_t)p.n_slots * p.slot_bytes + kCcSlotTailPad;
     const int L = cc_levels_per_lane(nlev);
-    cudaError_t err;
-#define CC_CASE(i, W, G, D)                                                                                        \
-    case i:                                                                                                        \
-        static_assert(kCcShapes[i].warps == W && kCcShapes[i].group == G && kCcShapes[i].depth == D, "shape table"); \
-        err = cc_launch_shape<T, W, G, D>(L, d, p.n_ctas, smem, nlev, (int)ldk, (int)ldk_w, (g.options[ICON_OPT_CC_L2_HINTS] & ~16) | (direct ? 16 : 0), abc, vn, w, ddt_vn, div, vort, p.progress, pace_base, pace_mask, pace_last, s); \
-        break;
-    switch (p.shape) {
-        CC_CASE(0, 8, 2, 6)
-        CC_CASE(1, 8, CC_S1_G, CC_S1_D)
-        default: err = cudaErrorInvalidValue;
-    }
-#undef CC_CASE
-    if (err == cudaSuccess && pace_mask) {
-        // every CTA adds one event per barrier it reaches: barriers k = 1 .. (its steps - 1) / period
-        p.pace_events += (int64_t)n_barriers * p.n_ctas;
-    }
+    const bool heavy = sizeof(T) == 8 && L == 3;
+    int pace_mask = period > 0 && p.progress && div != nullptr && heavy ? period - 1 : 0;      // fused fp64 step only
+    const int n_barriers = pace_mask ? (int)((p.min_steps - 1) / period) : 0;      // barriers every CTA reaches
+    if (n_barriers == 0) pace_mask = 0;
+    const int pace_last = n_barriers * period;
+    const unsigned long long per_launch = (unsigned long long)n_barriers * (unsigned long long)p.n_ctas;
+    const size_t smem = cc_fixed_smem<T>() + (size_t)p.n_slots * p.slot_bytes + kCcSlotTailPad;
+    const bool fused = div != nullptr;
+    cudaError_t err = cudaErrorInvalidValue;
+#define CC_ONE(LL, FF) \
+    if (L == LL && fused == FF) \
+        err = cc_launch_one<T, LL, FF>(d, g.device, p.n_ctas, smem, nlev, (int)ldk, (int)ldk_w, abc, vn, w, ddt_vn, div, vort, p.progress, per_launch, pace_mask, pace_last, s);
+    CC_ONE(1, false) CC_ONE(1, true) CC_ONE(3, false) CC_ONE(3, true)
+#undef CC_ONE
     return err == cudaSuccess ? 1 : -(int)err;
 }
 

@@ -33,8 +33,8 @@ def lib():
 _libgrids = {}
 
 
-# ICON_OPT_TENDENCY_KERNEL values; 40, 41 = kernel 4 (column cache) with ICON_OPT_CC_SHAPE 0, 1
-VARIANTS = [0, 1, 2, 3, 40, 41]
+# ICON_OPT_TENDENCY_KERNEL values (4 = column cache, the default wherever it holds the columns)
+VARIANTS = [0, 1, 2, 3, 4]
 
 
 def lib_grid(lib, k, seed=0, flags=0):
@@ -58,9 +58,6 @@ def run_gpu(torch, lib, g, vn, w, zh, nlev, variant, want_opt=False, sentinel=No
         return t
     ddt, div, vort = out(g.ne), out(g.nc), out(g.nv)
     opt = dict(vt=out(g.ne), ke_c=out(g.nc), vort=out(g.nv)) if want_opt else {}
-    if variant >= 40:         # 4x = column-cache kernel with pipeline shape x
-        g.set_option(lib.ICON_OPT_CC_SHAPE, variant - 40)
-        variant = 4
     g.set_option(lib.ICON_OPT_TENDENCY_KERNEL, variant)
     n0 = g.launch_count
     lib.dycore_velocity_tendencies(g, zh, d_vn, d_w, ddt, nlev, **opt)
@@ -185,8 +182,7 @@ def test_fp32_variant_permuted_r2b4(torch_cuda, lib, oracle_grid, variant):
     check_all(res, ref, 90, TOL["f32"])
 
 
-@pytest.mark.parametrize("shape", [0, 1])
-def test_column_cache_never_reads_a_stale_slot(torch_cuda, lib, oracle_grid, shape):
+def test_column_cache_never_reads_a_stale_slot(torch_cuda, lib, oracle_grid):
     """Kernel 4 keeps columns in shared memory across steps. Repeating ONE input hides a read that comes too
     early (the slot still holds the same column from the previous launch), so two different inputs alternate
     and every launch is compared with the oracle. This is the test that caught bulk copies of an earlier step
@@ -202,7 +198,6 @@ def test_column_cache_never_reads_a_stale_slot(torch_cuda, lib, oracle_grid, sha
         vn, w = np.nan_to_num(vn) * fv, np.nan_to_num(w) * fw
         ref = og.velocity_tendencies(vn, w, zh, nlev, with_scale=True)
         sets.append((torch.from_numpy(vn).to(dev), torch.from_numpy(w).to(dev), zh, ref))
-    g.set_option(lib.ICON_OPT_CC_SHAPE, shape)
     g.set_option(lib.ICON_OPT_TENDENCY_KERNEL, 4)
     for it in range(300):
         d_vn, d_w, zh, ref = sets[it % 2]
@@ -213,7 +208,7 @@ def test_column_cache_never_reads_a_stale_slot(torch_cuda, lib, oracle_grid, sha
         assert (err <= TOL["f64"] * ref["m_ddt"]).all(), "launch %d" % it
 
 
-@pytest.mark.parametrize("variant", [5, 40, 41, 3])
+@pytest.mark.parametrize("variant", [5, 4, 3])
 @pytest.mark.parametrize("k,seed,flags,nlev,ldk,ldk_w,cfg", [(4, 0, 0, 90, 96, 96, 1), (4, 0, 0, 90, 90, 92, 1), (2, 0, 0, 33, 34, 34, 1),
                                                          (1, 0, 0, 30, 30, 32, 1), (0, 0, 0, 3, 4, 4, 1),
                                                          (3, si.PERMUTE_SEED, 1, 40, 40, 42, 4)])
@@ -230,9 +225,6 @@ def test_dycore_step_matches_the_two_calls_and_the_oracle(torch_cuda, lib, oracl
     d_vn, d_w = torch.from_numpy(vn).to(dev), torch.from_numpy(w).to(dev)
     sentinel = -4321.25
     outs = [torch.full((n, ldk), sentinel, dtype=torch.float64, device=dev) for n in (g.ne, g.nc, g.nv)]
-    if variant >= 40:
-        g.set_option(lib.ICON_OPT_CC_SHAPE, variant - 40)
-        variant = 4
     g.set_option(lib.ICON_OPT_TENDENCY_KERNEL, variant)
     n0 = g.launch_count
     lib.dycore_step(g, zh, d_vn, d_w, outs[0], outs[1], outs[2], nlev)
@@ -246,7 +238,6 @@ def test_dycore_step_matches_the_two_calls_and_the_oracle(torch_cuda, lib, oracl
         assert (res[name][:, nlev:] == sentinel).all(), name
         assert not (res[name][:, :nlev] == sentinel).any(), name
     g.set_option(lib.ICON_OPT_TENDENCY_KERNEL, 5)
-    g.set_option(lib.ICON_OPT_CC_SHAPE, -1)
 
 
 @pytest.mark.parametrize("period", [0, 4, 16, 512])
@@ -267,7 +258,6 @@ def test_fused_step_pacing_barrier_periods(torch_cuda, lib, oracle_grid, period)
         ref = oracle_reference(og, vn, w, zh, nlev, False)
         sets.append((torch.from_numpy(vn).to(dev), torch.from_numpy(w).to(dev), zh, ref))
     g.set_option(lib.ICON_OPT_TENDENCY_KERNEL, 5)
-    g.set_option(lib.ICON_OPT_CC_SHAPE, -1)
     g.set_option(lib.ICON_OPT_CC_PACE, period)
     try:
         for it in range(6):
@@ -283,32 +273,38 @@ def test_fused_step_pacing_barrier_periods(torch_cuda, lib, oracle_grid, period)
         g.set_option(lib.ICON_OPT_CC_PACE, 512)
 
 
-@pytest.mark.parametrize("hints", [0, 3, 16, 19, 31])
-@pytest.mark.parametrize("dtype,nlev,ldk,ldk_w", [("f64", 90, 90, 92), ("f64", 33, 34, 34), ("f32", 90, 92, 92), ("f64", 3, 4, 4)])
-def test_column_cache_store_paths_and_hints(torch_cuda, lib, oracle_grid, hints, dtype, nlev, ldk, ldk_w):
-    """kernel 4: bulk stores (proxy fence, last < 16 bytes of a column stored directly) vs transposed coalesced stores,
-    with and without L2 eviction hints; tendency-only and fused step"""
+@pytest.mark.parametrize("tile", [16, 64, 0])
+@pytest.mark.parametrize("dtype,nlev,ldk,ldk_w", [("f64", 90, 96, 96), ("f64", 90, 90, 92), ("f64", 33, 34, 34), ("f32", 90, 96, 96),
+                                                   ("f32", 90, 92, 92), ("f64", 30, 32, 32), ("f64", 3, 4, 4), ("f64", 64, 64, 66),
+                                                   ("f64", 95, 96, 96)])
+def test_column_cache_level_mappings_and_tiles(torch_cuda, lib, oracle_grid, tile, dtype, nlev, ldk, ldk_w):
+    """kernel 4 with the default tiles, larger tiles and contiguous ranges; every level
+    mapping (one level per lane; pair + single with the single segment empty, partly and completely filled, odd and even
+    level counts so that the last pair is half valid); tendency-only and fused step"""
     torch = torch_cuda
-    og = oracle_grid(3)
-    g = lib_grid(lib, 3)
+    og = oracle_grid(4)
+    g = lib_grid(lib, 4)
     vn, w, zh = si.make_fields(1 if dtype == "f64" else 4, og.edge_xyz, og.edge_normal, og.nc, nlev=nlev, ldk=ldk, ldk_w=ldk_w,
                                dtype=dtype)
     ref = oracle_reference(og, vn, w, zh, nlev, dtype == "f32")
-    g.set_option(lib.ICON_OPT_CC_L2_HINTS, hints)
+    g.set_option(lib.ICON_OPT_CC_TILE, tile)
     try:
-        res = run_gpu(torch, lib, g, vn, w, zh, nlev, 40, sentinel=-77.5)
+        res = run_gpu(torch, lib, g, vn, w, zh, nlev, 4, sentinel=-77.5)
         check_all(res, ref, nlev, TOL[dtype])
         assert (res["ddt_vn"][:, nlev:] == -77.5).all()
         dev = torch.device("cuda:0")
         outs = [torch.full((n, ldk), -77.5, dtype=torch.from_numpy(vn).dtype, device=dev) for n in (g.ne, g.nc, g.nv)]
+        n0 = g.launch_count
         lib.dycore_step(g, zh, torch.from_numpy(vn).to(dev), torch.from_numpy(w).to(dev), outs[0], outs[1], outs[2], nlev)
         torch.cuda.synchronize()
+        assert g.launch_count - n0 == 1
         res = dict(ddt_vn=outs[0].cpu().numpy(), div=outs[1].cpu().numpy(), vort=outs[2].cpu().numpy())
         check_all(res, ref, nlev, TOL[dtype])
         for name in res:
             assert (res[name][:, nlev:] == -77.5).all(), name
+            assert not (res[name][:, :nlev] == -77.5).any(), name
     finally:
-        g.set_option(lib.ICON_OPT_CC_L2_HINTS, 19)
+        g.set_option(lib.ICON_OPT_CC_TILE, 16)
         g.set_option(lib.ICON_OPT_TENDENCY_KERNEL, 5)
 
 
@@ -350,14 +346,37 @@ def test_step_host_end_to_end(torch_cuda, lib, oracle_grid):
 
 
 # ----------------------------------------------------------------------------------------------
-# full-size configs (BASELINE.json configs[1..4]) in the launch configuration bench.py times:
-# sampled outputs the oracle computes one by one
+# full-size configs (BASELINE.json configs[1..4]): sampled outputs the oracle computes one by one.
+# Leg A is the call and the launch configuration bench.py times: dycore_step (one fused kernel) with bench.py's
+# column padding (whole 128-byte lines: ldk = ldk_w = 96 for 90 fp64 or fp32 levels, 32 for 30 fp64 levels), default
+# options (the pacing barrier armed at its default period), two alternating inputs. Leg B is the two separate
+# entry points of SURVEY.md 8(b) with unpadded columns.
 # ----------------------------------------------------------------------------------------------
 def _need_host_gb(gb):
     import psutil
     avail = psutil.virtual_memory().available / 2 ** 30
     if avail < gb:
         pytest.skip("needs %.0f GB of host memory, %.0f GB available" % (gb, avail))
+
+
+def bench_padding(nlev, f32):
+    """the leading dimensions bench.py uses (columns padded to whole 128-byte lines)"""
+    line = 32 if f32 else 16
+    return (nlev + line - 1) // line * line, (nlev + 1 + line - 1) // line * line
+
+
+def _sampled_check(torch, o, tag, config, outs, sizes, nlev, vn64, w64, zh, tol, nsamp, seed):
+    dev = outs[0].device
+    for what, arr, n in zip(("ddt_vn", "div", "vort"), outs, sizes):
+        idx, lev = si.sample_points(seed, n, nlev, nsamp)
+        got = arr[torch.from_numpy(idx).to(dev), torch.from_numpy(lev.astype(np.int64)).to(dev)].cpu().numpy().astype(np.float64)
+        want, m = o.sample(what, idx, lev, vn64, nlev, w=w64, z_half=zh)
+        err = np.abs(got - want)
+        assert (err <= tol * m).all(), "%s %s config %d: worst err/M %.3e" % (tag, what, config, (err / m).max())
+        # properties that hold at any size: every level of every column was written, no pad was touched
+        assert not torch.isnan(arr[:, :nlev]).any(), (tag, what)
+        if arr.shape[1] > nlev:
+            assert torch.isnan(arr[:, nlev:]).all(), (tag, what)
 
 
 @pytest.mark.slow
@@ -370,38 +389,68 @@ def test_full_size_sampled(torch_cuda, lib, oracle_mod, config, host_gb):
     seed = si.PERMUTE_SEED if cfg["permute"] else 0
     nlev = cfg["nlev"]
     f32 = cfg["dtype"] == "f32"
-    ldk = 92 if f32 else nlev            # fp32: ldk*4 must be a multiple of 16
-    ldk_w = 92 if f32 else nlev + 1 + (nlev + 1) % 2
+    tol = TOL[cfg["dtype"]]
     g = lib.IconGrid(cfg["k"], seed, flags)
     og = oracle_mod.Grid(cfg["k"], seed, flags)
+    o = og.rounded_f32() if f32 else og
     for name in ("c2e", "e2c", "e2v", "e2e4", "v2e"):          # bit-exact tables at full size
         assert np.array_equal(g.table_host(name), og.table(name)), name
-    vn, w, zh = si.make_fields(config, og.edge_xyz, og.edge_normal, og.nc, ldk=ldk, ldk_w=ldk_w)
     dev = torch.device("cuda:0")
-    d_vn, d_w = torch.from_numpy(vn).to(dev), torch.from_numpy(w).to(dev)
-    ddt = torch.full((g.ne, ldk), float("nan"), dtype=d_vn.dtype, device=dev)
-    div = torch.full((g.nc, ldk), float("nan"), dtype=d_vn.dtype, device=dev)
-    vort = torch.full((g.nv, ldk), float("nan"), dtype=d_vn.dtype, device=dev)
-    lib.dycore_velocity_tendencies(g, zh, d_vn, d_w, ddt, nlev)   # default = the variant bench.py times
-    lib.dycore_div_vort(g, d_vn, div, vort, nlev)
-    torch.cuda.synchronize()
-    o = og.rounded_f32() if f32 else og
-    vn64 = np.nan_to_num(vn.astype(np.float64)) if f32 else np.nan_to_num(vn)
-    w64 = np.nan_to_num(w.astype(np.float64)) if f32 else np.nan_to_num(w)
-    tol = TOL[cfg["dtype"]]
+    sizes = (g.ne, g.nc, g.nv)
     nsamp = 20000
-    for what, arr, n in (("ddt_vn", ddt, g.ne), ("div", div, g.nc), ("vort", vort, g.nv)):
-        idx, lev = si.sample_points(300 + config, n, nlev, nsamp)
-        got = arr[torch.from_numpy(idx).to(dev), torch.from_numpy(lev.astype(np.int64)).to(dev)].cpu().numpy().astype(np.float64)
-        want, m = o.sample(what, idx, lev, vn64, nlev, w=w64, z_half=zh)
-        err = np.abs(got - want)
-        assert (err <= tol * m).all(), "%s config %d: worst err/M %.3e" % (what, config, (err / m).max())
-        # properties that hold at any size: every level of every column was written
-        assert not torch.isnan(arr[:, :nlev]).any(), what
-    # discrete Gauss on the GPU result: area-weighted divergence sums to ~0 per level
+
+    # ---- leg A: dycore_step as bench.py launches it -------------------------------------------------------
+    ldk, ldk_w = bench_padding(nlev, f32)
+    vn, w, zh = si.make_fields(config, og.edge_xyz, og.edge_normal, og.nc, ldk=ldk, ldk_w=ldk_w)      # NaN pads
+    d_vn, d_w = torch.from_numpy(vn).to(dev), torch.from_numpy(w).to(dev)
+    fv, fw = -3.0, 5.0                                            # the second input: a rescaled copy (kept on the device)
+    d_vn2, d_w2 = d_vn * fv, d_w * fw
+
+    def fresh():
+        return [torch.full((n, ldk), float("nan"), dtype=d_vn.dtype, device=dev) for n in sizes]
+
+    def as64(a):
+        return np.nan_to_num(a.astype(np.float64)) if f32 else np.nan_to_num(a)
+    vn64, w64 = as64(vn), as64(w)
+    first = None
+    for it in range(4):                                           # A B A B: a stale slot would carry the OTHER input
+        second = it % 2 == 1
+        outs = fresh()
+        n0 = g.launch_count
+        lib.dycore_step(g, zh, d_vn2 if second else d_vn, d_w2 if second else d_w, outs[0], outs[1], outs[2], nlev)
+        torch.cuda.synchronize()
+        assert g.launch_count - n0 == 1, "dycore_step must be ONE fused kernel at every BASELINE config"
+        if second:
+            # the rescaled fields in the precision the device holds them (fp32: rounded products)
+            v2 = as64(d_vn2.cpu().numpy()) if it == 1 else v2
+            w2 = as64(d_w2.cpu().numpy()) if it == 1 else w2
+            _sampled_check(torch, o, "step B%d" % it, config, outs, sizes, nlev, v2, w2, zh, tol, nsamp, 400 + config)
+        else:
+            _sampled_check(torch, o, "step A%d" % it, config, outs, sizes, nlev, vn64, w64, zh, tol, nsamp, 300 + config)
+            if first is None:
+                first = [t.clone() for t in outs]
+            else:                                                 # the kernel is deterministic: bit-identical re-run
+                for a, b in zip(first, outs):
+                    assert torch.equal(torch.nan_to_num(a), torch.nan_to_num(b))
+    if second:
+        del v2, w2
+    # discrete Gauss on the GPU result (launch A): area-weighted divergence sums to ~0 per level
     a_c = torch.from_numpy(og.a_c).to(dev).to(torch.float64)
     l_e = torch.from_numpy(og.l_e).to(dev).to(torch.float64)
-    num = (a_c[:, None] * div[:, :nlev].to(torch.float64)).sum(0).abs()
+    num = (a_c[:, None] * first[1][:, :nlev].to(torch.float64)).sum(0).abs()
     den = (l_e[:, None] * d_vn[:, :nlev].to(torch.float64).abs()).sum(0)
     assert (num / den).max().item() < (1e-6 if f32 else 1e-13)
+    del first, outs, d_vn, d_w, d_vn2, d_w2, vn, w, vn64, w64
+    torch.cuda.empty_cache()
+
+    # ---- leg B: the two entry points of SURVEY.md 8(b), unpadded columns ----------------------------------
+    ldk = 92 if f32 else nlev            # fp32: ldk*4 must be a multiple of 16
+    ldk_w = 92 if f32 else nlev + 1 + (nlev + 1) % 2
+    vn, w, zh = si.make_fields(config, og.edge_xyz, og.edge_normal, og.nc, ldk=ldk, ldk_w=ldk_w)
+    d_vn, d_w = torch.from_numpy(vn).to(dev), torch.from_numpy(w).to(dev)
+    outs = fresh()
+    lib.dycore_velocity_tendencies(g, zh, d_vn, d_w, outs[0], nlev)
+    lib.dycore_div_vort(g, d_vn, outs[1], outs[2], nlev)
+    torch.cuda.synchronize()
+    _sampled_check(torch, o, "two calls", config, outs, sizes, nlev, as64(vn), as64(w), zh, tol, nsamp, 300 + config)
     g.close()
