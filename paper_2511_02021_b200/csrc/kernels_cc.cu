@@ -338,9 +338,15 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
                         }
                         __syncwarp();
                     }
-                    while (drained < s - (int)depth + 1) {
-                        mbar_wait(done_bar(drained % NB), (uint32_t)((drained / NB) & 1), 1, s);
-                        ++drained;
+                    // The producers run ahead of the consumers and spend most of their time right here, waiting for step
+                    // s - depth to drain. ONE warp polls the mbarrier, the others sleep in a hardware barrier: four
+                    // polling warps were 450 of the 2500 instructions the kernel issued per patch (profiles/r02_*),
+                    // pure heat in a kernel that runs into the board's power cap.
+                    if (drained < s - (int)depth + 1) {            // the same decision in every producer warp
+                        if (pw == 0)
+                            for (int t = drained; t < s - (int)depth + 1; ++t) mbar_wait(done_bar(t % NB), (uint32_t)((t / NB) & 1), 1, s);
+                        drained = s - (int)depth + 1;
+                        asm volatile("bar.sync 1, %0;" ::"n"(kCcProducers * 32) : "memory");
                     }
                     const uint32_t fb = full_bar(s % NB);
                     // Every producer warp announces the bytes of its own share before it issues them
@@ -394,6 +400,8 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
     // this lane's two read positions inside every slot
     const unsigned char* my_pair = slot_base + (L == 1 ? lane : 2 * lane) * (int)sizeof(T);
     const unsigned char* my_single = slot_base + (64 + lane) * (int)sizeof(T);
+    // and its two byte offsets inside every output column
+    const uint32_t st_pair = (uint32_t)((L == 1 ? lane : 2 * lane) * (int)sizeof(T)), st_single = (uint32_t)((64 + lane) * (int)sizeof(T));
 
     for (int s = grp; s < n_steps; s += NGRP) {
         const int64_t p = pb + (int64_t)s * G + wi;
@@ -435,16 +443,17 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
             // not push halo columns out of the L2); id < 0 = not ours
             auto ST = [&](T* base, int32_t id, const C& x) {
                 if (id < 0) return;
-                T* dst = reinterpret_cast<T*>(reinterpret_cast<unsigned char*>(base) + (uint64_t)(uint32_t)id * cs);
+                // one 64-bit column base (warp-uniform) plus the lane's two 32-bit byte offsets
+                unsigned char* col = reinterpret_cast<unsigned char*>(base) + (uint64_t)(uint32_t)id * cs;
                 if constexpr (L == 1) {
-                    if (po[0]) __stcs(dst + lane, x.v[0]);
+                    if (po[0]) __stcs(reinterpret_cast<T*>(col + st_pair), x.v[0]);
                 } else {
                     using P2 = typename Pair<T>::type;
                     P2 pr;
                     pr.x = x.v[0]; pr.y = x.v[1];
-                    if (po[1]) __stcs(reinterpret_cast<P2*>(dst) + lane, pr);
-                    else if (po[0]) __stcs(dst + 2 * lane, x.v[0]);
-                    if (po[2]) __stcs(dst + 64 + lane, x.v[2]);
+                    if (po[1]) __stcs(reinterpret_cast<P2*>(col + st_pair), pr);
+                    else if (po[0]) __stcs(reinterpret_cast<T*>(col + st_pair), x.v[0]);
+                    if (po[2]) __stcs(reinterpret_cast<T*>(col + st_single), x.v[2]);
                 }
             };
 
@@ -593,12 +602,21 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
                 const T* e4 = ec + 4 * (3 + x);
                 FORL H[3 + x].v[l] = (keX[x].v[l] - ke[x].v[l]) * e4[0] + tBo[x].v[l] * (e4[1] + (zm[x].v[l] + zc[x].v[l]));
             }
-            // ---- cell-centre w (S6); these are the last reads of the slots -----------------------
-            C wf[4], wx[3];
+            // ---- cell-centre w at the six owned edges (S6): w_e = c_lin(L) w_f(L) + c_lin(H) w_f(H); these are the
+            // last reads of the slots
+            C we[6];
+            {
+                C wf[4];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) wf[j] = WS(sX[12 + j]);
+                for (int j = 0; j < 4; ++j) wf[j] = WS(sX[12 + j]);
 #pragma unroll
-            for (int x = 0; x < 3; ++x) wx[x] = WS(sX[16 + x]);
+                for (int x = 0; x < 3; ++x) FORL we[x].v[l] = ec[4 * x + 2] * wf[x].v[l] + ec[4 * x + 3] * wf[3].v[l];
+#pragma unroll
+                for (int x = 0; x < 3; ++x) {
+                    const C wx = WS(sX[16 + x]);
+                    FORL we[3 + x].v[l] = ec[4 * (3 + x) + 2] * wf[x].v[l] + ec[4 * (3 + x) + 3] * wx.v[l];
+                }
+            }
             // everything this patch needs from the slots and its record is in registers: release the stage
             __syncwarp();
             if (lane == 0) mbar_arrive(done_bar(s % NB));
@@ -606,13 +624,9 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
             // ---- vertical part and the tendency (S6, S7) -----------------------------------------
 #pragma unroll
             for (int x = 0; x < 6; ++x) {
-                const int j = x % 3;
-                const C Dv = VD(x < 3 ? vI[j] : vB[2 * j]);
-                const C& wl = wf[j];
-                const C& wh = x < 3 ? wf[3] : wx[j];
-                const T* e4 = ec + 4 * x;
+                const C Dv = VD(x < 3 ? vI[x] : vB[2 * (x - 3)]);
                 C o;
-                FORL o.v[l] = -H[x].v[l] - (e4[2] * wl.v[l] + e4[3] * wh.v[l]) * Dv.v[l];
+                FORL o.v[l] = -H[x].v[l] - we[x].v[l] * Dv.v[l];
                 ST(ddt_vn, ido[x], o);
             }
         } else {
