@@ -24,6 +24,14 @@
  *   - Compute calls enqueue kernels on the caller's CUDA stream and return without synchronising.
  *     Field buffers are caller-owned, never retained; outputs must not alias inputs.
  *   - There is NO CPU fallback: compute calls return ICON_ECUDA when no CUDA device is usable.
+ *   - Device, stream and thread contract. A grid handle belongs to the CUDA device that was current at
+ *     icon_grid_create; every later call on it must be made with that device current (ICON_EINVAL otherwise).
+ *     The handle is logically const for the compute calls but caches tables and schedules that are built on the
+ *     first call for a new (dtype, nlev, ldk, ldk_w, z_half): such a first call allocates device memory and
+ *     synchronises; steady-state calls do neither and can be captured into a CUDA graph (capture after one
+ *     plain call with the same arguments). Calls on ONE handle must not overlap: use one stream at a time and one
+ *     host thread at a time per handle (the fused kernel keeps a chip-wide pacing counter per handle, the
+ *     unfused pipeline a workspace). Different handles are independent.
  */
 #ifndef ICON_DYCORE_H
 #define ICON_DYCORE_H
@@ -123,7 +131,7 @@ int icon_grid_table_host(const icon_grid_t* g, int which, const void** ptr, int*
 /* Device copy of a public table in user order, uploaded on first request and then cached.
  * dtype: ICON_F64 or ICON_F32 selects the element type of floating-point tables (ignored for
  * integer tables). ICON_EUNSUPPORTED on a ICON_HOST_ONLY grid. */
-int icon_grid_table_device(icon_grid_t* g, int which, int dtype, const void** dptr);
+int icon_grid_table_device(const icon_grid_t* g, int which, int dtype, const void** dptr);
 
 int icon_grid_set_option(icon_grid_t* g, int option, int value);
 
@@ -138,7 +146,7 @@ int icon_grid_set_option(icon_grid_t* g, int option, int value);
  * (out[6] + out[7] == nv: every vertex is written exactly once by the div/vort kernel).
  * ICON_EUNSUPPORTED if the tables do not describe a 4-child bisection hierarchy.
  */
-int icon_grid_worklist_stats(icon_grid_t* g, int64_t out[8]);
+int icon_grid_worklist_stats(const icon_grid_t* g, int64_t out[8]);
 
 /*
  * icon_grid_cc_schedule_check -- builds on the host (works on ICON_HOST_ONLY grids) the column-cache
@@ -151,7 +159,7 @@ int icon_grid_worklist_stats(icon_grid_t* g, int64_t out[8]);
  * ICON_EUNSUPPORTED: nlev or the memory size cannot hold the kernel; ICON_EINVAL: the check failed
  * (icon_last_error names the rule).
  */
-int icon_grid_cc_schedule_check(icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, int n_ctas, int smem_bytes,
+int icon_grid_cc_schedule_check(const icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, int n_ctas, int smem_bytes,
                                 int64_t out[8]);
 
 /*
@@ -162,7 +170,7 @@ int icon_grid_cc_schedule_check(icon_grid_t* g, int dtype, int nlev, int ldk, in
  *   vort(v,k) = sum_{j<6} geofac_rot(v,j) * vn(v2e[v][j], k)      (pentagon pad coefficient is 0)
  * vn [ne][ldk] dev in; div [nc][ldk], vort [nv][ldk] dev out. 1 <= nlev <= ldk.
  */
-int dycore_div_vort(icon_grid_t* g, int dtype, int nlev, int ldk,
+int dycore_div_vort(const icon_grid_t* g, int dtype, int nlev, int ldk,
                     const void* vn, void* div, void* vort, void* cuda_stream);
 
 /*
@@ -181,7 +189,7 @@ int dycore_div_vort(icon_grid_t* g, int dtype, int nlev, int ldk,
  * vt_opt [ne][ldk], ke_c_opt [nc][ldk], vort_opt [nv][ldk]: dev out, NULL = do not store.
  * 2 <= nlev <= ldk, nlev+1 <= ldk_w, nlev <= 4096.
  */
-int dycore_velocity_tendencies(icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w,
+int dycore_velocity_tendencies(const icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w,
                                const double* z_half,
                                const void* vn, const void* w, void* ddt_vn,
                                void* vt_opt, void* ke_c_opt, void* vort_opt, void* cuda_stream);
@@ -195,17 +203,18 @@ int dycore_velocity_tendencies(icon_grid_t* g, int dtype, int nlev, int ldk, int
  * the grid is a midpoint or corner of some patch; the lowest patch index stores it). Elsewhere it is the two
  * calls back to back. Same argument rules as the two calls; outputs must not alias inputs or each other.
  */
-int dycore_step(icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
+int dycore_step(const icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
                 const void* vn, const void* w, void* ddt_vn, void* div, void* vort, void* cuda_stream);
 
 /*
- * dycore_step_host -- one velocity-tendency + div/vort step with HOST field buffers (the
- * end-to-end path of bench.py): copies vn and w to the device, runs dycore_velocity_tendencies and
- * dycore_div_vort, copies ddt_vn, div and vort back, and synchronises. Host buffers should be
- * pinned for full PCIe bandwidth. Device staging buffers are owned by the grid handle and
- * allocated on first use. Same shapes and constraints as the two device calls.
+ * dycore_step_host -- dycore_step with HOST field buffers (the end-to-end leg of bench.py): copies vn and w to
+ * device staging buffers, runs dycore_step (one fused kernel where the column-cache kernel runs), copies ddt_vn, div
+ * and vort back, and synchronises. This is NOT how the paper runs the model (fields stay resident on the GPU,
+ * PAPER.md:97); it exists so that the whole path can be timed with the PCIe copies included. Host buffers should be
+ * pinned for full PCIe bandwidth. The staging buffers and the private stream are owned by the grid handle and allocated
+ * on first use. Same shapes and constraints as dycore_step.
  */
-int dycore_step_host(icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
+int dycore_step_host(const icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
                      const void* vn_host, const void* w_host,
                      void* ddt_vn_host, void* div_host, void* vort_host);
 

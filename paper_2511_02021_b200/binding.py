@@ -184,8 +184,31 @@ def _dtype_of(t):
     raise TypeError("fields must be float64 or float32 tensors")
 
 
+def _check_fields(fields, ldk_of=None):
+    """Cheap marshalling checks (no arithmetic): every field is a contiguous 2-D CUDA tensor of one dtype on one device
+    with the expected row count; fields that share a leading dimension have the same second dimension.
+    fields: (name, tensor or None, rows, group) with group naming the leading dimension the tensor must share."""
+    first, widths = None, {}
+    for name, t, rows, group in fields:
+        if t is None:
+            continue
+        if not hasattr(t, "is_cuda") or not t.is_cuda:
+            raise TypeError("%s must be a CUDA tensor (the library has no CPU path)" % name)
+        if t.dim() != 2 or not t.is_contiguous():
+            raise ValueError("%s must be a contiguous 2-D tensor [entities][levels]" % name)
+        if t.shape[0] != rows:
+            raise ValueError("%s has %d rows, the grid has %d" % (name, t.shape[0], rows))
+        if first is None:
+            first = t
+        elif t.dtype != first.dtype or t.device != first.device:
+            raise TypeError("%s: all fields must have one dtype and live on one device" % name)
+        if widths.setdefault(group, t.shape[1]) != t.shape[1]:
+            raise ValueError("%s: leading dimension %d differs from the other %s fields (%d)" % (name, t.shape[1], group, widths[group]))
+
+
 def dycore_div_vort(grid, vn, div, vort, nlev, stream=None):
     """S1+S2. vn [ne][ldk], div [nc][ldk], vort [nv][ldk]: CUDA tensors of one dtype."""
+    _check_fields((("vn", vn, grid.ne, "ldk"), ("div", div, grid.nc, "ldk"), ("vort", vort, grid.nv, "ldk")))
     _check(grid._L.dycore_div_vort(grid._h, _dtype_of(vn), int(nlev), int(vn.shape[1]), _dptr(vn), _dptr(div),
                                    _dptr(vort), _stream_ptr(stream)))
 
@@ -195,6 +218,8 @@ def dycore_velocity_tendencies(grid, z_half, vn, w, ddt_vn, nlev, vt=None, ke_c=
     z = np.ascontiguousarray(z_half, dtype=np.float64)
     if z.size != nlev + 1:
         raise ValueError("z_half must have nlev+1 entries")
+    _check_fields((("vn", vn, grid.ne, "ldk"), ("w", w, grid.nc, "ldk_w"), ("ddt_vn", ddt_vn, grid.ne, "ldk"),
+                   ("vt", vt, grid.ne, "ldk"), ("ke_c", ke_c, grid.nc, "ldk"), ("vort", vort, grid.nv, "ldk")))
     _check(grid._L.dycore_velocity_tendencies(grid._h, _dtype_of(vn), int(nlev), int(vn.shape[1]), int(w.shape[1]),
                                               _dptr(z), _dptr(vn), _dptr(w), _dptr(ddt_vn), _dptr(vt), _dptr(ke_c),
                                               _dptr(vort), _stream_ptr(stream)))
@@ -205,6 +230,8 @@ def dycore_step(grid, z_half, vn, w, ddt_vn, div, vort, nlev, stream=None):
     z = np.ascontiguousarray(z_half, dtype=np.float64)
     if z.size != nlev + 1:
         raise ValueError("z_half must have nlev+1 entries")
+    _check_fields((("vn", vn, grid.ne, "ldk"), ("w", w, grid.nc, "ldk_w"), ("ddt_vn", ddt_vn, grid.ne, "ldk"),
+                   ("div", div, grid.nc, "ldk"), ("vort", vort, grid.nv, "ldk")))
     _check(grid._L.dycore_step(grid._h, _dtype_of(vn), int(nlev), int(vn.shape[1]), int(w.shape[1]), _dptr(z), _dptr(vn),
                                _dptr(w), _dptr(ddt_vn), _dptr(div), _dptr(vort), _stream_ptr(stream)))
 

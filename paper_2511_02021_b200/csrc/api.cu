@@ -120,6 +120,7 @@ int ensure_coeffs(icon_grid* g, icon::DevCoeffs<T>& c) {
     if ((rc = upload_rows(g, h.inv_d_e, 1, ue, &c.inv_d_e))) return rc;
     if ((rc = upload_rows(g, h.f_e, 1, ue, &c.f_e))) return rc;
     if ((rc = upload_rows(g, h.c_lin, 2, ue, &c.c_lin))) return rc;
+    CU_TRY(cudaStreamSynchronize(cudaStreamLegacy));      // uploads ran on the legacy stream, callers may use non-blocking streams
     c.ready = true;
     return ICON_OK;
 }
@@ -172,6 +173,7 @@ int ensure_patch_tables(icon_grid* g, icon::DevPatchTables<T>& p) {
     if ((rc = upload_vec(g, h.mid_store, &p.mid_store))) return rc;
     if ((rc = upload_vec(g, h.mid_vertex, &p.mid_vertex))) return rc;
     p.n_patches = h.n_patches; p.n_tiles = h.n_tiles; p.max_halo = h.max_halo; p.max_vert = h.max_vert;
+    CU_TRY(cudaStreamSynchronize(cudaStreamLegacy));
     p.ready = true;
     return ICON_OK;
 }
@@ -186,6 +188,7 @@ int ensure_sc_tables(icon_grid* g, icon::DevScTables<T>& p) {
     if ((rc = upload_vec(g, g->sc_host.ids, &p.ids))) return rc;
     if ((rc = upload_vec(g, g->sc_host.coef, &p.coef))) return rc;
     p.n_patches = g->sc_host.n_patches;
+    CU_TRY(cudaStreamSynchronize(cudaStreamLegacy));
     p.ready = true;
     return ICON_OK;
 }
@@ -290,7 +293,9 @@ int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev, int64_t ld
     p.min_steps = 1 << 30;
     for (int b = 0; b < cs.n_ctas; ++b) p.min_steps = std::min(p.min_steps, cs.cta_step_begin[(size_t)b + 1] - cs.cta_step_begin[(size_t)b]);
     if ((rc = dev_alloc(g, 1, &p.progress))) return rc;
-    CU_TRY(cudaMemset(p.progress, 0, sizeof(unsigned long long)));      // synchronous: ordered before any later launch
+    CU_TRY(cudaMemset(p.progress, 0, sizeof(unsigned long long)));
+    // table uploads and the memset ran on the legacy stream; the caller's stream may be non-blocking
+    CU_TRY(cudaStreamSynchronize(cudaStreamLegacy));
     p.stats[0] = (int64_t)cs.steps.size(); p.stats[1] = cs.n_sync_steps; p.stats[2] = cs.n_vn_loads; p.stats[3] = cs.n_w_loads;
     p.stats[4] = cs.n_copies;
     p.ready = true;
@@ -329,7 +334,7 @@ void vertical_coefficients(const double* zh, int K, std::vector<double>& abc) {
     }
 }
 
-int get_level_coeffs(icon_grid* g, int dtype, int nlev, const double* z_half, cudaStream_t s, void** out) {
+int get_level_coeffs(icon_grid* g, int dtype, int nlev, const double* z_half, void** out) {
     for (int k = 0; k < nlev; ++k)
         if (!(z_half[k] > z_half[k + 1])) return fail(ICON_EINVAL, "z_half must be strictly decreasing");
     for (auto& lc : g->level_coeffs)
@@ -347,16 +352,18 @@ int get_level_coeffs(icon_grid* g, int dtype, int nlev, const double* z_half, cu
     if (dtype == ICON_F64) {
         double* d = nullptr;
         if ((rc = dev_alloc(g, abc.size(), &d))) return rc;
-        // pageable source: the runtime stages it before returning, so `abc` may die afterwards
-        CU_TRY(cudaMemcpyAsync(d, abc.data(), abc.size() * 8, cudaMemcpyHostToDevice, s));
+        CU_TRY(cudaMemcpy(d, abc.data(), abc.size() * 8, cudaMemcpyHostToDevice));
         lc.abc = d;
     } else {
         std::vector<float> f(abc.begin(), abc.end());
         float* d = nullptr;
         if ((rc = dev_alloc(g, f.size(), &d))) return rc;
-        CU_TRY(cudaMemcpyAsync(d, f.data(), f.size() * 4, cudaMemcpyHostToDevice, s));
+        CU_TRY(cudaMemcpy(d, f.data(), f.size() * 4, cudaMemcpyHostToDevice));
         lc.abc = d;
     }
+    // the coefficients are cached per z_half and reused by later calls on ANY stream: the upload (legacy stream) must
+    // have landed before this call's kernel, which may run on a non-blocking stream, reads them
+    CU_TRY(cudaStreamSynchronize(cudaStreamLegacy));
     if (g->level_coeffs.size() >= 16) {   // bounded cache
         dev_release(g, g->level_coeffs.front().abc);
         g->level_coeffs.erase(g->level_coeffs.begin());
@@ -372,9 +379,24 @@ int check_field(const void* p, const char* name) {
     return ICON_OK;
 }
 
+// true when the byte ranges [a, a + na) and [b, b + nb) intersect
+bool overlaps(const void* a, size_t na, const void* b, size_t nb) {
+    const uintptr_t pa = reinterpret_cast<uintptr_t>(a), pb = reinterpret_cast<uintptr_t>(b);
+    return a && b && pa < pb + nb && pb < pa + na;
+}
+
+int check_device(const icon_grid* g) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail_cuda(e, "cudaGetDevice");
+    if (dev != g->device) return fail(ICON_EINVAL, "the current CUDA device is not the device the grid was created on");
+    return ICON_OK;
+}
+
 int check_common(icon_grid* g, int dtype, int nlev, int ldk, int min_lev) {
     if (!g) return fail(ICON_EINVAL, "grid handle is NULL");
     if (g->host_only) return fail(ICON_ECUDA, "grid was created with ICON_HOST_ONLY: no device tables, and there is no CPU path");
+    if (int rc = check_device(g)) return rc;
     if (dtype != ICON_F64 && dtype != ICON_F32) return fail(ICON_EINVAL, "dtype must be ICON_F64 or ICON_F32");
     if (nlev < min_lev || nlev > 4096) return fail(ICON_EINVAL, "nlev out of range");
     if (ldk < nlev) return fail(ICON_EINVAL, "ldk < nlev");
@@ -410,7 +432,7 @@ int tendencies_impl(icon_grid* g, icon::DevCoeffs<T>& c, icon::DevPatchTables<T>
     int rc;
     if ((rc = ensure_coeffs(g, c))) return rc;
     void* abc = nullptr;
-    if ((rc = get_level_coeffs(g, dtype, nlev, z_half, s, &abc))) return rc;
+    if ((rc = get_level_coeffs(g, dtype, nlev, z_half, &abc))) return rc;
     const bool want_opt = vt_opt || ke_c_opt || vort_opt;
     int n;
     int variant = g->options[ICON_OPT_TENDENCY_KERNEL];
@@ -583,9 +605,11 @@ int icon_grid_table_host(const icon_grid_t* g, int which, const void** ptr, int*
     return ICON_OK;
 }
 
-int icon_grid_table_device(icon_grid_t* g, int which, int dtype, const void** dptr) {
+int icon_grid_table_device(const icon_grid_t* gc, int which, int dtype, const void** dptr) {
+    icon_grid* g = const_cast<icon_grid*>(gc);       // logically const: the device copies are a cache
     if (!g || !dptr) return fail(ICON_EINVAL, "NULL argument");
     if (g->host_only) return fail(ICON_EUNSUPPORTED, "grid was created with ICON_HOST_ONLY");
+    if (int rcd = check_device(g)) return rcd;
     if (dtype != ICON_F64 && dtype != ICON_F32) return fail(ICON_EINVAL, "dtype must be ICON_F64 or ICON_F32");
     TableInfo t;
     int rc = table_info(g, which, &t);
@@ -630,7 +654,8 @@ int icon_grid_set_option(icon_grid_t* g, int option, int value) {
 
 int64_t icon_grid_launch_count(const icon_grid_t* g) { return g ? g->launches : 0; }
 
-int icon_grid_worklist_stats(icon_grid_t* g, int64_t out[8]) {
+int icon_grid_worklist_stats(const icon_grid_t* gc, int64_t out[8]) {
+    icon_grid* g = const_cast<icon_grid*>(gc);
     if (!g || !out) return fail(ICON_EINVAL, "NULL argument");
     int rc = ensure_patch_host(g);
     if (rc) return rc;
@@ -649,8 +674,9 @@ int icon_grid_worklist_stats(icon_grid_t* g, int64_t out[8]) {
     return ICON_OK;
 }
 
-int icon_grid_cc_schedule_check(icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, int n_ctas, int smem_bytes,
+int icon_grid_cc_schedule_check(const icon_grid_t* gc, int dtype, int nlev, int ldk, int ldk_w, int n_ctas, int smem_bytes,
                                 int64_t out[8]) {
+    icon_grid* g = const_cast<icon_grid*>(gc);
     if (!g || !out) return fail(ICON_EINVAL, "NULL argument");
     if (dtype != ICON_F64 && dtype != ICON_F32) return fail(ICON_EINVAL, "dtype must be ICON_F64 or ICON_F32");
     if (nlev < 2 || ldk < nlev || ldk_w < nlev + 1 || n_ctas < 1 || smem_bytes < 1) return fail(ICON_EINVAL, "bad argument");
@@ -674,11 +700,18 @@ int icon_grid_cc_schedule_check(icon_grid_t* g, int dtype, int nlev, int ldk, in
     return ICON_OK;
 }
 
-int dycore_div_vort(icon_grid_t* g, int dtype, int nlev, int ldk, const void* vn, void* div, void* vort,
+int dycore_div_vort(const icon_grid_t* gc, int dtype, int nlev, int ldk, const void* vn, void* div, void* vort,
                     void* cuda_stream) {
+    icon_grid* g = const_cast<icon_grid*>(gc);       // logically const: lazily built tables are a cache
     int rc = check_common(g, dtype, nlev, ldk, 1);
     if (rc) return rc;
     if ((rc = check_field(vn, "vn")) || (rc = check_field(div, "div")) || (rc = check_field(vort, "vort"))) return rc;
+    {
+        const size_t es = dtype == ICON_F64 ? 8 : 4;
+        const size_t be = (size_t)g->host.ne * ldk * es, bc = (size_t)g->host.nc * ldk * es, bv = (size_t)g->host.nv * ldk * es;
+        if (overlaps(div, bc, vn, be) || overlaps(vort, bv, vn, be) || overlaps(div, bc, vort, bv))
+            return fail(ICON_EINVAL, "outputs must not alias the input or each other");
+    }
     cudaStream_t s = (cudaStream_t)cuda_stream;
     int n;
     if (dtype == ICON_F64) {
@@ -693,9 +726,10 @@ int dycore_div_vort(icon_grid_t* g, int dtype, int nlev, int ldk, const void* vn
     return ICON_OK;
 }
 
-int dycore_velocity_tendencies(icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
+int dycore_velocity_tendencies(const icon_grid_t* gc, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
                                const void* vn, const void* w, void* ddt_vn, void* vt_opt, void* ke_c_opt,
                                void* vort_opt, void* cuda_stream) {
+    icon_grid* g = const_cast<icon_grid*>(gc);
     int rc = check_common(g, dtype, nlev, ldk, 2);
     if (rc) return rc;
     if (ldk_w < nlev + 1) return fail(ICON_EINVAL, "ldk_w < nlev+1");
@@ -705,15 +739,27 @@ int dycore_velocity_tendencies(icon_grid_t* g, int dtype, int nlev, int ldk, int
     if (vt_opt && (rc = check_field(vt_opt, "vt_opt"))) return rc;
     if (ke_c_opt && (rc = check_field(ke_c_opt, "ke_c_opt"))) return rc;
     if (vort_opt && (rc = check_field(vort_opt, "vort_opt"))) return rc;
-    if (ddt_vn == vn || ddt_vn == w) return fail(ICON_EINVAL, "outputs must not alias inputs");
+    {
+        const size_t es = dtype == ICON_F64 ? 8 : 4;
+        const size_t be = (size_t)g->host.ne * ldk * es, bc = (size_t)g->host.nc * ldk * es, bv = (size_t)g->host.nv * ldk * es,
+                     bw = (size_t)g->host.nc * ldk_w * es;
+        const void* outs[4] = {ddt_vn, vt_opt, ke_c_opt, vort_opt};
+        const size_t ob[4] = {be, be, bc, bv};
+        for (int i = 0; i < 4; ++i) {
+            if (overlaps(outs[i], ob[i], vn, be) || overlaps(outs[i], ob[i], w, bw)) return fail(ICON_EINVAL, "outputs must not alias inputs");
+            for (int j = 0; j < i; ++j)
+                if (overlaps(outs[i], ob[i], outs[j], ob[j])) return fail(ICON_EINVAL, "outputs must not alias each other");
+        }
+    }
     cudaStream_t s = (cudaStream_t)cuda_stream;
     if (dtype == ICON_F64)
         return tendencies_impl<double>(g, g->c64, g->p64, g->s64, g->cc64, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, vt_opt, ke_c_opt, vort_opt, s);
     return tendencies_impl<float>(g, g->c32, g->p32, g->s32, g->cc32, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, vt_opt, ke_c_opt, vort_opt, s);
 }
 
-int dycore_step(icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, const double* z_half, const void* vn, const void* w,
+int dycore_step(const icon_grid_t* gc, int dtype, int nlev, int ldk, int ldk_w, const double* z_half, const void* vn, const void* w,
                 void* ddt_vn, void* div, void* vort, void* cuda_stream) {
+    icon_grid* g = const_cast<icon_grid*>(gc);
     int rc = check_common(g, dtype, nlev, ldk, 2);
     if (rc) return rc;
     if (ldk_w < nlev + 1) return fail(ICON_EINVAL, "ldk_w < nlev + 1");
@@ -723,8 +769,18 @@ int dycore_step(icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, const d
     if ((rc = check_field(vn, "vn")) || (rc = check_field(w, "w")) || (rc = check_field(ddt_vn, "ddt_vn")) ||
         (rc = check_field(div, "div")) || (rc = check_field(vort, "vort")))
         return rc;
-    if (ddt_vn == vn || ddt_vn == w || div == vn || div == w || vort == vn || vort == w || div == ddt_vn || vort == ddt_vn || div == vort)
-        return fail(ICON_EINVAL, "outputs must not alias inputs or each other");
+    {
+        const size_t be = (size_t)g->host.ne * ldk * es, bc = (size_t)g->host.nc * ldk * es, bv = (size_t)g->host.nv * ldk * es,
+                     bw = (size_t)g->host.nc * ldk_w * es;
+        const void* outs[3] = {ddt_vn, div, vort};
+        const size_t ob[3] = {be, bc, bv};
+        for (int i = 0; i < 3; ++i) {
+            if (overlaps(outs[i], ob[i], vn, be) || overlaps(outs[i], ob[i], w, bw))
+                return fail(ICON_EINVAL, "outputs must not alias inputs or each other");
+            for (int j = 0; j < i; ++j)
+                if (overlaps(outs[i], ob[i], outs[j], ob[j])) return fail(ICON_EINVAL, "outputs must not alias inputs or each other");
+        }
+    }
     cudaStream_t s = (cudaStream_t)cuda_stream;
     bool fused = false;
     if (dtype == ICON_F64)
@@ -737,8 +793,9 @@ int dycore_step(icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, const d
     return dycore_div_vort(g, dtype, nlev, ldk, vn, div, vort, cuda_stream);
 }
 
-int dycore_step_host(icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
+int dycore_step_host(const icon_grid_t* gc, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
                      const void* vn_host, const void* w_host, void* ddt_vn_host, void* div_host, void* vort_host) {
+    icon_grid* g = const_cast<icon_grid*>(gc);
     int rc = check_common(g, dtype, nlev, ldk, 2);
     if (rc) return rc;
     if (!vn_host || !w_host || !ddt_vn_host || !div_host || !vort_host) return fail(ICON_EINVAL, "NULL host buffer");

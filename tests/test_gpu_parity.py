@@ -323,6 +323,18 @@ def test_argument_errors_on_device(torch_cuda, lib):
     with pytest.raises(lib.IconError):                 # nlev > ldk
         lib.dycore_div_vort(g, vn, torch.zeros((g.nc, 6), dtype=torch.float64, device=dev),
                             torch.zeros((g.nv, 6), dtype=torch.float64, device=dev), 7)
+    with pytest.raises(lib.IconError):                 # outputs overlap each other (views of one buffer)
+        buf = torch.zeros((g.ne + g.nc, 6), dtype=torch.float64, device=dev)
+        lib.dycore_step(g, zh, vn, w, buf[:g.ne], buf[g.nc:g.nc + g.nc], torch.zeros((g.nv, 6), dtype=torch.float64, device=dev), 6)
+    with pytest.raises(ValueError):                    # wrong row count
+        lib.dycore_div_vort(g, vn, torch.zeros((g.nc + 1, 6), dtype=torch.float64, device=dev),
+                            torch.zeros((g.nv, 6), dtype=torch.float64, device=dev), 6)
+    with pytest.raises(ValueError):                    # non-contiguous view
+        lib.dycore_div_vort(g, torch.zeros((g.ne, 12), dtype=torch.float64, device=dev)[:, ::2],
+                            torch.zeros((g.nc, 6), dtype=torch.float64, device=dev), torch.zeros((g.nv, 6), dtype=torch.float64, device=dev), 6)
+    with pytest.raises(TypeError):                     # mixed dtypes
+        lib.dycore_div_vort(g, vn, torch.zeros((g.nc, 6), dtype=torch.float32, device=dev),
+                            torch.zeros((g.nv, 6), dtype=torch.float64, device=dev), 6)
     vn3 = torch.zeros((g.ne, 3), dtype=torch.float64, device=dev)   # ldk*8 not a multiple of 16
     with pytest.raises(lib.IconError):
         lib.dycore_div_vort(g, vn3, torch.zeros((g.nc, 3), dtype=torch.float64, device=dev),

@@ -141,3 +141,20 @@ def test_cc_schedule_merges_runs_on_the_canonical_grid():
     with pytest.raises(lib.IconError):
         g.cc_schedule_check(0, 200, 200, 202)        # nlev the kernel does not hold
     g.close()
+
+
+def test_binding_rejects_malformed_fields_before_the_library_sees_them():
+    """the ctypes binding only marshals, but it refuses what would become an illegal address or an out-of-bounds write:
+    host tensors, non-contiguous views, wrong row counts, mismatched leading dimensions or dtypes"""
+    import torch
+    g = lib.IconGrid(1, 0, binding.ICON_HOST_ONLY)
+    zh = np.linspace(3.0, 0.0, 5)
+    vn, w = torch.zeros((g.ne, 4), dtype=torch.float64), torch.zeros((g.nc, 6), dtype=torch.float64)
+    out = torch.zeros((g.ne, 4), dtype=torch.float64)
+    with pytest.raises(TypeError):                      # host tensors: there is no CPU path
+        lib.dycore_velocity_tendencies(g, zh, vn, w, out, 4)
+    with pytest.raises(TypeError):
+        lib.dycore_div_vort(g, vn, torch.zeros((g.nc, 4), dtype=torch.float64), torch.zeros((g.nv, 4), dtype=torch.float64), 4)
+    with pytest.raises(ValueError):                     # z_half of the wrong length
+        lib.dycore_step(g, zh[:-1], vn, w, out, out, out, 4)
+    g.close()
