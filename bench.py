@@ -479,6 +479,84 @@ def run_ours(args):
     return 0
 
 
+def run_launch_study(args):
+    """--launch-study (the paper replays small kernels as CUDA graphs): on the small
+    grids the step is one kernel of tens of microseconds, so the launch path matters. Times N dycore_step calls launched
+    one by one from Python through the C-ABI against the same N calls captured once into a CUDA graph and replayed, with
+    the 126 MB L2 left warm and flushed between steps. One JSON line."""
+    import torch
+    import paper_2511_02021_b200 as lib
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product has no CPU path")
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    lib.load_library()
+    n, out = 200, []
+    for k in (4, 5):
+        g = lib.IconGrid(k)
+        nlev, ldk = 90, 96
+        vn_h, w_h, zh = si.make_fields(1, g.table_host("edge_xyz"), g.table_host("edge_normal"), g.nc, nlev=nlev, ldk=ldk, ldk_w=ldk, pad_value=0.0)
+        vn, w = torch.from_numpy(vn_h).to(dev), torch.from_numpy(w_h).to(dev)
+        ddt, div, vort = (torch.zeros((m, ldk), dtype=torch.float64, device=dev) for m in (g.ne, g.nc, g.nv))
+        flush = torch.empty(256 * 2 ** 20, dtype=torch.uint8, device=dev)
+        step = lambda: lib.dycore_step(g, zh, vn, w, ddt, div, vort, nlev)
+        step()
+        torch.cuda.synchronize()
+        res = {"grid": "R2B%d x %d levels fp64" % (k, nlev), "points": g.ne * nlev, "steps": n}
+        for flushed in (False, True):
+            def body():
+                for _ in range(n):
+                    if flushed:
+                        flush.fill_(1)
+                    step()
+            # (a) launched one by one
+            body()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            body()
+            torch.cuda.synchronize()
+            t_stream = (time.perf_counter() - t0) / n
+            # (b) the same sequence captured once, replayed
+            side = torch.cuda.Stream()
+            side.wait_stream(torch.cuda.current_stream())
+            torch.cuda.synchronize()
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph):
+                body()
+            graph.replay()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            graph.replay()
+            torch.cuda.synchronize()
+            t_graph = (time.perf_counter() - t0) / n
+            # the flush alone, to subtract
+            t_flush = 0.0
+            if flushed:
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                for _ in range(n):
+                    flush.fill_(1)
+                torch.cuda.synchronize()
+                t_flush = (time.perf_counter() - t0) / n
+            key = "l2_flushed" if flushed else "l2_warm"
+            res[key] = {"us_per_step_stream": (t_stream - t_flush) * 1e6, "us_per_step_graph": (t_graph - t_flush) * 1e6,
+                        "us_flush": t_flush * 1e6, "gpts_stream": g.ne * nlev / (t_stream - t_flush) / 1e9,
+                        "gpts_graph": g.ne * nlev / (t_graph - t_flush) / 1e9}
+        # device time of one kernel alone (events), L2 warm
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        ts = []
+        for _ in range(20):
+            ev[0].record(); step(); ev[1].record()
+            torch.cuda.synchronize()
+            ts.append(ev[0].elapsed_time(ev[1]) * 1e3)
+        res["us_kernel_events_median"] = float(np.median(ts))
+        out.append(res)
+        g.close()
+    print(json.dumps({"launch_study": out, "what": "wall-clock microseconds per dycore_step over %d back-to-back steps: launched one "
+                      "by one through the C-ABI from Python vs captured once into a CUDA graph and replayed" % n}))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -495,7 +573,10 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-parity-spot", action="store_true", dest="no_parity_spot")
     ap.add_argument("--spot-points", type=int, default=3000, dest="spot_points")
+    ap.add_argument("--launch-study", action="store_true", dest="launch_study", help="CUDA-graph vs stream launches on R2B4 / R2B5")
     args = ap.parse_args()
+    if args.launch_study:
+        return run_launch_study(args)
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
     return run_reference(args) if args.impl == "reference" else run_ours(args)

@@ -64,6 +64,12 @@ def _load():
         f.argtypes = [P, ctypes.c_int, i64, P, i64, P, P, P, P]
     L.og_sample_ddt_vn.restype = None
     L.og_sample_ddt_vn.argtypes = [P, ctypes.c_int, i64, i64, P, P, P, i64, P, P, P, P]
+    L.og_w_tendency.restype = ctypes.c_int
+    L.og_w_tendency.argtypes = [P, ctypes.c_int, i64, i64, P, P, P, P, P]
+    L.og_sample_ddt_w.restype = None
+    L.og_sample_ddt_w.argtypes = [P, ctypes.c_int, i64, i64, P, P, P, i64, P, P, P, P]
+    L.og_ddt_w.restype = None
+    L.og_ddt_w.argtypes = [i64, ctypes.c_int, i64, i64, P, P, P, P, P, P, P, P, P]
     L.og_divergence.restype = None
     L.og_divergence.argtypes = [i64, ctypes.c_int, i64, P, P, P, P, P]
     L.og_vorticity.restype = None
@@ -90,7 +96,7 @@ _TABLES = {
     "edge_xyz": (np.float64, "e", 3), "edge_normal": (np.float64, "e", 3),
     "l_e": (np.float64, "e", 1), "d_e": (np.float64, "e", 1), "inv_d_e": (np.float64, "e", 1),
     "f_e": (np.float64, "e", 1), "c_lin": (np.float64, "e", 2), "rbf": (np.float64, "e", 4),
-    "a_c": (np.float64, "c", 1), "bln": (np.float64, "c", 3), "a_v": (np.float64, "v", 1),
+    "a_c": (np.float64, "c", 1), "bln": (np.float64, "c", 3), "adv_c": (np.float64, "c", 3), "a_v": (np.float64, "v", 1),
     "geofac_div": (np.float64, "c", 3), "geofac_rot": (np.float64, "v", 6),
 }
 TABLE_NAMES = tuple(_TABLES)
@@ -181,6 +187,17 @@ class Grid:
             out["m_ddt"] = m
         return out
 
+    def w_tendency(self, vn, w, z_half, nlev, with_scale=False):
+        """vertical-wind tendency ddt_w [nc][ldk_w] on the nlev+1 half levels (reading P-19)[, m_w]"""
+        vn, w, z_half = _f64(vn), _f64(w), _f64(z_half)
+        ldk, ldk_w = vn.shape[1], w.shape[1]
+        out = np.zeros((self.nc, ldk_w))
+        m = np.zeros((self.nc, ldk_w)) if with_scale else None
+        rc = self._L.og_w_tendency(self._h, nlev, ldk, ldk_w, _ptr(z_half), _ptr(vn), _ptr(w), _ptr(out), _ptr(m))
+        if rc:
+            raise RuntimeError("og_w_tendency rc=%d" % rc)
+        return (out, m) if with_scale else out
+
     # ---- sampled one-by-one evaluation (full-size parity) ----
     def sample(self, what, idx, lev, vn, nlev, w=None, z_half=None):
         vn = _f64(vn)
@@ -199,6 +216,11 @@ class Grid:
             z_half = _f64(z_half)
             self._L.og_sample_ddt_vn(self._h, nlev, ldk, w.shape[1], _ptr(z_half), _ptr(vn), _ptr(w), n,
                                      _ptr(idx), _ptr(lev), _ptr(out), _ptr(m))
+        elif what == "ddt_w":
+            w = _f64(w)
+            z_half = _f64(z_half)
+            self._L.og_sample_ddt_w(self._h, nlev, ldk, w.shape[1], _ptr(z_half), _ptr(vn), _ptr(w), n,
+                                    _ptr(idx), _ptr(lev), _ptr(out), _ptr(m))
         else:
             raise ValueError(what)
         return out, m
@@ -247,3 +269,15 @@ def velocity_tendencies_from_arrays(t, vn, w, z_half, nlev):
     L.og_ddt_vn(ne, nlev, ldk, ldk_w, _ptr(z_half), _ptr(e2c), _ptr(e2v), _ptr(inv_d), _ptr(f_e), _ptr(c_lin),
                 _ptr(vn), _ptr(w), _ptr(vt), _ptr(ke_c), _ptr(vort), _ptr(ddt), _ptr(m))
     return {"ddt_vn": ddt, "vt": vt, "ke_e": ke_e, "ke_c": ke_c, "vort": vort, "m_ddt": m}
+
+
+def w_tendency_from_arrays(t, vn, w, z_half, nlev):
+    """og_ddt_w on a dict ``t`` of explicit tables (c2e, e2c, inv_d_e, adv_c); returns (ddt_w, m_w)"""
+    L = _load()
+    vn, w, z_half = _f64(vn), _f64(w), _f64(z_half)
+    c2e, e2c = np.ascontiguousarray(t["c2e"], np.int32), np.ascontiguousarray(t["e2c"], np.int32)
+    inv_d, adv = _f64(t["inv_d_e"]), _f64(t["adv_c"])
+    nc, ldk, ldk_w = c2e.shape[0], vn.shape[1], w.shape[1]
+    out, m = np.zeros((nc, ldk_w)), np.zeros((nc, ldk_w))
+    L.og_ddt_w(nc, nlev, ldk, ldk_w, _ptr(z_half), _ptr(c2e), _ptr(e2c), _ptr(inv_d), _ptr(adv), _ptr(vn), _ptr(w), _ptr(out), _ptr(m))
+    return out, m

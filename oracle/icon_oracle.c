@@ -64,6 +64,7 @@ typedef struct og_grid {
     double *rbf;                    /* [ne][4] */
     double *a_c;                    /* [nc] */
     double *bln;                    /* [nc][3] */
+    double *adv_c;                  /* [nc][3] reading P-19: sum_j adv_c(c,j) n_j n_j^T = I in the tangent plane of c */
     double *a_v;                    /* [nv] */
     double *geofac_div;             /* [nc][3] */
     double *geofac_rot;             /* [nv][6] */
@@ -243,7 +244,7 @@ static void og_free_fields(og_grid *g)
     free(g->v2e); free(g->v2c); free(g->v_deg); free(g->c_os); free(g->v_os);
     free(g->vert_xyz); free(g->cell_xyz); free(g->edge_xyz); free(g->edge_normal);
     free(g->l_e); free(g->d_e); free(g->inv_d_e); free(g->f_e); free(g->c_lin); free(g->rbf);
-    free(g->a_c); free(g->bln); free(g->a_v); free(g->geofac_div); free(g->geofac_rot);
+    free(g->a_c); free(g->bln); free(g->adv_c); free(g->a_v); free(g->geofac_div); free(g->geofac_rot);
 }
 void og_grid_destroy(og_grid *g)
 {
@@ -458,6 +459,7 @@ static void og_build_geometry(og_grid *g)
     g->rbf = (double *)malloc(sizeof(double) * 4 * (size_t)ne);
     g->a_c = (double *)malloc(sizeof(double) * (size_t)nc);
     g->bln = (double *)malloc(sizeof(double) * 3 * (size_t)nc);
+    g->adv_c = (double *)malloc(sizeof(double) * 3 * (size_t)nc);
     g->a_v = (double *)malloc(sizeof(double) * (size_t)nv);
     g->geofac_div = (double *)malloc(sizeof(double) * 3 * (size_t)nc);
     g->geofac_rot = (double *)malloc(sizeof(double) * 6 * (size_t)nv);
@@ -524,6 +526,39 @@ static void og_build_geometry(og_grid *g)
         g->bln[3 * c] = (xi[1] * eta[2] - xi[2] * eta[1]) / det;
         g->bln[3 * c + 1] = (xi[2] * eta[0] - xi[0] * eta[2]) / det;
         g->bln[3 * c + 2] = (xi[0] * eta[1] - xi[1] * eta[0]) / det;
+    }
+    /* P-19: adv_c = the three weights a_j with sum_j a_j n_j n_j^T = I (2x2 identity) in the tangent plane at
+     * the cell centre, n_j = the edge normal projected onto that plane and normalised. With them
+     * sum_j a_j (u.n_j)(grad s.n_j) = u.grad s for locally constant u and grad s: the advection of a cell scalar
+     * by the normal wind components alone (no vertex values needed). Equilateral triangle: a_j = 2/3. */
+#pragma omp parallel for schedule(static)
+    for (int64_t c = 0; c < nc; ++c) {
+        const double *cc = g->cell_xyz + 3 * c;
+        const double *p0 = V + 3 * g->c2v[3 * c];
+        double d0 = dot3(p0, cc);
+        double e1[3] = { p0[0] - d0 * cc[0], p0[1] - d0 * cc[1], p0[2] - d0 * cc[2] };
+        normalize3(e1);
+        double e2[3];
+        cross3(cc, e1, e2);
+        double nx[3], ny[3];
+        for (int j = 0; j < 3; ++j) {
+            const double *nn = g->edge_normal + 3 * g->c2e[3 * c + j];
+            double px = dot3(nn, e1), py = dot3(nn, e2);
+            double len = sqrt(px * px + py * py);
+            nx[j] = px / len; ny[j] = py / len;
+        }
+        /* rows: n_x^2, n_x n_y, n_y^2; right-hand side (1, 0, 1); Cramer's rule */
+        double A[3][3], b[3] = { 1.0, 0.0, 1.0 };
+        for (int j = 0; j < 3; ++j) { A[0][j] = nx[j] * nx[j]; A[1][j] = nx[j] * ny[j]; A[2][j] = ny[j] * ny[j]; }
+        double det = A[0][0] * (A[1][1] * A[2][2] - A[1][2] * A[2][1]) - A[0][1] * (A[1][0] * A[2][2] - A[1][2] * A[2][0])
+                   + A[0][2] * (A[1][0] * A[2][1] - A[1][1] * A[2][0]);
+        for (int j = 0; j < 3; ++j) {
+            double M[3][3];
+            for (int r = 0; r < 3; ++r) for (int q = 0; q < 3; ++q) M[r][q] = (q == j) ? b[r] : A[r][q];
+            double dj = M[0][0] * (M[1][1] * M[2][2] - M[1][2] * M[2][1]) - M[0][1] * (M[1][0] * M[2][2] - M[1][2] * M[2][0])
+                      + M[0][2] * (M[1][0] * M[2][1] - M[1][1] * M[2][0]);
+            g->adv_c[3 * c + j] = dj / det;
+        }
     }
     /* P-8: dual area = sum over the fan of (v, x_e(i), c_i) and (v, c_i, x_e(i+1));
      * geofac_rot = d_e * v_os / A*_v (0 in the pentagon pad slot) */
@@ -636,6 +671,7 @@ og_grid *og_grid_round_f32(const og_grid *s)
     g->rbf = og_round_copy(s->rbf, 4 * ne);
     g->a_c = og_round_copy(s->a_c, nc);
     g->bln = og_round_copy(s->bln, 3 * nc);
+    g->adv_c = og_round_copy(s->adv_c, 3 * nc);
     g->a_v = og_round_copy(s->a_v, nv);
     g->geofac_div = og_round_copy(s->geofac_div, 3 * nc);
     g->geofac_rot = og_round_copy(s->geofac_rot, 6 * nv);
@@ -779,6 +815,83 @@ void og_ddt_vn(int64_t ne, int nlev, int64_t ldk, int64_t ldk_w, const double *z
     }
 }
 
+/* Vertical-wind tendency, reading P-19 (the other half of the velocity-tendency routine of
+ * the dycore; the paper prints none of it). w lives at cells on the nlev+1 half levels, k = 0 top.
+ *   interior half levels k = 1 .. nlev-1:
+ *     hadv(c,k) = sum_{j<3} adv_c(c,j) * vn_ie(e_j,k) * (w(c1(e_j),k) - w(c0(e_j),k)) * inv_d_e(e_j),  e_j = c2e[c][j]
+ *                 (normal wind interpolated to the half level, P-14; both factors follow the edge's own orientation)
+ *     vadv(c,k) = w(c,k) * (w(c,k-1) - w(c,k+1)) / (z_half[k-1] - z_half[k+1])
+ *     ddt_w(c,k) = -(hadv + vadv)
+ *   k = 0 and k = nlev (model top and surface: boundary conditions of w): ddt_w = 0.
+ * m_w (may be NULL) = P-16 scale: sum_j |adv_c| |vn_ie| (|w(c1)|+|w(c0)|) inv_d_e + |w(k)| (|w(k-1)|+|w(k+1)|)/dz. */
+void og_ddt_w(int64_t nc, int nlev, int64_t ldk, int64_t ldk_w, const double *z_half, const int32_t *c2e,
+              const int32_t *e2c, const double *inv_d_e, const double *adv_c, const double *vn, const double *w,
+              double *ddt_w, double *m_w)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t c = 0; c < nc; ++c) {
+        for (int k = 0; k <= nlev; ++k) {
+            double val = 0.0, m = 0.0;
+            if (k >= 1 && k <= nlev - 1) {
+                double hadv = 0.0;
+                for (int j = 0; j < 3; ++j) {
+                    int64_t e = c2e[3 * c + j];
+                    int64_t c0 = e2c[2 * e], c1 = e2c[2 * e + 1];
+                    double vie = og_vn_half(vn + e * ldk, nlev, z_half, k);
+                    double gw = (w[c1 * ldk_w + k] - w[c0 * ldk_w + k]) * inv_d_e[e];
+                    hadv += adv_c[3 * c + j] * vie * gw;
+                    m += fabs(adv_c[3 * c + j]) * fabs(vie) * (fabs(w[c1 * ldk_w + k]) + fabs(w[c0 * ldk_w + k])) * inv_d_e[e];
+                }
+                double dz2 = z_half[k - 1] - z_half[k + 1];
+                double vadv = w[c * ldk_w + k] * (w[c * ldk_w + k - 1] - w[c * ldk_w + k + 1]) / dz2;
+                m += fabs(w[c * ldk_w + k]) * (fabs(w[c * ldk_w + k - 1]) + fabs(w[c * ldk_w + k + 1])) / dz2;
+                val = -(hadv + vadv);
+            }
+            ddt_w[c * ldk_w + k] = val;
+            if (m_w) m_w[c * ldk_w + k] = m;
+        }
+    }
+}
+
+int og_w_tendency(const og_grid *g, int nlev, int64_t ldk, int64_t ldk_w, const double *z_half,
+                  const double *vn, const double *w, double *ddt_w, double *m_w)
+{
+    if (!g || nlev < 2 || ldk < nlev || ldk_w < nlev + 1) return -1;
+    for (int k = 0; k < nlev; ++k) if (!(z_half[k] > z_half[k + 1])) return -2;
+    og_ddt_w(g->nc, nlev, ldk, ldk_w, z_half, g->c2e, g->e2c, g->inv_d_e, g->adv_c, vn, w, ddt_w, m_w);
+    return 0;
+}
+
+/* sampled evaluation of ddt_w at (cell idx[i], half level lev[i]), same arithmetic as og_ddt_w */
+void og_sample_ddt_w(const og_grid *g, int nlev, int64_t ldk, int64_t ldk_w, const double *z_half,
+                     const double *vn, const double *w, int64_t n, const int64_t *idx, const int32_t *lev,
+                     double *val, double *scale)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) {
+        int64_t c = idx[i];
+        int k = lev[i];
+        double v = 0.0, m = 0.0;
+        if (k >= 1 && k <= nlev - 1) {
+            double hadv = 0.0;
+            for (int j = 0; j < 3; ++j) {
+                int64_t e = g->c2e[3 * c + j];
+                int64_t c0 = g->e2c[2 * e], c1 = g->e2c[2 * e + 1];
+                double vie = og_vn_half(vn + e * ldk, nlev, z_half, k);
+                double gw = (w[c1 * ldk_w + k] - w[c0 * ldk_w + k]) * g->inv_d_e[e];
+                hadv += g->adv_c[3 * c + j] * vie * gw;
+                m += fabs(g->adv_c[3 * c + j]) * fabs(vie) * (fabs(w[c1 * ldk_w + k]) + fabs(w[c0 * ldk_w + k])) * g->inv_d_e[e];
+            }
+            double dz2 = z_half[k - 1] - z_half[k + 1];
+            double vadv = w[c * ldk_w + k] * (w[c * ldk_w + k - 1] - w[c * ldk_w + k + 1]) / dz2;
+            m += fabs(w[c * ldk_w + k]) * (fabs(w[c * ldk_w + k - 1]) + fabs(w[c * ldk_w + k + 1])) / dz2;
+            v = -(hadv + vadv);
+        }
+        val[i] = v;
+        if (scale) scale[i] = m;
+    }
+}
+
 /* dycore_div_vort: S1 + S2 */
 int og_div_vort(const og_grid *g, int nlev, int64_t ldk, const double *vn, double *div, double *vort,
                 double *m_div, double *m_vort)
@@ -894,7 +1007,7 @@ const void *og_grid_table(const og_grid *g, const char *name)
 #define T(n) if (!strcmp(name, #n)) return g->n
     T(c2v); T(c2e); T(e2c); T(e2v); T(e2e4); T(v2e); T(v2c); T(v_deg); T(c_os); T(v_os);
     T(vert_xyz); T(cell_xyz); T(edge_xyz); T(edge_normal); T(l_e); T(d_e); T(inv_d_e); T(f_e);
-    T(c_lin); T(rbf); T(a_c); T(bln); T(a_v); T(geofac_div); T(geofac_rot);
+    T(c_lin); T(rbf); T(a_c); T(bln); T(adv_c); T(a_v); T(geofac_div); T(geofac_rot);
 #undef T
     return NULL;
 }

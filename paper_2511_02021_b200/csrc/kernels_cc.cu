@@ -127,7 +127,17 @@ struct CcDev {
     const int64_t* cta_step_begin;    // [n_ctas + 1]
     int n_slots;
     int slot_bytes;
+    int64_t ne, nc, nv;               // rows of the caller's fields (bounds asserts of the CC_DEBUG build)
 };
+
+#ifdef CC_DEBUG
+// the pool's own bounds checks (compute-sanitizer is closed on the B200 pool): every slot read stays inside the slot
+// pool + its readable pad, every output column id is a row of its field
+#define CC_ASSERT(cond, what, a, b) \
+    do { if (!(cond)) { printf("cc assert %s: block %d thread %d: %lld %lld\n", what, blockIdx.x, threadIdx.x, (long long)(a), (long long)(b)); __trap(); } } while (0)
+#else
+#define CC_ASSERT(cond, what, a, b) do { } while (0)
+#endif
 
 // ---- the L levels of one column a lane owns ---------------------------------------------------------
 // L == 3: v[0], v[1] = levels 2*lane, 2*lane+1 (one 16-byte access), v[2] = level 64+lane. L == 1: level = lane.
@@ -371,6 +381,8 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
                         const uint2 q = base == 0 ? e0 : __ldg(lraw + load_begin + base + mine);
                         // CcLoad: id | slot (bits 0..15) bytes/16 (bits 16..30) kind (bit 31)
                         const uint32_t slot = q.y & 0xffffu, kind = q.y >> 31, bytes = ((q.y >> 16) & 0x7fffu) << 4;
+                        CC_ASSERT(slot * (uint32_t)d.slot_bytes + bytes <= (uint32_t)d.n_slots * (uint32_t)d.slot_bytes && bytes > 0, "copy destination", slot, bytes);
+                        CC_ASSERT((uint64_t)q.x * (kind ? cs_w : cs) + bytes <= (uint64_t)(kind ? d.nc : d.ne) * (kind ? cs_w : cs), "copy source", q.x, kind);
                         const unsigned char* src = kind ? reinterpret_cast<const unsigned char*>(w) + (uint64_t)q.x * cs_w
                                                         : reinterpret_cast<const unsigned char*>(vn) + (uint64_t)q.x * cs;
                         bulk_g2s(slot0 + slot * (uint32_t)d.slot_bytes, src, bytes, fb);
@@ -416,6 +428,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
             // the slot (or of the next one; the pool ends with a readable pad) that only ever reach outputs through
             // the level-below neighbour of the last level, which VD masks.
             auto LD = [&](uint32_t off) {
+                CC_ASSERT(off % 16 == 0 && off + 96 * sizeof(T) <= (uint32_t)d.n_slots * (uint32_t)d.slot_bytes + kCcSlotTailPad, "slot offset", off, d.n_slots);
                 C c;
                 if constexpr (L == 1) {
                     c.v[0] = *reinterpret_cast<const T*>(my_pair + off);
@@ -443,6 +456,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
             // not push halo columns out of the L2); id < 0 = not ours
             auto ST = [&](T* base, int32_t id, const C& x) {
                 if (id < 0) return;
+                CC_ASSERT(id < (base == ddt_vn ? d.ne : base == div ? d.nc : d.nv), "output id", id, base == ddt_vn ? 0 : base == div ? 1 : 2);
                 // one 64-bit column base (warp-uniform) plus the lane's two 32-bit byte offsets
                 unsigned char* col = reinterpret_cast<unsigned char*>(base) + (uint64_t)(uint32_t)id * cs;
                 if constexpr (L == 1) {
@@ -689,6 +703,7 @@ int launch_tendencies_cc(const icon_grid& g, DevCcTables<T>& p, int nlev, int64_
     d.steps = p.steps; d.loads = p.loads; d.records = p.records;
     d.cta_patch_begin = p.cta_patch_begin; d.cta_step_begin = p.cta_step_begin;
     d.n_slots = p.n_slots; d.slot_bytes = p.slot_bytes;
+    d.ne = g.host.ne; d.nc = g.host.nc; d.nv = g.host.nv;
     // pacing: a barrier of the producers every `period` steps (power of two), counted in p.progress (never reset)
     const int period = g.options[ICON_OPT_CC_PACE];
     const int L = cc_levels_per_lane(nlev);

@@ -308,6 +308,57 @@ def test_column_cache_level_mappings_and_tiles(torch_cuda, lib, oracle_grid, til
         g.set_option(lib.ICON_OPT_TENDENCY_KERNEL, 5)
 
 
+@pytest.mark.parametrize("k,period", [(5, 4), (5, 512), (3, 16)])
+def test_dycore_step_replays_in_a_cuda_graph(torch_cuda, lib, oracle_grid, k, period):
+    """SURVEY.md 8(f) NEXT-4 (the paper's remedy for launch-bound small kernels): dycore_step captured once
+    into a CUDA graph and replayed 12 times on alternating inputs written into the captured buffers; every replay is
+    compared with the oracle. The pacing epoch lives on the device (a captured kernel argument would go stale): periods 4
+    and 16 arm many barriers per launch."""
+    torch = torch_cuda
+    og = oracle_grid(k)
+    g = lib_grid(lib, k)
+    dev = torch.device("cuda:0")
+    nlev = 90
+    sets = []
+    for cfg, fv in ((1, 1.0), (2, -2.0)):
+        vn, w, zh = si.make_fields(cfg, og.edge_xyz, og.edge_normal, og.nc, nlev=nlev, ldk=96, ldk_w=96)
+        vn, w = np.nan_to_num(vn) * fv, np.nan_to_num(w)
+        sets.append((torch.from_numpy(vn).to(dev), torch.from_numpy(w).to(dev), zh, oracle_reference(og, vn, w, zh, nlev, False)))
+    g.set_option(lib.ICON_OPT_TENDENCY_KERNEL, 5)
+    g.set_option(lib.ICON_OPT_CC_PACE, period)
+    try:
+        s_vn, s_w = sets[0][0].clone(), sets[0][1].clone()                       # the buffers the graph reads
+        outs = [torch.full((n, 96), float("nan"), dtype=torch.float64, device=dev) for n in (g.ne, g.nc, g.nv)]
+        zh = sets[0][2]
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):                                            # first call: builds and uploads the tables
+            lib.dycore_step(g, zh, s_vn, s_w, outs[0], outs[1], outs[2], nlev)
+        torch.cuda.current_stream().wait_stream(side)
+        torch.cuda.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph):
+            lib.dycore_step(g, zh, s_vn, s_w, outs[0], outs[1], outs[2], nlev)
+        for it in range(12):
+            d_vn, d_w, _, ref = sets[it % 2]
+            s_vn.copy_(d_vn)
+            s_w.copy_(d_w)
+            for o in outs:
+                o.fill_(float("nan"))
+            graph.replay()
+            torch.cuda.synchronize()
+            res = dict(ddt_vn=outs[0].cpu().numpy(), div=outs[1].cpu().numpy(), vort=outs[2].cpu().numpy())
+            check_all(res, ref, nlev, TOL["f64"])
+        # plain launches still work after the replays (the device-side epoch stays consistent)
+        for o in outs:
+            o.fill_(float("nan"))
+        lib.dycore_step(g, zh, sets[1][0], sets[1][1], outs[0], outs[1], outs[2], nlev)
+        torch.cuda.synchronize()
+        check_all(dict(ddt_vn=outs[0].cpu().numpy(), div=outs[1].cpu().numpy(), vort=outs[2].cpu().numpy()), sets[1][3], nlev, TOL["f64"])
+    finally:
+        g.set_option(lib.ICON_OPT_CC_PACE, 512)
+
+
 def test_argument_errors_on_device(torch_cuda, lib):
     torch = torch_cuda
     g = lib_grid(lib, 1)

@@ -494,6 +494,111 @@ def test_sampled_evaluation_matches_full_arrays(oracle_grid, k, flags):
 
 
 # ----------------------------------------------------------------------------------------------
+# vertical-wind tendency ddt_w (reading P-19)
+# ----------------------------------------------------------------------------------------------
+def _numpy_ddt_w(g, vn, w, zh, K):
+    """the definition of P-19 re-assembled with numpy (independent of og_ddt_w's loops)"""
+    dz = zh[:-1] - zh[1:]
+    gk = dz[:-1] / (dz[:-1] + dz[1:])
+    vn_ie = np.zeros((g.ne, K + 1))
+    vn_ie[:, 1:K] = gk * vn[:, 1:K] + (1 - gk) * vn[:, :K - 1]
+    gradw = (w[g.e2c[:, 1]] - w[g.e2c[:, 0]]) * g.inv_d_e[:, None]
+    hadv = sum(g.adv_c[:, j:j + 1] * (vn_ie * gradw)[g.c2e[:, j]] for j in range(3))
+    out = np.zeros((g.nc, K + 1))
+    dz2 = zh[:-2] - zh[2:]
+    out[:, 1:K] = -(hadv[:, 1:K] + w[:, 1:K] * (w[:, :K - 1] - w[:, 2:K + 1]) / dz2)
+    return out
+
+
+@pytest.mark.parametrize("k,seed,flags", [(0, 0, 0), (2, 0, 0), (4, 0, 0), (3, 4, 1)])
+def test_adv_c_reconstructs_the_identity(oracle_grid, k, seed, flags):
+    """P-19: the three weights of a cell satisfy sum_j adv_c(c,j) n_j n_j^T = I in the tangent plane at the cell centre
+    (so that sum_j adv_c (u.n_j)(grad s.n_j) = u.grad s), hence also sum_j adv_c = trace I = 2. Checked with numpy from the
+    exported positions and normals in a basis of its own (the identity does not depend on the basis)."""
+    g = oracle_grid(k, seed, flags)
+    cc = g.cell_xyz
+    ref = np.where(np.abs(cc[:, :1]) < 0.9, np.array([[1.0, 0, 0]]), np.array([[0, 1.0, 0]]))
+    e1 = np.cross(cc, ref)
+    e1 /= np.linalg.norm(e1, axis=1)[:, None]
+    e2 = np.cross(cc, e1)
+    S = np.zeros((g.nc, 2, 2))
+    for j in range(3):
+        n = g.edge_normal[g.c2e[:, j]]
+        p = np.stack([(n * e1).sum(1), (n * e2).sum(1)], 1)
+        p /= np.linalg.norm(p, axis=1)[:, None]
+        S += g.adv_c[:, j, None, None] * p[:, :, None] * p[:, None, :]
+    assert np.abs(S - np.eye(2)[None]).max() < 1e-13
+    assert np.abs(g.adv_c.sum(1) - 2).max() < 1e-13
+    assert (g.adv_c > 0.3).all() and (g.adv_c < 1.0).all()          # 2/3 each on an equilateral triangle
+
+
+def test_ddt_w_definition_and_special_cases(oracle_grid):
+    g = oracle_grid(2)
+    K = 7
+    zh = si.z_half_levels(K)
+    rng = np.random.default_rng(21)
+    vn = rng.standard_normal((g.ne, K)) * 10
+    w = rng.standard_normal((g.nc, K + 1))
+    got, m = g.w_tendency(vn, w, zh, K, with_scale=True)
+    want = _numpy_ddt_w(g, vn, w, zh, K)
+    assert (np.abs(got - want) <= 1e-14 * np.maximum(m, 1e-300))[:, 1:K].all()
+    assert (got[:, 0] == 0).all() and (got[:, K] == 0).all()          # top and surface: boundary conditions of w
+    # horizontally uniform w: no horizontal advection whatever vn; w linear in z: -w dw/dz exactly
+    b, c0 = 2.0e-4, 0.3
+    wl = np.repeat((c0 + b * zh)[None, :], g.nc, axis=0)
+    got = g.w_tendency(vn, wl, zh, K)
+    assert np.abs(got[:, 1:K] + (wl * b)[:, 1:K]).max() < 1e-13 * np.abs(wl * b).max()
+    # vn = 0: only the vertical part, for any w
+    got = g.w_tendency(np.zeros_like(vn), w, zh, K)
+    dz2 = zh[:-2] - zh[2:]
+    assert np.abs(got[:, 1:K] + w[:, 1:K] * (w[:, :K - 1] - w[:, 2:]) / dz2).max() < 1e-13
+    # two-sided pin of the tolerance scale
+    gradw_abs = (np.abs(w[g.e2c[:, 1]]) + np.abs(w[g.e2c[:, 0]])) * g.inv_d_e[:, None]
+    dz = zh[:-1] - zh[1:]
+    gk = dz[:-1] / (dz[:-1] + dz[1:])
+    vie = np.zeros((g.ne, K + 1))
+    vie[:, 1:K] = gk * vn[:, 1:K] + (1 - gk) * vn[:, :K - 1]
+    mm = sum(np.abs(g.adv_c[:, j:j + 1]) * (np.abs(vie) * gradw_abs)[g.c2e[:, j]] for j in range(3))
+    mm[:, 1:K] += np.abs(w[:, 1:K]) * (np.abs(w[:, :K - 1]) + np.abs(w[:, 2:])) / dz2
+    assert (m[:, 1:K] <= 1.0000001 * mm[:, 1:K]).all() and (m[:, 1:K] >= 0.9999999 * mm[:, 1:K]).all()
+    # sampled evaluation = full arrays
+    idx, lev = si.sample_points(5, g.nc, K + 1, 400)
+    val, ms = g.sample("ddt_w", idx, lev, vn, K, w=w, z_half=zh)
+    full, mfull = g.w_tendency(vn, w, zh, K, with_scale=True)
+    assert np.abs(val - full[idx, lev]).max() == 0 and np.abs(ms - mfull[idx, lev]).max() == 0
+
+
+def test_ddt_w_converges_to_the_advection_of_a_tilted_solid_body_flow(oracle_grid):
+    """Closed form: w(x) = w0 (x.z_hat) carried by the solid-body rotation u = a Omega' x x about a TILTED axis has
+    -u.grad w = -w0 (Omega' x x).z_hat at every level (uniform in z, so the vertical part vanishes). The discrete
+    ddt_w converges to it at first order; a weight set that does not reproduce u.grad s (e.g. bln in place of adv_c: half
+    the value) stays at an error of order one."""
+    om = 2.0e-6 * np.array([np.sin(0.7), 0.0, np.cos(0.7)])          # rad/s, tilted by 0.7 rad
+    w0, K = 0.5, 4
+    zh = si.z_half_levels(K)
+    errs = []
+    for k in (2, 3, 4):
+        g = oracle_grid(k)
+        u = np.cross(om[None, :], g.edge_xyz) * A                     # m/s at edge midpoints
+        vn = np.repeat((u * g.edge_normal).sum(1)[:, None], K, axis=1)
+        w = np.repeat((w0 * g.cell_xyz[:, 2])[:, None], K + 1, axis=1)
+        exact = -w0 * np.cross(om[None, :], g.cell_xyz)[:, 2]
+        got = g.w_tendency(vn, w, zh, K)
+        errs.append(np.abs(got[:, 1:K] - exact[:, None]).max() / np.abs(exact).max())
+    assert errs[2] < 0.03, errs
+    assert 1.6 < errs[0] / errs[1] < 4.6 and 1.6 < errs[1] / errs[2] < 4.6, errs
+    # teeth: the edge-to-cell interpolation weights bln (sum 1 instead of 2) give half the advection
+    g = oracle_grid(3)
+    u = np.cross(om[None, :], g.edge_xyz) * A
+    vn = np.repeat((u * g.edge_normal).sum(1)[:, None], K, axis=1)
+    w = np.repeat((w0 * g.cell_xyz[:, 2])[:, None], K + 1, axis=1)
+    gradw = (w[g.e2c[:, 1]] - w[g.e2c[:, 0]]) * g.inv_d_e[:, None]
+    half = -sum(g.bln[:, j:j + 1] * (vn[:, :1] * gradw[:, :1])[g.c2e[:, j]] for j in range(3))[:, 0]
+    exact = -w0 * np.cross(om[None, :], g.cell_xyz)[:, 2]
+    assert np.abs(half - exact).max() / np.abs(exact).max() > 0.3
+
+
+# ----------------------------------------------------------------------------------------------
 # seeded permutation (P-7)
 # ----------------------------------------------------------------------------------------------
 def _perm_from_positions(a_perm, a_canon, decimals=12):
