@@ -86,6 +86,8 @@ enum {
     ICON_TAB_A_V,          /* f64 [nv] dual-cell area, m^2 */
     ICON_TAB_GEOFAC_DIV,   /* f64 [nc][3] l_e*c_os/A_c */
     ICON_TAB_GEOFAC_ROT,   /* f64 [nv][6] d_e*v_os/A_v, 0 in the pentagon pad */
+    ICON_TAB_ADV_C,        /* f64 [nc][3] normal-component reconstruction weights of the vertical-wind tendency:
+                              sum_j adv_c(c,j) n_j n_j^T = I in the tangent plane of the cell (P-19) */
     ICON_TAB_COUNT
 };
 
@@ -193,6 +195,20 @@ int dycore_velocity_tendencies(const icon_grid_t* g, int dtype, int nlev, int ld
                                const double* z_half,
                                const void* vn, const void* w, void* ddt_vn,
                                void* vt_opt, void* ke_c_opt, void* vort_opt, void* cuda_stream);
+
+/*
+ * dycore_w_tendency -- SURVEY.md 8(f) NEXT-2: the vertical-wind tendency, the other half of the velocity-tendency
+ * routine of the dynamical core (PAPER.md:142 names the dycore; the paper prints none of its vertical-wind statements,
+ * reading P-19 of DESIGN.md section 3). w and ddt_w live at cells on the nlev+1 half levels, k = 0 at the top:
+ *   k = 1 .. nlev-1:  ddt_w(c,k) = -[ sum_{j<3} adv_c(c,j) * vn_ie(e_j,k) * (w(c1(e_j),k) - w(c0(e_j),k)) / d_e(e_j)
+ *                                     + w(c,k) * (w(c,k-1) - w(c,k+1)) / (z_half[k-1] - z_half[k+1]) ],  e_j = c2e[c][j],
+ *   k = 0 and k = nlev: ddt_w = 0 (the top and surface values of w are boundary conditions).
+ * vn_ie = vn interpolated linearly in z to the half level (P-14). z_half [nlev+1] HOST, strictly decreasing.
+ * vn [ne][ldk], w [nc][ldk_w] dev in; ddt_w [nc][ldk_w] dev out (levels 0 .. nlev written, pads untouched).
+ * 2 <= nlev <= ldk, nlev+1 <= ldk_w.
+ */
+int dycore_w_tendency(const icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
+                      const void* vn, const void* w, void* ddt_w, void* cuda_stream);
 
 /*
  * dycore_step -- one pass of the whole hot path: the outputs of

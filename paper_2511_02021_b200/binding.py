@@ -23,13 +23,13 @@ ICON_OPT_CC_PACE = 2
 
 TABLES = ("c2v", "c2e", "e2c", "e2v", "e2e4", "v2e", "v2c", "v_deg", "c_os", "v_os",
           "vert_xyz", "cell_xyz", "edge_xyz", "edge_normal", "l_e", "d_e", "inv_d_e", "f_e", "c_lin", "rbf",
-          "a_c", "bln", "a_v", "geofac_div", "geofac_rot")
+          "a_c", "bln", "a_v", "geofac_div", "geofac_rot", "adv_c")
 TABLE_ID = {n: i for i, n in enumerate(TABLES)}
 
 # every symbol include/icon_dycore.h declares
 EXPORTS = ("icon_grid_create", "icon_grid_destroy", "icon_grid_counts", "icon_grid_table_host",
            "icon_grid_table_device", "icon_grid_set_option", "icon_grid_worklist_stats", "icon_grid_cc_schedule_check", "dycore_div_vort", "dycore_velocity_tendencies",
-           "dycore_step", "dycore_step_host", "icon_grid_launch_count", "icon_last_error")
+           "dycore_step", "dycore_step_host", "dycore_w_tendency", "icon_grid_launch_count", "icon_last_error")
 
 
 class IconError(RuntimeError):
@@ -73,6 +73,8 @@ def load_library():
     L.dycore_div_vort.argtypes = [P, ci, ci, ci, P, P, P, P]
     L.dycore_velocity_tendencies.restype = ci
     L.dycore_velocity_tendencies.argtypes = [P, ci, ci, ci, ci, P, P, P, P, P, P, P, P]
+    L.dycore_w_tendency.restype = ci
+    L.dycore_w_tendency.argtypes = [P, ci, ci, ci, ci, P, P, P, P, P]
     L.dycore_step.restype = ci
     L.dycore_step.argtypes = [P, ci, ci, ci, ci, P, P, P, P, P, P, P]
     L.dycore_step_host.restype = ci
@@ -223,6 +225,16 @@ def dycore_velocity_tendencies(grid, z_half, vn, w, ddt_vn, nlev, vt=None, ke_c=
     _check(grid._L.dycore_velocity_tendencies(grid._h, _dtype_of(vn), int(nlev), int(vn.shape[1]), int(w.shape[1]),
                                               _dptr(z), _dptr(vn), _dptr(w), _dptr(ddt_vn), _dptr(vt), _dptr(ke_c),
                                               _dptr(vort), _stream_ptr(stream)))
+
+
+def dycore_w_tendency(grid, z_half, vn, w, ddt_w, nlev, stream=None):
+    """Vertical-wind tendency (reading P-19). vn [ne][ldk], w and ddt_w [nc][ldk_w] on the nlev+1 half levels."""
+    z = np.ascontiguousarray(z_half, dtype=np.float64)
+    if z.size != nlev + 1:
+        raise ValueError("z_half must have nlev+1 entries")
+    _check_fields((("vn", vn, grid.ne, "ldk"), ("w", w, grid.nc, "ldk_w"), ("ddt_w", ddt_w, grid.nc, "ldk_w")))
+    _check(grid._L.dycore_w_tendency(grid._h, _dtype_of(vn), int(nlev), int(vn.shape[1]), int(w.shape[1]), _dptr(z), _dptr(vn),
+                                     _dptr(w), _dptr(ddt_w), _stream_ptr(stream)))
 
 
 def dycore_step(grid, z_half, vn, w, ddt_vn, div, vort, nlev, stream=None):

@@ -120,6 +120,7 @@ int ensure_coeffs(icon_grid* g, icon::DevCoeffs<T>& c) {
     if ((rc = upload_rows(g, h.inv_d_e, 1, ue, &c.inv_d_e))) return rc;
     if ((rc = upload_rows(g, h.f_e, 1, ue, &c.f_e))) return rc;
     if ((rc = upload_rows(g, h.c_lin, 2, ue, &c.c_lin))) return rc;
+    if ((rc = upload_rows(g, h.adv_c, 3, uc, &c.adv_c))) return rc;
     CU_TRY(cudaStreamSynchronize(cudaStreamLegacy));      // uploads ran on the legacy stream, callers may use non-blocking streams
     c.ready = true;
     return ICON_OK;
@@ -334,17 +335,25 @@ void vertical_coefficients(const double* zh, int K, std::vector<double>& abc) {
     }
 }
 
-int get_level_coeffs(icon_grid* g, int dtype, int nlev, const double* z_half, void** out) {
+int get_level_coeffs(icon_grid* g, int dtype, int nlev, const double* z_half, void** out, void** out_wk = nullptr) {
     for (int k = 0; k < nlev; ++k)
         if (!(z_half[k] > z_half[k + 1])) return fail(ICON_EINVAL, "z_half must be strictly decreasing");
     for (auto& lc : g->level_coeffs)
         if (lc.dtype == dtype && (int)lc.z_half.size() == nlev + 1 &&
             std::memcmp(lc.z_half.data(), z_half, sizeof(double) * (nlev + 1)) == 0) {
             *out = lc.abc;
+            if (out_wk) *out_wk = lc.wk;
             return ICON_OK;
         }
     std::vector<double> abc;
     vertical_coefficients(z_half, nlev, abc);
+    // P-19: g_k = dz_{k-1} / (dz_{k-1} + dz_k) (weight of vn(k) in vn_ie(k)) and 1 / (z_half[k-1] - z_half[k+1]), k = 1 .. nlev-1
+    std::vector<double> wk(2 * ((size_t)nlev + 1), 0.0);
+    for (int k = 1; k <= nlev - 1; ++k) {
+        const double up = z_half[k - 1] - z_half[k], dn = z_half[k] - z_half[k + 1];
+        wk[(size_t)k] = up / (up + dn);
+        wk[(size_t)nlev + 1 + k] = 1.0 / (z_half[k - 1] - z_half[k + 1]);
+    }
     icon::LevelCoeffs lc;
     lc.dtype = dtype;
     lc.z_half.assign(z_half, z_half + nlev + 1);
@@ -354,22 +363,33 @@ int get_level_coeffs(icon_grid* g, int dtype, int nlev, const double* z_half, vo
         if ((rc = dev_alloc(g, abc.size(), &d))) return rc;
         CU_TRY(cudaMemcpy(d, abc.data(), abc.size() * 8, cudaMemcpyHostToDevice));
         lc.abc = d;
+        double* dw = nullptr;
+        if ((rc = dev_alloc(g, wk.size(), &dw))) return rc;
+        CU_TRY(cudaMemcpy(dw, wk.data(), wk.size() * 8, cudaMemcpyHostToDevice));
+        lc.wk = dw;
     } else {
         std::vector<float> f(abc.begin(), abc.end());
         float* d = nullptr;
         if ((rc = dev_alloc(g, f.size(), &d))) return rc;
         CU_TRY(cudaMemcpy(d, f.data(), f.size() * 4, cudaMemcpyHostToDevice));
         lc.abc = d;
+        std::vector<float> fw(wk.begin(), wk.end());
+        float* dw = nullptr;
+        if ((rc = dev_alloc(g, fw.size(), &dw))) return rc;
+        CU_TRY(cudaMemcpy(dw, fw.data(), fw.size() * 4, cudaMemcpyHostToDevice));
+        lc.wk = dw;
     }
     // the coefficients are cached per z_half and reused by later calls on ANY stream: the upload (legacy stream) must
     // have landed before this call's kernel, which may run on a non-blocking stream, reads them
     CU_TRY(cudaStreamSynchronize(cudaStreamLegacy));
     if (g->level_coeffs.size() >= 16) {   // bounded cache
         dev_release(g, g->level_coeffs.front().abc);
+        dev_release(g, g->level_coeffs.front().wk);
         g->level_coeffs.erase(g->level_coeffs.begin());
     }
     g->level_coeffs.push_back(lc);
     *out = lc.abc;
+    if (out_wk) *out_wk = lc.wk;
     return ICON_OK;
 }
 
@@ -515,6 +535,7 @@ int table_info(const icon_grid* g, int which, TableInfo* t) {
         case ICON_TAB_A_V: D(h.a_v, h.nv, 1); break;
         case ICON_TAB_GEOFAC_DIV: D(h.geofac_div, h.nc, 3); break;
         case ICON_TAB_GEOFAC_ROT: D(h.geofac_rot, h.nv, 6); break;
+        case ICON_TAB_ADV_C: D(h.adv_c, h.nc, 3); break;
         default: return fail(ICON_EINVAL, "unknown table selector");
     }
     return ICON_OK;
@@ -755,6 +776,34 @@ int dycore_velocity_tendencies(const icon_grid_t* gc, int dtype, int nlev, int l
     if (dtype == ICON_F64)
         return tendencies_impl<double>(g, g->c64, g->p64, g->s64, g->cc64, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, vt_opt, ke_c_opt, vort_opt, s);
     return tendencies_impl<float>(g, g->c32, g->p32, g->s32, g->cc32, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, vt_opt, ke_c_opt, vort_opt, s);
+}
+
+int dycore_w_tendency(const icon_grid_t* gc, int dtype, int nlev, int ldk, int ldk_w, const double* z_half, const void* vn,
+                      const void* w, void* ddt_w, void* cuda_stream) {
+    icon_grid* g = const_cast<icon_grid*>(gc);
+    int rc = check_common(g, dtype, nlev, ldk, 2);
+    if (rc) return rc;
+    const size_t es = dtype == ICON_F64 ? 8 : 4;
+    if (ldk_w < nlev + 1) return fail(ICON_EINVAL, "ldk_w < nlev + 1");
+    if (((int64_t)ldk_w * (int64_t)es) % 16) return fail(ICON_EINVAL, "ldk_w*sizeof(T) must be a multiple of 16");
+    if (!z_half) return fail(ICON_EINVAL, "z_half is NULL");
+    if ((rc = check_field(vn, "vn")) || (rc = check_field(w, "w")) || (rc = check_field(ddt_w, "ddt_w"))) return rc;
+    const size_t be = (size_t)g->host.ne * ldk * es, bw = (size_t)g->host.nc * ldk_w * es;
+    if (overlaps(ddt_w, bw, vn, be) || overlaps(ddt_w, bw, w, bw)) return fail(ICON_EINVAL, "outputs must not alias inputs");
+    void *abc = nullptr, *wk = nullptr;
+    if ((rc = get_level_coeffs(g, dtype, nlev, z_half, &abc, &wk))) return rc;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    int n;
+    if (dtype == ICON_F64) {
+        if ((rc = ensure_coeffs(g, g->c64))) return rc;
+        n = icon::launch_w_tendency<double>(*g, g->c64, nlev, ldk, ldk_w, (const double*)wk, (const double*)vn, (const double*)w, (double*)ddt_w, s);
+    } else {
+        if ((rc = ensure_coeffs(g, g->c32))) return rc;
+        n = icon::launch_w_tendency<float>(*g, g->c32, nlev, ldk, ldk_w, (const float*)wk, (const float*)vn, (const float*)w, (float*)ddt_w, s);
+    }
+    if (n < 0) return fail_cuda((cudaError_t)(-n), "kernel launch");
+    g->launches += n;
+    return ICON_OK;
 }
 
 int dycore_step(const icon_grid_t* gc, int dtype, int nlev, int ldk, int ldk_w, const double* z_half, const void* vn, const void* w,

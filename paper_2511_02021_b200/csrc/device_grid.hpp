@@ -26,6 +26,7 @@ struct DevCoeffs {
     T* inv_d_e = nullptr;     // [ne]
     T* f_e = nullptr;         // [ne]
     T* c_lin = nullptr;       // [ne][2]
+    T* adv_c = nullptr;       // [nc][3]
     bool ready = false;
 };
 
@@ -98,6 +99,7 @@ struct LevelCoeffs {
     std::vector<double> z_half;   // host key
     int dtype = 0;
     void* abc = nullptr;          // device [3][nlev] of T: A_k, B_k, C_k
+    void* wk = nullptr;           // device [2][nlev+1] of T: g_k of vn_ie(k), 1 / (z_half[k-1] - z_half[k+1]) (P-19)
 };
 
 struct Workspace {                // unfused pipeline intermediates, [n][ldk] of T

@@ -207,6 +207,7 @@ void build_geometry(HostGrid& g) {
     g.c_lin.resize(2 * (size_t)ne);
     g.rbf.resize(4 * (size_t)ne);
     g.bln.resize(3 * (size_t)nc);
+    g.adv_c.resize(3 * (size_t)nc);
     g.geofac_div.resize(3 * (size_t)nc);
     g.a_v.resize((size_t)nv);
     g.geofac_rot.resize(6 * (size_t)nv);
@@ -260,6 +261,21 @@ void build_geometry(HostGrid& g) {
         g.bln[3 * c] = w0 / s;
         g.bln[3 * c + 1] = w1 / s;
         g.bln[3 * c + 2] = w2 / s;
+        // P-19 normal-component reconstruction weights: sum_j a_j n_j n_j^T = I. With n_j = (cos t_j, sin t_j),
+        // n n^T = (I + R(2 t_j)) / 2, so the conditions are sum a_j = 2 and sum a_j z_j = 0 for the doubled-angle points
+        // z_j = (cos 2t_j, sin 2t_j): the barycentric weights of the origin in the triangle z_0 z_1 z_2, times 2.
+        double zx[3], zy[3];
+        for (int j = 0; j < 3; ++j) {
+            V3 n = ld3(g.edge_normal, g.c2e[3 * c + j]);
+            const double px = dot(n, e1), py = dot(n, e2), r2 = px * px + py * py;
+            zx[j] = (px * px - py * py) / r2;
+            zy[j] = 2.0 * px * py / r2;
+        }
+        const double b0 = zx[1] * zy[2] - zx[2] * zy[1], b1 = zx[2] * zy[0] - zx[0] * zy[2], b2 = zx[0] * zy[1] - zx[1] * zy[0];
+        const double bs = 0.5 * (b0 + b1 + b2);
+        g.adv_c[3 * c] = b0 / bs;
+        g.adv_c[3 * c + 1] = b1 / bs;
+        g.adv_c[3 * c + 2] = b2 / bs;
     }
     // P-8 dual areas, folded rotation factor
 #pragma omp parallel for schedule(static)

@@ -226,6 +226,52 @@ __global__ void __launch_bounds__(256) k_ddt_vn(int64_t ne, int nlev, int64_t ld
 }
 
 // ------------------------------------------------------------------------------------------
+// Vertical-wind tendency (reading P-19): one warp per cell column, lanes = half levels.
+//   ddt_w(c,k) = -[ sum_j adv_c(c,j) vn_ie(e_j,k) (w(c1_j,k) - w(c0_j,k)) inv_d_e(e_j) + w(c,k) (w(c,k-1) - w(c,k+1)) rdz2(k) ]
+// for k = 1 .. nlev-1, 0 at k = 0 and k = nlev. wk = [2][nlev+1]: g_k (weight of vn(k) in vn_ie(k), P-14) and
+// rdz2(k) = 1 / (z_half[k-1] - z_half[k+1]). Ids, cells and the folded coefficient adv_c * inv_d_e are warp-uniform.
+// ------------------------------------------------------------------------------------------
+template <class T>
+__global__ void __launch_bounds__(256) k_w_tend(int64_t nc, int nlev, int64_t ldk, int64_t ldk_w,
+                                                const int32_t* __restrict__ c2e, const int32_t* __restrict__ e2c,
+                                                const T* __restrict__ inv_d_e, const T* __restrict__ adv_c,
+                                                const int32_t* __restrict__ user_c, const int32_t* __restrict__ pos_e,
+                                                const T* __restrict__ wk, const T* __restrict__ vn, const T* __restrict__ w,
+                                                T* __restrict__ ddt_w) {
+    const int64_t p = (int64_t)blockIdx.x * 8 + warp_in_block();
+    if (p >= nc) return;
+    const int lane = lane_id();
+    const int64_t c = user_c ? user_c[p] : p;
+    const T *vcol[3], *w0[3], *w1[3];
+    T a[3];
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+        const int64_t e = ldg(c2e + 3 * p + j);
+        const int64_t pe = pos_e ? pos_e[e] : e;                 // row of the edge tables (work order)
+        vcol[j] = vn + e * ldk;
+        w0[j] = w + (int64_t)ldg(e2c + 2 * pe) * ldk_w;
+        w1[j] = w + (int64_t)ldg(e2c + 2 * pe + 1) * ldk_w;
+        a[j] = ldg(adv_c + 3 * p + j) * ldg(inv_d_e + pe);
+    }
+    const T* wc = w + c * ldk_w;
+    T* out = ddt_w + c * ldk_w;
+    for (int k = lane; k <= nlev; k += kWarp) {
+        T val = (T)0;
+        if (k >= 1 && k <= nlev - 1) {
+            const T g = ldg(wk + k), rdz2 = ldg(wk + nlev + 1 + k);
+            T hadv = (T)0;
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+                const T vie = g * vcol[j][k] + ((T)1 - g) * vcol[j][k - 1];
+                hadv += a[j] * vie * (w1[j][k] - w0[j][k]);
+            }
+            val = -(hadv + wc[k] * (wc[k - 1] - wc[k + 1]) * rdz2);
+        }
+        out[k] = val;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
 // fused gather kernel (variant 1): one warp per edge column, every intermediate recomputed in
 // registers from the 15-edge vn stencil; nothing but vn, w and the tables is read, nothing but
 // ddt_vn is written.
@@ -343,12 +389,24 @@ int launch_tendencies_fused(const icon_grid& g, const DevCoeffs<T>& c, int nlev,
     return err == cudaSuccess ? 1 : -(int)err;
 }
 
+template <class T>
+int launch_w_tendency(const icon_grid& g, const DevCoeffs<T>& c, int nlev, int64_t ldk, int64_t ldk_w, const T* wk,
+                      const T* vn, const T* w, T* ddt_w, cudaStream_t s) {
+    const int64_t nc = g.host.nc;
+    k_w_tend<T><<<blocks_for(nc, 8), 256, 0, s>>>(nc, nlev, ldk, ldk_w, g.tab.c2e, g.tab.e2c, c.inv_d_e, c.adv_c, g.tab.user_c,
+                                                  g.tab.pos_e, wk, vn, w, ddt_w);
+    cudaError_t err = cudaGetLastError();
+    return err == cudaSuccess ? 1 : -(int)err;
+}
+
 #define ICON_INSTANTIATE(T)                                                                                             \
     template int launch_div_vort<T>(const icon_grid&, const DevCoeffs<T>&, int, int64_t, const T*, T*, T*, cudaStream_t); \
     template int launch_tendencies_unfused<T>(const icon_grid&, const DevCoeffs<T>&, int, int64_t, int64_t, const T*,     \
                                               const T*, const T*, T*, T*, T*, T*, T*, cudaStream_t);                      \
     template int launch_tendencies_fused<T>(const icon_grid&, const DevCoeffs<T>&, int, int64_t, int64_t, const T*,       \
-                                            const T*, const T*, T*, T*, T*, T*, cudaStream_t);
+                                            const T*, const T*, T*, T*, T*, T*, cudaStream_t);                            \
+    template int launch_w_tendency<T>(const icon_grid&, const DevCoeffs<T>&, int, int64_t, int64_t, const T*, const T*,   \
+                                      const T*, T*, cudaStream_t);
 ICON_INSTANTIATE(double)
 ICON_INSTANTIATE(float)
 

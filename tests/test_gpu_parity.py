@@ -359,6 +359,42 @@ def test_dycore_step_replays_in_a_cuda_graph(torch_cuda, lib, oracle_grid, k, pe
         g.set_option(lib.ICON_OPT_CC_PACE, 512)
 
 
+# ----------------------------------------------------------------------------------------------
+# vertical-wind tendency (reading P-19)
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("k,seed,flags,nlev,ldk,ldk_w,dtype", [
+    (4, 0, 0, 90, 90, 92, "f64"), (4, 0, 0, 90, 96, 96, "f64"), (3, si.PERMUTE_SEED, 1, 40, 40, 42, "f64"),
+    (3, si.PERMUTE_SEED, 1 | 8, 40, 40, 42, "f64"), (4, si.PERMUTE_SEED, 1, 90, 92, 92, "f32"), (0, 0, 0, 2, 2, 4, "f64"),
+    (0, 0, 0, 3, 4, 4, "f64"), (1, 0, 0, 31, 32, 32, "f64"), (1, 0, 0, 33, 34, 34, "f64"), (2, 0, 0, 130, 130, 132, "f64")])
+def test_w_tendency_elementwise(torch_cuda, lib, oracle_mod, oracle_grid, k, seed, flags, nlev, ldk, ldk_w, dtype):
+    """dycore_w_tendency against og_w_tendency, every half level of every cell; pads stay untouched; also with the
+    oracle evaluating on the LIBRARY's exported tables (P-18)"""
+    torch = torch_cuda
+    og = oracle_grid(k, seed, flags & 1)
+    g = lib_grid(lib, k, seed, flags)
+    f32 = dtype == "f32"
+    vn, w, zh = si.make_fields(4 if flags & 1 else 1, og.edge_xyz, og.edge_normal, og.nc, nlev=nlev, ldk=ldk, ldk_w=ldk_w, dtype=dtype)
+    o = og.rounded_f32() if f32 else og
+    vn64, w64 = np.nan_to_num(vn.astype(np.float64)), np.nan_to_num(w.astype(np.float64))
+    want, m = o.w_tendency(vn64, w64, zh, nlev, with_scale=True)
+    dev = torch.device("cuda:0")
+    sentinel = -9.25
+    out = torch.full((g.nc, ldk_w), sentinel, dtype=torch.from_numpy(w).dtype, device=dev)
+    n0 = g.launch_count
+    lib.dycore_w_tendency(g, zh, torch.from_numpy(vn).to(dev), torch.from_numpy(w).to(dev), out, nlev)
+    torch.cuda.synchronize()
+    assert g.launch_count - n0 == 1
+    got = out.cpu().numpy().astype(np.float64)
+    err = np.abs(got[:, :nlev + 1] - want[:, :nlev + 1])
+    assert (err <= TOL[dtype] * m[:, :nlev + 1]).all(), "worst err/M %.3e" % (err / np.maximum(m[:, :nlev + 1], 1e-300)).max()
+    assert (got[:, 0] == 0).all() and (got[:, nlev] == 0).all()
+    assert (got[:, nlev + 1:] == sentinel).all()
+    if not f32:
+        t = {n: g.table_host(n) for n in ("c2e", "e2c", "inv_d_e", "adv_c")}
+        want2, m2 = oracle_mod.w_tendency_from_arrays(t, vn64, w64, zh, nlev)
+        assert (np.abs(got[:, :nlev + 1] - want2[:, :nlev + 1]) <= TOL[dtype] * m2[:, :nlev + 1]).all()
+
+
 def test_argument_errors_on_device(torch_cuda, lib):
     torch = torch_cuda
     g = lib_grid(lib, 1)
@@ -516,4 +552,16 @@ def test_full_size_sampled(torch_cuda, lib, oracle_mod, config, host_gb):
     lib.dycore_div_vort(g, d_vn, outs[1], outs[2], nlev)
     torch.cuda.synchronize()
     _sampled_check(torch, o, "two calls", config, outs, sizes, nlev, as64(vn), as64(w), zh, tol, nsamp, 300 + config)
+    # ---- leg C: the vertical-wind tendency on the same fields ----------------------------
+    ddt_w = torch.full((g.nc, ldk_w), float("nan"), dtype=d_vn.dtype, device=dev)
+    lib.dycore_w_tendency(g, zh, d_vn, d_w, ddt_w, nlev)
+    torch.cuda.synchronize()
+    idx, lev = si.sample_points(500 + config, g.nc, nlev + 1, nsamp)
+    got = ddt_w[torch.from_numpy(idx).to(dev), torch.from_numpy(lev.astype(np.int64)).to(dev)].cpu().numpy().astype(np.float64)
+    want, m = o.sample("ddt_w", idx, lev, as64(vn), nlev, w=as64(w), z_half=zh)
+    err = np.abs(got - want)
+    assert (err <= tol * m).all(), "ddt_w config %d: worst err/M %.3e" % (config, (err / np.maximum(m, 1e-300)).max())
+    assert not torch.isnan(ddt_w[:, :nlev + 1]).any()
+    if ldk_w > nlev + 1:
+        assert torch.isnan(ddt_w[:, nlev + 1:]).all()
     g.close()
