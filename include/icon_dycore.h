@@ -54,7 +54,7 @@ enum {
     ICON_PERMUTE = 1u,            /* seeded random renumbering of cells/edges/vertices (P-7, config 4) */
     ICON_LOCALITY_WORKLIST = 2u,  /* internal tables laid out in generation (spatially local) order and
                                      kernels walk that order; results are identical. Implied by
-                                     ICON_PERMUTE unless ICON_NO_WORKLIST is given. */
+                                     ICON_PERMUTE unless ICON_NO_WORKLIST is given (accepted, has no further effect). */
     ICON_HOST_ONLY = 4u,          /* build host tables only; no CUDA device is touched (table tests) */
     ICON_NO_WORKLIST = 8u         /* with ICON_PERMUTE: walk the permuted ids directly (ablation) */
 };
@@ -136,19 +136,6 @@ int icon_grid_table_host(const icon_grid_t* g, int which, const void** ptr, int*
 int icon_grid_table_device(const icon_grid_t* g, int which, int dtype, const void** dptr);
 
 int icon_grid_set_option(icon_grid_t* g, int option, int value);
-
-/*
- * icon_grid_worklist_stats -- builds (once, on the host; works on ICON_HOST_ONLY grids) the tile /
- * patch work-list the fused kernels walk (SURVEY.md 8(a) G3 "optional internal work-list ordering";
- * the index-lookup amortisation of PAPER.md:186) and reports its shape:
- *   out[0] patches (= nc/4)   out[1] tiles (16 patches = 64 cells each)
- *   out[2] halo-cell tasks    out[3] corner-vertex tasks (summed over tiles)
- *   out[4] largest halo count of a tile   out[5] largest vertex count of a tile
- *   out[6] midpoint vertices stored by patches   out[7] corner vertices stored by tiles
- * (out[6] + out[7] == nv: every vertex is written exactly once by the div/vort kernel).
- * ICON_EUNSUPPORTED if the tables do not describe a 4-child bisection hierarchy.
- */
-int icon_grid_worklist_stats(const icon_grid_t* g, int64_t out[8]);
 
 /*
  * icon_grid_cc_schedule_check -- builds on the host (works on ICON_HOST_ONLY grids) the column-cache

@@ -28,7 +28,7 @@ TABLE_ID = {n: i for i, n in enumerate(TABLES)}
 
 # every symbol include/icon_dycore.h declares
 EXPORTS = ("icon_grid_create", "icon_grid_destroy", "icon_grid_counts", "icon_grid_table_host",
-           "icon_grid_table_device", "icon_grid_set_option", "icon_grid_worklist_stats", "icon_grid_cc_schedule_check", "dycore_div_vort", "dycore_velocity_tendencies",
+           "icon_grid_table_device", "icon_grid_set_option", "icon_grid_cc_schedule_check", "dycore_div_vort", "dycore_velocity_tendencies",
            "dycore_step", "dycore_step_host", "dycore_w_tendency", "icon_grid_launch_count", "icon_last_error")
 
 
@@ -63,8 +63,6 @@ def load_library():
     L.icon_grid_table_device.argtypes = [P, ci, ci, ctypes.POINTER(P)]
     L.icon_grid_set_option.restype = ci
     L.icon_grid_set_option.argtypes = [P, ci, ci]
-    L.icon_grid_worklist_stats.restype = ci
-    L.icon_grid_worklist_stats.argtypes = [P, ctypes.POINTER(i64)]
     L.icon_grid_cc_schedule_check.restype = ci
     L.icon_grid_cc_schedule_check.argtypes = [P, ci, ci, ci, ci, ci, ci, ctypes.POINTER(i64)]
     L.icon_grid_launch_count.restype = i64
@@ -153,13 +151,6 @@ class IconGrid:
 
     def set_option(self, option, value):
         _check(self._L.icon_grid_set_option(self._h, option, value))
-
-    def worklist_stats(self):
-        """shape of the tile / patch work-list of the fused kernels (icon_grid_worklist_stats)"""
-        out = (ctypes.c_int64 * 8)()
-        _check(self._L.icon_grid_worklist_stats(self._h, out))
-        keys = ("patches", "tiles", "halo_tasks", "vertex_tasks", "max_halo", "max_vert", "mid_stored", "corner_stored")
-        return dict(zip(keys, [int(x) for x in out]))
 
     def cc_schedule_check(self, dtype, nlev, ldk, ldk_w, n_ctas=148, smem_bytes=232448):
         """build + independently validate the column-cache schedule of tendency kernel 4 (icon_grid_cc_schedule_check)"""

@@ -142,43 +142,6 @@ int upload_vec(icon_grid* g, const std::vector<S>& src, D** out) {
     return ICON_OK;
 }
 
-int ensure_patch_host(icon_grid* g) {
-    if (g->patch_host_ready) return ICON_OK;
-    std::string err;
-    try {
-        err = icon::build_patch_tables(g->host, g->patch_host);
-    } catch (const std::bad_alloc&) {
-        return fail(ICON_ENOMEM, "out of host memory while building the patch tables");
-    }
-    if (!err.empty()) return fail(ICON_EUNSUPPORTED, err);
-    g->patch_host_ready = true;
-    return ICON_OK;
-}
-
-// tile / patch work-list of the fused kernels: built on the host once, uploaded once per dtype
-template <class T>
-int ensure_patch_tables(icon_grid* g, icon::DevPatchTables<T>& p) {
-    if (p.ready) return ICON_OK;
-    int rc0 = ensure_patch_host(g);
-    if (rc0) return rc0;
-    const icon::PatchTables& h = g->patch_host;
-    int rc;
-    if ((rc = upload_vec(g, h.patch_ids, &p.patch_ids))) return rc;
-    if ((rc = upload_vec(g, h.patch_coef, &p.patch_coef))) return rc;
-    if ((rc = upload_vec(g, h.tile_hdr, &p.tile_hdr))) return rc;
-    if ((rc = upload_vec(g, h.halo_ids, &p.halo_ids))) return rc;
-    if ((rc = upload_vec(g, h.halo_coef, &p.halo_coef))) return rc;
-    if ((rc = upload_vec(g, h.vert_ids, &p.vert_ids))) return rc;
-    if ((rc = upload_vec(g, h.vert_coef, &p.vert_coef))) return rc;
-    if ((rc = upload_vec(g, h.vert_store, &p.vert_store))) return rc;
-    if ((rc = upload_vec(g, h.mid_store, &p.mid_store))) return rc;
-    if ((rc = upload_vec(g, h.mid_vertex, &p.mid_vertex))) return rc;
-    p.n_patches = h.n_patches; p.n_tiles = h.n_tiles; p.max_halo = h.max_halo; p.max_vert = h.max_vert;
-    CU_TRY(cudaStreamSynchronize(cudaStreamLegacy));
-    p.ready = true;
-    return ICON_OK;
-}
-
 int ensure_sc_host(icon_grid* g);
 
 template <class T>
@@ -443,8 +406,7 @@ int ensure_workspace(icon_grid* g, int dtype, int64_t ldk) {
 }
 
 template <class T>
-int tendencies_impl(icon_grid* g, icon::DevCoeffs<T>& c, icon::DevPatchTables<T>& pt, icon::DevScTables<T>& st,
-                    icon::DevCcTables<T>& ct, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
+int tendencies_impl(icon_grid* g, icon::DevCoeffs<T>& c, icon::DevScTables<T>& st, icon::DevCcTables<T>& ct, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
                     const void* vn, const void* w, void* ddt_vn, void* vt_opt, void* ke_c_opt, void* vort_opt,
                     cudaStream_t s, void* div_fused = nullptr, void* vort_fused = nullptr, bool* fused_done = nullptr) {
     // div_fused / vort_fused: dycore_step asks for S1 + S2 from the same pass; only the column-cache kernel can
@@ -456,17 +418,10 @@ int tendencies_impl(icon_grid* g, icon::DevCoeffs<T>& c, icon::DevPatchTables<T>
     const bool want_opt = vt_opt || ke_c_opt || vort_opt;
     int n;
     int variant = g->options[ICON_OPT_TENDENCY_KERNEL];
-    if (variant == 5) {
-        // auto, from the measurements on B200: the column cache wins where a lane owns
-        // three levels of 8-byte columns (33 <= nlev+1 <= 96, fp64); shallow columns are copy-request bound
-        // there and go to the exchange patch kernel, 4-byte columns to the self-contained patch kernel
-        variant = nlev + 1 <= 32 ? 2 : (sizeof(T) == 8 && icon::cc_levels_per_lane(nlev) == 3) ? 4 : 3;
-        // dycore_step: the fused column-cache pass beats tendency kernel + div_vort kernel in every measured regime
-        if (div_fused && icon::cc_levels_per_lane(nlev) != 0) variant = 4;
-    }
+    if (variant == 5) variant = 4;            // auto: the column cache wherever it can hold the columns (nlev <= 95)
     if (variant == 4 && !want_opt) {
         if ((rc = ensure_cc_tables(g, ct, nlev, ldk, ldk_w))) return rc;
-        if (ct.unsupported) variant = 3;      // level count / dtype the column cache cannot hold
+        if (ct.unsupported) variant = 3;      // level count the column cache cannot hold
     }
     if (variant != 4 || want_opt) div_fused = vort_fused = nullptr;
     if (fused_done) *fused_done = div_fused != nullptr;
@@ -481,17 +436,10 @@ int tendencies_impl(icon_grid* g, icon::DevCoeffs<T>& c, icon::DevPatchTables<T>
         T* vo = vort_opt ? (T*)vort_opt : (T*)g->ws.vort;
         n = icon::launch_tendencies_unfused<T>(*g, c, nlev, ldk, ldk_w, (const T*)abc, (const T*)vn, (const T*)w,
                                                (T*)ddt_vn, vt, (T*)g->ws.ke_e, kc, vo, s);
-    } else if (variant == 1) {
-        n = icon::launch_tendencies_fused<T>(*g, c, nlev, ldk, ldk_w, (const T*)abc, (const T*)vn, (const T*)w,
-                                             (T*)ddt_vn, nullptr, nullptr, nullptr, s);
-    } else if (variant == 3) {
+    } else {
         if ((rc = ensure_sc_tables(g, st))) return rc;
         n = icon::launch_tendencies_sc<T>(*g, st, nlev, ldk, ldk_w, (const T*)abc, (const T*)vn, (const T*)w,
                                           (T*)ddt_vn, s);
-    } else {
-        if ((rc = ensure_patch_tables(g, pt))) return rc;
-        n = icon::launch_tendencies_patch<T>(*g, pt, nlev, ldk, ldk_w, (const T*)abc, (const T*)vn, (const T*)w,
-                                             (T*)ddt_vn, s);
     }
     if (n < 0) return fail_cuda((cudaError_t)(-n), "kernel launch");
     g->launches += n;
@@ -668,32 +616,12 @@ int icon_grid_set_option(icon_grid_t* g, int option, int value) {
     if (option < 0 || option >= ICON_OPT_COUNT) return fail(ICON_EINVAL, "unknown option");
     if (option == ICON_OPT_CC_PACE && (value < 0 || value > 65536 || (value & (value - 1)))) return fail(ICON_EINVAL, "bad option value");
     if (option == ICON_OPT_CC_TILE && (value < 0 || value > 4096 || value % icon::kCcGroup)) return fail(ICON_EINVAL, "bad option value");
-    if (option == ICON_OPT_TENDENCY_KERNEL && (value < 0 || value > 5)) return fail(ICON_EINVAL, "bad option value");
+    if (option == ICON_OPT_TENDENCY_KERNEL && value != 0 && value != 3 && value != 4 && value != 5) return fail(ICON_EINVAL, "bad option value");
     g->options[option] = value;
     return ICON_OK;
 }
 
 int64_t icon_grid_launch_count(const icon_grid_t* g) { return g ? g->launches : 0; }
-
-int icon_grid_worklist_stats(const icon_grid_t* gc, int64_t out[8]) {
-    icon_grid* g = const_cast<icon_grid*>(gc);
-    if (!g || !out) return fail(ICON_EINVAL, "NULL argument");
-    int rc = ensure_patch_host(g);
-    if (rc) return rc;
-    const icon::PatchTables& h = g->patch_host;
-    out[0] = h.n_patches;
-    out[1] = h.n_tiles;
-    out[2] = (int64_t)(h.halo_ids.size() / icon::kHaloIdWords);
-    out[3] = (int64_t)(h.vert_ids.size() / icon::kVertIdWords);
-    out[4] = h.max_halo;
-    out[5] = h.max_vert;
-    int64_t mids = 0, cors = 0;
-    for (int32_t m : h.mid_store) mids += (m & 1) + ((m >> 1) & 1) + ((m >> 2) & 1);
-    for (int32_t v : h.vert_store) cors += v;
-    out[6] = mids;
-    out[7] = cors;
-    return ICON_OK;
-}
 
 int icon_grid_cc_schedule_check(const icon_grid_t* gc, int dtype, int nlev, int ldk, int ldk_w, int n_ctas, int smem_bytes,
                                 int64_t out[8]) {
@@ -774,8 +702,8 @@ int dycore_velocity_tendencies(const icon_grid_t* gc, int dtype, int nlev, int l
     }
     cudaStream_t s = (cudaStream_t)cuda_stream;
     if (dtype == ICON_F64)
-        return tendencies_impl<double>(g, g->c64, g->p64, g->s64, g->cc64, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, vt_opt, ke_c_opt, vort_opt, s);
-    return tendencies_impl<float>(g, g->c32, g->p32, g->s32, g->cc32, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, vt_opt, ke_c_opt, vort_opt, s);
+        return tendencies_impl<double>(g, g->c64, g->s64, g->cc64, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, vt_opt, ke_c_opt, vort_opt, s);
+    return tendencies_impl<float>(g, g->c32, g->s32, g->cc32, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, vt_opt, ke_c_opt, vort_opt, s);
 }
 
 int dycore_w_tendency(const icon_grid_t* gc, int dtype, int nlev, int ldk, int ldk_w, const double* z_half, const void* vn,
@@ -833,10 +761,10 @@ int dycore_step(const icon_grid_t* gc, int dtype, int nlev, int ldk, int ldk_w, 
     cudaStream_t s = (cudaStream_t)cuda_stream;
     bool fused = false;
     if (dtype == ICON_F64)
-        rc = tendencies_impl<double>(g, g->c64, g->p64, g->s64, g->cc64, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, nullptr,
+        rc = tendencies_impl<double>(g, g->c64, g->s64, g->cc64, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, nullptr,
                                      nullptr, nullptr, s, div, vort, &fused);
     else
-        rc = tendencies_impl<float>(g, g->c32, g->p32, g->s32, g->cc32, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, nullptr,
+        rc = tendencies_impl<float>(g, g->c32, g->s32, g->cc32, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, nullptr,
                                     nullptr, nullptr, s, div, vort, &fused);
     if (rc || fused) return rc;
     return dycore_div_vort(g, dtype, nlev, ldk, vn, div, vort, cuda_stream);

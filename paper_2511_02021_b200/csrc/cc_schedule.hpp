@@ -95,7 +95,7 @@ struct CcSchedule {
     std::vector<CcStep> steps;
     std::vector<CcLoad> loads;
     std::vector<uint16_t> patch_slots;       // [work position][kCcSlotWords], slot index
-    // statistics (icon_grid_worklist_stats, tests)
+    // statistics (icon_grid_cc_schedule_check, tests)
     int64_t n_sync_steps = 0, n_vn_loads = 0, n_w_loads = 0;   // columns loaded
     int64_t n_copies = 0;                                      // bulk copies (runs)
 };

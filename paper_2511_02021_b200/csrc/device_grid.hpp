@@ -8,7 +8,6 @@
 #include <vector>
 
 #include "host_grid.hpp"
-#include "patch_tables.hpp"
 #include "sc_tables.hpp"
 #include "cc_schedule.hpp"
 
@@ -44,25 +43,6 @@ struct DevTables {
     int32_t* pos_c = nullptr;
     int32_t* pos_e = nullptr;
     int32_t* pos_v = nullptr;
-};
-
-// Device copy of the tile / patch work-list of the fused kernels (patch_tables.hpp), coefficient
-// words in T.
-template <class T>
-struct DevPatchTables {
-    int32_t* patch_ids = nullptr;
-    T* patch_coef = nullptr;
-    int32_t* tile_hdr = nullptr;
-    int32_t* halo_ids = nullptr;
-    T* halo_coef = nullptr;
-    int32_t* vert_ids = nullptr;
-    T* vert_coef = nullptr;
-    int32_t* vert_store = nullptr;
-    int32_t* mid_store = nullptr;
-    int32_t* mid_vertex = nullptr;
-    int64_t n_patches = 0, n_tiles = 0;
-    int max_halo = 0, max_vert = 0;
-    bool ready = false;
 };
 
 // Device copy of the self-contained patch records (sc_tables.hpp), coefficient words in T.
@@ -128,10 +108,6 @@ struct icon_grid {
     icon::DevTables tab;
     icon::DevCoeffs<double> c64;
     icon::DevCoeffs<float> c32;
-    icon::PatchTables patch_host;                      // built on first use of a fused kernel
-    bool patch_host_ready = false;
-    icon::DevPatchTables<double> p64;
-    icon::DevPatchTables<float> p32;
     icon::ScTables sc_host;                            // built on first use of the self-contained kernel
     bool sc_host_ready = false;
     icon::DevScTables<double> s64;

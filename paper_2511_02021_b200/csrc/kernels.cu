@@ -271,69 +271,6 @@ __global__ void __launch_bounds__(256) k_w_tend(int64_t nc, int nlev, int64_t ld
     }
 }
 
-// ------------------------------------------------------------------------------------------
-// fused gather kernel (variant 1): one warp per edge column, every intermediate recomputed in
-// registers from the 15-edge vn stencil; nothing but vn, w and the tables is read, nothing but
-// ddt_vn is written.
-// ------------------------------------------------------------------------------------------
-template <class T>
-__global__ void __launch_bounds__(256) k_tend_gather(int64_t ne, int nlev, int64_t ldk, int64_t ldk_w,
-                                                     const int32_t* __restrict__ c2e, const int32_t* __restrict__ e2c,
-                                                     const int32_t* __restrict__ e2v, const int32_t* __restrict__ e2e4,
-                                                     const int32_t* __restrict__ v2e, const T* __restrict__ rbf,
-                                                     const T* __restrict__ bln, const T* __restrict__ geofac_rot,
-                                                     const T* __restrict__ inv_d_e, const T* __restrict__ f_e,
-                                                     const T* __restrict__ c_lin, const int32_t* __restrict__ user_e,
-                                                     const int32_t* __restrict__ pos_e, const int32_t* __restrict__ pos_c,
-                                                     const int32_t* __restrict__ pos_v, const T* __restrict__ abc,
-                                                     const T* __restrict__ vn, const T* __restrict__ w,
-                                                     T* __restrict__ ddt_vn) {
-    const int64_t p = (int64_t)blockIdx.x * 8 + warp_in_block();
-    if (p >= ne) return;
-    const int lane = lane_id();
-    const int64_t e = user_e ? user_e[p] : p;
-    const int64_t c[2] = {ldg(e2c + 2 * p), ldg(e2c + 2 * p + 1)};
-    const int64_t v[2] = {ldg(e2v + 2 * p), ldg(e2v + 2 * p + 1)};
-    const T inv_d = ldg(inv_d_e + p), f = ldg(f_e + p), cl0 = ldg(c_lin + 2 * p), cl1 = ldg(c_lin + 2 * p + 1);
-    const T* col = vn + e * ldk;
-    for (int k = lane; k < nlev; k += kWarp) {
-        // KE at the two cells: each from its three edges, each edge's vt from its four neighbours
-        T kec[2];
-#pragma unroll
-        for (int s = 0; s < 2; ++s) {
-            const int64_t pc = pos_c ? pos_c[c[s]] : c[s];
-            T acc = (T)0;
-#pragma unroll
-            for (int j = 0; j < 3; ++j) {
-                const int64_t ej = ldg(c2e + 3 * pc + j);
-                const int64_t pj = pos_e ? pos_e[ej] : ej;
-                T t = (T)0;
-#pragma unroll
-                for (int q = 0; q < 4; ++q) t += ldg(rbf + 4 * pj + q) * vn[(int64_t)ldg(e2e4 + 4 * pj + q) * ldk + k];
-                const T n = vn[ej * ldk + k];
-                acc += ldg(bln + 3 * pc + j) * ((T)0.5 * (n * n + t * t));
-            }
-            kec[s] = acc;
-        }
-        T zeta[2];
-#pragma unroll
-        for (int s = 0; s < 2; ++s) {
-            const int64_t pv = pos_v ? pos_v[v[s]] : v[s];
-            T acc = (T)0;
-#pragma unroll
-            for (int j = 0; j < 6; ++j) acc += ldg(geofac_rot + 6 * pv + j) * vn[(int64_t)ldg(v2e + 6 * pv + j) * ldk + k];
-            zeta[s] = acc;
-        }
-        T vt = (T)0;
-#pragma unroll
-        for (int q = 0; q < 4; ++q) vt += ldg(rbf + 4 * p + q) * vn[(int64_t)ldg(e2e4 + 4 * p + q) * ldk + k];
-        T H = (kec[1] - kec[0]) * inv_d + vt * (f + (T)0.5 * (zeta[0] + zeta[1]));
-        T wf0 = (T)0.5 * (w[c[0] * ldk_w + k] + w[c[0] * ldk_w + k + 1]);
-        T wf1 = (T)0.5 * (w[c[1] * ldk_w + k] + w[c[1] * ldk_w + k + 1]);
-        ddt_vn[e * ldk + k] = -(H + (cl0 * wf0 + cl1 * wf1) * vertical_diff(col, abc, nlev, k));
-    }
-}
-
 inline unsigned blocks_for(int64_t n, int per_block) { return (unsigned)((n + per_block - 1) / per_block); }
 
 }  // namespace
@@ -378,18 +315,6 @@ int launch_tendencies_unfused(const icon_grid& g, const DevCoeffs<T>& c, int nle
 }
 
 template <class T>
-int launch_tendencies_fused(const icon_grid& g, const DevCoeffs<T>& c, int nlev, int64_t ldk, int64_t ldk_w,
-                            const T* abc, const T* vn, const T* w, T* ddt_vn, T*, T*, T*, cudaStream_t s) {
-    const int64_t ne = g.host.ne;
-    k_tend_gather<T><<<blocks_for(ne, 8), 256, 0, s>>>(ne, nlev, ldk, ldk_w, g.tab.c2e, g.tab.e2c, g.tab.e2v, g.tab.e2e4,
-                                                       g.tab.v2e, c.rbf, c.bln, c.geofac_rot, c.inv_d_e, c.f_e, c.c_lin,
-                                                       g.tab.user_e, g.tab.pos_e, g.tab.pos_c, g.tab.pos_v, abc, vn, w,
-                                                       ddt_vn);
-    cudaError_t err = cudaGetLastError();
-    return err == cudaSuccess ? 1 : -(int)err;
-}
-
-template <class T>
 int launch_w_tendency(const icon_grid& g, const DevCoeffs<T>& c, int nlev, int64_t ldk, int64_t ldk_w, const T* wk,
                       const T* vn, const T* w, T* ddt_w, cudaStream_t s) {
     const int64_t nc = g.host.nc;
@@ -403,8 +328,6 @@ int launch_w_tendency(const icon_grid& g, const DevCoeffs<T>& c, int nlev, int64
     template int launch_div_vort<T>(const icon_grid&, const DevCoeffs<T>&, int, int64_t, const T*, T*, T*, cudaStream_t); \
     template int launch_tendencies_unfused<T>(const icon_grid&, const DevCoeffs<T>&, int, int64_t, int64_t, const T*,     \
                                               const T*, const T*, T*, T*, T*, T*, T*, cudaStream_t);                      \
-    template int launch_tendencies_fused<T>(const icon_grid&, const DevCoeffs<T>&, int, int64_t, int64_t, const T*,       \
-                                            const T*, const T*, T*, T*, T*, T*, cudaStream_t);                            \
     template int launch_w_tendency<T>(const icon_grid&, const DevCoeffs<T>&, int, int64_t, int64_t, const T*, const T*,   \
                                       const T*, T*, cudaStream_t);
 ICON_INSTANTIATE(double)

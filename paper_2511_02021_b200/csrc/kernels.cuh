@@ -20,22 +20,10 @@ int launch_tendencies_unfused(const icon_grid& g, const DevCoeffs<T>& c, int nle
                               const T* abc, const T* vn, const T* w, T* ddt_vn, T* vt, T* ke_e, T* ke_c, T* vort,
                               cudaStream_t s);
 
-// S3-S7, fused gather kernel: every intermediate stays on chip.
-template <class T>
-int launch_tendencies_fused(const icon_grid& g, const DevCoeffs<T>& c, int nlev, int64_t ldk, int64_t ldk_w,
-                            const T* abc, const T* vn, const T* w, T* ddt_vn, T* vt_opt, T* ke_c_opt, T* vort_opt,
-                            cudaStream_t s);
-
 // Vertical-wind tendency (reading P-19): wk = device [2][nlev+1], g_k and 1 / (z_half[k-1] - z_half[k+1]).
 template <class T>
 int launch_w_tendency(const icon_grid& g, const DevCoeffs<T>& c, int nlev, int64_t ldk, int64_t ldk_w, const T* wk,
                       const T* vn, const T* w, T* ddt_w, cudaStream_t s);
-
-// S2-S7, fused register-resident patch kernel (kernels_patch.cu): persistent CTAs walk the tile
-// work-list; reads vn, w and the tables, writes ddt_vn only.
-template <class T>
-int launch_tendencies_patch(const icon_grid& g, const DevPatchTables<T>& p, int nlev, int64_t ldk, int64_t ldk_w,
-                            const T* abc, const T* vn, const T* w, T* ddt_vn, cudaStream_t s);
 
 // S2-S7, self-contained patch kernel (kernels_sc.cu): one warp per patch, all level chunks of a
 // column in flight at once, no exchange between warps; reads vn, w and the records, writes ddt_vn.

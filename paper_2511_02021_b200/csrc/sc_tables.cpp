@@ -144,7 +144,7 @@ std::string build_sc_tables(const HostGrid& g, ScTables& t) {
         }
         for (int j = 0; j < 4; ++j) id[SID_T0 + j] = L.T[j];
         bool ok = true;
-        // nine tangential-wind stencils of the patch (neighbour order of patch_tables.cpp)
+        // nine tangential-wind stencils of the patch (fixed neighbour order, see build_sc_tables)
         const int32_t nb[9][4] = {
             {B[0], B[5], I[1], I[2]}, {B[1], B[2], I[2], I[0]}, {B[3], B[4], I[0], I[1]},
             {I[0], B[5], M[0], O[0]}, {B[2], I[1], M[1], O[1]}, {B[1], I[1], M[2], O[2]},

@@ -1,9 +1,10 @@
-// sc_tables.hpp -- work-list of the SELF-CONTAINED patch kernel (kernels_sc.cu; internal header).
+// sc_tables.hpp -- patch records, the work-list of the column-cache kernel (kernels_cc.cu) and of the
+// self-contained patch kernel (kernels_sc.cu); internal header.
 //
-// Same patch as patch_tables.hpp (four sibling cells T0..T3 of the generation order, interior
-// edges i0..i2, boundary edges b0..b5, outer cells X0..X5 with their edges om_j / oc_j), but a
-// patch record now carries everything its six owned edges (i0 i1 i2 b0 b2 b4) need, so one warp
-// finishes a patch without exchanging anything with other warps:
+// The grid is a recursive bisection, so the four sibling cells T0..T3 of the generation order always form one
+// PATCH with a fixed local topology: interior edges i0..i2, boundary edges b0..b5, outer cells X0..X5 with
+// their edges om_j / oc_j. A patch record carries everything its six owned edges (i0 i1 i2 b0 b2 b4) need, so one
+// warp finishes a patch without exchanging anything with other warps:
 //
 //   for each owned boundary edge b_j (j = 0, 2, 4; x = j/2) with outer cell X_j and corner vertex
 //   C_x (a, b, c):
@@ -43,7 +44,7 @@ enum {                // id slots
     SID_V0 = 44       // vertices ab bc ca a b c whose vorticity THIS patch stores (fused step), -1 = another patch does
 };
 enum {                // coefficient slots
-    SCF_RBF = 0,      // [9][4] i0 i1 i2 b0..b5, neighbour order of patch_tables.cpp
+    SCF_RBF = 0,      // [9][4] i0 i1 i2 b0..b5, fixed neighbour order, see build_sc_tables
     SCF_BLN = 36,     // [4][3] T0..T3 (x 1/2)
     SCF_ROT = 48,     // [3][6] midpoints ab bc ca (x 1/2)
     SCF_EDGE = 68,    // [6][4] owned i0 i1 i2 b0 b2 b4: s_inv_d, f_e, c_lin(L), c_lin(H)

@@ -87,18 +87,13 @@ def test_create_without_device_fails_loudly(L):
 
 @pytest.mark.parametrize("k,seed,flags", [(0, 0, 0), (1, 0, 0), (2, 0, 0), (3, 0, 0), (5, 0, 0), (6, 0, 0),
                                           (2, 4, 1), (4, 4, 1)])
-def test_worklist_covers_the_grid(L, k, seed, flags):
-    """host logic of the fused kernels: every patch passes the local-topology checks (canonical and
-    permuted ids), tiles are 16 patches, every vertex is stored exactly once by the div/vort walk"""
+def test_patch_records_cover_the_grid(L, k, seed, flags):
+    """host logic of the fused kernel (the internal work-list): every group of four sibling cells
+    passes the local-topology checks of csrc/sc_tables.cpp (canonical and permuted ids; a grid that is not a 4-child
+    bisection hierarchy, or a vertex no patch owns, is an error there), and the schedule built on the records replays"""
     g = lib.IconGrid(k, seed, flags | lib.ICON_HOST_ONLY)
-    s = g.worklist_stats()
-    assert s["patches"] == g.nc // 4
-    assert s["tiles"] == -(-s["patches"] // 16)
-    assert s["mid_stored"] + s["corner_stored"] == g.nv
-    assert s["corner_stored"] == g.nc // 8 + 2            # vertices of the parent grid: nc_parent/2 + 2
-    if k >= 2:                                            # a tile is one triangle three levels up
-        assert s["max_halo"] == 12 and s["max_vert"] == 15
-        assert s["halo_tasks"] == 12 * s["tiles"] and s["vertex_tasks"] == 15 * s["tiles"]
+    st = g.cc_schedule_check(0, 90, 96, 96)
+    assert st["steps"] >= -(-(g.nc // 4) // 4) and st["ctas"] >= 1
     g.close()
 
 
