@@ -173,10 +173,10 @@ int ensure_sc_host(icon_grid* g) {
 // A slot as large as the caller's column stride lets runs of consecutive columns arrive as one bulk
 // copy (the copy engine, not HBM, limits small copies); taken when it costs < 128 bytes per slot.
 template <class T>
-icon::CcGeometry cc_geometry(int nlev, int64_t ldk, int64_t ldk_w) {
+icon::CcGeometry cc_geometry(int nlev, int64_t ldk, int64_t ldk_w, bool dv = false) {
     icon::CcGeometry geom;
     geom.col_bytes[0] = (nlev * (int)sizeof(T) + 15) & ~15;
-    geom.col_bytes[1] = icon::cc_slot_bytes<T>(nlev);
+    geom.col_bytes[1] = dv ? geom.col_bytes[0] : icon::cc_slot_bytes<T>(nlev);      // div / vort only: no w column
     geom.stride_bytes[0] = (int)(ldk * (int64_t)sizeof(T));
     geom.stride_bytes[1] = (int)(ldk_w * (int64_t)sizeof(T));
     geom.slot_bytes = geom.col_bytes[1];
@@ -186,24 +186,25 @@ icon::CcGeometry cc_geometry(int nlev, int64_t ldk, int64_t ldk_w) {
 }
 
 template <class T>
-constexpr int cc_record_size() { return icon::kScCoefWords * (int)sizeof(T) + icon::kCcRecordTail; }
+constexpr int cc_record_size(int mode) { return icon::cc_coef_words(mode) * (int)sizeof(T) + icon::kCcRecordTail; }
 
 // Column-cache schedule + patch records for (T, nlev): built on the host once, uploaded once.
 // Returns ICON_OK with p.unsupported set when this (T, nlev) cannot use the kernel (the caller
 // then uses the self-contained patch kernel).
 template <class T>
-int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev, int64_t ldk, int64_t ldk_w) {
+int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev, int64_t ldk, int64_t ldk_w, bool dv = false) {
     const int tile = g->options[ICON_OPT_CC_TILE];
+    const int mode = dv ? icon::kCcDivVort : icon::kCcStep;
     if (p.nlev == nlev && p.ldk == ldk && p.ldk_w == ldk_w && p.tile == tile && (p.ready || p.unsupported))
         return ICON_OK;
     dev_release(g, p.steps); dev_release(g, p.loads); dev_release(g, p.records);
     dev_release(g, p.cta_patch_begin); dev_release(g, p.cta_step_begin); dev_release(g, p.progress);
     p = icon::DevCcTables<T>();
     p.nlev = nlev;
-    p.ldk = ldk; p.ldk_w = ldk_w; p.tile = tile;
-    const icon::CcGeometry geom = cc_geometry<T>(nlev, ldk, ldk_w);
+    p.ldk = ldk; p.ldk_w = ldk_w; p.tile = tile; p.dv = dv;
+    const icon::CcGeometry geom = cc_geometry<T>(nlev, ldk, ldk_w, dv);
     const int slot_bytes = geom.slot_bytes;
-    const int n_slots_max = icon::cc_max_slots<T>(slot_bytes, g->smem_optin);
+    const int n_slots_max = icon::cc_max_slots<T>(slot_bytes, g->smem_optin, mode);
     if (icon::cc_levels_per_lane(nlev) == 0 || nlev * (int)sizeof(T) < 16 || n_slots_max < icon::kScIdWords) {
         p.unsupported = true;
         return ICON_OK;
@@ -214,9 +215,10 @@ int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev, int64_t ld
     const int n_slots = std::min(n_slots_max, 65535);
     icon::CcSchedule cs;
     std::vector<unsigned char> rec;
-    const size_t rb = (size_t)cc_record_size<T>();
+    const size_t rb = (size_t)cc_record_size<T>(mode);
+    const int ncoef = icon::cc_coef_words(mode);
     try {
-        std::string err = icon::build_cc_schedule(sc, g->num_sms, n_slots, geom, icon::kCcGroup, icon::kCcDepth, tile, cs);
+        std::string err = icon::build_cc_schedule(sc, g->num_sms, n_slots, geom, icon::kCcGroup, icon::kCcDepth, tile, icon::cc_use_mask(mode), cs);
         if (!err.empty()) {
             p.unsupported = true;
             return ICON_OK;
@@ -227,8 +229,15 @@ int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev, int64_t ld
             unsigned char* r = rec.data() + (size_t)q * rb;
             T* cf = reinterpret_cast<T*>(r);
             const int64_t src = cs.patch_order[(size_t)q];       // record q belongs to work position q
-            for (int i = 0; i < icon::kScCoefWords; ++i) cf[i] = (T)sc.coef[(size_t)src * icon::kScCoefWords + i];
-            int32_t* oid = reinterpret_cast<int32_t*>(r + (size_t)icon::kScCoefWords * sizeof(T));
+            const double* scf = &sc.coef[(size_t)src * icon::kScCoefWords];
+            if (dv) {          // compact record: geofac_div, rot of the midpoints, rot of the corners
+                for (int i = 0; i < 12; ++i) cf[icon::DVF_DIV + i] = (T)scf[icon::SCF_DIV + i];
+                for (int i = 0; i < 20; ++i) cf[icon::DVF_ROT + i] = (T)scf[icon::SCF_ROT + i];
+                for (int i = 0; i < 20; ++i) cf[icon::DVF_XROT + i] = (T)(i < 18 ? scf[icon::SCF_XROT + i] : 0.0);
+            } else {
+                for (int i = 0; i < icon::kScCoefWords; ++i) cf[i] = (T)scf[i];
+            }
+            int32_t* oid = reinterpret_cast<int32_t*>(r + (size_t)ncoef * sizeof(T));
             const int32_t* id = &sc.ids[(size_t)src * icon::kScIdWords];
             for (int x = 0; x < 3; ++x) {
                 oid[x] = id[icon::SID_I0 + x];
@@ -236,11 +245,11 @@ int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev, int64_t ld
             }
             for (int x = 0; x < 4; ++x) oid[6 + x] = id[icon::SID_T0 + x];
             for (int x = 0; x < 6; ++x) oid[10 + x] = id[icon::SID_V0 + x];
-            for (int x = 0; x < 6; ++x) {          // c_lin halved: the kernel forms w(k) + w(k+1) (exact scaling)
+            for (int x = 0; x < 6 && !dv; ++x) {   // c_lin halved: the kernel forms w(k) + w(k+1) (exact scaling)
                 cf[icon::SCF_EDGE + 4 * x + 2] *= (T)0.5;
                 cf[icon::SCF_EDGE + 4 * x + 3] *= (T)0.5;
             }
-            uint32_t* so = reinterpret_cast<uint32_t*>(r + (size_t)icon::kScCoefWords * sizeof(T) + 4 * icon::kCcRecordIds);
+            uint32_t* so = reinterpret_cast<uint32_t*>(r + (size_t)ncoef * sizeof(T) + 4 * icon::kCcRecordIds);
             for (int i = 0; i < icon::kCcSlotWords; ++i)
                 so[i] = (uint32_t)cs.patch_slots[(size_t)q * icon::kCcSlotWords + i] * (uint32_t)slot_bytes;
             so[icon::kCcMaskWord] = cs.patch_slots[(size_t)q * icon::kCcSlotWords + icon::kCcMaskWord];
@@ -426,8 +435,8 @@ int tendencies_impl(icon_grid* g, icon::DevCoeffs<T>& c, icon::DevScTables<T>& s
     if (variant != 4 || want_opt) div_fused = vort_fused = nullptr;
     if (fused_done) *fused_done = div_fused != nullptr;
     if (variant == 4 && !want_opt) {
-        n = icon::launch_tendencies_cc<T>(*g, ct, nlev, ldk, ldk_w, (const T*)abc, (const T*)vn, (const T*)w, (T*)ddt_vn,
-                                          (T*)div_fused, (T*)vort_fused, s);
+        n = icon::launch_tendencies_cc<T>(*g, ct, div_fused ? icon::kCcStep : icon::kCcTend, nlev, ldk, ldk_w, (const T*)abc, (const T*)vn,
+                                          (const T*)w, (T*)ddt_vn, (T*)div_fused, (T*)vort_fused, s);
     } else if (variant == 0 || want_opt) {
         // optional outputs are produced by the unfused pipeline, which materialises them anyway
         if ((rc = ensure_workspace<T>(g, dtype, ldk))) return rc;
@@ -633,14 +642,22 @@ int icon_grid_cc_schedule_check(const icon_grid_t* gc, int dtype, int nlev, int 
     int rc = ensure_sc_host(g);
     if (rc) return rc;
     const bool f64 = dtype == ICON_F64;
-    const icon::CcGeometry geom = f64 ? cc_geometry<double>(nlev, ldk, ldk_w) : cc_geometry<float>(nlev, ldk, ldk_w);
-    const int n_slots = std::min(65535, f64 ? icon::cc_max_slots<double>(geom.slot_bytes, smem_bytes) : icon::cc_max_slots<float>(geom.slot_bytes, smem_bytes));
     icon::CcSchedule cs;
+    icon::CcGeometry geom;
     try {
-        std::string err = icon::build_cc_schedule(g->sc_host, n_ctas, n_slots, geom, icon::kCcGroup, icon::kCcDepth, g->options[ICON_OPT_CC_TILE], cs);
-        if (!err.empty()) return fail(ICON_EUNSUPPORTED, err);
-        err = icon::check_cc_schedule(g->sc_host, cs, g->host.ne, g->host.nc);
-        if (!err.empty()) return fail(ICON_EINVAL, err);
+        // the schedule of dycore_div_vort (27 vn columns per patch, compact records) first, then the one of the tendency /
+        // fused step, whose shape is reported
+        for (int mode : {(int)icon::kCcDivVort, (int)icon::kCcStep}) {
+            const bool dv = mode == icon::kCcDivVort;
+            geom = f64 ? cc_geometry<double>(nlev, ldk, ldk_w, dv) : cc_geometry<float>(nlev, ldk, ldk_w, dv);
+            const int n_slots = std::min(65535, f64 ? icon::cc_max_slots<double>(geom.slot_bytes, smem_bytes, mode)
+                                                    : icon::cc_max_slots<float>(geom.slot_bytes, smem_bytes, mode));
+            std::string err = icon::build_cc_schedule(g->sc_host, n_ctas, n_slots, geom, icon::kCcGroup, icon::kCcDepth,
+                                                      g->options[ICON_OPT_CC_TILE], icon::cc_use_mask(mode), cs);
+            if (!err.empty()) return fail(ICON_EUNSUPPORTED, err);
+            err = icon::check_cc_schedule(g->sc_host, cs, g->host.ne, g->host.nc);
+            if (!err.empty()) return fail(ICON_EINVAL, err + (dv ? " (div/vort schedule)" : ""));
+        }
     } catch (const std::bad_alloc&) {
         return fail(ICON_ENOMEM, "out of host memory while building the column-cache schedule");
     }
@@ -663,12 +680,27 @@ int dycore_div_vort(const icon_grid_t* gc, int dtype, int nlev, int ldk, const v
     }
     cudaStream_t s = (cudaStream_t)cuda_stream;
     int n;
+    // the column cache in its div / vort mode wherever it holds the columns (ICON_OPT_TENDENCY_KERNEL 4 or auto), else
+    // the gather kernel through L1
+    const bool want_cc = g->options[ICON_OPT_TENDENCY_KERNEL] >= 4 && nlev >= 2;
     if (dtype == ICON_F64) {
-        if ((rc = ensure_coeffs(g, g->c64))) return rc;
-        n = icon::launch_div_vort<double>(*g, g->c64, nlev, ldk, (const double*)vn, (double*)div, (double*)vort, s);
+        if (want_cc && (rc = ensure_cc_tables(g, g->dv64, nlev, ldk, ldk, true))) return rc;
+        if (want_cc && !g->dv64.unsupported) {
+            n = icon::launch_tendencies_cc<double>(*g, g->dv64, icon::kCcDivVort, nlev, ldk, ldk, nullptr, (const double*)vn, nullptr, nullptr,
+                                                   (double*)div, (double*)vort, s);
+        } else {
+            if ((rc = ensure_coeffs(g, g->c64))) return rc;
+            n = icon::launch_div_vort<double>(*g, g->c64, nlev, ldk, (const double*)vn, (double*)div, (double*)vort, s);
+        }
     } else {
-        if ((rc = ensure_coeffs(g, g->c32))) return rc;
-        n = icon::launch_div_vort<float>(*g, g->c32, nlev, ldk, (const float*)vn, (float*)div, (float*)vort, s);
+        if (want_cc && (rc = ensure_cc_tables(g, g->dv32, nlev, ldk, ldk, true))) return rc;
+        if (want_cc && !g->dv32.unsupported) {
+            n = icon::launch_tendencies_cc<float>(*g, g->dv32, icon::kCcDivVort, nlev, ldk, ldk, nullptr, (const float*)vn, nullptr, nullptr,
+                                                  (float*)div, (float*)vort, s);
+        } else {
+            if ((rc = ensure_coeffs(g, g->c32))) return rc;
+            n = icon::launch_div_vort<float>(*g, g->c32, nlev, ldk, (const float*)vn, (float*)div, (float*)vort, s);
+        }
     }
     if (n < 0) return fail_cuda((cudaError_t)(-n), "kernel launch");
     g->launches += n;

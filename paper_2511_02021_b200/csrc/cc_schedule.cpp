@@ -25,7 +25,7 @@ inline uint64_t key_of(int slot_in_patch, int32_t id) {
 }
 
 void simulate_cta(const ScTables& sc, const int64_t* order, int64_t pb, int64_t pe, int n_slots, const CcGeometry& geom, int kCcGroup,
-                  int max_depth, uint16_t* patch_slots, CtaResult& r) {
+                  int max_depth, uint64_t use, uint16_t* patch_slots, CtaResult& r) {
     const int64_t n_steps = (pe - pb + kCcGroup - 1) / kCcGroup;
     // pass 1: the distinct columns of every step
     std::vector<std::vector<uint64_t>> keys((size_t)n_steps);
@@ -33,7 +33,8 @@ void simulate_cta(const ScTables& sc, const int64_t* order, int64_t pb, int64_t 
         auto& ks = keys[(size_t)s];
         const int64_t p0 = pb + s * kCcGroup, p1 = std::min(pe, p0 + kCcGroup);
         for (int64_t p = p0; p < p1; ++p)
-            for (int i = 0; i < kRefs; ++i) ks.push_back(key_of(i, sc.ids[(size_t)order[p] * kScIdWords + i]));
+            for (int i = 0; i < kRefs; ++i)
+                if ((use >> i) & 1) ks.push_back(key_of(i, sc.ids[(size_t)order[p] * kScIdWords + i]));
         std::sort(ks.begin(), ks.end());
         ks.erase(std::unique(ks.begin(), ks.end()), ks.end());
     }
@@ -186,6 +187,10 @@ void simulate_cta(const ScTables& sc, const int64_t* order, int64_t pb, int64_t 
             // be in flight when step s starts (copies of different steps complete in any order)
             uint16_t mask = 0;
             for (int i = 0; i < kRefs; ++i) {
+                if (!((use >> i) & 1)) {          // a column this mode never reads
+                    o[i] = 0;
+                    continue;
+                }
                 const int32_t q = step_slot[key_of(i, sc.ids[(size_t)order[p] * kScIdWords + i])];
                 o[i] = (uint16_t)q;
                 const int64_t age = s - slot_loaded[(size_t)q];
@@ -200,7 +205,7 @@ void simulate_cta(const ScTables& sc, const int64_t* order, int64_t pb, int64_t 
 }  // namespace
 
 std::string build_cc_schedule(const ScTables& sc, int n_ctas, int n_slots, const CcGeometry& geom, int group, int depth,
-                              int tile, CcSchedule& out) {
+                              int tile, uint64_t use, CcSchedule& out) {
     const int kCcGroup = group;
     const int64_t np = sc.n_patches;
     if (np <= 0 || n_ctas <= 0) return "cc schedule: empty grid";
@@ -218,6 +223,7 @@ std::string build_cc_schedule(const ScTables& sc, int n_ctas, int n_slots, const
     out.group = group;
     out.depth = depth;
     out.tile = tile;
+    out.use = use;
     out.cta_patch_begin.resize((size_t)n_ctas + 1);
     // whole steps per CTA, spread evenly
     const int64_t total_steps = max_ctas;
@@ -248,7 +254,7 @@ std::string build_cc_schedule(const ScTables& sc, int n_ctas, int n_slots, const
 #pragma omp parallel for schedule(dynamic, 1)
     for (int b = 0; b < n_ctas; ++b)
         simulate_cta(sc, out.patch_order.data(), out.cta_patch_begin[(size_t)b], out.cta_patch_begin[(size_t)b + 1], n_slots, geom, group,
-                     depth, out.patch_slots.data(), res[(size_t)b]);
+                     depth, use, out.patch_slots.data(), res[(size_t)b]);
     out.cta_step_begin.assign((size_t)n_ctas + 1, 0);
     size_t n_loads = 0;
     for (int b = 0; b < n_ctas; ++b) {

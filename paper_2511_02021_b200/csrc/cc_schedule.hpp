@@ -48,6 +48,25 @@ struct CcWarps {
 constexpr int kCcMaxProducers = 8;
 constexpr int kCcAhead = 3;              // steps the producers read the schedule ahead; `loads` is padded for it
 constexpr int kCcBarrierBytes = 512;    // the mbarriers
+// What a launch of the kernel produces; each mode has a schedule of its own (DevCcTables::mode).
+enum { kCcTend = 0 /* ddt_vn */, kCcStep = 1 /* ddt_vn + div + vort */, kCcDivVort = 2 /* div + vort only */ };
+// kCcDivVort reads 27 of the 36 vn columns of a patch and no w column, and its records carry only the 52 coefficients it
+// needs: geofac_div [4][3], rot of the midpoints [3][6] (+2 pad), rot of the corners [3][6] (+2 pad)
+enum { DVF_DIV = 0, DVF_ROT = 12, DVF_XROT = 32, kCcDvCoefWords = 52 };
+#ifdef __CUDACC__
+#define CC_HD __host__ __device__
+#else
+#define CC_HD
+#endif
+CC_HD constexpr int cc_coef_words(int mode) { return mode == kCcDivVort ? (int)kCcDvCoefWords : (int)kScCoefWords; }
+// id slots (sc_tables.hpp) a mode reads: bit i of the mask = column i of the patch is needed
+constexpr uint64_t cc_use_mask(int mode) {
+    uint64_t all = (1ull << SID_PAD) - 1;
+    if (mode != kCcDivVort) return all;
+    uint64_t m = (1ull << SID_X0) - 1;                                   // i0..i2, b0..b5, om0..om5, oc0..oc5
+    for (int x = 0; x < 3; ++x) m |= 3ull << (SID_X0 + 5 * x + 3);       // n1, n2 of the three corners
+    return m;
+}
 // a patch record on the device = kScCoefWords coefficients (T), then kCcRecordIds int32 (user ids of
 // the outputs), then kCcSlotWords uint32 byte offsets of the slots; c_lin is
 // stored halved there (the kernel forms w(k) + w(k+1) = 2 w_f(k))
@@ -89,6 +108,7 @@ struct CcSchedule {
     int depth = 0;                           // steps a load may run ahead of its readers (pipeline depth)
     CcGeometry geom = {0, {0, 0}, {0, 0}};
     int tile = 0;                            // patches per round-robin tile (0 = contiguous ranges)
+    uint64_t use = 0;                        // cc_use_mask the schedule was built for
     std::vector<int64_t> patch_order;        // [n_patches] work position -> patch of the ScTables
     std::vector<int64_t> cta_patch_begin;    // [n_ctas + 1], work positions
     std::vector<int64_t> cta_step_begin;     // [n_ctas + 1]
@@ -103,8 +123,9 @@ struct CcSchedule {
 // Returns an empty string on success, else an error message (e.g. too few slots for one step).
 // `tile`: 0 = every CTA walks a contiguous range of the generation order; > 0 = tiles of that many
 // patches are dealt round-robin to the CTAs (CcSchedule::patch_order).
+// `use` = cc_use_mask(mode): the columns of a patch the kernel reads in that mode (slots of unused columns stay 0).
 std::string build_cc_schedule(const ScTables& sc, int n_ctas, int n_slots, const CcGeometry& geom, int group, int depth,
-                              int tile, CcSchedule& out);
+                              int tile, uint64_t use, CcSchedule& out);
 
 // cc_schedule_check.cpp: replays `cs` as the kernel would and checks the guarantees it relies on
 // (independent of the builder). Empty string = valid.

@@ -33,10 +33,10 @@ int launch_tendencies_sc(const icon_grid& g, const DevScTables<T>& p, int nlev, 
 
 // S2-S7, column-cache kernel (kernels_cc.cu): a producer warp streams whole vn / w columns into
 // shared-memory slots with bulk asynchronous copies following the host-built schedule
-// (cc_schedule.hpp); consumer warps finish one self-contained patch each from the slots. With div and
-// vort non-NULL the same pass also stores S1 and S2 (dycore_step); NULL = tendency only.
+// (cc_schedule.hpp); consumer warps finish one self-contained patch each from the slots. mode = kCcTend (ddt_vn),
+// kCcStep (ddt_vn + div + vort in one pass: dycore_step) or kCcDivVort (div + vort only, tables built for that mode).
 template <class T>
-int launch_tendencies_cc(const icon_grid& g, DevCcTables<T>& p, int nlev, int64_t ldk, int64_t ldk_w,
+int launch_tendencies_cc(const icon_grid& g, DevCcTables<T>& p, int mode, int nlev, int64_t ldk, int64_t ldk_w,
                          const T* abc, const T* vn, const T* w, T* ddt_vn, T* div, T* vort, cudaStream_t s);
 // shape helpers of that kernel: levels per lane (0 = nlev not supported), bytes of one w column
 // (the smallest possible slot), and how many slots of `slot_bytes` fit beside the fixed buffers in `smem_optin` bytes of shared memory
@@ -44,6 +44,6 @@ int cc_levels_per_lane(int nlev);
 template <class T>
 int cc_slot_bytes(int nlev);
 template <class T>
-int cc_max_slots(int slot_bytes, int smem_optin);
+int cc_max_slots(int slot_bytes, int smem_optin, int mode);
 
 }  // namespace icon

@@ -234,12 +234,14 @@ __device__ __forceinline__ void ld_slots(const uint32_t* __restrict__ p, uint32_
 }
 
 template <class T>
-__host__ __device__ constexpr int cc_record_bytes() { return kScCoefWords * (int)sizeof(T) + kCcRecordTail; }
+__host__ __device__ constexpr int cc_record_bytes(int mode) { return cc_coef_words(mode) * (int)sizeof(T) + kCcRecordTail; }
 
 // kCcWarps consumer warps in two groups of kCcGroup; group g runs the steps s = g (mod 2); ring depth kCcDepth.
-// FUSED: the same pass also stores div of the patch's four cells and the vorticity of the vertices the
-// patch owns (dycore_step): both are by-products of columns and sums the tendency needs anyway.
-template <class T, int L, bool FUSED>
+// MODE kCcTend: ddt_vn only (dycore_velocity_tendencies). MODE kCcStep: the same pass also stores div of the patch's four
+// cells and the vorticity of the vertices the patch owns (dycore_step): both are by-products of columns and sums the
+// tendency needs anyway. MODE kCcDivVort: ONLY div and vorticity (dycore_div_vort) from the 27 vn columns they need, with
+// compact records (52 coefficients) and a schedule of its own.
+template <class T, int L, int MODE>
 __global__ void __launch_bounds__((kCcWarps + CcWarps<T, L>::producers) * 32, 1)
 k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, const T* __restrict__ vn,
           const T* __restrict__ w, T* __restrict__ ddt_vn, T* __restrict__ div, T* __restrict__ vort,
@@ -247,8 +249,9 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
     extern __shared__ __align__(128) unsigned char smem[];
     using C = Col<T, L>;
     constexpr int W = kCcWarps, G = kCcGroup, D = kCcDepth;
+    constexpr bool FUSED = MODE != kCcTend, DVONLY = MODE == kCcDivVort;
     constexpr int kCcProducers = CcWarps<T, L>::producers;
-    constexpr int REC = cc_record_bytes<T>();
+    constexpr int REC = cc_record_bytes<T>(MODE), COEF = cc_coef_words(MODE);
     constexpr int NGRP = W / G;
     static_assert(W % G == 0 && W % 4 == 0 && D > NGRP && D <= 16, "bad pipeline shape");
     // the shuffle tells the compiler that the warp index is warp-uniform: branches on it (role, patch in range)
@@ -296,7 +299,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
         // the next multiple before every CTA, this one included, has added all of its events). Kept on the device so
         // that a captured CUDA graph replays correctly.
         unsigned long long pace_base = 0;
-        if (FUSED && !CcWarps<T, L>::light && pace_mask && lane == 0) {
+        if (MODE == kCcStep && !CcWarps<T, L>::light && pace_mask && lane == 0) {
             unsigned long long have;
             asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(have) : "l"(pace_counter) : "memory");
             pace_base = have - have % pace_per_launch;
@@ -332,7 +335,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
                     // compiled into the fused fp64 three-levels-per-lane kernel only: the tendency-only kernel lost 3 %
                     // to the mere presence of this block, and the light instantiations (fp32, one level per lane)
                     // slowed down by 40-50 % with the barrier active
-                    if (FUSED && !CcWarps<T, L>::light && pace_mask && s && (s & pace_mask) == 0 && s <= pace_last) {
+                    if (MODE == kCcStep && !CcWarps<T, L>::light && pace_mask && s && (s & pace_mask) == 0 && s <= pace_last) {
                         // every pace_mask + 1 steps the producers of all CTAs meet (bounded wait: pacing is an
                         // optimisation, never a condition for progress): SMs run at slightly different rates, and once
                         // the CTAs are rounds apart neighbouring tiles no longer share their halo columns through the L2
@@ -404,9 +407,9 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
         const int k = level_of<L>(lane, l);
         po[l] = k < nlev;
         below_missing[l] = k + 1 >= nlev;
-        cA[l] = po[l] ? __ldg(abc + k) : (T)0;
-        cB[l] = po[l] ? __ldg(abc + nlev + k) : (T)0;
-        cC[l] = po[l] ? __ldg(abc + 2 * nlev + k) : (T)0;
+        cA[l] = !DVONLY && po[l] ? __ldg(abc + k) : (T)0;
+        cB[l] = !DVONLY && po[l] ? __ldg(abc + nlev + k) : (T)0;
+        cC[l] = !DVONLY && po[l] ? __ldg(abc + 2 * nlev + k) : (T)0;
     }
     const uint64_t cs = (uint64_t)ldk * sizeof(T);
     // this lane's two read positions inside every slot
@@ -421,8 +424,8 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
         if (p < pe) {
             const unsigned char* rec = rec_base + ((s % D) * G + wi) * REC;
             const T* cf = reinterpret_cast<const T*>(rec);
-            const int32_t* oid = reinterpret_cast<const int32_t*>(rec + kScCoefWords * sizeof(T));
-            const uint32_t* sl = reinterpret_cast<const uint32_t*>(rec + kScCoefWords * sizeof(T) + kCcRecordIds * 4);
+            const int32_t* oid = reinterpret_cast<const int32_t*>(rec + COEF * sizeof(T));
+            const uint32_t* sl = reinterpret_cast<const uint32_t*>(rec + COEF * sizeof(T) + kCcRecordIds * 4);
 
             // Every lane reads its levels whether they exist or not: lanes past the column end pick up stale bytes of
             // the slot (or of the next one; the pool ends with a readable pad) that only ever reach outputs through
@@ -496,7 +499,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
             if constexpr (FUSED) {
                 // ---- S1: div of the four cells from their edges (slot order of SCF_BLN) ------------
                 T gd[12];
-                ld_coef(cf + SCF_DIV, gd);
+                ld_coef(cf + (DVONLY ? (int)DVF_DIV : (int)SCF_DIV), gd);
                 C dv;
                 FORL dv.v[l] = gd[0] * vB[0].v[l] + gd[1] * vI[0].v[l] + gd[2] * vB[5].v[l];
                 ST(div, ido[6], dv);
@@ -507,6 +510,46 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
                 FORL dv.v[l] = gd[9] * vI[1].v[l] + gd[10] * vI[2].v[l] + gd[11] * vI[0].v[l];
                 ST(div, ido[9], dv);
             }
+            if constexpr (DVONLY) {
+                // ---- S2 alone: the six vorticities from the patch's own columns, the om / oc columns and n1, n2 -------
+                T g18[20], gx[20];
+                ld_coef(cf + DVF_ROT, g18);
+                ld_coef(cf + DVF_XROT, gx);
+                uint32_t sX[12];                    // x0[3..4] x1[0..4] x2[0..4]
+                ld_slots(sl + SID_X0 + 3, sX);
+                C zm[3], zc[3];
+                FORL {
+                    zm[0].v[l] = g18[0] * vB[0].v[l] + g18[1] * vB[1].v[l] + g18[2] * vI[0].v[l] + g18[3] * vI[1].v[l];
+                    zm[1].v[l] = g18[6] * vB[2].v[l] + g18[7] * vB[3].v[l] + g18[8] * vI[1].v[l] + g18[9] * vI[2].v[l];
+                    zm[2].v[l] = g18[12] * vB[4].v[l] + g18[13] * vB[5].v[l] + g18[14] * vI[2].v[l] + g18[15] * vI[0].v[l];
+                    zc[0].v[l] = gx[0] * vB[0].v[l] + gx[5] * vB[5].v[l];
+                    zc[1].v[l] = gx[6] * vB[2].v[l] + gx[11] * vB[1].v[l];
+                    zc[2].v[l] = gx[12] * vB[4].v[l] + gx[17] * vB[3].v[l];
+                }
+#pragma unroll
+                for (int j = 0; j < 6; ++j) {
+                    const C vM = LD(sE[9 + j]), vO = LD(sE[15 + j]);
+                    axpy(zm[j / 2], g18[6 * (j / 2) + 4 + (j & 1)], vM);
+                    if (j & 1) {
+                        const int xn = ((j + 1) % 6) / 2;
+                        axpy(zc[xn], gx[6 * xn + 4], vO);
+                    } else {
+                        const int x = j / 2;
+                        const C n1 = LD(sX[5 * x]), n2 = LD(sX[5 * x + 1]);
+                        FORL zc[x].v[l] += gx[6 * x + 1] * vO.v[l] + gx[6 * x + 2] * n1.v[l] + gx[6 * x + 3] * n2.v[l];
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(done_bar(s % NB));
+#pragma unroll
+                for (int m = 0; m < 3; ++m) {
+                    C z2;
+                    FORL z2.v[l] = (T)2 * zm[m].v[l];
+                    ST(vort, ido[10 + m], z2);
+                    FORL z2.v[l] = (T)2 * zc[m].v[l];
+                    ST(vort, ido[13 + m], z2);
+                }
+            } else {
             // ---- interior edges: vt, KE_e; start the cell sums -------------------------------
             T r12[12];
             ld_coef(cf + SCF_RBF, r12);
@@ -643,6 +686,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
                 FORL o.v[l] = -H[x].v[l] - we[x].v[l] * Dv.v[l];
                 ST(ddt_vn, ido[x], o);
             }
+            }   // !DVONLY
         } else {
             __syncwarp();
             if (lane == 0) mbar_arrive(done_bar(s % NB));
@@ -656,29 +700,29 @@ template <class T>
 int cc_slot_bytes(int nlev) { return (((nlev + 1) * (int)sizeof(T) + 15) & ~15); }
 
 template <class T>
-static size_t cc_fixed_smem() {
-    return kCcBarrierBytes + (size_t)kCcDepth * kCcGroup * cc_record_bytes<T>();
+static size_t cc_fixed_smem(int mode) {
+    return kCcBarrierBytes + (size_t)kCcDepth * kCcGroup * cc_record_bytes<T>(mode);
 }
 
 template <class T>
-int cc_max_slots(int slot_bytes, int smem_optin) {
-    const long avail = (long)smem_optin - (long)cc_fixed_smem<T>() - kCcSlotTailPad;
+int cc_max_slots(int slot_bytes, int smem_optin, int mode) {
+    const long avail = (long)smem_optin - (long)cc_fixed_smem<T>(mode) - kCcSlotTailPad;
     if (avail <= 0) return 0;
     return (int)(avail / slot_bytes);
 }
-template int cc_max_slots<double>(int, int);
-template int cc_max_slots<float>(int, int);
+template int cc_max_slots<double>(int, int, int);
+template int cc_max_slots<float>(int, int, int);
 template int cc_slot_bytes<double>(int);
 template int cc_slot_bytes<float>(int);
 
 int cc_levels_per_lane(int nlev) { return nlev + 1 <= 32 ? 1 : nlev + 1 <= 96 ? 3 : 0; }
 
 namespace {
-template <class T, int L, bool FUSED>
+template <class T, int L, int MODE>
 cudaError_t cc_launch_one(const CcDev<T>& d, int device, int n_ctas, size_t smem, int nlev, int ldk, int ldk_w, const T* abc,
                           const T* vn, const T* w, T* ddt_vn, T* div, T* vort, unsigned long long* pc, unsigned long long ppl,
                           int pm, int pl, cudaStream_t s) {
-    auto k = k_tend_cc<T, L, FUSED>;
+    auto k = k_tend_cc<T, L, MODE>;
     // the opt-in for > 48 KB of dynamic shared memory is a per-DEVICE attribute of the function: remembered per device
     static std::mutex mu;
     static size_t configured[64] = {0};       // largest size this instantiation was opted in for, per device ordinal
@@ -697,7 +741,7 @@ cudaError_t cc_launch_one(const CcDev<T>& d, int device, int n_ctas, size_t smem
 }  // namespace
 
 template <class T>
-int launch_tendencies_cc(const icon_grid& g, DevCcTables<T>& p, int nlev, int64_t ldk, int64_t ldk_w,
+int launch_tendencies_cc(const icon_grid& g, DevCcTables<T>& p, int mode, int nlev, int64_t ldk, int64_t ldk_w,
                          const T* abc, const T* vn, const T* w, T* ddt_vn, T* div, T* vort, cudaStream_t s) {
     CcDev<T> d;
     d.steps = p.steps; d.loads = p.loads; d.records = p.records;
@@ -708,25 +752,26 @@ int launch_tendencies_cc(const icon_grid& g, DevCcTables<T>& p, int nlev, int64_
     const int period = g.options[ICON_OPT_CC_PACE];
     const int L = cc_levels_per_lane(nlev);
     const bool heavy = sizeof(T) == 8 && L == 3;
-    int pace_mask = period > 0 && p.progress && div != nullptr && heavy ? period - 1 : 0;      // fused fp64 step only
+    int pace_mask = period > 0 && p.progress && mode == kCcStep && heavy ? period - 1 : 0;      // fused fp64 step only
     const int n_barriers = pace_mask ? (int)((p.min_steps - 1) / period) : 0;      // barriers every CTA reaches
     if (n_barriers == 0) pace_mask = 0;
     const int pace_last = n_barriers * period;
     const unsigned long long per_launch = (unsigned long long)n_barriers * (unsigned long long)p.n_ctas;
-    const size_t smem = cc_fixed_smem<T>() + (size_t)p.n_slots * p.slot_bytes + kCcSlotTailPad;
-    const bool fused = div != nullptr;
+    if ((mode == kCcDivVort) != p.dv || (mode == kCcDivVort) != (ddt_vn == nullptr) || (mode == kCcTend) != (div == nullptr))
+        return -(int)cudaErrorInvalidValue;
+    const size_t smem = cc_fixed_smem<T>(mode) + (size_t)p.n_slots * p.slot_bytes + kCcSlotTailPad;
     cudaError_t err = cudaErrorInvalidValue;
-#define CC_ONE(LL, FF) \
-    if (L == LL && fused == FF) \
-        err = cc_launch_one<T, LL, FF>(d, g.device, p.n_ctas, smem, nlev, (int)ldk, (int)ldk_w, abc, vn, w, ddt_vn, div, vort, p.progress, per_launch, pace_mask, pace_last, s);
-    CC_ONE(1, false) CC_ONE(1, true) CC_ONE(3, false) CC_ONE(3, true)
+#define CC_ONE(LL, MM) \
+    if (L == LL && mode == MM) \
+        err = cc_launch_one<T, LL, MM>(d, g.device, p.n_ctas, smem, nlev, (int)ldk, (int)ldk_w, abc, vn, w, ddt_vn, div, vort, p.progress, per_launch, pace_mask, pace_last, s);
+    CC_ONE(1, kCcTend) CC_ONE(1, kCcStep) CC_ONE(1, kCcDivVort) CC_ONE(3, kCcTend) CC_ONE(3, kCcStep) CC_ONE(3, kCcDivVort)
 #undef CC_ONE
     return err == cudaSuccess ? 1 : -(int)err;
 }
 
-template int launch_tendencies_cc<double>(const icon_grid&, DevCcTables<double>&, int, int64_t, int64_t,
+template int launch_tendencies_cc<double>(const icon_grid&, DevCcTables<double>&, int, int, int64_t, int64_t,
                                           const double*, const double*, const double*, double*, double*, double*, cudaStream_t);
-template int launch_tendencies_cc<float>(const icon_grid&, DevCcTables<float>&, int, int64_t, int64_t,
+template int launch_tendencies_cc<float>(const icon_grid&, DevCcTables<float>&, int, int, int64_t, int64_t,
                                          const float*, const float*, const float*, float*, float*, float*, cudaStream_t);
 
 }  // namespace icon
