@@ -102,7 +102,7 @@ enum {
                                      5 = auto (default) = 4 wherever it can hold the columns. */
     ICON_OPT_CC_TILE = 1,         /* kernel 4: patches per tile of the round-robin work order (CTA b walks the tiles
                                      b, b + #CTAs, ... so that neighbouring tiles are in flight together and share
-                                     their halo columns through the L2); a multiple of 4; 0 = one contiguous range per
+                                     their halo columns through the L2); a multiple of 8; 0 = one contiguous range per
                                      CTA. Default 16. */
     ICON_OPT_CC_PACE = 2,         /* kernel 4: the producers of all CTAs meet every this many steps (power of two; bounded
                                      wait) so that the CTAs do not drift rounds apart and neighbouring tiles keep sharing

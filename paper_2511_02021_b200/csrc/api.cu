@@ -204,7 +204,7 @@ int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev, int64_t ld
     p.ldk = ldk; p.ldk_w = ldk_w; p.tile = tile; p.dv = dv;
     const icon::CcGeometry geom = cc_geometry<T>(nlev, ldk, ldk_w, dv);
     const int slot_bytes = geom.slot_bytes;
-    const int n_slots_max = icon::cc_max_slots<T>(slot_bytes, g->smem_optin, mode);
+    const int n_slots_max = icon::cc_max_slots<T>(slot_bytes, g->smem_optin, mode, nlev);
     if (icon::cc_levels_per_lane(nlev) == 0 || nlev * (int)sizeof(T) < 16 || n_slots_max < icon::kScIdWords) {
         p.unsupported = true;
         return ICON_OK;
@@ -218,7 +218,7 @@ int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev, int64_t ld
     const size_t rb = (size_t)cc_record_size<T>(mode);
     const int ncoef = icon::cc_coef_words(mode);
     try {
-        std::string err = icon::build_cc_schedule(sc, g->num_sms, n_slots, geom, icon::kCcGroup, icon::kCcDepth, tile, icon::cc_use_mask(mode), cs);
+        std::string err = icon::build_cc_schedule(sc, g->num_sms, n_slots, geom, icon::cc_patches_per_step_for(nlev), icon::kCcDepth, tile, icon::cc_use_mask(mode), cs);
         if (!err.empty()) {
             p.unsupported = true;
             return ICON_OK;
@@ -624,7 +624,7 @@ int icon_grid_set_option(icon_grid_t* g, int option, int value) {
     if (!g) return fail(ICON_EINVAL, "grid handle is NULL");
     if (option < 0 || option >= ICON_OPT_COUNT) return fail(ICON_EINVAL, "unknown option");
     if (option == ICON_OPT_CC_PACE && (value < 0 || value > 65536 || (value & (value - 1)))) return fail(ICON_EINVAL, "bad option value");
-    if (option == ICON_OPT_CC_TILE && (value < 0 || value > 4096 || value % icon::kCcGroup)) return fail(ICON_EINVAL, "bad option value");
+    if (option == ICON_OPT_CC_TILE && (value < 0 || value > 4096 || value % 8)) return fail(ICON_EINVAL, "bad option value");
     if (option == ICON_OPT_TENDENCY_KERNEL && value != 0 && value != 3 && value != 4 && value != 5) return fail(ICON_EINVAL, "bad option value");
     g->options[option] = value;
     return ICON_OK;
@@ -650,9 +650,9 @@ int icon_grid_cc_schedule_check(const icon_grid_t* gc, int dtype, int nlev, int 
         for (int mode : {(int)icon::kCcDivVort, (int)icon::kCcStep}) {
             const bool dv = mode == icon::kCcDivVort;
             geom = f64 ? cc_geometry<double>(nlev, ldk, ldk_w, dv) : cc_geometry<float>(nlev, ldk, ldk_w, dv);
-            const int n_slots = std::min(65535, f64 ? icon::cc_max_slots<double>(geom.slot_bytes, smem_bytes, mode)
-                                                    : icon::cc_max_slots<float>(geom.slot_bytes, smem_bytes, mode));
-            std::string err = icon::build_cc_schedule(g->sc_host, n_ctas, n_slots, geom, icon::kCcGroup, icon::kCcDepth,
+            const int n_slots = std::min(65535, f64 ? icon::cc_max_slots<double>(geom.slot_bytes, smem_bytes, mode, nlev)
+                                                    : icon::cc_max_slots<float>(geom.slot_bytes, smem_bytes, mode, nlev));
+            std::string err = icon::build_cc_schedule(g->sc_host, n_ctas, n_slots, geom, icon::cc_patches_per_step_for(nlev), icon::kCcDepth,
                                                       g->options[ICON_OPT_CC_TILE], icon::cc_use_mask(mode), cs);
             if (!err.empty()) return fail(ICON_EUNSUPPORTED, err);
             err = icon::check_cc_schedule(g->sc_host, cs, g->host.ne, g->host.nc);

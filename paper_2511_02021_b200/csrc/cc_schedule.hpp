@@ -27,20 +27,33 @@
 
 namespace icon {
 
+#ifdef __CUDACC__
+#define CC_HD __host__ __device__
+#else
+#define CC_HD
+#endif
+
 // Pipeline shape of the kernel (kernels_cc.cu): kCcWarps consumer warps in groups of kCcGroup (= patches per
 // step), ring of kCcDepth steps. Measured against 8/2/6 (two patches per step, ring of six) on B200: config 3
 // 5.11 -> 4.91 ms, config 4 4.01 -> 3.38 ms, config 5 12.25 -> 9.84 ms.
 constexpr int kCcWarps = 8, kCcGroup = 4, kCcDepth = 3;
+// Level mappings (template parameter L of the kernel = values a lane holds per column):
+//   L = 3 (33 <= nlev+1 <= 96): one patch per warp, a lane owns levels 2*lane, 2*lane+1 and 64+lane;
+//   L = 2 (nlev+1 <= 32): TWO patches per warp, one per half-warp, a lane owns levels 2*(lane%16), 2*(lane%16)+1 --
+//         a step is then 8 patches, and every per-patch cost of a warp (coefficient and slot lookups, waits, address
+//         arithmetic) is paid once per two patches.
+CC_HD constexpr int cc_patches_per_warp(int L) { return L == 2 ? 2 : 1; }
+CC_HD constexpr int cc_patches_per_step(int L) { return kCcGroup * cc_patches_per_warp(L); }
 // Producer warps are added to the consumers; the CTA is launched with the registers of the average warp and
 // re-balances them with setmaxnreg: producers keep CcWarps::producer_regs, consumers grow to CcWarps::consumer_regs
 // (the pool is what the LAUNCH allocated: 384 * 168 = (4 * 56 + 8 * 224) * 32 = 64512 registers).
 // 8-byte columns: 4 producer warps with 56 registers, 8 consumer warps with 224 (launch: 384 threads x 168).
 // 4-byte columns: the consumers need fewer registers and the columns are half as long, i.e. twice the copies per byte,
 // so a second producer warpgroup issues them: 8 producer warps with 40 registers, consumers 216 (launch: 512 x 128).
-// One level per lane (L = 1, nlev <= 31) is the same case: short columns, light consumers.
+// Shallow columns (L = 2, nlev <= 31) are the same case: short columns, light consumers.
 template <class T, int L>
 struct CcWarps {
-    static constexpr bool light = sizeof(T) == 4 || L == 1;
+    static constexpr bool light = sizeof(T) == 4 || L == 2;
     static constexpr int producers = light ? 8 : 4;
     static constexpr int producer_regs = light ? 40 : 56;
     static constexpr int consumer_regs = light ? 216 : 224;
@@ -53,11 +66,6 @@ enum { kCcTend = 0 /* ddt_vn */, kCcStep = 1 /* ddt_vn + div + vort */, kCcDivVo
 // kCcDivVort reads 27 of the 36 vn columns of a patch and no w column, and its records carry only the 52 coefficients it
 // needs: geofac_div [4][3], rot of the midpoints [3][6] (+2 pad), rot of the corners [3][6] (+2 pad)
 enum { DVF_DIV = 0, DVF_ROT = 12, DVF_XROT = 32, kCcDvCoefWords = 52 };
-#ifdef __CUDACC__
-#define CC_HD __host__ __device__
-#else
-#define CC_HD
-#endif
 CC_HD constexpr int cc_coef_words(int mode) { return mode == kCcDivVort ? (int)kCcDvCoefWords : (int)kScCoefWords; }
 // id slots (sc_tables.hpp) a mode reads: bit i of the mask = column i of the patch is needed
 constexpr uint64_t cc_use_mask(int mode) {

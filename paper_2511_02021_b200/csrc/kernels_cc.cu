@@ -13,7 +13,7 @@
 //     (~15 instead of 43 column fetches per patch), and the fetches are in flight one or more steps
 //     ahead of their readers without holding a single register;
 //   * a lane owns L = 3 levels of a column, the PAIR 2*lane, 2*lane+1 and the single level 64+lane
-//     (L = 1, nlev <= 31: level = lane): a coefficient / slot lookup, which is warp-uniform, is paid once
+//     (nlev <= 31: two patches per warp, see cc_schedule.hpp): a coefficient / slot lookup, which is warp-uniform, is paid once
 //     per 96 levels; a column is read with one 16-byte and one 8-byte conflict-free shared-memory load
 //     per lane, and an output column leaves STRAIGHT FROM REGISTERS with one 16-byte and one 8-byte
 //     coalesced streaming store -- no transposition through shared memory (the previous mapping, three
@@ -140,7 +140,8 @@ struct CcDev {
 #endif
 
 // ---- the L levels of one column a lane owns ---------------------------------------------------------
-// L == 3: v[0], v[1] = levels 2*lane, 2*lane+1 (one 16-byte access), v[2] = level 64+lane. L == 1: level = lane.
+// L == 3: v[0], v[1] = levels 2*lane, 2*lane+1 (one 16-byte access), v[2] = level 64+lane.
+// L == 2: v[0], v[1] = levels 2*(lane%16), 2*(lane%16)+1 of the half-warp's own patch.
 template <class T, int L>
 struct Col {
     T v[L];
@@ -148,7 +149,7 @@ struct Col {
 #define FORL _Pragma("unroll") for (int l = 0; l < L; ++l)
 
 template <int L>
-__device__ __forceinline__ int level_of(int lane, int l) { return L == 1 ? lane : (l < 2 ? 2 * lane + l : 64 + lane); }
+__device__ __forceinline__ int level_of(int lane, int l) { return L == 2 ? 2 * (lane & 15) + l : (l < 2 ? 2 * lane + l : 64 + lane); }
 
 template <class T> struct Pair;
 template <> struct Pair<double> { using type = double2; };
@@ -161,8 +162,9 @@ template <> struct Pair<float> { using type = float2; };
 template <class T, int L>
 __device__ __forceinline__ Col<T, L> level_up(const Col<T, L>& a, int lane) {
     Col<T, L> r;
-    if constexpr (L == 1) {
-        r.v[0] = __shfl_up_sync(kFull, a.v[0], 1);
+    if constexpr (L == 2) {
+        r.v[0] = __shfl_up_sync(kFull, a.v[1], 1, 16);        // inside the half-warp
+        r.v[1] = a.v[0];
     } else {
         r.v[0] = __shfl_up_sync(kFull, a.v[1], 1);
         r.v[1] = a.v[0];
@@ -173,8 +175,9 @@ __device__ __forceinline__ Col<T, L> level_up(const Col<T, L>& a, int lane) {
 template <class T, int L>
 __device__ __forceinline__ Col<T, L> level_down(const Col<T, L>& a, int lane) {
     Col<T, L> r;
-    if constexpr (L == 1) {
-        r.v[0] = __shfl_down_sync(kFull, a.v[0], 1);
+    if constexpr (L == 2) {
+        r.v[0] = a.v[1];
+        r.v[1] = __shfl_down_sync(kFull, a.v[0], 1, 16);
     } else {
         r.v[0] = a.v[1];
         r.v[1] = __shfl_sync(kFull, lane == 0 ? a.v[2] : a.v[0], (lane + 1) & 31);
@@ -249,6 +252,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
     extern __shared__ __align__(128) unsigned char smem[];
     using C = Col<T, L>;
     constexpr int W = kCcWarps, G = kCcGroup, D = kCcDepth;
+    constexpr int PPW = cc_patches_per_warp(L), PPS = G * PPW;      // patches per warp, per step
     constexpr bool FUSED = MODE != kCcTend, DVONLY = MODE == kCcDivVort;
     constexpr int kCcProducers = CcWarps<T, L>::producers;
     constexpr int REC = cc_record_bytes<T>(MODE), COEF = cc_coef_words(MODE);
@@ -259,7 +263,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
     const int warp = __shfl_sync(kFull, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem);                       // full[NB], done[NB]
     unsigned char* rec_base = smem + kCcBarrierBytes;
-    unsigned char* slot_base = rec_base + D * G * REC;
+    unsigned char* slot_base = rec_base + D * PPS * REC;
     const uint32_t bar0 = smem_u32(bars);
     auto full_bar = [&](int i) { return bar0 + 8u * (uint32_t)i; };
     // NB >= 2D-1 and >= NGRP+D: see the parity argument in the header comment
@@ -376,8 +380,8 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
                     if (rec_warp && lane == 0) {
                         // the records of a step's patches are consecutive in memory and in the ring: one copy
                         // (evict-first: a record is read once)
-                        const int64_t p = pb + (int64_t)s * G;
-                        const uint32_t dst = rec0 + (uint32_t)(((s % D) * G) * REC);
+                        const int64_t p = pb + (int64_t)s * PPS;
+                        const uint32_t dst = rec0 + (uint32_t)(((s % D) * PPS) * REC);
                         bulk_g2s_hint(dst, d.records + p * REC, n_pat * (uint32_t)REC, fb, pol_first);
                     }
                     for (int base = 0; base + mine < n_loads; base += 32 * kCcProducers) {
@@ -412,17 +416,25 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
         cC[l] = !DVONLY && po[l] ? __ldg(abc + 2 * nlev + k) : (T)0;
     }
     const uint64_t cs = (uint64_t)ldk * sizeof(T);
+    const int hl = L == 2 ? lane & 15 : lane, half = L == 2 ? lane >> 4 : 0;      // lane inside its patch, patch of the warp
     // this lane's two read positions inside every slot
-    const unsigned char* my_pair = slot_base + (L == 1 ? lane : 2 * lane) * (int)sizeof(T);
+    const unsigned char* my_pair = slot_base + 2 * hl * (int)sizeof(T);
     const unsigned char* my_single = slot_base + (64 + lane) * (int)sizeof(T);
     // and its two byte offsets inside every output column
-    const uint32_t st_pair = (uint32_t)((L == 1 ? lane : 2 * lane) * (int)sizeof(T)), st_single = (uint32_t)((64 + lane) * (int)sizeof(T));
+    const uint32_t st_pair = (uint32_t)(2 * hl * (int)sizeof(T)), st_single = (uint32_t)((64 + lane) * (int)sizeof(T));
 
     for (int s = grp; s < n_steps; s += NGRP) {
-        const int64_t p = pb + (int64_t)s * G + wi;
+        const int64_t p_first = pb + (int64_t)s * PPS + wi * PPW;       // the warp's first patch of this step
         mbar_wait(full_bar(s % NB), (uint32_t)((s / NB) & 1), 2, s);
-        if (p < pe) {
-            const unsigned char* rec = rec_base + ((s % D) * G + wi) * REC;
+        if (p_first < pe) {
+            // L == 2: the second half-warp's patch may lie past the end of the CTA's range (odd patch count): it then
+            // repeats the first one's reads and arithmetic and stores nothing
+            const bool live = p_first + half < pe;
+            const int my_patch = wi * PPW + (live ? half : 0);
+            if constexpr (L == 2) {
+                if (!live) { FORL po[l] = false; }
+            }
+            const unsigned char* rec = rec_base + ((s % D) * PPS + my_patch) * REC;
             const T* cf = reinterpret_cast<const T*>(rec);
             const int32_t* oid = reinterpret_cast<const int32_t*>(rec + COEF * sizeof(T));
             const uint32_t* sl = reinterpret_cast<const uint32_t*>(rec + COEF * sizeof(T) + kCcRecordIds * 4);
@@ -433,13 +445,9 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
             auto LD = [&](uint32_t off) {
                 CC_ASSERT(off % 16 == 0 && off + 96 * sizeof(T) <= (uint32_t)d.n_slots * (uint32_t)d.slot_bytes + kCcSlotTailPad, "slot offset", off, d.n_slots);
                 C c;
-                if constexpr (L == 1) {
-                    c.v[0] = *reinterpret_cast<const T*>(my_pair + off);
-                } else {
-                    const typename Pair<T>::type pr = *reinterpret_cast<const typename Pair<T>::type*>(my_pair + off);
-                    c.v[0] = pr.x; c.v[1] = pr.y;
-                    c.v[2] = *reinterpret_cast<const T*>(my_single + off);
-                }
+                const typename Pair<T>::type pr = *reinterpret_cast<const typename Pair<T>::type*>(my_pair + off);
+                c.v[0] = pr.x; c.v[1] = pr.y;
+                if constexpr (L == 3) c.v[2] = *reinterpret_cast<const T*>(my_single + off);
                 return c;
             };
             auto WS = [&](uint32_t off) {       // w(k) + w(k+1) = 2 w_f(k) (S6); the 1/2 is folded into c_lin
@@ -462,14 +470,12 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
                 CC_ASSERT(id < (base == ddt_vn ? d.ne : base == div ? d.nc : d.nv), "output id", id, base == ddt_vn ? 0 : base == div ? 1 : 2);
                 // one 64-bit column base (warp-uniform) plus the lane's two 32-bit byte offsets
                 unsigned char* col = reinterpret_cast<unsigned char*>(base) + (uint64_t)(uint32_t)id * cs;
-                if constexpr (L == 1) {
-                    if (po[0]) __stcs(reinterpret_cast<T*>(col + st_pair), x.v[0]);
-                } else {
-                    using P2 = typename Pair<T>::type;
-                    P2 pr;
-                    pr.x = x.v[0]; pr.y = x.v[1];
-                    if (po[1]) __stcs(reinterpret_cast<P2*>(col + st_pair), pr);
-                    else if (po[0]) __stcs(reinterpret_cast<T*>(col + st_pair), x.v[0]);
+                using P2 = typename Pair<T>::type;
+                P2 pr;
+                pr.x = x.v[0]; pr.y = x.v[1];
+                if (po[1]) __stcs(reinterpret_cast<P2*>(col + st_pair), pr);
+                else if (po[0]) __stcs(reinterpret_cast<T*>(col + st_pair), x.v[0]);
+                if constexpr (L == 3) {
                     if (po[2]) __stcs(reinterpret_cast<T*>(col + st_single), x.v[2]);
                 }
             };
@@ -477,7 +483,8 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
             // columns this patch shares with the steps s-1 .. s-D+1 were copied on THEIR barriers, and
             // copies of different steps land in any order: wait for the steps the record names
             {
-                const uint32_t mask = sl[kCcMaskWord];
+                uint32_t mask = sl[kCcMaskWord];
+                if constexpr (L == 2) mask |= __shfl_xor_sync(kFull, mask, 16);      // the warp waits for both patches' steps
 #pragma unroll
                 for (int r = 1; r < D; ++r)
                     if ((mask >> r) & 1u) mbar_wait(full_bar((s - r) % NB), (uint32_t)(((s - r) / NB) & 1), 3, s);
@@ -700,22 +707,24 @@ template <class T>
 int cc_slot_bytes(int nlev) { return (((nlev + 1) * (int)sizeof(T) + 15) & ~15); }
 
 template <class T>
-static size_t cc_fixed_smem(int mode) {
-    return kCcBarrierBytes + (size_t)kCcDepth * kCcGroup * cc_record_bytes<T>(mode);
+static size_t cc_fixed_smem(int mode, int L) {
+    return kCcBarrierBytes + (size_t)kCcDepth * cc_patches_per_step(L) * cc_record_bytes<T>(mode);
 }
 
 template <class T>
-int cc_max_slots(int slot_bytes, int smem_optin, int mode) {
-    const long avail = (long)smem_optin - (long)cc_fixed_smem<T>(mode) - kCcSlotTailPad;
+int cc_max_slots(int slot_bytes, int smem_optin, int mode, int nlev) {
+    const long avail = (long)smem_optin - (long)cc_fixed_smem<T>(mode, cc_levels_per_lane(nlev)) - kCcSlotTailPad;
     if (avail <= 0) return 0;
     return (int)(avail / slot_bytes);
 }
-template int cc_max_slots<double>(int, int, int);
-template int cc_max_slots<float>(int, int, int);
+template int cc_max_slots<double>(int, int, int, int);
+template int cc_max_slots<float>(int, int, int, int);
 template int cc_slot_bytes<double>(int);
 template int cc_slot_bytes<float>(int);
 
-int cc_levels_per_lane(int nlev) { return nlev + 1 <= 32 ? 1 : nlev + 1 <= 96 ? 3 : 0; }
+int cc_patches_per_step_for(int nlev) { return cc_patches_per_step(cc_levels_per_lane(nlev)); }
+int cc_levels_per_lane(int nlev);
+int cc_levels_per_lane(int nlev) { return nlev + 1 <= 32 ? 2 : nlev + 1 <= 96 ? 3 : 0; }
 
 namespace {
 template <class T, int L, int MODE>
@@ -759,12 +768,12 @@ int launch_tendencies_cc(const icon_grid& g, DevCcTables<T>& p, int mode, int nl
     const unsigned long long per_launch = (unsigned long long)n_barriers * (unsigned long long)p.n_ctas;
     if ((mode == kCcDivVort) != p.dv || (mode == kCcDivVort) != (ddt_vn == nullptr) || (mode == kCcTend) != (div == nullptr))
         return -(int)cudaErrorInvalidValue;
-    const size_t smem = cc_fixed_smem<T>(mode) + (size_t)p.n_slots * p.slot_bytes + kCcSlotTailPad;
+    const size_t smem = cc_fixed_smem<T>(mode, L) + (size_t)p.n_slots * p.slot_bytes + kCcSlotTailPad;
     cudaError_t err = cudaErrorInvalidValue;
 #define CC_ONE(LL, MM) \
     if (L == LL && mode == MM) \
         err = cc_launch_one<T, LL, MM>(d, g.device, p.n_ctas, smem, nlev, (int)ldk, (int)ldk_w, abc, vn, w, ddt_vn, div, vort, p.progress, per_launch, pace_mask, pace_last, s);
-    CC_ONE(1, kCcTend) CC_ONE(1, kCcStep) CC_ONE(1, kCcDivVort) CC_ONE(3, kCcTend) CC_ONE(3, kCcStep) CC_ONE(3, kCcDivVort)
+    CC_ONE(2, kCcTend) CC_ONE(2, kCcStep) CC_ONE(2, kCcDivVort) CC_ONE(3, kCcTend) CC_ONE(3, kCcStep) CC_ONE(3, kCcDivVort)
 #undef CC_ONE
     return err == cudaSuccess ? 1 : -(int)err;
 }
