@@ -210,6 +210,15 @@ int dycore_step(const icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, c
                 const void* vn, const void* w, void* ddt_vn, void* div, void* vort, void* cuda_stream);
 
 /*
+ * dycore_step_w -- dycore_step plus the vertical-wind tendency of dycore_w_tendency from the SAME pass: where the
+ * column-cache kernel runs, ddt_w of a patch's four cells is a by-product of the nine vn columns the patch holds in
+ * registers anyway and ten w columns (seven of them already in the column cache for ddt_vn): one kernel writes all four
+ * outputs. Elsewhere it is dycore_step followed by dycore_w_tendency. Argument rules of both.
+ */
+int dycore_step_w(const icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
+                  const void* vn, const void* w, void* ddt_vn, void* div, void* vort, void* ddt_w, void* cuda_stream);
+
+/*
  * dycore_step_host -- dycore_step with HOST field buffers (the end-to-end leg of bench.py): copies vn and w to
  * device staging buffers, runs dycore_step (one fused kernel where the column-cache kernel runs), copies ddt_vn, div
  * and vort back, and synchronises. This is NOT how the paper runs the model (fields stay resident on the GPU,

@@ -29,7 +29,7 @@ TABLE_ID = {n: i for i, n in enumerate(TABLES)}
 # every symbol include/icon_dycore.h declares
 EXPORTS = ("icon_grid_create", "icon_grid_destroy", "icon_grid_counts", "icon_grid_table_host",
            "icon_grid_table_device", "icon_grid_set_option", "icon_grid_cc_schedule_check", "dycore_div_vort", "dycore_velocity_tendencies",
-           "dycore_step", "dycore_step_host", "dycore_w_tendency", "icon_grid_launch_count", "icon_last_error")
+           "dycore_step", "dycore_step_host", "dycore_step_w", "dycore_w_tendency", "icon_grid_launch_count", "icon_last_error")
 
 
 class IconError(RuntimeError):
@@ -73,6 +73,8 @@ def load_library():
     L.dycore_velocity_tendencies.argtypes = [P, ci, ci, ci, ci, P, P, P, P, P, P, P, P]
     L.dycore_w_tendency.restype = ci
     L.dycore_w_tendency.argtypes = [P, ci, ci, ci, ci, P, P, P, P, P]
+    L.dycore_step_w.restype = ci
+    L.dycore_step_w.argtypes = [P, ci, ci, ci, ci, P, P, P, P, P, P, P, P]
     L.dycore_step.restype = ci
     L.dycore_step.argtypes = [P, ci, ci, ci, ci, P, P, P, P, P, P, P]
     L.dycore_step_host.restype = ci
@@ -237,6 +239,17 @@ def dycore_step(grid, z_half, vn, w, ddt_vn, div, vort, nlev, stream=None):
                    ("div", div, grid.nc, "ldk"), ("vort", vort, grid.nv, "ldk")))
     _check(grid._L.dycore_step(grid._h, _dtype_of(vn), int(nlev), int(vn.shape[1]), int(w.shape[1]), _dptr(z), _dptr(vn),
                                _dptr(w), _dptr(ddt_vn), _dptr(div), _dptr(vort), _stream_ptr(stream)))
+
+
+def dycore_step_w(grid, z_half, vn, w, ddt_vn, div, vort, ddt_w, nlev, stream=None):
+    """dycore_step plus ddt_w [nc][ldk_w] (reading P-19) from the same pass (one fused kernel where the column cache runs)."""
+    z = np.ascontiguousarray(z_half, dtype=np.float64)
+    if z.size != nlev + 1:
+        raise ValueError("z_half must have nlev+1 entries")
+    _check_fields((("vn", vn, grid.ne, "ldk"), ("w", w, grid.nc, "ldk_w"), ("ddt_vn", ddt_vn, grid.ne, "ldk"),
+                   ("div", div, grid.nc, "ldk"), ("vort", vort, grid.nv, "ldk"), ("ddt_w", ddt_w, grid.nc, "ldk_w")))
+    _check(grid._L.dycore_step_w(grid._h, _dtype_of(vn), int(nlev), int(vn.shape[1]), int(w.shape[1]), _dptr(z), _dptr(vn),
+                                 _dptr(w), _dptr(ddt_vn), _dptr(div), _dptr(vort), _dptr(ddt_w), _stream_ptr(stream)))
 
 
 def dycore_step_host(grid, z_half, vn_host, w_host, ddt_vn_host, div_host, vort_host, nlev):

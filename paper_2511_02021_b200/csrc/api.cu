@@ -192,16 +192,16 @@ constexpr int cc_record_size(int mode) { return icon::cc_coef_words(mode) * (int
 // Returns ICON_OK with p.unsupported set when this (T, nlev) cannot use the kernel (the caller
 // then uses the self-contained patch kernel).
 template <class T>
-int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev, int64_t ldk, int64_t ldk_w, bool dv = false) {
+int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev, int64_t ldk, int64_t ldk_w, int mode = icon::kCcStep) {
     const int tile = g->options[ICON_OPT_CC_TILE];
-    const int mode = dv ? icon::kCcDivVort : icon::kCcStep;
+    const bool dv = mode == icon::kCcDivVort;
     if (p.nlev == nlev && p.ldk == ldk && p.ldk_w == ldk_w && p.tile == tile && (p.ready || p.unsupported))
         return ICON_OK;
     dev_release(g, p.steps); dev_release(g, p.loads); dev_release(g, p.records);
     dev_release(g, p.cta_patch_begin); dev_release(g, p.cta_step_begin); dev_release(g, p.progress);
     p = icon::DevCcTables<T>();
     p.nlev = nlev;
-    p.ldk = ldk; p.ldk_w = ldk_w; p.tile = tile; p.dv = dv;
+    p.ldk = ldk; p.ldk_w = ldk_w; p.tile = tile; p.built_for = mode;
     const icon::CcGeometry geom = cc_geometry<T>(nlev, ldk, ldk_w, dv);
     const int slot_bytes = geom.slot_bytes;
     const int n_slots_max = icon::cc_max_slots<T>(slot_bytes, g->smem_optin, mode, nlev);
@@ -218,7 +218,7 @@ int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev, int64_t ld
     const size_t rb = (size_t)cc_record_size<T>(mode);
     const int ncoef = icon::cc_coef_words(mode);
     try {
-        std::string err = icon::build_cc_schedule(sc, g->num_sms, n_slots, geom, icon::cc_patches_per_step_for(nlev), icon::kCcDepth, tile, icon::cc_use_mask(mode), cs);
+        std::string err = icon::build_cc_schedule(sc, g->num_sms, n_slots, geom, icon::cc_patches_per_step_for(nlev, (int)sizeof(T), mode), icon::kCcDepth, tile, icon::cc_use_mask(mode), cs);
         if (!err.empty()) {
             p.unsupported = true;
             return ICON_OK;
@@ -235,7 +235,7 @@ int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev, int64_t ld
                 for (int i = 0; i < 20; ++i) cf[icon::DVF_ROT + i] = (T)scf[icon::SCF_ROT + i];
                 for (int i = 0; i < 20; ++i) cf[icon::DVF_XROT + i] = (T)(i < 18 ? scf[icon::SCF_XROT + i] : 0.0);
             } else {
-                for (int i = 0; i < icon::kScCoefWords; ++i) cf[i] = (T)scf[i];
+                for (int i = 0; i < ncoef; ++i) cf[i] = (T)scf[i];      // kCcStepW: with the twelve advection coefficients
             }
             int32_t* oid = reinterpret_cast<int32_t*>(r + (size_t)ncoef * sizeof(T));
             const int32_t* id = &sc.ids[(size_t)src * icon::kScIdWords];
@@ -645,18 +645,18 @@ int icon_grid_cc_schedule_check(const icon_grid_t* gc, int dtype, int nlev, int 
     icon::CcSchedule cs;
     icon::CcGeometry geom;
     try {
-        // the schedule of dycore_div_vort (27 vn columns per patch, compact records) first, then the one of the tendency /
-        // fused step, whose shape is reported
-        for (int mode : {(int)icon::kCcDivVort, (int)icon::kCcStep}) {
+        // the schedules of dycore_div_vort (27 vn columns per patch, compact records) and of dycore_step_w (all 46 columns)
+        // first, then the one of the tendency / fused step, whose shape is reported
+        for (int mode : {(int)icon::kCcDivVort, (int)icon::kCcStepW, (int)icon::kCcStep}) {
             const bool dv = mode == icon::kCcDivVort;
             geom = f64 ? cc_geometry<double>(nlev, ldk, ldk_w, dv) : cc_geometry<float>(nlev, ldk, ldk_w, dv);
             const int n_slots = std::min(65535, f64 ? icon::cc_max_slots<double>(geom.slot_bytes, smem_bytes, mode, nlev)
                                                     : icon::cc_max_slots<float>(geom.slot_bytes, smem_bytes, mode, nlev));
-            std::string err = icon::build_cc_schedule(g->sc_host, n_ctas, n_slots, geom, icon::cc_patches_per_step_for(nlev), icon::kCcDepth,
+            std::string err = icon::build_cc_schedule(g->sc_host, n_ctas, n_slots, geom, icon::cc_patches_per_step_for(nlev, f64 ? 8 : 4, mode), icon::kCcDepth,
                                                       g->options[ICON_OPT_CC_TILE], icon::cc_use_mask(mode), cs);
             if (!err.empty()) return fail(ICON_EUNSUPPORTED, err);
             err = icon::check_cc_schedule(g->sc_host, cs, g->host.ne, g->host.nc);
-            if (!err.empty()) return fail(ICON_EINVAL, err + (dv ? " (div/vort schedule)" : ""));
+            if (!err.empty()) return fail(ICON_EINVAL, err + (dv ? " (div/vort schedule)" : mode == icon::kCcStepW ? " (step + ddt_w schedule)" : ""));
         }
     } catch (const std::bad_alloc&) {
         return fail(ICON_ENOMEM, "out of host memory while building the column-cache schedule");
@@ -684,7 +684,7 @@ int dycore_div_vort(const icon_grid_t* gc, int dtype, int nlev, int ldk, const v
     // the gather kernel through L1
     const bool want_cc = g->options[ICON_OPT_TENDENCY_KERNEL] >= 4 && nlev >= 2;
     if (dtype == ICON_F64) {
-        if (want_cc && (rc = ensure_cc_tables(g, g->dv64, nlev, ldk, ldk, true))) return rc;
+        if (want_cc && (rc = ensure_cc_tables(g, g->dv64, nlev, ldk, ldk, icon::kCcDivVort))) return rc;
         if (want_cc && !g->dv64.unsupported) {
             n = icon::launch_tendencies_cc<double>(*g, g->dv64, icon::kCcDivVort, nlev, ldk, ldk, nullptr, (const double*)vn, nullptr, nullptr,
                                                    (double*)div, (double*)vort, s);
@@ -693,7 +693,7 @@ int dycore_div_vort(const icon_grid_t* gc, int dtype, int nlev, int ldk, const v
             n = icon::launch_div_vort<double>(*g, g->c64, nlev, ldk, (const double*)vn, (double*)div, (double*)vort, s);
         }
     } else {
-        if (want_cc && (rc = ensure_cc_tables(g, g->dv32, nlev, ldk, ldk, true))) return rc;
+        if (want_cc && (rc = ensure_cc_tables(g, g->dv32, nlev, ldk, ldk, icon::kCcDivVort))) return rc;
         if (want_cc && !g->dv32.unsupported) {
             n = icon::launch_tendencies_cc<float>(*g, g->dv32, icon::kCcDivVort, nlev, ldk, ldk, nullptr, (const float*)vn, nullptr, nullptr,
                                                   (float*)div, (float*)vort, s);
@@ -800,6 +800,61 @@ int dycore_step(const icon_grid_t* gc, int dtype, int nlev, int ldk, int ldk_w, 
                                     nullptr, nullptr, s, div, vort, &fused);
     if (rc || fused) return rc;
     return dycore_div_vort(g, dtype, nlev, ldk, vn, div, vort, cuda_stream);
+}
+
+int dycore_step_w(const icon_grid_t* gc, int dtype, int nlev, int ldk, int ldk_w, const double* z_half, const void* vn, const void* w,
+                  void* ddt_vn, void* div, void* vort, void* ddt_w, void* cuda_stream) {
+    icon_grid* g = const_cast<icon_grid*>(gc);
+    int rc = check_common(g, dtype, nlev, ldk, 2);
+    if (rc) return rc;
+    const size_t es = dtype == ICON_F64 ? 8 : 4;
+    if (ldk_w < nlev + 1) return fail(ICON_EINVAL, "ldk_w < nlev + 1");
+    if (((int64_t)ldk_w * (int64_t)es) % 16) return fail(ICON_EINVAL, "ldk_w*sizeof(T) must be a multiple of 16");
+    if (!z_half) return fail(ICON_EINVAL, "z_half is NULL");
+    if ((rc = check_field(vn, "vn")) || (rc = check_field(w, "w")) || (rc = check_field(ddt_vn, "ddt_vn")) ||
+        (rc = check_field(div, "div")) || (rc = check_field(vort, "vort")) || (rc = check_field(ddt_w, "ddt_w")))
+        return rc;
+    {
+        const size_t be = (size_t)g->host.ne * ldk * es, bc = (size_t)g->host.nc * ldk * es, bv = (size_t)g->host.nv * ldk * es,
+                     bw = (size_t)g->host.nc * ldk_w * es;
+        const void* outs[4] = {ddt_vn, div, vort, ddt_w};
+        const size_t ob[4] = {be, bc, bv, bw};
+        for (int i = 0; i < 4; ++i) {
+            if (overlaps(outs[i], ob[i], vn, be) || overlaps(outs[i], ob[i], w, bw))
+                return fail(ICON_EINVAL, "outputs must not alias inputs or each other");
+            for (int j = 0; j < i; ++j)
+                if (overlaps(outs[i], ob[i], outs[j], ob[j])) return fail(ICON_EINVAL, "outputs must not alias inputs or each other");
+        }
+    }
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const bool want_cc = g->options[ICON_OPT_TENDENCY_KERNEL] >= 4;
+    void *abc = nullptr, *wk = nullptr;
+    if ((rc = get_level_coeffs(g, dtype, nlev, z_half, &abc, &wk))) return rc;
+    int n = 0;
+    bool done = false;
+    if (want_cc && dtype == ICON_F64) {
+        if ((rc = ensure_cc_tables(g, g->sw64, nlev, ldk, ldk_w, icon::kCcStepW))) return rc;
+        if (!g->sw64.unsupported) {
+            n = icon::launch_tendencies_cc<double>(*g, g->sw64, icon::kCcStepW, nlev, ldk, ldk_w, (const double*)abc, (const double*)vn, (const double*)w,
+                                                   (double*)ddt_vn, (double*)div, (double*)vort, s, (const double*)wk, (double*)ddt_w);
+            done = true;
+        }
+    } else if (want_cc) {
+        if ((rc = ensure_cc_tables(g, g->sw32, nlev, ldk, ldk_w, icon::kCcStepW))) return rc;
+        if (!g->sw32.unsupported) {
+            n = icon::launch_tendencies_cc<float>(*g, g->sw32, icon::kCcStepW, nlev, ldk, ldk_w, (const float*)abc, (const float*)vn, (const float*)w,
+                                                  (float*)ddt_vn, (float*)div, (float*)vort, s, (const float*)wk, (float*)ddt_w);
+            done = true;
+        }
+    }
+    if (done) {
+        if (n < 0) return fail_cuda((cudaError_t)(-n), "kernel launch");
+        g->launches += n;
+        return ICON_OK;
+    }
+    // level counts the column cache cannot hold, or another tendency kernel selected: the separate calls
+    if ((rc = dycore_step(gc, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, div, vort, cuda_stream))) return rc;
+    return dycore_w_tendency(gc, dtype, nlev, ldk, ldk_w, z_half, vn, w, ddt_w, cuda_stream);
 }
 
 int dycore_step_host(const icon_grid_t* gc, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,

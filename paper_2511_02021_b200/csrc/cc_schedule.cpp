@@ -9,7 +9,7 @@
 namespace icon {
 namespace {
 
-constexpr int kRefs = SID_PAD;            // 43 columns per patch: 36 vn, then 7 w
+constexpr int kRefs = SID_PAD;            // 46 column slots per patch: 36 vn, then 10 w (the use mask says which a mode reads)
 constexpr int kFirstCell = SID_T0;        // id slots >= this are cell (w) columns
 constexpr int32_t kNever = 0x7fffffff;
 

@@ -41,8 +41,13 @@ constexpr int kCcWarps = 8, kCcGroup = 4, kCcDepth = 3;
 //   L = 3 (33 <= nlev+1 <= 96): one patch per warp, a lane owns levels 2*lane, 2*lane+1 and 64+lane;
 //   L = 2 (nlev+1 <= 32): TWO patches per warp, one per half-warp, a lane owns levels 2*(lane%16), 2*(lane%16)+1 --
 //         a step is then 8 patches, and every per-patch cost of a warp (coefficient and slot lookups, waits, address
-//         arithmetic) is paid once per two patches.
-CC_HD constexpr int cc_patches_per_warp(int L) { return L == 2 ? 2 : 1; }
+//         arithmetic) is paid once per two patches;
+//   L = 6 (4-byte columns, 33 <= nlev+1 <= 96, div / vort mode only): two patches per warp as well, a lane owns the
+//         three pairs 32*p + 2*(lane%16), +1 (p = 0, 1, 2). Measured at config 4: div_vort 2.08 -> 1.69 ms and the
+//         tendency alone 2.86 -> 2.37 ms, but the fused step 3.39 -> 3.61 ms (the consumers hold per-half ids and
+//         pointers besides six values per column and spill 100 bytes at 216 registers; with four producer warps and 232
+//         registers everything was slower). The tendency shares its schedule with the fused step, so both keep L = 3.
+CC_HD constexpr int cc_patches_per_warp(int L) { return L == 2 || L == 6 ? 2 : 1; }
 CC_HD constexpr int cc_patches_per_step(int L) { return kCcGroup * cc_patches_per_warp(L); }
 // Producer warps are added to the consumers; the CTA is launched with the registers of the average warp and
 // re-balances them with setmaxnreg: producers keep CcWarps::producer_regs, consumers grow to CcWarps::consumer_regs
@@ -62,15 +67,16 @@ constexpr int kCcMaxProducers = 8;
 constexpr int kCcAhead = 3;              // steps the producers read the schedule ahead; `loads` is padded for it
 constexpr int kCcBarrierBytes = 512;    // the mbarriers
 // What a launch of the kernel produces; each mode has a schedule of its own (DevCcTables::mode).
-enum { kCcTend = 0 /* ddt_vn */, kCcStep = 1 /* ddt_vn + div + vort */, kCcDivVort = 2 /* div + vort only */ };
+enum { kCcTend = 0 /* ddt_vn */, kCcStep = 1 /* ddt_vn + div + vort */, kCcDivVort = 2 /* div + vort only */,
+       kCcStepW = 3 /* ddt_vn + div + vort + ddt_w (P-19): three more w columns and twelve more coefficients per patch */ };
 // kCcDivVort reads 27 of the 36 vn columns of a patch and no w column, and its records carry only the 52 coefficients it
 // needs: geofac_div [4][3], rot of the midpoints [3][6] (+2 pad), rot of the corners [3][6] (+2 pad)
 enum { DVF_DIV = 0, DVF_ROT = 12, DVF_XROT = 32, kCcDvCoefWords = 52 };
-CC_HD constexpr int cc_coef_words(int mode) { return mode == kCcDivVort ? (int)kCcDvCoefWords : (int)kScCoefWords; }
+CC_HD constexpr int cc_coef_words(int mode) { return mode == kCcDivVort ? (int)kCcDvCoefWords : mode == kCcStepW ? (int)kScCoefWords : (int)SCF_ADV; }
 // id slots (sc_tables.hpp) a mode reads: bit i of the mask = column i of the patch is needed
 constexpr uint64_t cc_use_mask(int mode) {
-    uint64_t all = (1ull << SID_PAD) - 1;
-    if (mode != kCcDivVort) return all;
+    if (mode == kCcStepW) return (1ull << SID_PAD) - 1;                  // every column
+    if (mode != kCcDivVort) return (1ull << SID_XW0) - 1;                // 36 vn + 7 w: all but X1 X3 X5
     uint64_t m = (1ull << SID_X0) - 1;                                   // i0..i2, b0..b5, om0..om5, oc0..oc5
     for (int x = 0; x < 3; ++x) m |= 3ull << (SID_X0 + 5 * x + 3);       // n1, n2 of the three corners
     return m;
@@ -78,8 +84,8 @@ constexpr uint64_t cc_use_mask(int mode) {
 // a patch record on the device = kScCoefWords coefficients (T), then kCcRecordIds int32 (user ids of
 // the outputs), then kCcSlotWords uint32 byte offsets of the slots; c_lin is
 // stored halved there (the kernel forms w(k) + w(k+1) = 2 w_f(k))
-constexpr int kCcSlotWords = 48;     // per patch: 43 slots (order of sc_tables.hpp id slots), mask, pad
-constexpr int kCcMaskWord = 43;      // bit r set: one of the 43 columns was loaded by step s-r (0 < r < depth)
+constexpr int kCcSlotWords = 48;     // per patch: 46 slots (order of sc_tables.hpp id slots), mask, pad
+constexpr int kCcMaskWord = 46;      // bit r set: one of the patch's columns was loaded by step s-r (0 < r < depth)
 constexpr int kCcRecordIds = 16;     // int32: owned edges i0 i1 i2 b0 b2 b4, cells T0..T3, owned vertices ab bc ca a b c (-1 = not ours)
 constexpr int kCcRecordTail = 4 * kCcRecordIds + 4 * kCcSlotWords;
 // lanes past the end of a column read up to 3 * 32 levels * 8 bytes beyond their slot: readable pad after the last slot

@@ -67,7 +67,7 @@ struct DevCcTables {
     int nlev = -1;                 // the level count the slot size was derived from
     int64_t ldk = -1, ldk_w = -1;  // column strides the runs were merged for
     int tile = -1;                 // ICON_OPT_CC_TILE it was built with
-    bool dv = false;               // built for kCcDivVort (27 vn columns, compact records) instead of the tendency modes
+    int built_for = 1;             // kCcStep (serves kCcTend too), kCcDivVort (27 vn columns, compact records) or kCcStepW (+3 w columns)
     unsigned long long* progress = nullptr;   // device counter of the producers' pacing barriers, never reset
     int64_t min_steps = 0;         // steps of the CTA with the fewest (pacing barriers every CTA reaches)
     bool ready = false;
@@ -117,6 +117,8 @@ struct icon_grid {
     icon::DevCcTables<float> cc32;
     icon::DevCcTables<double> dv64;                    // the same for dycore_div_vort (mode kCcDivVort)
     icon::DevCcTables<float> dv32;
+    icon::DevCcTables<double> sw64;                    // the same for dycore_step_w (mode kCcStepW)
+    icon::DevCcTables<float> sw32;
     int smem_optin = 0;                                // cudaDevAttrMaxSharedMemoryPerBlockOptin
     std::vector<icon::LevelCoeffs> level_coeffs;
     icon::Workspace ws;

@@ -37,7 +37,8 @@ int launch_tendencies_sc(const icon_grid& g, const DevScTables<T>& p, int nlev, 
 // kCcStep (ddt_vn + div + vort in one pass: dycore_step) or kCcDivVort (div + vort only, tables built for that mode).
 template <class T>
 int launch_tendencies_cc(const icon_grid& g, DevCcTables<T>& p, int mode, int nlev, int64_t ldk, int64_t ldk_w,
-                         const T* abc, const T* vn, const T* w, T* ddt_vn, T* div, T* vort, cudaStream_t s);
+                         const T* abc, const T* vn, const T* w, T* ddt_vn, T* div, T* vort, cudaStream_t s,
+                         const T* wk = nullptr, T* ddt_w = nullptr);
 // shape helpers of that kernel: level mapping (values a lane holds per column; 0 = nlev not supported), bytes of one w column
 // (the smallest possible slot), and how many slots of `slot_bytes` fit beside the fixed buffers in `smem_optin` bytes of shared memory
 int cc_levels_per_lane(int nlev);
@@ -45,6 +46,7 @@ template <class T>
 int cc_slot_bytes(int nlev);
 template <class T>
 int cc_max_slots(int slot_bytes, int smem_optin, int mode, int nlev);
-int cc_patches_per_step_for(int nlev);
+int cc_patches_per_step_for(int nlev, int elem_bytes, int mode);
+int cc_level_mapping(int nlev, int elem_bytes, int mode);     // template parameter L of the kernel for this level count, element size and mode
 
 }  // namespace icon

@@ -142,6 +142,7 @@ struct CcDev {
 // ---- the L levels of one column a lane owns ---------------------------------------------------------
 // L == 3: v[0], v[1] = levels 2*lane, 2*lane+1 (one 16-byte access), v[2] = level 64+lane.
 // L == 2: v[0], v[1] = levels 2*(lane%16), 2*(lane%16)+1 of the half-warp's own patch.
+// L == 6: v[2p], v[2p+1] = levels 32*p + 2*(lane%16), +1 of the half-warp's own patch (p = 0, 1, 2).
 template <class T, int L>
 struct Col {
     T v[L];
@@ -149,7 +150,9 @@ struct Col {
 #define FORL _Pragma("unroll") for (int l = 0; l < L; ++l)
 
 template <int L>
-__device__ __forceinline__ int level_of(int lane, int l) { return L == 2 ? 2 * (lane & 15) + l : (l < 2 ? 2 * lane + l : 64 + lane); }
+__device__ __forceinline__ int level_of(int lane, int l) {
+    return L == 2 ? 2 * (lane & 15) + l : L == 6 ? 32 * (l >> 1) + 2 * (lane & 15) + (l & 1) : (l < 2 ? 2 * lane + l : 64 + lane);
+}
 
 template <class T> struct Pair;
 template <> struct Pair<double> { using type = double2; };
@@ -165,6 +168,15 @@ __device__ __forceinline__ Col<T, L> level_up(const Col<T, L>& a, int lane) {
     if constexpr (L == 2) {
         r.v[0] = __shfl_up_sync(kFull, a.v[1], 1, 16);        // inside the half-warp
         r.v[1] = a.v[0];
+    } else if constexpr (L == 6) {
+        // rotate right by one inside the half-warp; its last lane hands the end of the PREVIOUS pair segment to lane 0
+        const int src = ((lane + 15) & 15) | (lane & 16);
+        const bool last = (lane & 15) == 15;
+#pragma unroll
+        for (int p = 0; p < 3; ++p) {
+            r.v[2 * p] = __shfl_sync(kFull, last && p > 0 ? a.v[2 * p - 1] : a.v[2 * p + 1], src);
+            r.v[2 * p + 1] = a.v[2 * p];
+        }
     } else {
         r.v[0] = __shfl_up_sync(kFull, a.v[1], 1);
         r.v[1] = a.v[0];
@@ -178,6 +190,15 @@ __device__ __forceinline__ Col<T, L> level_down(const Col<T, L>& a, int lane) {
     if constexpr (L == 2) {
         r.v[0] = a.v[1];
         r.v[1] = __shfl_down_sync(kFull, a.v[0], 1, 16);
+    } else if constexpr (L == 6) {
+        // rotate left by one inside the half-warp; its first lane hands the start of the NEXT pair segment to lane 15
+        const int src = ((lane + 1) & 15) | (lane & 16);
+        const bool first = (lane & 15) == 0;
+#pragma unroll
+        for (int p = 0; p < 3; ++p) {
+            r.v[2 * p] = a.v[2 * p + 1];
+            r.v[2 * p + 1] = __shfl_sync(kFull, first && p < 2 ? a.v[2 * p + 2] : a.v[2 * p], src);
+        }
     } else {
         r.v[0] = a.v[1];
         r.v[1] = __shfl_sync(kFull, lane == 0 ? a.v[2] : a.v[0], (lane + 1) & 31);
@@ -248,12 +269,13 @@ template <class T, int L, int MODE>
 __global__ void __launch_bounds__((kCcWarps + CcWarps<T, L>::producers) * 32, 1)
 k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, const T* __restrict__ vn,
           const T* __restrict__ w, T* __restrict__ ddt_vn, T* __restrict__ div, T* __restrict__ vort,
-          unsigned long long* pace_counter, unsigned long long pace_per_launch, int pace_mask, int pace_last) {
+          unsigned long long* pace_counter, unsigned long long pace_per_launch, int pace_mask, int pace_last,
+          const T* __restrict__ wk, T* __restrict__ ddt_w) {
     extern __shared__ __align__(128) unsigned char smem[];
     using C = Col<T, L>;
     constexpr int W = kCcWarps, G = kCcGroup, D = kCcDepth;
     constexpr int PPW = cc_patches_per_warp(L), PPS = G * PPW;      // patches per warp, per step
-    constexpr bool FUSED = MODE != kCcTend, DVONLY = MODE == kCcDivVort;
+    constexpr bool FUSED = MODE != kCcTend, DVONLY = MODE == kCcDivVort, WTEND = MODE == kCcStepW;
     constexpr int kCcProducers = CcWarps<T, L>::producers;
     constexpr int REC = cc_record_bytes<T>(MODE), COEF = cc_coef_words(MODE);
     constexpr int NGRP = W / G;
@@ -303,7 +325,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
         // the next multiple before every CTA, this one included, has added all of its events). Kept on the device so
         // that a captured CUDA graph replays correctly.
         unsigned long long pace_base = 0;
-        if (MODE == kCcStep && !CcWarps<T, L>::light && pace_mask && lane == 0) {
+        if ((MODE == kCcStep || MODE == kCcStepW) && !CcWarps<T, L>::light && pace_mask && lane == 0) {
             unsigned long long have;
             asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(have) : "l"(pace_counter) : "memory");
             pace_base = have - have % pace_per_launch;
@@ -339,7 +361,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
                     // compiled into the fused fp64 three-levels-per-lane kernel only: the tendency-only kernel lost 3 %
                     // to the mere presence of this block, and the light instantiations (fp32, one level per lane)
                     // slowed down by 40-50 % with the barrier active
-                    if (MODE == kCcStep && !CcWarps<T, L>::light && pace_mask && s && (s & pace_mask) == 0 && s <= pace_last) {
+                    if ((MODE == kCcStep || MODE == kCcStepW) && !CcWarps<T, L>::light && pace_mask && s && (s & pace_mask) == 0 && s <= pace_last) {
                         // every pace_mask + 1 steps the producers of all CTAs meet (bounded wait: pacing is an
                         // optimisation, never a condition for progress): SMs run at slightly different rates, and once
                         // the CTAs are rounds apart neighbouring tiles no longer share their halo columns through the L2
@@ -415,8 +437,20 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
         cB[l] = !DVONLY && po[l] ? __ldg(abc + nlev + k) : (T)0;
         cC[l] = !DVONLY && po[l] ? __ldg(abc + 2 * nlev + k) : (T)0;
     }
-    const uint64_t cs = (uint64_t)ldk * sizeof(T);
-    const int hl = L == 2 ? lane & 15 : lane, half = L == 2 ? lane >> 4 : 0;      // lane inside its patch, patch of the warp
+    // vertical-wind tendency (mode kCcStepW, P-19): weight of vn(k) in vn_ie(k), 1 / (z_half[k-1] - z_half[k+1]) (both 0
+    // outside the interior half levels 1 .. nlev-1, so that ddt_w comes out 0 at the top and the surface) and the half
+    // levels that exist in a w / ddt_w column
+    T wg[L], wrdz[L];
+    bool pow_[L], w_int[L];
+    FORL {
+        const int k = level_of<L>(lane, l);
+        pow_[l] = WTEND && k <= nlev;
+        w_int[l] = WTEND && k >= 1 && k <= nlev - 1;
+        wg[l] = w_int[l] ? __ldg(wk + k) : (T)0;
+        wrdz[l] = w_int[l] ? __ldg(wk + nlev + 1 + k) : (T)0;
+    }
+    const uint64_t cs = (uint64_t)ldk * sizeof(T), cs_wout = (uint64_t)ldk_w * sizeof(T);
+    const int hl = PPW == 2 ? lane & 15 : lane, half = PPW == 2 ? lane >> 4 : 0;      // lane inside its patch, patch of the warp
     // this lane's two read positions inside every slot
     const unsigned char* my_pair = slot_base + 2 * hl * (int)sizeof(T);
     const unsigned char* my_single = slot_base + (64 + lane) * (int)sizeof(T);
@@ -431,8 +465,8 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
             // repeats the first one's reads and arithmetic and stores nothing
             const bool live = p_first + half < pe;
             const int my_patch = wi * PPW + (live ? half : 0);
-            if constexpr (L == 2) {
-                if (!live) { FORL po[l] = false; }
+            if constexpr (PPW == 2) {
+                if (!live) { FORL { po[l] = false; pow_[l] = false; } }
             }
             const unsigned char* rec = rec_base + ((s % D) * PPS + my_patch) * REC;
             const T* cf = reinterpret_cast<const T*>(rec);
@@ -445,9 +479,15 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
             auto LD = [&](uint32_t off) {
                 CC_ASSERT(off % 16 == 0 && off + 96 * sizeof(T) <= (uint32_t)d.n_slots * (uint32_t)d.slot_bytes + kCcSlotTailPad, "slot offset", off, d.n_slots);
                 C c;
-                const typename Pair<T>::type pr = *reinterpret_cast<const typename Pair<T>::type*>(my_pair + off);
+                using P2 = typename Pair<T>::type;
+                const P2 pr = *reinterpret_cast<const P2*>(my_pair + off);
                 c.v[0] = pr.x; c.v[1] = pr.y;
                 if constexpr (L == 3) c.v[2] = *reinterpret_cast<const T*>(my_single + off);
+                if constexpr (L == 6) {
+                    const P2 p1 = *reinterpret_cast<const P2*>(my_pair + off + 32 * sizeof(T));
+                    const P2 p2 = *reinterpret_cast<const P2*>(my_pair + off + 64 * sizeof(T));
+                    c.v[2] = p1.x; c.v[3] = p1.y; c.v[4] = p2.x; c.v[5] = p2.y;
+                }
                 return c;
             };
             auto WS = [&](uint32_t off) {       // w(k) + w(k+1) = 2 w_f(k) (S6); the 1/2 is folded into c_lin
@@ -478,13 +518,21 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
                 if constexpr (L == 3) {
                     if (po[2]) __stcs(reinterpret_cast<T*>(col + st_single), x.v[2]);
                 }
+                if constexpr (L == 6) {
+#pragma unroll
+                    for (int q = 1; q < 3; ++q) {
+                        pr.x = x.v[2 * q]; pr.y = x.v[2 * q + 1];
+                        if (po[2 * q + 1]) __stcs(reinterpret_cast<P2*>(col + st_pair + 32 * q * sizeof(T)), pr);
+                        else if (po[2 * q]) __stcs(reinterpret_cast<T*>(col + st_pair + 32 * q * sizeof(T)), x.v[2 * q]);
+                    }
+                }
             };
 
             // columns this patch shares with the steps s-1 .. s-D+1 were copied on THEIR barriers, and
             // copies of different steps land in any order: wait for the steps the record names
             {
                 uint32_t mask = sl[kCcMaskWord];
-                if constexpr (L == 2) mask |= __shfl_xor_sync(kFull, mask, 16);      // the warp waits for both patches' steps
+                if constexpr (PPW == 2) mask |= __shfl_xor_sync(kFull, mask, 16);      // the warp waits for both patches' steps
 #pragma unroll
                 for (int r = 1; r < D; ++r)
                     if ((mask >> r) & 1u) mbar_wait(full_bar((s - r) % NB), (uint32_t)(((s - r) / NB) & 1), 3, s);
@@ -516,6 +564,60 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
                 ST(div, ido[8], dv);
                 FORL dv.v[l] = gd[9] * vI[1].v[l] + gd[10] * vI[2].v[l] + gd[11] * vI[0].v[l];
                 ST(div, ido[9], dv);
+            }
+            if constexpr (WTEND) {
+                // ---- vertical-wind tendency of the four cells (P-19), while only the nine in-patch columns are live ----
+                // ddt_w(c,k) = -[ sum_j a(c,j) vn_ie(e_j,k) (w(cell across e_j,k) - w(c,k)) + w(c,k) (w(c,k-1) - w(c,k+1)) rdz2(k) ]
+                T av[12];
+                ld_coef(cf + SCF_ADV, av);
+                uint32_t sW[12];                    // T0..T3 X0 X2 X4 X1 X3 X5 + mask + pad
+                ld_slots(sl + SID_T0, sW);
+                C wT[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) wT[j] = LD(sW[j]);
+                auto VIE = [&](const C& x) {        // vn at the half level k: g_k vn(k) + (1 - g_k) vn(k-1); 0 outside 1 .. nlev-1
+                    const C up = level_up(x, lane);
+                    C o;
+                    FORL o.v[l] = w_int[l] ? wg[l] * x.v[l] + ((T)1 - wg[l]) * up.v[l] : (T)0;
+                    return o;
+                };
+                C acc[4];
+                {
+                    const C v0 = VIE(vI[0]), v1 = VIE(vI[1]), v2 = VIE(vI[2]);
+                    FORL {
+                        acc[3].v[l] = av[9] * v1.v[l] * (wT[1].v[l] - wT[3].v[l]) + av[10] * v2.v[l] * (wT[2].v[l] - wT[3].v[l]) +
+                                      av[11] * v0.v[l] * (wT[0].v[l] - wT[3].v[l]);
+                        acc[0].v[l] = av[1] * v0.v[l] * (wT[3].v[l] - wT[0].v[l]);
+                        acc[1].v[l] = av[5] * v1.v[l] * (wT[3].v[l] - wT[1].v[l]);
+                        acc[2].v[l] = av[6] * v2.v[l] * (wT[3].v[l] - wT[2].v[l]);
+                    }
+                }
+#pragma unroll
+                for (int j = 0; j < 6; ++j) {
+                    constexpr int cell_of[6] = {0, 1, 1, 2, 2, 0};
+                    constexpr int bslot[6] = {0, 3, 4, 7, 8, 2};
+                    constexpr int xslot[6] = {4, 7, 5, 8, 6, 9};      // X0 X1 X2 X3 X4 X5 inside sW
+                    const C wx = LD(sW[xslot[j]]);
+                    const C v = VIE(vB[j]);
+                    FORL acc[cell_of[j]].v[l] += av[bslot[j]] * v.v[l] * (wx.v[l] - wT[cell_of[j]].v[l]);
+                }
+#pragma unroll
+                for (int c4 = 0; c4 < 4; ++c4) {
+                    const C up = level_up(wT[c4], lane), dn = level_down(wT[c4], lane);
+                    C o;
+                    // the neighbours of the first and last half level do not exist (stale values): rdz2 is 0 there, select
+                    FORL o.v[l] = w_int[l] ? -(acc[c4].v[l] + wT[c4].v[l] * (up.v[l] - dn.v[l]) * wrdz[l]) : (T)0;
+                    const int32_t id = ido[6 + c4];
+                    unsigned char* col = reinterpret_cast<unsigned char*>(ddt_w) + (uint64_t)(uint32_t)id * cs_wout;
+                    using P2 = typename Pair<T>::type;
+                    P2 pr;
+                    pr.x = o.v[0]; pr.y = o.v[1];
+                    if (pow_[1]) __stcs(reinterpret_cast<P2*>(col + st_pair), pr);
+                    else if (pow_[0]) __stcs(reinterpret_cast<T*>(col + st_pair), o.v[0]);
+                    if constexpr (L == 3) {
+                        if (pow_[2]) __stcs(reinterpret_cast<T*>(col + st_single), o.v[2]);
+                    }
+                }
             }
             if constexpr (DVONLY) {
                 // ---- S2 alone: the six vorticities from the patch's own columns, the om / oc columns and n1, n2 -------
@@ -713,7 +815,7 @@ static size_t cc_fixed_smem(int mode, int L) {
 
 template <class T>
 int cc_max_slots(int slot_bytes, int smem_optin, int mode, int nlev) {
-    const long avail = (long)smem_optin - (long)cc_fixed_smem<T>(mode, cc_levels_per_lane(nlev)) - kCcSlotTailPad;
+    const long avail = (long)smem_optin - (long)cc_fixed_smem<T>(mode, cc_level_mapping(nlev, (int)sizeof(T), mode)) - kCcSlotTailPad;
     if (avail <= 0) return 0;
     return (int)(avail / slot_bytes);
 }
@@ -722,15 +824,18 @@ template int cc_max_slots<float>(int, int, int, int);
 template int cc_slot_bytes<double>(int);
 template int cc_slot_bytes<float>(int);
 
-int cc_patches_per_step_for(int nlev) { return cc_patches_per_step(cc_levels_per_lane(nlev)); }
-int cc_levels_per_lane(int nlev);
 int cc_levels_per_lane(int nlev) { return nlev + 1 <= 32 ? 2 : nlev + 1 <= 96 ? 3 : 0; }
+int cc_level_mapping(int nlev, int elem_bytes, int mode) {
+    const int l = cc_levels_per_lane(nlev);
+    return l == 3 && elem_bytes == 4 && mode == kCcDivVort ? 6 : l;
+}
+int cc_patches_per_step_for(int nlev, int elem_bytes, int mode) { return cc_patches_per_step(cc_level_mapping(nlev, elem_bytes, mode)); }
 
 namespace {
 template <class T, int L, int MODE>
 cudaError_t cc_launch_one(const CcDev<T>& d, int device, int n_ctas, size_t smem, int nlev, int ldk, int ldk_w, const T* abc,
                           const T* vn, const T* w, T* ddt_vn, T* div, T* vort, unsigned long long* pc, unsigned long long ppl,
-                          int pm, int pl, cudaStream_t s) {
+                          int pm, int pl, const T* wk, T* ddt_w, cudaStream_t s) {
     auto k = k_tend_cc<T, L, MODE>;
     // the opt-in for > 48 KB of dynamic shared memory is a per-DEVICE attribute of the function: remembered per device
     static std::mutex mu;
@@ -744,14 +849,14 @@ cudaError_t cc_launch_one(const CcDev<T>& d, int device, int n_ctas, size_t smem
             if (known) configured[device] = smem;
         }
     }
-    k<<<(unsigned)n_ctas, (kCcWarps + CcWarps<T, L>::producers) * 32, smem, s>>>(d, nlev, ldk, ldk_w, abc, vn, w, ddt_vn, div, vort, pc, ppl, pm, pl);
+    k<<<(unsigned)n_ctas, (kCcWarps + CcWarps<T, L>::producers) * 32, smem, s>>>(d, nlev, ldk, ldk_w, abc, vn, w, ddt_vn, div, vort, pc, ppl, pm, pl, wk, ddt_w);
     return cudaGetLastError();
 }
 }  // namespace
 
 template <class T>
 int launch_tendencies_cc(const icon_grid& g, DevCcTables<T>& p, int mode, int nlev, int64_t ldk, int64_t ldk_w,
-                         const T* abc, const T* vn, const T* w, T* ddt_vn, T* div, T* vort, cudaStream_t s) {
+                         const T* abc, const T* vn, const T* w, T* ddt_vn, T* div, T* vort, cudaStream_t s, const T* wk, T* ddt_w) {
     CcDev<T> d;
     d.steps = p.steps; d.loads = p.loads; d.records = p.records;
     d.cta_patch_begin = p.cta_patch_begin; d.cta_step_begin = p.cta_step_begin;
@@ -759,28 +864,33 @@ int launch_tendencies_cc(const icon_grid& g, DevCcTables<T>& p, int mode, int nl
     d.ne = g.host.ne; d.nc = g.host.nc; d.nv = g.host.nv;
     // pacing: a barrier of the producers every `period` steps (power of two), counted in p.progress (never reset)
     const int period = g.options[ICON_OPT_CC_PACE];
-    const int L = cc_levels_per_lane(nlev);
+    const int L = cc_level_mapping(nlev, (int)sizeof(T), mode);
     const bool heavy = sizeof(T) == 8 && L == 3;
-    int pace_mask = period > 0 && p.progress && mode == kCcStep && heavy ? period - 1 : 0;      // fused fp64 step only
+    int pace_mask = period > 0 && p.progress && (mode == kCcStep || mode == kCcStepW) && heavy ? period - 1 : 0;      // fused fp64 step only
     const int n_barriers = pace_mask ? (int)((p.min_steps - 1) / period) : 0;      // barriers every CTA reaches
     if (n_barriers == 0) pace_mask = 0;
     const int pace_last = n_barriers * period;
     const unsigned long long per_launch = (unsigned long long)n_barriers * (unsigned long long)p.n_ctas;
-    if ((mode == kCcDivVort) != p.dv || (mode == kCcDivVort) != (ddt_vn == nullptr) || (mode == kCcTend) != (div == nullptr))
+    // the tables must have been built for this mode (kCcTend runs on the tables of kCcStep: same columns, same records)
+    if ((mode == kCcTend ? (int)kCcStep : mode) != p.built_for || (mode == kCcDivVort) != (ddt_vn == nullptr) || (mode == kCcTend || mode == kCcDivVort ? false : div == nullptr) || (mode == kCcTend && div != nullptr) ||
+        (mode == kCcStepW) != (ddt_w != nullptr))
         return -(int)cudaErrorInvalidValue;
     const size_t smem = cc_fixed_smem<T>(mode, L) + (size_t)p.n_slots * p.slot_bytes + kCcSlotTailPad;
     cudaError_t err = cudaErrorInvalidValue;
 #define CC_ONE(LL, MM) \
     if (L == LL && mode == MM) \
-        err = cc_launch_one<T, LL, MM>(d, g.device, p.n_ctas, smem, nlev, (int)ldk, (int)ldk_w, abc, vn, w, ddt_vn, div, vort, p.progress, per_launch, pace_mask, pace_last, s);
-    CC_ONE(2, kCcTend) CC_ONE(2, kCcStep) CC_ONE(2, kCcDivVort) CC_ONE(3, kCcTend) CC_ONE(3, kCcStep) CC_ONE(3, kCcDivVort)
+        err = cc_launch_one<T, LL, MM>(d, g.device, p.n_ctas, smem, nlev, (int)ldk, (int)ldk_w, abc, vn, w, ddt_vn, div, vort, p.progress, per_launch, pace_mask, pace_last, wk, ddt_w, s);
+    CC_ONE(2, kCcTend) CC_ONE(2, kCcStep) CC_ONE(2, kCcDivVort) CC_ONE(3, kCcTend) CC_ONE(3, kCcStep)
+    CC_ONE(2, kCcStepW) CC_ONE(3, kCcStepW)
+    constexpr int LDV = sizeof(T) == 4 ? 6 : 3;          // deep columns in the div / vort mode
+    CC_ONE(LDV, kCcDivVort)
 #undef CC_ONE
     return err == cudaSuccess ? 1 : -(int)err;
 }
 
 template int launch_tendencies_cc<double>(const icon_grid&, DevCcTables<double>&, int, int, int64_t, int64_t,
-                                          const double*, const double*, const double*, double*, double*, double*, cudaStream_t);
+                                          const double*, const double*, const double*, double*, double*, double*, cudaStream_t, const double*, double*);
 template int launch_tendencies_cc<float>(const icon_grid&, DevCcTables<float>&, int, int, int64_t, int64_t,
-                                         const float*, const float*, const float*, float*, float*, float*, cudaStream_t);
+                                         const float*, const float*, const float*, float*, float*, float*, cudaStream_t, const float*, float*);
 
 }  // namespace icon

@@ -70,6 +70,22 @@ struct View {
         }
         return true;
     }
+    // adv_c(c,.) * inv_d_e of the edge, re-ordered to the edge slots e[0..2], signed so that the advection term of cell c
+    // reads out * vn_ie * (w(cell across the edge) - w(c)): + if c is e2c[.][0] of the edge, - if it is e2c[.][1] (P-19)
+    bool adv_row(int32_t c, const int32_t e[3], double out[3]) const {
+        bool used[3] = {false, false, false};
+        for (int s = 0; s < 3; ++s) {
+            int hit = -1;
+            for (int q = 0; q < 3; ++q)
+                if (!used[q] && g.c2e[3 * (int64_t)c + q] == e[s]) { hit = q; break; }
+            if (hit < 0) return false;
+            used[hit] = true;
+            const int64_t ed = e[s];
+            const double sign = g.e2c[2 * ed] == c ? 1.0 : -1.0;
+            out[s] = sign * g.adv_c[3 * (int64_t)c + hit] * g.inv_d_e[ed];
+        }
+        return true;
+    }
     bool bln_row(int32_t c, const int32_t e[3], double scale, double out[3]) const {
         bool used[3] = {false, false, false};
         for (int s = 0; s < 3; ++s) {
@@ -154,6 +170,8 @@ std::string build_sc_tables(const HostGrid& g, ScTables& t) {
         const int32_t cell_e[4][3] = {{B[0], I[0], B[5]}, {B[1], B[2], I[1]}, {I[2], B[3], B[4]}, {I[1], I[2], I[0]}};
         for (int j = 0; j < 4; ++j) ok &= c.bln_row(L.T[j], cell_e[j], 0.5, cf + SCF_BLN + 3 * j);
         for (int j = 0; j < 4; ++j) ok &= c.div_row(L.T[j], cell_e[j], cf + SCF_DIV + 3 * j);
+        for (int j = 0; j < 4; ++j) ok &= c.adv_row(L.T[j], cell_e[j], cf + SCF_ADV + 3 * j);
+        for (int x = 0; x < 3; ++x) id[SID_XW0 + x] = L.X[2 * x + 1];
         {
             const int32_t vs[6] = {L.vab, L.vbc, L.vca, L.va, L.vb, L.vc};
             for (int j = 0; j < 6; ++j) id[SID_V0 + j] = vs[j];

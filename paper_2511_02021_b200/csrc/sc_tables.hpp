@@ -29,8 +29,8 @@
 
 namespace icon {
 
-constexpr int kScIdWords = 52;      // int32 per patch: 36 edges, 7 cells, 1 pad, 6 vertices, 2 pad (208 B)
-constexpr int kScCoefWords = 160;   // floating-point words per patch; every group starts on a multiple of 4 words
+constexpr int kScIdWords = 56;      // int32 per patch: 36 edges, 10 cells, 2 pad, 6 vertices, 2 pad (224 B)
+constexpr int kScCoefWords = 172;   // floating-point words per patch; every group starts on a multiple of 4 words
 
 enum {                // id slots
     SID_I0 = 0,       // i0 i1 i2
@@ -40,8 +40,9 @@ enum {                // id slots
     SID_X0 = 21,      // [3][5]: pm0 pm1 pcf n1 n2 of owned boundary edges b0, b2, b4
     SID_T0 = 36,      // T0..T3
     SID_XC0 = 40,     // X0 X2 X4
-    SID_PAD = 43,
-    SID_V0 = 44       // vertices ab bc ca a b c whose vorticity THIS patch stores (fused step), -1 = another patch does
+    SID_XW0 = 43,     // X1 X3 X5: the other three outer cells, read by the vertical-wind tendency only
+    SID_PAD = 46,     // number of column slots: 36 vn (edges) then 10 w (cells)
+    SID_V0 = 48       // vertices ab bc ca a b c whose vorticity THIS patch stores (fused step), -1 = another patch does
 };
 enum {                // coefficient slots
     SCF_RBF = 0,      // [9][4] i0 i1 i2 b0..b5, fixed neighbour order, see build_sc_tables
@@ -53,7 +54,9 @@ enum {                // coefficient slots
     SCF_XBL = 116,    // [3][3] bln of X_j over (b_j, om_j, oc_j) (x 1/2)
     SCF_XROT = 128,   // [3][6] rot of C_x over (b_j, oc_j, n1, n2, oc_jp, b_jp) (x 1/2)
     SCF_USED = 146,
-    SCF_DIV = 148     // [4][3] geofac_div of T0..T3 over the cell edges in the order of SCF_BLN
+    SCF_DIV = 148,    // [4][3] geofac_div of T0..T3 over the cell edges in the order of SCF_BLN
+    SCF_ADV = 160     // [4][3] +-adv_c * inv_d_e of T0..T3 over the same edges (P-19); sign such that the term is
+                      //        coefficient * vn_ie * (w(cell across the edge) - w(this cell))
 };
 
 struct ScTables {

@@ -395,6 +395,46 @@ def test_w_tendency_elementwise(torch_cuda, lib, oracle_mod, oracle_grid, k, see
         assert (np.abs(got[:, :nlev + 1] - want2[:, :nlev + 1]) <= TOL[dtype] * m2[:, :nlev + 1]).all()
 
 
+@pytest.mark.parametrize("k,seed,flags,nlev,ldk,ldk_w,dtype", [
+    (4, 0, 0, 90, 96, 96, "f64"), (4, 0, 0, 90, 90, 92, "f64"), (3, si.PERMUTE_SEED, 1, 40, 40, 42, "f64"),
+    (4, si.PERMUTE_SEED, 1, 90, 96, 96, "f32"), (2, 0, 0, 30, 32, 32, "f64"), (1, 0, 0, 31, 32, 32, "f64"), (2, 0, 0, 33, 34, 34, "f64"),
+    (2, 0, 0, 65, 66, 66, "f64"), (2, 0, 0, 95, 96, 96, "f64"), (0, 0, 0, 3, 4, 4, "f64"), (2, 0, 0, 130, 130, 132, "f64"),
+    (3, 0, 0, 30, 32, 32, "f32")])
+def test_dycore_step_w_all_four_outputs(torch_cuda, lib, oracle_grid, k, seed, flags, nlev, ldk, ldk_w, dtype):
+    """dycore_step_w: ddt_vn, div, vort AND ddt_w from one pass (one fused kernel where the column cache runs; nlev = 130
+    takes the separate calls). Two launches on different inputs; every level of every column written once, pads untouched."""
+    torch = torch_cuda
+    og = oracle_grid(k, seed, flags & 1)
+    g = lib_grid(lib, k, seed, flags)
+    f32 = dtype == "f32"
+    dev = torch.device("cuda:0")
+    o = og.rounded_f32() if f32 else og
+    g.set_option(lib.ICON_OPT_TENDENCY_KERNEL, 5)
+    for cfg, fv in ((1, 1.0), (2, -2.5)):
+        vn, w, zh = si.make_fields(cfg, og.edge_xyz, og.edge_normal, og.nc, nlev=nlev, ldk=ldk, ldk_w=ldk_w, dtype=dtype)
+        vn = (vn * fv).astype(vn.dtype)
+        ref = oracle_reference(og, vn, w, zh, nlev, f32)
+        vn64, w64 = np.nan_to_num(vn.astype(np.float64)), np.nan_to_num(w.astype(np.float64))
+        want_w, m_w = o.w_tendency(vn64, w64, zh, nlev, with_scale=True)
+        tdt = torch.from_numpy(vn).dtype
+        sentinel = -4321.25
+        outs = [torch.full((n, ldk), sentinel, dtype=tdt, device=dev) for n in (g.ne, g.nc, g.nv)]
+        dw = torch.full((g.nc, ldk_w), sentinel, dtype=tdt, device=dev)
+        n0 = g.launch_count
+        lib.dycore_step_w(g, zh, torch.from_numpy(vn).to(dev), torch.from_numpy(w).to(dev), outs[0], outs[1], outs[2], dw, nlev)
+        torch.cuda.synchronize()
+        assert g.launch_count - n0 == (1 if nlev + 1 <= 96 else 3)
+        res = dict(ddt_vn=outs[0].cpu().numpy(), div=outs[1].cpu().numpy(), vort=outs[2].cpu().numpy())
+        check_all(res, ref, nlev, TOL[dtype])
+        for name in res:
+            assert (res[name][:, nlev:] == sentinel).all(), name
+            assert not (res[name][:, :nlev] == sentinel).any(), name
+        got = dw.cpu().numpy().astype(np.float64)
+        err = np.abs(got[:, :nlev + 1] - want_w[:, :nlev + 1])
+        assert (err <= TOL[dtype] * m_w[:, :nlev + 1]).all(), "ddt_w worst err/M %.3e" % (err / np.maximum(m_w[:, :nlev + 1], 1e-300)).max()
+        assert (got[:, 0] == 0).all() and (got[:, nlev] == 0).all() and (got[:, nlev + 1:] == sentinel).all()
+
+
 def test_argument_errors_on_device(torch_cuda, lib):
     torch = torch_cuda
     g = lib_grid(lib, 1)
@@ -564,4 +604,15 @@ def test_full_size_sampled(torch_cuda, lib, oracle_mod, config, host_gb):
     assert not torch.isnan(ddt_w[:, :nlev + 1]).any()
     if ldk_w > nlev + 1:
         assert torch.isnan(ddt_w[:, nlev + 1:]).all()
+    # the same from the fused pass (dycore_step_w: one kernel, four outputs)
+    outs = fresh()
+    ddt_w2 = torch.full((g.nc, ldk_w), float("nan"), dtype=d_vn.dtype, device=dev)
+    n0 = g.launch_count
+    lib.dycore_step_w(g, zh, d_vn, d_w, outs[0], outs[1], outs[2], ddt_w2, nlev)
+    torch.cuda.synchronize()
+    assert g.launch_count - n0 == 1
+    _sampled_check(torch, o, "step_w", config, outs, sizes, nlev, as64(vn), as64(w), zh, tol, nsamp, 300 + config)
+    got2 = ddt_w2[torch.from_numpy(idx).to(dev), torch.from_numpy(lev.astype(np.int64)).to(dev)].cpu().numpy().astype(np.float64)
+    assert (np.abs(got2 - want) <= tol * m).all(), "fused ddt_w config %d" % config
+    assert not torch.isnan(ddt_w2[:, :nlev + 1]).any()
     g.close()

@@ -110,7 +110,7 @@ def test_cc_schedule_replays_correctly(k, seed, flags):
             g.set_option(lib.ICON_OPT_CC_TILE, tile)
             st = g.cc_schedule_check(dtype, nlev, ldk, ldk_w, n_ctas=148, smem_bytes=232448)
             np_ = g.nc // 4
-            group = 8 if nlev + 1 <= 32 else 4          # shallow columns: two patches per warp, eight per step
+            group = 8 if nlev + 1 <= 32 else 4      # shallow columns: two patches per warp, eight per step (reported: the tendency schedule)
             assert st["ctas"] == min(148, -(-np_ // (tile or group)))
             assert st["steps"] >= -(-np_ // group)
             # every patch needs its 36 + 7 columns at least once per CTA range, never more than 43 per patch
