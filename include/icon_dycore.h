@@ -103,7 +103,7 @@ enum {
     ICON_OPT_CC_TILE = 1,         /* kernel 4: patches per tile of the round-robin work order (CTA b walks the tiles
                                      b, b + #CTAs, ... so that neighbouring tiles are in flight together and share
                                      their halo columns through the L2); a multiple of 8; 0 = one contiguous range per
-                                     CTA. Default 16. */
+                                     CTA; -1 = auto (default): 16 for deep 8-byte columns, 64 for short or 4-byte ones. */
     ICON_OPT_CC_PACE = 2,         /* kernel 4: the producers of all CTAs meet every this many steps (power of two; bounded
                                      wait) so that the CTAs do not drift rounds apart and neighbouring tiles keep sharing
                                      halo columns through the L2; 0 = never. Default 512; fused fp64 step (dycore_step) only. */

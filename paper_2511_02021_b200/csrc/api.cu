@@ -188,12 +188,22 @@ icon::CcGeometry cc_geometry(int nlev, int64_t ldk, int64_t ldk_w, bool dv = fal
 template <class T>
 constexpr int cc_record_size(int mode) { return icon::cc_coef_words(mode) * (int)sizeof(T) + icon::kCcRecordTail; }
 
-// Column-cache schedule + patch records for (T, nlev): built on the host once, uploaded once.
+// ICON_OPT_CC_TILE -1 = auto: 16 patches for deep 8-byte columns (a tile then just fits the slot pool), 64 where the
+// columns are short or 4-byte wide (three to four times as many slots; measured config 5: 8.56 -> 8.30 ms, config 4
+// tendency 2.86 -> 2.71 ms)
+template <class T>
+int cc_resolve_tile(const icon_grid* g, int nlev) {
+    const int opt = g->options[ICON_OPT_CC_TILE];
+    if (opt >= 0) return opt;
+    return sizeof(T) == 8 && icon::cc_levels_per_lane(nlev) == 3 ? 16 : 64;
+}
+
+// Column-cache schedule + patch records for (T, nlev, mode): built on the host once, uploaded once.
 // Returns ICON_OK with p.unsupported set when this (T, nlev) cannot use the kernel (the caller
 // then uses the self-contained patch kernel).
 template <class T>
 int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev, int64_t ldk, int64_t ldk_w, int mode = icon::kCcStep) {
-    const int tile = g->options[ICON_OPT_CC_TILE];
+    const int tile = cc_resolve_tile<T>(g, nlev);
     const bool dv = mode == icon::kCcDivVort;
     if (p.nlev == nlev && p.ldk == ldk && p.ldk_w == ldk_w && p.tile == tile && (p.ready || p.unsupported))
         return ICON_OK;
@@ -516,7 +526,7 @@ int icon_grid_create(int bisections_k, uint64_t seed, unsigned flags, icon_grid_
     g->seed = seed;
     g->host_only = (flags & ICON_HOST_ONLY) != 0;
     g->options[ICON_OPT_TENDENCY_KERNEL] = 5;
-    g->options[ICON_OPT_CC_TILE] = 16;
+    g->options[ICON_OPT_CC_TILE] = -1;
     g->options[ICON_OPT_CC_PACE] = 512;
     try {
         std::string err = icon::build_host_grid(bisections_k, seed, (flags & ICON_PERMUTE) != 0, g->host);
@@ -624,7 +634,7 @@ int icon_grid_set_option(icon_grid_t* g, int option, int value) {
     if (!g) return fail(ICON_EINVAL, "grid handle is NULL");
     if (option < 0 || option >= ICON_OPT_COUNT) return fail(ICON_EINVAL, "unknown option");
     if (option == ICON_OPT_CC_PACE && (value < 0 || value > 65536 || (value & (value - 1)))) return fail(ICON_EINVAL, "bad option value");
-    if (option == ICON_OPT_CC_TILE && (value < 0 || value > 4096 || value % 8)) return fail(ICON_EINVAL, "bad option value");
+    if (option == ICON_OPT_CC_TILE && (value < -1 || value > 4096 || (value > 0 && value % 8))) return fail(ICON_EINVAL, "bad option value");
     if (option == ICON_OPT_TENDENCY_KERNEL && value != 0 && value != 3 && value != 4 && value != 5) return fail(ICON_EINVAL, "bad option value");
     g->options[option] = value;
     return ICON_OK;
@@ -653,7 +663,7 @@ int icon_grid_cc_schedule_check(const icon_grid_t* gc, int dtype, int nlev, int 
             const int n_slots = std::min(65535, f64 ? icon::cc_max_slots<double>(geom.slot_bytes, smem_bytes, mode, nlev)
                                                     : icon::cc_max_slots<float>(geom.slot_bytes, smem_bytes, mode, nlev));
             std::string err = icon::build_cc_schedule(g->sc_host, n_ctas, n_slots, geom, icon::cc_patches_per_step_for(nlev, f64 ? 8 : 4, mode), icon::kCcDepth,
-                                                      g->options[ICON_OPT_CC_TILE], icon::cc_use_mask(mode), cs);
+                                                      f64 ? cc_resolve_tile<double>(g, nlev) : cc_resolve_tile<float>(g, nlev), icon::cc_use_mask(mode), cs);
             if (!err.empty()) return fail(ICON_EUNSUPPORTED, err);
             err = icon::check_cc_schedule(g->sc_host, cs, g->host.ne, g->host.nc);
             if (!err.empty()) return fail(ICON_EINVAL, err + (dv ? " (div/vort schedule)" : mode == icon::kCcStepW ? " (step + ddt_w schedule)" : ""));

@@ -304,7 +304,7 @@ def test_column_cache_level_mappings_and_tiles(torch_cuda, lib, oracle_grid, til
             assert (res[name][:, nlev:] == -77.5).all(), name
             assert not (res[name][:, :nlev] == -77.5).any(), name
     finally:
-        g.set_option(lib.ICON_OPT_CC_TILE, 16)
+        g.set_option(lib.ICON_OPT_CC_TILE, -1)
         g.set_option(lib.ICON_OPT_TENDENCY_KERNEL, 5)
 
 

@@ -106,12 +106,13 @@ def test_cc_schedule_replays_correctly(k, seed, flags):
     g = lib.IconGrid(k, seed, flags | binding.ICON_HOST_ONLY)
     for dtype, nlev, ldk, ldk_w in ((0, 90, 96, 96), (0, 90, 90, 92), (1, 90, 92, 92), (1, 90, 96, 96), (0, 30, 30, 32), (0, 30, 32, 32),
                                     (0, 2, 2, 4), (0, 65, 66, 66)):
-        for tile in (16, 0, 64):
+        for tile in (16, 0, 64, -1):
             g.set_option(lib.ICON_OPT_CC_TILE, tile)
             st = g.cc_schedule_check(dtype, nlev, ldk, ldk_w, n_ctas=148, smem_bytes=232448)
             np_ = g.nc // 4
             group = 8 if nlev + 1 <= 32 else 4      # shallow columns: two patches per warp, eight per step (reported: the tendency schedule)
-            assert st["ctas"] == min(148, -(-np_ // (tile or group)))
+            eff = tile if tile >= 0 else (16 if (dtype == 0 and nlev + 1 > 32) else 64)
+            assert st["ctas"] == min(148, -(-np_ // (eff or group)))
             assert st["steps"] >= -(-np_ // group)
             # every patch needs its 36 + 7 columns at least once per CTA range, never more than 43 per patch
             assert 6 * np_ <= st["vn_columns"] <= 36 * np_ and 4 * np_ <= st["w_columns"] <= 7 * np_
