@@ -440,14 +440,11 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
     // vertical-wind tendency (mode kCcStepW, P-19): weight of vn(k) in vn_ie(k), 1 / (z_half[k-1] - z_half[k+1]) (both 0
     // outside the interior half levels 1 .. nlev-1, so that ddt_w comes out 0 at the top and the surface) and the half
     // levels that exist in a w / ddt_w column
-    T wg[L], wrdz[L];
     bool pow_[L], w_int[L];
     FORL {
         const int k = level_of<L>(lane, l);
         pow_[l] = WTEND && k <= nlev;
         w_int[l] = WTEND && k >= 1 && k <= nlev - 1;
-        wg[l] = w_int[l] ? __ldg(wk + k) : (T)0;
-        wrdz[l] = w_int[l] ? __ldg(wk + nlev + 1 + k) : (T)0;
     }
     const uint64_t cs = (uint64_t)ldk * sizeof(T), cs_wout = (uint64_t)ldk_w * sizeof(T);
     const int hl = PPW == 2 ? lane & 15 : lane, half = PPW == 2 ? lane >> 4 : 0;      // lane inside its patch, patch of the warp
@@ -568,6 +565,14 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
             if constexpr (WTEND) {
                 // ---- vertical-wind tendency of the four cells (P-19), while only the nine in-patch columns are live ----
                 // ddt_w(c,k) = -[ sum_j a(c,j) vn_ie(e_j,k) (w(cell across e_j,k) - w(c,k)) + w(c,k) (w(c,k-1) - w(c,k+1)) rdz2(k) ]
+                // the two per-level constants are fetched here (L1-resident after the first patch) instead of living in
+                // registers for the whole kernel: the fused instantiation sits at its register limit
+                T wg[L], wrdz[L];
+                FORL {
+                    const int k = level_of<L>(lane, l);
+                    wg[l] = w_int[l] ? __ldg(wk + k) : (T)0;
+                    wrdz[l] = w_int[l] ? __ldg(wk + nlev + 1 + k) : (T)0;
+                }
                 T av[12];
                 ld_coef(cf + SCF_ADV, av);
                 uint32_t sW[12];                    // T0..T3 X0 X2 X4 X1 X3 X5 + mask + pad
