@@ -1,5 +1,8 @@
 // kernels_cc.cu -- column-cache kernel for the velocity tendency and, fused
-// into the same pass on request, divergence and vorticity (S1, S2: dycore_step), sm_100a.
+// into the same pass on request, divergence and vorticity (S1, S2: dycore_step), sm_100a. Four modes (template
+// parameter MODE, cc_schedule.hpp): kCcTend = ddt_vn (dycore_velocity_tendencies), kCcStep = ddt_vn + div + vort
+// (dycore_step), kCcDivVort = div + vort alone from the 27 vn columns they need (dycore_div_vort), kCcStepW = kCcStep
+// plus the vertical-wind tendency ddt_w (dycore_step_w, reading P-19).
 //
 // One warp finishes one self-contained patch (sc_tables.hpp: four sibling cells, six owned edges,
 // 36 vn + 7 w columns, no exchange between warps), lanes = levels. The vn / w columns do not come
@@ -20,7 +23,7 @@
 //     consecutive levels per lane, paid 12 L1 wavefronts per output column for it, 144 of ~740 per
 //     patch); the vertical stencil (S6) costs two shuffles up and two down per column (inside the pair
 //     the neighbour level is in the lane's own registers);
-//   * FUSED: div of the patch's four cells comes from the nine in-patch columns, and the sums zm, zc
+//   * kCcStep: div of the patch's four cells comes from the nine in-patch columns, and the sums zm, zc
 //     the tendency needs ARE half the vorticity at the patch's three midpoint and three corner
 //     vertices; every vertex of the grid is one of those for some patch, the lowest patch stores it.
 //
