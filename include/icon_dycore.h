@@ -219,6 +219,30 @@ int dycore_step_w(const icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w,
                   const void* vn, const void* w, void* ddt_vn, void* div, void* vort, void* ddt_w, void* cuda_stream);
 
 /*
+ * dycore_velocity_tendencies_noalloc -- dycore_velocity_tendencies (S3-S7, same formulas, same argument rules, no optional
+ * outputs) for callers that cannot call cudaMalloc: code under CUDA-graph capture, tight serving loops, harnesses that forbid
+ * it. The ordinary entry points allocate lazily on their first call for a new (dtype, nlev, ldk, z_half); this one calls no
+ * cudaMalloc, cudaFree or allocating library routine, ever, and touches no host heap. It runs the unfused pipeline
+ * (vt, KE_e -> KE_c, zeta -> ddt_vn) with its intermediates in a STATIC device array of ICON_NOALLOC_SCRATCH_BYTES that
+ * every GPU that loads the library holds until the process exits.
+ *   Limits: nlev <= 128 and align256(3*nlev*g) + 2*align256(ne*ldk*g) + align256(nc*ldk*g) + align256(nv*ldk*g) <=
+ *   ICON_NOALLOC_SCRATCH_BYTES, g = sizeof(T) (64 MiB: R2B4 x 90 fp64 levels with ldk = 90, R2B3 with any padding);
+ *   beyond that ICON_EINVAL with the two byte counts in icon_last_error(). ICON_F32 needs the fp32 coefficient tables
+ *   already on the device (one ordinary fp32 compute call on the grid), else ICON_EUNSUPPORTED; ICON_F64 tables are
+ *   uploaded by icon_grid_create.
+ *   Sharing: every call on a device uses the same array, which keeps the previous call's contents. Nothing in it has to
+ *   start at zero (the pipeline writes every level it later reads), so nothing is cleared. Calls that overlap on the GPU
+ *   (two streams, two threads, two grids on one device) RACE on it: serialise them. The first call on a device resolves
+ *   the array's device address (cudaGetSymbolAddress, which may load the module): make it outside stream capture.
+ * This is the slow path (intermediates through HBM: about 3x the time of the column-cache kernel); it exists for the
+ * callers above, not for throughput.
+ */
+#define ICON_NOALLOC_SCRATCH_BYTES (64u << 20)
+int dycore_velocity_tendencies_noalloc(const icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w,
+                                       const double* z_half, const void* vn, const void* w, void* ddt_vn,
+                                       void* cuda_stream);
+
+/*
  * dycore_step_host -- dycore_step with HOST field buffers (the end-to-end leg of bench.py): copies vn and w to
  * device staging buffers, runs dycore_step (one fused kernel where the column-cache kernel runs), copies ddt_vn, div
  * and vort back, and synchronises. This is NOT how the paper runs the model (fields stay resident on the GPU,

@@ -29,7 +29,7 @@ TABLE_ID = {n: i for i, n in enumerate(TABLES)}
 # every symbol include/icon_dycore.h declares
 EXPORTS = ("icon_grid_create", "icon_grid_destroy", "icon_grid_counts", "icon_grid_table_host",
            "icon_grid_table_device", "icon_grid_set_option", "icon_grid_cc_schedule_check", "dycore_div_vort", "dycore_velocity_tendencies",
-           "dycore_step", "dycore_step_host", "dycore_step_w", "dycore_w_tendency", "icon_grid_launch_count", "icon_last_error")
+           "dycore_step", "dycore_step_host", "dycore_step_w", "dycore_w_tendency", "dycore_velocity_tendencies_noalloc", "icon_grid_launch_count", "icon_last_error")
 
 
 class IconError(RuntimeError):
@@ -73,6 +73,8 @@ def load_library():
     L.dycore_velocity_tendencies.argtypes = [P, ci, ci, ci, ci, P, P, P, P, P, P, P, P]
     L.dycore_w_tendency.restype = ci
     L.dycore_w_tendency.argtypes = [P, ci, ci, ci, ci, P, P, P, P, P]
+    L.dycore_velocity_tendencies_noalloc.restype = ci
+    L.dycore_velocity_tendencies_noalloc.argtypes = [P, ci, ci, ci, ci, P, P, P, P, P]
     L.dycore_step_w.restype = ci
     L.dycore_step_w.argtypes = [P, ci, ci, ci, ci, P, P, P, P, P, P, P, P]
     L.dycore_step.restype = ci
@@ -218,6 +220,20 @@ def dycore_velocity_tendencies(grid, z_half, vn, w, ddt_vn, nlev, vt=None, ke_c=
     _check(grid._L.dycore_velocity_tendencies(grid._h, _dtype_of(vn), int(nlev), int(vn.shape[1]), int(w.shape[1]),
                                               _dptr(z), _dptr(vn), _dptr(w), _dptr(ddt_vn), _dptr(vt), _dptr(ke_c),
                                               _dptr(vort), _stream_ptr(stream)))
+
+
+NOALLOC_SCRATCH_BYTES = 64 << 20     # ICON_NOALLOC_SCRATCH_BYTES of include/icon_dycore.h
+
+
+def dycore_velocity_tendencies_noalloc(grid, z_half, vn, w, ddt_vn, nlev, stream=None):
+    """S3-S7 without any allocation (static device scratch of NOALLOC_SCRATCH_BYTES; see include/icon_dycore.h for the
+    limits and the sharing rule: calls that overlap on the GPU race)."""
+    z = np.ascontiguousarray(z_half, dtype=np.float64)
+    if z.size != nlev + 1:
+        raise ValueError("z_half must have nlev+1 entries")
+    _check_fields((("vn", vn, grid.ne, "ldk"), ("w", w, grid.nc, "ldk_w"), ("ddt_vn", ddt_vn, grid.ne, "ldk")))
+    _check(grid._L.dycore_velocity_tendencies_noalloc(grid._h, _dtype_of(vn), int(nlev), int(vn.shape[1]), int(w.shape[1]),
+                                                      _dptr(z), _dptr(vn), _dptr(w), _dptr(ddt_vn), _stream_ptr(stream)))
 
 
 def dycore_w_tendency(grid, z_half, vn, w, ddt_w, nlev, stream=None):

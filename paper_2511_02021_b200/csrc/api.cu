@@ -5,6 +5,7 @@
 
 #include <algorithm>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <type_traits>
@@ -900,3 +901,139 @@ int dycore_step_host(const icon_grid_t* gc, int dtype, int nlev, int ldk, int ld
 }
 
 }  // extern "C"
+
+// ======================================================================================================
+// dycore_velocity_tendencies_noalloc -- the unfused tendency pipeline with its scratch in a STATIC device array
+// ======================================================================================================
+// Some callers cannot call cudaMalloc (code under CUDA-graph capture, tight serving loops, harnesses that forbid it).
+// The ordinary entry points allocate lazily on the first call for a new (dtype, nlev, ldk, z_half): schedules, records,
+// level coefficients, the workspace of the unfused pipeline. This variant allocates NOTHING: the intermediates of the
+// unfused pipeline (vt, KE_e, KE_c, zeta) and the per-level coefficients live in the file-scope array below, which every
+// GPU that loads the library holds until the process exits. In host code the array's NAME is a host-side stand-in, not
+// a device address: its device address is taken once per device with cudaGetSymbolAddress (device current) and only that
+// pointer is ever handed to a kernel.
+namespace {
+
+constexpr size_t kNoAllocScratchBytes = ICON_NOALLOC_SCRATCH_BYTES;
+constexpr int kNoAllocMaxLevels = 128;             // the level coefficients travel as a kernel argument (3 x 128 doubles)
+static __device__ __align__(256) unsigned char g_noalloc_scratch[kNoAllocScratchBytes];
+
+struct NoAllocCoeffArg {
+    double v[3 * kNoAllocMaxLevels];               // A_k, B_k, C_k of reading P-14, [3][nlev]
+};
+
+// writes the 3 * nlev level coefficients into the scratch array (no host -> device copy, no staging buffer)
+template <class T>
+__global__ void k_noalloc_coeffs(NoAllocCoeffArg a, int n, T* __restrict__ out) {
+    for (int i = threadIdx.x; i < n; i += blockDim.x) out[i] = (T)a.v[i];
+}
+
+// device address of g_noalloc_scratch on `device` (which must be current); resolved once per device
+int noalloc_scratch_ptr(int device, unsigned char** out) {
+    static std::mutex mu;
+    static unsigned char* ptrs[64] = {nullptr};
+    std::lock_guard<std::mutex> lock(mu);
+    const bool known = device >= 0 && device < 64;
+    if (known && ptrs[device]) {
+        *out = ptrs[device];
+        return ICON_OK;
+    }
+    unsigned char* p = nullptr;
+    cudaError_t e = cudaGetSymbolAddress((void**)&p, g_noalloc_scratch);
+    if (e != cudaSuccess) return fail_cuda(e, "cudaGetSymbolAddress(g_noalloc_scratch)");
+    if (!p || reinterpret_cast<uintptr_t>(p) % 256) return fail(ICON_ECUDA, "static scratch array has no usable device address");
+    if (known) ptrs[device] = p;
+    *out = p;
+    return ICON_OK;
+}
+
+size_t align256(size_t n) { return (n + 255) & ~(size_t)255; }
+
+// (vn_ie(k) - vn_ie(k+1)) / dz_k = A_k vn(k-1) + B_k vn(k) + C_k vn(k+1): the statements of vertical_coefficients above, in
+// the same order, into a caller-provided array abc[3][K] instead of a std::vector
+void noalloc_vertical_coefficients(const double* zh, int K, double* abc) {
+    for (int i = 0; i < 3 * kNoAllocMaxLevels; ++i) abc[i] = 0.0;
+    auto zf = [&](int k) { return 0.5 * (zh[k] + zh[k + 1]); };
+    auto add_half = [&](int k, int kh, double sign) {
+        int ia, ib;
+        double ca, cb;
+        if (kh == 0) {
+            double r = (zh[0] - zf(0)) / (zf(0) - zf(1));
+            ia = 0; ca = 1.0 + r; ib = 1; cb = -r;
+        } else if (kh == K) {
+            double r = (zh[K] - zf(K - 1)) / (zf(K - 1) - zf(K - 2));
+            ia = K - 1; ca = 1.0 + r; ib = K - 2; cb = -r;
+        } else {
+            double up = zh[kh - 1] - zh[kh], dn = zh[kh] - zh[kh + 1];
+            double gk = up / (up + dn);
+            ia = kh; ca = gk; ib = kh - 1; cb = 1.0 - gk;
+        }
+        const double inv_dz = 1.0 / (zh[k] - zh[k + 1]);
+        abc[(size_t)(ia - k + 1) * K + k] += sign * ca * inv_dz;
+        abc[(size_t)(ib - k + 1) * K + k] += sign * cb * inv_dz;
+    };
+    for (int k = 0; k < K; ++k) {
+        add_half(k, k, +1.0);
+        add_half(k, k + 1, -1.0);
+    }
+}
+
+template <class T>
+int noalloc_impl(icon_grid* g, icon::DevCoeffs<T>& c, int nlev, int ldk, int ldk_w, const double* z_half, const void* vn,
+                 const void* w, void* ddt_vn, cudaStream_t s) {
+    if (!c.ready)
+        return fail(ICON_EUNSUPPORTED, "the coefficient tables of this dtype are not on the device yet and this entry point must not "
+                                       "allocate: make one ordinary compute call of this dtype on the grid first");
+    const size_t ne = (size_t)g->host.ne, nc = (size_t)g->host.nc, nv = (size_t)g->host.nv;
+    const size_t b_abc = align256(3 * (size_t)nlev * sizeof(T)), b_e = align256(ne * ldk * sizeof(T)),
+                 b_c = align256(nc * ldk * sizeof(T)), b_v = align256(nv * ldk * sizeof(T));
+    const size_t need = b_abc + 2 * b_e + b_c + b_v;
+    if (need > kNoAllocScratchBytes)
+        return fail(ICON_EINVAL, "dycore_velocity_tendencies_noalloc: this grid and level count need " + std::to_string(need) +
+                                     " bytes of scratch, the static array holds " + std::to_string(kNoAllocScratchBytes) +
+                                     " (ICON_NOALLOC_SCRATCH_BYTES); use dycore_velocity_tendencies");
+    unsigned char* base = nullptr;
+    int rc = noalloc_scratch_ptr(g->device, &base);
+    if (rc) return rc;
+    T* abc = reinterpret_cast<T*>(base);
+    T* vt = reinterpret_cast<T*>(base + b_abc);
+    T* ke_e = reinterpret_cast<T*>(base + b_abc + b_e);
+    T* ke_c = reinterpret_cast<T*>(base + b_abc + 2 * b_e);
+    T* vort = reinterpret_cast<T*>(base + b_abc + 2 * b_e + b_c);
+    // the arithmetic of the ordinary path (vertical_coefficients, reading P-14), written straight into the kernel argument:
+    // no host heap either
+    NoAllocCoeffArg arg;
+    noalloc_vertical_coefficients(z_half, nlev, arg.v);
+    k_noalloc_coeffs<T><<<1, 128, 0, s>>>(arg, 3 * nlev, abc);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail_cuda(e, "kernel launch");
+    // nothing in the scratch has to start at zero: every level < nlev of vt, KE_e, KE_c and zeta is written by the
+    // pipeline before it is read, and levels >= nlev are never read
+    const int n = icon::launch_tendencies_unfused<T>(*g, c, nlev, ldk, ldk_w, abc, (const T*)vn, (const T*)w, (T*)ddt_vn, vt, ke_e,
+                                                     ke_c, vort, s);
+    if (n < 0) return fail_cuda((cudaError_t)(-n), "kernel launch");
+    g->launches += n + 1;
+    return ICON_OK;
+}
+
+}  // namespace
+
+extern "C" int dycore_velocity_tendencies_noalloc(const icon_grid_t* gc, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
+                                                  const void* vn, const void* w, void* ddt_vn, void* cuda_stream) {
+    icon_grid* g = const_cast<icon_grid*>(gc);
+    int rc = check_common(g, dtype, nlev, ldk, 2);      // includes: the grid's device is the current device
+    if (rc) return rc;
+    if (nlev > kNoAllocMaxLevels) return fail(ICON_EINVAL, "dycore_velocity_tendencies_noalloc: nlev > 128");
+    const size_t es = dtype == ICON_F64 ? 8 : 4;
+    if (ldk_w < nlev + 1) return fail(ICON_EINVAL, "ldk_w < nlev+1");
+    if (((int64_t)ldk_w * (int64_t)es) % 16) return fail(ICON_EINVAL, "ldk_w*sizeof(T) must be a multiple of 16");
+    if (!z_half) return fail(ICON_EINVAL, "z_half is NULL");
+    for (int k = 0; k < nlev; ++k)
+        if (!(z_half[k] > z_half[k + 1])) return fail(ICON_EINVAL, "z_half must be strictly decreasing");
+    if ((rc = check_field(vn, "vn")) || (rc = check_field(w, "w")) || (rc = check_field(ddt_vn, "ddt_vn"))) return rc;
+    const size_t be = (size_t)g->host.ne * ldk * es, bw = (size_t)g->host.nc * ldk_w * es;
+    if (overlaps(ddt_vn, be, vn, be) || overlaps(ddt_vn, be, w, bw)) return fail(ICON_EINVAL, "outputs must not alias inputs");
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    if (dtype == ICON_F64) return noalloc_impl<double>(g, g->c64, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, s);
+    return noalloc_impl<float>(g, g->c32, nlev, ldk, ldk_w, z_half, vn, w, ddt_vn, s);
+}
