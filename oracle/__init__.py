@@ -70,6 +70,10 @@ def _load():
     L.og_sample_ddt_w.argtypes = [P, ctypes.c_int, i64, i64, P, P, P, i64, P, P, P, P]
     L.og_ddt_w.restype = None
     L.og_ddt_w.argtypes = [i64, ctypes.c_int, i64, i64, P, P, P, P, P, P, P, P, P]
+    L.og_metric_from_zhalf.restype = None
+    L.og_metric_from_zhalf.argtypes = [i64, ctypes.c_int, i64, i64, P, P, P]
+    L.og_velocity_tendencies_metric.restype = ctypes.c_int
+    L.og_velocity_tendencies_metric.argtypes = [P, ctypes.c_int, i64, i64, P, P, P, P, P, P, P, P, P, P, P]
     L.og_divergence.restype = None
     L.og_divergence.argtypes = [i64, ctypes.c_int, i64, P, P, P, P, P]
     L.og_vorticity.restype = None
@@ -95,7 +99,7 @@ _TABLES = {
     "vert_xyz": (np.float64, "v", 3), "cell_xyz": (np.float64, "c", 3),
     "edge_xyz": (np.float64, "e", 3), "edge_normal": (np.float64, "e", 3),
     "l_e": (np.float64, "e", 1), "d_e": (np.float64, "e", 1), "inv_d_e": (np.float64, "e", 1),
-    "f_e": (np.float64, "e", 1), "c_lin": (np.float64, "e", 2), "rbf": (np.float64, "e", 4),
+    "f_e": (np.float64, "e", 1), "c_lin": (np.float64, "e", 2), "cgrad": (np.float64, "e", 2), "rbf": (np.float64, "e", 4),
     "a_c": (np.float64, "c", 1), "bln": (np.float64, "c", 3), "adv_c": (np.float64, "c", 3), "a_v": (np.float64, "v", 1),
     "geofac_div": (np.float64, "c", 3), "geofac_rot": (np.float64, "v", 6),
 }
@@ -198,6 +202,25 @@ class Grid:
             raise RuntimeError("og_w_tendency rc=%d" % rc)
         return (out, m) if with_scale else out
 
+    def velocity_tendencies_metric(self, vn, w, wgt_e, inv_ddqz_e, ddxn_z, ddxt_z, nlev, with_scale=False):
+        """metric variant of S3-S7 (reading P-20); returns dict(ddt_vn, vt, ke_c, vort[, m_ddt])"""
+        vn, w = _f64(vn), _f64(w)
+        wgt_e, inv_ddqz_e, ddxn_z, ddxt_z = _f64(wgt_e), _f64(inv_ddqz_e), _f64(ddxn_z), _f64(ddxt_z)
+        ldk, ldk_w = vn.shape[1], w.shape[1]
+        assert wgt_e.shape == (self.ne, ldk_w) and inv_ddqz_e.shape == ddxn_z.shape == ddxt_z.shape == (self.ne, ldk)
+        out = {n: np.zeros((self.ne, ldk)) for n in ("ddt_vn", "vt")}
+        out["ke_c"] = np.zeros((self.nc, ldk))
+        out["vort"] = np.zeros((self.nv, ldk))
+        m = np.zeros((self.ne, ldk)) if with_scale else None
+        rc = self._L.og_velocity_tendencies_metric(self._h, nlev, ldk, ldk_w, _ptr(wgt_e), _ptr(inv_ddqz_e), _ptr(ddxn_z),
+                                                   _ptr(ddxt_z), _ptr(vn), _ptr(w), _ptr(out["ddt_vn"]), _ptr(out["vt"]),
+                                                   _ptr(out["ke_c"]), _ptr(out["vort"]), _ptr(m))
+        if rc:
+            raise RuntimeError("og_velocity_tendencies_metric rc=%d" % rc)
+        if with_scale:
+            out["m_ddt"] = m
+        return out
+
     # ---- sampled one-by-one evaluation (full-size parity) ----
     def sample(self, what, idx, lev, vn, nlev, w=None, z_half=None):
         vn = _f64(vn)
@@ -281,3 +304,14 @@ def w_tendency_from_arrays(t, vn, w, z_half, nlev):
     out, m = np.zeros((nc, ldk_w)), np.zeros((nc, ldk_w))
     L.og_ddt_w(nc, nlev, ldk, ldk_w, _ptr(z_half), _ptr(c2e), _ptr(e2c), _ptr(inv_d), _ptr(adv), _ptr(vn), _ptr(w), _ptr(out), _ptr(m))
     return out, m
+
+
+def metric_from_zhalf(z_half_e, nlev, ldk):
+    """(wgt_e [ne][ldk_w], inv_ddqz_e [ne][ldk]) of reading P-20 from the half-level heights z_half_e [ne][ldk_w] of every
+    edge column (strictly decreasing in k); pads are NaN"""
+    L = _load()
+    z = _f64(z_half_e)
+    ne, ldk_w = z.shape
+    wgt, inv = np.full((ne, ldk_w), np.nan), np.full((ne, ldk), np.nan)
+    L.og_metric_from_zhalf(ne, nlev, ldk, ldk_w, _ptr(z), _ptr(wgt), _ptr(inv))
+    return wgt, inv

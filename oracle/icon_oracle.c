@@ -61,6 +61,7 @@ typedef struct og_grid {
     double *edge_normal;            /* [ne][3] */
     double *l_e, *d_e, *inv_d_e, *f_e; /* [ne] */
     double *c_lin;                  /* [ne][2] */
+    double *cgrad;                  /* [ne][2] reading P-20: distance-weighted KE-gradient coefficients */
     double *rbf;                    /* [ne][4] */
     double *a_c;                    /* [nc] */
     double *bln;                    /* [nc][3] */
@@ -243,7 +244,7 @@ static void og_free_fields(og_grid *g)
     free(g->c2v); free(g->c2e); free(g->e2c); free(g->e2v); free(g->e2e4);
     free(g->v2e); free(g->v2c); free(g->v_deg); free(g->c_os); free(g->v_os);
     free(g->vert_xyz); free(g->cell_xyz); free(g->edge_xyz); free(g->edge_normal);
-    free(g->l_e); free(g->d_e); free(g->inv_d_e); free(g->f_e); free(g->c_lin); free(g->rbf);
+    free(g->l_e); free(g->d_e); free(g->inv_d_e); free(g->f_e); free(g->c_lin); free(g->cgrad); free(g->rbf);
     free(g->a_c); free(g->bln); free(g->adv_c); free(g->a_v); free(g->geofac_div); free(g->geofac_rot);
 }
 void og_grid_destroy(og_grid *g)
@@ -456,6 +457,7 @@ static void og_build_geometry(og_grid *g)
     g->inv_d_e = (double *)malloc(sizeof(double) * (size_t)ne);
     g->f_e = (double *)malloc(sizeof(double) * (size_t)ne);
     g->c_lin = (double *)malloc(sizeof(double) * 2 * (size_t)ne);
+    g->cgrad = (double *)malloc(sizeof(double) * 2 * (size_t)ne);
     g->rbf = (double *)malloc(sizeof(double) * 4 * (size_t)ne);
     g->a_c = (double *)malloc(sizeof(double) * (size_t)nc);
     g->bln = (double *)malloc(sizeof(double) * 3 * (size_t)nc);
@@ -496,6 +498,10 @@ static void og_build_geometry(og_grid *g)
         g->f_e[e] = 2.0 * OG_OMEGA * x[2];
         g->c_lin[2 * e] = arc3(x, c1) / de;
         g->c_lin[2 * e + 1] = arc3(x, c0) / de;
+        /* P-20: cgrad(e,0) = (a1/a0)/d_e multiplies KE_c(c0), cgrad(e,1) = (a0/a1)/d_e multiplies KE_c(c1),
+         * a0 = arc(x_e,c0), a1 = arc(x_e,c1), d_e in metres */
+        g->cgrad[2 * e] = (arc3(x, c1) / arc3(x, c0)) / (de * a);
+        g->cgrad[2 * e + 1] = (arc3(x, c0) / arc3(x, c1)) / (de * a);
     }
     /* G2 folded factor: geofac_div = l_e * c_os / A_c */
 #pragma omp parallel for schedule(static)
@@ -668,6 +674,7 @@ og_grid *og_grid_round_f32(const og_grid *s)
     g->inv_d_e = og_round_copy(s->inv_d_e, ne);
     g->f_e = og_round_copy(s->f_e, ne);
     g->c_lin = og_round_copy(s->c_lin, 2 * ne);
+    g->cgrad = og_round_copy(s->cgrad, 2 * ne);
     g->rbf = og_round_copy(s->rbf, 4 * ne);
     g->a_c = og_round_copy(s->a_c, nc);
     g->bln = og_round_copy(s->bln, 3 * nc);
@@ -924,6 +931,102 @@ int og_velocity_tendencies(const og_grid *g, int nlev, int64_t ldk, int64_t ldk_
 }
 
 /* ------------------------------------------------------------------ */
+/* Reading P-20: the ICON-faithful metric variant of S5-S7 on the "terrain following hybrid
+ * sigma height grid" of PAPER.md:56. The paper prints none of it; the reading is in DESIGN.md section 3.
+ *
+ * Metric columns per EDGE (inputs of the operator, static in a model run):
+ *   wgt_e     [ne][ldk_w] half levels k = 0..nlev: k = 1..nlev-1 weight of vn(k) in vn_ie(k) (vn(k-1) gets 1 - wgt);
+ *                         k = 0 and k = nlev: the ratios r of the two-point linear extrapolation
+ *                         vn_ie(0) = vn(0) + r (vn(0) - vn(1)),  vn_ie(nlev) = vn(nlev-1) + r (vn(nlev-1) - vn(nlev-2))
+ *   inv_ddqz_e[ne][ldk]   1 / layer thickness at the edge
+ *   ddxn_z, ddxt_z [ne][ldk]  slopes dz/dn, dz/dt of the full-level coordinate surface at the edge midpoint
+ *                             (n = n_e, t = t_e = n_e x x_e, reading P-4)
+ * og_metric_from_zhalf derives the first two from the half-level heights of every edge column. */
+void og_metric_from_zhalf(int64_t ne, int nlev, int64_t ldk, int64_t ldk_w, const double *z_half_e,
+                          double *wgt_e, double *inv_ddqz_e)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t e = 0; e < ne; ++e) {
+        const double *zh = z_half_e + e * ldk_w;
+        for (int k = 0; k < nlev; ++k) inv_ddqz_e[e * ldk + k] = 1.0 / (zh[k] - zh[k + 1]);
+        for (int k = 1; k <= nlev - 1; ++k) {
+            double up = zh[k - 1] - zh[k], dn = zh[k] - zh[k + 1];
+            wgt_e[e * ldk_w + k] = up / (up + dn);
+        }
+        {   /* ends: (z_half - z_full) / (z_full - z_full of the next level inwards) = dz_0 / (dz_0 + dz_1) */
+            double d0 = zh[0] - zh[1], d1 = zh[1] - zh[2];
+            wgt_e[e * ldk_w] = d0 / (d0 + d1);
+            double dl = zh[nlev - 1] - zh[nlev], dm = zh[nlev - 2] - zh[nlev - 1];
+            wgt_e[e * ldk_w + nlev] = dl / (dl + dm);
+        }
+    }
+}
+
+/* vn at half level k of one edge column with per-edge weights (P-20) */
+static double og_vn_half_metric(const double *col, int nlev, const double *wg, int k)
+{
+    if (k == 0) return col[0] + wg[0] * (col[0] - col[1]);
+    if (k == nlev) return col[nlev - 1] + wg[nlev] * (col[nlev - 1] - col[nlev - 2]);
+    return wg[k] * col[k] + (1.0 - wg[k]) * col[k - 1];
+}
+
+/* S5-S7, metric variant:
+ *   gradK  = cgrad(e,1) KE_c(c1) - cgrad(e,0) KE_c(c0) + KE_e(e) (cgrad(e,0) - cgrad(e,1))      (second-order at x_e)
+ *   H      = gradK + vt (f_e + 1/2 (zeta(v0) + zeta(v1)))
+ *   w_cc   = vn ddxn_z + vt ddxt_z                  (contravariant correction: the wind's climb along the surface)
+ *   V      = (w_e - w_cc) (vn_ie(k) - vn_ie(k+1)) inv_ddqz_e,   w_e as in S6
+ *   ddt_vn = -(H + V)
+ * m (may be NULL): sum of the absolute values of the terms. */
+void og_ddt_vn_metric(int64_t ne, int nlev, int64_t ldk, int64_t ldk_w, const int32_t *e2c, const int32_t *e2v,
+                      const double *cgrad, const double *f_e, const double *c_lin, const double *wgt_e,
+                      const double *inv_ddqz_e, const double *ddxn_z, const double *ddxt_z, const double *vn,
+                      const double *w, const double *vt, const double *ke_e, const double *ke_c, const double *vort,
+                      double *ddt_vn, double *m_ddt)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t e = 0; e < ne; ++e) {
+        int64_t c0 = e2c[2 * e], c1 = e2c[2 * e + 1], v0 = e2v[2 * e], v1 = e2v[2 * e + 1];
+        const double *col = vn + e * ldk, *wg = wgt_e + e * ldk_w;
+        double g0 = cgrad[2 * e], g1 = cgrad[2 * e + 1];
+        for (int k = 0; k < nlev; ++k) {
+            int64_t i = e * ldk + k;
+            double gradk = g1 * ke_c[c1 * ldk + k] - g0 * ke_c[c0 * ldk + k] + ke_e[i] * (g0 - g1);
+            double zeta_e = 0.5 * (vort[v0 * ldk + k] + vort[v1 * ldk + k]);
+            double H = gradk + vt[i] * (f_e[e] + zeta_e);
+            double wf0 = 0.5 * (w[c0 * ldk_w + k] + w[c0 * ldk_w + k + 1]);
+            double wf1 = 0.5 * (w[c1 * ldk_w + k] + w[c1 * ldk_w + k + 1]);
+            double w_e = c_lin[2 * e] * wf0 + c_lin[2 * e + 1] * wf1;
+            double w_cc = vn[i] * ddxn_z[i] + vt[i] * ddxt_z[i];
+            double up = og_vn_half_metric(col, nlev, wg, k), dn = og_vn_half_metric(col, nlev, wg, k + 1);
+            double Vt = (w_e - w_cc) * (up - dn) * inv_ddqz_e[i];
+            ddt_vn[i] = -(H + Vt);
+            if (m_ddt)
+                m_ddt[i] = g1 * fabs(ke_c[c1 * ldk + k]) + g0 * fabs(ke_c[c0 * ldk + k]) + fabs(ke_e[i]) * fabs(g0 - g1)
+                    + fabs(vt[i]) * (fabs(f_e[e]) + 0.5 * (fabs(vort[v0 * ldk + k]) + fabs(vort[v1 * ldk + k])))
+                    + (fabs(w_e) + fabs(vn[i] * ddxn_z[i]) + fabs(vt[i] * ddxt_z[i])) * (fabs(up) + fabs(dn)) * inv_ddqz_e[i];
+        }
+    }
+}
+
+int og_velocity_tendencies_metric(const og_grid *g, int nlev, int64_t ldk, int64_t ldk_w, const double *wgt_e,
+                                  const double *inv_ddqz_e, const double *ddxn_z, const double *ddxt_z,
+                                  const double *vn, const double *w, double *ddt_vn, double *vt, double *ke_c,
+                                  double *vort, double *m_ddt)
+{
+    if (!g || nlev < 3 || ldk < nlev || ldk_w < nlev + 1) return -1;
+    double *ke_e = (double *)malloc(sizeof(double) * (size_t)(g->ne * ldk));
+    if (!ke_e) return -3;
+    og_tangential_wind(g->ne, nlev, ldk, g->e2e4, g->rbf, vn, vt);
+    og_kinetic_energy_edge(g->ne, nlev, ldk, vn, vt, ke_e);
+    og_kinetic_energy_cell(g->nc, nlev, ldk, g->c2e, g->bln, ke_e, ke_c);
+    og_vorticity(g->nv, nlev, ldk, g->v2e, g->geofac_rot, vn, vort, NULL);
+    og_ddt_vn_metric(g->ne, nlev, ldk, ldk_w, g->e2c, g->e2v, g->cgrad, g->f_e, g->c_lin, wgt_e, inv_ddqz_e, ddxn_z,
+                     ddxt_z, vn, w, vt, ke_e, ke_c, vort, ddt_vn, m_ddt);
+    free(ke_e);
+    return 0;
+}
+
+/* ------------------------------------------------------------------ */
 /* One-by-one evaluation of sampled outputs (full-size parity tests):   */
 /* the same definitions, evaluated for a single (entity, level) without  */
 /* any full-array intermediate.                                         */
@@ -1007,7 +1110,7 @@ const void *og_grid_table(const og_grid *g, const char *name)
 #define T(n) if (!strcmp(name, #n)) return g->n
     T(c2v); T(c2e); T(e2c); T(e2v); T(e2e4); T(v2e); T(v2c); T(v_deg); T(c_os); T(v_os);
     T(vert_xyz); T(cell_xyz); T(edge_xyz); T(edge_normal); T(l_e); T(d_e); T(inv_d_e); T(f_e);
-    T(c_lin); T(rbf); T(a_c); T(bln); T(adv_c); T(a_v); T(geofac_div); T(geofac_rot);
+    T(c_lin); T(cgrad); T(rbf); T(a_c); T(bln); T(adv_c); T(a_v); T(geofac_div); T(geofac_rot);
 #undef T
     return NULL;
 }

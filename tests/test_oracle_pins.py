@@ -599,6 +599,146 @@ def test_ddt_w_converges_to_the_advection_of_a_tilted_solid_body_flow(oracle_gri
 
 
 # ----------------------------------------------------------------------------------------------
+# metric variant (reading P-20): weighted KE gradient, per-edge vertical metrics,
+# contravariant correction of w
+# ----------------------------------------------------------------------------------------------
+def _tilted_setup(g, K, h_top, h0, gam, u0, w0):
+    """A hybrid terrain-following grid z(x, k) = zflat_k + h(x) (1 - zflat_k / h_top), h = h0 (x . p), flat at the top;
+    vn = (1 + gam z) vn_solid_body sampled at the heights of every edge column, w = w0. All analytic, numpy only."""
+    zflat = si.z_half_levels(K, h_top=h_top)
+    zf = 0.5 * (zflat[:-1] + zflat[1:])
+    p = np.array([np.sin(0.9) * np.cos(0.4), np.sin(0.9) * np.sin(0.4), np.cos(0.9)])
+    x = g.edge_xyz
+    h = h0 * (x @ p)
+    zh_e = zflat[None, :] + h[:, None] * (1 - zflat[None, :] / h_top)
+    zfull_e = zf[None, :] + h[:, None] * (1 - zf[None, :] / h_top)
+    gradh = h0 * (p[None, :] - (x @ p)[:, None] * x) / A             # horizontal gradient of h on the sphere of radius A
+    t = np.cross(g.edge_normal, x)                                    # t_e = n_e x x_e (P-4)
+    zn = (gradh * g.edge_normal).sum(1)[:, None] * (1 - zf[None, :] / h_top)
+    zt = (gradh * t).sum(1)[:, None] * (1 - zf[None, :] / h_top)
+    vn_sb = si.solid_body_vn(x, g.edge_normal, u0)
+    vt_sb = (u0 * np.cross(np.array([0, 0, 1.0])[None, :], x) * t).sum(1)
+    prof = 1 + gam * zfull_e
+    sinp = x[:, 2]
+    cosp = np.sqrt(1 - sinp ** 2)
+    north = (np.array([0, 0, 1.0])[None, :] - sinp[:, None] * x) / cosp[:, None]
+    nn = (north * g.edge_normal).sum(1)
+    exact = -((prof ** 2 * (u0 * u0 / A) + prof * 2 * OMEGA * u0) * (sinp * cosp * nn)[:, None]) - w0 * gam * vn_sb[:, None]
+    return dict(zflat=zflat, zh_e=zh_e, zn=zn, zt=zt, vn=prof * vn_sb[:, None], w=np.full((g.nc, K + 1), w0), vn_sb=vn_sb,
+                vt_sb=vt_sb, prof=prof, exact=exact)
+
+
+@pytest.mark.parametrize("k,seed,flags", [(0, 0, 0), (2, 0, 0), (4, 0, 0), (3, 4, 1)])
+def test_cgrad_is_second_order_from_geometry(oracle_grid, k, seed, flags):
+    """P-20: gradK = cgrad1 K(c1) - cgrad0 K(c0) + K(x_e) (cgrad0 - cgrad1) is exact for K constant (by construction), linear
+    AND quadratic along the dual arc: with signed abscissae -a0, +a1 (numpy arc distances, metres)
+    cgrad1 a1 + cgrad0 a0 = 1 and cgrad1 a1^2 - cgrad0 a0^2 = 0. Swapping the two columns fails the second identity wherever
+    a0 != a1; the plain centred difference (1/d_e, 1/d_e) fails it too."""
+    g = oracle_grid(k, seed, flags)
+    x, c0, c1 = g.edge_xyz, g.cell_xyz[g.e2c[:, 0]], g.cell_xyz[g.e2c[:, 1]]
+    a0, a1 = _arc(x, c0) * A, _arc(x, c1) * A
+    assert np.abs(g.cgrad[:, 1] * a1 + g.cgrad[:, 0] * a0 - 1).max() < 1e-13
+    assert np.abs(g.cgrad[:, 1] * a1 ** 2 - g.cgrad[:, 0] * a0 ** 2).max() < 1e-13 * (a0 + a1).max()
+    swapped = np.abs(g.cgrad[:, 0] * a1 ** 2 - g.cgrad[:, 1] * a0 ** 2).max() / (a0 + a1).max()
+    assert swapped > 1e-3
+    assert np.abs(g.cgrad[:, 0] - (a1 / a0) / g.d_e).max() < 1e-13 / g.d_e.min()
+
+
+def test_metric_from_zhalf_and_vertical_exactness_per_edge(oracle_mod, oracle_grid):
+    """per-edge level heights: weights and inverse thicknesses against numpy; the vertical term is exact for vn linear in z
+    in every column although every column has its own heights, both ends included"""
+    g = oracle_grid(1)
+    K = 7
+    rng = np.random.default_rng(31)
+    zflat = si.z_half_levels(K)
+    zh_e = zflat[None, :] * (1 + 0.3 * rng.random((g.ne, 1))) + 50.0 * rng.random((g.ne, 1))       # stretched and shifted per edge
+    wgt, inv = oracle_mod.metric_from_zhalf(zh_e, K, K)
+    dz = zh_e[:, :-1] - zh_e[:, 1:]
+    assert np.abs(inv * dz - 1).max() < 1e-15
+    assert np.abs(wgt[:, 1:K] - dz[:, :-1] / (dz[:, :-1] + dz[:, 1:])).max() < 1e-15
+    assert np.abs(wgt[:, 0] - dz[:, 0] / (dz[:, 0] + dz[:, 1])).max() < 1e-15
+    assert np.abs(wgt[:, K] - dz[:, K - 1] / (dz[:, K - 1] + dz[:, K - 2])).max() < 1e-15
+    zf = 0.5 * (zh_e[:, :-1] + zh_e[:, 1:])
+    b = (1.0 + rng.random(g.ne)) * 1e-3
+    vn = 2.0 + b[:, None] * zf
+    w = np.repeat((1.0 + 50.0 * g.cell_xyz[:, 0])[:, None], K + 1, axis=1) * (1.0 + 0.1 * np.arange(K + 1))[None, :]
+    zero = np.zeros((g.ne, K))
+    o1 = g.velocity_tendencies_metric(vn, w, wgt, inv, zero, zero, K)["ddt_vn"]
+    o0 = g.velocity_tendencies_metric(vn, np.zeros_like(w), wgt, inv, zero, zero, K)["ddt_vn"]
+    x, c0, c1 = g.edge_xyz, g.cell_xyz[g.e2c[:, 0]], g.cell_xyz[g.e2c[:, 1]]
+    a0, a1 = _arc(x, c0), _arc(x, c1)
+    wf = 0.5 * (w[:, :-1] + w[:, 1:])
+    w_e = (a1[:, None] * wf[g.e2c[:, 0]] + a0[:, None] * wf[g.e2c[:, 1]]) / (a0 + a1)[:, None]
+    want = -w_e * b[:, None]
+    assert np.abs((o1 - o0) - want).max() / np.abs(want).max() < 1e-10
+
+
+def test_metric_variant_on_flat_levels_differs_only_by_the_weighted_gradient(oracle_mod, oracle_grid):
+    """flat levels, zero slopes: ddt_metric - ddt_plain = -(weighted gradK - centred gradK), re-assembled with numpy from
+    the oracle's KE_c and a numpy KE_e; the tolerance scale M(p) is the sum of the absolute terms (two-sided)"""
+    g = oracle_grid(2)
+    K = 6
+    rng = np.random.default_rng(33)
+    vn = rng.standard_normal((g.ne, K)) * 8
+    w = rng.standard_normal((g.nc, K + 1))
+    zh = si.z_half_levels(K)
+    wgt, inv = oracle_mod.metric_from_zhalf(np.repeat(zh[None, :], g.ne, axis=0), K, K)
+    zero = np.zeros((g.ne, K))
+    om = g.velocity_tendencies_metric(vn, w, wgt, inv, zero, zero, K, with_scale=True)
+    op = g.velocity_tendencies(vn, w, zh, K, with_scale=True)
+    ke_e = 0.5 * (vn * vn + op["vt"] ** 2)
+    kc = op["ke_c"]
+    c0, c1 = g.e2c[:, 0], g.e2c[:, 1]
+    gw = g.cgrad[:, 1:] * kc[c1] - g.cgrad[:, :1] * kc[c0] + ke_e * (g.cgrad[:, :1] - g.cgrad[:, 1:])
+    gp = (kc[c1] - kc[c0]) * g.inv_d_e[:, None]
+    assert (np.abs((om["ddt_vn"] - op["ddt_vn"]) + (gw - gp)) <= 1e-13 * (om["m_ddt"] + op["m_ddt"])).all()
+    assert np.abs(gw - gp).max() > 1e-3 * np.abs(gp).max()            # the weighting is not a no-op on this grid
+    m = g.cgrad[:, 1:] * np.abs(kc[c1]) + g.cgrad[:, :1] * np.abs(kc[c0]) + np.abs(ke_e) * np.abs(g.cgrad[:, :1] - g.cgrad[:, 1:]) \
+        + (op["m_ddt"] - (np.abs(kc[c1]) + np.abs(kc[c0])) * g.inv_d_e[:, None])
+    assert (om["m_ddt"] <= 1.000001 * m).all() and (om["m_ddt"] >= 0.999999 * m).all()
+
+
+def test_contravariant_correction_closed_form(oracle_mod, oracle_grid):
+    """On coordinate surfaces z(x, k) the horizontal operators see (d/dn)|_s = (d/dn)|_z + z_n d/dz; collecting the metric
+    terms of dK/dn and vt zeta gives exactly -(vn z_n + vt z_t) dvn/dz (P-20), i.e. vertical advection with the
+    contravariant velocity w - vn z_n - vt z_t. Pin of that term alone: the difference of the oracle with and without the
+    slopes equals +(vn z_n + vt z_t) gam vn_sb, with vt the ANALYTIC tangential wind; a wrong sign gives a relative
+    error of 2, swapped slopes 2.3. Values: R2B2..4 3.3e-3, 1.8e-3, 1.3e-3 (the RBF reconstruction of vt)."""
+    K, gam = 6, 4.0e-5
+    errs = []
+    for k in (2, 3, 4):
+        g = oracle_grid(k)
+        s = _tilted_setup(g, K, 3.0e4, 9.0e3, gam, 20.0, 0.1)
+        wgt, inv = oracle_mod.metric_from_zhalf(s["zh_e"], K, K)
+        a = g.velocity_tendencies_metric(s["vn"], s["w"], wgt, inv, s["zn"], s["zt"], K)["ddt_vn"]
+        b = g.velocity_tendencies_metric(s["vn"], s["w"], wgt, inv, 0 * s["zn"], 0 * s["zt"], K)["ddt_vn"]
+        want = (s["vn"] * s["zn"] + s["prof"] * s["vt_sb"][:, None] * s["zt"]) * gam * s["vn_sb"][:, None]
+        errs.append(np.abs((a - b) - want).max() / np.abs(want).max())
+        assert np.abs((a - b) + want).max() / np.abs(want).max() > 1.9
+    assert errs[0] < 5e-3 and errs[1] < 3e-3 and errs[2] < 2e-3, errs
+
+
+def test_metric_tendency_converges_on_a_tilted_grid(oracle_mod, oracle_grid):
+    """the whole tendency on the tilted grid against the z-coordinate closed form of the flat pin (the physical field is the
+    same, only the coordinate surfaces tilt): first-order convergence as on flat levels, and dropping the correction
+    doubles the error at R2B4. Values with / without: R2B2 8.2e-3 / 8.3e-3, R2B3 4.3e-3 / 5.6e-3, R2B4 2.7e-3 / 5.7e-3."""
+    K, gam = 6, 4.0e-5
+    with_c, without = [], []
+    for k in (2, 3, 4):
+        g = oracle_grid(k)
+        s = _tilted_setup(g, K, 3.0e4, 9.0e3, gam, 20.0, 0.1)
+        wgt, inv = oracle_mod.metric_from_zhalf(s["zh_e"], K, K)
+        a = g.velocity_tendencies_metric(s["vn"], s["w"], wgt, inv, s["zn"], s["zt"], K)["ddt_vn"]
+        b = g.velocity_tendencies_metric(s["vn"], s["w"], wgt, inv, 0 * s["zn"], 0 * s["zt"], K)["ddt_vn"]
+        scale = np.abs(s["exact"]).max()
+        with_c.append(np.abs(a - s["exact"]).max() / scale)
+        without.append(np.abs(b - s["exact"]).max() / scale)
+    assert with_c[0] < 1.0e-2 and with_c[1] < 5.5e-3 and with_c[2] < 3.5e-3, with_c
+    assert with_c[0] / with_c[2] > 2.4
+    assert without[2] > 1.8 * with_c[2], (with_c, without)
+
+
+# ----------------------------------------------------------------------------------------------
 # seeded permutation (P-7)
 # ----------------------------------------------------------------------------------------------
 def _perm_from_positions(a_perm, a_canon, decimals=12):
