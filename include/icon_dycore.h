@@ -88,6 +88,7 @@ enum {
     ICON_TAB_GEOFAC_ROT,   /* f64 [nv][6] d_e*v_os/A_v, 0 in the pentagon pad */
     ICON_TAB_ADV_C,        /* f64 [nc][3] normal-component reconstruction weights of the vertical-wind tendency:
                               sum_j adv_c(c,j) n_j n_j^T = I in the tangent plane of the cell (P-19) */
+    ICON_TAB_CGRAD,        /* f64 [ne][2] distance-weighted KE-gradient coefficients (a1/a0)/d_e, (a0/a1)/d_e (P-20) */
     ICON_TAB_COUNT
 };
 
@@ -196,6 +197,35 @@ int dycore_velocity_tendencies(const icon_grid_t* g, int dtype, int nlev, int ld
  */
 int dycore_w_tendency(const icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
                       const void* vn, const void* w, void* ddt_w, void* cuda_stream);
+
+/*
+ * dycore_metric_from_zhalf -- SURVEY.md 8(f) NEXT-1, set-up of the metric variant (reading P-20; PAPER.md:56 names the
+ * "terrain following hybrid sigma height grid", the paper prints no formula): from the half-level heights of every EDGE
+ * column, z_half_e [ne][ldk_w] dev in (strictly decreasing in k, levels 0 .. nlev), derives
+ *   wgt_e      [ne][ldk_w] dev out: k = 1 .. nlev-1 the weight of vn(k) in vn_ie(k), dz(k-1) / (dz(k-1) + dz(k));
+ *                                   k = 0, k = nlev the linear-extrapolation ratios dz0/(dz0+dz1), dz(K-1)/(dz(K-1)+dz(K-2))
+ *   inv_ddqz_e [ne][ldk]   dev out: 1 / dz(k), dz(k) = z_half_e(k) - z_half_e(k+1).
+ * Static in a model run: not part of any timed region. 3 <= nlev <= ldk, nlev+1 <= ldk_w; pads untouched.
+ */
+int dycore_metric_from_zhalf(const icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, const void* z_half_e,
+                             void* wgt_e, void* inv_ddqz_e, void* cuda_stream);
+
+/*
+ * dycore_velocity_tendencies_metric -- SURVEY.md 8(f) NEXT-1: S3-S7 in their ICON-faithful metric form (reading P-20).
+ * S3, S4, S2 as in dycore_velocity_tendencies (along the coordinate surfaces), then
+ *   gradK  = cgrad(e,1) KE_c(c1) - cgrad(e,0) KE_c(c0) + KE_e(e) (cgrad(e,0) - cgrad(e,1))        (ICON_TAB_CGRAD)
+ *   vn_ie  = per-edge weights: k = 1..nlev-1: wgt_e vn(k) + (1 - wgt_e) vn(k-1); ends: vn(0) + wgt_e(0) (vn(0) - vn(1)),
+ *            vn(nlev-1) + wgt_e(nlev) (vn(nlev-1) - vn(nlev-2))
+ *   ddt_vn = -[ gradK + vt (f_e + 1/2(zeta(v0)+zeta(v1)))
+ *               + (w_e - vn ddxn_z - vt ddxt_z) (vn_ie(k) - vn_ie(k+1)) inv_ddqz_e ],   w_e as in S6.
+ * wgt_e [ne][ldk_w], inv_ddqz_e, ddxn_z, ddxt_z [ne][ldk] dev in (ddxn_z, ddxt_z = slopes dz/dn, dz/dt of the full-level
+ * coordinate surface at the edge midpoint, t = n x x_e); vn [ne][ldk], w [nc][ldk_w] dev in; ddt_vn [ne][ldk] dev out.
+ * One fused column-cache kernel where it holds the columns (nlev <= 95; the metric columns of an owned edge are read
+ * straight from global memory, each exactly once), else the unfused pipeline. 3 <= nlev <= ldk, nlev+1 <= ldk_w.
+ */
+int dycore_velocity_tendencies_metric(const icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w,
+                                      const void* wgt_e, const void* inv_ddqz_e, const void* ddxn_z, const void* ddxt_z,
+                                      const void* vn, const void* w, void* ddt_vn, void* cuda_stream);
 
 /*
  * dycore_step -- one pass of the whole hot path: the outputs of

@@ -23,13 +23,13 @@ ICON_OPT_CC_PACE = 2
 
 TABLES = ("c2v", "c2e", "e2c", "e2v", "e2e4", "v2e", "v2c", "v_deg", "c_os", "v_os",
           "vert_xyz", "cell_xyz", "edge_xyz", "edge_normal", "l_e", "d_e", "inv_d_e", "f_e", "c_lin", "rbf",
-          "a_c", "bln", "a_v", "geofac_div", "geofac_rot", "adv_c")
+          "a_c", "bln", "a_v", "geofac_div", "geofac_rot", "adv_c", "cgrad")
 TABLE_ID = {n: i for i, n in enumerate(TABLES)}
 
 # every symbol include/icon_dycore.h declares
 EXPORTS = ("icon_grid_create", "icon_grid_destroy", "icon_grid_counts", "icon_grid_table_host",
            "icon_grid_table_device", "icon_grid_set_option", "icon_grid_cc_schedule_check", "dycore_div_vort", "dycore_velocity_tendencies",
-           "dycore_step", "dycore_step_host", "dycore_step_w", "dycore_w_tendency", "dycore_velocity_tendencies_noalloc", "icon_grid_launch_count", "icon_last_error")
+           "dycore_step", "dycore_step_host", "dycore_step_w", "dycore_w_tendency", "dycore_velocity_tendencies_noalloc", "dycore_metric_from_zhalf", "dycore_velocity_tendencies_metric", "icon_grid_launch_count", "icon_last_error")
 
 
 class IconError(RuntimeError):
@@ -75,6 +75,10 @@ def load_library():
     L.dycore_w_tendency.argtypes = [P, ci, ci, ci, ci, P, P, P, P, P]
     L.dycore_velocity_tendencies_noalloc.restype = ci
     L.dycore_velocity_tendencies_noalloc.argtypes = [P, ci, ci, ci, ci, P, P, P, P, P]
+    L.dycore_metric_from_zhalf.restype = ci
+    L.dycore_metric_from_zhalf.argtypes = [P, ci, ci, ci, ci, P, P, P, P]
+    L.dycore_velocity_tendencies_metric.restype = ci
+    L.dycore_velocity_tendencies_metric.argtypes = [P, ci, ci, ci, ci, P, P, P, P, P, P, P, P]
     L.dycore_step_w.restype = ci
     L.dycore_step_w.argtypes = [P, ci, ci, ci, ci, P, P, P, P, P, P, P, P]
     L.dycore_step.restype = ci
@@ -234,6 +238,23 @@ def dycore_velocity_tendencies_noalloc(grid, z_half, vn, w, ddt_vn, nlev, stream
     _check_fields((("vn", vn, grid.ne, "ldk"), ("w", w, grid.nc, "ldk_w"), ("ddt_vn", ddt_vn, grid.ne, "ldk")))
     _check(grid._L.dycore_velocity_tendencies_noalloc(grid._h, _dtype_of(vn), int(nlev), int(vn.shape[1]), int(w.shape[1]),
                                                       _dptr(z), _dptr(vn), _dptr(w), _dptr(ddt_vn), _stream_ptr(stream)))
+
+
+def dycore_metric_from_zhalf(grid, z_half_e, wgt_e, inv_ddqz_e, nlev, stream=None):
+    """Set-up of the metric variant (reading P-20): z_half_e, wgt_e [ne][ldk_w], inv_ddqz_e [ne][ldk]: CUDA tensors."""
+    _check_fields((("z_half_e", z_half_e, grid.ne, "ldk_w"), ("wgt_e", wgt_e, grid.ne, "ldk_w"), ("inv_ddqz_e", inv_ddqz_e, grid.ne, "ldk")))
+    _check(grid._L.dycore_metric_from_zhalf(grid._h, _dtype_of(z_half_e), int(nlev), int(inv_ddqz_e.shape[1]), int(z_half_e.shape[1]),
+                                            _dptr(z_half_e), _dptr(wgt_e), _dptr(inv_ddqz_e), _stream_ptr(stream)))
+
+
+def dycore_velocity_tendencies_metric(grid, wgt_e, inv_ddqz_e, ddxn_z, ddxt_z, vn, w, ddt_vn, nlev, stream=None):
+    """S3-S7 in their metric form (reading P-20): weighted KE gradient, per-edge vertical metrics, contravariant correction."""
+    _check_fields((("vn", vn, grid.ne, "ldk"), ("w", w, grid.nc, "ldk_w"), ("ddt_vn", ddt_vn, grid.ne, "ldk"),
+                   ("wgt_e", wgt_e, grid.ne, "ldk_w"), ("inv_ddqz_e", inv_ddqz_e, grid.ne, "ldk"), ("ddxn_z", ddxn_z, grid.ne, "ldk"),
+                   ("ddxt_z", ddxt_z, grid.ne, "ldk")))
+    _check(grid._L.dycore_velocity_tendencies_metric(grid._h, _dtype_of(vn), int(nlev), int(vn.shape[1]), int(w.shape[1]), _dptr(wgt_e),
+                                                     _dptr(inv_ddqz_e), _dptr(ddxn_z), _dptr(ddxt_z), _dptr(vn), _dptr(w), _dptr(ddt_vn),
+                                                     _stream_ptr(stream)))
 
 
 def dycore_w_tendency(grid, z_half, vn, w, ddt_w, nlev, stream=None):

@@ -122,6 +122,7 @@ int ensure_coeffs(icon_grid* g, icon::DevCoeffs<T>& c) {
     if ((rc = upload_rows(g, h.f_e, 1, ue, &c.f_e))) return rc;
     if ((rc = upload_rows(g, h.c_lin, 2, ue, &c.c_lin))) return rc;
     if ((rc = upload_rows(g, h.adv_c, 3, uc, &c.adv_c))) return rc;
+    if ((rc = upload_rows(g, h.cgrad, 2, ue, &c.cgrad))) return rc;
     CU_TRY(cudaStreamSynchronize(cudaStreamLegacy));      // uploads ran on the legacy stream, callers may use non-blocking streams
     c.ready = true;
     return ICON_OK;
@@ -504,6 +505,7 @@ int table_info(const icon_grid* g, int which, TableInfo* t) {
         case ICON_TAB_GEOFAC_DIV: D(h.geofac_div, h.nc, 3); break;
         case ICON_TAB_GEOFAC_ROT: D(h.geofac_rot, h.nv, 6); break;
         case ICON_TAB_ADV_C: D(h.adv_c, h.nc, 3); break;
+        case ICON_TAB_CGRAD: D(h.cgrad, h.ne, 2); break;
         default: return fail(ICON_EINVAL, "unknown table selector");
     }
     return ICON_OK;
@@ -811,6 +813,87 @@ int dycore_step(const icon_grid_t* gc, int dtype, int nlev, int ldk, int ldk_w, 
                                     nullptr, nullptr, s, div, vort, &fused);
     if (rc || fused) return rc;
     return dycore_div_vort(g, dtype, nlev, ldk, vn, div, vort, cuda_stream);
+}
+
+int dycore_metric_from_zhalf(const icon_grid_t* gc, int dtype, int nlev, int ldk, int ldk_w, const void* z_half_e, void* wgt_e,
+                             void* inv_ddqz_e, void* cuda_stream) {
+    icon_grid* g = const_cast<icon_grid*>(gc);
+    int rc = check_common(g, dtype, nlev, ldk, 3);
+    if (rc) return rc;
+    const size_t es = dtype == ICON_F64 ? 8 : 4;
+    if (ldk_w < nlev + 1) return fail(ICON_EINVAL, "ldk_w < nlev + 1");
+    if (((int64_t)ldk_w * (int64_t)es) % 16) return fail(ICON_EINVAL, "ldk_w*sizeof(T) must be a multiple of 16");
+    if ((rc = check_field(z_half_e, "z_half_e")) || (rc = check_field(wgt_e, "wgt_e")) || (rc = check_field(inv_ddqz_e, "inv_ddqz_e")))
+        return rc;
+    const size_t bw = (size_t)g->host.ne * ldk_w * es, bk = (size_t)g->host.ne * ldk * es;
+    if (overlaps(wgt_e, bw, z_half_e, bw) || overlaps(inv_ddqz_e, bk, z_half_e, bw) || overlaps(wgt_e, bw, inv_ddqz_e, bk))
+        return fail(ICON_EINVAL, "outputs must not alias the input or each other");
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const int n = dtype == ICON_F64
+                      ? icon::launch_metric_from_zhalf<double>(*g, nlev, ldk, ldk_w, (const double*)z_half_e, (double*)wgt_e, (double*)inv_ddqz_e, s)
+                      : icon::launch_metric_from_zhalf<float>(*g, nlev, ldk, ldk_w, (const float*)z_half_e, (float*)wgt_e, (float*)inv_ddqz_e, s);
+    if (n < 0) return fail_cuda((cudaError_t)(-n), "kernel launch");
+    g->launches += n;
+    return ICON_OK;
+}
+
+}  // extern "C"
+
+namespace {
+template <class T>
+int tendencies_metric_impl(icon_grid* g, icon::DevCoeffs<T>& c, icon::DevCcTables<T>& ct, int dtype, int nlev, int ldk, int ldk_w,
+                           const void* wgt, const void* inv, const void* zn, const void* zt, const void* vn, const void* w, void* ddt_vn,
+                           cudaStream_t s) {
+    int rc;
+    if ((rc = ensure_coeffs(g, c))) return rc;
+    int n;
+    if (g->options[ICON_OPT_TENDENCY_KERNEL] >= 4) {
+        if ((rc = ensure_cc_tables(g, ct, nlev, ldk, ldk_w, icon::kCcTendM))) return rc;
+        if (!ct.unsupported) {
+            icon::CcMetric<T> m{(const T*)wgt, (const T*)inv, (const T*)zn, (const T*)zt};
+            n = icon::launch_tendencies_cc<T>(*g, ct, icon::kCcTendM, nlev, ldk, ldk_w, nullptr, (const T*)vn, (const T*)w, (T*)ddt_vn, nullptr,
+                                              nullptr, s, nullptr, nullptr, &m);
+            if (n < 0) return fail_cuda((cudaError_t)(-n), "kernel launch");
+            g->launches += n;
+            return ICON_OK;
+        }
+    }
+    // level counts the column cache cannot hold, or ICON_OPT_TENDENCY_KERNEL 0 / 3: the unfused pipeline with its metric last stage
+    if ((rc = ensure_workspace<T>(g, dtype, ldk))) return rc;
+    n = icon::launch_tendencies_unfused_metric<T>(*g, c, nlev, ldk, ldk_w, (const T*)wgt, (const T*)inv, (const T*)zn, (const T*)zt,
+                                                  (const T*)vn, (const T*)w, (T*)ddt_vn, (T*)g->ws.vt, (T*)g->ws.ke_e, (T*)g->ws.ke_c,
+                                                  (T*)g->ws.vort, s);
+    if (n < 0) return fail_cuda((cudaError_t)(-n), "kernel launch");
+    g->launches += n;
+    return ICON_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int dycore_velocity_tendencies_metric(const icon_grid_t* gc, int dtype, int nlev, int ldk, int ldk_w, const void* wgt_e,
+                                      const void* inv_ddqz_e, const void* ddxn_z, const void* ddxt_z, const void* vn, const void* w,
+                                      void* ddt_vn, void* cuda_stream) {
+    icon_grid* g = const_cast<icon_grid*>(gc);
+    int rc = check_common(g, dtype, nlev, ldk, 3);
+    if (rc) return rc;
+    const size_t es = dtype == ICON_F64 ? 8 : 4;
+    if (ldk_w < nlev + 1) return fail(ICON_EINVAL, "ldk_w < nlev + 1");
+    if (((int64_t)ldk_w * (int64_t)es) % 16) return fail(ICON_EINVAL, "ldk_w*sizeof(T) must be a multiple of 16");
+    if ((rc = check_field(wgt_e, "wgt_e")) || (rc = check_field(inv_ddqz_e, "inv_ddqz_e")) || (rc = check_field(ddxn_z, "ddxn_z")) ||
+        (rc = check_field(ddxt_z, "ddxt_z")) || (rc = check_field(vn, "vn")) || (rc = check_field(w, "w")) || (rc = check_field(ddt_vn, "ddt_vn")))
+        return rc;
+    {
+        const size_t be = (size_t)g->host.ne * ldk * es, bew = (size_t)g->host.ne * ldk_w * es, bw = (size_t)g->host.nc * ldk_w * es;
+        const void* ins[6] = {wgt_e, inv_ddqz_e, ddxn_z, ddxt_z, vn, w};
+        const size_t ib[6] = {bew, be, be, be, be, bw};
+        for (int i = 0; i < 6; ++i)
+            if (overlaps(ddt_vn, be, ins[i], ib[i])) return fail(ICON_EINVAL, "outputs must not alias inputs");
+    }
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    if (dtype == ICON_F64)
+        return tendencies_metric_impl<double>(g, g->c64, g->m64, dtype, nlev, ldk, ldk_w, wgt_e, inv_ddqz_e, ddxn_z, ddxt_z, vn, w, ddt_vn, s);
+    return tendencies_metric_impl<float>(g, g->c32, g->m32, dtype, nlev, ldk, ldk_w, wgt_e, inv_ddqz_e, ddxn_z, ddxt_z, vn, w, ddt_vn, s);
 }
 
 int dycore_step_w(const icon_grid_t* gc, int dtype, int nlev, int ldk, int ldk_w, const double* z_half, const void* vn, const void* w,

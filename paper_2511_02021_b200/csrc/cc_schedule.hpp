@@ -68,11 +68,15 @@ constexpr int kCcAhead = 3;              // steps the producers read the schedul
 constexpr int kCcBarrierBytes = 512;    // the mbarriers
 // What a launch of the kernel produces; each mode has a schedule of its own (DevCcTables::mode).
 enum { kCcTend = 0 /* ddt_vn */, kCcStep = 1 /* ddt_vn + div + vort */, kCcDivVort = 2 /* div + vort only */,
-       kCcStepW = 3 /* ddt_vn + div + vort + ddt_w (P-19): three more w columns and twelve more coefficients per patch */ };
+       kCcStepW = 3 /* ddt_vn + div + vort + ddt_w (P-19): three more w columns and twelve more coefficients per patch */,
+       kCcTendM = 4 /* ddt_vn in its metric form (P-20): 24 more coefficients per patch; the four metric columns of an owned
+                       edge are read straight from global memory */ };
 // kCcDivVort reads 27 of the 36 vn columns of a patch and no w column, and its records carry only the 52 coefficients it
 // needs: geofac_div [4][3], rot of the midpoints [3][6] (+2 pad), rot of the corners [3][6] (+2 pad)
 enum { DVF_DIV = 0, DVF_ROT = 12, DVF_XROT = 32, kCcDvCoefWords = 52 };
-CC_HD constexpr int cc_coef_words(int mode) { return mode == kCcDivVort ? (int)kCcDvCoefWords : mode == kCcStepW ? (int)kScCoefWords : (int)SCF_ADV; }
+CC_HD constexpr int cc_coef_words(int mode) {
+    return mode == kCcDivVort ? (int)kCcDvCoefWords : mode == kCcTendM ? (int)kScCoefWords : mode == kCcStepW ? (int)SCF_CGRAD : (int)SCF_ADV;
+}
 // id slots (sc_tables.hpp) a mode reads: bit i of the mask = column i of the patch is needed
 constexpr uint64_t cc_use_mask(int mode) {
     if (mode == kCcStepW) return (1ull << SID_PAD) - 1;                  // every column

@@ -26,6 +26,7 @@ struct DevCoeffs {
     T* f_e = nullptr;         // [ne]
     T* c_lin = nullptr;       // [ne][2]
     T* adv_c = nullptr;       // [nc][3]
+    T* cgrad = nullptr;       // [ne][2]
     bool ready = false;
 };
 
@@ -119,6 +120,8 @@ struct icon_grid {
     icon::DevCcTables<float> dv32;
     icon::DevCcTables<double> sw64;                    // the same for dycore_step_w (mode kCcStepW)
     icon::DevCcTables<float> sw32;
+    icon::DevCcTables<double> m64;                     // the same for dycore_velocity_tendencies_metric (mode kCcTendM)
+    icon::DevCcTables<float> m32;
     int smem_optin = 0;                                // cudaDevAttrMaxSharedMemoryPerBlockOptin
     std::vector<icon::LevelCoeffs> level_coeffs;
     icon::Workspace ws;

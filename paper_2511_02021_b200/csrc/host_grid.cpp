@@ -205,6 +205,7 @@ void build_geometry(HostGrid& g) {
     g.inv_d_e.resize((size_t)ne);
     g.f_e.resize((size_t)ne);
     g.c_lin.resize(2 * (size_t)ne);
+    g.cgrad.resize(2 * (size_t)ne);
     g.rbf.resize(4 * (size_t)ne);
     g.bln.resize(3 * (size_t)nc);
     g.adv_c.resize(3 * (size_t)nc);
@@ -235,6 +236,9 @@ void build_geometry(HostGrid& g) {
         g.f_e[e] = 2.0 * kOmega * x.z;
         g.c_lin[2 * e] = arc(x, c1) / de;
         g.c_lin[2 * e + 1] = arc(x, c0) / de;
+        // P-20 distance-weighted KE-gradient coefficients, from the two linear weights: c_lin0 / c_lin1 = a1 / a0
+        g.cgrad[2 * e] = (g.c_lin[2 * e] / g.c_lin[2 * e + 1]) * g.inv_d_e[e];
+        g.cgrad[2 * e + 1] = (g.c_lin[2 * e + 1] / g.c_lin[2 * e]) * g.inv_d_e[e];
     }
     // folded divergence factor and P-10 bilinear (gnomonic-plane) weights
 #pragma omp parallel for schedule(static)

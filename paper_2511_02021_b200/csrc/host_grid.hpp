@@ -16,7 +16,7 @@ struct HostGrid {
     std::vector<int8_t> c_os, v_os;
     // geometry / coefficients (G2)
     std::vector<double> vert_xyz, cell_xyz, edge_xyz, edge_normal;
-    std::vector<double> l_e, d_e, inv_d_e, f_e, c_lin, rbf, a_c, bln, a_v, geofac_div, geofac_rot, adv_c;
+    std::vector<double> l_e, d_e, inv_d_e, f_e, c_lin, rbf, a_c, bln, a_v, geofac_div, geofac_rot, adv_c, cgrad;
     // generation (hierarchical, spatially local) order: user id of the entity at canonical
     // position p. Empty when the user numbering IS the canonical one.
     std::vector<int32_t> user_of_pos_c, user_of_pos_e, user_of_pos_v;

@@ -271,6 +271,64 @@ __global__ void __launch_bounds__(256) k_w_tend(int64_t nc, int nlev, int64_t ld
     }
 }
 
+// ------------------------------------------------------------------------------------------
+// Metric variant (reading P-20), plain kernels: set-up of the per-edge vertical metrics and the
+// last stage of the unfused pipeline. One warp per edge column, lanes = levels.
+// ------------------------------------------------------------------------------------------
+template <class T>
+__global__ void __launch_bounds__(256) k_metric_from_zhalf(int64_t ne, int nlev, int64_t ldk, int64_t ldk_w,
+                                                           const T* __restrict__ zh, T* __restrict__ wgt, T* __restrict__ inv) {
+    const int64_t e = (int64_t)blockIdx.x * 8 + warp_in_block();
+    if (e >= ne) return;
+    const T* z = zh + e * ldk_w;
+    for (int k = lane_id(); k <= nlev; k += kWarp) {
+        if (k < nlev) inv[e * ldk + k] = (T)1 / (z[k] - z[k + 1]);
+        T up, dn;
+        if (k == 0) { up = z[0] - z[1]; dn = z[1] - z[2]; }                                   // dz0 / (dz0 + dz1)
+        else if (k == nlev) { up = z[nlev - 1] - z[nlev]; dn = z[nlev - 2] - z[nlev - 1]; }   // dz(K-1) / (dz(K-1) + dz(K-2))
+        else { up = z[k - 1] - z[k]; dn = z[k] - z[k + 1]; }
+        wgt[e * ldk_w + k] = up / (up + dn);
+    }
+}
+
+template <class T>
+__global__ void __launch_bounds__(256) k_ddt_vn_metric(int64_t ne, int nlev, int64_t ldk, int64_t ldk_w,
+                                                       const int32_t* __restrict__ e2c, const int32_t* __restrict__ e2v,
+                                                       const T* __restrict__ cgrad, const T* __restrict__ f_e,
+                                                       const T* __restrict__ c_lin, const int32_t* __restrict__ user_e,
+                                                       const T* __restrict__ wgt, const T* __restrict__ inv,
+                                                       const T* __restrict__ zn, const T* __restrict__ zt,
+                                                       const T* __restrict__ vn, const T* __restrict__ w,
+                                                       const T* __restrict__ vt, const T* __restrict__ ke_e,
+                                                       const T* __restrict__ ke_c, const T* __restrict__ vort,
+                                                       T* __restrict__ ddt_vn) {
+    const int64_t p = (int64_t)blockIdx.x * 8 + warp_in_block();
+    if (p >= ne) return;
+    const int lane = lane_id();
+    const int64_t e = user_e ? user_e[p] : p;
+    const int64_t c0 = ldg(e2c + 2 * p), c1 = ldg(e2c + 2 * p + 1), v0 = ldg(e2v + 2 * p), v1 = ldg(e2v + 2 * p + 1);
+    const T g0 = ldg(cgrad + 2 * p), g1 = ldg(cgrad + 2 * p + 1), f = ldg(f_e + p), cl0 = ldg(c_lin + 2 * p), cl1 = ldg(c_lin + 2 * p + 1);
+    const T* col = vn + e * ldk;
+    const T* wg = wgt + e * ldk_w;
+    auto half = [&](int k) {
+        if (k == 0) return col[0] + wg[0] * (col[0] - col[1]);
+        if (k == nlev) return col[nlev - 1] + wg[nlev] * (col[nlev - 1] - col[nlev - 2]);
+        return wg[k] * col[k] + ((T)1 - wg[k]) * col[k - 1];
+    };
+    for (int k = lane; k < nlev; k += kWarp) {
+        const int64_t i = e * ldk + k;
+        const T t = vt[i];
+        const T gradk = g1 * ke_c[c1 * ldk + k] - g0 * ke_c[c0 * ldk + k] + ke_e[i] * (g0 - g1);
+        const T zeta_e = (T)0.5 * (vort[v0 * ldk + k] + vort[v1 * ldk + k]);
+        const T H = gradk + t * (f + zeta_e);
+        const T wf0 = (T)0.5 * (w[c0 * ldk_w + k] + w[c0 * ldk_w + k + 1]);
+        const T wf1 = (T)0.5 * (w[c1 * ldk_w + k] + w[c1 * ldk_w + k + 1]);
+        const T w_e = cl0 * wf0 + cl1 * wf1;
+        const T w_cc = col[k] * zn[i] + t * zt[i];
+        ddt_vn[i] = -(H + (w_e - w_cc) * (half(k) - half(k + 1)) * inv[i]);
+    }
+}
+
 inline unsigned blocks_for(int64_t n, int per_block) { return (unsigned)((n + per_block - 1) / per_block); }
 
 }  // namespace
@@ -315,6 +373,30 @@ int launch_tendencies_unfused(const icon_grid& g, const DevCoeffs<T>& c, int nle
 }
 
 template <class T>
+int launch_metric_from_zhalf(const icon_grid& g, int nlev, int64_t ldk, int64_t ldk_w, const T* zh, T* wgt, T* inv, cudaStream_t s) {
+    const int64_t ne = g.host.ne;
+    k_metric_from_zhalf<T><<<blocks_for(ne, 8), 256, 0, s>>>(ne, nlev, ldk, ldk_w, zh, wgt, inv);
+    cudaError_t err = cudaGetLastError();
+    return err == cudaSuccess ? 1 : -(int)err;
+}
+
+template <class T>
+int launch_tendencies_unfused_metric(const icon_grid& g, const DevCoeffs<T>& c, int nlev, int64_t ldk, int64_t ldk_w, const T* wgt,
+                                     const T* inv, const T* zn, const T* zt, const T* vn, const T* w, T* ddt_vn, T* vt, T* ke_e,
+                                     T* ke_c, T* vort, cudaStream_t s) {
+    const int64_t nc = g.host.nc, ne = g.host.ne, nv = g.host.nv;
+    k_vt_kee<T><<<blocks_for(ne, 8), 256, 0, s>>>(ne, nlev, ldk, g.tab.e2e4, c.rbf, g.tab.user_e, vn, vt, ke_e);
+    unsigned nb = blocks_for(nc, 8), nbv = blocks_for(nv, 4);
+    if (nbv > nb) nb = nbv;
+    k_kec_vort<T><<<nb, 384, 0, s>>>(nc, nv, nlev, ldk, g.tab.c2e, c.bln, g.tab.v2e, c.geofac_rot, g.tab.user_c,
+                                     g.tab.user_v, ke_e, vn, ke_c, vort);
+    k_ddt_vn_metric<T><<<blocks_for(ne, 8), 256, 0, s>>>(ne, nlev, ldk, ldk_w, g.tab.e2c, g.tab.e2v, c.cgrad, c.f_e, c.c_lin,
+                                                         g.tab.user_e, wgt, inv, zn, zt, vn, w, vt, ke_e, ke_c, vort, ddt_vn);
+    cudaError_t err = cudaGetLastError();
+    return err == cudaSuccess ? 3 : -(int)err;
+}
+
+template <class T>
 int launch_w_tendency(const icon_grid& g, const DevCoeffs<T>& c, int nlev, int64_t ldk, int64_t ldk_w, const T* wk,
                       const T* vn, const T* w, T* ddt_w, cudaStream_t s) {
     const int64_t nc = g.host.nc;
@@ -329,7 +411,11 @@ int launch_w_tendency(const icon_grid& g, const DevCoeffs<T>& c, int nlev, int64
     template int launch_tendencies_unfused<T>(const icon_grid&, const DevCoeffs<T>&, int, int64_t, int64_t, const T*,     \
                                               const T*, const T*, T*, T*, T*, T*, T*, cudaStream_t);                      \
     template int launch_w_tendency<T>(const icon_grid&, const DevCoeffs<T>&, int, int64_t, int64_t, const T*, const T*,   \
-                                      const T*, T*, cudaStream_t);
+                                      const T*, T*, cudaStream_t);                                                        \
+    template int launch_metric_from_zhalf<T>(const icon_grid&, int, int64_t, int64_t, const T*, T*, T*, cudaStream_t);    \
+    template int launch_tendencies_unfused_metric<T>(const icon_grid&, const DevCoeffs<T>&, int, int64_t, int64_t,        \
+                                                     const T*, const T*, const T*, const T*, const T*, const T*, T*, T*,  \
+                                                     T*, T*, T*, cudaStream_t);
 ICON_INSTANTIATE(double)
 ICON_INSTANTIATE(float)
 

@@ -25,6 +25,14 @@ template <class T>
 int launch_w_tendency(const icon_grid& g, const DevCoeffs<T>& c, int nlev, int64_t ldk, int64_t ldk_w, const T* wk,
                       const T* vn, const T* w, T* ddt_w, cudaStream_t s);
 
+// Metric variant (reading P-20): set-up of the per-edge vertical metrics, and the unfused pipeline with its metric last stage.
+template <class T>
+int launch_metric_from_zhalf(const icon_grid& g, int nlev, int64_t ldk, int64_t ldk_w, const T* zh, T* wgt, T* inv, cudaStream_t s);
+template <class T>
+int launch_tendencies_unfused_metric(const icon_grid& g, const DevCoeffs<T>& c, int nlev, int64_t ldk, int64_t ldk_w, const T* wgt,
+                                     const T* inv, const T* zn, const T* zt, const T* vn, const T* w, T* ddt_vn, T* vt, T* ke_e,
+                                     T* ke_c, T* vort, cudaStream_t s);
+
 // S2-S7, self-contained patch kernel (kernels_sc.cu): one warp per patch, all level chunks of a
 // column in flight at once, no exchange between warps; reads vn, w and the records, writes ddt_vn.
 template <class T>
@@ -35,10 +43,15 @@ int launch_tendencies_sc(const icon_grid& g, const DevScTables<T>& p, int nlev, 
 // shared-memory slots with bulk asynchronous copies following the host-built schedule
 // (cc_schedule.hpp); consumer warps finish one self-contained patch each from the slots. mode = kCcTend (ddt_vn),
 // kCcStep (ddt_vn + div + vort in one pass: dycore_step) or kCcDivVort (div + vort only, tables built for that mode).
+// device pointers of the metric columns of reading P-20 (mode kCcTendM)
+template <class T>
+struct CcMetric {
+    const T *wgt, *inv, *zn, *zt;      // wgt_e [ne][ldk_w]; inv_ddqz_e, ddxn_z, ddxt_z [ne][ldk]
+};
 template <class T>
 int launch_tendencies_cc(const icon_grid& g, DevCcTables<T>& p, int mode, int nlev, int64_t ldk, int64_t ldk_w,
                          const T* abc, const T* vn, const T* w, T* ddt_vn, T* div, T* vort, cudaStream_t s,
-                         const T* wk = nullptr, T* ddt_w = nullptr);
+                         const T* wk = nullptr, T* ddt_w = nullptr, const CcMetric<T>* met = nullptr);
 // shape helpers of that kernel: level mapping (values a lane holds per column; 0 = nlev not supported), bytes of one w column
 // (the smallest possible slot), and how many slots of `slot_bytes` fit beside the fixed buffers in `smem_optin` bytes of shared memory
 int cc_levels_per_lane(int nlev);

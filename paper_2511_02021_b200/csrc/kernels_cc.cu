@@ -2,7 +2,8 @@
 // into the same pass on request, divergence and vorticity (S1, S2: dycore_step), sm_100a. Four modes (template
 // parameter MODE, cc_schedule.hpp): kCcTend = ddt_vn (dycore_velocity_tendencies), kCcStep = ddt_vn + div + vort
 // (dycore_step), kCcDivVort = div + vort alone from the 27 vn columns they need (dycore_div_vort), kCcStepW = kCcStep
-// plus the vertical-wind tendency ddt_w (dycore_step_w, reading P-19).
+// plus the vertical-wind tendency ddt_w (dycore_step_w, reading P-19), kCcTendM = ddt_vn in its metric form
+// (dycore_velocity_tendencies_metric, reading P-20).
 //
 // One warp finishes one self-contained patch (sc_tables.hpp: four sibling cells, six owned edges,
 // 36 vn + 7 w columns, no exchange between warps), lanes = levels. The vn / w columns do not come
@@ -273,12 +274,13 @@ __global__ void __launch_bounds__((kCcWarps + CcWarps<T, L>::producers) * 32, 1)
 k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, const T* __restrict__ vn,
           const T* __restrict__ w, T* __restrict__ ddt_vn, T* __restrict__ div, T* __restrict__ vort,
           unsigned long long* pace_counter, unsigned long long pace_per_launch, int pace_mask, int pace_last,
-          const T* __restrict__ wk, T* __restrict__ ddt_w) {
+          const T* __restrict__ wk, T* __restrict__ ddt_w, CcMetric<T> met) {
     extern __shared__ __align__(128) unsigned char smem[];
     using C = Col<T, L>;
     constexpr int W = kCcWarps, G = kCcGroup, D = kCcDepth;
     constexpr int PPW = cc_patches_per_warp(L), PPS = G * PPW;      // patches per warp, per step
-    constexpr bool FUSED = MODE != kCcTend, DVONLY = MODE == kCcDivVort, WTEND = MODE == kCcStepW;
+    constexpr bool METRIC = MODE == kCcTendM;
+    constexpr bool FUSED = MODE != kCcTend && !METRIC, DVONLY = MODE == kCcDivVort, WTEND = MODE == kCcStepW;
     constexpr int kCcProducers = CcWarps<T, L>::producers;
     constexpr int REC = cc_record_bytes<T>(MODE), COEF = cc_coef_words(MODE);
     constexpr int NGRP = W / G;
@@ -436,9 +438,9 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
         const int k = level_of<L>(lane, l);
         po[l] = k < nlev;
         below_missing[l] = k + 1 >= nlev;
-        cA[l] = !DVONLY && po[l] ? __ldg(abc + k) : (T)0;
-        cB[l] = !DVONLY && po[l] ? __ldg(abc + nlev + k) : (T)0;
-        cC[l] = !DVONLY && po[l] ? __ldg(abc + 2 * nlev + k) : (T)0;
+        cA[l] = !DVONLY && !METRIC && po[l] ? __ldg(abc + k) : (T)0;
+        cB[l] = !DVONLY && !METRIC && po[l] ? __ldg(abc + nlev + k) : (T)0;
+        cC[l] = !DVONLY && !METRIC && po[l] ? __ldg(abc + 2 * nlev + k) : (T)0;
     }
     // vertical-wind tendency (mode kCcStepW, P-19): weight of vn(k) in vn_ie(k), 1 / (z_half[k-1] - z_half[k+1]) (both 0
     // outside the interior half levels 1 .. nlev-1, so that ddt_w comes out 0 at the top and the surface) and the half
@@ -446,7 +448,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
     bool pow_[L], w_int[L];
     FORL {
         const int k = level_of<L>(lane, l);
-        pow_[l] = WTEND && k <= nlev;
+        pow_[l] = (WTEND || METRIC) && k <= nlev;
         w_int[l] = WTEND && k >= 1 && k <= nlev - 1;
     }
     const uint64_t cs = (uint64_t)ldk * sizeof(T), cs_wout = (uint64_t)ldk_w * sizeof(T);
@@ -526,6 +528,44 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
                         else if (po[2 * q]) __stcs(reinterpret_cast<T*>(col + st_pair + 32 * q * sizeof(T)), x.v[2 * q]);
                     }
                 }
+            };
+
+            // one column of a caller's field straight from global memory, in the lane's level mapping (metric columns of
+            // an owned edge: used by this patch only, so they bypass the column cache); levels that do not exist read as 0
+            auto GL = [&](const T* base, int32_t id, uint64_t stride, const bool (&valid)[L]) {
+                using P2 = typename Pair<T>::type;
+                const unsigned char* col = reinterpret_cast<const unsigned char*>(base) + (uint64_t)(uint32_t)id * stride;
+                C c;
+                FORL c.v[l] = (T)0;
+                constexpr int NP = L == 6 ? 3 : 1;
+#pragma unroll
+                for (int q = 0; q < NP; ++q) {
+                    const unsigned char* a = col + st_pair + 32 * q * sizeof(T);
+                    if (valid[2 * q + 1]) {
+                        const P2 pr = __ldcs(reinterpret_cast<const P2*>(a));
+                        c.v[2 * q] = pr.x; c.v[2 * q + 1] = pr.y;
+                    } else if (valid[2 * q]) {
+                        c.v[2 * q] = __ldcs(reinterpret_cast<const T*>(a));
+                    }
+                }
+                if constexpr (L == 3) {
+                    if (valid[2]) c.v[2] = __ldcs(reinterpret_cast<const T*>(col + st_single));
+                }
+                return c;
+            };
+            // (vn_ie(k) - vn_ie(k+1)) inv_ddqz with the per-edge weights of reading P-20 (wg on half levels, two-point
+            // extrapolation at both ends); neighbours that do not exist are never selected
+            auto VDM = [&](const C& x, const C& wg, const C& inv) {
+                const C up = level_up(x, lane), dn = level_down(x, lane), wgd = level_down(wg, lane);
+                C o;
+                FORL {
+                    const int k = level_of<L>(lane, l);
+                    const bool top = k == 0, bot = k == nlev - 1;
+                    const T vk = (top ? x.v[l] : up.v[l]) + wg.v[l] * (x.v[l] - (top ? dn.v[l] : up.v[l]));
+                    const T vk1 = x.v[l] + wgd.v[l] * (bot ? x.v[l] - up.v[l] : dn.v[l] - x.v[l]);
+                    o.v[l] = po[l] ? (vk - vk1) * inv.v[l] : (T)0;
+                }
+                return o;
             };
 
             // columns this patch shares with the steps s-1 .. s-D+1 were copied on THEIR barriers, and
@@ -761,9 +801,14 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
                 }
             }
             // ---- horizontal part H of the six owned edges (S5); frees the KE / vorticity columns ----
-            T ec[24];
-            ld_coef(cf + SCF_EDGE, ec);
+            // the 24 edge coefficients: in registers for the whole tail, except in the metric form, which has 24 more and
+            // reads each one where it is used (both arrays in registers spilled 220 bytes)
+            T ec[METRIC ? 4 : 24];
+            if constexpr (!METRIC) ld_coef(cf + SCF_EDGE, ec);
+            auto EC = [&](int i) { return METRIC ? cf[SCF_EDGE + i] : ec[METRIC ? 0 : i]; };
             C H[6];
+            C Wc[METRIC ? 6 : 1];               // metric form: contravariant correction vn dz/dn + vt dz/dt of the owned edges
+            if constexpr (!METRIC) {
 #pragma unroll
             for (int x = 0; x < 3; ++x) {       // interior: i0 (ab, ca), i1 (ab, bc), i2 (bc, ca); cells (T_x, T3)
                 const C& za = x == 2 ? zm[1] : zm[0];
@@ -776,6 +821,29 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
                 const T* e4 = ec + 4 * (3 + x);
                 FORL H[3 + x].v[l] = (keX[x].v[l] - ke[x].v[l]) * e4[0] + tBo[x].v[l] * (e4[1] + (zm[x].v[l] + zc[x].v[l]));
             }
+            } else {
+                // reading P-20: gradK = gH KE_c(H) - gL KE_c(L) + gE (vn^2 + vt^2) (second order at the edge midpoint), and
+                // w_cc while vt is still in registers; the slope columns come straight from global memory
+#pragma unroll
+                for (int x = 0; x < 6; ++x) {
+                    const C& v = x < 3 ? vI[x] : vB[2 * (x - 3)];
+                    const C& t = x < 3 ? tI[x] : tBo[x - 3];
+                    const C& kL = ke[x % 3];
+                    const C& kH = x < 3 ? ke[3] : keX[x - 3];
+                    const C& za = x < 3 ? (x == 2 ? zm[1] : zm[0]) : zm[x - 3];
+                    const C& zb = x < 3 ? (x == 1 ? zm[1] : zm[2]) : zc[x - 3];
+                    T e4[4];
+                    ld_coef(cf + SCF_EDGE + 4 * x, e4);
+                    T m4[4];                            // per edge: 24 more coefficients held across the loop spilled 650 bytes
+                    ld_coef(cf + SCF_CGRAD + 4 * x, m4);
+                    const C zn = GL(met.zn, ido[x], cs, po), zt = GL(met.zt, ido[x], cs, po);
+                    FORL {
+                        H[x].v[l] = m4[1] * kH.v[l] - m4[0] * kL.v[l] + m4[2] * (v.v[l] * v.v[l] + t.v[l] * t.v[l]) +
+                                    t.v[l] * (e4[1] + (za.v[l] + zb.v[l]));
+                        Wc[x].v[l] = v.v[l] * zn.v[l] + t.v[l] * zt.v[l];
+                    }
+                }
+            }
             // ---- cell-centre w at the six owned edges (S6): w_e = c_lin(L) w_f(L) + c_lin(H) w_f(H); these are the
             // last reads of the slots
             C we[6];
@@ -784,11 +852,11 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
 #pragma unroll
                 for (int j = 0; j < 4; ++j) wf[j] = WS(sX[12 + j]);
 #pragma unroll
-                for (int x = 0; x < 3; ++x) FORL we[x].v[l] = ec[4 * x + 2] * wf[x].v[l] + ec[4 * x + 3] * wf[3].v[l];
+                for (int x = 0; x < 3; ++x) FORL we[x].v[l] = EC(4 * x + 2) * wf[x].v[l] + EC(4 * x + 3) * wf[3].v[l];
 #pragma unroll
                 for (int x = 0; x < 3; ++x) {
                     const C wx = WS(sX[16 + x]);
-                    FORL we[3 + x].v[l] = ec[4 * (3 + x) + 2] * wf[x].v[l] + ec[4 * (3 + x) + 3] * wx.v[l];
+                    FORL we[3 + x].v[l] = EC(4 * (3 + x) + 2) * wf[x].v[l] + EC(4 * (3 + x) + 3) * wx.v[l];
                 }
             }
             // everything this patch needs from the slots and its record is in registers: release the stage
@@ -798,9 +866,16 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
             // ---- vertical part and the tendency (S6, S7) -----------------------------------------
 #pragma unroll
             for (int x = 0; x < 6; ++x) {
-                const C Dv = VD(x < 3 ? vI[x] : vB[2 * (x - 3)]);
+                const C& v = x < 3 ? vI[x] : vB[2 * (x - 3)];
                 C o;
-                FORL o.v[l] = -H[x].v[l] - we[x].v[l] * Dv.v[l];
+                if constexpr (METRIC) {
+                    const C wg = GL(met.wgt, ido[x], cs_wout, pow_), inv = GL(met.inv, ido[x], cs, po);
+                    const C Dv = VDM(v, wg, inv);
+                    FORL o.v[l] = -H[x].v[l] - (we[x].v[l] - Wc[x].v[l]) * Dv.v[l];
+                } else {
+                    const C Dv = VD(v);
+                    FORL o.v[l] = -H[x].v[l] - we[x].v[l] * Dv.v[l];
+                }
                 ST(ddt_vn, ido[x], o);
             }
             }   // !DVONLY
@@ -843,7 +918,7 @@ namespace {
 template <class T, int L, int MODE>
 cudaError_t cc_launch_one(const CcDev<T>& d, int device, int n_ctas, size_t smem, int nlev, int ldk, int ldk_w, const T* abc,
                           const T* vn, const T* w, T* ddt_vn, T* div, T* vort, unsigned long long* pc, unsigned long long ppl,
-                          int pm, int pl, const T* wk, T* ddt_w, cudaStream_t s) {
+                          int pm, int pl, const T* wk, T* ddt_w, const CcMetric<T>& met, cudaStream_t s) {
     auto k = k_tend_cc<T, L, MODE>;
     // the opt-in for > 48 KB of dynamic shared memory is a per-DEVICE attribute of the function: remembered per device
     static std::mutex mu;
@@ -857,14 +932,15 @@ cudaError_t cc_launch_one(const CcDev<T>& d, int device, int n_ctas, size_t smem
             if (known) configured[device] = smem;
         }
     }
-    k<<<(unsigned)n_ctas, (kCcWarps + CcWarps<T, L>::producers) * 32, smem, s>>>(d, nlev, ldk, ldk_w, abc, vn, w, ddt_vn, div, vort, pc, ppl, pm, pl, wk, ddt_w);
+    k<<<(unsigned)n_ctas, (kCcWarps + CcWarps<T, L>::producers) * 32, smem, s>>>(d, nlev, ldk, ldk_w, abc, vn, w, ddt_vn, div, vort, pc, ppl, pm, pl, wk, ddt_w, met);
     return cudaGetLastError();
 }
 }  // namespace
 
 template <class T>
 int launch_tendencies_cc(const icon_grid& g, DevCcTables<T>& p, int mode, int nlev, int64_t ldk, int64_t ldk_w,
-                         const T* abc, const T* vn, const T* w, T* ddt_vn, T* div, T* vort, cudaStream_t s, const T* wk, T* ddt_w) {
+                         const T* abc, const T* vn, const T* w, T* ddt_vn, T* div, T* vort, cudaStream_t s, const T* wk, T* ddt_w,
+                         const CcMetric<T>* met) {
     CcDev<T> d;
     d.steps = p.steps; d.loads = p.loads; d.records = p.records;
     d.cta_patch_begin = p.cta_patch_begin; d.cta_step_begin = p.cta_step_begin;
@@ -880,16 +956,18 @@ int launch_tendencies_cc(const icon_grid& g, DevCcTables<T>& p, int mode, int nl
     const int pace_last = n_barriers * period;
     const unsigned long long per_launch = (unsigned long long)n_barriers * (unsigned long long)p.n_ctas;
     // the tables must have been built for this mode (kCcTend runs on the tables of kCcStep: same columns, same records)
-    if ((mode == kCcTend ? (int)kCcStep : mode) != p.built_for || (mode == kCcDivVort) != (ddt_vn == nullptr) || (mode == kCcTend || mode == kCcDivVort ? false : div == nullptr) || (mode == kCcTend && div != nullptr) ||
-        (mode == kCcStepW) != (ddt_w != nullptr))
+    const bool wants_div = mode == kCcStep || mode == kCcStepW || mode == kCcDivVort;
+    if ((mode == kCcTend ? (int)kCcStep : mode) != p.built_for || (mode == kCcDivVort) != (ddt_vn == nullptr) || wants_div != (div != nullptr) ||
+        (mode == kCcStepW) != (ddt_w != nullptr) || (mode == kCcTendM) != (met != nullptr))
         return -(int)cudaErrorInvalidValue;
+    const CcMetric<T> metric = met ? *met : CcMetric<T>{nullptr, nullptr, nullptr, nullptr};
     const size_t smem = cc_fixed_smem<T>(mode, L) + (size_t)p.n_slots * p.slot_bytes + kCcSlotTailPad;
     cudaError_t err = cudaErrorInvalidValue;
 #define CC_ONE(LL, MM) \
     if (L == LL && mode == MM) \
-        err = cc_launch_one<T, LL, MM>(d, g.device, p.n_ctas, smem, nlev, (int)ldk, (int)ldk_w, abc, vn, w, ddt_vn, div, vort, p.progress, per_launch, pace_mask, pace_last, wk, ddt_w, s);
+        err = cc_launch_one<T, LL, MM>(d, g.device, p.n_ctas, smem, nlev, (int)ldk, (int)ldk_w, abc, vn, w, ddt_vn, div, vort, p.progress, per_launch, pace_mask, pace_last, wk, ddt_w, metric, s);
     CC_ONE(2, kCcTend) CC_ONE(2, kCcStep) CC_ONE(2, kCcDivVort) CC_ONE(3, kCcTend) CC_ONE(3, kCcStep)
-    CC_ONE(2, kCcStepW) CC_ONE(3, kCcStepW)
+    CC_ONE(2, kCcStepW) CC_ONE(3, kCcStepW) CC_ONE(2, kCcTendM) CC_ONE(3, kCcTendM)
     constexpr int LDV = sizeof(T) == 4 ? 6 : 3;          // deep columns in the div / vort mode
     CC_ONE(LDV, kCcDivVort)
 #undef CC_ONE
@@ -897,8 +975,8 @@ int launch_tendencies_cc(const icon_grid& g, DevCcTables<T>& p, int mode, int nl
 }
 
 template int launch_tendencies_cc<double>(const icon_grid&, DevCcTables<double>&, int, int, int64_t, int64_t,
-                                          const double*, const double*, const double*, double*, double*, double*, cudaStream_t, const double*, double*);
+                                          const double*, const double*, const double*, double*, double*, double*, cudaStream_t, const double*, double*, const CcMetric<double>*);
 template int launch_tendencies_cc<float>(const icon_grid&, DevCcTables<float>&, int, int, int64_t, int64_t,
-                                         const float*, const float*, const float*, float*, float*, float*, cudaStream_t, const float*, float*);
+                                         const float*, const float*, const float*, float*, float*, float*, cudaStream_t, const float*, float*, const CcMetric<float>*);
 
 }  // namespace icon

@@ -192,13 +192,18 @@ std::string build_sc_tables(const HostGrid& g, ScTables& t) {
             const int64_t e = own[x];
             const int32_t c0 = g.e2c[2 * e], c1 = g.e2c[2 * e + 1];
             double* o = cf + SCF_EDGE + 4 * x;
+            double* m = cf + SCF_CGRAD + 4 * x;     // P-20: cgrad(e,1) KE_c(c1) - cgrad(e,0) KE_c(c0) + KE_e (cgrad(e,0) - cgrad(e,1))
             if (c0 == lo[x] && c1 == hi[x]) {
                 o[0] = g.inv_d_e[e]; o[2] = g.c_lin[2 * e]; o[3] = g.c_lin[2 * e + 1];
+                m[0] = g.cgrad[2 * e]; m[1] = g.cgrad[2 * e + 1];
             } else if (c0 == hi[x] && c1 == lo[x]) {
                 o[0] = -g.inv_d_e[e]; o[2] = g.c_lin[2 * e + 1]; o[3] = g.c_lin[2 * e];
+                m[0] = -g.cgrad[2 * e + 1]; m[1] = -g.cgrad[2 * e];
             } else {
                 ok = false;
             }
+            m[2] = 0.5 * (m[0] - m[1]);
+            m[3] = 0.0;
             o[1] = g.f_e[e];
         }
         // the outer ring of the three owned boundary edges

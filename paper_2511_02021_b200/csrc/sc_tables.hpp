@@ -30,7 +30,7 @@
 namespace icon {
 
 constexpr int kScIdWords = 56;      // int32 per patch: 36 edges, 10 cells, 2 pad, 6 vertices, 2 pad (224 B)
-constexpr int kScCoefWords = 172;   // floating-point words per patch; every group starts on a multiple of 4 words
+constexpr int kScCoefWords = 196;   // floating-point words per patch; every group starts on a multiple of 4 words
 
 enum {                // id slots
     SID_I0 = 0,       // i0 i1 i2
@@ -55,8 +55,10 @@ enum {                // coefficient slots
     SCF_XROT = 128,   // [3][6] rot of C_x over (b_j, oc_j, n1, n2, oc_jp, b_jp) (x 1/2)
     SCF_USED = 146,
     SCF_DIV = 148,    // [4][3] geofac_div of T0..T3 over the cell edges in the order of SCF_BLN
-    SCF_ADV = 160     // [4][3] +-adv_c * inv_d_e of T0..T3 over the same edges (P-19); sign such that the term is
+    SCF_ADV = 160,    // [4][3] +-adv_c * inv_d_e of T0..T3 over the same edges (P-19); sign such that the term is
                       //        coefficient * vn_ie * (w(cell across the edge) - w(this cell))
+    SCF_CGRAD = 172   // [6][4] owned i0 i1 i2 b0 b2 b4 (P-20): gL, gH, gE, pad with
+                      //        gradK = gH KE_c(H) - gL KE_c(L) + gE (vn^2 + vt^2), gE = (gL - gH) / 2
 };
 
 struct ScTables {

@@ -111,3 +111,42 @@ def sample_points(seed, n_entities, nlev, n):
     idx[:4] = [0, 0, n_entities - 1, n_entities - 1]
     lev[:4] = [0, nlev - 1, 0, nlev - 1]
     return idx, lev
+
+
+def make_metric_heights(config, edge_xyz, edge_normal, nlev, ldk, ldk_w, dtype="f64", h_top=H_TOP, pad_value=np.nan):
+    """Seeded synthetic terrain-following level heights for the metric variant (reading P-20 of DESIGN.md): inputs only.
+
+    Terrain h(x) = a few seeded Gaussian mountains (up to ~3 km) on the unit sphere; hybrid levels
+    z_half_e(e,k) = z_flat(k) + h(x_e) * (1 - z_flat(k) / h_top)  (terrain following at the ground, flat at the top);
+    slopes of the full-level surfaces at the edge midpoint along n_e and along n_e x x_e. Stand-in for the model's own
+    orography and SLEVE levels, which are not available. Returns z_half_e [ne][ldk_w], ddxn_z, ddxt_z [ne][ldk].
+    """
+    rng = np.random.Generator(np.random.PCG64(3000 + config))
+    n_mtn = 6
+    centres = rng.standard_normal((n_mtn, 3))
+    centres /= np.linalg.norm(centres, axis=1)[:, None]
+    heights = 1000.0 + 2000.0 * rng.random(n_mtn)
+    widths = 0.15 + 0.25 * rng.random(n_mtn)                 # radians
+    ne = edge_xyz.shape[0]
+    h = np.zeros(ne)
+    grad = np.zeros((ne, 3))                                 # tangential gradient on the sphere of radius 6.371e6 m
+    for c, hh, wd in zip(centres, heights, widths):
+        d2 = ((edge_xyz - c[None, :]) ** 2).sum(1)           # squared chord distance
+        gm = hh * np.exp(-d2 / wd ** 2)
+        h += gm
+        g3 = gm[:, None] * (-2.0 / wd ** 2) * (edge_xyz - c[None, :])
+        g3 -= (g3 * edge_xyz).sum(1)[:, None] * edge_xyz
+        grad += g3 / 6.371e6
+    zflat = z_half_levels(nlev, h_top)
+    zf = 0.5 * (zflat[:-1] + zflat[1:])
+    tang = np.cross(edge_normal, edge_xyz)
+    zh = np.full((ne, ldk_w), pad_value)
+    zh[:, :nlev + 1] = zflat[None, :] + h[:, None] * (1.0 - zflat[None, :] / h_top)
+    zn = np.full((ne, ldk), pad_value)
+    zt = np.full((ne, ldk), pad_value)
+    decay = (1.0 - zf / h_top)[None, :]
+    zn[:, :nlev] = (grad * edge_normal).sum(1)[:, None] * decay
+    zt[:, :nlev] = (grad * tang).sum(1)[:, None] * decay
+    if dtype == "f32":
+        zh, zn, zt = zh.astype(np.float32), zn.astype(np.float32), zt.astype(np.float32)
+    return zh, zn, zt

@@ -435,6 +435,63 @@ def test_dycore_step_w_all_four_outputs(torch_cuda, lib, oracle_grid, k, seed, f
         assert (got[:, 0] == 0).all() and (got[:, nlev] == 0).all() and (got[:, nlev + 1:] == sentinel).all()
 
 
+# ----------------------------------------------------------------------------------------------
+# metric variant (reading P-20)
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", [5, 0])
+@pytest.mark.parametrize("k,seed,flags,nlev,ldk,ldk_w,dtype", [
+    (4, 0, 0, 90, 96, 96, "f64"), (4, 0, 0, 90, 90, 92, "f64"), (3, si.PERMUTE_SEED, 1, 40, 40, 42, "f64"),
+    (4, si.PERMUTE_SEED, 1, 90, 96, 96, "f32"), (2, 0, 0, 30, 32, 32, "f64"), (1, 0, 0, 31, 32, 32, "f64"), (2, 0, 0, 33, 34, 34, "f64"),
+    (2, 0, 0, 64, 64, 66, "f64"), (2, 0, 0, 65, 66, 66, "f64"), (2, 0, 0, 95, 96, 96, "f64"), (0, 0, 0, 3, 4, 4, "f64"),
+    (2, 0, 0, 130, 130, 132, "f64"), (3, 0, 0, 30, 32, 32, "f32")])
+def test_metric_variant_elementwise(torch_cuda, lib, oracle_mod, oracle_grid, variant, k, seed, flags, nlev, ldk, ldk_w, dtype):
+    """dycore_metric_from_zhalf and dycore_velocity_tendencies_metric against the oracle on a seeded terrain-following grid:
+    the fused column-cache mode (variant 5 = auto; nlev = 130 falls back) and the unfused pipeline (variant 0); two launches
+    on different inputs; every level written once, pads untouched"""
+    torch = torch_cuda
+    og = oracle_grid(k, seed, flags & 1)
+    g = lib_grid(lib, k, seed, flags)
+    f32 = dtype == "f32"
+    dev = torch.device("cuda:0")
+    o = og.rounded_f32() if f32 else og
+    zh_e, zn, zt = si.make_metric_heights(1, og.edge_xyz, og.edge_normal, nlev, ldk, ldk_w, dtype=dtype)
+    tdt = torch.float32 if f32 else torch.float64
+    d_zh = torch.from_numpy(zh_e).to(dev)
+    sentinel = -6.75
+    d_wgt = torch.full((g.ne, ldk_w), sentinel, dtype=tdt, device=dev)
+    d_inv = torch.full((g.ne, ldk), sentinel, dtype=tdt, device=dev)
+    lib.dycore_metric_from_zhalf(g, d_zh, d_wgt, d_inv, nlev)
+    torch.cuda.synchronize()
+    wgt_o, inv_o = oracle_mod.metric_from_zhalf(np.nan_to_num(zh_e.astype(np.float64)), nlev, ldk)
+    rel = 1e-5 if f32 else 1e-12          # the thicknesses of fp32 heights of 30 km carry ~1e-4 relative rounding themselves:
+    wgt_g, inv_g = d_wgt.cpu().numpy().astype(np.float64), d_inv.cpu().numpy().astype(np.float64)
+    if not f32:                           # compared in fp64 only; fp32 goes on with the device's own metrics below
+        assert np.abs(wgt_g[:, :nlev + 1] - wgt_o[:, :nlev + 1]).max() <= rel
+        assert np.abs(inv_g[:, :nlev] / inv_o[:, :nlev] - 1).max() <= rel
+    assert (wgt_g[:, nlev + 1:] == sentinel).all() and (inv_g[:, nlev:] == sentinel).all()
+    # the operator is compared on the metrics the DEVICE derived (inputs of the operator; fp32: rounded to fp32 there)
+    wgt_in, inv_in = np.nan_to_num(np.where(wgt_g == sentinel, 0, wgt_g)), np.nan_to_num(np.where(inv_g == sentinel, 0, inv_g))
+    zn64, zt64 = np.nan_to_num(zn.astype(np.float64)), np.nan_to_num(zt.astype(np.float64))
+    d_zn, d_zt = torch.from_numpy(zn).to(dev), torch.from_numpy(zt).to(dev)
+    g.set_option(lib.ICON_OPT_TENDENCY_KERNEL, variant)
+    try:
+        for cfg, fv in ((1, 1.0), (2, -2.5)):
+            vn, w, _ = si.make_fields(cfg, og.edge_xyz, og.edge_normal, og.nc, nlev=nlev, ldk=ldk, ldk_w=ldk_w, dtype=dtype)
+            vn = (vn * fv).astype(vn.dtype)
+            vn64, w64 = np.nan_to_num(vn.astype(np.float64)), np.nan_to_num(w.astype(np.float64))
+            ref = o.velocity_tendencies_metric(vn64, w64, wgt_in, inv_in, zn64, zt64, nlev, with_scale=True)
+            out = torch.full((g.ne, ldk), sentinel, dtype=tdt, device=dev)
+            n0 = g.launch_count
+            lib.dycore_velocity_tendencies_metric(g, d_wgt, d_inv, d_zn, d_zt, torch.from_numpy(vn).to(dev), torch.from_numpy(w).to(dev), out, nlev)
+            torch.cuda.synchronize()
+            assert g.launch_count - n0 == (1 if (variant == 5 and nlev + 1 <= 96) else 3)
+            got = out.cpu().numpy().astype(np.float64)
+            assert_close("ddt_vn (metric)", got, ref["ddt_vn"], ref["m_ddt"], TOL[dtype], nlev)
+            assert (got[:, nlev:] == sentinel).all() and not (got[:, :nlev] == sentinel).any()
+    finally:
+        g.set_option(lib.ICON_OPT_TENDENCY_KERNEL, 5)
+
+
 def test_argument_errors_on_device(torch_cuda, lib):
     torch = torch_cuda
     g = lib_grid(lib, 1)
