@@ -74,6 +74,8 @@ def _load():
     L.og_metric_from_zhalf.argtypes = [i64, ctypes.c_int, i64, i64, P, P, P]
     L.og_velocity_tendencies_metric.restype = ctypes.c_int
     L.og_velocity_tendencies_metric.argtypes = [P, ctypes.c_int, i64, i64, P, P, P, P, P, P, P, P, P, P, P]
+    L.og_sample_ddt_vn_metric.restype = None
+    L.og_sample_ddt_vn_metric.argtypes = [P, ctypes.c_int, i64, i64, P, P, P, P, P, P, i64, P, P, P, P]
     L.og_divergence.restype = None
     L.og_divergence.argtypes = [i64, ctypes.c_int, i64, P, P, P, P, P]
     L.og_vorticity.restype = None
@@ -220,6 +222,18 @@ class Grid:
         if with_scale:
             out["m_ddt"] = m
         return out
+
+    def sample_metric(self, idx, lev, vn, w, wgt_e, inv_ddqz_e, ddxn_z, ddxt_z, nlev):
+        """ddt_vn of the metric variant (P-20) at the points (edge idx[i], level lev[i]); the metric arrays are used as they
+        are (any dtype-compatible contiguous float64 arrays of the fields' shapes). Returns (values, M)."""
+        vn, w = _f64(vn), _f64(w)
+        wgt_e, inv_ddqz_e, ddxn_z, ddxt_z = _f64(wgt_e), _f64(inv_ddqz_e), _f64(ddxn_z), _f64(ddxt_z)
+        idx = np.ascontiguousarray(idx, dtype=np.int64)
+        lev = np.ascontiguousarray(lev, dtype=np.int32)
+        out, m = np.zeros(idx.size), np.zeros(idx.size)
+        self._L.og_sample_ddt_vn_metric(self._h, nlev, vn.shape[1], w.shape[1], _ptr(wgt_e), _ptr(inv_ddqz_e), _ptr(ddxn_z),
+                                        _ptr(ddxt_z), _ptr(vn), _ptr(w), idx.size, _ptr(idx), _ptr(lev), _ptr(out), _ptr(m))
+        return out, m
 
     # ---- sampled one-by-one evaluation (full-size parity) ----
     def sample(self, what, idx, lev, vn, nlev, w=None, z_half=None):

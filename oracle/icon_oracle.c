@@ -1101,6 +1101,36 @@ void og_sample_ddt_vn(const og_grid *g, int nlev, int64_t ldk, int64_t ldk_w, co
     }
 }
 
+/* metric variant (P-20), one point at a time: the definitions of og_ddt_vn_metric without any full-array intermediate */
+void og_sample_ddt_vn_metric(const og_grid *g, int nlev, int64_t ldk, int64_t ldk_w, const double *wgt_e,
+                             const double *inv_ddqz_e, const double *ddxn_z, const double *ddxt_z, const double *vn,
+                             const double *w, int64_t n, const int64_t *idx, const int32_t *lev, double *out, double *m_out)
+{
+    for (int64_t i = 0; i < n; ++i) {
+        int64_t e = idx[i]; int k = lev[i];
+        int64_t c0 = g->e2c[2 * e], c1 = g->e2c[2 * e + 1], v0 = g->e2v[2 * e], v1 = g->e2v[2 * e + 1];
+        double kc0 = og_pt_ke_c(g, ldk, vn, c0, k), kc1 = og_pt_ke_c(g, ldk, vn, c1, k);
+        double z0 = og_pt_vort(g, ldk, vn, v0, k, NULL), z1 = og_pt_vort(g, ldk, vn, v1, k, NULL);
+        double vt = og_pt_vt(g, ldk, vn, e, k);
+        double vne = vn[e * ldk + k];
+        double ke_e = 0.5 * (vne * vne + vt * vt);
+        double g0 = g->cgrad[2 * e], g1 = g->cgrad[2 * e + 1];
+        double gradk = g1 * kc1 - g0 * kc0 + ke_e * (g0 - g1);
+        double H = gradk + vt * (g->f_e[e] + 0.5 * (z0 + z1));
+        double wf0 = 0.5 * (w[c0 * ldk_w + k] + w[c0 * ldk_w + k + 1]);
+        double wf1 = 0.5 * (w[c1 * ldk_w + k] + w[c1 * ldk_w + k + 1]);
+        double w_e = g->c_lin[2 * e] * wf0 + g->c_lin[2 * e + 1] * wf1;
+        int64_t j = e * ldk + k;
+        double w_cc = vne * ddxn_z[j] + vt * ddxt_z[j];
+        const double *col = vn + e * ldk, *wg = wgt_e + e * ldk_w;
+        double up = og_vn_half_metric(col, nlev, wg, k), dn = og_vn_half_metric(col, nlev, wg, k + 1);
+        out[i] = -(H + (w_e - w_cc) * (up - dn) * inv_ddqz_e[j]);
+        m_out[i] = g1 * fabs(kc1) + g0 * fabs(kc0) + fabs(ke_e) * fabs(g0 - g1)
+            + fabs(vt) * (fabs(g->f_e[e]) + 0.5 * (fabs(z0) + fabs(z1)))
+            + (fabs(w_e) + fabs(vne * ddxn_z[j]) + fabs(vt * ddxt_z[j])) * (fabs(up) + fabs(dn)) * inv_ddqz_e[j];
+    }
+}
+
 /* accessors for the Python wrapper (struct layout stays private to C) */
 int64_t og_grid_nc(const og_grid *g) { return g->nc; }
 int64_t og_grid_ne(const og_grid *g) { return g->ne; }

@@ -591,6 +591,19 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
                 const int4 a = reinterpret_cast<const int4*>(oid)[i];
                 ido[4 * i] = a.x; ido[4 * i + 1] = a.y; ido[4 * i + 2] = a.z; ido[4 * i + 3] = a.w;
             }
+            if constexpr (METRIC) {
+                // Request the 24 metric columns of this patch (4 fields x 6 owned edges, 6 lines of 128 bytes each for 90 fp64
+                // levels) into the L2 now: they are needed ~2 us from now, straight from global memory, and a DRAM round trip
+                // per batch was what bounded this mode (12.8 ms at config 3 before). One line per lane and request.
+                for (int i = hl; i < 24 * 8; i += 32 / PPW) {          // two patches per warp: every half-warp covers its own patch
+                    const int colm = i >> 3, line = i & 7, field = colm / 6, edge = colm - 6 * field;
+                    const unsigned char* base = reinterpret_cast<const unsigned char*>(field == 0 ? met.wgt : field == 1 ? met.inv : field == 2 ? met.zn : met.zt);
+                    const uint64_t first = (uint64_t)(uint32_t)oid[edge] * (field == 0 ? cs_wout : cs);
+                    const uint64_t last = first + (uint64_t)(nlev + (field == 0 ? 1 : 0)) * sizeof(T) - 1;
+                    const uint64_t at = (first & ~(uint64_t)127) + ((uint64_t)line << 7);       // only lines that hold bytes of the column
+                    if (at <= last && live) asm volatile("prefetch.global.L2 [%0];" ::"l"(base + at));
+                }
+            }
             if constexpr (FUSED) {
                 // ---- S1: div of the four cells from their edges (slot order of SCF_BLN) ------------
                 T gd[12];
@@ -801,14 +814,62 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
                 }
             }
             // ---- horizontal part H of the six owned edges (S5); frees the KE / vorticity columns ----
-            // the 24 edge coefficients: in registers for the whole tail, except in the metric form, which has 24 more and
-            // reads each one where it is used (both arrays in registers spilled 220 bytes)
-            T ec[METRIC ? 4 : 24];
-            if constexpr (!METRIC) ld_coef(cf + SCF_EDGE, ec);
-            auto EC = [&](int i) { return METRIC ? cf[SCF_EDGE + i] : ec[METRIC ? 0 : i]; };
+            if constexpr (METRIC) {
+                // ---- metric form (reading P-20). One loop over the owned edges fetches the four metric columns of an edge in
+                // ONE batch, straight from global memory (requested into the L2 when the patch started, see above): six
+                // dependent round trips per patch instead of twelve. It leaves two columns per edge, A = -H + w_cc Dv and
+                // Dv, and frees the KE / vorticity / vt columns; w at the edges follows as in the plain form.
+                C A[6], Dq[6];
+#pragma unroll
+                for (int x = 0; x < 6; ++x) {
+                    const C& v = x < 3 ? vI[x] : vB[2 * (x - 3)];
+                    const C& t = x < 3 ? tI[x] : tBo[x - 3];
+                    const C& kL = ke[x % 3];
+                    const C& kH = x < 3 ? ke[3] : keX[x - 3];
+                    const C& za = x < 3 ? (x == 2 ? zm[1] : zm[0]) : zm[x - 3];
+                    const C& zb = x < 3 ? (x == 1 ? zm[1] : zm[2]) : zc[x - 3];      // i0: (ab, ca), i1: (ab, bc), i2: (bc, ca)
+                    const C zn = GL(met.zn, ido[x], cs, po), zt = GL(met.zt, ido[x], cs, po);
+                    const C wg = GL(met.wgt, ido[x], cs_wout, pow_), inv = GL(met.inv, ido[x], cs, po);
+                    T e4[4], m4[4];                     // f_e | gL, gH, gE: read where they are used (both groups in registers spilled)
+                    ld_coef(cf + SCF_EDGE + 4 * x, e4);
+                    ld_coef(cf + SCF_CGRAD + 4 * x, m4);
+                    const C Dv = VDM(v, wg, inv);
+                    FORL {
+                        // gradK = gH KE_c(H) - gL KE_c(L) + gE (vn^2 + vt^2): second order at the edge midpoint
+                        const T Hh = m4[1] * kH.v[l] - m4[0] * kL.v[l] + m4[2] * (v.v[l] * v.v[l] + t.v[l] * t.v[l]) +
+                                     t.v[l] * (e4[1] + (za.v[l] + zb.v[l]));
+                        const T wcc = v.v[l] * zn.v[l] + t.v[l] * zt.v[l];      // contravariant correction
+                        A[x].v[l] = wcc * Dv.v[l] - Hh;
+                        Dq[x].v[l] = Dv.v[l];
+                    }
+                }
+                C we[6];
+                {
+                    C wf[4];
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) wf[j] = WS(sX[12 + j]);
+#pragma unroll
+                    for (int x = 0; x < 3; ++x)
+                        FORL we[x].v[l] = cf[SCF_EDGE + 4 * x + 2] * wf[x].v[l] + cf[SCF_EDGE + 4 * x + 3] * wf[3].v[l];
+#pragma unroll
+                    for (int x = 0; x < 3; ++x) {
+                        const C wx = WS(sX[16 + x]);
+                        FORL we[3 + x].v[l] = cf[SCF_EDGE + 4 * (3 + x) + 2] * wf[x].v[l] + cf[SCF_EDGE + 4 * (3 + x) + 3] * wx.v[l];
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(done_bar(s % NB));
+#pragma unroll
+                for (int x = 0; x < 6; ++x) {
+                    C o;
+                    FORL o.v[l] = A[x].v[l] - we[x].v[l] * Dq[x].v[l];
+                    ST(ddt_vn, ido[x], o);
+                }
+            } else {
+            // ---- horizontal part H of the six owned edges (S5); frees the KE / vorticity columns ----
+            T ec[24];
+            ld_coef(cf + SCF_EDGE, ec);
             C H[6];
-            C Wc[METRIC ? 6 : 1];               // metric form: contravariant correction vn dz/dn + vt dz/dt of the owned edges
-            if constexpr (!METRIC) {
 #pragma unroll
             for (int x = 0; x < 3; ++x) {       // interior: i0 (ab, ca), i1 (ab, bc), i2 (bc, ca); cells (T_x, T3)
                 const C& za = x == 2 ? zm[1] : zm[0];
@@ -821,29 +882,6 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
                 const T* e4 = ec + 4 * (3 + x);
                 FORL H[3 + x].v[l] = (keX[x].v[l] - ke[x].v[l]) * e4[0] + tBo[x].v[l] * (e4[1] + (zm[x].v[l] + zc[x].v[l]));
             }
-            } else {
-                // reading P-20: gradK = gH KE_c(H) - gL KE_c(L) + gE (vn^2 + vt^2) (second order at the edge midpoint), and
-                // w_cc while vt is still in registers; the slope columns come straight from global memory
-#pragma unroll
-                for (int x = 0; x < 6; ++x) {
-                    const C& v = x < 3 ? vI[x] : vB[2 * (x - 3)];
-                    const C& t = x < 3 ? tI[x] : tBo[x - 3];
-                    const C& kL = ke[x % 3];
-                    const C& kH = x < 3 ? ke[3] : keX[x - 3];
-                    const C& za = x < 3 ? (x == 2 ? zm[1] : zm[0]) : zm[x - 3];
-                    const C& zb = x < 3 ? (x == 1 ? zm[1] : zm[2]) : zc[x - 3];
-                    T e4[4];
-                    ld_coef(cf + SCF_EDGE + 4 * x, e4);
-                    T m4[4];                            // per edge: 24 more coefficients held across the loop spilled 650 bytes
-                    ld_coef(cf + SCF_CGRAD + 4 * x, m4);
-                    const C zn = GL(met.zn, ido[x], cs, po), zt = GL(met.zt, ido[x], cs, po);
-                    FORL {
-                        H[x].v[l] = m4[1] * kH.v[l] - m4[0] * kL.v[l] + m4[2] * (v.v[l] * v.v[l] + t.v[l] * t.v[l]) +
-                                    t.v[l] * (e4[1] + (za.v[l] + zb.v[l]));
-                        Wc[x].v[l] = v.v[l] * zn.v[l] + t.v[l] * zt.v[l];
-                    }
-                }
-            }
             // ---- cell-centre w at the six owned edges (S6): w_e = c_lin(L) w_f(L) + c_lin(H) w_f(H); these are the
             // last reads of the slots
             C we[6];
@@ -852,11 +890,11 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
 #pragma unroll
                 for (int j = 0; j < 4; ++j) wf[j] = WS(sX[12 + j]);
 #pragma unroll
-                for (int x = 0; x < 3; ++x) FORL we[x].v[l] = EC(4 * x + 2) * wf[x].v[l] + EC(4 * x + 3) * wf[3].v[l];
+                for (int x = 0; x < 3; ++x) FORL we[x].v[l] = ec[4 * x + 2] * wf[x].v[l] + ec[4 * x + 3] * wf[3].v[l];
 #pragma unroll
                 for (int x = 0; x < 3; ++x) {
                     const C wx = WS(sX[16 + x]);
-                    FORL we[3 + x].v[l] = EC(4 * (3 + x) + 2) * wf[x].v[l] + EC(4 * (3 + x) + 3) * wx.v[l];
+                    FORL we[3 + x].v[l] = ec[4 * (3 + x) + 2] * wf[x].v[l] + ec[4 * (3 + x) + 3] * wx.v[l];
                 }
             }
             // everything this patch needs from the slots and its record is in registers: release the stage
@@ -866,18 +904,12 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
             // ---- vertical part and the tendency (S6, S7) -----------------------------------------
 #pragma unroll
             for (int x = 0; x < 6; ++x) {
-                const C& v = x < 3 ? vI[x] : vB[2 * (x - 3)];
+                const C Dv = VD(x < 3 ? vI[x] : vB[2 * (x - 3)]);
                 C o;
-                if constexpr (METRIC) {
-                    const C wg = GL(met.wgt, ido[x], cs_wout, pow_), inv = GL(met.inv, ido[x], cs, po);
-                    const C Dv = VDM(v, wg, inv);
-                    FORL o.v[l] = -H[x].v[l] - (we[x].v[l] - Wc[x].v[l]) * Dv.v[l];
-                } else {
-                    const C Dv = VD(v);
-                    FORL o.v[l] = -H[x].v[l] - we[x].v[l] * Dv.v[l];
-                }
+                FORL o.v[l] = -H[x].v[l] - we[x].v[l] * Dv.v[l];
                 ST(ddt_vn, ido[x], o);
             }
+            }   // !METRIC
             }   // !DVONLY
         } else {
             __syncwarp();

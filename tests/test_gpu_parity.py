@@ -672,4 +672,30 @@ def test_full_size_sampled(torch_cuda, lib, oracle_mod, config, host_gb):
     got2 = ddt_w2[torch.from_numpy(idx).to(dev), torch.from_numpy(lev.astype(np.int64)).to(dev)].cpu().numpy().astype(np.float64)
     assert (np.abs(got2 - want) <= tol * m).all(), "fused ddt_w config %d" % config
     assert not torch.isnan(ddt_w2[:, :nlev + 1]).any()
+    del outs, ddt_w, ddt_w2
+    torch.cuda.empty_cache()
+    # ---- leg D: the metric variant on the same fields, seeded terrain-following levels ----------
+    zh_e, zn, zt = si.make_metric_heights(config, og.edge_xyz, og.edge_normal, nlev, ldk, ldk_w, dtype=cfg["dtype"])
+    d_zh = torch.from_numpy(zh_e).to(dev)
+    del zh_e
+    d_wgt = torch.full((g.ne, ldk_w), float("nan"), dtype=d_vn.dtype, device=dev)
+    d_inv = torch.full((g.ne, ldk), float("nan"), dtype=d_vn.dtype, device=dev)
+    lib.dycore_metric_from_zhalf(g, d_zh, d_wgt, d_inv, nlev)
+    del d_zh
+    d_zn, d_zt = torch.from_numpy(zn).to(dev), torch.from_numpy(zt).to(dev)
+    out = torch.full((g.ne, ldk), float("nan"), dtype=d_vn.dtype, device=dev)
+    n0 = g.launch_count
+    lib.dycore_velocity_tendencies_metric(g, d_wgt, d_inv, d_zn, d_zt, d_vn, d_w, out, nlev)
+    torch.cuda.synchronize()
+    assert g.launch_count - n0 == 1
+    idx, lev = si.sample_points(600 + config, g.ne, nlev, nsamp)
+    got = out[torch.from_numpy(idx).to(dev), torch.from_numpy(lev.astype(np.int64)).to(dev)].cpu().numpy().astype(np.float64)
+    # the oracle evaluates on the metrics the device derived (inputs of the operator), pads read as 0
+    wgt_h, inv_h = as64(d_wgt.cpu().numpy()), as64(d_inv.cpu().numpy())
+    want, m = o.sample_metric(idx, lev, as64(vn), as64(w), wgt_h, inv_h, as64(zn), as64(zt), nlev)
+    err = np.abs(got - want)
+    assert (err <= tol * m).all(), "metric ddt_vn config %d: worst err/M %.3e" % (config, (err / np.maximum(m, 1e-300)).max())
+    assert not torch.isnan(out[:, :nlev]).any()
+    if ldk > nlev:
+        assert torch.isnan(out[:, nlev:]).all()
     g.close()

@@ -698,6 +698,23 @@ def test_metric_variant_on_flat_levels_differs_only_by_the_weighted_gradient(ora
     assert (om["m_ddt"] <= 1.000001 * m).all() and (om["m_ddt"] >= 0.999999 * m).all()
 
 
+def test_metric_sampled_evaluation_matches_full_arrays(oracle_mod, oracle_grid):
+    g = oracle_grid(3, 7, 1)
+    K = 9
+    rng = np.random.default_rng(41)
+    vn = rng.standard_normal((g.ne, K + 1)) * 6          # ldk > nlev
+    w = rng.standard_normal((g.nc, K + 3))
+    zh_e, zn, zt = si.make_metric_heights(1, g.edge_xyz, g.edge_normal, K, K + 1, K + 3, pad_value=0.0)
+    zn, zt = zn * 50, zt * 50                            # slopes of a few per cent
+    wgt, inv = oracle_mod.metric_from_zhalf(zh_e, K, K + 1)
+    wgt, inv = np.nan_to_num(wgt), np.nan_to_num(inv)
+    full = g.velocity_tendencies_metric(vn, w, wgt, inv, zn, zt, K, with_scale=True)
+    idx, lev = si.sample_points(2, g.ne, K, 600)
+    val, ms = g.sample_metric(idx, lev, vn, w, wgt, inv, zn, zt, K)
+    assert (np.abs(val - full["ddt_vn"][idx, lev]) <= 1e-14 * full["m_ddt"][idx, lev]).all()
+    assert np.abs(ms - full["m_ddt"][idx, lev]).max() <= 1e-14 * np.abs(full["m_ddt"]).max()
+
+
 def test_contravariant_correction_closed_form(oracle_mod, oracle_grid):
     """On coordinate surfaces z(x, k) the horizontal operators see (d/dn)|_s = (d/dn)|_z + z_n d/dz; collecting the metric
     terms of dK/dn and vt zeta gives exactly -(vn z_n + vt z_t) dvn/dz (P-20), i.e. vertical advection with the
