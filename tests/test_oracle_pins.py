@@ -827,3 +827,103 @@ def test_fp32_rounded_grid(oracle_grid):
     assert (r.c2e == g.c2e).all()
     for name in ("rbf", "bln", "geofac_div", "geofac_rot", "inv_d_e", "f_e", "c_lin"):
         assert (r.table(name) == g.table(name).astype(np.float32).astype(np.float64)).all()
+
+
+# ----------------------------------------------------------------------------------------------
+# domain decomposition (reading P-21): oracle/decomposition.py
+# ----------------------------------------------------------------------------------------------
+def _random_fields(g, nlev, seed):
+    rng = np.random.default_rng(seed)
+    vn = rng.normal(0.0, 10.0, (g.ne, nlev))
+    w = rng.normal(0.0, 0.5, (g.nc, nlev + 1))
+    return vn, w, si.z_half_levels(nlev)
+
+
+def test_decomposition_read_sets_against_brute_force_perturbation(oracle_grid):
+    """every vn column (then every w column) of R2B1 is perturbed in turn; the outputs of the oracle's operators that
+    change are exactly the ones whose read set, written out from S1-S7, holds that column. A forgotten neighbour, a
+    pentagon pad counted as a read, or e2c / e2v swapped fails here."""
+    from oracle import decomposition as dd
+    g = oracle_grid(1)
+    nlev = 4
+    vn, w, zh = _random_fields(g, nlev, 11)
+    base = g.velocity_tendencies(vn, w, zh, nlev)["ddt_vn"][:, :nlev].copy()
+    div0, vort0 = (a[:, :nlev].copy() for a in g.div_vort(vn, nlev))
+    reads = [dd.ddt_vn_reads(g, e) for e in range(g.ne)]
+    for col in range(g.ne):
+        p = vn.copy()
+        p[col] *= 1.5
+        p[col] += 3.0
+        got = set(np.nonzero(np.any(g.velocity_tendencies(p, w, zh, nlev)["ddt_vn"][:, :nlev] != base, axis=1))[0].tolist())
+        want = {e for e in range(g.ne) if col in reads[e][0]}
+        assert got == want, col
+        div1, vort1 = g.div_vort(p, nlev)
+        got_c = set(np.nonzero(np.any(div1[:, :nlev] != div0, axis=1))[0].tolist())
+        got_v = set(np.nonzero(np.any(vort1[:, :nlev] != vort0, axis=1))[0].tolist())
+        assert got_c == {c for c in range(g.nc) if col in dd.div_reads(g, c)}, col
+        assert got_v == {v for v in range(g.nv) if col in dd.vort_reads(g, v)}, col
+    for col in range(g.nc):
+        p = w.copy()
+        p[col] += 0.7
+        got = set(np.nonzero(np.any(g.velocity_tendencies(vn, p, zh, nlev)["ddt_vn"][:, :nlev] != base, axis=1))[0].tolist())
+        assert got == {e for e in range(g.ne) if col in reads[e][1]}, col
+
+
+@pytest.mark.parametrize("k", [1, 3])
+def test_decomposition_stencil_size(oracle_grid, k):
+    """"the ddt_vn stencil spans 15 distinct edges" -- away from the pentagons; next to a pentagon the
+    fan of one end vertex has one edge fewer"""
+    from oracle import decomposition as dd
+    g = oracle_grid(k)
+    n = np.array([len(dd.ddt_vn_reads(g, e)[0]) for e in range(g.ne)])
+    pent = np.nonzero(g.v_deg == 5)[0]
+    near = np.zeros(g.ne, dtype=bool)
+    near[g.v2e[pent, :5].ravel()] = True            # the five fan edges of each pentagon
+    assert (n[~near] == 15).all()
+    assert (n[near] == 14).all() and near.sum() == 60
+    assert all(len(dd.ddt_vn_reads(g, e)[1]) == 2 for e in range(0, g.ne, 7))
+
+
+def test_decomposition_ranges_closed_forms():
+    from oracle import decomposition as dd
+    for nc, R in ((80, 1), (80, 3), (320, 7), (1280, 8), (5120, 148)):
+        P = nc // 4
+        own = dd.cell_owner(nc, R)
+        assert own.min() == 0 and own.max() == R - 1 and (np.diff(own) >= 0).all()       # contiguous, in rank order
+        assert (own.reshape(-1, 4) == own[::4, None]).all()                                # whole parents
+        sizes = np.bincount(own, minlength=R)
+        assert sizes.sum() == nc and sizes.max() - sizes.min() <= 4                        # balanced to one parent
+        for r in range(R):
+            lo, hi = dd.part_range(P, R, r)
+            assert (own[4 * lo:4 * hi] == r).all() and hi - lo == sizes[r] // 4
+    # equal ranges where R divides P: rank r owns cells [r Nc / R, (r+1) Nc / R)
+    own = dd.cell_owner(1280, 8)
+    assert (own == np.arange(1280) // 160).all()
+
+
+def test_decomposition_required_columns_and_ownership(oracle_grid):
+    """the union over the owned points; with one rank it is every column; an ownership that gives an edge to a rank
+    owning neither of its cells is reported"""
+    from oracle import decomposition as dd
+    g = oracle_grid(2)
+    e_all, c_all = dd.required_columns(g, range(g.ne), range(g.nc), range(g.nv))
+    assert (e_all == np.arange(g.ne)).all() and (c_all == np.arange(g.nc)).all()
+    co = dd.cell_owner(g.nc, 4)
+    eo = co[g.e2c[:, 0]]                                  # lower cell's rank owns the edge
+    vo = np.array([co[g.v2c[v][:g.v_deg[v]]].min() for v in range(g.nv)])
+    assert dd.check_ownership(g, 4, eo, vo) == []
+    bad = eo.copy()
+    interior = np.nonzero(co[g.e2c[:, 0]] == co[g.e2c[:, 1]])[0]
+    bad[interior[0]] = (bad[interior[0]] + 1) % 4
+    assert dd.check_ownership(g, 4, bad, vo) != []
+    # the halo of rank 1: every required edge not owned lies within two cell rings of an owned cell (SURVEY 8(e))
+    mine = np.nonzero(eo == 1)[0]
+    need_e, need_c = dd.required_columns(g, mine, np.nonzero(co == 1)[0], np.nonzero(vo == 1)[0])
+    ring = set(np.nonzero(co == 1)[0].tolist())
+    for _ in range(2):
+        ring |= {int(c) for e in range(g.ne) if int(g.e2c[e][0]) in ring or int(g.e2c[e][1]) in ring for c in g.e2c[e]}
+        ring |= {int(c) for v in range(g.nv) for c in g.v2c[v][:g.v_deg[v]]
+                 if any(int(x) in ring for x in g.v2c[v][:g.v_deg[v]])}
+    ring_edges = {int(e) for c in ring for e in g.c2e[c]}
+    assert set(need_e.tolist()) <= ring_edges and set(need_c.tolist()) <= ring
+    assert len(need_e) > len(mine) and set(mine.tolist()) <= set(need_e.tolist())
