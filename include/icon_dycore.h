@@ -47,7 +47,7 @@ typedef struct icon_grid icon_grid_t;   /* opaque; owns host and device copies o
 enum { ICON_OK = 0, ICON_EINVAL = -1, ICON_ENOMEM = -2, ICON_ECUDA = -3, ICON_EUNSUPPORTED = -4 };
 enum { ICON_F64 = 0, ICON_F32 = 1 };
 /* element types reported by icon_grid_table_host */
-enum { ICON_T_I32 = 10, ICON_T_I8 = 11, ICON_T_F64 = 12, ICON_T_F32 = 13 };
+enum { ICON_T_I32 = 10, ICON_T_I8 = 11, ICON_T_F64 = 12, ICON_T_F32 = 13, ICON_T_I64 = 14 };
 
 /* icon_grid_create flags */
 enum {
@@ -283,6 +283,57 @@ int dycore_velocity_tendencies_noalloc(const icon_grid_t* g, int dtype, int nlev
 int dycore_step_host(const icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
                      const void* vn_host, const void* w_host,
                      void* ddt_vn_host, void* div_host, void* vort_host);
+
+/*
+ * ---- horizontal domain decomposition (reading P-21 in DESIGN.md section 3) ----
+ * The paper runs the model on subdomains of the horizontal grid that exchange halos point to point.
+ * Rank `part` of `n_parts` owns the parent triangles floor(part P / n_parts) <= q < floor((part+1) P / n_parts) of the
+ * hierarchical numbering, P = nc / 4 (cells 4q .. 4q+3); an edge or vertex shared by two ranks is owned by the rank whose
+ * patch stores it, so every output point of the grid has exactly one owner.
+ *
+ * icon_grid_create_part -- the LOCAL grid of one rank. Flags: 0 or ICON_HOST_ONLY (a decomposed grid is never
+ * permuted). Its counts (icon_grid_counts) are LOCAL: ne = owned + halo edges, nc = owned + halo cells, nv = owned
+ * vertices. Local rows: [0, n_owned) the owned points in ascending global id, then the halo, grouped by owner rank
+ * ascending and by global id within a rank, so what one peer sends is ONE contiguous block of rows.
+ * Fields passed to the compute calls are local: vn [ne][ldk], w [nc][ldk_w] with their halo rows filled (dycore_halo_pack
+ * on the owner, any transport, receive in place), outputs ddt_vn [ne][ldk] (rows < ne_owned written), div [nc][ldk]
+ * (rows < nc_owned written), vort [nv][ldk]. On a local grid the calls served by the column-cache kernel work
+ * (dycore_step, dycore_step_w, dycore_velocity_tendencies without optional outputs, dycore_div_vort,
+ * dycore_velocity_tendencies_metric; nlev <= 95 for 8-byte, 127 for 4-byte columns); every other call and every global
+ * table selector returns ICON_EUNSUPPORTED. Host memory: the call builds the GLOBAL grid once and drops it.
+ * Errors: ICON_EINVAL (k, flags, n_parts < 1 or > nc/4, part), ICON_ENOMEM, ICON_ECUDA.
+ */
+int icon_grid_create_part(int bisections_k, unsigned flags, int n_parts, int part, icon_grid_t** out);
+
+/* icon_part_info -- out[0] n_parts (0: not a local grid), [1] part, [2] nc_owned, [3] ne_owned, [4] nv_owned, [5] nc_local,
+ * [6] ne_local, [7] nc_global, [8] ne_global, [9] nv_global, [10] first owned parent, [11] one past the last. */
+int icon_part_info(const icon_grid_t* g, int64_t out[12]);
+
+/* icon_part_table -- host pointers into the handle (valid until destroy). */
+enum {
+    ICON_PART_L2G_CELL = 0,    /* int32 [nc]  global id of local cell row */
+    ICON_PART_L2G_EDGE,        /* int32 [ne] */
+    ICON_PART_L2G_VERT,        /* int32 [nv] */
+    ICON_PART_RECV_BEGIN_EDGE, /* int64 [n_parts+1] rows [b[q], b[q+1]) of a local edge field are owned by rank q */
+    ICON_PART_RECV_BEGIN_CELL, /* int64 [n_parts+1] the same for cell fields */
+    ICON_PART_SEND_BEGIN_EDGE, /* int64 [n_parts+1] rows [b[q], b[q+1]) of the packed buffer go to rank q */
+    ICON_PART_SEND_BEGIN_CELL,
+    ICON_PART_SEND_IDS_EDGE,   /* int32 [b[n_parts]] local (owned) row packed at each position, the receiver's order */
+    ICON_PART_SEND_IDS_CELL,
+    ICON_PART_COUNT
+};
+int icon_part_table(const icon_grid_t* g, int which, const void** ptr, int* dtype, int64_t* count);
+
+/*
+ * dycore_halo_pack -- the send side of the exchange: gathers whole rows of a local field into one contiguous buffer,
+ *   send_buf[i][0..ld) = field[send_ids[i]][0..ld),   i < send_begin[n_parts]
+ * kind 0 = edge field (vn), 1 = cell field (w); ld = row stride in elements, ld*sizeof(T) a multiple of 16; field and
+ * send_buf dev, not overlapping. Rows [send_begin[q], send_begin[q+1]) of send_buf are what rank q receives into rows
+ * [recv_begin[part], recv_begin[part+1]) of ITS local field: with an all-to-all of those splits (NCCL grouped send / recv
+ * over NVLink) the receive lands in place and nothing is unpacked. One kernel launch, asynchronous on cuda_stream.
+ */
+int dycore_halo_pack(const icon_grid_t* g, int dtype, int kind, int ld, const void* field, void* send_buf,
+                     void* cuda_stream);
 
 /* number of kernels the library has launched through this handle since creation */
 int64_t icon_grid_launch_count(const icon_grid_t* g);

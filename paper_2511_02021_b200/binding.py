@@ -29,7 +29,8 @@ TABLE_ID = {n: i for i, n in enumerate(TABLES)}
 # every symbol include/icon_dycore.h declares
 EXPORTS = ("icon_grid_create", "icon_grid_destroy", "icon_grid_counts", "icon_grid_table_host",
            "icon_grid_table_device", "icon_grid_set_option", "icon_grid_cc_schedule_check", "dycore_div_vort", "dycore_velocity_tendencies",
-           "dycore_step", "dycore_step_host", "dycore_step_w", "dycore_w_tendency", "dycore_velocity_tendencies_noalloc", "dycore_metric_from_zhalf", "dycore_velocity_tendencies_metric", "icon_grid_launch_count", "icon_last_error")
+           "dycore_step", "dycore_step_host", "dycore_step_w", "dycore_w_tendency", "dycore_velocity_tendencies_noalloc", "dycore_metric_from_zhalf", "dycore_velocity_tendencies_metric", "icon_grid_launch_count", "icon_last_error",
+           "icon_grid_create_part", "icon_part_info", "icon_part_table", "dycore_halo_pack")
 
 
 class IconError(RuntimeError):
@@ -85,6 +86,14 @@ def load_library():
     L.dycore_step.argtypes = [P, ci, ci, ci, ci, P, P, P, P, P, P, P]
     L.dycore_step_host.restype = ci
     L.dycore_step_host.argtypes = [P, ci, ci, ci, ci, P, P, P, P, P, P]
+    L.icon_grid_create_part.restype = ci
+    L.icon_grid_create_part.argtypes = [ci, ctypes.c_uint, ci, ci, ctypes.POINTER(P)]
+    L.icon_part_info.restype = ci
+    L.icon_part_info.argtypes = [P, ctypes.POINTER(i64)]
+    L.icon_part_table.restype = ci
+    L.icon_part_table.argtypes = [P, ci, ctypes.POINTER(P), ctypes.POINTER(ci), ctypes.POINTER(i64)]
+    L.dycore_halo_pack.restype = ci
+    L.dycore_halo_pack.argtypes = [P, ci, ci, ci, P, P, P]
     L.icon_last_error.restype = ctypes.c_char_p
     L.icon_last_error.argtypes = []
     _lib = L
@@ -116,16 +125,29 @@ def _stream_ptr(stream):
     return ctypes.c_void_p(stream.cuda_stream)
 
 
-_NP = {ICON_T_I32: np.int32, ICON_T_I8: np.int8, ICON_T_F64: np.float64, ICON_T_F32: np.float32}
+ICON_T_I64 = 14
+_NP = {ICON_T_I32: np.int32, ICON_T_I8: np.int8, ICON_T_F64: np.float64, ICON_T_F32: np.float32, ICON_T_I64: np.int64}
+
+# icon_part_table selectors (include/icon_dycore.h)
+PART_TABLES = ("l2g_cell", "l2g_edge", "l2g_vert", "recv_begin_edge", "recv_begin_cell", "send_begin_edge", "send_begin_cell",
+               "send_ids_edge", "send_ids_cell")
+PART_INFO = ("n_parts", "part", "nc_owned", "ne_owned", "nv_owned", "nc_local", "ne_local", "nc_global", "ne_global", "nv_global",
+             "parent_lo", "parent_hi")
 
 
 class IconGrid:
     """icon_grid_t handle (R2Bk grid + tables on host and device)."""
 
-    def __init__(self, k, seed=0, flags=0):
+    def __init__(self, k, seed=0, flags=0, n_parts=0, part=0):
+        """n_parts > 0: the LOCAL grid of rank `part` of `n_parts` (icon_grid_create_part; counts are local)"""
         self._L = load_library()
         h = ctypes.c_void_p()
-        _check(self._L.icon_grid_create(int(k), int(seed), int(flags), ctypes.byref(h)))
+        if n_parts:
+            if seed:
+                raise ValueError("a decomposed grid keeps the hierarchical numbering: no seed")
+            _check(self._L.icon_grid_create_part(int(k), int(flags), int(n_parts), int(part), ctypes.byref(h)))
+        else:
+            _check(self._L.icon_grid_create(int(k), int(seed), int(flags), ctypes.byref(h)))
         self._h = h
         self.k, self.seed, self.flags = int(k), int(seed), int(flags)
         nc, ne, nv = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int64()
@@ -156,6 +178,23 @@ class IconGrid:
         p = ctypes.c_void_p()
         _check(self._L.icon_grid_table_device(self._h, TABLE_ID[name], dtype, ctypes.byref(p)))
         return p.value
+
+    def part_info(self):
+        out = (ctypes.c_int64 * 12)()
+        _check(self._L.icon_part_info(self._h, out))
+        return dict(zip(PART_INFO, [int(x) for x in out]))
+
+    def part_table(self, name):
+        """numpy view (do not write) of a table of the local grid: PART_TABLES"""
+        ptr, dt, n = ctypes.c_void_p(), ctypes.c_int(), ctypes.c_int64()
+        _check(self._L.icon_part_table(self._h, PART_TABLES.index(name), ctypes.byref(ptr), ctypes.byref(dt), ctypes.byref(n)))
+        npdt = np.dtype(_NP[dt.value])
+        if n.value == 0:
+            return np.zeros(0, dtype=npdt)
+        buf = (ctypes.c_char * (n.value * npdt.itemsize)).from_address(ptr.value)
+        a = np.frombuffer(buf, dtype=npdt, count=n.value)
+        a.flags.writeable = False
+        return a
 
     def set_option(self, option, value):
         _check(self._L.icon_grid_set_option(self._h, option, value))
@@ -287,6 +326,16 @@ def dycore_step_w(grid, z_half, vn, w, ddt_vn, div, vort, ddt_w, nlev, stream=No
                    ("div", div, grid.nc, "ldk"), ("vort", vort, grid.nv, "ldk"), ("ddt_w", ddt_w, grid.nc, "ldk_w")))
     _check(grid._L.dycore_step_w(grid._h, _dtype_of(vn), int(nlev), int(vn.shape[1]), int(w.shape[1]), _dptr(z), _dptr(vn),
                                  _dptr(w), _dptr(ddt_vn), _dptr(div), _dptr(vort), _dptr(ddt_w), _stream_ptr(stream)))
+
+
+def dycore_halo_pack(grid, kind, field, send_buf, stream=None):
+    """send side of the halo exchange: send_buf[i] = field[send_ids[i]], whole rows. kind 0 = edge
+    field, 1 = cell field; field [n_local][ld], send_buf [n_send][ld]: CUDA tensors of one dtype."""
+    rows = grid.ne if kind == 0 else grid.nc
+    n_send = len(grid.part_table("send_ids_edge" if kind == 0 else "send_ids_cell"))
+    _check_fields((("field", field, rows, "ld"), ("send_buf", send_buf, n_send, "ld")))
+    _check(grid._L.dycore_halo_pack(grid._h, _dtype_of(field), int(kind), int(field.shape[1]), _dptr(field), _dptr(send_buf),
+                                    _stream_ptr(stream)))
 
 
 def dycore_step_host(grid, z_half, vn_host, w_host, ddt_vn_host, div_host, vort_host, nlev):

@@ -9,8 +9,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libicon_dycore.so")
-SOURCES = ["api.cu", "kernels.cu", "kernels_sc.cu", "kernels_cc.cu", "host_grid.cpp", "sc_tables.cpp", "cc_schedule.cpp", "cc_schedule_check.cpp"]
-HEADERS = ["device_grid.hpp", "host_grid.hpp", "sc_tables.hpp", "cc_schedule.hpp", "kernels.cuh", os.path.join("..", "..", "include", "icon_dycore.h")]
+SOURCES = ["api.cu", "kernels.cu", "kernels_sc.cu", "kernels_cc.cu", "host_grid.cpp", "sc_tables.cpp", "cc_schedule.cpp", "cc_schedule_check.cpp", "partition.cpp"]
+HEADERS = ["device_grid.hpp", "host_grid.hpp", "sc_tables.hpp", "cc_schedule.hpp", "partition.hpp", "kernels.cuh", os.path.join("..", "..", "include", "icon_dycore.h")]
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
     "-Xcompiler", "-fPIC,-fopenmp,-O2", "-shared", "-lgomp",

@@ -109,6 +109,8 @@ int upload_index_tables(icon_grid* g) {
 template <class T>
 int ensure_coeffs(icon_grid* g, icon::DevCoeffs<T>& c) {
     if (c.ready) return ICON_OK;
+    if (g->part.n_parts)      // a local grid holds patch records only: no global tables to upload
+        return fail(ICON_EUNSUPPORTED, "this call (or this kernel option / level count) needs the global tables: not available on a grid made by icon_grid_create_part");
     const icon::HostGrid& h = g->host;
     const auto& uc = g->worklist ? h.user_of_pos_c : kIdentity;
     const auto& ue = g->worklist ? h.user_of_pos_e : kIdentity;
@@ -433,7 +435,7 @@ int tendencies_impl(icon_grid* g, icon::DevCoeffs<T>& c, icon::DevScTables<T>& s
     // div_fused / vort_fused: dycore_step asks for S1 + S2 from the same pass; only the column-cache kernel can
     // (it sets *fused_done), with any other kernel the caller launches dycore_div_vort afterwards
     int rc;
-    if ((rc = ensure_coeffs(g, c))) return rc;
+    if (!g->part.n_parts && (rc = ensure_coeffs(g, c))) return rc;
     void* abc = nullptr;
     if ((rc = get_level_coeffs(g, dtype, nlev, z_half, &abc))) return rc;
     const bool want_opt = vt_opt || ke_c_opt || vort_opt;
@@ -444,6 +446,7 @@ int tendencies_impl(icon_grid* g, icon::DevCoeffs<T>& c, icon::DevScTables<T>& s
         if ((rc = ensure_cc_tables(g, ct, nlev, ldk, ldk_w))) return rc;
         if (ct.unsupported) variant = 3;      // level count the column cache cannot hold
     }
+    if (g->part.n_parts && (variant != 4 || want_opt) && (rc = ensure_coeffs(g, c))) return rc;      // fails: column cache only
     if (variant != 4 || want_opt) div_fused = vort_fused = nullptr;
     if (fused_done) *fused_done = div_fused != nullptr;
     if (variant == 4 && !want_opt) {
@@ -474,6 +477,7 @@ struct TableInfo {
     int cols;
 };
 int table_info(const icon_grid* g, int which, TableInfo* t) {
+    if (g->part.n_parts) return fail(ICON_EUNSUPPORTED, "a grid made by icon_grid_create_part holds no global tables (icon_part_table has the local ones)");
     const icon::HostGrid& h = g->host;
     auto I = [&](const std::vector<int32_t>& v, int64_t rows, int cols) { *t = {v.data(), ICON_T_I32, rows, cols}; };
     auto B = [&](const std::vector<int8_t>& v, int64_t rows, int cols) { *t = {v.data(), ICON_T_I8, rows, cols}; };
@@ -644,6 +648,124 @@ int icon_grid_set_option(icon_grid_t* g, int option, int value) {
 }
 
 int64_t icon_grid_launch_count(const icon_grid_t* g) { return g ? g->launches : 0; }
+
+// ---- horizontal domain decomposition (reading P-21; partition.hpp) ----------------------------------
+int icon_grid_create_part(int bisections_k, unsigned flags, int n_parts, int part, icon_grid_t** out) {
+    if (!out) return fail(ICON_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (bisections_k < 0 || bisections_k > 9) return fail(ICON_EINVAL, "bisections_k must be in 0..9");
+    if (flags & ~(unsigned)ICON_HOST_ONLY)
+        return fail(ICON_EINVAL, "icon_grid_create_part: flags must be 0 or ICON_HOST_ONLY (a decomposed grid keeps the hierarchical numbering)");
+    if (n_parts < 1 || part < 0 || part >= n_parts) return fail(ICON_EINVAL, "icon_grid_create_part: need n_parts >= 1 and 0 <= part < n_parts");
+    icon_grid* g = new (std::nothrow) icon_grid();
+    if (!g) return fail(ICON_ENOMEM, "out of host memory");
+    g->flags = flags;
+    g->host_only = (flags & ICON_HOST_ONLY) != 0;
+    g->options[ICON_OPT_TENDENCY_KERNEL] = 5;
+    g->options[ICON_OPT_CC_TILE] = -1;
+    g->options[ICON_OPT_CC_PACE] = 512;
+    try {
+        // the global grid and its patch records live only inside this block
+        icon::HostGrid global;
+        std::string err = icon::build_host_grid(bisections_k, 0, false, global);
+        icon::ScTables gsc;
+        if (err.empty()) err = icon::build_sc_tables(global, gsc);
+        if (err.empty()) err = icon::build_partition(gsc, global.nc, global.ne, global.nv, n_parts, part, g->sc_host, g->part);
+        if (!err.empty()) {
+            delete g;
+            return fail(ICON_EINVAL, err);
+        }
+    } catch (const std::bad_alloc&) {
+        delete g;
+        return fail(ICON_ENOMEM, "out of host memory while building the local grid");
+    }
+    g->sc_host_ready = true;
+    g->host.level_k = bisections_k;
+    g->host.nc = g->part.nc_local;       // every size check and every kernel sees the LOCAL counts
+    g->host.ne = g->part.ne_local;
+    g->host.nv = g->part.nv_owned;
+    if (!g->host_only) {
+        int ndev = 0;
+        cudaError_t e = cudaGetDeviceCount(&ndev);
+        if (e != cudaSuccess || ndev == 0) {
+            delete g;
+            return fail(ICON_ECUDA, "no usable CUDA device (there is no CPU fallback)");
+        }
+        int rc = ICON_OK;
+        e = cudaGetDevice(&g->device);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&g->num_sms, cudaDevAttrMultiProcessorCount, g->device);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&g->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, g->device);
+        if (e != cudaSuccess) rc = fail_cuda(e, "cudaGetDevice");
+        for (int kind = 0; kind < 2 && rc == ICON_OK; ++kind) rc = upload_vec(g, g->part.send_ids[kind], &g->d_send_ids[kind]);
+        if (rc == ICON_OK && cudaStreamSynchronize(cudaStreamLegacy) != cudaSuccess) rc = fail(ICON_ECUDA, "upload of the send lists failed");
+        if (rc != ICON_OK) {
+            std::string keep = t_last_error;
+            icon_grid_destroy(g);
+            t_last_error = keep;
+            return rc;
+        }
+    }
+    *out = g;
+    return ICON_OK;
+}
+
+int icon_part_info(const icon_grid_t* g, int64_t out[12]) {
+    if (!g || !out) return fail(ICON_EINVAL, "NULL argument");
+    const icon::PartTables& p = g->part;
+    const int64_t v[12] = {p.n_parts, p.part, p.nc_owned, p.ne_owned, p.nv_owned, p.nc_local, p.ne_local,
+                           p.nc_global, p.ne_global, p.nv_global, p.patch_lo, p.patch_hi};
+    for (int i = 0; i < 12; ++i) out[i] = v[i];
+    return ICON_OK;
+}
+
+int icon_part_table(const icon_grid_t* g, int which, const void** ptr, int* dtype, int64_t* count) {
+    if (!g) return fail(ICON_EINVAL, "grid handle is NULL");
+    if (!g->part.n_parts) return fail(ICON_EUNSUPPORTED, "icon_part_table: the grid was not made by icon_grid_create_part");
+    const icon::PartTables& p = g->part;
+    const void* d = nullptr;
+    int64_t n = 0;
+    int dt = ICON_T_I32;
+    auto I32 = [&](const std::vector<int32_t>& v) { d = v.data(); n = (int64_t)v.size(); dt = ICON_T_I32; };
+    auto I64 = [&](const std::vector<int64_t>& v) { d = v.data(); n = (int64_t)v.size(); dt = ICON_T_I64; };
+    switch (which) {
+        case ICON_PART_L2G_CELL: I32(p.l2g_c); break;
+        case ICON_PART_L2G_EDGE: I32(p.l2g_e); break;
+        case ICON_PART_L2G_VERT: I32(p.l2g_v); break;
+        case ICON_PART_RECV_BEGIN_EDGE: I64(p.recv_begin[0]); break;
+        case ICON_PART_RECV_BEGIN_CELL: I64(p.recv_begin[1]); break;
+        case ICON_PART_SEND_BEGIN_EDGE: I64(p.send_begin[0]); break;
+        case ICON_PART_SEND_BEGIN_CELL: I64(p.send_begin[1]); break;
+        case ICON_PART_SEND_IDS_EDGE: I32(p.send_ids[0]); break;
+        case ICON_PART_SEND_IDS_CELL: I32(p.send_ids[1]); break;
+        default: return fail(ICON_EINVAL, "unknown partition table selector");
+    }
+    if (ptr) *ptr = d;
+    if (dtype) *dtype = dt;
+    if (count) *count = n;
+    return ICON_OK;
+}
+
+int dycore_halo_pack(const icon_grid_t* gc, int dtype, int kind, int ld, const void* field, void* send_buf, void* cuda_stream) {
+    icon_grid* g = const_cast<icon_grid*>(gc);       // logically const: only the launch counter moves
+    if (!g) return fail(ICON_EINVAL, "grid handle is NULL");
+    if (!g->part.n_parts) return fail(ICON_EUNSUPPORTED, "dycore_halo_pack: the grid was not made by icon_grid_create_part");
+    if (g->host_only) return fail(ICON_ECUDA, "grid was created with ICON_HOST_ONLY: no device tables, and there is no CPU path");
+    if (int rc = check_device(g)) return rc;
+    if (dtype != ICON_F64 && dtype != ICON_F32) return fail(ICON_EINVAL, "dtype must be ICON_F64 or ICON_F32");
+    if (kind != 0 && kind != 1) return fail(ICON_EINVAL, "kind must be 0 (edge field) or 1 (cell field)");
+    const int64_t es = dtype == ICON_F64 ? 8 : 4;
+    if (ld < 1 || ((int64_t)ld * es) % 16) return fail(ICON_EINVAL, "ld*sizeof(T) must be a positive multiple of 16");
+    const int64_t n = (int64_t)g->part.send_ids[kind].size();
+    if (n == 0) return ICON_OK;                      // nothing to send (one rank, or no neighbour reads this kind)
+    if (int rc = check_field(field, "field")) return rc;
+    if (int rc = check_field(send_buf, "send_buf")) return rc;
+    const int64_t rows = kind == 0 ? g->part.ne_local : g->part.nc_local;
+    if (overlaps(send_buf, (size_t)(n * ld * es), field, (size_t)(rows * ld * es))) return fail(ICON_EINVAL, "send_buf must not overlap the field");
+    const int k = icon::launch_halo_pack(g->d_send_ids[kind], n, (int64_t)ld * es, field, send_buf, (cudaStream_t)cuda_stream);
+    if (k < 0) return fail_cuda((cudaError_t)(-k), "kernel launch");
+    g->launches += k;
+    return ICON_OK;
+}
 
 int icon_grid_cc_schedule_check(const icon_grid_t* gc, int dtype, int nlev, int ldk, int ldk_w, int n_ctas, int smem_bytes,
                                 int64_t out[8]) {
@@ -845,7 +967,7 @@ int tendencies_metric_impl(icon_grid* g, icon::DevCoeffs<T>& c, icon::DevCcTable
                            const void* wgt, const void* inv, const void* zn, const void* zt, const void* vn, const void* w, void* ddt_vn,
                            cudaStream_t s) {
     int rc;
-    if ((rc = ensure_coeffs(g, c))) return rc;
+    if (!g->part.n_parts && (rc = ensure_coeffs(g, c))) return rc;
     int n;
     if (g->options[ICON_OPT_TENDENCY_KERNEL] >= 4) {
         if ((rc = ensure_cc_tables(g, ct, nlev, ldk, ldk_w, icon::kCcTendM))) return rc;
@@ -859,6 +981,7 @@ int tendencies_metric_impl(icon_grid* g, icon::DevCoeffs<T>& c, icon::DevCcTable
         }
     }
     // level counts the column cache cannot hold, or ICON_OPT_TENDENCY_KERNEL 0 / 3: the unfused pipeline with its metric last stage
+    if (g->part.n_parts && (rc = ensure_coeffs(g, c))) return rc;      // fails: column cache only
     if ((rc = ensure_workspace<T>(g, dtype, ldk))) return rc;
     n = icon::launch_tendencies_unfused_metric<T>(*g, c, nlev, ldk, ldk_w, (const T*)wgt, (const T*)inv, (const T*)zn, (const T*)zt,
                                                   (const T*)vn, (const T*)w, (T*)ddt_vn, (T*)g->ws.vt, (T*)g->ws.ke_e, (T*)g->ws.ke_c,
@@ -1106,6 +1229,7 @@ extern "C" int dycore_velocity_tendencies_noalloc(const icon_grid_t* gc, int dty
     icon_grid* g = const_cast<icon_grid*>(gc);
     int rc = check_common(g, dtype, nlev, ldk, 2);      // includes: the grid's device is the current device
     if (rc) return rc;
+    if (g->part.n_parts) return fail(ICON_EUNSUPPORTED, "dycore_velocity_tendencies_noalloc: not on a grid made by icon_grid_create_part");
     if (nlev > kNoAllocMaxLevels) return fail(ICON_EINVAL, "dycore_velocity_tendencies_noalloc: nlev > 128");
     const size_t es = dtype == ICON_F64 ? 8 : 4;
     if (ldk_w < nlev + 1) return fail(ICON_EINVAL, "ldk_w < nlev+1");

@@ -10,6 +10,7 @@
 #include "host_grid.hpp"
 #include "sc_tables.hpp"
 #include "cc_schedule.hpp"
+#include "partition.hpp"
 
 namespace icon {
 
@@ -130,4 +131,6 @@ struct icon_grid {
     std::vector<void*> owned;                          // every device allocation, freed on destroy
     int options[8] = {0};
     int64_t launches = 0;
+    icon::PartTables part;                             // part.n_parts > 0: the local grid of one rank (icon_grid_create_part)
+    int32_t* d_send_ids[2] = {nullptr, nullptr};       // device copies of part.send_ids (dycore_halo_pack)
 };

@@ -26,6 +26,9 @@ int launch_w_tendency(const icon_grid& g, const DevCoeffs<T>& c, int nlev, int64
                       const T* vn, const T* w, T* ddt_w, cudaStream_t s);
 
 // Metric variant (reading P-20): set-up of the per-edge vertical metrics, and the unfused pipeline with its metric last stage.
+// dycore_halo_pack: out[i] = rows[ids[i]], rows of row_bytes (a multiple of 16) bytes
+int launch_halo_pack(const int32_t* ids, int64_t n_rows, int64_t row_bytes, const void* field, void* out, cudaStream_t s);
+
 template <class T>
 int launch_metric_from_zhalf(const icon_grid& g, int nlev, int64_t ldk, int64_t ldk_w, const T* zh, T* wgt, T* inv, cudaStream_t s);
 template <class T>
