@@ -618,6 +618,127 @@ def run_launch_study(args):
     return 0
 
 
+def run_decomposed(args):
+    """--parts R (reading P-21): the fused step on the LOCAL grid of one rank of R, strong scaling
+    (total work fixed = the config's grid). Under torchrun with WORLD_SIZE == R every rank holds its part and a step is
+    pack(vn) + pack(w) + two all_to_all_single over NCCL + dycore_step; value = the GLOBAL points / the slowest rank's
+    time. With one process it times ONE rank's share of that step (--part r, default R // 2) on one GPU: the two pack
+    kernels and the local dycore_step, halo rows filled once from the global field; there is no transport on one GPU and
+    the line says so. One JSON line."""
+    import torch
+    import torch.distributed as dist
+    import paper_2511_02021_b200 as lib
+    from paper_2511_02021_b200.halo import HaloExchange
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product has no CPU path")
+    R = args.parts
+    if world > 1 and world != R:
+        raise SystemExit("bench.py --parts %d under torchrun needs WORLD_SIZE == %d" % (R, R))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    lib.load_library()
+    cfg = si.CONFIGS[args.config]
+    if cfg["permute"]:
+        raise SystemExit("bench.py --parts: a decomposed grid keeps the hierarchical numbering (configs without permutation)")
+    nlev, f32 = cfg["nlev"], cfg["dtype"] == "f32"
+    gsize = 4 if f32 else 8
+    line = 32 if f32 else 16
+    ldk = args.ldk or (nlev + line - 1) // line * line
+    ldk_w = args.ldk_w or (nlev + 1 + line - 1) // line * line
+    part = rank if world > 1 else (args.part if args.part >= 0 else R // 2)
+    t0 = time.perf_counter()
+    g = lib.IconGrid(cfg["k"], n_parts=R, part=part)
+    t_grid = time.perf_counter() - t0
+    info = g.part_info()
+    le, lc = g.part_table("l2g_edge").astype(np.int64), g.part_table("l2g_cell").astype(np.int64)
+    # the global synthetic state (DESIGN.md section 4), of which this rank keeps its rows; geometry from a host-only grid
+    gg = lib.IconGrid(cfg["k"], flags=lib.ICON_HOST_ONLY)
+    vn_h, w_h, zh = si.make_fields(args.config, gg.table_host("edge_xyz"), gg.table_host("edge_normal"), gg.nc, ldk=ldk, ldk_w=ldk_w,
+                                   pad_value=0.0)
+    gg.close()
+    tdt = torch.float32 if f32 else torch.float64
+    vn, w = torch.from_numpy(vn_h[le]).to(dev), torch.from_numpy(w_h[lc]).to(dev)
+    del vn_h, w_h
+    if world > 1:                     # halo rows must come through the exchange
+        vn[info["ne_owned"]:] = float("nan")
+        w[info["nc_owned"]:] = float("nan")
+    ddt = torch.zeros((g.ne, ldk), dtype=tdt, device=dev)
+    div = torch.zeros((g.nc, ldk), dtype=tdt, device=dev)
+    vort = torch.zeros((g.nv, ldk), dtype=tdt, device=dev)
+    hx = HaloExchange(g)
+    sbuf = [hx.send_buffer(0, vn), hx.send_buffer(1, w)]
+    l2_flush = torch.empty(256 * 2 ** 20, dtype=torch.uint8, device=dev)      # a rank's share may be L2 resident: flush
+
+    def step(evs=None):
+        l2_flush.fill_(1)
+        if evs:
+            evs[0].record()
+        if world > 1:
+            hx.exchange(vn, 0)
+            hx.exchange(w, 1)
+        else:
+            lib.dycore_halo_pack(g, 0, vn, sbuf[0])
+            lib.dycore_halo_pack(g, 1, w, sbuf[1])
+        if evs:
+            evs[1].record()
+        lib.dycore_step(g, zh, vn, w, ddt, div, vort, nlev)
+        if evs:
+            evs[2].record()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    n0 = g.launch_count
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    for i in range(args.steps):
+        step(evs[i])
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    t_ex = np.array([e[0].elapsed_time(e[1]) for e in evs]) * 1e-3
+    t_st = np.array([e[1].elapsed_time(e[2]) for e in evs]) * 1e-3
+    t_all = max_over_ranks(float((t_ex + t_st).mean()), dev)
+    launches = g.launch_count - n0
+    pts_owned = info["ne_owned"] * nlev
+    pts_global = info["ne_global"] * nlev
+    send_rows = (sum(hx.send_rows[0]), sum(hx.send_rows[1]))
+    recv_rows = (info["ne_local"] - info["ne_owned"], info["nc_local"] - info["nc_owned"])
+    bytes_tend, bytes_dv = algorithmic_bytes(info["nc_owned"], info["ne_owned"], info["nv_owned"], nlev, gsize)
+    # the fused step's compulsory bytes as run_ours counts them, on the owned points, plus the halo columns it reads
+    bytes_step = bytes_tend + (info["nc_owned"] + info["nv_owned"]) * nlev * gsize + info["nc_owned"] * 3 * gsize \
+        + (recv_rows[0] * nlev + recv_rows[1] * (nlev + 1)) * gsize
+    peak, peak_src = peak_hbm_gbs()
+    dec = {"n_parts": R, "part": part, "transport": "nccl all_to_all_single" if world > 1 else "none (one process: one rank's kernels only)",
+           "cells_owned": info["nc_owned"], "edges_owned": info["ne_owned"], "edges_halo": recv_rows[0], "cells_halo": recv_rows[1],
+           "halo_fraction_edges": recv_rows[0] / info["ne_owned"], "peers": int(sum(1 for x in hx.recv_rows[0] if x)),
+           "send_bytes_per_step": (send_rows[0] * ldk + send_rows[1] * ldk_w) * gsize,
+           "recv_bytes_per_step": (recv_rows[0] * ldk + recv_rows[1] * ldk_w) * gsize,
+           "exchange_ms" if world > 1 else "pack_ms": float(t_ex.mean() * 1e3), "local_step_ms": float(t_st.mean() * 1e3),
+           "local_step_ms_min": float(t_st.min() * 1e3),
+           "local_step_frac_of_hbm_roofline": bytes_step / float(t_st.mean()) / 1e9 / peak, "peak_source": peak_src,
+           "local_grid_build_s": t_grid}
+    if rank == 0:
+        value = (pts_global if world > 1 else pts_owned) / t_all / 1e9
+        print(json.dumps({"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+                          "ms_per_step": t_all * 1e3, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+                          "dtype": "f32" if f32 else "f64", "data": "synthetic",
+                          "config": {"workload": workload_name(args.config) + (", decomposed over %d ranks" % R if world > 1 else
+                                                                               ", rank %d of %d only (its owned points)" % (part, R)),
+                                     "l2": "flushed between steps", "ldk": ldk, "ldk_w": ldk_w},
+                          "gpu_launches": int(launches), "decomposed": dec}))
+    g.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -635,10 +756,14 @@ def main():
     ap.add_argument("--no-parity-spot", action="store_true", dest="no_parity_spot")
     ap.add_argument("--no-metric", action="store_true", dest="no_metric", help="skip the metric-variant leg (saves 4 more field-sized arrays)")
     ap.add_argument("--spot-points", type=int, default=3000, dest="spot_points")
+    ap.add_argument("--parts", type=int, default=0, help="decomposed sweep over this many ranks (SURVEY 8(f) NEXT-3); see run_decomposed")
+    ap.add_argument("--part", type=int, default=-1, help="with --parts and one process: the rank to time (default parts // 2)")
     ap.add_argument("--launch-study", action="store_true", dest="launch_study", help="CUDA-graph vs stream launches on R2B4 / R2B5")
     args = ap.parse_args()
     if args.launch_study:
         return run_launch_study(args)
+    if args.parts:
+        return run_decomposed(args)
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
     return run_reference(args) if args.impl == "reference" else run_ours(args)

@@ -194,3 +194,44 @@ def test_decomposed_other_calls_and_rejections(torch_cuda, lib, oracle_grid):
         assert ei.value.code == -4
     finally:
         g.close()
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("config,R,part,host_gb", [(2, 8, 3, 6), (3, 8, 5, 60)])
+def test_full_size_decomposed_sampled(torch_cuda, lib, oracle_mod, config, R, part, host_gb):
+    """one rank of eight at BASELINE.json's sizes, in the launch configuration `bench.py --parts 8` times (padded leading
+    dimensions, halo rows holding the owners' values): the owned outputs on sampled points the oracle computes one by one,
+    and the properties that hold at any size (every owned level written once, no halo row and no pad written)"""
+    import psutil
+    torch = torch_cuda
+    if psutil.virtual_memory().available / 2 ** 30 < host_gb:
+        pytest.skip("needs %d GB of host memory" % host_gb)
+    from test_gpu_parity import bench_padding
+    cfg = si.CONFIGS[config]
+    nlev = cfg["nlev"]
+    dev = torch.device("cuda:0")
+    og = oracle_mod.Grid(cfg["k"])
+    ldk, ldk_w = bench_padding(nlev, False)
+    vn, w, zh = si.make_fields(config, og.edge_xyz, og.edge_normal, og.nc, ldk=ldk, ldk_w=ldk_w, pad_value=0.0)
+    g = lib.IconGrid(cfg["k"], n_parts=R, part=part)
+    try:
+        i = g.part_info()
+        assert (i["nc_global"], i["ne_global"]) == (og.nc, og.ne) and i["nc_owned"] == og.nc // R
+        l2g = [g.part_table("l2g_" + n).astype(np.int64) for n in ("edge", "cell", "vert")]
+        d_vn, d_w = torch.from_numpy(vn[l2g[0]]).to(dev), torch.from_numpy(w[l2g[1]]).to(dev)
+        sent = float("nan")
+        outs = [torch.full((n, ldk), sent, dtype=torch.float64, device=dev) for n in (g.ne, g.nc, g.nv)]
+        n0 = g.launch_count
+        lib.dycore_step(g, zh, d_vn, d_w, outs[0], outs[1], outs[2], nlev)
+        torch.cuda.synchronize()
+        assert g.launch_count - n0 == 1
+        for what, arr, rows, n_owned in zip(("ddt_vn", "div", "vort"), outs, l2g, (i["ne_owned"], i["nc_owned"], i["nv_owned"])):
+            idx, lev = si.sample_points(900 + config, n_owned, nlev, 20000)
+            got = arr[torch.from_numpy(idx).to(dev), torch.from_numpy(lev.astype(np.int64)).to(dev)].cpu().numpy()
+            want, m = og.sample(what, rows[idx], lev, vn, nlev, w=w, z_half=zh)
+            err = np.abs(got - want)
+            assert (err <= 1e-12 * m).all(), "%s config %d: worst err/M %.3e" % (what, config, (err / m).max())
+            assert not torch.isnan(arr[:n_owned, :nlev]).any(), what
+            assert torch.isnan(arr[n_owned:]).all() and torch.isnan(arr[:, nlev:]).all(), what
+    finally:
+        g.close()
