@@ -48,7 +48,14 @@ constexpr int kCcWarps = 8, kCcGroup = 4, kCcDepth = 3;
 //         pointers besides six values per column and spill 100 bytes at 216 registers; with four producer warps and 232
 //         registers everything was slower). The tendency shares its schedule with the fused step, so both keep L = 3.
 CC_HD constexpr int cc_patches_per_warp(int L) { return L == 2 || L == 6 ? 2 : 1; }
-CC_HD constexpr int cc_patches_per_step(int L) { return kCcGroup * cc_patches_per_warp(L); }
+// Consumer warps of a CTA as a function of the column type and the level mapping: kCcWarps everywhere. The shape is a
+// parameter because 4-byte columns were tried with SIXTEEN consumer warps (two groups of eight, eight patches per step,
+// 104 registers each, four producer warps; launch 640 x 96): the consumers then spill 96-288 bytes and config 4 measured
+// 3.29 ms against 3.37 ms for the fused step and 2.76 against 2.72 ms for the tendency -- the 8-warp kernel is not bound
+// by the number of warps a scheduler can pick from (profiles/r02_experiments.md).
+CC_HD constexpr int cc_consumer_warps(int elem_bytes, int L) { return (void)elem_bytes, (void)L, kCcWarps; }
+CC_HD constexpr int cc_group(int elem_bytes, int L) { return cc_consumer_warps(elem_bytes, L) / 2; }
+CC_HD constexpr int cc_patches_per_step(int elem_bytes, int L) { return cc_group(elem_bytes, L) * cc_patches_per_warp(L); }
 // Producer warps are added to the consumers; the CTA is launched with the registers of the average warp and
 // re-balances them with setmaxnreg: producers keep CcWarps::producer_regs, consumers grow to CcWarps::consumer_regs
 // (the pool is what the LAUNCH allocated: 384 * 168 = (4 * 56 + 8 * 224) * 32 = 64512 registers).
@@ -56,12 +63,16 @@ CC_HD constexpr int cc_patches_per_step(int L) { return kCcGroup * cc_patches_pe
 // 4-byte columns: the consumers need fewer registers and the columns are half as long, i.e. twice the copies per byte,
 // so a second producer warpgroup issues them: 8 producer warps with 40 registers, consumers 216 (launch: 512 x 128).
 // Shallow columns (L = 2, nlev <= 31) are the same case: short columns, light consumers.
+// (`wide`: the 16-consumer shape that was tried for 4-byte columns, see cc_consumer_warps; never true now.)
 template <class T, int L>
 struct CcWarps {
     static constexpr bool light = sizeof(T) == 4 || L == 2;
-    static constexpr int producers = light ? 8 : 4;
+    static constexpr bool wide = cc_consumer_warps((int)sizeof(T), L) > kCcWarps;
+    static constexpr int consumers = cc_consumer_warps((int)sizeof(T), L);
+    static constexpr int group = cc_group((int)sizeof(T), L);
+    static constexpr int producers = wide ? 4 : light ? 8 : 4;
     static constexpr int producer_regs = light ? 40 : 56;
-    static constexpr int consumer_regs = light ? 216 : 224;
+    static constexpr int consumer_regs = wide ? 104 : light ? 216 : 224;
 };
 constexpr int kCcMaxProducers = 8;
 constexpr int kCcAhead = 3;              // steps the producers read the schedule ahead; `loads` is padded for it

@@ -270,14 +270,14 @@ __host__ __device__ constexpr int cc_record_bytes(int mode) { return cc_coef_wor
 // tendency needs anyway. MODE kCcDivVort: ONLY div and vorticity (dycore_div_vort) from the 27 vn columns they need, with
 // compact records (52 coefficients) and a schedule of its own.
 template <class T, int L, int MODE>
-__global__ void __launch_bounds__((kCcWarps + CcWarps<T, L>::producers) * 32, 1)
+__global__ void __launch_bounds__((CcWarps<T, L>::consumers + CcWarps<T, L>::producers) * 32, 1)
 k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, const T* __restrict__ vn,
           const T* __restrict__ w, T* __restrict__ ddt_vn, T* __restrict__ div, T* __restrict__ vort,
           unsigned long long* pace_counter, unsigned long long pace_per_launch, int pace_mask, int pace_last,
           const T* __restrict__ wk, T* __restrict__ ddt_w, CcMetric<T> met) {
     extern __shared__ __align__(128) unsigned char smem[];
     using C = Col<T, L>;
-    constexpr int W = kCcWarps, G = kCcGroup, D = kCcDepth;
+    constexpr int W = CcWarps<T, L>::consumers, G = CcWarps<T, L>::group, D = kCcDepth;
     constexpr int PPW = cc_patches_per_warp(L), PPS = G * PPW;      // patches per warp, per step
     constexpr bool METRIC = MODE == kCcTendM;
     constexpr bool FUSED = MODE != kCcTend && !METRIC, DVONLY = MODE == kCcDivVort, WTEND = MODE == kCcStepW;
@@ -925,7 +925,7 @@ int cc_slot_bytes(int nlev) { return (((nlev + 1) * (int)sizeof(T) + 15) & ~15);
 
 template <class T>
 static size_t cc_fixed_smem(int mode, int L) {
-    return kCcBarrierBytes + (size_t)kCcDepth * cc_patches_per_step(L) * cc_record_bytes<T>(mode);
+    return kCcBarrierBytes + (size_t)kCcDepth * cc_patches_per_step((int)sizeof(T), L) * cc_record_bytes<T>(mode);
 }
 
 template <class T>
@@ -944,7 +944,7 @@ int cc_level_mapping(int nlev, int elem_bytes, int mode) {
     const int l = cc_levels_per_lane(nlev);
     return l == 3 && elem_bytes == 4 && mode == kCcDivVort ? 6 : l;
 }
-int cc_patches_per_step_for(int nlev, int elem_bytes, int mode) { return cc_patches_per_step(cc_level_mapping(nlev, elem_bytes, mode)); }
+int cc_patches_per_step_for(int nlev, int elem_bytes, int mode) { return cc_patches_per_step(elem_bytes, cc_level_mapping(nlev, elem_bytes, mode)); }
 
 namespace {
 template <class T, int L, int MODE>
@@ -964,7 +964,7 @@ cudaError_t cc_launch_one(const CcDev<T>& d, int device, int n_ctas, size_t smem
             if (known) configured[device] = smem;
         }
     }
-    k<<<(unsigned)n_ctas, (kCcWarps + CcWarps<T, L>::producers) * 32, smem, s>>>(d, nlev, ldk, ldk_w, abc, vn, w, ddt_vn, div, vort, pc, ppl, pm, pl, wk, ddt_w, met);
+    k<<<(unsigned)n_ctas, (CcWarps<T, L>::consumers + CcWarps<T, L>::producers) * 32, smem, s>>>(d, nlev, ldk, ldk_w, abc, vn, w, ddt_vn, div, vort, pc, ppl, pm, pl, wk, ddt_w, met);
     return cudaGetLastError();
 }
 }  // namespace
