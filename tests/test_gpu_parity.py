@@ -276,7 +276,7 @@ def test_fused_step_pacing_barrier_periods(torch_cuda, lib, oracle_grid, period)
 @pytest.mark.parametrize("tile", [16, 64, 0])
 @pytest.mark.parametrize("dtype,nlev,ldk,ldk_w", [("f64", 90, 96, 96), ("f64", 90, 90, 92), ("f64", 33, 34, 34), ("f32", 90, 96, 96),
                                                    ("f32", 90, 92, 92), ("f64", 30, 32, 32), ("f64", 3, 4, 4), ("f64", 64, 64, 66),
-                                                   ("f64", 95, 96, 96)])
+                                                   ("f64", 95, 96, 96), ("f32", 30, 32, 32), ("f32", 31, 32, 32)])
 def test_column_cache_level_mappings_and_tiles(torch_cuda, lib, oracle_grid, tile, dtype, nlev, ldk, ldk_w):
     """kernel 4 with the default tiles, larger tiles and contiguous ranges; every level
     mapping (one level per lane; pair + single with the single segment empty, partly and completely filled, odd and even
