@@ -248,6 +248,8 @@ int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev, int64_t ld
                 for (int i = 0; i < 12; ++i) cf[icon::DVF_DIV + i] = (T)scf[icon::SCF_DIV + i];
                 for (int i = 0; i < 20; ++i) cf[icon::DVF_ROT + i] = (T)scf[icon::SCF_ROT + i];
                 for (int i = 0; i < 20; ++i) cf[icon::DVF_XROT + i] = (T)(i < 18 ? scf[icon::SCF_XROT + i] : 0.0);
+            } else if (mode == icon::kCcWTend) {          // compact record: the twelve advection coefficients
+                for (int i = 0; i < icon::kCcWCoefWords; ++i) cf[icon::WF_ADV + i] = (T)scf[icon::SCF_ADV + i];
             } else {
                 for (int i = 0; i < ncoef; ++i) cf[i] = (T)scf[i];      // kCcStepW: with the twelve advection coefficients
             }
@@ -259,7 +261,7 @@ int ensure_cc_tables(icon_grid* g, icon::DevCcTables<T>& p, int nlev, int64_t ld
             }
             for (int x = 0; x < 4; ++x) oid[6 + x] = id[icon::SID_T0 + x];
             for (int x = 0; x < 6; ++x) oid[10 + x] = id[icon::SID_V0 + x];
-            for (int x = 0; x < 6 && !dv; ++x) {   // c_lin halved: the kernel forms w(k) + w(k+1) (exact scaling)
+            for (int x = 0; x < 6 && !dv && mode != icon::kCcWTend; ++x) {   // c_lin halved: the kernel forms w(k) + w(k+1) (exact scaling)
                 cf[icon::SCF_EDGE + 4 * x + 2] *= (T)0.5;
                 cf[icon::SCF_EDGE + 4 * x + 3] *= (T)0.5;
             }
@@ -782,7 +784,7 @@ int icon_grid_cc_schedule_check(const icon_grid_t* gc, int dtype, int nlev, int 
     try {
         // the schedules of dycore_div_vort (27 vn columns per patch, compact records) and of dycore_step_w (all 46 columns)
         // first, then the one of the tendency / fused step, whose shape is reported
-        for (int mode : {(int)icon::kCcDivVort, (int)icon::kCcStepW, (int)icon::kCcStep}) {
+        for (int mode : {(int)icon::kCcDivVort, (int)icon::kCcWTend, (int)icon::kCcStepW, (int)icon::kCcStep}) {
             const bool dv = mode == icon::kCcDivVort;
             geom = f64 ? cc_geometry<double>(nlev, ldk, ldk_w, dv) : cc_geometry<float>(nlev, ldk, ldk_w, dv);
             const int n_slots = std::min(65535, f64 ? icon::cc_max_slots<double>(geom.slot_bytes, smem_bytes, mode, nlev)
@@ -791,7 +793,7 @@ int icon_grid_cc_schedule_check(const icon_grid_t* gc, int dtype, int nlev, int 
                                                       f64 ? cc_resolve_tile<double>(g, nlev) : cc_resolve_tile<float>(g, nlev), icon::cc_use_mask(mode), cs);
             if (!err.empty()) return fail(ICON_EUNSUPPORTED, err);
             err = icon::check_cc_schedule(g->sc_host, cs, g->host.ne, g->host.nc);
-            if (!err.empty()) return fail(ICON_EINVAL, err + (dv ? " (div/vort schedule)" : mode == icon::kCcStepW ? " (step + ddt_w schedule)" : ""));
+            if (!err.empty()) return fail(ICON_EINVAL, err + (dv ? " (div/vort schedule)" : mode == icon::kCcStepW ? " (step + ddt_w schedule)" : mode == icon::kCcWTend ? " (ddt_w schedule)" : ""));
         }
     } catch (const std::bad_alloc&) {
         return fail(ICON_ENOMEM, "out of host memory while building the column-cache schedule");
@@ -889,12 +891,27 @@ int dycore_w_tendency(const icon_grid_t* gc, int dtype, int nlev, int ldk, int l
     if ((rc = get_level_coeffs(g, dtype, nlev, z_half, &abc, &wk))) return rc;
     cudaStream_t s = (cudaStream_t)cuda_stream;
     int n;
+    // the column cache in its ddt_w mode wherever it holds the columns (ICON_OPT_TENDENCY_KERNEL 4 or auto), else the gather
+    // kernel through L1
+    const bool want_cc = g->options[ICON_OPT_TENDENCY_KERNEL] >= 4;
     if (dtype == ICON_F64) {
-        if ((rc = ensure_coeffs(g, g->c64))) return rc;
-        n = icon::launch_w_tendency<double>(*g, g->c64, nlev, ldk, ldk_w, (const double*)wk, (const double*)vn, (const double*)w, (double*)ddt_w, s);
+        if (want_cc && (rc = ensure_cc_tables(g, g->wt64, nlev, ldk, ldk_w, icon::kCcWTend))) return rc;
+        if (want_cc && !g->wt64.unsupported) {
+            n = icon::launch_tendencies_cc<double>(*g, g->wt64, icon::kCcWTend, nlev, ldk, ldk_w, nullptr, (const double*)vn, (const double*)w, nullptr,
+                                                   nullptr, nullptr, s, (const double*)wk, (double*)ddt_w);
+        } else {
+            if ((rc = ensure_coeffs(g, g->c64))) return rc;
+            n = icon::launch_w_tendency<double>(*g, g->c64, nlev, ldk, ldk_w, (const double*)wk, (const double*)vn, (const double*)w, (double*)ddt_w, s);
+        }
     } else {
-        if ((rc = ensure_coeffs(g, g->c32))) return rc;
-        n = icon::launch_w_tendency<float>(*g, g->c32, nlev, ldk, ldk_w, (const float*)wk, (const float*)vn, (const float*)w, (float*)ddt_w, s);
+        if (want_cc && (rc = ensure_cc_tables(g, g->wt32, nlev, ldk, ldk_w, icon::kCcWTend))) return rc;
+        if (want_cc && !g->wt32.unsupported) {
+            n = icon::launch_tendencies_cc<float>(*g, g->wt32, icon::kCcWTend, nlev, ldk, ldk_w, nullptr, (const float*)vn, (const float*)w, nullptr,
+                                                  nullptr, nullptr, s, (const float*)wk, (float*)ddt_w);
+        } else {
+            if ((rc = ensure_coeffs(g, g->c32))) return rc;
+            n = icon::launch_w_tendency<float>(*g, g->c32, nlev, ldk, ldk_w, (const float*)wk, (const float*)vn, (const float*)w, (float*)ddt_w, s);
+        }
     }
     if (n < 0) return fail_cuda((cudaError_t)(-n), "kernel launch");
     g->launches += n;

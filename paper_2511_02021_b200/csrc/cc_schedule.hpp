@@ -81,16 +81,21 @@ constexpr int kCcBarrierBytes = 512;    // the mbarriers
 enum { kCcTend = 0 /* ddt_vn */, kCcStep = 1 /* ddt_vn + div + vort */, kCcDivVort = 2 /* div + vort only */,
        kCcStepW = 3 /* ddt_vn + div + vort + ddt_w (P-19): three more w columns and twelve more coefficients per patch */,
        kCcTendM = 4 /* ddt_vn in its metric form (P-20): 24 more coefficients per patch; the four metric columns of an owned
-                       edge are read straight from global memory */ };
+                       edge are read straight from global memory */,
+       kCcWTend = 5 /* ddt_w alone (dycore_w_tendency, P-19): the nine in-patch vn columns and the ten w columns of a patch,
+                       compact records of twelve coefficients */ };
 // kCcDivVort reads 27 of the 36 vn columns of a patch and no w column, and its records carry only the 52 coefficients it
 // needs: geofac_div [4][3], rot of the midpoints [3][6] (+2 pad), rot of the corners [3][6] (+2 pad)
 enum { DVF_DIV = 0, DVF_ROT = 12, DVF_XROT = 32, kCcDvCoefWords = 52 };
+// kCcWTend: the records carry only SCF_ADV [4][3]
+enum { WF_ADV = 0, kCcWCoefWords = 12 };
 CC_HD constexpr int cc_coef_words(int mode) {
-    return mode == kCcDivVort ? (int)kCcDvCoefWords : mode == kCcTendM ? (int)kScCoefWords : mode == kCcStepW ? (int)SCF_CGRAD : (int)SCF_ADV;
+    return mode == kCcDivVort ? (int)kCcDvCoefWords : mode == kCcWTend ? (int)kCcWCoefWords : mode == kCcTendM ? (int)kScCoefWords : mode == kCcStepW ? (int)SCF_CGRAD : (int)SCF_ADV;
 }
 // id slots (sc_tables.hpp) a mode reads: bit i of the mask = column i of the patch is needed
 constexpr uint64_t cc_use_mask(int mode) {
     if (mode == kCcStepW) return (1ull << SID_PAD) - 1;                  // every column
+    if (mode == kCcWTend) return ((1ull << SID_OM0) - 1) | (((1ull << SID_PAD) - 1) & ~((1ull << SID_T0) - 1));      // i0..i2 b0..b5 | all ten cells
     if (mode != kCcDivVort) return (1ull << SID_XW0) - 1;                // 36 vn + 7 w: all but X1 X3 X5
     uint64_t m = (1ull << SID_X0) - 1;                                   // i0..i2, b0..b5, om0..om5, oc0..oc5
     for (int x = 0; x < 3; ++x) m |= 3ull << (SID_X0 + 5 * x + 3);       // n1, n2 of the three corners

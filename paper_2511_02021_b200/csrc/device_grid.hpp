@@ -121,6 +121,8 @@ struct icon_grid {
     icon::DevCcTables<float> dv32;
     icon::DevCcTables<double> sw64;                    // the same for dycore_step_w (mode kCcStepW)
     icon::DevCcTables<float> sw32;
+    icon::DevCcTables<double> wt64;                    // the same for dycore_w_tendency (mode kCcWTend)
+    icon::DevCcTables<float> wt32;
     icon::DevCcTables<double> m64;                     // the same for dycore_velocity_tendencies_metric (mode kCcTendM)
     icon::DevCcTables<float> m32;
     int smem_optin = 0;                                // cudaDevAttrMaxSharedMemoryPerBlockOptin

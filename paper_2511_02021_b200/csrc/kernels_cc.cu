@@ -1,8 +1,9 @@
 // kernels_cc.cu -- column-cache kernel for the velocity tendency and, fused
-// into the same pass on request, divergence and vorticity (S1, S2: dycore_step), sm_100a. Four modes (template
+// into the same pass on request, divergence and vorticity (S1, S2: dycore_step), sm_100a. Six modes (template
 // parameter MODE, cc_schedule.hpp): kCcTend = ddt_vn (dycore_velocity_tendencies), kCcStep = ddt_vn + div + vort
 // (dycore_step), kCcDivVort = div + vort alone from the 27 vn columns they need (dycore_div_vort), kCcStepW = kCcStep
-// plus the vertical-wind tendency ddt_w (dycore_step_w, reading P-19), kCcTendM = ddt_vn in its metric form
+// plus the vertical-wind tendency ddt_w (dycore_step_w, reading P-19), kCcWTend = ddt_w alone (dycore_w_tendency) from the
+// nine in-patch vn columns and the ten w columns of a patch, kCcTendM = ddt_vn in its metric form
 // (dycore_velocity_tendencies_metric, reading P-20).
 //
 // One warp finishes one self-contained patch (sc_tables.hpp: four sibling cells, six owned edges,
@@ -280,7 +281,8 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
     constexpr int W = CcWarps<T, L>::consumers, G = CcWarps<T, L>::group, D = kCcDepth;
     constexpr int PPW = cc_patches_per_warp(L), PPS = G * PPW;      // patches per warp, per step
     constexpr bool METRIC = MODE == kCcTendM;
-    constexpr bool FUSED = MODE != kCcTend && !METRIC, DVONLY = MODE == kCcDivVort, WTEND = MODE == kCcStepW;
+    constexpr bool WONLY = MODE == kCcWTend;
+    constexpr bool FUSED = MODE != kCcTend && !METRIC && !WONLY, DVONLY = MODE == kCcDivVort, WTEND = MODE == kCcStepW || WONLY;
     constexpr int kCcProducers = CcWarps<T, L>::producers;
     constexpr int REC = cc_record_bytes<T>(MODE), COEF = cc_coef_words(MODE);
     constexpr int NGRP = W / G;
@@ -587,7 +589,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
 
             int32_t ido[16];                    // owned edges i0 i1 i2 b0 b2 b4 | cells T0..T3 | vertices ab bc ca a b c (-1 = not ours)
 #pragma unroll
-            for (int i = 0; i < (FUSED ? 4 : 2); ++i) {
+            for (int i = 0; i < (FUSED ? 4 : WONLY ? 3 : 2); ++i) {
                 const int4 a = reinterpret_cast<const int4*>(oid)[i];
                 ido[4 * i] = a.x; ido[4 * i + 1] = a.y; ido[4 * i + 2] = a.z; ido[4 * i + 3] = a.w;
             }
@@ -630,7 +632,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
                     wrdz[l] = w_int[l] ? __ldg(wk + nlev + 1 + k) : (T)0;
                 }
                 T av[12];
-                ld_coef(cf + SCF_ADV, av);
+                ld_coef(cf + (WONLY ? (int)WF_ADV : (int)SCF_ADV), av);
                 uint32_t sW[12];                    // T0..T3 X0 X2 X4 X1 X3 X5 + mask + pad
                 ld_slots(sl + SID_T0, sW);
                 C wT[4];
@@ -661,6 +663,10 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
                     const C wx = LD(sW[xslot[j]]);
                     const C v = VIE(vB[j]);
                     FORL acc[cell_of[j]].v[l] += av[bslot[j]] * v.v[l] * (wx.v[l] - wT[cell_of[j]].v[l]);
+                }
+                if constexpr (WONLY) {              // ddt_w alone: that was the last slot read of the patch
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(done_bar(s % NB));
                 }
 #pragma unroll
                 for (int c4 = 0; c4 < 4; ++c4) {
@@ -719,7 +725,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
                     FORL z2.v[l] = (T)2 * zc[m].v[l];
                     ST(vort, ido[13 + m], z2);
                 }
-            } else {
+            } else if constexpr (!WONLY) {
             // ---- interior edges: vt, KE_e; start the cell sums -------------------------------
             T r12[12];
             ld_coef(cf + SCF_RBF, r12);
@@ -910,7 +916,7 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
                 ST(ddt_vn, ido[x], o);
             }
             }   // !METRIC
-            }   // !DVONLY
+            }   // !DVONLY && !WONLY
         } else {
             __syncwarp();
             if (lane == 0) mbar_arrive(done_bar(s % NB));
@@ -989,8 +995,9 @@ int launch_tendencies_cc(const icon_grid& g, DevCcTables<T>& p, int mode, int nl
     const unsigned long long per_launch = (unsigned long long)n_barriers * (unsigned long long)p.n_ctas;
     // the tables must have been built for this mode (kCcTend runs on the tables of kCcStep: same columns, same records)
     const bool wants_div = mode == kCcStep || mode == kCcStepW || mode == kCcDivVort;
-    if ((mode == kCcTend ? (int)kCcStep : mode) != p.built_for || (mode == kCcDivVort) != (ddt_vn == nullptr) || wants_div != (div != nullptr) ||
-        (mode == kCcStepW) != (ddt_w != nullptr) || (mode == kCcTendM) != (met != nullptr))
+    const bool no_ddt_vn = mode == kCcDivVort || mode == kCcWTend;
+    if ((mode == kCcTend ? (int)kCcStep : mode) != p.built_for || no_ddt_vn != (ddt_vn == nullptr) || wants_div != (div != nullptr) ||
+        (mode == kCcStepW || mode == kCcWTend) != (ddt_w != nullptr) || (mode == kCcTendM) != (met != nullptr))
         return -(int)cudaErrorInvalidValue;
     const CcMetric<T> metric = met ? *met : CcMetric<T>{nullptr, nullptr, nullptr, nullptr};
     const size_t smem = cc_fixed_smem<T>(mode, L) + (size_t)p.n_slots * p.slot_bytes + kCcSlotTailPad;
@@ -999,7 +1006,7 @@ int launch_tendencies_cc(const icon_grid& g, DevCcTables<T>& p, int mode, int nl
     if (L == LL && mode == MM) \
         err = cc_launch_one<T, LL, MM>(d, g.device, p.n_ctas, smem, nlev, (int)ldk, (int)ldk_w, abc, vn, w, ddt_vn, div, vort, p.progress, per_launch, pace_mask, pace_last, wk, ddt_w, metric, s);
     CC_ONE(2, kCcTend) CC_ONE(2, kCcStep) CC_ONE(2, kCcDivVort) CC_ONE(3, kCcTend) CC_ONE(3, kCcStep)
-    CC_ONE(2, kCcStepW) CC_ONE(3, kCcStepW) CC_ONE(2, kCcTendM) CC_ONE(3, kCcTendM)
+    CC_ONE(2, kCcStepW) CC_ONE(3, kCcStepW) CC_ONE(2, kCcTendM) CC_ONE(3, kCcTendM) CC_ONE(2, kCcWTend) CC_ONE(3, kCcWTend)
     constexpr int LDV = sizeof(T) == 4 ? 6 : 3;          // deep columns in the div / vort mode
     CC_ONE(LDV, kCcDivVort)
 #undef CC_ONE

@@ -362,37 +362,48 @@ def test_dycore_step_replays_in_a_cuda_graph(torch_cuda, lib, oracle_grid, k, pe
 # ----------------------------------------------------------------------------------------------
 # vertical-wind tendency (reading P-19)
 # ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", [5, 0])
 @pytest.mark.parametrize("k,seed,flags,nlev,ldk,ldk_w,dtype", [
     (4, 0, 0, 90, 90, 92, "f64"), (4, 0, 0, 90, 96, 96, "f64"), (3, si.PERMUTE_SEED, 1, 40, 40, 42, "f64"),
     (3, si.PERMUTE_SEED, 1 | 8, 40, 40, 42, "f64"), (4, si.PERMUTE_SEED, 1, 90, 92, 92, "f32"), (0, 0, 0, 2, 2, 4, "f64"),
-    (0, 0, 0, 3, 4, 4, "f64"), (1, 0, 0, 31, 32, 32, "f64"), (1, 0, 0, 33, 34, 34, "f64"), (2, 0, 0, 130, 130, 132, "f64")])
-def test_w_tendency_elementwise(torch_cuda, lib, oracle_mod, oracle_grid, k, seed, flags, nlev, ldk, ldk_w, dtype):
+    (0, 0, 0, 3, 4, 4, "f64"), (1, 0, 0, 31, 32, 32, "f64"), (1, 0, 0, 33, 34, 34, "f64"), (2, 0, 0, 130, 130, 132, "f64"),
+    (2, 0, 0, 30, 32, 32, "f64"), (2, 0, 0, 64, 64, 66, "f64"), (2, 0, 0, 65, 66, 66, "f64"), (2, 0, 0, 95, 96, 96, "f64"),
+    (3, 0, 0, 30, 32, 32, "f32"), (3, 0, 0, 63, 64, 64, "f32")])
+def test_w_tendency_elementwise(torch_cuda, lib, oracle_mod, oracle_grid, variant, k, seed, flags, nlev, ldk, ldk_w, dtype):
     """dycore_w_tendency against og_w_tendency, every half level of every cell; pads stay untouched; also with the
-    oracle evaluating on the LIBRARY's exported tables (P-18)"""
+    oracle evaluating on the LIBRARY's exported tables (P-18). variant 5 (auto): the column cache in its ddt_w mode
+    (nlev = 130 falls back to the gather kernel); variant 0: the gather kernel. Two launches on different inputs (a stale
+    slot of the cache would carry the other input)."""
     torch = torch_cuda
     og = oracle_grid(k, seed, flags & 1)
     g = lib_grid(lib, k, seed, flags)
     f32 = dtype == "f32"
-    vn, w, zh = si.make_fields(4 if flags & 1 else 1, og.edge_xyz, og.edge_normal, og.nc, nlev=nlev, ldk=ldk, ldk_w=ldk_w, dtype=dtype)
     o = og.rounded_f32() if f32 else og
-    vn64, w64 = np.nan_to_num(vn.astype(np.float64)), np.nan_to_num(w.astype(np.float64))
-    want, m = o.w_tendency(vn64, w64, zh, nlev, with_scale=True)
     dev = torch.device("cuda:0")
     sentinel = -9.25
-    out = torch.full((g.nc, ldk_w), sentinel, dtype=torch.from_numpy(w).dtype, device=dev)
-    n0 = g.launch_count
-    lib.dycore_w_tendency(g, zh, torch.from_numpy(vn).to(dev), torch.from_numpy(w).to(dev), out, nlev)
-    torch.cuda.synchronize()
-    assert g.launch_count - n0 == 1
-    got = out.cpu().numpy().astype(np.float64)
-    err = np.abs(got[:, :nlev + 1] - want[:, :nlev + 1])
-    assert (err <= TOL[dtype] * m[:, :nlev + 1]).all(), "worst err/M %.3e" % (err / np.maximum(m[:, :nlev + 1], 1e-300)).max()
-    assert (got[:, 0] == 0).all() and (got[:, nlev] == 0).all()
-    assert (got[:, nlev + 1:] == sentinel).all()
-    if not f32:
-        t = {n: g.table_host(n) for n in ("c2e", "e2c", "inv_d_e", "adv_c")}
-        want2, m2 = oracle_mod.w_tendency_from_arrays(t, vn64, w64, zh, nlev)
-        assert (np.abs(got[:, :nlev + 1] - want2[:, :nlev + 1]) <= TOL[dtype] * m2[:, :nlev + 1]).all()
+    g.set_option(lib.ICON_OPT_TENDENCY_KERNEL, variant)
+    try:
+        for cfg, fv in ((4 if flags & 1 else 1, 1.0), (2, -2.5)):
+            vn, w, zh = si.make_fields(cfg, og.edge_xyz, og.edge_normal, og.nc, nlev=nlev, ldk=ldk, ldk_w=ldk_w, dtype=dtype)
+            vn = (vn * fv).astype(vn.dtype)
+            vn64, w64 = np.nan_to_num(vn.astype(np.float64)), np.nan_to_num(w.astype(np.float64))
+            want, m = o.w_tendency(vn64, w64, zh, nlev, with_scale=True)
+            out = torch.full((g.nc, ldk_w), sentinel, dtype=torch.from_numpy(w).dtype, device=dev)
+            n0 = g.launch_count
+            lib.dycore_w_tendency(g, zh, torch.from_numpy(vn).to(dev), torch.from_numpy(w).to(dev), out, nlev)
+            torch.cuda.synchronize()
+            assert g.launch_count - n0 == 1
+            got = out.cpu().numpy().astype(np.float64)
+            err = np.abs(got[:, :nlev + 1] - want[:, :nlev + 1])
+            assert (err <= TOL[dtype] * m[:, :nlev + 1]).all(), "worst err/M %.3e" % (err / np.maximum(m[:, :nlev + 1], 1e-300)).max()
+            assert (got[:, 0] == 0).all() and (got[:, nlev] == 0).all()
+            assert (got[:, nlev + 1:] == sentinel).all()
+            if not f32:
+                t = {n: g.table_host(n) for n in ("c2e", "e2c", "inv_d_e", "adv_c")}
+                want2, m2 = oracle_mod.w_tendency_from_arrays(t, vn64, w64, zh, nlev)
+                assert (np.abs(got[:, :nlev + 1] - want2[:, :nlev + 1]) <= TOL[dtype] * m2[:, :nlev + 1]).all()
+    finally:
+        g.set_option(lib.ICON_OPT_TENDENCY_KERNEL, 5)
 
 
 @pytest.mark.parametrize("k,seed,flags,nlev,ldk,ldk_w,dtype", [

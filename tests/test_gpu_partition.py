@@ -174,8 +174,11 @@ def test_decomposed_other_calls_and_rejections(torch_cuda, lib, oracle_grid):
         torch.cuda.synchronize()
         close("metric ddt_vn", ddt3.cpu().numpy(), wantm["ddt_vn"], wantm["m_ddt"], le, ne_o, nlev)
         # refused: everything that needs the global tables
-        for call in (lambda: lib.dycore_w_tendency(g, zh, d_vn, d_w, ddw, nlev),
-                     lambda: lib.dycore_velocity_tendencies(g, zh, d_vn, d_w, ddt, nlev, vt=torch.zeros_like(ddt)),
+        ddw2 = torch.zeros_like(ddw)
+        lib.dycore_w_tendency(g, zh, d_vn, d_w, ddw2, nlev)                 # the column cache's ddt_w mode: runs on a local grid
+        torch.cuda.synchronize()
+        close("w_tendency", ddw2.cpu().numpy(), want_w, m_w, lc, nc_o, nlev + 1)
+        for call in (lambda: lib.dycore_velocity_tendencies(g, zh, d_vn, d_w, ddt, nlev, vt=torch.zeros_like(ddt)),
                      lambda: lib.dycore_velocity_tendencies_noalloc(g, zh, d_vn, d_w, ddt, nlev),
                      lambda: g.table_device("c2e")):
             with pytest.raises(lib.IconError) as ei:
