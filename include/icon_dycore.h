@@ -193,7 +193,8 @@ int dycore_velocity_tendencies(const icon_grid_t* g, int dtype, int nlev, int ld
  *   k = 0 and k = nlev: ddt_w = 0 (the top and surface values of w are boundary conditions).
  * vn_ie = vn interpolated linearly in z to the half level (P-14). z_half [nlev+1] HOST, strictly decreasing.
  * vn [ne][ldk], w [nc][ldk_w] dev in; ddt_w [nc][ldk_w] dev out (levels 0 .. nlev written, pads untouched).
- * 2 <= nlev <= ldk, nlev+1 <= ldk_w.
+ * 2 <= nlev <= ldk, nlev+1 <= ldk_w. One kernel: the column cache in its ddt_w mode (nine vn and ten w columns per
+ * patch) where it holds the columns, else (ICON_OPT_TENDENCY_KERNEL 0 / 3, deeper columns) a gather kernel through L1.
  */
 int dycore_w_tendency(const icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
                       const void* vn, const void* w, void* ddt_w, void* cuda_stream);
@@ -298,7 +299,7 @@ int dycore_step_host(const icon_grid_t* g, int dtype, int nlev, int ldk, int ldk
  * Fields passed to the compute calls are local: vn [ne][ldk], w [nc][ldk_w] with their halo rows filled (dycore_halo_pack
  * on the owner, any transport, receive in place), outputs ddt_vn [ne][ldk] (rows < ne_owned written), div [nc][ldk]
  * (rows < nc_owned written), vort [nv][ldk]. On a local grid the calls served by the column-cache kernel work
- * (dycore_step, dycore_step_w, dycore_velocity_tendencies without optional outputs, dycore_div_vort,
+ * (dycore_step, dycore_step_w, dycore_velocity_tendencies without optional outputs, dycore_div_vort, dycore_w_tendency,
  * dycore_velocity_tendencies_metric; nlev <= 95 for 8-byte, 127 for 4-byte columns); every other call and every global
  * table selector returns ICON_EUNSUPPORTED. Host memory: the call builds the GLOBAL grid once and drops it.
  * Errors: ICON_EINVAL (k, flags, n_parts < 1 or > nc/4, part), ICON_ENOMEM, ICON_ECUDA.
