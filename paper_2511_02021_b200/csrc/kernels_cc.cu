@@ -821,11 +821,13 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
             }
             // ---- horizontal part H of the six owned edges (S5); frees the KE / vorticity columns ----
             if constexpr (METRIC) {
-                // ---- metric form (reading P-20). One loop over the owned edges fetches the four metric columns of an edge in
-                // ONE batch, straight from global memory (requested into the L2 when the patch started, see above): six
-                // dependent round trips per patch instead of twelve. It leaves two columns per edge, A = -H + w_cc Dv and
-                // Dv, and frees the KE / vorticity / vt columns; w at the edges follows as in the plain form.
-                C A[6], Dq[6];
+                // ---- metric form (reading P-20), in three phases. (1) The part of H that needs no metric column,
+                // A0 = -(gH KE_c(H) - gL KE_c(L) + gE (vn^2 + vt^2) + vt (f + zeta_e)), frees the KE / vorticity columns.
+                // (2) w at the owned edges: the last slot reads, the step is released. (3) One pass over the owned edges with
+                // the four metric columns of an edge fetched in ONE batch straight from global memory (requested into the L2
+                // when the patch started), the batch of the NEXT edge in flight while this one is used; each output column
+                // leaves as soon as it is complete.
+                C A0[6];
 #pragma unroll
                 for (int x = 0; x < 6; ++x) {
                     const C& v = x < 3 ? vI[x] : vB[2 * (x - 3)];
@@ -834,20 +836,12 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
                     const C& kH = x < 3 ? ke[3] : keX[x - 3];
                     const C& za = x < 3 ? (x == 2 ? zm[1] : zm[0]) : zm[x - 3];
                     const C& zb = x < 3 ? (x == 1 ? zm[1] : zm[2]) : zc[x - 3];      // i0: (ab, ca), i1: (ab, bc), i2: (bc, ca)
-                    const C zn = GL(met.zn, ido[x], cs, po), zt = GL(met.zt, ido[x], cs, po);
-                    const C wg = GL(met.wgt, ido[x], cs_wout, pow_), inv = GL(met.inv, ido[x], cs, po);
-                    T e4[4], m4[4];                     // f_e | gL, gH, gE: read where they are used (both groups in registers spilled)
+                    T e4[4], m4[4];                     // f_e | gL, gH, gE: read where they are used
                     ld_coef(cf + SCF_EDGE + 4 * x, e4);
                     ld_coef(cf + SCF_CGRAD + 4 * x, m4);
-                    const C Dv = VDM(v, wg, inv);
-                    FORL {
-                        // gradK = gH KE_c(H) - gL KE_c(L) + gE (vn^2 + vt^2): second order at the edge midpoint
-                        const T Hh = m4[1] * kH.v[l] - m4[0] * kL.v[l] + m4[2] * (v.v[l] * v.v[l] + t.v[l] * t.v[l]) +
-                                     t.v[l] * (e4[1] + (za.v[l] + zb.v[l]));
-                        const T wcc = v.v[l] * zn.v[l] + t.v[l] * zt.v[l];      // contravariant correction
-                        A[x].v[l] = wcc * Dv.v[l] - Hh;
-                        Dq[x].v[l] = Dv.v[l];
-                    }
+                    // gradK = gH KE_c(H) - gL KE_c(L) + gE (vn^2 + vt^2): second order at the edge midpoint
+                    FORL A0[x].v[l] = -(m4[1] * kH.v[l] - m4[0] * kL.v[l] + m4[2] * (v.v[l] * v.v[l] + t.v[l] * t.v[l]) +
+                                        t.v[l] * (e4[1] + (za.v[l] + zb.v[l])));
                 }
                 C we[6];
                 {
@@ -865,11 +859,23 @@ k_tend_cc(CcDev<T> d, int nlev, int ldk, int ldk_w, const T* __restrict__ abc, c
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(done_bar(s % NB));
+                C zn = GL(met.zn, ido[0], cs, po), zt = GL(met.zt, ido[0], cs, po);
+                C wg = GL(met.wgt, ido[0], cs_wout, pow_), inv = GL(met.inv, ido[0], cs, po);
 #pragma unroll
                 for (int x = 0; x < 6; ++x) {
+                    const C& v = x < 3 ? vI[x] : vB[2 * (x - 3)];
+                    const C& t = x < 3 ? tI[x] : tBo[x - 3];
+                    C zn1, zt1, wg1, inv1;
+                    if (x < 5) {                        // the next edge's batch goes out before this one is used
+                        zn1 = GL(met.zn, ido[x + 1], cs, po); zt1 = GL(met.zt, ido[x + 1], cs, po);
+                        wg1 = GL(met.wgt, ido[x + 1], cs_wout, pow_); inv1 = GL(met.inv, ido[x + 1], cs, po);
+                    }
+                    const C Dv = VDM(v, wg, inv);
                     C o;
-                    FORL o.v[l] = A[x].v[l] - we[x].v[l] * Dq[x].v[l];
+                    // V = (w_e - w_cc) Dv with the contravariant correction w_cc = vn ddxn_z + vt ddxt_z
+                    FORL o.v[l] = A0[x].v[l] - (we[x].v[l] - (v.v[l] * zn.v[l] + t.v[l] * zt.v[l])) * Dv.v[l];
                     ST(ddt_vn, ido[x], o);
+                    if (x < 5) { zn = zn1; zt = zt1; wg = wg1; inv = inv1; }
                 }
             } else {
             // ---- horizontal part H of the six owned edges (S5); frees the KE / vorticity columns ----
