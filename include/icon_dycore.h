@@ -274,12 +274,14 @@ int dycore_velocity_tendencies_noalloc(const icon_grid_t* g, int dtype, int nlev
                                        void* cuda_stream);
 
 /*
- * dycore_step_host -- dycore_step with HOST field buffers (the end-to-end leg of bench.py): copies vn and w to
- * device staging buffers, runs dycore_step (one fused kernel where the column-cache kernel runs), copies ddt_vn, div
- * and vort back, and synchronises. This is NOT how the paper runs the model (fields stay resident on the GPU,
- * PAPER.md:97); it exists so that the whole path can be timed with the PCIe copies included. Host buffers should be
- * pinned for full PCIe bandwidth. The staging buffers and the private stream are owned by the grid handle and allocated
- * on first use. Same shapes and constraints as dycore_step.
+ * dycore_step_host -- the step with HOST field buffers (the end-to-end leg of bench.py): copies vn and w to device staging
+ * buffers, computes ddt_vn, div and vort, copies them back, and synchronises. The copies are the cost (22 GB per step at
+ * R2B8 x 90 fp64), so the call runs the two entry points instead of the fused one and overlaps them with the link in both
+ * directions: vn goes up first, dycore_div_vort (which reads nothing else) runs as soon as it has arrived and div / vort go
+ * down while w is still going up; then dycore_velocity_tendencies, then ddt_vn down. This is NOT how the paper runs the
+ * model (fields stay resident on the GPU); it exists so that the whole path can be timed with the PCIe copies
+ * included. Host buffers should be pinned for full PCIe bandwidth. The staging buffers, three private streams and their
+ * events are owned by the grid handle and allocated on first use. Same shapes and constraints as dycore_step.
  */
 int dycore_step_host(const icon_grid_t* g, int dtype, int nlev, int ldk, int ldk_w, const double* z_half,
                      const void* vn_host, const void* w_host,

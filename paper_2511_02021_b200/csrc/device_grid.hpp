@@ -95,7 +95,9 @@ struct HostStage {                // device staging for dycore_step_host
     int dtype = -1;
     int64_t ldk = 0, ldk_w = 0;
     void *vn = nullptr, *w = nullptr, *ddt = nullptr, *div = nullptr, *vort = nullptr;
-    cudaStream_t stream = nullptr;
+    cudaStream_t stream = nullptr;                      // kernels
+    cudaStream_t stream_in = nullptr, stream_out = nullptr;      // host -> device, device -> host copies
+    cudaEvent_t ev_vn = nullptr, ev_w = nullptr, ev_dv = nullptr, ev_t = nullptr;
 };
 
 }  // namespace icon
